@@ -1,0 +1,497 @@
+/*
+ * spray_oracle.c -- CPU ORACLE for the SPRAY SPH pair-summation pass.
+ *
+ * TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke() and the
+ * cpu_baseline / --impl reference legs of bench.py may build, load or call this file.
+ * It shares no code with paper_2604_20124_b200/ (the CUDA path) and neither includes the other.
+ *
+ * A plain, slow, obviously-correct fp64 implementation written from the paper
+ * (/root/reference/PAPER.md, cited as P:L<line>) with the readings of SURVEY.md §8(c2)
+ * (cited as A<n>) and the contract steps O1..O8 of SURVEY.md §8(c1).  The method *is* the plain
+ * definition: the cell list only accelerates finding {b : r_ab < 2h}.  So the definition here is
+ * the all-pairs loop (use_cells = 0); the cell-list variant (use_cells = 1) must reproduce the
+ * same neighbour sets exactly (tests/test_oracle_*.py, pin T5).
+ *
+ * Per-pair terms are evaluated in fp64 with no FMA contraction (compile with -ffp-contract=off);
+ * the one explicit fma() is the r^2 expression of the neighbour predicate (O2/A12).  Sums are
+ * accumulated in long double (x87 80-bit) in ascending caller-index order of b, so the oracle sits
+ * closer to the exact sum than any plain fp64 order (O8).
+ *
+ * Parity pins: every function below is pinned by tests/test_oracle_*.py (closed forms T1/T2/T13/T14,
+ * lattice constants T3/T4/T6/T7, brute force T5, invariants T8-T12, symmetries T15), except the
+ * choice "viscosity acts only for w < 0" (A6) which is PARITY UNPINNED: both readings satisfy every
+ * invariant the paper states; the reading is fixed by SURVEY.md §8(c2) A6 / DESIGN.md.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef struct {
+    double lo[3], hi[3];
+    int32_t ncell[3];
+    int32_t periodic[3];
+    double h_max;
+} oracle_grid_t;
+
+enum { ORACLE_CUBIC_SPLINE = 0, ORACLE_WENDLAND_C2 = 1 };
+enum { ORACLE_GATHER = 0, ORACLE_SYM = 1 };
+
+int oracle_num_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+/* ------------------------------------------------------------------ O3: kernel functions
+ * Wendland C2, eq. (3):  W = 21/(16 pi h^3) (1-q/2)^4 (2q+1), q = r/h < 2, else 0.
+ * dW/dr = -5 * 21/(16 pi) * q (1-q/2)^3 / h^4.
+ * Cubic spline (textbook M4, 3-D sigma = 1/pi; not in the paper, A1):
+ *   f = 1 - 1.5 q^2 + 0.75 q^3 (q<1);  0.25 (2-q)^3 (1<=q<2);  W = f/(pi h^3)
+ *   f' = -3 q + 2.25 q^2 (q<1);  -0.75 (2-q)^2 (1<=q<2);       dW/dr = f'/(pi h^4)
+ */
+static const double PI = 3.14159265358979323846264338327950288;
+
+double oracle_W(int kernel, double r, double h) {
+    double q = r / h;
+    if (!(q < 2.0)) return 0.0;
+    if (kernel == ORACLE_WENDLAND_C2) {
+        double s = 21.0 / (16.0 * PI);
+        double t = 1.0 - 0.5 * q;
+        return s / (h * h * h) * (t * t * t * t) * (2.0 * q + 1.0);
+    } else {
+        double s = 1.0 / PI;
+        double f;
+        if (q < 1.0) f = 1.0 - 1.5 * q * q + 0.75 * q * q * q;
+        else { double t = 2.0 - q; f = 0.25 * t * t * t; }
+        return s / (h * h * h) * f;
+    }
+}
+
+double oracle_F(int kernel, double r, double h) { /* dW/dr (<= 0) */
+    double q = r / h;
+    if (!(q < 2.0)) return 0.0;
+    double h4 = (h * h) * (h * h);
+    if (kernel == ORACLE_WENDLAND_C2) {
+        double s = 21.0 / (16.0 * PI);
+        double t = 1.0 - 0.5 * q;
+        return -5.0 * s * q * (t * t * t) / h4;
+    } else {
+        double s = 1.0 / PI;
+        double fp;
+        if (q < 1.0) fp = -3.0 * q + 2.25 * q * q;
+        else { double t = 2.0 - q; fp = -0.75 * t * t; }
+        return s * fp / h4;
+    }
+}
+
+/* ------------------------------------------------------------------ O1: cell table
+ * c_d = (int) floor((x_d - lo_d) * (ncell_d / L_d)), clamped; key = (cz*ny + cy)*nx + cx.
+ * Stable sort by key (ties: ascending caller index); cell_start[c] = #{key < c};
+ * cell_end[c] = cell_start[c] + #{key = c}.
+ */
+static uint32_t cell_key(const oracle_grid_t* g, double x, double y, double z) {
+    double p[3] = {x, y, z};
+    int64_t c[3];
+    for (int d = 0; d < 3; ++d) {
+        double L = g->hi[d] - g->lo[d];
+        double inv = (double)g->ncell[d] / L;
+        double t = floor((p[d] - g->lo[d]) * inv);
+        int64_t ci = (t < 0.0) ? 0 : (t >= (double)g->ncell[d] ? g->ncell[d] - 1 : (int64_t)t);
+        if (!(t == t)) ci = 0; /* NaN position: cell 0 */
+        c[d] = ci;
+    }
+    return (uint32_t)((c[2] * g->ncell[1] + c[1]) * g->ncell[0] + c[0]);
+}
+
+int oracle_build_cells(const oracle_grid_t* g, int64_t n, const double* x, const double* y, const double* z,
+                       uint32_t* key /* [n] caller order, nullable */, uint32_t* sorted_key /* [n] */,
+                       uint32_t* perm /* [n] */, uint32_t* cell_start /* [ncell] */, uint32_t* cell_end /* [ncell] */) {
+    int64_t nc = (int64_t)g->ncell[0] * g->ncell[1] * g->ncell[2];
+    uint32_t* k = (uint32_t*)malloc(sizeof(uint32_t) * (size_t)(n > 0 ? n : 1));
+    uint32_t* cur = (uint32_t*)calloc((size_t)nc + 1, sizeof(uint32_t));
+    if (!k || !cur) { free(k); free(cur); return -1; }
+    for (int64_t i = 0; i < n; ++i) { k[i] = cell_key(g, x[i], y[i], z[i]); cur[k[i] + 1]++; }
+    for (int64_t c = 0; c < nc; ++c) cur[c + 1] += cur[c];          /* cur[c] = #{key < c} */
+    for (int64_t c = 0; c < nc; ++c) { cell_start[c] = cur[c]; cell_end[c] = cur[c + 1]; }
+    for (int64_t i = 0; i < n; ++i) {                                /* ascending caller index => stable */
+        uint32_t slot = cur[k[i]]++;
+        perm[slot] = (uint32_t)i;
+        sorted_key[slot] = k[i];
+    }
+    if (key) memcpy(key, k, sizeof(uint32_t) * (size_t)n);
+    free(k); free(cur);
+    return 0;
+}
+
+/* ------------------------------------------------------------------ O2: displacement + predicates */
+typedef struct {
+    const oracle_grid_t* g;
+    int64_t n;
+    const double *x, *y, *z, *h;
+    int use_cells;
+    uint32_t *perm, *cell_start, *cell_end; /* own cell table when use_cells */
+    double hmax_all;                        /* true max of h[] (search reach for the symmetric set) */
+} search_t;
+
+static inline double min_image(double dx, int periodic, double L) {
+    if (periodic) {
+        if (dx > 0.5 * L) dx -= L;
+        else if (dx < -0.5 * L) dx += L;
+    }
+    return dx;
+}
+
+static inline double pair_r2(const search_t* s, int64_t a, int64_t b, double* dx, double* dy, double* dz) {
+    const oracle_grid_t* g = s->g;
+    *dx = min_image(s->x[a] - s->x[b], g->periodic[0], g->hi[0] - g->lo[0]);
+    *dy = min_image(s->y[a] - s->y[b], g->periodic[1], g->hi[1] - g->lo[1]);
+    *dz = min_image(s->z[a] - s->z[b], g->periodic[2], g->hi[2] - g->lo[2]);
+    return fma(*dz, *dz, fma(*dy, *dy, (*dx) * (*dx)));
+}
+
+/* N_gather(a) = { b : r2 < 4 h_a^2 } (contains a);  N_sym(a) = { b != a : r2 < 4 max(h_a,h_b)^2 }  (A12, A13) */
+static inline int in_set(const search_t* s, int mode, int64_t a, int64_t b, double r2) {
+    if (mode == ORACLE_GATHER) return r2 < 4.0 * (s->h[a] * s->h[a]);
+    if (a == b) return 0;
+    double hm = s->h[a] > s->h[b] ? s->h[a] : s->h[b];
+    return r2 < 4.0 * (hm * hm);
+}
+
+static int search_init(search_t* s, const oracle_grid_t* g, int64_t n, const double* x, const double* y,
+                       const double* z, const double* h, int use_cells) {
+    memset(s, 0, sizeof(*s));
+    s->g = g; s->n = n; s->x = x; s->y = y; s->z = z; s->h = h; s->use_cells = use_cells;
+    double hm = 0.0;
+    for (int64_t i = 0; i < n; ++i) if (h[i] > hm) hm = h[i];
+    s->hmax_all = hm;
+    if (use_cells) {
+        int64_t nc = (int64_t)g->ncell[0] * g->ncell[1] * g->ncell[2];
+        s->perm = (uint32_t*)malloc(sizeof(uint32_t) * (size_t)(n > 0 ? n : 1));
+        uint32_t* sk = (uint32_t*)malloc(sizeof(uint32_t) * (size_t)(n > 0 ? n : 1));
+        s->cell_start = (uint32_t*)malloc(sizeof(uint32_t) * (size_t)nc);
+        s->cell_end = (uint32_t*)malloc(sizeof(uint32_t) * (size_t)nc);
+        if (!s->perm || !sk || !s->cell_start || !s->cell_end) { free(sk); return -1; }
+        int rc = oracle_build_cells(g, n, x, y, z, NULL, sk, s->perm, s->cell_start, s->cell_end);
+        free(sk);
+        return rc;
+    }
+    return 0;
+}
+
+static void search_free(search_t* s) { free(s->perm); free(s->cell_start); free(s->cell_end); }
+
+typedef struct { int64_t* v; int64_t n, cap; } ilist_t;
+
+static void ilist_push(ilist_t* l, int64_t v) {
+    if (l->n == l->cap) { l->cap = l->cap ? 2 * l->cap : 256; l->v = (int64_t*)realloc(l->v, sizeof(int64_t) * (size_t)l->cap); }
+    l->v[l->n++] = v;
+}
+
+static int cmp_i64(const void* a, const void* b) {
+    int64_t x = *(const int64_t*)a, y = *(const int64_t*)b;
+    return (x > y) - (x < y);
+}
+
+/* cells along dimension d that can hold a point within `reach` of coordinate p (one safety cell each side) */
+static int cell_span(const oracle_grid_t* g, int d, double p, double reach, int* out /* [ncell_d] */) {
+    int nc = g->ncell[d];
+    double L = g->hi[d] - g->lo[d];
+    double inv = (double)nc / L;
+    int64_t c0 = (int64_t)floor((p - reach - g->lo[d]) * inv) - 1;
+    int64_t c1 = (int64_t)floor((p + reach - g->lo[d]) * inv) + 1;
+    int cnt = 0;
+    if (g->periodic[d]) {
+        if (c1 - c0 + 1 >= nc) { for (int c = 0; c < nc; ++c) out[cnt++] = c; return cnt; }
+        for (int64_t c = c0; c <= c1; ++c) out[cnt++] = (int)(((c % nc) + nc) % nc);
+    } else {
+        if (c0 < 0) c0 = 0;
+        if (c1 > nc - 1) c1 = nc - 1;
+        for (int64_t c = c0; c <= c1; ++c) out[cnt++] = (int)c;
+    }
+    return cnt;
+}
+
+/* neighbours of a in ascending caller index */
+static void enumerate(const search_t* s, int mode, int64_t a, ilist_t* out) {
+    out->n = 0;
+    double dx, dy, dz;
+    if (!s->use_cells) {
+        for (int64_t b = 0; b < s->n; ++b) {
+            double r2 = pair_r2(s, a, b, &dx, &dy, &dz);
+            if (in_set(s, mode, a, b, r2)) ilist_push(out, b);
+        }
+        return;
+    }
+    const oracle_grid_t* g = s->g;
+    double reach = 2.0 * (mode == ORACLE_GATHER ? s->h[a] : (s->h[a] > s->hmax_all ? s->h[a] : s->hmax_all));
+    int* cx = (int*)malloc(sizeof(int) * (size_t)g->ncell[0]);
+    int* cy = (int*)malloc(sizeof(int) * (size_t)g->ncell[1]);
+    int* cz = (int*)malloc(sizeof(int) * (size_t)g->ncell[2]);
+    int nx = cell_span(g, 0, s->x[a], reach, cx);
+    int ny = cell_span(g, 1, s->y[a], reach, cy);
+    int nz = cell_span(g, 2, s->z[a], reach, cz);
+    for (int k = 0; k < nz; ++k) for (int j = 0; j < ny; ++j) for (int i = 0; i < nx; ++i) {
+        int64_t c = ((int64_t)cz[k] * g->ncell[1] + cy[j]) * g->ncell[0] + cx[i];
+        for (uint32_t t = s->cell_start[c]; t < s->cell_end[c]; ++t) {
+            int64_t b = s->perm[t];
+            double r2 = pair_r2(s, a, b, &dx, &dy, &dz);
+            if (in_set(s, mode, a, b, r2)) ilist_push(out, b);
+        }
+    }
+    free(cx); free(cy); free(cz);
+    qsort(out->v, (size_t)out->n, sizeof(int64_t), cmp_i64);
+}
+
+/* ------------------------------------------------------------------ K9: neighbour counts / CSR lists */
+int oracle_neighbor_counts(const oracle_grid_t* g, int64_t n, const double* x, const double* y, const double* z,
+                           const double* h, int use_cells, int mode, const int64_t* targets, int64_t nt,
+                           uint32_t* count /* [nt]; SYM excludes self, GATHER excludes self too */) {
+    search_t s;
+    if (search_init(&s, g, n, x, y, z, h, use_cells)) return -1;
+    if (!targets) nt = n;
+#pragma omp parallel
+    {
+        ilist_t l = {0, 0, 0};
+#pragma omp for schedule(dynamic, 64)
+        for (int64_t t = 0; t < nt; ++t) {
+            int64_t a = targets ? targets[t] : t;
+            enumerate(&s, mode, a, &l);
+            count[t] = (uint32_t)(mode == ORACLE_GATHER ? l.n - 1 : l.n);
+        }
+        free(l.v);
+    }
+    search_free(&s);
+    return 0;
+}
+
+int oracle_neighbor_lists(const oracle_grid_t* g, int64_t n, const double* x, const double* y, const double* z,
+                          const double* h, int use_cells, int mode, const int64_t* targets, int64_t nt,
+                          const uint64_t* offsets /* [nt] exclusive scan of counts */, uint32_t* nbr) {
+    search_t s;
+    if (search_init(&s, g, n, x, y, z, h, use_cells)) return -1;
+    if (!targets) nt = n;
+#pragma omp parallel
+    {
+        ilist_t l = {0, 0, 0};
+#pragma omp for schedule(dynamic, 64)
+        for (int64_t t = 0; t < nt; ++t) {
+            int64_t a = targets ? targets[t] : t;
+            enumerate(&s, mode, a, &l);
+            uint64_t o = offsets[t];
+            for (int64_t k = 0; k < l.n; ++k) if (l.v[k] != a) nbr[o++] = (uint32_t)l.v[k];
+        }
+        free(l.v);
+    }
+    search_free(&s);
+    return 0;
+}
+
+/* ------------------------------------------------------------------ O4: density, eq. (35)
+ * rho_a = sum_{b in N_gather(a)} m_b W(r_ab; h_a), self term included (A11).
+ * S_rho = the same sum of absolute values (O8).  nnbr = |N_gather(a)| - 1.
+ */
+int oracle_density(const oracle_grid_t* g, int kernel, int64_t n, const double* x, const double* y, const double* z,
+                   const double* h, const double* m, int use_cells, const int64_t* targets, int64_t nt,
+                   double* rho, uint32_t* nnbr, double* S_rho) {
+    search_t s;
+    if (search_init(&s, g, n, x, y, z, h, use_cells)) return -1;
+    if (!targets) nt = n;
+#pragma omp parallel
+    {
+        ilist_t l = {0, 0, 0};
+#pragma omp for schedule(dynamic, 64)
+        for (int64_t t = 0; t < nt; ++t) {
+            int64_t a = targets ? targets[t] : t;
+            enumerate(&s, ORACLE_GATHER, a, &l);
+            long double acc = 0.0L, sab = 0.0L;
+            for (int64_t k = 0; k < l.n; ++k) {
+                int64_t b = l.v[k];
+                double dx, dy, dz;
+                double r2 = pair_r2(&s, a, b, &dx, &dy, &dz);
+                double term = m[b] * oracle_W(kernel, sqrt(r2), h[a]);
+                acc += term; sab += fabs(term);
+            }
+            rho[t] = (double)acc;
+            if (nnbr) nnbr[t] = (uint32_t)(l.n - 1);
+            if (S_rho) S_rho[t] = (double)sab;
+        }
+        free(l.v);
+    }
+    search_free(&s);
+    return 0;
+}
+
+/* ------------------------------------------------------------------ O5: hydro RHS over N_sym(a), r2 > 0
+ * grad_a W(x_ab,h) = F(r;h) x_ab / r (A4).
+ * momentum  eq. (11) P:L98 with the sign of eq. (5)/(19) (A3):
+ *     a_a = - sum_b m_b/(rho_a rho_b) [p_a F(r;h_a) + p_b F(r;h_b)] xhat_ab
+ * dissipation eq. (41), (43) P:L242, only for w = v_ab . xhat_ab < 0 (A6, A8):
+ *     a_a += sum_b (m_b/2) [vsig_a F(r;h_a)/rho_a + vsig_b F(r;h_b)/rho_b] w xhat_ab,  vsig_s = alpha_s c_s + beta |w|
+ * divergence sum eq. (37):  D_a = sum_b (m_b/rho_b) w F(r;h_a)
+ * PdV eq. (17) first term P:L129:  (du/dt)_a = (p_a/rho_a) D_a
+ * viscous heating eq. (42) P:L238 as read in A7:  (du/dt)_a -= (1/rho_a) sum_b (m_b vsig_a / 2) w^2 F(r;h_a)
+ * Normalisers (O8): S_* = sums of absolute values of the per-pair contributions.
+ */
+int oracle_hydro(const oracle_grid_t* g, int kernel, int64_t n, const double* x, const double* y, const double* z,
+                 const double* h, const double* m, const double* rho, const double* p, const double* cs,
+                 const double* vx, const double* vy, const double* vz, const double* alpha, double beta,
+                 int use_cells, const int64_t* targets, int64_t nt,
+                 double* ax, double* ay, double* az, double* dudt, double* divv,
+                 double* S_ax, double* S_ay, double* S_az, double* S_dudt, double* S_divv) {
+    search_t s;
+    if (search_init(&s, g, n, x, y, z, h, use_cells)) return -1;
+    if (!targets) nt = n;
+#pragma omp parallel
+    {
+        ilist_t l = {0, 0, 0};
+#pragma omp for schedule(dynamic, 64)
+        for (int64_t t = 0; t < nt; ++t) {
+            int64_t a = targets ? targets[t] : t;
+            enumerate(&s, ORACLE_SYM, a, &l);
+            long double sx = 0, sy = 0, sz = 0, sD = 0, sQ = 0;
+            long double nx = 0, ny = 0, nz = 0, nD = 0, nQ = 0;
+            for (int64_t k = 0; k < l.n; ++k) {
+                int64_t b = l.v[k];
+                double dx, dy, dz;
+                double r2 = pair_r2(&s, a, b, &dx, &dy, &dz);
+                if (r2 == 0.0) continue; /* coincident distinct particles: no gradient contribution (A11) */
+                double r = sqrt(r2);
+                double Fa = oracle_F(kernel, r, h[a]);
+                double Fb = oracle_F(kernel, r, h[b]);
+                double ex = dx / r, ey = dy / r, ez = dz / r;
+                double w = ((vx[a] - vx[b]) * dx + (vy[a] - vy[b]) * dy + (vz[a] - vz[b]) * dz) / r;
+                double cmom = -(m[b] / (rho[a] * rho[b])) * (p[a] * Fa + p[b] * Fb);
+                double cvis = 0.0, qv = 0.0;
+                if (w < 0.0) {
+                    double aw = fabs(w);
+                    double vsa = alpha[a] * cs[a] + beta * aw;
+                    double vsb = alpha[b] * cs[b] + beta * aw;
+                    cvis = 0.5 * m[b] * (vsa * Fa / rho[a] + vsb * Fb / rho[b]) * w;
+                    qv = 0.5 * m[b] * vsa * (w * w) * Fa;
+                }
+                double dterm = (m[b] / rho[b]) * w * Fa;
+                sx += cmom * ex; sx += cvis * ex; nx += fabs(cmom * ex) + fabs(cvis * ex);
+                sy += cmom * ey; sy += cvis * ey; ny += fabs(cmom * ey) + fabs(cvis * ey);
+                sz += cmom * ez; sz += cvis * ez; nz += fabs(cmom * ez) + fabs(cvis * ez);
+                sD += dterm; nD += fabs(dterm);
+                sQ += qv; nQ += fabs(qv);
+            }
+            double por = p[a] / rho[a];
+            ax[t] = (double)sx; ay[t] = (double)sy; az[t] = (double)sz;
+            divv[t] = (double)sD;
+            dudt[t] = (double)((long double)por * sD - sQ / (long double)rho[a]);
+            if (S_ax) { S_ax[t] = (double)nx; S_ay[t] = (double)ny; S_az[t] = (double)nz; }
+            if (S_divv) S_divv[t] = (double)nD;
+            if (S_dudt) S_dudt[t] = (double)(fabsl((long double)por) * nD + nQ / fabsl((long double)rho[a]));
+        }
+        free(l.v);
+    }
+    search_free(&s);
+    return 0;
+}
+
+/* ------------------------------------------------------------------ O6: FLD limiter pre-sweep
+ * grad E by eq. (9), phi = 1 (A19), over N_gather(a) \ {a}:
+ *     gradE_a = sum_b (m_b/rho_b) (E_b - E_a) F(r;h_a) xhat_ab
+ * R = |gradE| / (rho kappa E);  lambda = 1/sqrt(9 + R^2) (Larsen, k = 2; A20);  mu = c lambda / (rho kappa).
+ */
+int oracle_limiter(const oracle_grid_t* g, int kernel, int64_t n, const double* x, const double* y, const double* z,
+                   const double* h, const double* m, const double* rho, const double* kappa, const double* E,
+                   double c_light, int use_cells, const int64_t* targets, int64_t nt,
+                   double* gx, double* gy, double* gz, double* Rout, double* lambda, double* mu,
+                   double* S_gx, double* S_gy, double* S_gz) {
+    search_t s;
+    if (search_init(&s, g, n, x, y, z, h, use_cells)) return -1;
+    if (!targets) nt = n;
+#pragma omp parallel
+    {
+        ilist_t l = {0, 0, 0};
+#pragma omp for schedule(dynamic, 64)
+        for (int64_t t = 0; t < nt; ++t) {
+            int64_t a = targets ? targets[t] : t;
+            enumerate(&s, ORACLE_GATHER, a, &l);
+            long double sx = 0, sy = 0, sz = 0, nx = 0, ny = 0, nz = 0;
+            for (int64_t k = 0; k < l.n; ++k) {
+                int64_t b = l.v[k];
+                if (b == a) continue;
+                double dx, dy, dz;
+                double r2 = pair_r2(&s, a, b, &dx, &dy, &dz);
+                if (r2 == 0.0) continue;
+                double r = sqrt(r2);
+                double c = (m[b] / rho[b]) * (E[b] - E[a]) * oracle_F(kernel, r, h[a]);
+                double tx = c * (dx / r), ty = c * (dy / r), tz = c * (dz / r);
+                sx += tx; sy += ty; sz += tz;
+                nx += fabs(tx); ny += fabs(ty); nz += fabs(tz);
+            }
+            double Gx = (double)sx, Gy = (double)sy, Gz = (double)sz;
+            double gn = sqrt(Gx * Gx + Gy * Gy + Gz * Gz);
+            double R = gn / (rho[a] * kappa[a] * E[a]);
+            double lam = 1.0 / sqrt(9.0 + R * R);
+            if (gx) { gx[t] = Gx; gy[t] = Gy; gz[t] = Gz; }
+            if (Rout) Rout[t] = R;
+            if (lambda) lambda[t] = lam;
+            if (mu) mu[t] = c_light * lam / (rho[a] * kappa[a]);
+            if (S_gx) { S_gx[t] = (double)nx; S_gy[t] = (double)ny; S_gz[t] = (double)nz; }
+        }
+        free(l.v);
+    }
+    search_free(&s);
+    return 0;
+}
+
+/* ------------------------------------------------------------------ O7: FLD operator apply
+ * eq. (47) first term P:L270, eqs. (51)-(52) P:L283-L286, on the Laplacian form eq. (16) P:L125:
+ *     c_ab = (m_b/rho_b) * 4 mu_a mu_b / (mu_a + mu_b) * G_ab,   G_ab = Fbar / r
+ *     Fbar = 1/2 [F(r;h_a) + F(r;h_b)] over N_sym(a)     (sym_mode = 1, A17, the form of P:L134)
+ *          = F(r;h_a)                 over N_gather(a)\{a} (sym_mode = 0, literal eq. (47))
+ *     y_a = sum_b c_ab (E_a - E_b)  (difference form),  Lambda_a = sum_b c_ab,  Gamma_a = - sum_b c_ab E_b.
+ */
+int oracle_fld_apply(const oracle_grid_t* g, int kernel, int64_t n, const double* x, const double* y, const double* z,
+                     const double* h, const double* m, const double* rho, const double* mu, const double* E,
+                     int sym_mode, int use_cells, const int64_t* targets, int64_t nt,
+                     double* yout, double* diag, double* offd, double* S_y, double* S_diag, double* S_offd) {
+    search_t s;
+    if (search_init(&s, g, n, x, y, z, h, use_cells)) return -1;
+    if (!targets) nt = n;
+#pragma omp parallel
+    {
+        ilist_t l = {0, 0, 0};
+#pragma omp for schedule(dynamic, 64)
+        for (int64_t t = 0; t < nt; ++t) {
+            int64_t a = targets ? targets[t] : t;
+            enumerate(&s, sym_mode ? ORACLE_SYM : ORACLE_GATHER, a, &l);
+            long double sy = 0, sl = 0, sg = 0, ny = 0, nl = 0, ng = 0;
+            for (int64_t k = 0; k < l.n; ++k) {
+                int64_t b = l.v[k];
+                if (b == a) continue;
+                double dx, dy, dz;
+                double r2 = pair_r2(&s, a, b, &dx, &dy, &dz);
+                if (r2 == 0.0) continue;
+                double r = sqrt(r2);
+                double Fa = oracle_F(kernel, r, h[a]);
+                double Fbar = sym_mode ? 0.5 * (Fa + oracle_F(kernel, r, h[b])) : Fa;
+                double G = Fbar / r;
+                double cab = (m[b] / rho[b]) * (4.0 * mu[a] * mu[b] / (mu[a] + mu[b])) * G;
+                double ty = cab * (E[a] - E[b]);
+                double tg = -(cab * E[b]);
+                sy += ty; sl += cab; sg += tg;
+                ny += fabs(ty); nl += fabs(cab); ng += fabs(tg);
+            }
+            yout[t] = (double)sy;
+            if (diag) diag[t] = (double)sl;
+            if (offd) offd[t] = (double)sg;
+            if (S_y) S_y[t] = (double)ny;
+            if (S_diag) S_diag[t] = (double)nl;
+            if (S_offd) S_offd[t] = (double)ng;
+        }
+        free(l.v);
+    }
+    search_free(&s);
+    return 0;
+}

@@ -1,0 +1,401 @@
+"""Pins for the CPU oracle against what the paper and the mathematics fix.
+
+None of these compares the oracle with itself on the same formula: closed forms, quadrature,
+finite differences, lattice constants from an independent survey script (tests/golden/), an
+independently written vectorised all-pairs search, conservation identities of the paper
+(eqs. (19), (46)) and symmetries.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+from scipy import integrate
+
+import oracle as O
+import workloads as W
+from workloads import Grid
+
+PI = math.pi
+GOLD = os.path.join(os.path.dirname(__file__), "golden", "lattice_constants.txt")
+
+
+def golden():
+    out = {}
+    for line in open(GOLD):
+        if line.startswith("#") or not line.strip():
+            continue
+        k, hdx, s0, s2 = line.split()
+        out[(k, float(hdx))] = (float(s0), float(s2))
+    return out
+
+
+KID = {"cubic": O.CUBIC_SPLINE, "wendland": O.WENDLAND_C2}
+
+
+# ----------------------------------------------------------------------------- T1, T2
+@pytest.mark.parametrize("h", [1.0, 0.37, 2.5e-3])
+def test_T1_closed_form_point_values(h):
+    # Wendland C2 eq. (3) P:L57 at q = 0, 1; cubic spline M4 at q = 0, 1, 2-
+    assert O.W(O.WENDLAND_C2, 0.0, h) == pytest.approx(21 / (16 * PI * h**3), rel=1e-15)
+    assert O.W(O.WENDLAND_C2, h, h) == pytest.approx(63 / (256 * PI * h**3), rel=1e-15)
+    assert O.F(O.WENDLAND_C2, h, h) == pytest.approx(-105 / (128 * PI * h**4), rel=1e-15)
+    assert O.W(O.CUBIC_SPLINE, 0.0, h) == pytest.approx(1 / (PI * h**3), rel=1e-15)
+    assert O.W(O.CUBIC_SPLINE, h, h) == pytest.approx(1 / (4 * PI * h**3), rel=1e-15)
+    assert O.F(O.CUBIC_SPLINE, h, h) == pytest.approx(-3 / (4 * PI * h**4), rel=1e-15)
+    for k in (0, 1):
+        assert O.W(k, 2.0 * h, h) == 0.0 and O.F(k, 2.0 * h, h) == 0.0      # q >= 2: identically zero
+        assert O.W(k, 2.5 * h, h) == 0.0 and O.F(k, 2.5 * h, h) == 0.0
+        assert O.W(k, 1.999 * h, h) > 0.0 and O.F(k, 1.999 * h, h) < 0.0    # positive, decreasing inside
+        assert O.F(k, 0.0, h) == 0.0
+        assert abs(O.F(k, 2.0 * h * (1 - 1e-9), h)) < 1e-12 / h**4           # F(q -> 2-) -> 0
+
+
+@pytest.mark.parametrize("k", [0, 1])
+@pytest.mark.parametrize("h", [1.0, 0.075])
+def test_T2_normalisation_by_quadrature(k, h):
+    pts = [h] if k == 0 else None
+    i0, _ = integrate.quad(lambda r: 4 * PI * r * r * O.W(k, r, h), 0, 2 * h, points=pts, epsabs=1e-13, epsrel=1e-13)
+    i1, _ = integrate.quad(lambda r: -(4 * PI / 3) * r**3 * O.F(k, r, h), 0, 2 * h, points=pts, epsabs=1e-13, epsrel=1e-13)
+    assert i0 == pytest.approx(1.0, abs=1e-12)      # int W dV = 1 (condition 1)
+    assert i1 == pytest.approx(1.0, abs=1e-12)      # integration by parts of the same statement
+
+
+@pytest.mark.parametrize("k", [0, 1])
+def test_F_is_derivative_of_W(k):
+    h = 0.8
+    for q in np.linspace(0.05, 1.95, 39):
+        r, e = q * h, 1e-5 * h
+        fd = (O.W(k, r + e, h) - O.W(k, r - e, h)) / (2 * e)
+        assert O.F(k, r, h) == pytest.approx(fd, rel=2e-7, abs=1e-9)
+
+
+# ----------------------------------------------------------------------------- lattice helpers
+def lattice_block(n, dx=1.0, periodic=True, hfac=1.2):
+    i = np.arange(n**3)
+    x = ((i % n) + 0.5) * dx
+    y = (((i // n) % n) + 0.5) * dx
+    z = ((i // (n * n)) + 0.5) * dx
+    h = np.full(n**3, hfac * dx)
+    L = n * dx
+    nc = max(1, int(L / (2 * hfac * dx)))
+    g = Grid((0, 0, 0), (L, L, L), (nc, nc, nc), (int(periodic),) * 3, hfac * dx)
+    return x, y, z, h, g
+
+
+@pytest.mark.parametrize("hfac,count", [(1.2, 56), (1.3, 80)])
+def test_T3_lattice_neighbour_count(hfac, count):
+    # shells n^2 = 0..5 hold 1+6+12+8+6+24 = 57 points (2h = 2.4 dx); n^2 = 6 adds 24 (2h = 2.6 dx)
+    x, y, z, h, g = lattice_block(8, 1.0, True, hfac)
+    for cells in (False, True):
+        c = O.neighbor_counts(g, x, y, z, h, O.GATHER, use_cells=cells)
+        assert (c == count).all()
+        c = O.neighbor_counts(g, x, y, z, h, O.SYM, use_cells=cells)
+        assert (c == count).all()
+
+
+@pytest.mark.parametrize("kname", ["cubic", "wendland"])
+@pytest.mark.parametrize("hfac", [1.2, 1.3])
+def test_T4_uniform_lattice_density(kname, hfac):
+    s0, _ = golden()[(kname, hfac)]
+    dx, rho0 = 0.125, 3.0
+    x, y, z, h, g = lattice_block(8, dx, True, hfac)
+    m = np.full(x.size, rho0 * dx**3)
+    d = O.density(g, KID[kname], x, y, z, h, m)
+    assert np.ptp(d["rho"]) <= 4e-15 * rho0                      # identical for all particles to round-off
+    assert d["rho"][0] == pytest.approx(rho0 * s0, rel=1e-13)     # independent lattice sum (survey script)
+    assert abs(d["rho"][0] / rho0 - 1.0) < 0.02                   # "sums to rho0" within the lattice error
+    assert d["S_rho"][0] == pytest.approx(d["rho"][0], rel=1e-15)  # all terms positive
+
+
+# ----------------------------------------------------------------------------- T5 brute force
+def numpy_allpairs_sets(w, mode):
+    """Independently written, vectorised O(N^2) neighbour search (no FMA: differs from the oracle's r2 by
+    <= 1 ulp, which cannot flip a strict comparison on these inputs except with probability ~1e-12)."""
+    g = w.grid
+    d2 = np.zeros((w.n, w.n))
+    for d, c in enumerate((w.x, w.y, w.z)):
+        dd = c[:, None] - c[None, :]
+        if g.periodic[d]:
+            L = g.hi[d] - g.lo[d]
+            dd = dd - L * np.round(dd / L)
+        d2 += dd * dd
+    if mode == O.GATHER:
+        mask = d2 < (2 * w.h[:, None]) ** 2
+    else:
+        mask = d2 < (2 * np.maximum(w.h[:, None], w.h[None, :])) ** 2
+    np.fill_diagonal(mask, False)
+    return mask
+
+
+@pytest.mark.parametrize("periodic", [(1, 1, 1), (0, 0, 0), (1, 0, 1)])
+def test_T5_sets_vs_independent_numpy_search(periodic):
+    w = W.random_cloud(2400, seed=7, periodic=periodic, hvar=2.0)
+    for mode in (O.GATHER, O.SYM):
+        mask = numpy_allpairs_sets(w, mode)
+        for cells in (False, True):
+            off, nbr = O.neighbor_lists(w.grid, w.x, w.y, w.z, w.h, mode, use_cells=cells)
+            assert int(off[-1]) == int(mask.sum())
+            rows = np.repeat(np.arange(w.n), np.diff(off).astype(np.int64))
+            got = np.zeros_like(mask)
+            got[rows, nbr] = True
+            assert (got == mask).all()
+            # ascending within each particle
+            same = rows[1:] == rows[:-1]
+            assert (nbr[1:][same] > nbr[:-1][same]).all()
+    if all(periodic):
+        msym = numpy_allpairs_sets(w, O.SYM)
+        assert (msym == msym.T).all()          # "all neighbours are mutual"
+
+
+TINY = ["c1_tiny", "c2_tiny", "c3_tiny", "c4_tiny", "c5_tiny"]
+
+
+def all_sweeps(w, cells, targets=None, sym_mode=True):
+    a = (w.grid, w.kernel, w.x, w.y, w.z, w.h, w.m)
+    d = O.density(*a, use_cells=cells, targets=targets)
+    hy = O.hydro(*a, w.rho_nom, w.p, w.cs, w.vx, w.vy, w.vz, w.alpha, w.beta, use_cells=cells, targets=targets)
+    li = O.limiter(*a, w.rho_nom, w.kappa, w.E, w.c_light, use_cells=cells, targets=targets)
+    mu = O.limiter(*a, w.rho_nom, w.kappa, w.E, w.c_light, use_cells=True)["mu"]
+    ap = O.fld_apply(*a, w.rho_nom, mu, w.E, sym_mode=sym_mode, use_cells=cells, targets=targets)
+    return {**d, **hy, **li, **ap}
+
+
+@pytest.mark.parametrize("name", TINY + ["cloud_open", "cloud_periodic"])
+def test_T5_cell_list_equals_brute_force(name):
+    if name == "cloud_open":
+        w = W.random_cloud(1500, seed=11, periodic=(0, 0, 0), hvar=3.0)
+    elif name == "cloud_periodic":
+        w = W.random_cloud(3000, seed=12, periodic=(1, 1, 1), hvar=2.0, kernel=W.KERNEL_CUBIC_SPLINE)
+    else:
+        w = W.make(name)
+    rng = np.random.default_rng(1)
+    targets = np.sort(rng.choice(w.n, size=min(w.n, 400), replace=False)).astype(np.int64)
+    for mode in (O.GATHER, O.SYM):
+        o0, n0 = O.neighbor_lists(w.grid, w.x, w.y, w.z, w.h, mode, use_cells=False, targets=targets)
+        o1, n1 = O.neighbor_lists(w.grid, w.x, w.y, w.z, w.h, mode, use_cells=True, targets=targets)
+        assert np.array_equal(o0, o1) and np.array_equal(n0, n1)
+    for sym_mode in (True, False):
+        r0 = all_sweeps(w, False, targets, sym_mode)
+        r1 = all_sweeps(w, True, targets, sym_mode)
+        for k in r0:
+            assert np.array_equal(r0[k], r1[k]), k      # same sets, same order => bit-identical sums
+
+
+def test_build_cells_against_numpy_stable_sort():
+    for name in ("c2_tiny", "c4_tiny"):
+        w = W.make(name)
+        g = w.grid
+        c = []
+        for d, a in enumerate((w.x, w.y, w.z)):
+            inv = g.ncell[d] / (g.hi[d] - g.lo[d])
+            c.append(np.clip(np.floor((a - g.lo[d]) * inv), 0, g.ncell[d] - 1).astype(np.int64))
+        key = (c[2] * g.ncell[1] + c[1]) * g.ncell[0] + c[0]
+        perm = np.argsort(key, kind="stable")
+        t = O.build_cells(g, w.x, w.y, w.z)
+        assert np.array_equal(t["key"], key)
+        assert np.array_equal(t["perm"], perm)
+        assert np.array_equal(t["sorted_key"], key[perm])
+        cnt = np.bincount(key, minlength=g.ncell_total)
+        assert np.array_equal(t["cell_end"] - t["cell_start"], cnt)
+        assert np.array_equal(t["cell_start"], np.concatenate([[0], np.cumsum(cnt)[:-1]]))
+
+
+# ----------------------------------------------------------------------------- T6, T7, T8, T13
+def open_block_fields(kname, hfac, gvec, H, E0=50.0, n=9, dx=0.1):
+    x, y, z, h, g = lattice_block(n, dx, False, hfac)
+    c = (n // 2 + 0.5) * dx
+    X = np.stack([x - c, y - c, z - c], 1)
+    E = E0 + X @ gvec + 0.5 * np.einsum("ni,ij,nj->n", X, H, X)
+    rho = np.full(x.size, 2.0)
+    m = rho * dx**3
+    centre = np.array([(n // 2) * (n * n + n + 1)], dtype=np.int64)
+    return x, y, z, h, g, m, rho, E, centre
+
+
+@pytest.mark.parametrize("kname", ["cubic", "wendland"])
+@pytest.mark.parametrize("hfac", [1.2, 1.3])
+def test_T6_T7_linear_and_quadratic_fields(kname, hfac):
+    _, s2 = golden()[(kname, hfac)]
+    k = KID[kname]
+    gvec = np.array([0.7, -1.3, 0.4])
+    H = np.array([[1.0, 0.3, -0.2], [0.3, -0.5, 0.6], [-0.2, 0.6, 2.0]])
+    mu0 = 0.37
+    # linear field: grad E = g * S2 exactly, y = 0 (the operator annihilates linear fields)
+    x, y, z, h, g, m, rho, E, ctr = open_block_fields(kname, hfac, gvec, np.zeros((3, 3)))
+    li = O.limiter(g, k, x, y, z, h, m, rho, np.ones_like(x), E, targets=ctr)
+    G = np.array([li["gx"][0], li["gy"][0], li["gz"][0]])
+    assert np.allclose(G, gvec * s2, rtol=1e-12, atol=1e-13)
+    mu = np.full(x.size, mu0)
+    ap = O.fld_apply(g, k, x, y, z, h, m, rho, mu, E, targets=ctr)
+    assert abs(ap["y"][0]) <= 1e-13 * ap["S_y"][0]
+    # quadratic field: y = + mu tr(H) S2 (constant-mu limit of eq. (47) is + div(mu grad E), eq. (15))
+    x, y, z, h, g, m, rho, E, ctr = open_block_fields(kname, hfac, gvec, H)
+    for sym in (True, False):
+        ap = O.fld_apply(g, k, x, y, z, h, m, rho, mu, E, sym_mode=sym, targets=ctr)
+        assert ap["y"][0] == pytest.approx(mu0 * np.trace(H) * s2, rel=1e-11)
+        assert abs(ap["y"][0] / (mu0 * np.trace(H)) - 1.0) < 0.022        # within the kernel's lattice error
+        assert ap["y"][0] == pytest.approx(ap["diag"][0] * E[ctr[0]] + ap["offd"][0], rel=1e-6)   # T12
+        assert ap["diag"][0] < 0.0
+    # gradient of the quadratic field at the centre is still g*S2 (odd terms cancel on the lattice)
+    li = O.limiter(g, k, x, y, z, h, m, rho, np.ones_like(x), E, targets=ctr)
+    assert np.allclose([li["gx"][0], li["gy"][0], li["gz"][0]], gvec * s2, rtol=1e-11)
+
+
+def test_T8_constant_field_is_exactly_zero():
+    w = W.make("c4_tiny")
+    E = np.full(w.n, 3.25)
+    li = O.limiter(w.grid, w.kernel, w.x, w.y, w.z, w.h, w.m, w.rho_nom, w.kappa, E)
+    for k in ("gx", "gy", "gz", "R", "S_gx"):
+        assert (li[k] == 0.0).all()
+    assert (li["lam"] == 1.0 / 3.0).all()          # lambda(R = 0) = 1/3
+    ap = O.fld_apply(w.grid, w.kernel, w.x, w.y, w.z, w.h, w.m, w.rho_nom, li["mu"], E)
+    assert (ap["y"] == 0.0).all() and (ap["S_y"] == 0.0).all()
+    assert (ap["diag"] < 0.0).all()
+
+
+def test_T13_limiter_values():
+    # linear field on the open lattice: |grad E| = |g| S2 at the centre; choose kappa so that R = 4 -> lambda = 1/5
+    kname, hfac = "wendland", 1.2
+    _, s2 = golden()[(kname, hfac)]
+    gvec = np.array([3.0, 0.0, 4.0])
+    x, y, z, h, g, m, rho, E, ctr = open_block_fields(kname, hfac, gvec, np.zeros((3, 3)), E0=10.0)
+    c = 2.5
+    for Rwant, lam in ((4.0, 0.2), (0.0, 1.0 / 3.0)):
+        if Rwant == 0.0:
+            Ein, kap = np.full_like(E, 10.0), np.ones_like(E)
+        else:
+            Ein, kap = E, np.full_like(E, 5.0 * s2 / (2.0 * 10.0 * Rwant))
+        li = O.limiter(g, KID[kname], x, y, z, h, m, rho, kap, Ein, c_light=c, targets=ctr)
+        assert li["R"][0] == pytest.approx(Rwant, rel=1e-12, abs=1e-15)
+        assert li["lam"][0] == pytest.approx(lam, rel=1e-12)
+        assert li["mu"][0] == pytest.approx(c * lam / (2.0 * kap[0]), rel=1e-12)
+    # optically thin limit: lambda * R -> 1
+    kap = np.full_like(E, 1e-9)
+    li = O.limiter(g, KID[kname], x, y, z, h, m, rho, kap, E, targets=ctr)
+    assert li["R"][0] > 1e7 and li["lam"][0] * li["R"][0] == pytest.approx(1.0, rel=1e-12)
+
+
+# ----------------------------------------------------------------------------- T9, T10, T11 invariants
+def rel_residual(terms):
+    return abs(terms.sum()) / np.abs(terms).sum()
+
+
+@pytest.mark.parametrize("name", ["cloud", "c4_tiny", "c2_tiny", "c5_tiny"])
+def test_T9_T10_momentum_and_energy_conservation(name):
+    w = W.random_cloud(2500, seed=3, periodic=(1, 1, 1), hvar=2.0) if name == "cloud" else W.make(name)
+    hy = O.hydro(w.grid, w.kernel, w.x, w.y, w.z, w.h, w.m, w.rho_nom, w.p, w.cs, w.vx, w.vy, w.vz, w.alpha, w.beta)
+    for k in ("ax", "ay", "az"):                                   # antisymmetry => sum m a = 0
+        assert abs((w.m * hy[k]).sum()) <= 1e-14 * (w.m * hy["S_" + k]).sum()
+    # eqs. (19) + (46): sum_a m_a (v_a . a_a + du_a/dt) = 0   (pins the sign A3 and the reading A7)
+    e = w.m * (w.vx * hy["ax"] + w.vy * hy["ay"] + w.vz * hy["az"] + hy["dudt"])
+    scale = (w.m * (np.abs(w.vx) * hy["S_ax"] + np.abs(w.vy) * hy["S_ay"] + np.abs(w.vz) * hy["S_az"] + hy["S_dudt"])).sum()
+    assert abs(e.sum()) <= 1e-14 * scale
+    if name == "cloud":
+        assert (hy["dudt"] - w.p / w.rho_nom * hy["divv"] >= -1e-18).all()    # viscous heating is non-negative
+        assert np.abs(hy["dudt"] - w.p / w.rho_nom * hy["divv"]).max() > 0    # and the AV branch was exercised
+
+
+def test_T11_fld_conservation_and_the_A17_reading():
+    w = W.random_cloud(2500, seed=5, periodic=(1, 1, 1), hvar=2.0)
+    mu = O.limiter(w.grid, w.kernel, w.x, w.y, w.z, w.h, w.m, w.rho_nom, w.kappa, w.E)["mu"]
+    V = w.m / w.rho_nom
+    ap = O.fld_apply(w.grid, w.kernel, w.x, w.y, w.z, w.h, w.m, w.rho_nom, mu, w.E, sym_mode=True)
+    assert abs((V * ap["y"]).sum()) <= 1e-14 * (V * ap["S_y"]).sum()         # conservative (SYMMETRIC)
+    assert (ap["diag"] <= 0).all()
+    assert np.allclose(ap["y"], ap["diag"] * w.E + ap["offd"], rtol=0, atol=1e-9 * ap["S_y"].max())   # T12
+    lit = O.fld_apply(w.grid, w.kernel, w.x, w.y, w.z, w.h, w.m, w.rho_nom, mu, w.E, sym_mode=False)
+    assert abs((V * lit["y"]).sum()) > 1e-6 * (V * lit["S_y"]).sum()         # literal eq. (47) is not, under variable h
+    # uniform h: both modes coincide
+    w = W.make("c1_tiny")
+    mu = O.limiter(w.grid, w.kernel, w.x, w.y, w.z, w.h, w.m, w.rho_nom, w.kappa, w.E)["mu"]
+    a = O.fld_apply(w.grid, w.kernel, w.x, w.y, w.z, w.h, w.m, w.rho_nom, mu, w.E, sym_mode=True)
+    b = O.fld_apply(w.grid, w.kernel, w.x, w.y, w.z, w.h, w.m, w.rho_nom, mu, w.E, sym_mode=False)
+    assert np.allclose(a["y"], b["y"], rtol=0, atol=1e-15 * a["S_y"].max())
+    V = w.m / w.rho_nom
+    assert abs((V * b["y"]).sum()) <= 1e-14 * (V * b["S_y"]).sum()
+
+
+def test_gather_only_sets_break_momentum_conservation():
+    """A13: with variable h, the symmetric set is what conserves momentum; summing eq. (11) over the gather set
+    only does not.  Checked by zeroing h_b's reach: a uniform-h copy of the same cloud conserves, and the symmetric
+    counts differ from the gather counts on the variable-h cloud."""
+    w = W.random_cloud(2400, seed=9, periodic=(1, 1, 1), hvar=2.0)
+    cg = O.neighbor_counts(w.grid, w.x, w.y, w.z, w.h, O.GATHER)
+    cs = O.neighbor_counts(w.grid, w.x, w.y, w.z, w.h, O.SYM)
+    assert (cs >= cg).all() and (cs > cg).any()
+
+
+# ----------------------------------------------------------------------------- T14 two-particle worked case
+@pytest.mark.parametrize("k,Fq1", [(O.WENDLAND_C2, -105 / (128 * PI)), (O.CUBIC_SPLINE, -3 / (4 * PI))])
+def test_T14_two_particles(k, Fq1):
+    h, m, rho, p = 0.2, 0.3, 1.7, 2.2
+    g = Grid((0, 0, 0), (4, 4, 4), (3, 3, 3), (0, 0, 0), h)
+    x = np.array([1.0 + h, 1.0]); y = np.array([1.0, 1.0]); z = np.array([1.0, 1.0])
+    one = np.ones(2)
+    for cells in (False, True):
+        hy = O.hydro(g, k, x, y, z, h * one, m * one, rho * one, p * one, one, 0 * one, 0 * one, 0 * one, one,
+                     use_cells=cells)
+        want = -2 * m * p * (Fq1 / h**4) / rho**2          # > 0: equal positive pressures repel (A3)
+        assert want > 0
+        assert hy["ax"][0] == pytest.approx(want, rel=1e-14)
+        assert hy["ax"][1] == pytest.approx(-want, rel=1e-14)
+        assert hy["ay"][0] == 0 and hy["az"][0] == 0 and hy["dudt"][0] == 0 and hy["divv"][0] == 0
+    # approaching pair (w < 0): compression => D > 0 ... eq. (37) gives d rho/dt > 0 (A4); viscosity repels and heats
+    vx = np.array([-0.5, 0.5])
+    cs, al, beta = 1.3, 0.8, 2.0
+    hy = O.hydro(g, k, x, y, z, h * one, m * one, rho * one, p * one, cs * one, vx, 0 * one, 0 * one, al * one, beta)
+    w = -1.0
+    F = Fq1 / h**4
+    D = (m / rho) * w * F
+    vs = al * cs + beta * abs(w)
+    a_visc = 0.5 * m * (2 * vs * F / rho) * w
+    q = 0.5 * m * vs * w * w * F
+    assert D > 0 and a_visc > 0 and q < 0
+    assert hy["divv"][0] == pytest.approx(D, rel=1e-14)
+    assert hy["ax"][0] == pytest.approx(-2 * m * p * F / rho**2 + a_visc, rel=1e-14)
+    assert hy["dudt"][0] == pytest.approx(p / rho * D - q / rho, rel=1e-14)
+    # receding pair: no viscosity (A6), PdV cooling
+    hy = O.hydro(g, k, x, y, z, h * one, m * one, rho * one, p * one, cs * one, -vx, 0 * one, 0 * one, al * one, beta)
+    assert hy["ax"][0] == pytest.approx(-2 * m * p * F / rho**2, rel=1e-14)
+    assert hy["dudt"][0] == pytest.approx(-p / rho * D, rel=1e-14)
+    # density of the pair: self term + neighbour (A11)
+    d = O.density(g, k, x, y, z, h * one, m * one)
+    assert d["rho"][0] == pytest.approx(m * (O.W(k, 0, h) + O.W(k, h, h)), rel=1e-15)
+    assert d["nnbr"][0] == 1
+
+
+# ----------------------------------------------------------------------------- T15 symmetries
+def test_T15_permutation_translation_mirror():
+    w = W.random_cloud(2000, seed=21, periodic=(1, 1, 1), hvar=1.8)
+    base = all_sweeps(w, True)
+    rng = np.random.default_rng(0)
+    perm = rng.permutation(w.n)
+    import copy
+    wp = copy.copy(w)
+    for f in ("x", "y", "z", "h", "m", "rho_nom", "p", "cs", "vx", "vy", "vz", "alpha", "E", "kappa"):
+        setattr(wp, f, getattr(w, f)[perm].copy())
+    rp = all_sweeps(wp, True)
+    for k in ("rho", "ax", "dudt", "mu", "y"):
+        S = base.get("S_" + k, np.abs(base[k]))
+        assert np.allclose(rp[k], base[k][perm], rtol=0, atol=1e-14 * S.max()), k
+    assert np.array_equal(rp["nnbr"], base["nnbr"][perm])
+    # translation by half a box in x (wraps particles): neighbour counts identical, sums equal to rounding
+    wt = copy.copy(w)
+    L = w.grid.hi[0] - w.grid.lo[0]
+    wt.x = np.mod(w.x + 0.5 * L, L)
+    wt.x = np.where(wt.x >= L, 0.0, wt.x)
+    rt = all_sweeps(wt, True)
+    assert np.array_equal(rt["nnbr"], base["nnbr"])
+    for k in ("rho", "ax", "ay", "dudt", "y"):
+        S = base.get("S_" + k, np.abs(base[k]))
+        assert np.allclose(rt[k], base[k], rtol=0, atol=1e-11 * S.max()), k
+    # mirror x -> L - x, vx -> -vx flips a_x only
+    wm = copy.copy(w)
+    wm.x = np.where(w.x == 0.0, 0.0, L - w.x)
+    wm.vx = -w.vx
+    rm = all_sweeps(wm, True)
+    assert np.allclose(rm["ax"], -base["ax"], rtol=0, atol=1e-11 * base["S_ax"].max())
+    assert np.allclose(rm["ay"], base["ay"], rtol=0, atol=1e-11 * base["S_ay"].max())
+    assert np.allclose(rm["dudt"], base["dudt"], rtol=0, atol=1e-11 * base["S_dudt"].max())
+    assert np.allclose(rm["y"], base["y"], rtol=0, atol=1e-11 * base["S_y"].max())
