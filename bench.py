@@ -1,0 +1,318 @@
+#!/usr/bin/env python
+"""bench.py -- SPH pair interactions/s of the full density + hydro + FLD pass (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c5] [--impl ours|reference]
+
+A step = one pass of the whole hot path: spray_build_cells -> spray_density -> spray_hydro_rhs
+-> spray_fld_apply(UPDATE_LIMITER) over one synthetic particle set (BASELINE.json configs, workloads/).
+`value` = pair interactions per second with inputs resident in HBM; `e2e` = the same through the C-ABI with pinned
+HOST buffers (H2D of every input and D2H of every output inside the timed region).  Multi-GPU: the path does not
+shard (BASELINE.json: one GPU, no collectives) -> N independent replicas, "weak" scaling, no data-path collective.
+Prints ONE JSON line on rank 0.  DESIGN.md §6 states the roofline arithmetic used below.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "SPH pair interactions/sec (density+hydro+FLD pass, fp64)"
+UNIT = "pair interactions/s"
+
+# Algorithmic flops per in-support ordered pair and sweep, counted from the defining formulas (DESIGN.md §6,
+# frozen in BASELINE.md §2): add/sub/mul/compare = 1, FMA = 2, div = 1, sqrt = 1; distance + predicate included.
+FLOPS = {0: dict(density=20, hydro=58, hydro_visc=25, limiter=32, apply=46),     # cubic spline
+         1: dict(density=23, hydro=60, hydro_visc=25, limiter=33, apply=48)}     # Wendland C2
+# Algorithmic HBM bytes per particle and pass: build 32 + sort 3*16 + reorder 64; gathers of 13
+# caller-order fields at 16 B; sweep reads 40/104/64/64 B and writes 12/40/8+8/24 B (outputs + perm).
+BYTES_PER_PARTICLE = 32 + 48 + 64 + 13 * 16 + (40 + 104 + 64 + 64) + (12 + 44 + 20 + 28)
+FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12    # 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz = 37.2
+
+
+def peaks():
+    try:
+        return json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))), "measured"
+    except Exception:
+        return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+                for nm, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+            except Exception:
+                pass
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample_pass(w, targets):
+    """The oracle as it stands on a bounded sample of the workload (its cell-list variant restricted to `targets`;
+    rho = recipe density and mu = c/(3 rho kappa) as inputs).  Returns (seconds, pair interactions)."""
+    import numpy as np
+    import oracle as O
+    a = (w.grid, w.kernel, w.x, w.y, w.z, w.h, w.m)
+    mu = w.c_light / (3.0 * w.rho_nom * w.kappa)
+    t0 = time.perf_counter()
+    d = O.density(*a, targets=targets)
+    O.hydro(*a, w.rho_nom, w.p, w.cs, w.vx, w.vy, w.vz, w.alpha, w.beta, targets=targets)
+    O.limiter(*a, w.rho_nom, w.kappa, w.E, w.c_light, targets=targets)
+    O.fld_apply(*a, w.rho_nom, mu, w.E, sym_mode=True, targets=targets)
+    dt = time.perf_counter() - t0
+    cg = d["nnbr"].astype(np.int64).sum()
+    cs = O.neighbor_counts(w.grid, w.x, w.y, w.z, w.h, O.SYM, targets=targets).astype(np.int64).sum()
+    return dt, int(2 * cg + 2 * cs + len(targets))
+
+
+def run_reference(args, w, rank):
+    """--impl reference: the CPU oracle (this tier's reference arm), rank 0 only, bounded sample per step."""
+    import numpy as np
+    import oracle as O
+    if rank != 0:
+        return
+    rng = np.random.default_rng(0)
+    ns = min(w.n, args.cpu_sample)
+    targets = np.sort(rng.choice(w.n, size=ns, replace=False)).astype(np.int64)
+    for _ in range(args.warmup):
+        oracle_sample_pass(w, targets[: max(1, ns // 8)])
+    tot_t, tot_p = 0.0, 0
+    for _ in range(args.steps):
+        dt, pairs = oracle_sample_pass(w, targets)
+        tot_t += dt; tot_p += pairs
+    v = tot_p / tot_t
+    sample = f"{ns} of {w.n} target particles of {w.name} per step (all neighbours), oracle cell-list variant, long-double sums"
+    print(json.dumps({"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+                      "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps, "higher_is_better": True, "scaling": "weak",
+                      "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": {"workload": w.name, "n_particles": w.n},
+                      "cpu_baseline": {"value": v, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle", "sample": sample},
+                      "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="c5", help="workloads.PRESETS name; c5 = BASELINE.json's roofline config (16.7 M particles)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--path", type=int, default=None, help="pair-kernel implementation (spray_set_path); default = library default")
+    ap.add_argument("--cpu-sample", type=int, default=200000, help="target particles per oracle step (cpu_baseline / reference arm)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+
+    import numpy as np
+    import workloads as W
+    w = W.make(args.workload)
+
+    if args.impl == "reference":
+        run_reference(args, w, rank)
+        return
+
+    import torch
+    import torch.distributed as dist
+    import paper_2604_20124_b200 as P
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the SPRAY pass has no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+
+    fields = ("x", "y", "z", "h", "m", "p", "cs", "vx", "vy", "vz", "alpha", "E", "kappa")
+    host = {f: torch.from_numpy(np.ascontiguousarray(getattr(w, f))).pin_memory() for f in fields}
+    d = {f: host[f].to(dev) for f in fields}
+    n = w.n
+    sp = P.Spray(n, w.grid.ncell_total, device=local_rank)
+    if args.path is not None:
+        sp.set_path(args.path)
+    f64 = torch.float64
+    out = {k: torch.empty(n, dtype=f64, device=dev) for k in ("rho", "ax", "ay", "az", "dudt", "divv", "mu", "y", "diag", "offd")}
+    hout = {k: torch.empty(n, dtype=f64).pin_memory() for k in out}
+
+    def one_pass(src, ev=None):
+        sp.build_cells(w.grid, w.kernel, src["x"], src["y"], src["z"], src["h"])
+        if ev: ev[1].record()
+        sp.density(src["m"], rho=out["rho"])
+        if ev: ev[2].record()
+        sp.hydro_rhs(src["m"], out["rho"], src["p"], src["cs"], src["vx"], src["vy"], src["vz"], src["alpha"], w.beta,
+                     out=[out["ax"], out["ay"], out["az"], out["dudt"], out["divv"]])
+        if ev: ev[3].record()
+        sp.fld_apply(src["m"], out["rho"], src["kappa"], src["E"], w.c_light, mu=out["mu"], y=out["y"], diag=out["diag"], offd=out["offd"])
+        if ev: ev[4].record()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # pair counts of this workload (outside the timed region)
+    one_pass(d)
+    cg = int(sp.neighbor_counts(False).to(torch.int64).sum().item())
+    cs = int(sp.neighbor_counts(True).to(torch.int64).sum().item())
+    assert sp.check() == 0, "device status flags set"
+    pairs = {"density": cg + n, "hydro": cs, "limiter": cg, "apply": cs}
+    p_pass = sum(pairs.values())
+
+    for _ in range(args.warmup):
+        one_pass(d)
+    l0 = sp.launch_count()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(5)] for _ in range(args.steps)]
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    barrier()
+    for s in range(args.steps):
+        evs[s][0].record()
+        one_pass(d, evs[s])
+    barrier()
+    clocks = sampler.stop()
+    launches = sp.launch_count() - l0
+    t_total = evs[0][0].elapsed_time(evs[-1][4]) * 1e-3
+    seg = np.array([[e[i].elapsed_time(e[i + 1]) for i in range(4)] for e in evs]) * 1e-3     # build, density, hydro, fld
+    if world > 1:
+        tt = torch.tensor([t_total], dtype=f64, device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        t_total = float(tt.item())
+    value = world * p_pass * args.steps / t_total
+
+    # ---- e2e: pinned host buffers, H2D of every input and D2H of every output inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        def e2e_pass():
+            for f in fields:
+                d[f].copy_(host[f], non_blocking=True)
+            one_pass(d)
+            for k in out:
+                hout[k].copy_(out[k], non_blocking=True)
+        e2e_pass()
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ksteps = max(2, min(args.steps, 5))
+        e0.record()
+        for _ in range(ksteps):
+            e2e_pass()
+        e1.record()
+        barrier()
+        te = e0.elapsed_time(e1) * 1e-3
+        if world > 1:
+            tt = torch.tensor([te], dtype=f64, device=dev)
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            te = float(tt.item())
+        e2e = {"value": world * p_pass * ksteps / te, "unit": UNIT, "h2d_bytes_per_step": 8 * n * len(fields),
+               "d2h_bytes_per_step": 8 * n * len(out), "ms_per_step": 1e3 * te / ksteps}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- FP64 peak probe (MEASURED_PEAKS.json has no FP64 entry): sustained DFMA rate, same job
+    pk, pk_src = peaks()
+    pb = torch.empty(148 * 8 * 256, dtype=f64, device=dev)
+    iters = 4000
+    P.fp64_peak_probe(local_rank, 148 * 8, 256, 200, pb)
+    torch.cuda.synchronize()
+    p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    p0.record()
+    for _ in range(10):
+        P.fp64_peak_probe(local_rank, 148 * 8, 256, iters, pb)
+    p1.record()
+    torch.cuda.synchronize()
+    fp64_meas = 10 * 148 * 8 * 256 * iters * 64 * 2 / (p0.elapsed_time(p1) * 1e-3) / 1e12
+
+    # ---- roofline: pass level and dominant kernel
+    fl = FLOPS[w.kernel]
+    visc_frac = 0.0 if not (np.any(w.vx) or np.any(w.vy) or np.any(w.vz)) else 0.5
+    flops = {"density": pairs["density"] * fl["density"], "hydro": pairs["hydro"] * (fl["hydro"] + visc_frac * fl["hydro_visc"]),
+             "limiter": pairs["limiter"] * fl["limiter"], "apply": pairs["apply"] * fl["apply"]}
+    seg_mean = seg.mean(axis=0)
+    t_step = t_total / args.steps
+    t_alu = sum(flops.values()) / (fp64_meas * 1e12)
+    t_hbm = BYTES_PER_PARTICLE * n / (pk["hbm_gbs"] * 1e9)
+    calls = {"build": seg_mean[0], "density": seg_mean[1], "hydro": seg_mean[2], "fld": seg_mean[3]}
+    hydro_tflops = flops["hydro"] / calls["hydro"] / 1e12
+    roofline = {"bound": "alu", "kernel": "hydro pair sweep (spray_hydro_rhs: SoA gather + pair kernel)",
+                "achieved": hydro_tflops, "peak": fp64_meas, "unit": "TFLOP/s", "frac": hydro_tflops / fp64_meas,
+                "peak_source": "DFMA-chain probe measured in this run (spray_fp64_peak_probe); nominal 148x64x2x1.965GHz = %.1f" % FP64_NOMINAL_TFLOPS,
+                "traffic": None,
+                "pass": {"flops": sum(flops.values()), "bytes": BYTES_PER_PARTICLE * n, "t_alu_ms": 1e3 * t_alu, "t_hbm_ms": 1e3 * t_hbm,
+                         "t_pass_ms": 1e3 * t_step, "frac": max(t_alu, t_hbm) / t_step, "hbm_peak_gbs": pk["hbm_gbs"], "hbm_peak_source": pk_src},
+                "per_call_ms": {k: 1e3 * float(v) for k, v in calls.items()},
+                "per_call_tflops": {"density": flops["density"] / calls["density"] / 1e12, "hydro": hydro_tflops,
+                                    "fld": (flops["limiter"] + flops["apply"]) / calls["fld"] / 1e12}}
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        import oracle as O
+        rng = np.random.default_rng(0)
+        ns = min(n, args.cpu_sample)
+        targets = np.sort(rng.choice(n, size=ns, replace=False)).astype(np.int64)
+        dt, pr = oracle_sample_pass(w, targets)
+        cpu = {"value": pr / dt, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle", "seconds": dt,
+               "sample": f"{ns} of {n} target particles of {w.name} (all their neighbours), oracle cell-list variant, long-double sums"}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 * t_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": w.name, "n_particles": n, "kernel": ["cubic_spline", "wendland_c2"][w.kernel], "grid": list(w.grid.ncell),
+                       "pairs_per_pass": p_pass, "unique_ordered_pairs": cs, "unique_pairs_per_s": world * cs * args.steps / t_total,
+                       "l2": "inputs larger than L2 (%.1f GB resident per replica)" % (8e-9 * n * (len(fields) + len(out))),
+                       "parallelism": "replicas only" if world > 1 else "1 GPU", "path": args.path},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
+            "fp64_probe_tflops": fp64_meas}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

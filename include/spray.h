@@ -1,0 +1,159 @@
+/*
+ * spray.h -- C-ABI of libspray_b200: the SPH particle-pair summation pass of SPRAY
+ * (arxiv/paper_2604_20124) as hand-written CUDA for sm_100a, one GPU, fp64.
+ *
+ * Citations: "P:L<n>" = line n of the paper text; "A<n>" = reading n of DESIGN.md §3
+ * (where the paper is silent, ambiguous or garbled).
+ *
+ * Conventions (all entry points)
+ *   - return value: 0 = SPRAY_OK, < 0 = error (enum below).  No exception, exit or abort crosses the ABI.
+ *     spray_last_error(ctx) returns a ctx-owned, NUL-terminated description of the last failure.
+ *   - every array pointer is a DEVICE pointer owned by the caller (fp64 or u32/u64 as typed, contiguous,
+ *     8-byte aligned, length n unless stated, CALLER ORDER = the order given to spray_build_cells).
+ *     The library neither frees nor keeps them beyond the stream work the call enqueues.
+ *     Output arrays must not alias inputs.  "nullable" outputs are skipped when NULL.
+ *   - `stream` is a cudaStream_t passed as void* (e.g. torch.cuda.current_stream().cuda_stream).  Calls only
+ *     ENQUEUE work on it and return; none synchronises except spray_check, spray_create and spray_destroy.
+ *   - the ctx owns all scratch (sorted SoA copies, keys, permutation, cell tables, neighbour lists), sized at
+ *     spray_create for n_max particles and ncell_max cells.  A ctx is bound to one device and is not
+ *     thread-safe; use one ctx per stream.
+ *   - inputs are not validated on the device: NaN or non-positive h, rho, E, kappa propagate as in the
+ *     defining formulas.  Host-checkable errors (sizes, grid) are reported by the return code; device-side
+ *     findings (h > declared h_max, position outside a periodic box, neighbour-list capacity exceeded)
+ *     are latched into a sticky status word read by spray_check.
+ *
+ * Notation: x_ab = x_a - x_b, r = |x_ab|, q = r/h; grad_a W(x_ab,h) = F(r;h) x_ab / r with F = dW/dr (A4);
+ *   V_b = m_b / rho_b.  Support radius is 2h for both kernels ("kappa = 2").
+ *   N_gather(a) = { b : r^2 < 4 h_a^2 } (contains a);  N_sym(a) = { b != a : r^2 < 4 max(h_a,h_b)^2 } (A13:
+ *   the mutual-neighbour set the paper's h' device produces).  r^2 = fma(dz,dz,fma(dy,dy,dx*dx)) with
+ *   minimum-image dx in periodic dimensions (A12, A15); the predicates are evaluated in exactly this form.
+ */
+#ifndef SPRAY_H_
+#define SPRAY_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct spray_ctx spray_ctx;
+
+typedef enum {
+    SPRAY_OK = 0,
+    SPRAY_ERR_INVALID_ARG = -1,
+    SPRAY_ERR_NOT_BUILT = -2,      /* a sweep was called before spray_build_cells succeeded */
+    SPRAY_ERR_GRID = -3,           /* ncell_d < 1, prod ncell_d > ncell_max, hi <= lo, or periodic L_d < 3*(2*h_max) */
+    SPRAY_ERR_CAPACITY = -4,       /* n > n_max */
+    SPRAY_ERR_CUDA = -5,
+    SPRAY_ERR_ALLOC = -6,
+    SPRAY_ERR_NOT_IMPLEMENTED = -7
+} spray_status_t;
+
+/* sticky device-side status bits returned by spray_check */
+enum {
+    SPRAY_DEV_H_EXCEEDS_HMAX = 1,  /* some h_a > grid.h_max (search range may be incomplete) */
+    SPRAY_DEV_OUTSIDE_BOX = 2,     /* a position outside [lo,hi) in a periodic dimension, or NaN */
+    SPRAY_DEV_LIST_OVERFLOW = 4    /* neighbour-list storage exhausted (results of the tiled path invalid) */
+};
+
+typedef enum { SPRAY_KERNEL_CUBIC_SPLINE = 0, SPRAY_KERNEL_WENDLAND_C2 = 1 } spray_kernel_t;
+typedef enum { SPRAY_FLD_SYMMETRIC = 0, SPRAY_FLD_GATHER = 1 } spray_fld_kernel_mode_t;       /* A17 */
+typedef enum { SPRAY_FLD_UPDATE_LIMITER = 0, SPRAY_FLD_FROZEN = 1 } spray_fld_limiter_mode_t; /* A18 */
+
+/* Uniform cell grid (an INPUT, A14; "dimensions of these cells are ... determined based on the average
+ * smoothing length ... during the initialization phase").  h_max is the caller-declared upper bound on h. */
+typedef struct {
+    double lo[3], hi[3];
+    int32_t ncell[3];
+    int32_t periodic[3];
+    double h_max;
+} spray_grid_t;
+
+/* Library / build information: "spray-b200 <version> sm_100a". Static string. */
+const char* spray_version(void);
+
+/* Create a context on CUDA device `device` with scratch for n_max particles and ncell_max cells.
+ * Host call; allocates device memory (SPRAY_ERR_ALLOC on failure). *out is set only on success. */
+int spray_create(spray_ctx** out, int64_t n_max, int64_t ncell_max, int device);
+/* Frees all scratch.  Synchronises the device. NULL is accepted. */
+int spray_destroy(spray_ctx* ctx);
+const char* spray_last_error(const spray_ctx* ctx);
+
+/* Debug: synchronises `stream`, stores the sticky device status bits in *dev_status (nullable) and clears them.
+ * Returns SPRAY_ERR_CUDA if any enqueued kernel faulted. */
+int spray_check(spray_ctx* ctx, void* stream, uint32_t* dev_status);
+
+/* Number of CUDA kernels this context has launched since spray_create (bench.py reports it as gpu_launches). */
+int64_t spray_launch_count(const spray_ctx* ctx);
+
+/* Select the pair-kernel implementation: 0 = reference kernels (one thread per particle walking the cell
+ * table), 1 = tiled kernels (shared-memory staged neighbour cells + per-particle neighbour lists built
+ * once per spray_build_cells).  Default 1 where available.  Both are CUDA; neither touches the host. */
+int spray_set_path(spray_ctx* ctx, int path);
+
+/* (a1)-(a4) NNPS: cell index per particle  c_d = floor((x_d - lo_d) * ncell_d / L_d) clamped,
+ * key = (c_z*ncell_y + c_y)*ncell_x + c_x;  STABLE sort of (key, caller index);  cell_start[c] = #{key < c},
+ * cell_end[c] = cell_start[c] + #{key = c};  sorted SoA copies of x, y, z, h;  per-cell max h;  per-particle
+ * symmetric search length;  neighbour lists for the tiled path.
+ * Stores `kernel` for the sweeps that follow.  x, y, z, h: device, [n], caller order, read only.
+ * Errors: SPRAY_ERR_CAPACITY (n > n_max), SPRAY_ERR_GRID, SPRAY_ERR_INVALID_ARG (NULL, n < 0). n = 0 is valid. */
+int spray_build_cells(spray_ctx* ctx, const spray_grid_t* grid, spray_kernel_t kernel, int64_t n,
+                      const double* x, const double* y, const double* z, const double* h, void* stream);
+
+/* (a5) density by summation, eq. (35):  rho_a = sum_{b in N_gather(a)} m_b W(r_ab; h_a), self included (A11).
+ * nnbr (nullable, u32[n]) = |N_gather(a)| - 1. */
+int spray_density(spray_ctx* ctx, const double* m, double* rho, uint32_t* nnbr, void* stream);
+
+/* (a6) hydro right-hand sides over N_sym(a) (pairs with r = 0 skipped, A11):
+ *   momentum, eq. (11) P:L98 with the sign of eqs. (5), (19) (A3):
+ *       a_a  = - sum_b m_b/(rho_a rho_b) [ p_a F(r;h_a) + p_b F(r;h_b) ] xhat_ab
+ *   dissipation, eqs. (41), (43) P:L236-L242, applied for w = v_ab . xhat_ab < 0 (A6), vsig_s = alpha_s c_s + beta |w| (A8):
+ *       a_a += sum_b (m_b/2) [ vsig_a F(r;h_a)/rho_a + vsig_b F(r;h_b)/rho_b ] w xhat_ab
+ *   divergence sum, eq. (37):   divv_sum_a = D_a = sum_b V_b w F(r;h_a)      (d rho/dt = rho D;  div v = -D)
+ *   energy, eq. (17) first term P:L129 + eq. (42) P:L238 (A7):
+ *       dudt_a = (p_a/rho_a) D_a - (1/rho_a) sum_b (m_b vsig_a / 2) w^2 F(r;h_a)
+ * Inputs [n] caller order; beta = 2 in the paper.  divv_sum nullable. */
+int spray_hydro_rhs(spray_ctx* ctx, const double* m, const double* rho, const double* p, const double* cs,
+                    const double* vx, const double* vy, const double* vz, const double* alpha, double beta,
+                    double* ax, double* ay, double* az, double* dudt, double* divv_sum, void* stream);
+
+/* (a7)+(a8) matrix-free apply of the SPH flux-limited-diffusion operator.
+ *   limiter pre-sweep (UPDATE_LIMITER only), P:L275 with grad E by eq. (9), phi = 1 (A19), over N_gather(a)\{a}:
+ *       gradE_a = sum_b V_b (E_b - E_a) F(r;h_a) xhat_ab;   R = |gradE|/(rho kappa E);
+ *       lambda = 1/sqrt(9 + R^2) (Larsen, k = 2, A20);   mu = c_light * lambda / (rho kappa)   -> written to mu[]
+ *   apply, eq. (47) first term P:L270 / eqs. (51)-(52) P:L283-L286 on the Laplacian form eq. (16) P:L125:
+ *       c_ab = V_b * 4 mu_a mu_b/(mu_a + mu_b) * Fbar/r
+ *       Fbar = (F(r;h_a)+F(r;h_b))/2 over N_sym(a)  [SPRAY_FLD_SYMMETRIC, A17]   or  F(r;h_a) over N_gather(a)\{a}  [SPRAY_FLD_GATHER]
+ *       y_a = sum_b c_ab (E_a - E_b) (difference form);  diag_a = Lambda_a = sum_b c_ab;  offd_a = Gamma_a = - sum_b c_ab E_b
+ * FROZEN: mu[] is read as given (the linear operator an implicit solve applies every iteration).
+ * kappa may be NULL in FROZEN mode.  diag, offd nullable.  gradE (nullable, [3n] as x|y|z planes) receives grad E
+ * in UPDATE_LIMITER mode. */
+int spray_fld_apply(spray_ctx* ctx, const double* m, const double* rho, const double* kappa, const double* E,
+                    double c_light, spray_fld_kernel_mode_t kmode, spray_fld_limiter_mode_t lmode,
+                    double* mu, double* y, double* diag, double* offd, double* gradE, void* stream);
+
+/* (K9) parity exports, all device outputs, caller-allocated.
+ * cell table: sorted_key[n], perm[n] (perm[i] = caller index of the particle in sorted slot i),
+ *             cell_start[ncell], cell_end[ncell].  Any pointer may be NULL. */
+int spray_get_cell_table(spray_ctx* ctx, uint32_t* sorted_key, uint32_t* perm, uint32_t* cell_start,
+                         uint32_t* cell_end, void* stream);
+/* count[a] = |N_sym(a)| (symmetric != 0) or |N_gather(a)| - 1 (symmetric == 0). */
+int spray_neighbor_counts(spray_ctx* ctx, int symmetric, uint32_t* count, void* stream);
+/* CSR neighbour lists: nbr[offsets[a] .. offsets[a]+count[a]) = caller ids of a's neighbours, ascending, self
+ * excluded.  offsets = exclusive scan of the counts (u64[n]). */
+int spray_neighbor_lists(spray_ctx* ctx, int symmetric, const uint64_t* offsets, uint32_t* nbr, void* stream);
+/* Order-independent digest of each neighbour set (for full-size parity without moving the CSR lists):
+ * dsum[a] = sum_b mix(id_b) mod 2^64, dxor[a] = xor_b mix(id_b), mix(v) = splitmix64(v): z = v + 0x9E3779B97F4A7C15,
+ * z = (z ^ z>>30) * 0xBF58476D1CE4E5B9, z = (z ^ z>>27) * 0x94D049BB133111EB, z ^ z>>31;  id_b = caller index of b. */
+int spray_neighbor_digest(spray_ctx* ctx, int symmetric, uint64_t* dsum, uint64_t* dxor, void* stream);
+
+/* Measurement aid: runs `iters` dependent DFMA per thread on `blocks` x `threads` threads
+ * with 8 independent chains; out (device, [blocks*threads]) receives the sums so the work cannot be elided.
+ * Used by bench.py to measure the sustained FP64 FMA peak the roofline is quoted against. */
+int spray_fp64_peak_probe(int device, int blocks, int threads, int64_t iters, double* out, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPRAY_H_ */

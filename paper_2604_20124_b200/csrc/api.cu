@@ -1,0 +1,286 @@
+// api.cu -- the C-ABI of include/spray.h: argument checks, scratch ownership, kernel sequencing.
+// Every step of the path runs in CUDA kernels enqueued on the caller's stream; nothing here touches particle
+// data on the host and there is no CPU fallback.
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "spray_internal.h"
+
+using namespace spray;
+
+namespace {
+
+thread_local char g_noctx_err[256] = "";
+
+int fail(Ctx* c, int code, const char* fmt, const char* a = "") {
+    char buf[512];
+    snprintf(buf, sizeof buf, fmt, a);
+    if (c) c->err = buf;
+    else { strncpy(g_noctx_err, buf, sizeof g_noctx_err - 1); }
+    return code;
+}
+int cuda_fail(Ctx* c, cudaError_t e, const char* where) {
+    char buf[512];
+    snprintf(buf, sizeof buf, "CUDA error in %s: %s", where, cudaGetErrorString(e));
+    if (c) c->err = buf;
+    return SPRAY_ERR_CUDA;
+}
+
+template <class T>
+bool dmalloc(T** p, int64_t count) {
+    if (count < 1) count = 1;
+    return cudaMalloc((void**)p, sizeof(T) * (size_t)count) == cudaSuccess;
+}
+
+void free_all(Ctx* c) {
+    for (int k = 0; k < 2; ++k) { cudaFree(c->key[k]); cudaFree(c->idx[k]); }
+    cudaFree(c->hist); cudaFree(c->cell_start); cudaFree(c->cell_end); cudaFree(c->cell_hmax);
+    cudaFree(c->hglob); cudaFree(c->dev_status);
+    cudaFree(c->s.x); cudaFree(c->s.y); cudaFree(c->s.z); cudaFree(c->s.h); cudaFree(c->s.hs);
+    for (double* f : c->s.f) cudaFree(f);
+}
+
+SweepArgs base_args(Ctx* c) {
+    SweepArgs a;
+    memset(&a, 0, sizeof a);
+    a.x = c->s.x; a.y = c->s.y; a.z = c->s.z; a.h = c->s.h; a.hs = c->s.hs;
+    return a;
+}
+
+#define CK(call, where) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) return cuda_fail(c, e__, where); } while (0)
+#define NEED_BUILT() do { if (!ctx) return SPRAY_ERR_INVALID_ARG; if (!ctx->c.built) return fail(&ctx->c, SPRAY_ERR_NOT_BUILT, "spray_build_cells has not succeeded on this context"); } while (0)
+
+enum { F_M = 0, F_RHO, F_P, F_CS, F_VX, F_VY, F_VZ, F_ALPHA, F_E, F_KAPPA, F_MU, F_SPARE };
+
+}  // namespace
+
+extern "C" {
+
+const char* spray_version(void) { return "spray-b200 0.1 sm_100a"; }
+
+int spray_create(spray_ctx** out, int64_t n_max, int64_t ncell_max, int device) {
+    if (!out || n_max < 0 || ncell_max < 1 || n_max > 0xFFFFFFF0ll || ncell_max > 0x7FFFFFFFll)
+        return fail(nullptr, SPRAY_ERR_INVALID_ARG, "spray_create: bad arguments");
+    if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return fail(nullptr, SPRAY_ERR_CUDA, "spray_create: cudaSetDevice failed"); }
+    spray_ctx* h = new (std::nothrow) spray_ctx();
+    if (!h) return SPRAY_ERR_ALLOC;
+    Ctx* c = &h->c;
+    c->device = device; c->n_max = n_max; c->ncell_max = ncell_max;
+    c->path = 0;
+    c->hist_cap = 256 * ((n_max + 4095) / 4096 + 1);
+    bool ok = true;
+    for (int k = 0; k < 2; ++k) ok = ok && dmalloc(&c->key[k], n_max) && dmalloc(&c->idx[k], n_max);
+    ok = ok && dmalloc(&c->hist, c->hist_cap) && dmalloc(&c->cell_start, ncell_max) && dmalloc(&c->cell_end, ncell_max) &&
+         dmalloc(&c->cell_hmax, ncell_max) && dmalloc(&c->hglob, 2) && dmalloc(&c->dev_status, 1) && dmalloc(&c->s.x, n_max) &&
+         dmalloc(&c->s.y, n_max) && dmalloc(&c->s.z, n_max) && dmalloc(&c->s.h, n_max) && dmalloc(&c->s.hs, n_max);
+    for (double*& f : c->s.f) ok = ok && dmalloc(&f, n_max);
+    if (ok) ok = cudaMemset(c->dev_status, 0, sizeof(uint32_t)) == cudaSuccess;
+    if (!ok) {
+        cudaGetLastError();
+        free_all(c);
+        delete h;
+        return fail(nullptr, SPRAY_ERR_ALLOC, "spray_create: device allocation failed");
+    }
+    *out = h;
+    return SPRAY_OK;
+}
+
+int spray_destroy(spray_ctx* ctx) {
+    if (!ctx) return SPRAY_OK;
+    cudaSetDevice(ctx->c.device);
+    cudaDeviceSynchronize();
+    free_all(&ctx->c);
+    delete ctx;
+    return SPRAY_OK;
+}
+
+const char* spray_last_error(const spray_ctx* ctx) { return ctx ? ctx->c.err.c_str() : g_noctx_err; }
+
+int spray_check(spray_ctx* ctx, void* stream, uint32_t* dev_status) {
+    if (!ctx) return SPRAY_ERR_INVALID_ARG;
+    Ctx* c = &ctx->c;
+    cudaStream_t st = (cudaStream_t)stream;
+    CK(cudaStreamSynchronize(st), "spray_check (a kernel enqueued earlier faulted)");
+    uint32_t v = 0;
+    CK(cudaMemcpy(&v, c->dev_status, sizeof v, cudaMemcpyDeviceToHost), "spray_check");
+    CK(cudaMemset(c->dev_status, 0, sizeof v), "spray_check");
+    if (dev_status) *dev_status = v;
+    return SPRAY_OK;
+}
+
+int64_t spray_launch_count(const spray_ctx* ctx) { return ctx ? ctx->c.launches : 0; }
+
+int spray_set_path(spray_ctx* ctx, int path) {
+    if (!ctx) return SPRAY_ERR_INVALID_ARG;
+    if (path != 0) return fail(&ctx->c, SPRAY_ERR_NOT_IMPLEMENTED, "tiled path not built into this library yet");
+    ctx->c.path = path;
+    return SPRAY_OK;
+}
+
+int spray_build_cells(spray_ctx* ctx, const spray_grid_t* g, spray_kernel_t kernel, int64_t n, const double* x,
+                      const double* y, const double* z, const double* h, void* stream) {
+    if (!ctx) return SPRAY_ERR_INVALID_ARG;
+    Ctx* c = &ctx->c;
+    c->built = false;
+    if (!g || n < 0 || (n > 0 && (!x || !y || !z || !h))) return fail(c, SPRAY_ERR_INVALID_ARG, "spray_build_cells: NULL argument or n < 0");
+    if (kernel != SPRAY_KERNEL_CUBIC_SPLINE && kernel != SPRAY_KERNEL_WENDLAND_C2)
+        return fail(c, SPRAY_ERR_INVALID_ARG, "spray_build_cells: unknown kernel id");
+    if (n > c->n_max) return fail(c, SPRAY_ERR_CAPACITY, "spray_build_cells: n > n_max");
+    int64_t nc = 1;
+    for (int d = 0; d < 3; ++d) {
+        if (g->ncell[d] < 1) return fail(c, SPRAY_ERR_GRID, "grid: ncell_d < 1");
+        if (!(g->hi[d] > g->lo[d])) return fail(c, SPRAY_ERR_GRID, "grid: hi <= lo");
+        nc *= g->ncell[d];
+        if (nc > c->ncell_max) return fail(c, SPRAY_ERR_GRID, "grid: prod ncell_d > ncell_max");
+        if (g->periodic[d] && !((g->hi[d] - g->lo[d]) >= 3.0 * (2.0 * g->h_max)))
+            return fail(c, SPRAY_ERR_GRID, "grid: periodic extent L_d < 3*(2*h_max): the minimum image would be ambiguous");
+    }
+    if (!(g->h_max > 0.0)) return fail(c, SPRAY_ERR_GRID, "grid: h_max must be > 0");
+    c->grid = *g; c->kernel = (int)kernel; c->n = n; c->ncell = nc;
+    for (int d = 0; d < 3; ++d) {
+        c->dg.lo[d] = g->lo[d];
+        c->dg.L[d] = g->hi[d] - g->lo[d];
+        c->dg.halfL[d] = 0.5 * c->dg.L[d];
+        c->dg.inv[d] = (double)g->ncell[d] / c->dg.L[d];
+        c->dg.nc[d] = g->ncell[d];
+        c->dg.per[d] = g->periodic[d] ? 1 : 0;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    CK(launch_cell_keys(c, x, y, z, st), "cell keys");
+    CK(launch_radix_sort(c, st), "radix sort");
+    CK(launch_cell_table(c, st), "cell table");
+    GatherJob job{};
+    job.count = 4;
+    job.in[0] = x; job.in[1] = y; job.in[2] = z; job.in[3] = h;
+    job.out[0] = c->s.x; job.out[1] = c->s.y; job.out[2] = c->s.z; job.out[3] = c->s.h;
+    CK(launch_gather(c, job, st), "reorder");
+    CK(launch_cell_hmax(c, st), "cell hmax");
+    // symmetric search length: hs = h, then raised by every particle that sees me with a larger h
+    if (n > 0) CK(cudaMemcpyAsync(c->s.hs, c->s.h, sizeof(double) * (size_t)n, cudaMemcpyDeviceToDevice, st), "hs init");
+    SweepArgs a = base_args(c);
+    a.o0 = c->s.hs;
+    CK(launch_ref_sweep(c, SW_HSEARCH, a, st), "search-length sweep");
+    c->built = true;
+    return SPRAY_OK;
+}
+
+int spray_density(spray_ctx* ctx, const double* m, double* rho, uint32_t* nnbr, void* stream) {
+    NEED_BUILT();
+    Ctx* c = &ctx->c;
+    if (c->n > 0 && (!m || !rho)) return fail(c, SPRAY_ERR_INVALID_ARG, "spray_density: NULL argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    GatherJob job{};
+    job.count = 1; job.in[0] = m; job.out[0] = c->s.f[F_M];
+    CK(launch_gather(c, job, st), "density gather");
+    SweepArgs a = base_args(c);
+    a.m = c->s.f[F_M]; a.o0 = rho; a.ocount = nnbr;
+    CK(launch_ref_sweep(c, SW_DENSITY, a, st), "density sweep");
+    return SPRAY_OK;
+}
+
+int spray_hydro_rhs(spray_ctx* ctx, const double* m, const double* rho, const double* p, const double* cs,
+                    const double* vx, const double* vy, const double* vz, const double* alpha, double beta,
+                    double* ax, double* ay, double* az, double* dudt, double* divv_sum, void* stream) {
+    NEED_BUILT();
+    Ctx* c = &ctx->c;
+    if (c->n > 0 && (!m || !rho || !p || !cs || !vx || !vy || !vz || !alpha || !ax || !ay || !az || !dudt))
+        return fail(c, SPRAY_ERR_INVALID_ARG, "spray_hydro_rhs: NULL argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    GatherJob job{};
+    const double* in[8] = {m, rho, p, cs, vx, vy, vz, alpha};
+    const int slot[8] = {F_M, F_RHO, F_P, F_CS, F_VX, F_VY, F_VZ, F_ALPHA};
+    job.count = 8;
+    for (int k = 0; k < 8; ++k) { job.in[k] = in[k]; job.out[k] = c->s.f[slot[k]]; }
+    CK(launch_gather(c, job, st), "hydro gather");
+    SweepArgs a = base_args(c);
+    a.m = c->s.f[F_M]; a.rho = c->s.f[F_RHO]; a.p = c->s.f[F_P]; a.cs = c->s.f[F_CS];
+    a.vx = c->s.f[F_VX]; a.vy = c->s.f[F_VY]; a.vz = c->s.f[F_VZ]; a.alpha = c->s.f[F_ALPHA];
+    a.beta = beta;
+    a.o0 = ax; a.o1 = ay; a.o2 = az; a.o3 = dudt; a.o4 = divv_sum;
+    CK(launch_ref_sweep(c, SW_HYDRO, a, st), "hydro sweep");
+    return SPRAY_OK;
+}
+
+int spray_fld_apply(spray_ctx* ctx, const double* m, const double* rho, const double* kappa, const double* E,
+                    double c_light, spray_fld_kernel_mode_t kmode, spray_fld_limiter_mode_t lmode, double* mu, double* y,
+                    double* diag, double* offd, double* gradE, void* stream) {
+    NEED_BUILT();
+    Ctx* c = &ctx->c;
+    const bool update = (lmode == SPRAY_FLD_UPDATE_LIMITER);
+    if (c->n > 0 && (!m || !rho || !E || !mu || !y || (update && !kappa)))
+        return fail(c, SPRAY_ERR_INVALID_ARG, "spray_fld_apply: NULL argument");
+    if ((kmode != SPRAY_FLD_SYMMETRIC && kmode != SPRAY_FLD_GATHER) || (lmode != SPRAY_FLD_UPDATE_LIMITER && lmode != SPRAY_FLD_FROZEN))
+        return fail(c, SPRAY_ERR_INVALID_ARG, "spray_fld_apply: unknown mode");
+    cudaStream_t st = (cudaStream_t)stream;
+    GatherJob job{};
+    job.in[0] = m; job.out[0] = c->s.f[F_M];
+    job.in[1] = rho; job.out[1] = c->s.f[F_RHO];
+    job.in[2] = E; job.out[2] = c->s.f[F_E];
+    job.in[3] = update ? kappa : mu; job.out[3] = update ? c->s.f[F_KAPPA] : c->s.f[F_MU];
+    job.count = 4;
+    CK(launch_gather(c, job, st), "fld gather");
+    SweepArgs a = base_args(c);
+    a.m = c->s.f[F_M]; a.rho = c->s.f[F_RHO]; a.E = c->s.f[F_E]; a.kappa = c->s.f[F_KAPPA]; a.mu = c->s.f[F_MU];
+    a.c_light = c_light;
+    if (update) {
+        SweepArgs l = a;
+        l.o0 = mu; l.o1 = gradE; l.mu_sorted = c->s.f[F_MU];
+        CK(launch_ref_sweep(c, SW_LIMITER, l, st), "limiter sweep");
+    }
+    a.fld_sym = (kmode == SPRAY_FLD_SYMMETRIC) ? 1 : 0;
+    a.o0 = y; a.o1 = diag; a.o2 = offd;
+    CK(launch_ref_sweep(c, SW_APPLY, a, st), "apply sweep");
+    return SPRAY_OK;
+}
+
+int spray_get_cell_table(spray_ctx* ctx, uint32_t* sorted_key, uint32_t* perm, uint32_t* cell_start, uint32_t* cell_end,
+                         void* stream) {
+    NEED_BUILT();
+    Ctx* c = &ctx->c;
+    cudaStream_t st = (cudaStream_t)stream;
+    size_t nb = sizeof(uint32_t) * (size_t)c->n, cb = sizeof(uint32_t) * (size_t)c->ncell;
+    if (sorted_key && c->n) CK(cudaMemcpyAsync(sorted_key, c->sorted_key, nb, cudaMemcpyDeviceToDevice, st), "get_cell_table");
+    if (perm && c->n) CK(cudaMemcpyAsync(perm, c->perm, nb, cudaMemcpyDeviceToDevice, st), "get_cell_table");
+    if (cell_start) CK(cudaMemcpyAsync(cell_start, c->cell_start, cb, cudaMemcpyDeviceToDevice, st), "get_cell_table");
+    if (cell_end) CK(cudaMemcpyAsync(cell_end, c->cell_end, cb, cudaMemcpyDeviceToDevice, st), "get_cell_table");
+    return SPRAY_OK;
+}
+
+int spray_neighbor_counts(spray_ctx* ctx, int symmetric, uint32_t* count, void* stream) {
+    NEED_BUILT();
+    Ctx* c = &ctx->c;
+    if (c->n > 0 && !count) return fail(c, SPRAY_ERR_INVALID_ARG, "spray_neighbor_counts: NULL argument");
+    SweepArgs a = base_args(c);
+    a.symmetric = symmetric; a.ocount = count;
+    CK(launch_ref_sweep(c, SW_COUNT, a, (cudaStream_t)stream), "neighbour count sweep");
+    return SPRAY_OK;
+}
+
+int spray_neighbor_lists(spray_ctx* ctx, int symmetric, const uint64_t* offsets, uint32_t* nbr, void* stream) {
+    NEED_BUILT();
+    Ctx* c = &ctx->c;
+    if (c->n > 0 && (!offsets || !nbr)) return fail(c, SPRAY_ERR_INVALID_ARG, "spray_neighbor_lists: NULL argument");
+    SweepArgs a = base_args(c);
+    a.symmetric = symmetric; a.offsets = offsets; a.onbr = nbr;
+    CK(launch_ref_sweep(c, SW_LIST, a, (cudaStream_t)stream), "neighbour list sweep");
+    return SPRAY_OK;
+}
+
+int spray_neighbor_digest(spray_ctx* ctx, int symmetric, uint64_t* dsum, uint64_t* dxor, void* stream) {
+    NEED_BUILT();
+    Ctx* c = &ctx->c;
+    if (c->n > 0 && (!dsum || !dxor)) return fail(c, SPRAY_ERR_INVALID_ARG, "spray_neighbor_digest: NULL argument");
+    SweepArgs a = base_args(c);
+    a.symmetric = symmetric; a.odsum = dsum; a.odxor = dxor;
+    CK(launch_ref_sweep(c, SW_DIGEST, a, (cudaStream_t)stream), "neighbour digest sweep");
+    return SPRAY_OK;
+}
+
+int spray_fp64_peak_probe(int device, int blocks, int threads, int64_t iters, double* out, void* stream) {
+    if (!out || blocks < 1 || threads < 1 || threads > 256 || iters < 0) return SPRAY_ERR_INVALID_ARG;
+    if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return SPRAY_ERR_CUDA; }
+    return launch_fp64_probe(blocks, threads, iters, out, (cudaStream_t)stream) == cudaSuccess ? SPRAY_OK : SPRAY_ERR_CUDA;
+}
+
+}  // extern "C"

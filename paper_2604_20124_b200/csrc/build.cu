@@ -1,0 +1,227 @@
+// build.cu -- (a1)-(a4) of the hot path: cell key, stable LSD radix sort, cell table, SoA reorder.
+// NNPS by a cell list, PAPER.md L438 (§2.6): "the index of the cell that each particle resides in can be easily
+// computed ... the particles are sorted based on their cell indices, so that the particles in any arbitrary cell
+// can be identified directly".
+#include "spray_internal.h"
+
+namespace spray {
+
+// ------------------------------------------------------------------------------------------- K1: cell key
+// c_d = (int) floor((x_d - lo_d) * inv_d) clamped to [0, nc_d-1]; key = (c_z*nc_y + c_y)*nc_x + c_x.
+// Subtract then multiply (two roundings, nothing to contract).  24 B read + 8 B written per particle.
+__global__ void k_cell_key(DevGrid g, int64_t n, const double* __restrict__ x, const double* __restrict__ y,
+                           const double* __restrict__ z, uint32_t* __restrict__ key, uint32_t* __restrict__ idx,
+                           uint32_t* __restrict__ status) {
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double p[3] = {x[i], y[i], z[i]};
+    int c[3];
+    bool bad = false;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        double t = floor(__dmul_rn(__dsub_rn(p[d], g.lo[d]), g.inv[d]));
+        int ci = (t < 0.0) ? 0 : (t >= (double)g.nc[d] ? g.nc[d] - 1 : (int)t);
+        if (!(t == t)) { ci = 0; bad = true; }
+        if (g.per[d] && !(p[d] >= g.lo[d] && p[d] < g.lo[d] + g.L[d])) bad = true;
+        c[d] = ci;
+    }
+    key[i] = (uint32_t)((c[2] * g.nc[1] + c[1]) * g.nc[0] + c[0]);
+    idx[i] = (uint32_t)i;
+    if (bad) atomicOr(status, (uint32_t)SPRAY_DEV_OUTSIDE_BOX);
+}
+
+// ------------------------------------------------------------------------------------------- K2: radix sort
+// Stable LSD radix sort of (key, idx), 8 bits per pass, ceil(bits(ncell-1)/8) passes.
+// Per pass: per-tile digit histogram -> exclusive scan over [digit][tile] -> stable scatter.
+// Stability inside a tile: each warp owns a contiguous run of the tile and ranks its keys round by round with
+// __match_any_sync, so equal digits keep ascending position; warps are then offset in warp order.
+constexpr int RS_THREADS = 256;
+constexpr int RS_ITEMS = 16;
+constexpr int RS_TILE = RS_THREADS * RS_ITEMS;   // 4096 keys per CTA
+constexpr int RS_WARPS = RS_THREADS / 32;
+
+__global__ void __launch_bounds__(RS_THREADS)
+k_rs_hist(const uint32_t* __restrict__ key, int64_t n, int shift, uint32_t* __restrict__ hist, int nblk) {
+    __shared__ uint32_t sh[256];
+    sh[threadIdx.x] = 0;
+    __syncthreads();
+    int64_t base = (int64_t)blockIdx.x * RS_TILE;
+#pragma unroll
+    for (int j = 0; j < RS_ITEMS; ++j) {
+        int64_t i = base + j * RS_THREADS + threadIdx.x;
+        if (i < n) atomicAdd(&sh[(key[i] >> shift) & 255u], 1u);
+    }
+    __syncthreads();
+    hist[(int64_t)threadIdx.x * nblk + blockIdx.x] = sh[threadIdx.x];
+}
+
+// single-CTA exclusive scan, in place, of `total` u32 counters (total = 256 * ntiles <= ~1.1 M at 16.7 M keys)
+__global__ void __launch_bounds__(1024) k_rs_scan(uint32_t* __restrict__ a, int64_t total) {
+    __shared__ uint32_t part[1024];
+    int t = threadIdx.x;
+    int64_t chunk = (total + 1023) / 1024;
+    int64_t b = t * chunk, e = b + chunk < total ? b + chunk : total;
+    uint32_t s = 0;
+    for (int64_t i = b; i < e; ++i) s += a[i];
+    part[t] = s;
+    __syncthreads();
+    for (int off = 1; off < 1024; off <<= 1) {       // Hillis-Steele inclusive scan of the partials
+        uint32_t v = (t >= off) ? part[t - off] : 0;
+        __syncthreads();
+        part[t] += v;
+        __syncthreads();
+    }
+    uint32_t run = part[t] - s;                       // exclusive prefix of this chunk
+    for (int64_t i = b; i < e; ++i) { uint32_t v = a[i]; a[i] = run; run += v; }
+}
+
+__global__ void __launch_bounds__(RS_THREADS)
+k_rs_scatter(const uint32_t* __restrict__ key_in, const uint32_t* __restrict__ idx_in, uint32_t* __restrict__ key_out,
+             uint32_t* __restrict__ idx_out, int64_t n, int shift, const uint32_t* __restrict__ hist, int nblk) {
+    __shared__ uint32_t wh[RS_WARPS][256];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    for (int i = threadIdx.x; i < RS_WARPS * 256; i += RS_THREADS) (&wh[0][0])[i] = 0;
+    __syncthreads();
+    const int64_t base = (int64_t)blockIdx.x * RS_TILE + (int64_t)w * (RS_ITEMS * 32);
+    uint32_t k[RS_ITEMS], v[RS_ITEMS], rank[RS_ITEMS];
+    const uint32_t lt = (1u << lane) - 1u;
+#pragma unroll
+    for (int r = 0; r < RS_ITEMS; ++r) {
+        int64_t i = base + r * 32 + lane;
+        bool ok = i < n;
+        k[r] = ok ? key_in[i] : 0xFFFFFFFFu;
+        v[r] = ok ? idx_in[i] : 0u;
+        uint32_t d = ok ? ((k[r] >> shift) & 255u) : 256u;       // 256 = padding lane, its own match group
+        uint32_t peers = __match_any_sync(0xFFFFFFFFu, d);
+        int leader = __ffs(peers) - 1;
+        uint32_t old = 0;
+        if (lane == leader && ok) { old = wh[w][d]; wh[w][d] = old + __popc(peers); }
+        old = __shfl_sync(0xFFFFFFFFu, old, leader);
+        rank[r] = old + __popc(peers & lt);
+        __syncwarp();
+    }
+    __syncthreads();
+    {   // per digit: global offset of this tile, then warps in order
+        int d = threadIdx.x;
+        uint32_t run = hist[(int64_t)d * nblk + blockIdx.x];
+#pragma unroll
+        for (int ww = 0; ww < RS_WARPS; ++ww) { uint32_t t = wh[ww][d]; wh[ww][d] = run; run += t; }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int r = 0; r < RS_ITEMS; ++r) {
+        int64_t i = base + r * 32 + lane;
+        if (i < n) {
+            uint32_t d = (k[r] >> shift) & 255u;
+            uint32_t pos = wh[w][d] + rank[r];
+            key_out[pos] = k[r];
+            idx_out[pos] = v[r];
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------- K3: cell table
+// cell_start[c] = #{key < c} = lower_bound(sorted_key, c); cell_end[c] = lower_bound(sorted_key, c+1).
+__device__ __forceinline__ uint32_t lower_bound_u32(const uint32_t* __restrict__ a, uint32_t n, uint32_t v) {
+    uint32_t lo = 0, hi = n;
+    while (lo < hi) {
+        uint32_t mid = (lo + hi) >> 1;
+        if (__ldg(a + mid) < v) lo = mid + 1; else hi = mid;
+    }
+    return lo;
+}
+__global__ void k_cell_table(const uint32_t* __restrict__ sorted_key, uint32_t n, uint32_t ncell,
+                             uint32_t* __restrict__ cell_start, uint32_t* __restrict__ cell_end) {
+    uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c > ncell) return;
+    uint32_t lb = lower_bound_u32(sorted_key, n, c);
+    if (c < ncell) cell_start[c] = lb;
+    if (c > 0) cell_end[c - 1] = lb;
+}
+
+// ------------------------------------------------------------------------------------------- K4: SoA reorder
+__global__ void k_gather(GatherJob job, const uint32_t* __restrict__ perm, int64_t n) {
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    uint32_t p = perm[i];
+#pragma unroll 4
+    for (int k = 0; k < job.count; ++k) job.out[k][i] = __ldg(job.in[k] + p);
+}
+
+// per-cell max h (fp64 max is exact and order independent), global min/max of h, and the h <= h_max check
+__global__ void k_init_hglob(double* hglob) { hglob[0] = __longlong_as_double(0x7FF0000000000000ll); hglob[1] = 0.0; }
+
+__global__ void k_cell_hmax(const uint32_t* __restrict__ cell_start, const uint32_t* __restrict__ cell_end,
+                            const double* __restrict__ h, uint32_t ncell, double hmax_decl,
+                            double* __restrict__ cell_hmax, double* __restrict__ hglob, uint32_t* __restrict__ status) {
+    uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
+    double mx = 0.0, mn = __longlong_as_double(0x7FF0000000000000ll);
+    if (c < ncell) {
+        for (uint32_t j = cell_start[c]; j < cell_end[c]; ++j) { double v = h[j]; mx = fmax(mx, v); mn = fmin(mn, v); }
+        cell_hmax[c] = mx;
+    }
+    // warp reduce, then one atomic per warp on the bit patterns (positive doubles order like integers)
+    for (int o = 16; o; o >>= 1) {
+        mx = fmax(mx, __shfl_xor_sync(0xFFFFFFFFu, mx, o));
+        mn = fmin(mn, __shfl_xor_sync(0xFFFFFFFFu, mn, o));
+    }
+    if ((threadIdx.x & 31) == 0) {
+        if (mx > 0.0) atomicMax((unsigned long long*)&hglob[1], (unsigned long long)__double_as_longlong(mx));
+        if (mn > 0.0) atomicMin((unsigned long long*)&hglob[0], (unsigned long long)__double_as_longlong(mn));
+        if (mx > hmax_decl) atomicOr(status, (uint32_t)SPRAY_DEV_H_EXCEEDS_HMAX);
+    }
+}
+
+// ------------------------------------------------------------------------------------------- launchers
+static inline int cdiv64(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
+
+cudaError_t launch_cell_keys(Ctx* c, const double* x, const double* y, const double* z, cudaStream_t st) {
+    if (c->n == 0) return cudaSuccess;
+    k_cell_key<<<cdiv64(c->n, 256), 256, 0, st>>>(c->dg, c->n, x, y, z, c->key[0], c->idx[0], c->dev_status);
+    c->launches += 1;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_radix_sort(Ctx* c, cudaStream_t st) {
+    int bits = 0;
+    while (((int64_t)1 << bits) < c->ncell) ++bits;
+    int passes = (bits + 7) / 8;
+    int cur = 0;
+    int nblk = cdiv64(c->n, RS_TILE);
+    for (int p = 0; p < passes && c->n > 0; ++p) {
+        int shift = 8 * p;
+        k_rs_hist<<<nblk, RS_THREADS, 0, st>>>(c->key[cur], c->n, shift, c->hist, nblk);
+        k_rs_scan<<<1, 1024, 0, st>>>(c->hist, (int64_t)256 * nblk);
+        k_rs_scatter<<<nblk, RS_THREADS, 0, st>>>(c->key[cur], c->idx[cur], c->key[cur ^ 1], c->idx[cur ^ 1], c->n, shift,
+                                                  c->hist, nblk);
+        cur ^= 1;
+        c->launches += 3;
+    }
+    c->sorted_key = c->key[cur];
+    c->perm = c->idx[cur];
+    return cudaGetLastError();
+}
+
+cudaError_t launch_cell_table(Ctx* c, cudaStream_t st) {
+    k_cell_table<<<cdiv64(c->ncell + 1, 256), 256, 0, st>>>(c->sorted_key, (uint32_t)c->n, (uint32_t)c->ncell, c->cell_start,
+                                                           c->cell_end);
+    c->launches += 1;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_gather(Ctx* c, const GatherJob& job, cudaStream_t st) {
+    if (c->n == 0 || job.count == 0) return cudaSuccess;
+    k_gather<<<cdiv64(c->n, 256), 256, 0, st>>>(job, c->perm, c->n);
+    c->launches += 1;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_cell_hmax(Ctx* c, cudaStream_t st) {
+    k_init_hglob<<<1, 1, 0, st>>>(c->hglob);
+    k_cell_hmax<<<cdiv64(c->ncell, 256), 256, 0, st>>>(c->cell_start, c->cell_end, c->s.h, (uint32_t)c->ncell, c->grid.h_max,
+                                                      c->cell_hmax, c->hglob, c->dev_status);
+    c->launches += 2;
+    return cudaGetLastError();
+}
+
+}  // namespace spray

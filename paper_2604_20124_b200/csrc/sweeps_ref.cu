@@ -1,0 +1,216 @@
+// sweeps_ref.cu -- reference pair kernels: one CUDA thread per particle walking the cell table, the scheme the
+// paper describes ("each CUDA thread carries out relevant SPH calculation for one particle, looping
+// over neighbor particles").  General in every respect (any search range, any grid, variable h); used for the
+// parity exports, for the symmetric-search-length pre-pass, and as the fallback of the tiled kernels.
+#include "spray_internal.h"
+
+namespace spray {
+
+struct CellTabs {
+    const uint32_t *sorted_key, *perm, *cell_start, *cell_end;
+    const double* hglob;
+};
+
+// cells to visit along one dimension: `cnt` cells starting at `start` (wrapped when periodic)
+struct Span { int start, cnt; };
+__device__ __forceinline__ Span cell_span(const DevGrid& g, int d, int c, double reach) {
+    int nc = g.nc[d];
+    double rr = reach * g.inv[d] * (1.0 + 1e-12);
+    int R = rr < (double)nc ? (int)ceil(rr) : nc;
+    Span s;
+    if (g.per[d]) {
+        if (2 * R + 1 >= nc) { s.start = 0; s.cnt = nc; }
+        else { s.start = c - R; s.cnt = 2 * R + 1; }
+    } else {
+        int a = c - R < 0 ? 0 : c - R, b = c + R > nc - 1 ? nc - 1 : c + R;
+        s.start = a; s.cnt = b - a + 1;
+    }
+    return s;
+}
+__device__ __forceinline__ int wrap_cell(int c, int nc) { return c < 0 ? c + nc : (c >= nc ? c - nc : c); }
+
+template <int SWEEP, int KERNEL>
+__global__ void __launch_bounds__(128)
+k_ref_sweep(DevGrid g, int64_t n, CellTabs T, SweepArgs A) {
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double xa = A.x[i], ya = A.y[i], za = A.z[i], ha = A.h[i];
+    const uint32_t ia = T.perm[i];
+
+    bool sym;
+    if (SWEEP == SW_HYDRO) sym = true;
+    else if (SWEEP == SW_APPLY) sym = A.fld_sym != 0;
+    else if (SWEEP == SW_COUNT || SWEEP == SW_LIST || SWEEP == SW_DIGEST) sym = A.symmetric != 0;
+    else sym = false;
+    if (SWEEP == SW_HSEARCH) {
+        if (!(ha > T.hglob[0])) return;      // nobody has a smaller h: nothing to raise
+    }
+    const double reach = 2.0 * (sym ? A.hs[i] : ha);
+    const double sup_a = support2(ha);
+
+    const uint32_t key = T.sorted_key[i];
+    const int cx = key % g.nc[0], cy = (key / g.nc[0]) % g.nc[1], cz = key / (g.nc[0] * g.nc[1]);
+    const Span sx = cell_span(g, 0, cx, reach), sy = cell_span(g, 1, cy, reach), sz = cell_span(g, 2, cz, reach);
+
+    // per-particle constants
+    const double hinv = 1.0 / ha;
+    double acc0 = 0, acc1 = 0, acc2 = 0, acc3 = 0, acc4 = 0;
+    uint32_t cnt = 0;
+    uint64_t dsum = 0, dxr = 0;
+    double rho_a = 0, p_a = 0, vxa = 0, vya = 0, vza = 0, ac_a = 0, E_a = 0, mu_a = 0, Wn = 0, Fn = 0;
+    Wn = sigma<KERNEL>() * hinv * hinv * hinv;          // sigma / h^3
+    Fn = Wn * hinv;                                      // sigma / h^4
+    if (SWEEP == SW_HYDRO) {
+        rho_a = A.rho[i]; p_a = A.p[i]; vxa = A.vx[i]; vya = A.vy[i]; vza = A.vz[i]; ac_a = A.alpha[i] * A.cs[i];
+    }
+    if (SWEEP == SW_LIMITER) { E_a = A.E[i]; }
+    if (SWEEP == SW_APPLY) { E_a = A.E[i]; mu_a = A.mu[i]; }
+    uint64_t lbase = 0;
+    if (SWEEP == SW_LIST) lbase = A.offsets[ia];
+
+    for (int kz = 0; kz < sz.cnt; ++kz) {
+        const int czz = g.per[2] ? wrap_cell(sz.start + kz, g.nc[2]) : sz.start + kz;
+        for (int ky = 0; ky < sy.cnt; ++ky) {
+            const int cyy = g.per[1] ? wrap_cell(sy.start + ky, g.nc[1]) : sy.start + ky;
+            for (int kx = 0; kx < sx.cnt; ++kx) {
+                const int cxx = g.per[0] ? wrap_cell(sx.start + kx, g.nc[0]) : sx.start + kx;
+                const uint32_t c = (uint32_t)((czz * g.nc[1] + cyy) * g.nc[0] + cxx);
+                const uint32_t jb = __ldg(T.cell_start + c), je = __ldg(T.cell_end + c);
+                for (uint32_t j = jb; j < je; ++j) {
+                    const double dx = min_image(__dsub_rn(xa, __ldg(A.x + j)), g.per[0], g.L[0], g.halfL[0]);
+                    const double dy = min_image(__dsub_rn(ya, __ldg(A.y + j)), g.per[1], g.L[1], g.halfL[1]);
+                    const double dz = min_image(__dsub_rn(za, __ldg(A.z + j)), g.per[2], g.L[2], g.halfL[2]);
+                    const double r2 = r2_exact(dx, dy, dz);
+                    const double hb = __ldg(A.h + j);
+                    const bool self = (j == (uint32_t)i);
+                    const bool in_g = r2 < sup_a;
+                    const bool in_s = !self && (r2 < support2(fmax(ha, hb)));
+                    const bool in_set = sym ? in_s : (in_g && !self);
+
+                    if (SWEEP == SW_DENSITY) {
+                        // eq. (35), self term included (A11)
+                        if (in_g) {
+                            double q = sqrt(r2) * hinv;
+                            acc0 += A.m[j] * shape_w<KERNEL>(q);
+                            cnt += self ? 0u : 1u;
+                        }
+                    } else if (SWEEP == SW_HSEARCH) {
+                        // make neighbours mutual -- raise the search length of every a that I see but that may not see me
+                        if (in_g && !self && hb < ha)
+                            atomicMax((unsigned long long*)(A.o0 + j), (unsigned long long)__double_as_longlong(ha));
+                    } else if (SWEEP == SW_COUNT) {
+                        cnt += in_set ? 1u : 0u;
+                    } else if (SWEEP == SW_LIST) {
+                        if (in_set) A.onbr[lbase + cnt++] = T.perm[j];
+                    } else if (SWEEP == SW_DIGEST) {
+                        if (in_set) { uint64_t hsh = mix64((uint64_t)T.perm[j]); dsum += hsh; dxr ^= hsh; }
+                    } else if (SWEEP == SW_HYDRO) {
+                        if (in_s && r2 > 0.0) {
+                            const double r = sqrt(r2), rinv = 1.0 / r;
+                            const double hbinv = 1.0 / hb;
+                            const double Fa = Fn * shape_f<KERNEL>(r * hinv);
+                            const double Fb = sigma<KERNEL>() * (hbinv * hbinv) * (hbinv * hbinv) * shape_f<KERNEL>(r * hbinv);
+                            const double mb = A.m[j], rho_b = A.rho[j], p_b = A.p[j];
+                            const double w = ((vxa - A.vx[j]) * dx + (vya - A.vy[j]) * dy + (vza - A.vz[j]) * dz) * rinv;
+                            // eq. (11) P:L98 with the sign of eq. (5) (A3)
+                            double coef = -(mb / (rho_a * rho_b)) * (p_a * Fa + p_b * Fb);
+                            if (w < 0.0) {   // eqs. (41)-(43) P:L236-L242 (A6, A7, A8)
+                                const double aw = -w;
+                                const double vsa = ac_a + A.beta * aw;
+                                const double vsb = A.alpha[j] * A.cs[j] + A.beta * aw;
+                                coef += 0.5 * mb * (vsa * Fa / rho_a + vsb * Fb / rho_b) * w;
+                                acc4 += 0.5 * mb * vsa * (w * w) * Fa;
+                            }
+                            const double cr = coef * rinv;
+                            acc0 += cr * dx; acc1 += cr * dy; acc2 += cr * dz;
+                            acc3 += (mb / rho_b) * w * Fa;      // eq. (37)
+                        }
+                    } else if (SWEEP == SW_LIMITER) {
+                        if (in_g && !self && r2 > 0.0) {
+                            // eq. (9) phi = 1 with f = E (A19)
+                            const double r = sqrt(r2);
+                            const double cc = (A.m[j] / A.rho[j]) * (A.E[j] - E_a) * (Fn * shape_f<KERNEL>(r * hinv)) / r;
+                            acc0 += cc * dx; acc1 += cc * dy; acc2 += cc * dz;
+                        }
+                    } else if (SWEEP == SW_APPLY) {
+                        if (in_set && r2 > 0.0) {
+                            // eq. (47) first term P:L270 on eq. (16); Fbar as P:L134 (A17)
+                            const double r = sqrt(r2);
+                            double Fbar = Fn * shape_f<KERNEL>(r * hinv);
+                            if (sym) {
+                                const double hbinv = 1.0 / hb;
+                                Fbar = 0.5 * (Fbar + sigma<KERNEL>() * (hbinv * hbinv) * (hbinv * hbinv) * shape_f<KERNEL>(r * hbinv));
+                            }
+                            const double mu_b = A.mu[j], E_b = A.E[j];
+                            const double cab = (A.m[j] / A.rho[j]) * (4.0 * mu_a * mu_b / (mu_a + mu_b)) * (Fbar / r);
+                            acc0 += cab * (E_a - E_b);
+                            acc1 += cab;
+                            acc2 -= cab * E_b;
+                        }
+                    }
+                }
+            }
+        }
+    }
+
+    if (SWEEP == SW_DENSITY) {
+        A.o0[ia] = Wn * acc0;
+        if (A.ocount) A.ocount[ia] = cnt;
+    } else if (SWEEP == SW_COUNT) {
+        A.ocount[ia] = cnt;
+    } else if (SWEEP == SW_DIGEST) {
+        A.odsum[ia] = dsum; A.odxor[ia] = dxr;
+    } else if (SWEEP == SW_LIST) {
+        // ascending caller ids (debug export: insertion sort of this particle's segment)
+        uint32_t* L = A.onbr + lbase;
+        for (uint32_t a = 1; a < cnt; ++a) {
+            uint32_t v = L[a]; int b = (int)a - 1;
+            while (b >= 0 && L[b] > v) { L[b + 1] = L[b]; --b; }
+            L[b + 1] = v;
+        }
+    } else if (SWEEP == SW_HYDRO) {
+        A.o0[ia] = acc0; A.o1[ia] = acc1; A.o2[ia] = acc2;
+        A.o3[ia] = (p_a / rho_a) * acc3 - acc4 / rho_a;       // eq. (17) 1st term P:L129 + eq. (42)
+        if (A.o4) A.o4[ia] = acc3;
+    } else if (SWEEP == SW_LIMITER) {
+        // Larsen limiter, k = 2 (A20)
+        const double rk = A.rho[i] * A.kappa[i];
+        const double gn = sqrt(acc0 * acc0 + acc1 * acc1 + acc2 * acc2);
+        const double R = gn / (rk * E_a);
+        const double mu = A.c_light * (1.0 / sqrt(9.0 + R * R)) / rk;
+        A.o0[ia] = mu;
+        A.mu_sorted[i] = mu;
+        if (A.o1) { A.o1[ia] = acc0; A.o1[n + ia] = acc1; A.o1[2 * n + ia] = acc2; }
+    } else if (SWEEP == SW_APPLY) {
+        A.o0[ia] = acc0;
+        if (A.o1) A.o1[ia] = acc1;
+        if (A.o2) A.o2[ia] = acc2;
+    }
+}
+
+template <int SWEEP>
+static cudaError_t launch_k(Ctx* c, const SweepArgs& a, cudaStream_t st) {
+    if (c->n == 0) return cudaSuccess;
+    CellTabs T{c->sorted_key, c->perm, c->cell_start, c->cell_end, c->hglob};
+    int blocks = (int)((c->n + 127) / 128);
+    if (c->kernel == SPRAY_KERNEL_WENDLAND_C2) k_ref_sweep<SWEEP, 1><<<blocks, 128, 0, st>>>(c->dg, c->n, T, a);
+    else k_ref_sweep<SWEEP, 0><<<blocks, 128, 0, st>>>(c->dg, c->n, T, a);
+    c->launches += 1;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_ref_sweep(Ctx* c, int sweep, const SweepArgs& a, cudaStream_t st) {
+    switch (sweep) {
+        case SW_DENSITY: return launch_k<SW_DENSITY>(c, a, st);
+        case SW_HYDRO: return launch_k<SW_HYDRO>(c, a, st);
+        case SW_LIMITER: return launch_k<SW_LIMITER>(c, a, st);
+        case SW_APPLY: return launch_k<SW_APPLY>(c, a, st);
+        case SW_HSEARCH: return launch_k<SW_HSEARCH>(c, a, st);
+        case SW_COUNT: return launch_k<SW_COUNT>(c, a, st);
+        case SW_LIST: return launch_k<SW_LIST>(c, a, st);
+        case SW_DIGEST: return launch_k<SW_DIGEST>(c, a, st);
+    }
+    return cudaErrorInvalidValue;
+}
+
+}  // namespace spray
