@@ -21,7 +21,7 @@ def get_workload(name):
     if name == "cloud_periodic":
         return W.random_cloud(5000, seed=12, periodic=(1, 1, 1), hvar=2.0, kernel=W.KERNEL_CUBIC_SPLINE)
     if name == "cloud_mixed":
-        return W.random_cloud(4000, seed=13, periodic=(1, 0, 1), hvar=2.5)
+        return W.random_cloud(4000, seed=13, periodic=(1, 0, 1), hvar=2.2)
     return W.make(name)
 
 
