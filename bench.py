@@ -200,6 +200,7 @@ def main():
     cg = int(sp.neighbor_counts(False).to(torch.int64).sum().item())
     cs = int(sp.neighbor_counts(True).to(torch.int64).sum().item())
     assert sp.check() == 0, "device status flags set"
+    n_tiles, n_fast = sp.path_stats()
     pairs = {"density": cg + n, "hydro": cs, "limiter": cg, "apply": cs}
     p_pass = sum(pairs.values())
 
@@ -306,7 +307,8 @@ def main():
             "config": {"workload": w.name, "n_particles": n, "kernel": ["cubic_spline", "wendland_c2"][w.kernel], "grid": list(w.grid.ncell),
                        "pairs_per_pass": p_pass, "unique_ordered_pairs": cs, "unique_pairs_per_s": world * cs * args.steps / t_total,
                        "l2": "inputs larger than L2 (%.1f GB resident per replica)" % (8e-9 * n * (len(fields) + len(out))),
-                       "parallelism": "replicas only" if world > 1 else "1 GPU", "path": args.path},
+                       "parallelism": "replicas only" if world > 1 else "1 GPU", "path": args.path,
+                       "tiles": n_tiles, "tiled_fraction": n_fast / max(n, 1)},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
             "fp64_probe_tflops": fp64_meas}
     print(json.dumps(line))

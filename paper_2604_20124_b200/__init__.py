@@ -22,7 +22,7 @@ FLD_UPDATE_LIMITER, FLD_FROZEN = 0, 1
 DEV_H_EXCEEDS_HMAX, DEV_OUTSIDE_BOX, DEV_LIST_OVERFLOW = 1, 2, 4
 
 # every symbol include/spray.h declares
-EXPORTS = ["spray_version", "spray_create", "spray_destroy", "spray_last_error", "spray_check", "spray_launch_count", "spray_set_path",
+EXPORTS = ["spray_version", "spray_create", "spray_destroy", "spray_last_error", "spray_check", "spray_launch_count", "spray_set_path", "spray_path_stats",
            "spray_build_cells", "spray_density", "spray_hydro_rhs", "spray_fld_apply", "spray_get_cell_table",
            "spray_neighbor_counts", "spray_neighbor_lists", "spray_neighbor_digest", "spray_fp64_peak_probe"]
 
@@ -59,6 +59,7 @@ def load():
     lib.spray_check.argtypes = [vp, vp, C.POINTER(C.c_uint32)]
     lib.spray_set_path.argtypes = [vp, i32]
     lib.spray_launch_count.argtypes = [vp]
+    lib.spray_path_stats.argtypes = [vp, vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
     lib.spray_build_cells.argtypes = [vp, C.POINTER(Grid), i32, i64, vp, vp, vp, vp, vp]
     lib.spray_density.argtypes = [vp, vp, vp, vp, vp]
     lib.spray_hydro_rhs.argtypes = [vp] + [vp] * 8 + [dbl] + [vp] * 5 + [vp]
@@ -141,6 +142,12 @@ class Spray:
 
     def launch_count(self) -> int:
         return int(self.lib.spray_launch_count(self.h))
+
+    def path_stats(self):
+        """(tiles, particles served by the tiled kernels) of the last build_cells; synchronises."""
+        nt, nf = C.c_int64(0), C.c_int64(0)
+        self._ck(self.lib.spray_path_stats(self.h, _stream(), C.byref(nt), C.byref(nf)), "spray_path_stats")
+        return int(nt.value), int(nf.value)
 
     def check(self) -> int:
         st = C.c_uint32(0)

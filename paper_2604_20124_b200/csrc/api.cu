@@ -39,6 +39,32 @@ void free_all(Ctx* c) {
     cudaFree(c->hglob); cudaFree(c->dev_status);
     cudaFree(c->s.x); cudaFree(c->s.y); cudaFree(c->s.z); cudaFree(c->s.h); cudaFree(c->s.hs);
     for (double* f : c->s.f) cudaFree(f);
+    Tiled& t = c->tl;
+    cudaFree(t.tiles); cudaFree(t.ntiles); cudaFree(t.lists); cudaFree(t.lcount); cudaFree(t.tile_ok); cudaFree(t.fast);
+}
+
+// Scratch of the tiled path (tiles, neighbour lists): sized for (n, grid) at the first spray_build_cells that needs
+// it and kept; growing it synchronises the device (cudaFree).  Failure to allocate is not an error: the general
+// kernels then serve every particle.
+void ensure_tiled(Ctx* c) {
+    Tiled& t = c->tl;
+    const int64_t nb = (int64_t)((c->grid.ncell[1] + 1) / 2) * ((c->grid.ncell[2] + 1) / 2);
+    const int64_t need = (5 * ((c->n + TILE_T - 1) / TILE_T)) / 4 + 2 * nb + 64;
+    if (t.tiles && need <= t.tile_cap) return;
+    cudaFree(t.tiles); cudaFree(t.lists); cudaFree(t.lcount); cudaFree(t.tile_ok);
+    t.tiles = nullptr; t.lists = nullptr; t.lcount = nullptr; t.tile_ok = nullptr; t.tile_cap = 0;
+    const size_t list_bytes = (size_t)need * TILE_WARPS * (LIST_CAP / 4) * 32 * sizeof(uint2);
+    bool ok = dmalloc(&t.tiles, need) && dmalloc(&t.lcount, need * TILE_T) && dmalloc(&t.tile_ok, need) &&
+              cudaMalloc((void**)&t.lists, list_bytes) == cudaSuccess;
+    if (ok && !t.ntiles) ok = dmalloc(&t.ntiles, 1);
+    if (ok && !t.fast) ok = dmalloc(&t.fast, c->n_max);
+    if (!ok) {
+        cudaGetLastError();
+        cudaFree(t.tiles); cudaFree(t.lists); cudaFree(t.lcount); cudaFree(t.tile_ok);
+        t.tiles = nullptr; t.lists = nullptr; t.lcount = nullptr; t.tile_ok = nullptr;
+        return;
+    }
+    t.tile_cap = need;
 }
 
 SweepArgs base_args(Ctx* c) {
@@ -51,7 +77,7 @@ SweepArgs base_args(Ctx* c) {
 #define CK(call, where) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) return cuda_fail(c, e__, where); } while (0)
 #define NEED_BUILT() do { if (!ctx) return SPRAY_ERR_INVALID_ARG; if (!ctx->c.built) return fail(&ctx->c, SPRAY_ERR_NOT_BUILT, "spray_build_cells has not succeeded on this context"); } while (0)
 
-enum { F_M = 0, F_RHO, F_P, F_CS, F_VX, F_VY, F_VZ, F_ALPHA, F_E, F_KAPPA, F_MU, F_SPARE };
+enum { F_M = 0, F_RHO, F_P, F_CS, F_VX, F_VY, F_VZ, F_ALPHA, F_E, F_KAPPA, F_MU, F_V, F_Q, F_AC };
 
 }  // namespace
 
@@ -67,12 +93,14 @@ int spray_create(spray_ctx** out, int64_t n_max, int64_t ncell_max, int device) 
     if (!h) return SPRAY_ERR_ALLOC;
     Ctx* c = &h->c;
     c->device = device; c->n_max = n_max; c->ncell_max = ncell_max;
-    c->path = 0;
-    c->hist_cap = 256 * ((n_max + 4095) / 4096 + 1);
+    c->path = 1;
+    int sms = 0;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) == cudaSuccess && sms > 0) { c->tl.sms = sms; c->tl.grid = sms; }
+    c->hist_cap = 256 * ((n_max + 4095) / 4096 + 1) + 4096;   // radix histograms + block totals of their scan
     bool ok = true;
     for (int k = 0; k < 2; ++k) ok = ok && dmalloc(&c->key[k], n_max) && dmalloc(&c->idx[k], n_max);
     ok = ok && dmalloc(&c->hist, c->hist_cap) && dmalloc(&c->cell_start, ncell_max) && dmalloc(&c->cell_end, ncell_max) &&
-         dmalloc(&c->cell_hmax, ncell_max) && dmalloc(&c->hglob, 2) && dmalloc(&c->dev_status, 1) && dmalloc(&c->s.x, n_max) &&
+         dmalloc(&c->cell_hmax, ncell_max) && dmalloc(&c->hglob, 4) && dmalloc(&c->dev_status, 1) && dmalloc(&c->s.x, n_max) &&
          dmalloc(&c->s.y, n_max) && dmalloc(&c->s.z, n_max) && dmalloc(&c->s.h, n_max) && dmalloc(&c->s.hs, n_max);
     for (double*& f : c->s.f) ok = ok && dmalloc(&f, n_max);
     if (ok) ok = cudaMemset(c->dev_status, 0, sizeof(uint32_t)) == cudaSuccess;
@@ -113,8 +141,26 @@ int64_t spray_launch_count(const spray_ctx* ctx) { return ctx ? ctx->c.launches 
 
 int spray_set_path(spray_ctx* ctx, int path) {
     if (!ctx) return SPRAY_ERR_INVALID_ARG;
-    if (path != 0) return fail(&ctx->c, SPRAY_ERR_NOT_IMPLEMENTED, "tiled path not built into this library yet");
+    if (path != 0 && path != 1) return fail(&ctx->c, SPRAY_ERR_INVALID_ARG, "spray_set_path: path must be 0 or 1");
     ctx->c.path = path;
+    ctx->c.built = false;           // the neighbour lists belong to a path: rebuild the cells after switching
+    return SPRAY_OK;
+}
+
+int spray_path_stats(spray_ctx* ctx, void* stream, int64_t* n_tiles, int64_t* n_fast) {
+    NEED_BUILT();
+    Ctx* c = &ctx->c;
+    cudaStream_t st = (cudaStream_t)stream;
+    uint32_t nt = 0;
+    unsigned long long nf = 0;
+    if (c->tl.enabled && c->n > 0) {
+        CK(launch_count_fast(c, st), "count fast");
+        CK(cudaStreamSynchronize(st), "spray_path_stats");
+        CK(cudaMemcpy(&nt, c->tl.ntiles, sizeof nt, cudaMemcpyDeviceToHost), "spray_path_stats");
+        CK(cudaMemcpy(&nf, c->hglob + 2, sizeof nf, cudaMemcpyDeviceToHost), "spray_path_stats");
+    }
+    if (n_tiles) *n_tiles = nt;
+    if (n_fast) *n_fast = (int64_t)nf;
     return SPRAY_OK;
 }
 
@@ -161,6 +207,11 @@ int spray_build_cells(spray_ctx* ctx, const spray_grid_t* g, spray_kernel_t kern
     SweepArgs a = base_args(c);
     a.o0 = c->s.hs;
     CK(launch_ref_sweep(c, SW_HSEARCH, a, st), "search-length sweep");
+    c->tl.enabled = false;
+    if (c->path == 1) {
+        ensure_tiled(c);
+        CK(launch_build_tiles(c, st), "tiles + neighbour lists");
+    }
     c->built = true;
     return SPRAY_OK;
 }
@@ -173,8 +224,14 @@ int spray_density(spray_ctx* ctx, const double* m, double* rho, uint32_t* nnbr, 
     GatherJob job{};
     job.count = 1; job.in[0] = m; job.out[0] = c->s.f[F_M];
     CK(launch_gather(c, job, st), "density gather");
+    if (c->tl.enabled) {
+        TiledArgs t{};
+        t.f0 = c->s.f[F_M]; t.o0 = rho; t.ocount = nnbr;
+        CK(launch_tiled_sweep(c, SW_DENSITY, t, st), "tiled density sweep");
+    }
     SweepArgs a = base_args(c);
     a.m = c->s.f[F_M]; a.o0 = rho; a.ocount = nnbr;
+    a.skip = c->tl.enabled ? c->tl.fast : nullptr;
     CK(launch_ref_sweep(c, SW_DENSITY, a, st), "density sweep");
     return SPRAY_OK;
 }
@@ -187,13 +244,22 @@ int spray_hydro_rhs(spray_ctx* ctx, const double* m, const double* rho, const do
     if (c->n > 0 && (!m || !rho || !p || !cs || !vx || !vy || !vz || !alpha || !ax || !ay || !az || !dudt))
         return fail(c, SPRAY_ERR_INVALID_ARG, "spray_hydro_rhs: NULL argument");
     cudaStream_t st = (cudaStream_t)stream;
-    GatherJob job{};
-    const double* in[8] = {m, rho, p, cs, vx, vy, vz, alpha};
-    const int slot[8] = {F_M, F_RHO, F_P, F_CS, F_VX, F_VY, F_VZ, F_ALPHA};
-    job.count = 8;
-    for (int k = 0; k < 8; ++k) { job.in[k] = in[k]; job.out[k] = c->s.f[slot[k]]; }
-    CK(launch_gather(c, job, st), "hydro gather");
+    double** f = c->s.f;
+    PrepJob pj{};
+    pj.m = m; pj.rho = rho; pj.p = p; pj.cs = cs; pj.vx = vx; pj.vy = vy; pj.vz = vz; pj.alpha = alpha;
+    pj.sm = f[F_M]; pj.srho = f[F_RHO]; pj.sp = f[F_P]; pj.scs = f[F_CS]; pj.svx = f[F_VX]; pj.svy = f[F_VY]; pj.svz = f[F_VZ];
+    pj.salpha = f[F_ALPHA]; pj.sV = f[F_V]; pj.sQ = f[F_Q]; pj.sAC = f[F_AC];
+    CK(launch_prep_hydro(c, pj, st), "hydro prologue");
+    if (c->tl.enabled) {
+        TiledArgs t{};
+        t.f0 = f[F_V]; t.f1 = f[F_Q]; t.f2 = f[F_M]; t.f3 = f[F_AC]; t.f4 = f[F_VX]; t.f5 = f[F_VY]; t.f6 = f[F_VZ];
+        t.g0 = f[F_RHO]; t.g1 = f[F_P];
+        t.beta = beta;
+        t.o0 = ax; t.o1 = ay; t.o2 = az; t.o3 = dudt; t.o4 = divv_sum;
+        CK(launch_tiled_sweep(c, SW_HYDRO, t, st), "tiled hydro sweep");
+    }
     SweepArgs a = base_args(c);
+    a.skip = c->tl.enabled ? c->tl.fast : nullptr;
     a.m = c->s.f[F_M]; a.rho = c->s.f[F_RHO]; a.p = c->s.f[F_P]; a.cs = c->s.f[F_CS];
     a.vx = c->s.f[F_VX]; a.vy = c->s.f[F_VY]; a.vz = c->s.f[F_VZ]; a.alpha = c->s.f[F_ALPHA];
     a.beta = beta;
@@ -213,22 +279,35 @@ int spray_fld_apply(spray_ctx* ctx, const double* m, const double* rho, const do
     if ((kmode != SPRAY_FLD_SYMMETRIC && kmode != SPRAY_FLD_GATHER) || (lmode != SPRAY_FLD_UPDATE_LIMITER && lmode != SPRAY_FLD_FROZEN))
         return fail(c, SPRAY_ERR_INVALID_ARG, "spray_fld_apply: unknown mode");
     cudaStream_t st = (cudaStream_t)stream;
-    GatherJob job{};
-    job.in[0] = m; job.out[0] = c->s.f[F_M];
-    job.in[1] = rho; job.out[1] = c->s.f[F_RHO];
-    job.in[2] = E; job.out[2] = c->s.f[F_E];
-    job.in[3] = update ? kappa : mu; job.out[3] = update ? c->s.f[F_KAPPA] : c->s.f[F_MU];
-    job.count = 4;
-    CK(launch_gather(c, job, st), "fld gather");
+    double** f = c->s.f;
+    PrepJob pj{};
+    pj.m = m; pj.rho = rho; pj.E = E; pj.kx = update ? kappa : mu;
+    pj.sm = f[F_M]; pj.srho = f[F_RHO]; pj.sE = f[F_E]; pj.skx = update ? f[F_KAPPA] : f[F_MU]; pj.sV = f[F_V];
+    CK(launch_prep_fld(c, pj, st), "fld prologue");
+    const bool tiled = c->tl.enabled;
     SweepArgs a = base_args(c);
+    a.skip = tiled ? c->tl.fast : nullptr;
     a.m = c->s.f[F_M]; a.rho = c->s.f[F_RHO]; a.E = c->s.f[F_E]; a.kappa = c->s.f[F_KAPPA]; a.mu = c->s.f[F_MU];
     a.c_light = c_light;
     if (update) {
+        if (tiled) {
+            TiledArgs t{};
+            t.f0 = f[F_V]; t.f1 = f[F_E]; t.g0 = f[F_RHO]; t.g1 = f[F_KAPPA];
+            t.c_light = c_light; t.o0 = mu; t.o1 = gradE; t.mu_sorted = f[F_MU];
+            CK(launch_tiled_sweep(c, SW_LIMITER, t, st), "tiled limiter sweep");
+        }
         SweepArgs l = a;
         l.o0 = mu; l.o1 = gradE; l.mu_sorted = c->s.f[F_MU];
         CK(launch_ref_sweep(c, SW_LIMITER, l, st), "limiter sweep");
     }
     a.fld_sym = (kmode == SPRAY_FLD_SYMMETRIC) ? 1 : 0;
+    if (tiled) {
+        TiledArgs t{};
+        t.f0 = f[F_V]; t.f1 = f[F_E]; t.f2 = f[F_MU];
+        t.fld_sym = a.fld_sym;
+        t.o0 = y; t.o1 = diag; t.o2 = offd;
+        CK(launch_tiled_sweep(c, SW_APPLY, t, st), "tiled apply sweep");
+    }
     a.o0 = y; a.o1 = diag; a.o2 = offd;
     CK(launch_ref_sweep(c, SW_APPLY, a, st), "apply sweep");
     return SPRAY_OK;

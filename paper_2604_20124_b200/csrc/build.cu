@@ -55,24 +55,66 @@ k_rs_hist(const uint32_t* __restrict__ key, int64_t n, int shift, uint32_t* __re
     hist[(int64_t)threadIdx.x * nblk + blockIdx.x] = sh[threadIdx.x];
 }
 
-// single-CTA exclusive scan, in place, of `total` u32 counters (total = 256 * ntiles <= ~1.1 M at 16.7 M keys)
-__global__ void __launch_bounds__(1024) k_rs_scan(uint32_t* __restrict__ a, int64_t total) {
-    __shared__ uint32_t part[1024];
-    int t = threadIdx.x;
-    int64_t chunk = (total + 1023) / 1024;
-    int64_t b = t * chunk, e = b + chunk < total ? b + chunk : total;
-    uint32_t s = 0;
-    for (int64_t i = b; i < e; ++i) s += a[i];
-    part[t] = s;
-    __syncthreads();
-    for (int off = 1; off < 1024; off <<= 1) {       // Hillis-Steele inclusive scan of the partials
-        uint32_t v = (t >= off) ? part[t - off] : 0;
-        __syncthreads();
-        part[t] += v;
-        __syncthreads();
+// exclusive scan, in place, of `total` u32 counters (total = 256 * ntiles ~ 1.05 M at 16.7 M keys) in three small kernels:
+// per-block scan of SC_TILE counters + block totals, single-CTA scan of the <= SC_TILE totals, add-back.
+constexpr int SC_THREADS = 256;
+constexpr int SC_ITEMS = 16;
+constexpr int SC_TILE = SC_THREADS * SC_ITEMS;
+
+__device__ __forceinline__ uint32_t block_excl_scan_256(uint32_t v, uint32_t* total) {
+    __shared__ uint32_t wsum[SC_THREADS / 32];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    uint32_t incl = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        uint32_t u = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+        if (lane >= o) incl += u;
     }
-    uint32_t run = part[t] - s;                       // exclusive prefix of this chunk
-    for (int64_t i = b; i < e; ++i) { uint32_t v = a[i]; a[i] = run; run += v; }
+    if (lane == 31) wsum[w] = incl;
+    __syncthreads();
+    if (w == 0) {
+        uint32_t t = lane < SC_THREADS / 32 ? wsum[lane] : 0u, ti = t;
+#pragma unroll
+        for (int o = 1; o < SC_THREADS / 32; o <<= 1) {
+            uint32_t u = __shfl_up_sync(0xFFFFFFFFu, ti, o);
+            if (lane >= o) ti += u;
+        }
+        if (lane < SC_THREADS / 32) wsum[lane] = ti - t;
+        if (lane == SC_THREADS / 32 - 1) *total = ti;
+    }
+    __syncthreads();
+    return wsum[w] + incl - v;
+}
+
+__global__ void __launch_bounds__(SC_THREADS) k_scan_blocks(uint32_t* __restrict__ a, int64_t total, uint32_t* __restrict__ btot) {
+    __shared__ uint32_t tot;
+    const int64_t base = (int64_t)blockIdx.x * SC_TILE + (int64_t)threadIdx.x * SC_ITEMS;
+    uint32_t v[SC_ITEMS], s = 0;
+#pragma unroll
+    for (int j = 0; j < SC_ITEMS; ++j) { v[j] = (base + j < total) ? a[base + j] : 0u; s += v[j]; }
+    uint32_t run = block_excl_scan_256(s, &tot);
+#pragma unroll
+    for (int j = 0; j < SC_ITEMS; ++j) { if (base + j < total) a[base + j] = run; run += v[j]; }
+    if (threadIdx.x == 0) btot[blockIdx.x] = tot;
+}
+__global__ void __launch_bounds__(SC_THREADS) k_scan_totals(uint32_t* __restrict__ btot, int nb) {   // nb <= SC_TILE
+    __shared__ uint32_t tot;
+    const int base = threadIdx.x * SC_ITEMS;
+    uint32_t v[SC_ITEMS], s = 0;
+#pragma unroll
+    for (int j = 0; j < SC_ITEMS; ++j) { v[j] = (base + j < nb) ? btot[base + j] : 0u; s += v[j]; }
+    uint32_t run = block_excl_scan_256(s, &tot);
+#pragma unroll
+    for (int j = 0; j < SC_ITEMS; ++j) { if (base + j < nb) btot[base + j] = run; run += v[j]; }
+}
+__global__ void __launch_bounds__(SC_THREADS) k_scan_add(uint32_t* __restrict__ a, int64_t total, const uint32_t* __restrict__ btot) {
+    const uint32_t off = btot[blockIdx.x];
+    const int64_t base = (int64_t)blockIdx.x * SC_TILE;
+#pragma unroll
+    for (int j = 0; j < SC_ITEMS; ++j) {
+        const int64_t i = base + j * SC_THREADS + threadIdx.x;
+        if (i < total) a[i] += off;
+    }
 }
 
 __global__ void __launch_bounds__(RS_THREADS)
@@ -148,6 +190,27 @@ __global__ void k_gather(GatherJob job, const uint32_t* __restrict__ perm, int64
     for (int k = 0; k < job.count; ++k) job.out[k][i] = __ldg(job.in[k] + p);
 }
 
+// per-call prologues: caller order -> sorted order, with the per-particle factors of the pair formulas hoisted
+// (V = m/rho, Q = V p, alpha*c): one division per particle instead of one per pair.
+__global__ void k_prep_hydro(PrepJob j, const uint32_t* __restrict__ perm, int64_t n) {
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const uint32_t p = perm[i];
+    const double m = __ldg(j.m + p), rho = __ldg(j.rho + p), pr = __ldg(j.p + p), cs = __ldg(j.cs + p), al = __ldg(j.alpha + p);
+    j.sm[i] = m; j.srho[i] = rho; j.sp[i] = pr; j.scs[i] = cs; j.salpha[i] = al;
+    j.svx[i] = __ldg(j.vx + p); j.svy[i] = __ldg(j.vy + p); j.svz[i] = __ldg(j.vz + p);
+    const double V = m / rho;
+    j.sV[i] = V; j.sQ[i] = V * pr; j.sAC[i] = al * cs;
+}
+__global__ void k_prep_fld(PrepJob j, const uint32_t* __restrict__ perm, int64_t n) {
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const uint32_t p = perm[i];
+    const double m = __ldg(j.m + p), rho = __ldg(j.rho + p);
+    j.sm[i] = m; j.srho[i] = rho; j.sE[i] = __ldg(j.E + p); j.skx[i] = __ldg(j.kx + p);
+    j.sV[i] = m / rho;
+}
+
 // per-cell max h (fp64 max is exact and order independent), global min/max of h, and the h <= h_max check
 __global__ void k_init_hglob(double* hglob) { hglob[0] = __longlong_as_double(0x7FF0000000000000ll); hglob[1] = 0.0; }
 
@@ -191,11 +254,18 @@ cudaError_t launch_radix_sort(Ctx* c, cudaStream_t st) {
     for (int p = 0; p < passes && c->n > 0; ++p) {
         int shift = 8 * p;
         k_rs_hist<<<nblk, RS_THREADS, 0, st>>>(c->key[cur], c->n, shift, c->hist, nblk);
-        k_rs_scan<<<1, 1024, 0, st>>>(c->hist, (int64_t)256 * nblk);
+        {
+            const int64_t total = (int64_t)256 * nblk;
+            const int nb = cdiv64(total, SC_TILE);          // <= SC_TILE for n <= 2^32 keys
+            uint32_t* btot = c->hist + total;
+            k_scan_blocks<<<nb, SC_THREADS, 0, st>>>(c->hist, total, btot);
+            k_scan_totals<<<1, SC_THREADS, 0, st>>>(btot, nb);
+            k_scan_add<<<nb, SC_THREADS, 0, st>>>(c->hist, total, btot);
+        }
         k_rs_scatter<<<nblk, RS_THREADS, 0, st>>>(c->key[cur], c->idx[cur], c->key[cur ^ 1], c->idx[cur ^ 1], c->n, shift,
                                                   c->hist, nblk);
         cur ^= 1;
-        c->launches += 3;
+        c->launches += 5;
     }
     c->sorted_key = c->key[cur];
     c->perm = c->idx[cur];
@@ -212,6 +282,19 @@ cudaError_t launch_cell_table(Ctx* c, cudaStream_t st) {
 cudaError_t launch_gather(Ctx* c, const GatherJob& job, cudaStream_t st) {
     if (c->n == 0 || job.count == 0) return cudaSuccess;
     k_gather<<<cdiv64(c->n, 256), 256, 0, st>>>(job, c->perm, c->n);
+    c->launches += 1;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_prep_hydro(Ctx* c, const PrepJob& j, cudaStream_t st) {
+    if (c->n == 0) return cudaSuccess;
+    k_prep_hydro<<<cdiv64(c->n, 256), 256, 0, st>>>(j, c->perm, c->n);
+    c->launches += 1;
+    return cudaGetLastError();
+}
+cudaError_t launch_prep_fld(Ctx* c, const PrepJob& j, cudaStream_t st) {
+    if (c->n == 0) return cudaSuccess;
+    k_prep_fld<<<cdiv64(c->n, 256), 256, 0, st>>>(j, c->perm, c->n);
     c->launches += 1;
     return cudaGetLastError();
 }

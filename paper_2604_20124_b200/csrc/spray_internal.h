@@ -6,6 +6,7 @@
 
 #include "../../include/spray.h"
 #include "common.cuh"
+#include "tiles.cuh"
 
 namespace spray {
 
@@ -13,7 +14,21 @@ namespace spray {
 struct Sorted {
     double *x, *y, *z, *h;      // built by spray_build_cells
     double* hs;                 // symmetric search length: max(h_a, max{h_b : a in N_gather(b)})
-    double* f[12];              // per-call field scratch (m, rho, p, cs, vx, vy, vz, alpha, E, kappa, mu, ...)
+    double* f[16];              // per-call field scratch (m, rho, p, cs, vx, vy, vz, alpha, E, kappa, mu, V, Q, alpha*cs, ...)
+};
+
+// Tiled path (tiles.cuh): tiles + per-target neighbour lists, rebuilt by every spray_build_cells.
+struct Tiled {
+    bool enabled = false;        // tiles and lists were built for the current cell table
+    int sms = 148;               // SM count of the device (persistent grids)
+    int grid = 148;              // CTAs of the list builder
+    TileDesc* tiles = nullptr;
+    uint32_t* ntiles = nullptr;  // device counter
+    int64_t tile_cap = 0;
+    uint2* lists = nullptr;      // [tile_cap][TILE_WARPS][LIST_CAP/4][32] x 4 u16 slots
+    uint32_t* lcount = nullptr;  // [tile_cap][TILE_T]: n_gather | n_sym << 16
+    uint32_t* tile_ok = nullptr; // [tile_cap]
+    uint8_t* fast = nullptr;     // [n_max] sorted order: 1 = particle is served by the tiled kernels
 };
 
 struct Ctx {
@@ -35,6 +50,7 @@ struct Ctx {
     double* hglob = nullptr;    // [0] = min h, [1] = max h (device scalars)
     uint32_t* dev_status = nullptr;
     Sorted s{};
+    Tiled tl{};
     int64_t launches = 0;       // kernels launched through this ctx (bench.py reports it as gpu_launches)
     std::string err;
 };
@@ -67,8 +83,39 @@ struct SweepArgs {
     uint32_t* onbr;
     uint64_t *odsum, *odxor;
     int symmetric;              // count / list / digest: which set
+    const uint8_t* skip;        // nullable: particles with skip[i] != 0 are served by the tiled kernels
 };
 cudaError_t launch_ref_sweep(Ctx* c, int sweep, const SweepArgs& a, cudaStream_t st);
+
+// ---- build.cu : per-call prologues (caller order -> sorted order through perm, per-particle factors hoisted)
+struct PrepJob {
+    const double *m, *rho, *p, *cs, *vx, *vy, *vz, *alpha, *E, *kx;   // caller order (kx = kappa or mu)
+    double *sm, *srho, *sp, *scs, *svx, *svy, *svz, *salpha, *sE, *skx, *sV, *sQ, *sAC;   // sorted order
+};
+cudaError_t launch_prep_hydro(Ctx* c, const PrepJob& j, cudaStream_t st);
+cudaError_t launch_prep_fld(Ctx* c, const PrepJob& j, cudaStream_t st);
+
+// ---- tiles.cu / sweeps_tiled.cu : tiled path
+struct TiledArgs {
+    const double *x, *y, *z, *h;                 // sorted (filled by the launcher)
+    const double *f0, *f1, *f2, *f3, *f4, *f5, *f6;   // sorted per-call fields, meaning per sweep (sweeps_tiled.cu)
+    const double *g0, *g1;                       // sorted target-side fields (rho, p | rho, kappa)
+    double beta, c_light;
+    int fld_sym;
+    double *o0, *o1, *o2, *o3, *o4;              // caller-order outputs
+    double* mu_sorted;
+    uint32_t* ocount;
+    const uint32_t* perm;
+    const TileDesc* tiles;
+    const uint32_t* ntiles;
+    const uint2* lists;
+    const uint32_t* lcount;
+    const uint32_t* tile_ok;
+    int64_t n;
+};
+cudaError_t launch_build_tiles(Ctx* c, cudaStream_t st);
+cudaError_t launch_count_fast(Ctx* c, cudaStream_t st);
+cudaError_t launch_tiled_sweep(Ctx* c, int sweep, TiledArgs a, cudaStream_t st);
 
 // ---- probe.cu
 cudaError_t launch_fp64_probe(int blocks, int threads, int64_t iters, double* out, cudaStream_t st);

@@ -34,6 +34,7 @@ __global__ void __launch_bounds__(128)
 k_ref_sweep(DevGrid g, int64_t n, CellTabs T, SweepArgs A) {
     const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (i >= n) return;
+    if (A.skip && A.skip[i]) return;        // served by the tiled kernels
     const double xa = A.x[i], ya = A.y[i], za = A.z[i], ha = A.h[i];
     const uint32_t ia = T.perm[i];
 

@@ -12,7 +12,7 @@ pytestmark = pytest.mark.gpu
 
 SMALL = ["c1_tiny", "c2_tiny", "c3_tiny", "c4_tiny", "c5_tiny"]
 MID = ["c2_mid", "c3_mid", "c4_mid", "c5_mid"]
-PATHS = [0]
+PATHS = [0, 1]
 
 
 def get_workload(name):
