@@ -39,38 +39,52 @@ void free_all(Ctx* c) {
     cudaFree(c->hglob); cudaFree(c->dev_status);
     cudaFree(c->s.x); cudaFree(c->s.y); cudaFree(c->s.z); cudaFree(c->s.h); cudaFree(c->s.hs);
     for (double* f : c->s.f) cudaFree(f);
+    Packed& k = c->pk;
+    cudaFree(k.p0); cudaFree(k.p1); cudaFree(k.hh); cudaFree(k.t0); cudaFree(k.me); cudaFree(k.e1);
+    for (double2* r : k.s) cudaFree(r);
     Tiled& t = c->tl;
-    cudaFree(t.tiles); cudaFree(t.ntiles); cudaFree(t.lists); cudaFree(t.lcount); cudaFree(t.tile_ok); cudaFree(t.fast);
+    cudaFree(t.tiles); cudaFree(t.bcount); cudaFree(t.pool); cudaFree(t.ctr); cudaFree(t.winfo); cudaFree(t.lcount);
+    cudaFree(t.tflags); cudaFree(t.fast);
 }
 
 // Scratch of the tiled path (tiles, neighbour lists): sized for (n, grid) at the first spray_build_cells that needs
 // it and kept; growing it synchronises the device (cudaFree).  Failure to allocate is not an error: the general
 // kernels then serve every particle.
+constexpr int64_t POOL_U2_PER_PARTICLE = 32;      // 128 scheduled u16 entries per particle on average
+
 void ensure_tiled(Ctx* c) {
     Tiled& t = c->tl;
     const int64_t nb = (int64_t)((c->grid.ncell[1] + 1) / 2) * ((c->grid.ncell[2] + 1) / 2);
     const int64_t need = (5 * ((c->n + TILE_T - 1) / TILE_T)) / 4 + 2 * nb + 64;
-    if (t.tiles && need <= t.tile_cap) return;
-    cudaFree(t.tiles); cudaFree(t.lists); cudaFree(t.lcount); cudaFree(t.tile_ok);
-    t.tiles = nullptr; t.lists = nullptr; t.lcount = nullptr; t.tile_ok = nullptr; t.tile_cap = 0;
-    const size_t list_bytes = (size_t)need * TILE_WARPS * (LIST_CAP / 4) * 32 * sizeof(uint2);
-    bool ok = dmalloc(&t.tiles, need) && dmalloc(&t.lcount, need * TILE_T) && dmalloc(&t.tile_ok, need) &&
-              cudaMalloc((void**)&t.lists, list_bytes) == cudaSuccess;
-    if (ok && !t.ntiles) ok = dmalloc(&t.ntiles, 1);
+    const int64_t pool_need = c->n * POOL_U2_PER_PARTICLE + 4096;
+    if (t.tiles && need <= t.tile_cap && nb <= t.bundle_cap && pool_need <= t.pool_cap) return;
+    cudaFree(t.tiles); cudaFree(t.bcount); cudaFree(t.pool); cudaFree(t.winfo); cudaFree(t.lcount); cudaFree(t.tflags);
+    t.tiles = nullptr; t.bcount = nullptr; t.pool = nullptr; t.winfo = nullptr; t.lcount = nullptr; t.tflags = nullptr;
+    t.tile_cap = 0; t.bundle_cap = 0; t.pool_cap = 0;
+    bool ok = dmalloc(&t.tiles, need) && dmalloc(&t.bcount, nb + 4096 + 64) && dmalloc(&t.winfo, need * TILE_WARPS) &&
+              dmalloc(&t.lcount, need * TILE_T) && dmalloc(&t.tflags, need) && dmalloc(&t.pool, pool_need);
+    if (ok && !t.ctr) ok = dmalloc(&t.ctr, CTR_COUNT);
     if (ok && !t.fast) ok = dmalloc(&t.fast, c->n_max);
     if (!ok) {
         cudaGetLastError();
-        cudaFree(t.tiles); cudaFree(t.lists); cudaFree(t.lcount); cudaFree(t.tile_ok);
-        t.tiles = nullptr; t.lists = nullptr; t.lcount = nullptr; t.tile_ok = nullptr;
+        cudaFree(t.tiles); cudaFree(t.bcount); cudaFree(t.pool); cudaFree(t.winfo); cudaFree(t.lcount); cudaFree(t.tflags);
+        t.tiles = nullptr; t.bcount = nullptr; t.pool = nullptr; t.winfo = nullptr; t.lcount = nullptr; t.tflags = nullptr;
         return;
     }
-    t.tile_cap = need;
+    t.tile_cap = need; t.bundle_cap = nb; t.pool_cap = pool_need;
 }
 
 SweepArgs base_args(Ctx* c) {
     SweepArgs a;
     memset(&a, 0, sizeof a);
     a.x = c->s.x; a.y = c->s.y; a.z = c->s.z; a.h = c->s.h; a.hs = c->s.hs;
+    return a;
+}
+
+// general-kernel arguments of a sweep that the tiled kernels ran first: skip what they served
+SweepArgs fallback_args(Ctx* c) {
+    SweepArgs a = base_args(c);
+    if (c->tl.enabled) { a.skip = c->tl.fast; a.nfast = c->tl.ctr + CTR_NFAST; }
     return a;
 }
 
@@ -95,7 +109,7 @@ int spray_create(spray_ctx** out, int64_t n_max, int64_t ncell_max, int device) 
     c->device = device; c->n_max = n_max; c->ncell_max = ncell_max;
     c->path = 1;
     int sms = 0;
-    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) == cudaSuccess && sms > 0) { c->tl.sms = sms; c->tl.grid = sms; }
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) == cudaSuccess && sms > 0) c->tl.sms = sms;
     c->hist_cap = 256 * ((n_max + 4095) / 4096 + 1) + 4096;   // radix histograms + block totals of their scan
     bool ok = true;
     for (int k = 0; k < 2; ++k) ok = ok && dmalloc(&c->key[k], n_max) && dmalloc(&c->idx[k], n_max);
@@ -103,6 +117,10 @@ int spray_create(spray_ctx** out, int64_t n_max, int64_t ncell_max, int device) 
          dmalloc(&c->cell_hmax, ncell_max) && dmalloc(&c->hglob, 4) && dmalloc(&c->dev_status, 1) && dmalloc(&c->s.x, n_max) &&
          dmalloc(&c->s.y, n_max) && dmalloc(&c->s.z, n_max) && dmalloc(&c->s.h, n_max) && dmalloc(&c->s.hs, n_max);
     for (double*& f : c->s.f) ok = ok && dmalloc(&f, n_max);
+    Packed& k = c->pk;
+    ok = ok && dmalloc(&k.p0, n_max) && dmalloc(&k.p1, n_max) && dmalloc(&k.hh, n_max) && dmalloc(&k.t0, n_max) &&
+         dmalloc(&k.me, n_max) && dmalloc(&k.e1, n_max);
+    for (double2*& r : k.s) ok = ok && dmalloc(&r, n_max);
     if (ok) ok = cudaMemset(c->dev_status, 0, sizeof(uint32_t)) == cudaSuccess;
     if (!ok) {
         cudaGetLastError();
@@ -151,16 +169,13 @@ int spray_path_stats(spray_ctx* ctx, void* stream, int64_t* n_tiles, int64_t* n_
     NEED_BUILT();
     Ctx* c = &ctx->c;
     cudaStream_t st = (cudaStream_t)stream;
-    uint32_t nt = 0;
-    unsigned long long nf = 0;
+    unsigned long long v[CTR_COUNT] = {0, 0, 0, 0};
     if (c->tl.enabled && c->n > 0) {
-        CK(launch_count_fast(c, st), "count fast");
         CK(cudaStreamSynchronize(st), "spray_path_stats");
-        CK(cudaMemcpy(&nt, c->tl.ntiles, sizeof nt, cudaMemcpyDeviceToHost), "spray_path_stats");
-        CK(cudaMemcpy(&nf, c->hglob + 2, sizeof nf, cudaMemcpyDeviceToHost), "spray_path_stats");
+        CK(cudaMemcpy(v, c->tl.ctr, sizeof v, cudaMemcpyDeviceToHost), "spray_path_stats");
     }
-    if (n_tiles) *n_tiles = nt;
-    if (n_fast) *n_fast = (int64_t)nf;
+    if (n_tiles) *n_tiles = (int64_t)v[CTR_NTILES];
+    if (n_fast) *n_fast = (int64_t)v[CTR_NFAST];
     return SPRAY_OK;
 }
 
@@ -196,18 +211,14 @@ int spray_build_cells(spray_ctx* ctx, const spray_grid_t* g, spray_kernel_t kern
     CK(launch_cell_keys(c, x, y, z, st), "cell keys");
     CK(launch_radix_sort(c, st), "radix sort");
     CK(launch_cell_table(c, st), "cell table");
-    GatherJob job{};
-    job.count = 4;
-    job.in[0] = x; job.in[1] = y; job.in[2] = z; job.in[3] = h;
-    job.out[0] = c->s.x; job.out[1] = c->s.y; job.out[2] = c->s.z; job.out[3] = c->s.h;
-    CK(launch_gather(c, job, st), "reorder");
+    c->tl.enabled = false;
+    CK(launch_reorder_build(c, x, y, z, h, st), "reorder");
     CK(launch_cell_hmax(c, st), "cell hmax");
     // symmetric search length: hs = h, then raised by every particle that sees me with a larger h
     if (n > 0) CK(cudaMemcpyAsync(c->s.hs, c->s.h, sizeof(double) * (size_t)n, cudaMemcpyDeviceToDevice, st), "hs init");
     SweepArgs a = base_args(c);
     a.o0 = c->s.hs;
     CK(launch_ref_sweep(c, SW_HSEARCH, a, st), "search-length sweep");
-    c->tl.enabled = false;
     if (c->path == 1) {
         ensure_tiled(c);
         CK(launch_build_tiles(c, st), "tiles + neighbour lists");
@@ -221,17 +232,14 @@ int spray_density(spray_ctx* ctx, const double* m, double* rho, uint32_t* nnbr, 
     Ctx* c = &ctx->c;
     if (c->n > 0 && (!m || !rho)) return fail(c, SPRAY_ERR_INVALID_ARG, "spray_density: NULL argument");
     cudaStream_t st = (cudaStream_t)stream;
-    GatherJob job{};
-    job.count = 1; job.in[0] = m; job.out[0] = c->s.f[F_M];
-    CK(launch_gather(c, job, st), "density gather");
+    CK(launch_prep_density(c, m, st), "density prologue");
     if (c->tl.enabled) {
         TiledArgs t{};
-        t.f0 = c->s.f[F_M]; t.o0 = rho; t.ocount = nnbr;
+        t.o0 = rho; t.ocount = nnbr;
         CK(launch_tiled_sweep(c, SW_DENSITY, t, st), "tiled density sweep");
     }
-    SweepArgs a = base_args(c);
+    SweepArgs a = fallback_args(c);
     a.m = c->s.f[F_M]; a.o0 = rho; a.ocount = nnbr;
-    a.skip = c->tl.enabled ? c->tl.fast : nullptr;
     CK(launch_ref_sweep(c, SW_DENSITY, a, st), "density sweep");
     return SPRAY_OK;
 }
@@ -252,16 +260,13 @@ int spray_hydro_rhs(spray_ctx* ctx, const double* m, const double* rho, const do
     CK(launch_prep_hydro(c, pj, st), "hydro prologue");
     if (c->tl.enabled) {
         TiledArgs t{};
-        t.f0 = f[F_V]; t.f1 = f[F_Q]; t.f2 = f[F_M]; t.f3 = f[F_AC]; t.f4 = f[F_VX]; t.f5 = f[F_VY]; t.f6 = f[F_VZ];
-        t.g0 = f[F_RHO]; t.g1 = f[F_P];
         t.beta = beta;
         t.o0 = ax; t.o1 = ay; t.o2 = az; t.o3 = dudt; t.o4 = divv_sum;
         CK(launch_tiled_sweep(c, SW_HYDRO, t, st), "tiled hydro sweep");
     }
-    SweepArgs a = base_args(c);
-    a.skip = c->tl.enabled ? c->tl.fast : nullptr;
-    a.m = c->s.f[F_M]; a.rho = c->s.f[F_RHO]; a.p = c->s.f[F_P]; a.cs = c->s.f[F_CS];
-    a.vx = c->s.f[F_VX]; a.vy = c->s.f[F_VY]; a.vz = c->s.f[F_VZ]; a.alpha = c->s.f[F_ALPHA];
+    SweepArgs a = fallback_args(c);
+    a.m = f[F_M]; a.rho = f[F_RHO]; a.p = f[F_P]; a.cs = f[F_CS];
+    a.vx = f[F_VX]; a.vy = f[F_VY]; a.vz = f[F_VZ]; a.alpha = f[F_ALPHA];
     a.beta = beta;
     a.o0 = ax; a.o1 = ay; a.o2 = az; a.o3 = dudt; a.o4 = divv_sum;
     CK(launch_ref_sweep(c, SW_HYDRO, a, st), "hydro sweep");
@@ -281,29 +286,26 @@ int spray_fld_apply(spray_ctx* ctx, const double* m, const double* rho, const do
     cudaStream_t st = (cudaStream_t)stream;
     double** f = c->s.f;
     PrepJob pj{};
-    pj.m = m; pj.rho = rho; pj.E = E; pj.kx = update ? kappa : mu;
+    pj.m = m; pj.rho = rho; pj.E = E; pj.kx = update ? kappa : mu; pj.kx_is_mu = update ? 0 : 1;
     pj.sm = f[F_M]; pj.srho = f[F_RHO]; pj.sE = f[F_E]; pj.skx = update ? f[F_KAPPA] : f[F_MU]; pj.sV = f[F_V];
     CK(launch_prep_fld(c, pj, st), "fld prologue");
     const bool tiled = c->tl.enabled;
-    SweepArgs a = base_args(c);
-    a.skip = tiled ? c->tl.fast : nullptr;
-    a.m = c->s.f[F_M]; a.rho = c->s.f[F_RHO]; a.E = c->s.f[F_E]; a.kappa = c->s.f[F_KAPPA]; a.mu = c->s.f[F_MU];
+    SweepArgs a = fallback_args(c);
+    a.m = f[F_M]; a.rho = f[F_RHO]; a.E = f[F_E]; a.kappa = f[F_KAPPA]; a.mu = f[F_MU];
     a.c_light = c_light;
     if (update) {
         if (tiled) {
             TiledArgs t{};
-            t.f0 = f[F_V]; t.f1 = f[F_E]; t.g0 = f[F_RHO]; t.g1 = f[F_KAPPA];
-            t.c_light = c_light; t.o0 = mu; t.o1 = gradE; t.mu_sorted = f[F_MU];
+            t.c_light = c_light; t.o0 = mu; t.o1 = gradE;
             CK(launch_tiled_sweep(c, SW_LIMITER, t, st), "tiled limiter sweep");
         }
         SweepArgs l = a;
-        l.o0 = mu; l.o1 = gradE; l.mu_sorted = c->s.f[F_MU];
+        l.o0 = mu; l.o1 = gradE; l.mu_sorted = f[F_MU]; l.me_sorted = c->pk.me;
         CK(launch_ref_sweep(c, SW_LIMITER, l, st), "limiter sweep");
     }
     a.fld_sym = (kmode == SPRAY_FLD_SYMMETRIC) ? 1 : 0;
     if (tiled) {
         TiledArgs t{};
-        t.f0 = f[F_V]; t.f1 = f[F_E]; t.f2 = f[F_MU];
         t.fld_sym = a.fld_sym;
         t.o0 = y; t.o1 = diag; t.o2 = offd;
         CK(launch_tiled_sweep(c, SW_APPLY, t, st), "tiled apply sweep");

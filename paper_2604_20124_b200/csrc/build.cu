@@ -181,8 +181,27 @@ __global__ void k_cell_table(const uint32_t* __restrict__ sorted_key, uint32_t n
     if (c > 0) cell_end[c - 1] = lb;
 }
 
-// ------------------------------------------------------------------------------------------- K4: SoA reorder
-__global__ void k_gather(GatherJob job, const uint32_t* __restrict__ perm, int64_t n) {
+// ------------------------------------------------------------------------------------------- K4: reorder by cell
+// Sorted copies of (x, y, z, h): structure-of-arrays for the general kernels and 16-byte records (x,y), (z,h),
+// (1/h, FN_K/h^4) for the tiled kernels.  64 B written per particle and layout.
+__global__ void k_reorder_build(const uint32_t* __restrict__ perm, int64_t n, const double* __restrict__ x,
+                                const double* __restrict__ y, const double* __restrict__ z, const double* __restrict__ h,
+                                double* __restrict__ sx, double* __restrict__ sy, double* __restrict__ sz, double* __restrict__ sh,
+                                double2* __restrict__ p0, double2* __restrict__ p1, double2* __restrict__ hh, double fnk) {
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const uint32_t p = perm[i];
+    const double xv = __ldg(x + p), yv = __ldg(y + p), zv = __ldg(z + p), hv = __ldg(h + p);
+    sx[i] = xv; sy[i] = yv; sz[i] = zv; sh[i] = hv;
+    p0[i] = make_double2(xv, yv);
+    p1[i] = make_double2(zv, hv);
+    const double hinv = 1.0 / hv, h2 = hinv * hinv;
+    hh[i] = make_double2(hinv, fnk * (h2 * h2));
+}
+
+// out[k][i] = in[k][perm[i]]; with only_if_slow the kernel does nothing when the tiled kernels serve every particle
+__global__ void k_gather(GatherJob job, const uint32_t* __restrict__ perm, int64_t n, const unsigned long long* __restrict__ nfast) {
+    if (nfast && *nfast == (unsigned long long)n) return;
     int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (i >= n) return;
     uint32_t p = perm[i];
@@ -191,24 +210,54 @@ __global__ void k_gather(GatherJob job, const uint32_t* __restrict__ perm, int64
 }
 
 // per-call prologues: caller order -> sorted order, with the per-particle factors of the pair formulas hoisted
-// (V = m/rho, Q = V p, alpha*c): one division per particle instead of one per pair.
-__global__ void k_prep_hydro(PrepJob j, const uint32_t* __restrict__ perm, int64_t n) {
+// (V = m/rho, Q = V p, alpha*c, p/rho, 1/rho): one division per particle instead of one per pair.  The packed
+// records feed the tiled kernels; the structure-of-arrays copies feed the general kernels and are written only
+// when some particle is left to them (*nfast != n).
+struct PackedOut { double2 *s0, *s1, *s2, *s3, *t0, *me; double* e1; const double2* p1; };
+
+__global__ void k_prep_density(const double* __restrict__ m, const uint32_t* __restrict__ perm, int64_t n, PackedOut o,
+                               double* __restrict__ sm, const unsigned long long* __restrict__ nfast) {
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double mv = __ldg(m + perm[i]);
+    o.s0[i] = make_double2(o.p1[i].x, mv);
+    if (!nfast || *nfast != (unsigned long long)n) sm[i] = mv;
+}
+__global__ void k_prep_hydro(PrepJob j, const uint32_t* __restrict__ perm, int64_t n, PackedOut o,
+                             const unsigned long long* __restrict__ nfast) {
     int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (i >= n) return;
     const uint32_t p = perm[i];
     const double m = __ldg(j.m + p), rho = __ldg(j.rho + p), pr = __ldg(j.p + p), cs = __ldg(j.cs + p), al = __ldg(j.alpha + p);
-    j.sm[i] = m; j.srho[i] = rho; j.sp[i] = pr; j.scs[i] = cs; j.salpha[i] = al;
-    j.svx[i] = __ldg(j.vx + p); j.svy[i] = __ldg(j.vy + p); j.svz[i] = __ldg(j.vz + p);
+    const double vx = __ldg(j.vx + p), vy = __ldg(j.vy + p), vz = __ldg(j.vz + p);
+    const double ia = 1.0 / rho;
     const double V = m / rho;
-    j.sV[i] = V; j.sQ[i] = V * pr; j.sAC[i] = al * cs;
+    o.s0[i] = make_double2(o.p1[i].x, V);
+    o.s1[i] = make_double2(V * pr, vx);
+    o.s2[i] = make_double2(vy, vz);
+    o.s3[i] = make_double2(m, al * cs);
+    o.t0[i] = make_double2(pr * ia, ia);
+    if (!nfast || *nfast != (unsigned long long)n) {
+        j.sm[i] = m; j.srho[i] = rho; j.sp[i] = pr; j.scs[i] = cs; j.salpha[i] = al;
+        j.svx[i] = vx; j.svy[i] = vy; j.svz[i] = vz;
+        j.sV[i] = V; j.sQ[i] = V * pr; j.sAC[i] = al * cs;
+    }
 }
-__global__ void k_prep_fld(PrepJob j, const uint32_t* __restrict__ perm, int64_t n) {
+__global__ void k_prep_fld(PrepJob j, const uint32_t* __restrict__ perm, int64_t n, PackedOut o,
+                           const unsigned long long* __restrict__ nfast) {
     int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (i >= n) return;
     const uint32_t p = perm[i];
-    const double m = __ldg(j.m + p), rho = __ldg(j.rho + p);
-    j.sm[i] = m; j.srho[i] = rho; j.sE[i] = __ldg(j.E + p); j.skx[i] = __ldg(j.kx + p);
-    j.sV[i] = m / rho;
+    const double m = __ldg(j.m + p), rho = __ldg(j.rho + p), E = __ldg(j.E + p), kx = __ldg(j.kx + p);
+    const double V = m / rho;
+    o.s0[i] = make_double2(o.p1[i].x, V);
+    o.e1[i] = E;
+    if (j.kx_is_mu) o.me[i] = make_double2(kx, E);
+    else o.t0[i] = make_double2(rho * kx, 0.0);
+    if (!nfast || *nfast != (unsigned long long)n) {
+        j.sm[i] = m; j.srho[i] = rho; j.sE[i] = E; j.skx[i] = kx;
+        j.sV[i] = V;
+    }
 }
 
 // per-cell max h (fp64 max is exact and order independent), global min/max of h, and the h <= h_max check
@@ -279,23 +328,53 @@ cudaError_t launch_cell_table(Ctx* c, cudaStream_t st) {
     return cudaGetLastError();
 }
 
-cudaError_t launch_gather(Ctx* c, const GatherJob& job, cudaStream_t st) {
-    if (c->n == 0 || job.count == 0) return cudaSuccess;
-    k_gather<<<cdiv64(c->n, 256), 256, 0, st>>>(job, c->perm, c->n);
+cudaError_t launch_reorder_build(Ctx* c, const double* x, const double* y, const double* z, const double* h, cudaStream_t st) {
+    if (c->n == 0) return cudaSuccess;
+    k_reorder_build<<<cdiv64(c->n, 256), 256, 0, st>>>(c->perm, c->n, x, y, z, h, c->s.x, c->s.y, c->s.z, c->s.h, c->pk.p0, c->pk.p1,
+                                                       c->pk.hh, c->kernel == SPRAY_KERNEL_WENDLAND_C2 ? kFnWend : kFnCubic);
     c->launches += 1;
     return cudaGetLastError();
 }
 
+static const unsigned long long* nfast_ptr(Ctx* c) { return c->tl.enabled ? c->tl.ctr + CTR_NFAST : nullptr; }
+static PackedOut packed_out(Ctx* c) {
+    PackedOut o{c->pk.s[0], c->pk.s[1], c->pk.s[2], c->pk.s[3], c->pk.t0, c->pk.me, c->pk.e1, c->pk.p1};
+    return o;
+}
+
+cudaError_t launch_gather(Ctx* c, const GatherJob& job, bool only_if_slow, cudaStream_t st) {
+    if (c->n == 0 || job.count == 0) return cudaSuccess;
+    k_gather<<<cdiv64(c->n, 256), 256, 0, st>>>(job, c->perm, c->n, only_if_slow ? nfast_ptr(c) : nullptr);
+    c->launches += 1;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_prep_density(Ctx* c, const double* m, cudaStream_t st) {
+    if (c->n == 0) return cudaSuccess;
+    k_prep_density<<<cdiv64(c->n, 256), 256, 0, st>>>(m, c->perm, c->n, packed_out(c), c->s.f[0], nfast_ptr(c));
+    c->launches += 1;
+    return cudaGetLastError();
+}
 cudaError_t launch_prep_hydro(Ctx* c, const PrepJob& j, cudaStream_t st) {
     if (c->n == 0) return cudaSuccess;
-    k_prep_hydro<<<cdiv64(c->n, 256), 256, 0, st>>>(j, c->perm, c->n);
+    k_prep_hydro<<<cdiv64(c->n, 256), 256, 0, st>>>(j, c->perm, c->n, packed_out(c), nfast_ptr(c));
     c->launches += 1;
     return cudaGetLastError();
 }
 cudaError_t launch_prep_fld(Ctx* c, const PrepJob& j, cudaStream_t st) {
     if (c->n == 0) return cudaSuccess;
-    k_prep_fld<<<cdiv64(c->n, 256), 256, 0, st>>>(j, c->perm, c->n);
+    k_prep_fld<<<cdiv64(c->n, 256), 256, 0, st>>>(j, c->perm, c->n, packed_out(c), nfast_ptr(c));
     c->launches += 1;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_excl_scan_u32(Ctx* c, uint32_t* a, int64_t total, uint32_t* scratch, cudaStream_t st) {
+    if (total <= 0) return cudaSuccess;
+    const int nb = cdiv64(total, SC_TILE);            // <= SC_TILE
+    k_scan_blocks<<<nb, SC_THREADS, 0, st>>>(a, total, scratch);
+    k_scan_totals<<<1, SC_THREADS, 0, st>>>(scratch, nb);
+    k_scan_add<<<nb, SC_THREADS, 0, st>>>(a, total, scratch);
+    c->launches += 3;
     return cudaGetLastError();
 }
 

@@ -21,6 +21,14 @@ constexpr double kPi = 3.14159265358979323846264338327950288;
 constexpr double kSigmaCubic = 1.0 / kPi;            // M4 cubic spline, 3-D (A1)
 constexpr double kSigmaWend = 21.0 / (16.0 * kPi);   // Wendland C2, 3-D, eq. (3)
 
+// The tiled kernels evaluate the kernels through rescaled shape functions (sweeps_tiled.cu):
+//   cubic:    W = kWnCubic / h^3 * (t2^3 - t1^3),  t2 = 2 - q, t1 = cbrt(4) (1 - q)_+ ;  F = kFnCubic / h^4 * (s1^2 - t2^2), s1 = (2 - 2q)_+
+//   Wendland: W = kWnWend / h^3 * t^4 (2q + 1),    t = (1 - q/2)_+ ;                     F = kFnWend / h^4 * q t^3
+constexpr double kWnCubic = 0.25 * kSigmaCubic;
+constexpr double kFnCubic = 0.75 * kSigmaCubic;
+constexpr double kWnWend = kSigmaWend;
+constexpr double kFnWend = -5.0 * kSigmaWend;
+
 __device__ __forceinline__ double dmax0(double a) { return a > 0.0 ? a : 0.0; }
 
 // ---- kernel shape functions of q = r/h, clamped so that they vanish identically for q >= 2 ("0 for q >= 2").

@@ -10,33 +10,50 @@
 
 namespace spray {
 
-// Particle store in SORTED order (structure-of-arrays; BASELINE.json "reordered by cell after the sort").
+// Particle store in SORTED order, structure-of-arrays (BASELINE.json "reordered by cell after the sort"): used by
+// the general one-thread-per-particle kernels (parity exports, search-length pre-pass, fallback of the tiled path).
 struct Sorted {
     double *x, *y, *z, *h;      // built by spray_build_cells
     double* hs;                 // symmetric search length: max(h_a, max{h_b : a in N_gather(b)})
     double* f[16];              // per-call field scratch (m, rho, p, cs, vx, vy, vz, alpha, E, kappa, mu, V, Q, alpha*cs, ...)
 };
 
-// Tiled path (tiles.cuh): tiles + per-target neighbour lists, rebuilt by every spray_build_cells.
+// Particle store in SORTED order as 16-byte records (two fp64 fields per record): what the tiled kernels stage into
+// shared memory and gather with one 128-bit load per record.
+struct Packed {
+    double2* p0;                // (x, y)                       built by spray_build_cells
+    double2* p1;                // (z, h)                       built by spray_build_cells
+    double2* hh;                // (1/h, FN_K / h^4)            built by spray_build_cells (FN_K: sweeps_tiled.cu)
+    double2* s[4];              // per-call source-side records (meaning per sweep, sweeps_tiled.cu)
+    double2* t0;                // per-call target-side record
+    double2* me;                // (mu, E) of the FLD apply
+    double* e1;                 // E of the limiter pre-sweep
+};
+
+// Tiled path (tiles.cuh): tiles + scheduled per-thread neighbour lists, rebuilt by every spray_build_cells.
 struct Tiled {
     bool enabled = false;        // tiles and lists were built for the current cell table
     int sms = 148;               // SM count of the device (persistent grids)
-    int grid = 148;              // CTAs of the list builder
     TileDesc* tiles = nullptr;
-    uint32_t* ntiles = nullptr;  // device counter
     int64_t tile_cap = 0;
-    uint2* lists = nullptr;      // [tile_cap][TILE_WARPS][LIST_CAP/4][32] x 4 u16 slots
+    uint32_t* bcount = nullptr;  // [bundle_cap + 1 + scan scratch] tiles per bundle -> exclusive scan
+    int64_t bundle_cap = 0;
+    uint2* pool = nullptr;       // list storage: per warp a block of rounds/4 x 32 lanes x (4 u16 slots)
+    int64_t pool_cap = 0;        // in uint2 units
+    unsigned long long* ctr = nullptr;   // [0] pool cursor, [1] particles served by the tiled kernels, [2] tiles, [3] work counter
+    uint2* winfo = nullptr;      // [tile_cap][TILE_WARPS]: (pool offset, rounds)
     uint32_t* lcount = nullptr;  // [tile_cap][TILE_T]: n_gather | n_sym << 16
-    uint32_t* tile_ok = nullptr; // [tile_cap]
+    uint32_t* tflags = nullptr;  // [tile_cap]: TILE_FLAG_*
     uint8_t* fast = nullptr;     // [n_max] sorted order: 1 = particle is served by the tiled kernels
 };
+enum { CTR_POOL = 0, CTR_NFAST = 1, CTR_NTILES = 2, CTR_WORK = 3, CTR_COUNT = 4 };
 
 struct Ctx {
     int device = 0;
     int64_t n_max = 0, ncell_max = 0;
     int64_t n = 0, ncell = 0;
     bool built = false;
-    int path = 0;               // 0 = reference kernels, 1 = tiled kernels
+    int path = 0;               // 0 = general kernels only, 1 = tiled kernels (+ general kernels for what they decline)
     int kernel = 0;
     spray_grid_t grid{};
     DevGrid dg{};
@@ -50,6 +67,7 @@ struct Ctx {
     double* hglob = nullptr;    // [0] = min h, [1] = max h (device scalars)
     uint32_t* dev_status = nullptr;
     Sorted s{};
+    Packed pk{};
     Tiled tl{};
     int64_t launches = 0;       // kernels launched through this ctx (bench.py reports it as gpu_launches)
     std::string err;
@@ -65,10 +83,12 @@ struct GatherJob {              // out[k][i] = in[k][perm[i]] for k < count
 cudaError_t launch_cell_keys(Ctx* c, const double* x, const double* y, const double* z, cudaStream_t st);
 cudaError_t launch_radix_sort(Ctx* c, cudaStream_t st);      // sets c->sorted_key / c->perm
 cudaError_t launch_cell_table(Ctx* c, cudaStream_t st);
-cudaError_t launch_gather(Ctx* c, const GatherJob& job, cudaStream_t st);
+cudaError_t launch_reorder_build(Ctx* c, const double* x, const double* y, const double* z, const double* h, cudaStream_t st);
+cudaError_t launch_gather(Ctx* c, const GatherJob& job, bool only_if_slow, cudaStream_t st);
 cudaError_t launch_cell_hmax(Ctx* c, cudaStream_t st);
+cudaError_t launch_excl_scan_u32(Ctx* c, uint32_t* a, int64_t total, uint32_t* scratch, cudaStream_t st);
 
-// ---- sweeps_ref.cu : reference pair kernels (one thread per particle)
+// ---- sweeps_ref.cu : general pair kernels (one thread per particle)
 struct SweepArgs {
     // sorted inputs
     const double *x, *y, *z, *h, *hs;
@@ -78,44 +98,36 @@ struct SweepArgs {
     // caller-order outputs (written through perm)
     double *o0, *o1, *o2, *o3, *o4, *o5;
     double* mu_sorted;          // limiter: also keeps mu in sorted order for the apply that follows
+    double2* me_sorted;         // limiter: (mu, E) record of the tiled apply
     uint32_t* ocount;
     const uint64_t* offsets;
     uint32_t* onbr;
     uint64_t *odsum, *odxor;
     int symmetric;              // count / list / digest: which set
     const uint8_t* skip;        // nullable: particles with skip[i] != 0 are served by the tiled kernels
+    const unsigned long long* nfast;   // nullable: device count of such particles (== n: nothing to do)
 };
 cudaError_t launch_ref_sweep(Ctx* c, int sweep, const SweepArgs& a, cudaStream_t st);
 
 // ---- build.cu : per-call prologues (caller order -> sorted order through perm, per-particle factors hoisted)
 struct PrepJob {
     const double *m, *rho, *p, *cs, *vx, *vy, *vz, *alpha, *E, *kx;   // caller order (kx = kappa or mu)
-    double *sm, *srho, *sp, *scs, *svx, *svy, *svz, *salpha, *sE, *skx, *sV, *sQ, *sAC;   // sorted order
+    double *sm, *srho, *sp, *scs, *svx, *svy, *svz, *salpha, *sE, *skx, *sV, *sQ, *sAC;   // sorted order (general kernels)
+    int kx_is_mu;
 };
+cudaError_t launch_prep_density(Ctx* c, const double* m, cudaStream_t st);
 cudaError_t launch_prep_hydro(Ctx* c, const PrepJob& j, cudaStream_t st);
 cudaError_t launch_prep_fld(Ctx* c, const PrepJob& j, cudaStream_t st);
 
 // ---- tiles.cu / sweeps_tiled.cu : tiled path
 struct TiledArgs {
-    const double *x, *y, *z, *h;                 // sorted (filled by the launcher)
-    const double *f0, *f1, *f2, *f3, *f4, *f5, *f6;   // sorted per-call fields, meaning per sweep (sweeps_tiled.cu)
-    const double *g0, *g1;                       // sorted target-side fields (rho, p | rho, kappa)
     double beta, c_light;
     int fld_sym;
     double *o0, *o1, *o2, *o3, *o4;              // caller-order outputs
-    double* mu_sorted;
     uint32_t* ocount;
-    const uint32_t* perm;
-    const TileDesc* tiles;
-    const uint32_t* ntiles;
-    const uint2* lists;
-    const uint32_t* lcount;
-    const uint32_t* tile_ok;
-    int64_t n;
 };
 cudaError_t launch_build_tiles(Ctx* c, cudaStream_t st);
-cudaError_t launch_count_fast(Ctx* c, cudaStream_t st);
-cudaError_t launch_tiled_sweep(Ctx* c, int sweep, TiledArgs a, cudaStream_t st);
+cudaError_t launch_tiled_sweep(Ctx* c, int sweep, const TiledArgs& a, cudaStream_t st);
 
 // ---- probe.cu
 cudaError_t launch_fp64_probe(int blocks, int threads, int64_t iters, double* out, cudaStream_t st);

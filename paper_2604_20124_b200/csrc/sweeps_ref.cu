@@ -32,6 +32,7 @@ __device__ __forceinline__ int wrap_cell(int c, int nc) { return c < 0 ? c + nc 
 template <int SWEEP, int KERNEL>
 __global__ void __launch_bounds__(128)
 k_ref_sweep(DevGrid g, int64_t n, CellTabs T, SweepArgs A) {
+    if (A.nfast && *A.nfast == (unsigned long long)n) return;   // the tiled kernels serve every particle
     const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (i >= n) return;
     if (A.skip && A.skip[i]) return;        // served by the tiled kernels
@@ -181,6 +182,7 @@ k_ref_sweep(DevGrid g, int64_t n, CellTabs T, SweepArgs A) {
         const double mu = A.c_light * (1.0 / sqrt(9.0 + R * R)) / rk;
         A.o0[ia] = mu;
         A.mu_sorted[i] = mu;
+        if (A.me_sorted) A.me_sorted[i] = make_double2(mu, E_a);
         if (A.o1) { A.o1[ia] = acc0; A.o1[n + ia] = acc1; A.o1[2 * n + ia] = acc2; }
     } else if (SWEEP == SW_APPLY) {
         A.o0[ia] = acc0;

@@ -1,217 +1,328 @@
 // sweeps_tiled.cu -- the tiled pair kernels: density (eq. (35)), hydro RHS (eqs. (11), (17), (37), (41)-(43)),
 // FLD limiter pre-sweep (eq. (9)) and FLD operator apply (eqs. (16), (47), (51)-(52)) of PAPER.md.
 //
-// One persistent CTA per SM walks the tiles of tiles.cuh.  Per tile it stages the candidate particles' fields
-// (structure-of-arrays, fp64, positions moved to the periodic image next to the tile) into shared memory, then
-// every thread owns ONE target particle and runs down its prebuilt neighbour list (u16 slots, tiles.cu): no
-// distance test on rejected candidates, all 32 lanes busy with accepted pairs, one reciprocal square root per pair
-// (MUFU.RSQ64H seed + one third-order correction), per-particle factors hoisted into the prologue kernels.
-// Results are written to caller order through the sort permutation.  No floating-point atomics: each target is
-// summed by one thread in list order, so results are bitwise reproducible.
+// One persistent CTA of 512 threads per SM walks the tiles of tiles.cuh.  Per tile it stages the candidate
+// particles' fields as 16-byte records (two fp64 fields each, positions moved to the periodic image next to the
+// tile) into shared memory; then two threads share ONE target particle, each running down its scheduled half-list
+// (u16 slots, tiles.cu): no distance test on rejected candidates, all 32 lanes busy with accepted pairs, one
+// 128-bit shared-memory load per record with the 8 lanes of a wavefront mostly in 8 different banks, one
+// reciprocal square root per pair (MUFU.RSQ64H seed + Newton), per-particle factors hoisted into the prologue
+// kernels, kernel normalisations hoisted out of the pair loop where h is uniform over the tile.  Results are
+// written to caller order through the sort permutation.  No floating-point atomics: each half-list is summed in
+// list order and the two halves are added by a shuffle, so results are bitwise reproducible.
 #include "spray_internal.h"
 #include "tiles.cuh"
 
+#ifndef SPRAY_NEWTON_ORDER
+#define SPRAY_NEWTON_ORDER 3
+#endif
+
 namespace spray {
 
-// 1/sqrt(x) for normal positive x to ~1e-16 relative: hardware seed (>= 20 bits) and one third-order step
-// y (1 + e/2 + 3 e^2/8), e = 1 - x y^2.
+// 1/sqrt(x) for normal positive x: hardware seed and one Newton step of order SPRAY_NEWTON_ORDER
+// (2: y (1 + e/2); 3: y (1 + e/2 + 3 e^2/8)), e = 1 - x y^2.
 __device__ __forceinline__ double rsqrt_fast(double x) {
     double y;
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
     const double t = x * y;
     const double e = fma(-t, y, 1.0);
+#if SPRAY_NEWTON_ORDER == 2
+    return fma(0.5 * y, e, y);
+#else
     const double p = fma(0.375, e, 0.5);
-    const double ye = y * e;
-    return fma(ye, p, y);
+    return fma(y * e, p, y);
+#endif
 }
-// 1/x for normal positive x: hardware seed and one third-order step y (1 + e + e^2), e = 1 - x y.
+// 1/x for normal positive x: hardware seed and one step y (1 + e [+ e^2]), e = 1 - x y.
 __device__ __forceinline__ double rcp_fast(double x) {
     double y;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
     const double e = fma(-x, y, 1.0);
-    const double p = fma(e, e, e);
-    return fma(y, p, y);
+#if SPRAY_NEWTON_ORDER == 2
+    return fma(y, e, y);
+#else
+    return fma(y, fma(e, e, e), y);
+#endif
 }
 
-template <int SWEEP> struct NField;
-template <> struct NField<SW_DENSITY> { static constexpr int v = 4; };    // x y z m
-template <> struct NField<SW_HYDRO> { static constexpr int v = 11; };     // x y z hinv V Q m AC vx vy vz
-template <> struct NField<SW_LIMITER> { static constexpr int v = 5; };    // x y z V E
-template <> struct NField<SW_APPLY> { static constexpr int v = 7; };      // x y z hinv V mu E
+// Rescaled shape functions (common.cuh): W = kWn / h^3 * wshape(q), F = dW/dr = kFn / h^4 * gshape(q).
+// CLAMP = false is used where every listed pair is known to be inside the support (uniform h over the tile):
+// rounding can then leave 2 - q at -1e-13 at worst, which contributes nothing at the tolerance of the pass.
+template <int KERNEL, bool CLAMP>
+__device__ __forceinline__ double wshape(double q) {
+    if (KERNEL == 1) {                       // Wendland C2, eq. (3): (1-q/2)^4 (2q+1)
+        double t = fma(-0.5, q, 1.0);
+        if (CLAMP) t = dmax0(t);
+        const double t2 = t * t;
+        return (t2 * t2) * fma(2.0, q, 1.0);
+    } else {                                 // cubic spline (A1): (2-q)^3 - 4 (1-q)_+^3
+        constexpr double C = 1.5874010519681994748;      // cbrt(4)
+        double t2 = 2.0 - q;
+        if (CLAMP) t2 = dmax0(t2);
+        const double t1 = dmax0(fma(-C, q, C));
+        return fma(t2 * t2, t2, -((t1 * t1) * t1));
+    }
+}
+template <int KERNEL, bool CLAMP>
+__device__ __forceinline__ double gshape(double q) {
+    if (KERNEL == 1) {                       // q (1-q/2)^3
+        double t = fma(-0.5, q, 1.0);
+        if (CLAMP) t = dmax0(t);
+        return (q * t) * (t * t);
+    } else {                                 // (2-2q)_+^2 - (2-q)^2
+        double t2 = 2.0 - q;
+        if (CLAMP) t2 = dmax0(t2);
+        const double s1 = dmax0(fma(-2.0, q, 2.0));
+        return fma(s1, s1, -(t2 * t2));
+    }
+}
+template <int KERNEL> __device__ __forceinline__ double wn_k() { return KERNEL == 1 ? kWnWend : kWnCubic; }
+template <int KERNEL> __device__ __forceinline__ double w0_k() { return KERNEL == 1 ? 1.0 : 4.0; }   // wshape(0)
+
+// Records staged per candidate (16 bytes each) and extra fp64 arrays
+template <int SWEEP> struct NRec;
+template <> struct NRec<SW_DENSITY> { static constexpr int v = 2, e = 0; };   // (x,y) (z,m)
+template <> struct NRec<SW_HYDRO> { static constexpr int v = 6, e = 0; };     // (x,y) (z,V) (Q,vx) (vy,vz) (m,alpha c) (1/h,Fn)
+template <> struct NRec<SW_LIMITER> { static constexpr int v = 2, e = 1; };   // (x,y) (z,V) | E
+template <> struct NRec<SW_APPLY> { static constexpr int v = 4, e = 0; };     // (x,y) (z,V) (mu,E) (1/h,Fn)
+
+struct SweepIn {
+    const double2* rec[6];           // sorted global records, in the order of NRec
+    const double* e1;                // sorted E (limiter)
+    const double2* p1;               // (z, h)
+    const double2* hh;               // (1/h, Fn)
+    const double2* t0;               // per-call target record
+    const double2* me;               // (mu, E)
+    double2* me_out;                 // limiter: (mu, E) for the apply
+    double* mu_sorted;               // limiter: mu in sorted order for the general kernels
+    const uint32_t* perm;
+    const TileDesc* tiles;
+    const unsigned long long* ctr;
+    const uint2* pool;
+    const uint2* winfo;
+    const uint32_t* lcount;
+    const uint32_t* tflags;
+    int64_t n;
+    double beta, c_light;
+    int fld_sym;
+    double *o0, *o1, *o2, *o3, *o4;
+    uint32_t* ocount;
+};
+
+struct Acc { double a0, a1, a2, a3, a4; };
+struct Tgt {                         // per-target constants
+    double x, y, z, hinv, fn;
+    double c0, c1, c2, c3, c4, c5;   // per sweep (see k_tiled_sweep)
+};
+
+// One pair (target, slot s).  F = staged records ([record][TILE_CMAXP] double2), Ee = staged E (limiter).
+// UNI: every particle of the tile has the target's h, so F(r;h_b) = F(r;h_a), the normalisation kFn/h^4 is applied
+// once per target after the loop (k_tiled_sweep) and no support clamp is needed.
+template <int SWEEP, int KERNEL, bool UNI>
+__device__ __forceinline__ void pair_body(const double2* __restrict__ F, const double* __restrict__ Ee, uint32_t s, const Tgt& T,
+                                          double beta, bool sym, Acc& acc) {
+    const double2 d0 = F[s], d1 = F[TILE_CMAXP + s];
+    const double dx = T.x - d0.x, dy = T.y - d0.y, dz = T.z - d1.x;
+    const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+    const double y = rsqrt_fast(r2);                     // 1/r  (r2 > 0: coincident pairs never reach the tiled lists)
+    const double r = r2 * y;
+    const double qa = r * T.hinv;
+    if (SWEEP == SW_DENSITY) {
+        // eq. (35)
+        acc.a0 = fma(d1.y, wshape<KERNEL, !UNI>(qa), acc.a0);
+    } else if (SWEEP == SW_HYDRO) {
+        const double2 d2 = F[2 * TILE_CMAXP + s], d3 = F[3 * TILE_CMAXP + s];
+        const double Vb = d1.y, Qb = d2.x;
+        const double dvx = T.c3 - d2.y, dvy = T.c4 - d3.x, dvz = T.c5 - d3.y;
+        const double vr = fma(dvz, dz, fma(dvy, dy, dvx * dx));           // v_ab . x_ab = w r
+        if (UNI) {
+            const double G = gshape<KERNEL, false>(qa) * y;               // F / (r kFn/h^4)
+            // eq. (11) P:L98 with the sign of eq. (5) (A3): -(m_b/(rho_a rho_b)) (p_a F_a + p_b F_b) x_ab / r
+            double c = fma(Vb, T.c0, Qb * T.c1);
+            if (vr < 0.0) {                  // eqs. (41)-(43) P:L236-L242 (A6, A7, A8)
+                const double2 d4 = F[4 * TILE_CMAXP + s];
+                const double w = vr * y, hw = 0.5 * w;
+                const double vsa = fma(-beta, w, T.c2), vsb = fma(-beta, w, d4.y);
+                c = fma(-hw, fma(d4.x * T.c1, vsa, Vb * vsb), c);
+                acc.a4 = fma((hw * w) * (d4.x * vsa), G * r, acc.a4);
+            }
+            const double cg = c * G;
+            acc.a0 = fma(cg, dx, acc.a0); acc.a1 = fma(cg, dy, acc.a1); acc.a2 = fma(cg, dz, acc.a2);
+            acc.a3 = fma(Vb * G, vr, acc.a3);                             // eq. (37)
+        } else {
+            const double2 d5 = F[5 * TILE_CMAXP + s];
+            const double Ga = (gshape<KERNEL, true>(qa) * y) * T.fn;
+            const double Gb = (gshape<KERNEL, true>(r * d5.x) * y) * d5.y;
+            double c = fma(Vb * T.c0, Ga, (Qb * T.c1) * Gb);
+            if (vr < 0.0) {
+                const double2 d4 = F[4 * TILE_CMAXP + s];
+                const double w = vr * y, hw = 0.5 * w;
+                const double vsa = fma(-beta, w, T.c2), vsb = fma(-beta, w, d4.y);
+                c = fma(-hw, fma((d4.x * T.c1) * vsa, Ga, (Vb * vsb) * Gb), c);
+                acc.a4 = fma((hw * w) * (d4.x * vsa), Ga * r, acc.a4);
+            }
+            acc.a0 = fma(c, dx, acc.a0); acc.a1 = fma(c, dy, acc.a1); acc.a2 = fma(c, dz, acc.a2);
+            acc.a3 = fma(Vb * Ga, vr, acc.a3);
+        }
+    } else if (SWEEP == SW_LIMITER) {
+        // eq. (9) phi = 1 with f = E (A19): h_a only
+        const double G = gshape<KERNEL, !UNI>(qa) * y;
+        const double cc = (d1.y * (Ee[s] - T.c0)) * G;
+        acc.a0 = fma(cc, dx, acc.a0); acc.a1 = fma(cc, dy, acc.a1); acc.a2 = fma(cc, dz, acc.a2);
+    } else {
+        // eq. (47) first term P:L270 on eq. (16); Fbar as P:L134 (A17)
+        const double2 d2 = F[2 * TILE_CMAXP + s];
+        double G;
+        if (UNI) {
+            G = gshape<KERNEL, false>(qa) * y;
+        } else {
+            double Fbar = gshape<KERNEL, true>(qa) * T.fn;
+            if (sym) {
+                const double2 d3 = F[3 * TILE_CMAXP + s];
+                Fbar = 0.5 * fma(gshape<KERNEL, true>(r * d3.x), d3.y, Fbar);
+            }
+            G = Fbar * y;
+        }
+        const double hm = (T.c2 * d2.x) * rcp_fast(T.c1 + d2.x);          // 4 mu_a mu_b / (mu_a + mu_b)
+        const double cab = (d1.y * hm) * G;
+        acc.a0 = fma(cab, T.c0 - d2.y, acc.a0);                           // difference form (O7)
+        acc.a1 += cab;
+    }
+}
+
+template <int SWEEP, int KERNEL, bool UNI>
+__device__ __forceinline__ void pair_loop(const double2* __restrict__ F, const double* __restrict__ Ee, const uint2* __restrict__ lp,
+                                          uint32_t R, const Tgt& T, double beta, bool sym, Acc& acc) {
+    uint2 cur = R ? __ldg(lp) : make_uint2(0u, 0u);
+    for (uint32_t r4 = 0; r4 < R; r4 += 4) {
+        const uint2 nxt = (r4 + 4 < R) ? __ldg(lp + (size_t)(r4 / 4 + 1) * 32) : make_uint2(0u, 0u);
+        pair_body<SWEEP, KERNEL, UNI>(F, Ee, cur.x & 0xFFFFu, T, beta, sym, acc);
+        pair_body<SWEEP, KERNEL, UNI>(F, Ee, cur.x >> 16, T, beta, sym, acc);
+        pair_body<SWEEP, KERNEL, UNI>(F, Ee, cur.y & 0xFFFFu, T, beta, sym, acc);
+        pair_body<SWEEP, KERNEL, UNI>(F, Ee, cur.y >> 16, T, beta, sym, acc);
+        cur = nxt;
+    }
+}
+
+template <int SWEEP> struct MinBlocks { static constexpr int v = (SWEEP == SW_DENSITY || SWEEP == SW_LIMITER) ? 2 : 1; };
 
 template <int SWEEP, int KERNEL>
-__global__ void __launch_bounds__(TILE_T, 1)
-k_tiled_sweep(DevGrid g, CellTable ct, TiledArgs A) {
-    constexpr int NF = NField<SWEEP>::v;
+__global__ void __launch_bounds__(TILE_THREADS, MinBlocks<SWEEP>::v)
+k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
+    constexpr int NV = NRec<SWEEP>::v;
     extern __shared__ __align__(16) unsigned char smem[];
     __shared__ TileS S;
-    double* F = reinterpret_cast<double*>(smem);                 // F[f * TILE_CMAX + slot]
+    double2* F = reinterpret_cast<double2*>(smem);               // F[record * TILE_CMAXP + slot]
+    double* Ee = reinterpret_cast<double*>(F + (size_t)NV * TILE_CMAXP);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const uint32_t ntiles = *A.ntiles;
+    const int u = tid & 1, tgt = tid >> 1;
+    const uint32_t ntiles = (uint32_t)A.ctr[CTR_NTILES];
     const bool sym = (SWEEP == SW_HYDRO) || (SWEEP == SW_APPLY && A.fld_sym != 0);
+    // dummy slots: far away, every weight zero, so that a padded list entry adds exactly nothing
+    if (tid < TILE_NDUMMY) {
+        const double far = g.lo[0] - 1.0e4 * g.L[0];
+#pragma unroll
+        for (int v = 0; v < NV; ++v) F[v * TILE_CMAXP + TILE_CMAX + tid] = make_double2(0.0, 0.0);
+        F[TILE_CMAX + tid] = make_double2(far, g.lo[1]);
+        F[TILE_CMAXP + TILE_CMAX + tid] = make_double2(g.lo[2], 0.0);
+        if (SWEEP == SW_APPLY) F[2 * TILE_CMAXP + TILE_CMAX + tid] = make_double2(1.0, 0.0);
+        if (NRec<SWEEP>::e) Ee[TILE_CMAX + tid] = 0.0;
+    }
 
     for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-        if (!A.tile_ok[tile]) continue;
+        const uint32_t flags = A.tflags[tile];
+        if (!(flags & TILE_FLAG_OK)) continue;
+        const bool uni = (flags & TILE_FLAG_UNIH) != 0;
         const TileDesc td = A.tiles[tile];
-        __syncthreads();
+        __syncthreads();                                         // previous tile done with the staged records
         tile_setup(td, g, ct, S);
-        const uint32_t ncand = S.ncand;
-        // ---- stage candidate fields
-        for (uint32_t s = tid; s < ncand; s += TILE_T) {
-            const int q = tile_slot_range(S, s);
-            const uint32_t gi = S.r_start[q] + (s - S.r_base[q]);
-            if (gi >= S.r_vstart[q] && gi < S.r_vend[q]) {
-                F[0 * TILE_CMAX + s] = A.x[gi] - S.r_shift[q][0] * g.L[0];
-                F[1 * TILE_CMAX + s] = A.y[gi] - S.r_shift[q][1] * g.L[1];
-                F[2 * TILE_CMAX + s] = A.z[gi] - S.r_shift[q][2] * g.L[2];
-                if (SWEEP == SW_DENSITY) {
-                    F[3 * TILE_CMAX + s] = A.f0[gi];                                   // m
-                } else if (SWEEP == SW_HYDRO) {
-                    F[3 * TILE_CMAX + s] = 1.0 / A.h[gi];
-                    F[4 * TILE_CMAX + s] = A.f0[gi];                                   // V = m/rho
-                    F[5 * TILE_CMAX + s] = A.f1[gi];                                   // Q = V p
-                    F[6 * TILE_CMAX + s] = A.f2[gi];                                   // m
-                    F[7 * TILE_CMAX + s] = A.f3[gi];                                   // alpha c
-                    F[8 * TILE_CMAX + s] = A.f4[gi];
-                    F[9 * TILE_CMAX + s] = A.f5[gi];
-                    F[10 * TILE_CMAX + s] = A.f6[gi];
-                } else if (SWEEP == SW_LIMITER) {
-                    F[3 * TILE_CMAX + s] = A.f0[gi];                                   // V
-                    F[4 * TILE_CMAX + s] = A.f1[gi];                                   // E
-                } else {
-                    F[3 * TILE_CMAX + s] = 1.0 / A.h[gi];
-                    F[4 * TILE_CMAX + s] = A.f0[gi];                                   // V
-                    F[5 * TILE_CMAX + s] = A.f2[gi];                                   // mu
-                    F[6 * TILE_CMAX + s] = A.f1[gi];                                   // E
+        // ---- stage the candidate records: one warp per range
+        for (int q = warp; q < (int)S.nranges; q += TILE_WARPS) {
+            const uint32_t vs = S.r_vstart[q], len = S.r_vend[q] - vs, base = S.r_base[q];
+            const double shx = S.r_shift[q][0] * g.L[0], shy = S.r_shift[q][1] * g.L[1], shz = S.r_shift[q][2] * g.L[2];
+            for (uint32_t k = lane; k < len; k += 32) {
+#pragma unroll
+                for (int v = 0; v < NV; ++v) {
+                    if (uni && ((SWEEP == SW_HYDRO && v == 5) || (SWEEP == SW_APPLY && v == 3))) continue;
+                    double2 val = A.rec[v][vs + k];
+                    if (v == 0) { val.x -= shx; val.y -= shy; }
+                    if (v == 1) val.x -= shz;
+                    F[v * TILE_CMAXP + base + k] = val;
                 }
+                if (NRec<SWEEP>::e) Ee[base + k] = A.e1[vs + k];
             }
         }
         // ---- this thread's target
-        const bool active = tid < (int)td.nt;
-        uint32_t i = 0, nloop = 0, ng = 0;
-        double xa = 0, ya = 0, za = 0, hinv = 1, Wn = 0, Fn = 0;
-        double a0 = 0, a1 = 0, a2 = 0, a3 = 0, a4 = 0, a5 = 0;           // per-sweep target constants
+        const bool active = tgt < (int)td.nt;
+        uint32_t i = 0;
+        Tgt T{};
         if (active) {
-            i = tile_target(td, S, tid);
-            const uint32_t cnt = A.lcount[(size_t)tile * TILE_T + tid];
-            ng = cnt & 0xFFFFu;
-            nloop = sym ? (cnt >> 16) : ng;
-            xa = A.x[i]; ya = A.y[i]; za = A.z[i];
-            hinv = 1.0 / A.h[i];
-            Wn = sigma<KERNEL>() * hinv * hinv * hinv;
-            Fn = Wn * hinv;
-            if (SWEEP == SW_DENSITY) { a0 = A.f0[i]; }
+            i = tile_target(td, S, tgt);
+            const double2 xy = A.rec[0][i], zh = A.p1[i], hv = A.hh[i];
+            T.x = xy.x; T.y = xy.y; T.z = zh.x; T.hinv = hv.x; T.fn = hv.y;
+            if (SWEEP == SW_DENSITY) T.c0 = A.rec[1][i].y;                                   // m_a
             if (SWEEP == SW_HYDRO) {
-                const double rho_a = A.g0[i], p_a = A.g1[i];
-                a0 = 1.0 / rho_a;                 // IA
-                a1 = p_a * a0;                    // PA = p_a / rho_a
-                a2 = A.f3[i];                     // alpha_a c_a
-                a3 = A.f4[i]; a4 = A.f5[i]; a5 = A.f6[i];
+                const double2 t0 = A.t0[i], q1 = A.rec[2][i], q2 = A.rec[3][i];
+                T.c0 = t0.x; T.c1 = t0.y;                                                    // p_a/rho_a, 1/rho_a
+                T.c2 = A.rec[4][i].y;                                                        // alpha_a c_a
+                T.c3 = q1.y; T.c4 = q2.x; T.c5 = q2.y;                                       // v_a
             }
-            if (SWEEP == SW_LIMITER) { a0 = A.f1[i]; }
-            if (SWEEP == SW_APPLY) { a0 = A.f1[i]; a1 = A.f2[i]; }
+            if (SWEEP == SW_LIMITER) T.c0 = A.e1[i];                                         // E_a
+            if (SWEEP == SW_APPLY) { const double2 me = A.rec[2][i]; T.c0 = me.y; T.c1 = me.x; T.c2 = 4.0 * me.x; }
         }
-        uint32_t nmax = nloop;
-#pragma unroll
-        for (int o = 16; o; o >>= 1) nmax = max(nmax, __shfl_xor_sync(0xFFFFFFFFu, nmax, o));
+        const uint2 wi = A.winfo[(size_t)tile * TILE_WARPS + warp];
         __syncthreads();
 
-        double acc0 = 0, acc1 = 0, acc2 = 0, acc3 = 0, acc4 = 0;
-        const uint2* lp = A.lists + list_block_u2(tile, warp) + lane;
-        uint2 cur = nmax ? lp[0] : make_uint2(0u, 0u);
-        for (uint32_t k0 = 0; k0 < nmax; k0 += 4) {
-            const uint2 nxt = (k0 + 4 < nmax) ? lp[(size_t)(k0 / 4 + 1) * 32] : make_uint2(0u, 0u);
-            const uint32_t ee[4] = {cur.x & 0xFFFFu, cur.x >> 16, cur.y & 0xFFFFu, cur.y >> 16};
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                if (k0 + j < nloop) {
-                    const uint32_t s = ee[j] & 0x7FFFu;
-                    const double dx = xa - F[0 * TILE_CMAX + s];
-                    const double dy = ya - F[1 * TILE_CMAX + s];
-                    const double dz = za - F[2 * TILE_CMAX + s];
-                    const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-                    const double rinv = r2 > 0.0 ? rsqrt_fast(r2) : 0.0;
-                    const double r = r2 * rinv;
-                    if (SWEEP == SW_DENSITY) {
-                        // eq. (35)
-                        acc0 = fma(F[3 * TILE_CMAX + s], shape_w<KERNEL>(r * hinv), acc0);
-                    } else if (SWEEP == SW_HYDRO) {
-                        const double hbinv = F[3 * TILE_CMAX + s];
-                        const double hb2 = hbinv * hbinv;
-                        const double Fa = Fn * shape_f<KERNEL>(r * hinv);
-                        const double Fb = (sigma<KERNEL>() * (hb2 * hb2)) * shape_f<KERNEL>(r * hbinv);
-                        const double Vb = F[4 * TILE_CMAX + s], Qb = F[5 * TILE_CMAX + s];
-                        const double w = ((a3 - F[8 * TILE_CMAX + s]) * dx + (a4 - F[9 * TILE_CMAX + s]) * dy +
-                                          (a5 - F[10 * TILE_CMAX + s]) * dz) * rinv;
-                        const double VFa = Vb * Fa;
-                        // eq. (11) P:L98 with the sign of eq. (5) (A3): -(m_b/(rho_a rho_b)) (p_a F_a + p_b F_b)
-                        double coef = -fma(VFa, a1, (Qb * a0) * Fb);
-                        if (w < 0.0) {               // eqs. (41)-(43) P:L236-L242 (A6, A7, A8)
-                            const double mb = F[6 * TILE_CMAX + s];
-                            const double aw = -w;
-                            const double vsa = fma(A.beta, aw, a2);
-                            const double vsb = fma(A.beta, aw, F[7 * TILE_CMAX + s]);
-                            const double mFa = mb * Fa;
-                            coef = fma(0.5 * w, fma(mFa * a0, vsa, (Vb * Fb) * vsb), coef);
-                            acc4 = fma(0.5 * (w * w), mFa * vsa, acc4);
-                        }
-                        const double cr = coef * rinv;
-                        acc0 = fma(cr, dx, acc0); acc1 = fma(cr, dy, acc1); acc2 = fma(cr, dz, acc2);
-                        acc3 = fma(VFa, w, acc3);    // eq. (37)
-                    } else if (SWEEP == SW_LIMITER) {
-                        // eq. (9) phi = 1 with f = E (A19)
-                        const double cc = (F[3 * TILE_CMAX + s] * (F[4 * TILE_CMAX + s] - a0)) * ((Fn * shape_f<KERNEL>(r * hinv)) * rinv);
-                        acc0 = fma(cc, dx, acc0); acc1 = fma(cc, dy, acc1); acc2 = fma(cc, dz, acc2);
-                    } else {
-                        // eq. (47) first term P:L270 on eq. (16); Fbar as P:L134 (A17)
-                        double Fbar = Fn * shape_f<KERNEL>(r * hinv);
-                        if (sym) {
-                            const double hbinv = F[3 * TILE_CMAX + s];
-                            const double hb2 = hbinv * hbinv;
-                            Fbar = 0.5 * fma(sigma<KERNEL>() * (hb2 * hb2), shape_f<KERNEL>(r * hbinv), Fbar);
-                        }
-                        const double mu_b = F[5 * TILE_CMAX + s], E_b = F[6 * TILE_CMAX + s];
-                        const double hm = (4.0 * a1) * mu_b * rcp_fast(a1 + mu_b);
-                        const double cab = (F[4 * TILE_CMAX + s] * hm) * (Fbar * rinv);
-                        acc0 = fma(cab, a0 - E_b, acc0);
-                        acc1 += cab;
-                        acc2 = fma(-cab, E_b, acc2);
-                    }
-                }
-            }
-            cur = nxt;
+        Acc acc{0, 0, 0, 0, 0};
+        const uint2* lp = A.pool + wi.x + lane;
+        if (uni) pair_loop<SWEEP, KERNEL, true>(F, Ee, lp, wi.y, T, A.beta, sym, acc);
+        else pair_loop<SWEEP, KERNEL, false>(F, Ee, lp, wi.y, T, A.beta, sym, acc);
+        // ---- add the two half-lists of the target
+        acc.a0 += __shfl_xor_sync(0xFFFFFFFFu, acc.a0, 1);
+        if (SWEEP != SW_DENSITY) acc.a1 += __shfl_xor_sync(0xFFFFFFFFu, acc.a1, 1);
+        if (SWEEP == SW_HYDRO || SWEEP == SW_LIMITER) acc.a2 += __shfl_xor_sync(0xFFFFFFFFu, acc.a2, 1);
+        if (SWEEP == SW_HYDRO) {
+            acc.a3 += __shfl_xor_sync(0xFFFFFFFFu, acc.a3, 1);
+            acc.a4 += __shfl_xor_sync(0xFFFFFFFFu, acc.a4, 1);
         }
 
-        if (active) {
+        if (active && u == 0) {
             const uint32_t ia = A.perm[i];
+            const double sc = uni ? T.fn : 1.0;                  // kFn / h_a^4 where it was hoisted out of the loop
             if (SWEEP == SW_DENSITY) {
-                A.o0[ia] = Wn * (acc0 + a0);         // self term m_a W(0; h_a): both shape functions are 1 at q = 0 (A11)
-                if (A.ocount) A.ocount[ia] = ng;
+                // self term m_a W(0; h_a) (A11)
+                const double wn = wn_k<KERNEL>() * (T.hinv * T.hinv) * T.hinv;
+                A.o0[ia] = wn * fma(T.c0, w0_k<KERNEL>(), acc.a0);
+                if (A.ocount) A.ocount[ia] = A.lcount[(size_t)tile * TILE_T + tgt] & 0xFFFFu;
             } else if (SWEEP == SW_HYDRO) {
-                A.o0[ia] = acc0; A.o1[ia] = acc1; A.o2[ia] = acc2;
-                A.o3[ia] = a1 * acc3 - acc4 * a0;    // eq. (17) 1st term P:L129 + eq. (42)
-                if (A.o4) A.o4[ia] = acc3;
+                A.o0[ia] = -(sc * acc.a0); A.o1[ia] = -(sc * acc.a1); A.o2[ia] = -(sc * acc.a2);
+                const double D = sc * acc.a3;
+                A.o3[ia] = T.c0 * D - (sc * acc.a4) * T.c1;      // eq. (17) 1st term P:L129 + eq. (42)
+                if (A.o4) A.o4[ia] = D;
             } else if (SWEEP == SW_LIMITER) {
-                // Larsen limiter, k = 2 (A20)
-                const double rk = A.g0[i] * A.g1[i];
-                const double gn = sqrt(acc0 * acc0 + acc1 * acc1 + acc2 * acc2);
-                const double R = gn / (rk * a0);
-                const double mu = A.c_light * (1.0 / sqrt(9.0 + R * R)) / rk;
+                // Larsen limiter, k = 2 (A20); the limiter sum always carries kFn/h_a^4 outside
+                const double gx = T.fn * acc.a0, gy = T.fn * acc.a1, gz = T.fn * acc.a2;
+                const double rk = A.t0[i].x;                     // rho_a kappa_a
+                const double gn = sqrt(gx * gx + gy * gy + gz * gz);
+                const double Rl = gn / (rk * T.c0);
+                const double mu = A.c_light * (1.0 / sqrt(9.0 + Rl * Rl)) / rk;
                 A.o0[ia] = mu;
+                A.me_out[i] = make_double2(mu, T.c0);
                 A.mu_sorted[i] = mu;
-                if (A.o1) { A.o1[ia] = acc0; A.o1[A.n + ia] = acc1; A.o1[2 * A.n + ia] = acc2; }
+                if (A.o1) { A.o1[ia] = gx; A.o1[A.n + ia] = gy; A.o1[2 * A.n + ia] = gz; }
             } else {
-                A.o0[ia] = acc0;
-                if (A.o1) A.o1[ia] = acc1;
-                if (A.o2) A.o2[ia] = acc2;
+                const double yv = sc * acc.a0, lam = sc * acc.a1;
+                A.o0[ia] = yv;
+                if (A.o1) A.o1[ia] = lam;
+                if (A.o2) A.o2[ia] = fma(-lam, T.c0, yv);        // Gamma = y - Lambda E_a  (eq. (52))
             }
         }
     }
 }
 
 template <int SWEEP>
-static cudaError_t launch_t(Ctx* c, const TiledArgs& a, cudaStream_t st) {
-    constexpr size_t smem = sizeof(double) * NField<SWEEP>::v * TILE_CMAX;
+static cudaError_t launch_t(Ctx* c, const SweepIn& a, cudaStream_t st) {
+    constexpr size_t smem = sizeof(double2) * NRec<SWEEP>::v * TILE_CMAXP + sizeof(double) * NRec<SWEEP>::e * TILE_CMAXP;
     static bool attr_done = false;
     if (!attr_done) {
         cudaError_t e = cudaFuncSetAttribute(k_tiled_sweep<SWEEP, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -220,24 +331,32 @@ static cudaError_t launch_t(Ctx* c, const TiledArgs& a, cudaStream_t st) {
         attr_done = true;
     }
     CellTable ct{c->cell_start, c->cell_end};
-    const int per_sm = (int)((220 * 1024) / (smem + sizeof(TileS) + 1024));
-    const int grid = c->tl.sms * (per_sm < 1 ? 1 : (per_sm > 4 ? 4 : per_sm));
-    if (c->kernel == SPRAY_KERNEL_WENDLAND_C2) k_tiled_sweep<SWEEP, 1><<<grid, TILE_T, smem, st>>>(c->dg, ct, a);
-    else k_tiled_sweep<SWEEP, 0><<<grid, TILE_T, smem, st>>>(c->dg, ct, a);
+    const int grid = c->tl.sms * MinBlocks<SWEEP>::v;
+    if (c->kernel == SPRAY_KERNEL_WENDLAND_C2) k_tiled_sweep<SWEEP, 1><<<grid, TILE_THREADS, smem, st>>>(c->dg, ct, a);
+    else k_tiled_sweep<SWEEP, 0><<<grid, TILE_THREADS, smem, st>>>(c->dg, ct, a);
     c->launches += 1;
     return cudaGetLastError();
 }
 
-cudaError_t launch_tiled_sweep(Ctx* c, int sweep, TiledArgs a, cudaStream_t st) {
+cudaError_t launch_tiled_sweep(Ctx* c, int sweep, const TiledArgs& t, cudaStream_t st) {
     if (c->n == 0) return cudaSuccess;
-    a.tiles = c->tl.tiles; a.ntiles = c->tl.ntiles; a.lists = c->tl.lists; a.lcount = c->tl.lcount; a.tile_ok = c->tl.tile_ok;
-    a.perm = c->perm; a.n = c->n;
-    a.x = c->s.x; a.y = c->s.y; a.z = c->s.z; a.h = c->s.h;
+    SweepIn a{};
+    const Packed& pk = c->pk;
+    a.p1 = pk.p1; a.hh = pk.hh; a.t0 = pk.t0; a.me = pk.me; a.me_out = pk.me; a.mu_sorted = c->s.f[10]; a.e1 = pk.e1;
+    a.perm = c->perm; a.tiles = c->tl.tiles; a.ctr = c->tl.ctr; a.pool = c->tl.pool; a.winfo = c->tl.winfo;
+    a.lcount = c->tl.lcount; a.tflags = c->tl.tflags; a.n = c->n;
+    a.beta = t.beta; a.c_light = t.c_light; a.fld_sym = t.fld_sym;
+    a.o0 = t.o0; a.o1 = t.o1; a.o2 = t.o2; a.o3 = t.o3; a.o4 = t.o4; a.ocount = t.ocount;
+    a.rec[0] = pk.p0; a.rec[1] = pk.s[0];
     switch (sweep) {
         case SW_DENSITY: return launch_t<SW_DENSITY>(c, a, st);
-        case SW_HYDRO: return launch_t<SW_HYDRO>(c, a, st);
+        case SW_HYDRO:
+            a.rec[2] = pk.s[1]; a.rec[3] = pk.s[2]; a.rec[4] = pk.s[3]; a.rec[5] = pk.hh;
+            return launch_t<SW_HYDRO>(c, a, st);
         case SW_LIMITER: return launch_t<SW_LIMITER>(c, a, st);
-        case SW_APPLY: return launch_t<SW_APPLY>(c, a, st);
+        case SW_APPLY:
+            a.rec[2] = pk.me; a.rec[3] = pk.hh;
+            return launch_t<SW_APPLY>(c, a, st);
     }
     return cudaErrorInvalidValue;
 }

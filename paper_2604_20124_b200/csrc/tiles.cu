@@ -3,135 +3,170 @@
 // NNPS, PAPER.md L434-L446 (§2.6): the cell list identifies the particles of the 27 cells around a target; "a
 // majority of computational time is spent on searching and identifying neighboring particles" (L436).  Here the
 // search is done ONCE per cell build and its result -- for every target the list of its mutual neighbours N_sym
-// (L442 "ensure all neighbors are mutual"), gather neighbours first -- is kept as u16 slots of the tile's
-// candidate layout (tiles.cuh), so the four pair sweeps that follow (and every later spray_fld_apply of an
-// implicit solve, L327) run their pair bodies at full lane occupancy with no distance test on rejected candidates.
+// (L442 "ensure all neighbors are mutual") -- is kept as u16 slots of the tile's candidate layout (tiles.cuh), so
+// the four pair sweeps that follow (and every later spray_fld_apply of an implicit solve, L327) run their pair
+// bodies at full lane occupancy with no distance test on rejected candidates.
 //
-// The candidate test is done in two steps: an fp32 prefilter on tile-relative coordinates (conservative margin,
-// off the FP64 pipe), then the exact contract predicate in fp64 (common.cuh: r2_exact / support2 / min_image) on the
-// survivors, so the sets are bit-identical to the definition.
+// The candidate test is an fp32 prefilter on tile-relative coordinates; a hit closer to a support boundary than
+// the fp32 error bound (or to r = 0) is re-tested with the exact contract predicate in fp64 (common.cuh:
+// r2_exact / support2 / min_image), so the sets are bit-identical to the definition.
+//
+// SCHEDULED LISTS.  The pair kernels gather 16-byte records of their neighbours from shared memory; 8 lanes form
+// one 128-byte wavefront and conflict when two of them read different records of the same bank (slot & 7).  A
+// target's neighbours are therefore split between its two threads bank by bank, and each thread's half-list is
+// emitted in an order that walks the banks in phase with the other lanes of its 8-lane group: lane j spends
+// rounds [t R / 8, (t + 1) R / 8) in bank (j + t) & 7, entries that do not fit their phase fill the holes of other
+// phases, the remaining holes are dummy slots (records that contribute exactly zero).
 #include "spray_internal.h"
 #include "tiles.cuh"
 
 namespace spray {
 
 // ------------------------------------------------------------------------------------------- tile construction
-// One thread per bundle of 2 x 2 rows walks the columns and emits tiles greedily: up to TILE_T targets, at most
-// TILE_CMAX candidate slots, at most TILE_BXMAX columns.  A column whose own candidate set does not fit is left to
-// the general kernels (its particles keep fast[i] = 0).
-__device__ uint32_t bundle_col_count(const DevGrid& g, const CellTable& ct, int y0, int nyr, int z0, int nzr, int cx) {
-    uint32_t c = 0;
-    for (int rz = 0; rz < nzr; ++rz)
-        for (int ry = 0; ry < nyr; ++ry) {
-            const uint32_t id = cell_id(g, cx, y0 + ry, z0 + rz);
-            c += ct.cell_end[id] - ct.cell_start[id];
-        }
-    return c;
+// One warp per bundle of 2 x 2 rows walks the columns and cuts tiles greedily: up to TILE_T targets, at most
+// TILE_CMAX candidate slots, at most TILE_BXMAX columns.  Lane l < 16 owns candidate row l (rz * 4 + ry).  A column
+// whose own candidate set does not fit is left to the general kernels.  Run twice: EMIT = false counts the tiles
+// of every bundle, EMIT = true writes them at the scanned offsets, so the tile order is deterministic and follows
+// the grid (consecutive tiles share candidate rows in L2).
+struct RowRef {                      // one candidate row of a bundle
+    const uint32_t *cs, *ce;         // cell_start / cell_end of the row (indexed by column)
+    bool valid;
+    bool target;                     // the row is one of the bundle's own rows
+};
+__device__ __forceinline__ uint32_t row_count(const RowRef& r, int xlo, int xhi, int nx, bool per) {
+    if (!r.valid) return 0u;
+    if (per) {
+        if (xlo < 0) return (r.ce[nx - 1] - r.cs[xlo + nx]) + (r.ce[xhi] - r.cs[0]);
+        if (xhi >= nx) return (r.ce[nx - 1] - r.cs[xlo]) + (r.ce[xhi - nx] - r.cs[0]);
+    } else {
+        xlo = xlo < 0 ? 0 : xlo;
+        xhi = xhi > nx - 1 ? nx - 1 : xhi;
+    }
+    return r.ce[xhi] - r.cs[xlo];
 }
-__device__ uint32_t tile_ncand(const TileDesc& td, const DevGrid& g, const CellTable& ct) {
-    uint32_t tot = 0;
-    RangeGeo R;
-    for (int q = 0; q < 32; ++q)
-        if (tile_range(td, g, ct, q >> 1, q & 1, R)) tot += range_padded_len(R.vs, R.ve);
-    return tot;
+__device__ __forceinline__ uint32_t warp_sum(uint32_t v) {
+#pragma unroll
+    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
+    return v;
 }
 
-__global__ void k_make_tiles(DevGrid g, CellTable ct, const double* __restrict__ hglob, TileDesc* __restrict__ tiles,
-                             uint32_t* __restrict__ ntiles, uint32_t cap, uint32_t* __restrict__ status) {
+template <bool EMIT>
+__global__ void __launch_bounds__(256)
+k_make_tiles(DevGrid g, CellTable ct, const double* __restrict__ hglob, uint32_t* __restrict__ bcount,
+             TileDesc* __restrict__ tiles, uint32_t cap, unsigned long long* __restrict__ ctr) {
     const int nby = (g.nc[1] + 1) / 2, nbz = (g.nc[2] + 1) / 2;
-    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    const int b = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
     if (b >= nby * nbz) return;
     // every neighbour within one cell: 2 h_max <= cell edge in every dimension (tiny safety margin)
     const double hmax = hglob[1];
+    bool ok = true;
     for (int d = 0; d < 3; ++d)
-        if (!(2.0 * hmax * g.inv[d] * (1.0 + 1e-9) <= 1.0)) return;
+        if (!(2.0 * hmax * g.inv[d] * (1.0 + 1e-9) <= 1.0)) ok = false;
     const int nx = g.nc[0];
-    TileDesc td;
-    td.y0 = (int16_t)(2 * (b % nby)); td.z0 = (int16_t)(2 * (b / nby));
-    td.nyr = (uint8_t)min(2, g.nc[1] - td.y0); td.nzr = (uint8_t)min(2, g.nc[2] - td.z0);
-    td.pad = 0; td.pad2 = 0;
+    const int y0 = 2 * (b % nby), z0 = 2 * (b / nby);
+    const int nyr = min(2, g.nc[1] - y0), nzr = min(2, g.nc[2] - z0);
+    RowRef row;
+    {
+        const int ry = lane & 3, rz = (lane >> 2) & 3;
+        int cy = y0 - 1 + ry, cz = z0 - 1 + rz;
+        row.valid = lane < 16 && ry < nyr + 2 && rz < nzr + 2;
+        if (cy < 0) { if (g.per[1]) cy += g.nc[1]; else row.valid = false; }
+        else if (cy >= g.nc[1]) { if (g.per[1]) cy -= g.nc[1]; else row.valid = false; }
+        if (cz < 0) { if (g.per[2]) cz += g.nc[2]; else row.valid = false; }
+        else if (cz >= g.nc[2]) { if (g.per[2]) cz -= g.nc[2]; else row.valid = false; }
+        row.target = row.valid && ry >= 1 && ry <= nyr && rz >= 1 && rz <= nzr;
+        const uint32_t base = row.valid ? cell_id(g, 0, cy, cz) : 0u;
+        row.cs = ct.cell_start + base; row.ce = ct.cell_end + base;
+    }
+    const bool per = g.per[0] != 0;
+    uint32_t ntl = 0;
+    const uint32_t obase = EMIT ? bcount[b] : 0u;
     int cxa = 0;
     uint32_t skip = 0;
-    while (cxa < nx) {
-        td.cxa = (int16_t)cxa; td.cxb = (int16_t)cxa; td.skip = skip;
-        if (tile_ncand(td, g, ct) > (uint32_t)TILE_CMAX) { ++cxa; skip = 0; continue; }   // column not tileable
+    while (ok && cxa < nx) {
+        if (warp_sum(row_count(row, cxa - 1, cxa + 1, nx, per)) > (uint32_t)TILE_CMAX) { ++cxa; skip = 0; continue; }   // column not tileable
         uint32_t nt = 0;
-        int next_cxa = nx;
+        int cxb = cxa, next_cxa = nx;
         uint32_t next_skip = 0;
         for (int cx = cxa; cx < nx; ++cx) {
             if (cx > cxa) {
                 const int ext = cx - cxa + 1;
-                TileDesc t2 = td;
-                t2.cxb = (int16_t)cx;
-                if (ext > TILE_BXMAX || (g.per[0] && ext + 2 > nx) || tile_ncand(t2, g, ct) > (uint32_t)TILE_CMAX) {
+                if (ext > TILE_BXMAX || (per && ext + 2 > nx) ||
+                    warp_sum(row_count(row, cxa - 1, cx + 1, nx, per)) > (uint32_t)TILE_CMAX) {
                     next_cxa = cx; next_skip = 0; break;
                 }
             }
-            uint32_t c = bundle_col_count(g, ct, td.y0, td.nyr, td.z0, td.nzr, cx);
+            uint32_t c = warp_sum(row.target ? row.ce[cx] - row.cs[cx] : 0u);
             if (cx == cxa) c -= skip;
             const uint32_t take = min(c, (uint32_t)TILE_T - nt);
             nt += take;
-            td.cxb = (int16_t)cx;
+            cxb = cx;
             if (take < c) { next_cxa = cx; next_skip = (cx == cxa ? skip : 0u) + take; break; }
             if (nt == (uint32_t)TILE_T) { next_cxa = cx + 1; next_skip = 0; break; }
         }
         if (nt > 0) {
-            td.nt = nt;
-            const uint32_t idx = atomicAdd(ntiles, 1u);
-            if (idx < cap) tiles[idx] = td;
-            else atomicOr(status, (uint32_t)SPRAY_DEV_LIST_OVERFLOW);   // dropped tile: its particles use the general kernels
+            if (EMIT && lane == 0 && obase + ntl < cap) {
+                TileDesc td;
+                td.y0 = (int16_t)y0; td.z0 = (int16_t)z0; td.cxa = (int16_t)cxa; td.cxb = (int16_t)cxb;
+                td.nyr = (uint8_t)nyr; td.nzr = (uint8_t)nzr; td.pad = 0; td.skip = skip; td.nt = nt; td.pad2 = 0;
+                tiles[obase + ntl] = td;
+            }
+            ++ntl;
         }
         cxa = next_cxa; skip = next_skip;
     }
+    if (!EMIT) {
+        if (lane == 0) bcount[b] = ntl;
+    } else if (b == nby * nbz - 1 && lane == 0) {
+        const uint32_t total = obase + ntl;
+        ctr[CTR_NTILES] = total < cap ? total : cap;
+        if (total > cap) ctr[CTR_NTILES] = cap;      // dropped tiles: their particles use the general kernels
+    }
 }
-__global__ void k_clamp_ntiles(uint32_t* ntiles, uint32_t cap) { if (*ntiles > cap) *ntiles = cap; }
 
 // ------------------------------------------------------------------------------------------- list builder
 struct ListArgs {
-    const double *x, *y, *z, *h;       // sorted
+    const double2 *p0, *p1;            // sorted (x, y), (z, h)
     const TileDesc* tiles;
-    const uint32_t* ntiles;
-    uint2* lists;                      // [tile][warp][LIST_CAP/4][32] x 4 u16
+    unsigned long long* ctr;           // CTR_*
+    uint2* pool;
+    unsigned long long pool_cap;       // uint2 units
+    uint2* winfo;                      // [tile][warp]: (pool offset, rounds)
     uint32_t* lcount;                  // [tile][TILE_T]: n_gather | n_sym << 16
+    uint32_t* tflags;                  // [tile]
     uint8_t* fast;                     // [n] sorted order: 1 = served by the tiled kernels
-    uint32_t* tile_ok;                 // [tile]
+    const double* hglob;
     uint32_t* status;
-    int64_t n;
 };
 
-constexpr size_t BL_OFF_F4 = 0;                                             // float4 [CMAX]
-constexpr size_t BL_OFF_XYZH = BL_OFF_F4 + sizeof(float4) * TILE_CMAX;      // double [4][CMAX]
-constexpr size_t BL_OFF_L2 = 0;                                             // second list buffer aliases f4 + xyzh
-constexpr size_t BL_OFF_GIDX = BL_OFF_XYZH + sizeof(double) * 4 * TILE_CMAX;// uint32 [CMAX]
-constexpr size_t BL_OFF_L = BL_OFF_GIDX + sizeof(uint32_t) * TILE_CMAX;     // uint16 [LIST_CAPP][TILE_T]
-constexpr size_t BL_OFF_COL = BL_OFF_L + sizeof(uint16_t) * LIST_CAPP * TILE_T;   // uint16 [MAXR][BXMAX + 3]
-constexpr size_t BL_SMEM = BL_OFF_COL + sizeof(uint16_t) * TILE_MAXR * (TILE_BXMAX + 4);
-static_assert(sizeof(uint16_t) * LIST_CAP * TILE_T <= BL_OFF_GIDX, "second list buffer must fit under gidx");
-static_assert(BL_SMEM + sizeof(TileS) + 64 <= 227 * 1024, "list builder shared memory");
+constexpr int COLW = TILE_BXMAX + 4;
+constexpr size_t BL_OFF_F4 = 0;                                                        // float4 [CMAXP]
+constexpr size_t BL_OFF_B = BL_OFF_F4 + sizeof(float4) * TILE_CMAXP;                   // u16 [4][LIST_BC][TILE_THREADS]
+constexpr size_t BL_OFF_COL = BL_OFF_B + sizeof(uint16_t) * 4 * LIST_BC * TILE_THREADS;// u16 [MAXR][COLW]
+constexpr size_t BL_SMEM = BL_OFF_COL + sizeof(uint16_t) * TILE_MAXR * COLW;
+static_assert(BL_SMEM + sizeof(TileS) + 256 <= 227 * 1024, "list builder shared memory");
 
-__global__ void __launch_bounds__(TILE_T, 1)
+__device__ __forceinline__ uint32_t get8(unsigned long long x, int b) { return (uint32_t)(x >> (8 * b)) & 0xFFu; }
+
+__global__ void __launch_bounds__(TILE_THREADS, 1)
 k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
     extern __shared__ __align__(16) unsigned char smem[];
     __shared__ TileS S;
-    __shared__ int s_bad;
+    __shared__ int s_bad, s_nonuni;
     float4* f4 = reinterpret_cast<float4*>(smem + BL_OFF_F4);
-    double* sx = reinterpret_cast<double*>(smem + BL_OFF_XYZH);
-    double* sy = sx + TILE_CMAX;
-    double* sz = sy + TILE_CMAX;
-    double* sh = sz + TILE_CMAX;
-    uint32_t* gidx = reinterpret_cast<uint32_t*>(smem + BL_OFF_GIDX);
-    uint16_t* L = reinterpret_cast<uint16_t*>(smem + BL_OFF_L);        // [k][tid]
-    uint16_t* L2 = reinterpret_cast<uint16_t*>(smem + BL_OFF_L2);      // [k][tid], valid after the exact phase
-    uint16_t* colofs = reinterpret_cast<uint16_t*>(smem + BL_OFF_COL); // [range][TILE_BXMAX + 4]
+    uint16_t* B = reinterpret_cast<uint16_t*>(smem + BL_OFF_B);        // [(b * LIST_BC + k) * TILE_THREADS + tid]
+    uint16_t* colofs = reinterpret_cast<uint16_t*>(smem + BL_OFF_COL); // [range][COLW]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const uint32_t ntiles = *A.ntiles;
+    const int u = tid & 1, tgt = tid >> 1, j = lane & 7;
+    const uint32_t ntiles = (uint32_t)A.ctr[CTR_NTILES];
+    const float Rmax = 2.0f * (float)A.hglob[1] * 1.000001f;
 
     for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
         const TileDesc td = A.tiles[tile];
         __syncthreads();                                                // previous tile done with smem
-        if (tid == 0) s_bad = 0;
+        if (tid == 0) { s_bad = 0; s_nonuni = 0; }
         tile_setup(td, g, ct, S);
-        const uint32_t ncand = S.ncand;
         const int ncolv = td.cxb - td.cxa + 3;                          // virtual columns 0 .. ncolv-1
         // tile origin (centre of the tile's cell block) for the fp32 relative coordinates
         const double ox = g.lo[0] + (0.5 * (td.cxa + td.cxb + 1)) / g.inv[0];
@@ -140,53 +175,54 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
         // bound on the absolute error of an fp32 relative coordinate difference: 2 roundings of magnitude <= ext
         const float ext = (float)fmax(fmax((0.5 * ncolv + 0.5) / g.inv[0], 2.5 / g.inv[1]), 2.5 / g.inv[2]);
         const float E = ext * 2.4e-7f;                                  // 4 * 2^-24 * ext
+        const float Am = 4.4f * Rmax * E + 5.0f * E * E;
 
         // ---- per-range column offsets (slot of the first particle of each column, relative to r_base)
-        for (int w = tid; w < (int)S.nranges * (TILE_BXMAX + 4); w += TILE_T) {
-            const int q = w / (TILE_BXMAX + 4), j = w % (TILE_BXMAX + 4);
+        for (int w = tid; w < (int)S.nranges * COLW; w += TILE_THREADS) {
+            const int q = w / COLW, jj = w % COLW;
             const int4 ge = S.r_geo[q];
-            if (j <= ge.y) {
-                const uint32_t gs = (j < ge.y) ? ct.cell_start[ge.w + j] : S.r_vend[q];
-                colofs[q * (TILE_BXMAX + 4) + j] = (uint16_t)(gs - S.r_start[q]);
+            if (jj <= ge.y) {
+                const uint32_t gs = (jj < ge.y) ? ct.cell_start[ge.w + jj] : S.r_vend[q];
+                colofs[q * COLW + jj] = (uint16_t)(gs - S.r_vstart[q]);
             }
         }
-        // ---- stage the candidates
-        for (uint32_t s = tid; s < ncand; s += TILE_T) {
-            const int q = tile_slot_range(S, s);
-            const uint32_t gi = S.r_start[q] + (s - S.r_base[q]);
-            const bool valid = gi >= S.r_vstart[q] && gi < S.r_vend[q];
-            if (valid) {
-                const double xb = A.x[gi], yb = A.y[gi], zb = A.z[gi], hb = A.h[gi];
-                sx[s] = xb; sy[s] = yb; sz[s] = zb; sh[s] = hb;
-                gidx[s] = gi | ((uint32_t)q << 27);                     // n < 2^27 guaranteed by the launcher
-                // image position next to the tile: x_b - shift*L
-                const float fx = (float)((xb - S.r_shift[q][0] * g.L[0]) - ox);
-                const float fy = (float)((yb - S.r_shift[q][1] * g.L[1]) - oy);
-                const float fz = (float)((zb - S.r_shift[q][2] * g.L[2]) - oz);
-                const float Rb = 2.0f * (float)hb * 1.000001f;
-                f4[s] = make_float4(fx, fy, fz, Rb * Rb * 1.00001f + 4.4f * Rb * E + 5.0f * E * E);
-            } else {
-                gidx[s] = 0xFFFFFFFFu;
-                f4[s] = make_float4(3.0e18f, 3.0e18f, 3.0e18f, 0.0f);
+        // ---- stage the candidates: one warp per range
+        {
+            const unsigned long long h0 = (unsigned long long)__double_as_longlong(A.p1[S.r_vstart[0]].y);
+            bool nonuni = false;
+            for (int q = warp; q < (int)S.nranges; q += TILE_WARPS) {
+                const uint32_t vs = S.r_vstart[q], len = S.r_vend[q] - vs, base = S.r_base[q];
+                const double shx = S.r_shift[q][0] * g.L[0], shy = S.r_shift[q][1] * g.L[1], shz = S.r_shift[q][2] * g.L[2];
+                for (uint32_t k = lane; k < len; k += 32) {
+                    const double2 xy = A.p0[vs + k], zh = A.p1[vs + k];
+                    // image position next to the tile: x_b - shift*L
+                    const float fx = (float)((xy.x - shx) - ox);
+                    const float fy = (float)((xy.y - shy) - oy);
+                    const float fz = (float)((zh.x - shz) - oz);
+                    const float Rb = 2.0f * (float)zh.y;
+                    f4[base + k] = make_float4(fx, fy, fz, Rb * Rb);
+                    nonuni |= (unsigned long long)__double_as_longlong(zh.y) != h0;
+                }
             }
+            if (nonuni) s_nonuni = 1;
         }
         // ---- this thread's target
-        const bool active = tid < (int)td.nt;
+        const bool active = tgt < (int)td.nt;
         uint32_t i = 0;
         double xa = 0, ya = 0, za = 0, ha = 0;
         int tcol = 0, trow = 0;
         if (active) {
-            const uint32_t p = td.skip + (uint32_t)tid;
-            int lo = 0, hi = (int)S.ncells;
-            while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (S.c_pre[mid] <= p) lo = mid; else hi = mid; }
-            i = S.c_first[lo] + (p - S.c_pre[lo]);
+            int e;
+            i = tile_target(td, S, tgt, &e);
             const int nrows = td.nyr * td.nzr;
-            tcol = lo / nrows; trow = lo % nrows;
-            xa = A.x[i]; ya = A.y[i]; za = A.z[i]; ha = A.h[i];
+            tcol = e / nrows; trow = e % nrows;
+            const double2 xy = A.p0[i], zh = A.p1[i];
+            xa = xy.x; ya = xy.y; za = zh.x; ha = zh.y;
         }
         const float fax = (float)(xa - ox), fay = (float)(ya - oy), faz = (float)(za - oz);
-        const float Ra = 2.0f * (float)ha * 1.000001f;
-        const float thr_a = active ? Ra * Ra * 1.00001f + 4.4f * Ra * E + 5.0f * E * E : -1.0f;
+        const float Ra = 2.0f * (float)ha;
+        const float Ta = active ? Ra * Ra : -1.0f;
+        const float Ta_hi = fmaf(Ta, 1.00001f, Am), Ta_lo = fmaf(Ta, 0.99999f, -Am);
         // warp window in virtual columns / candidate rows
         int cmin = active ? tcol : 1 << 20, cmax = active ? tcol : -1;
         int ymin = active ? trow % td.nyr : 4, ymax = active ? trow % td.nyr : -1;
@@ -199,8 +235,10 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
         }
         __syncthreads();
 
-        // ---- phase 1: fp32 prefilter, all lanes test the same candidate (shared-memory broadcast)
-        uint32_t cnt = 0;
+        // ---- scan: fp32 prefilter, the even (odd) thread of a target tests the even (odd) slots; all lanes of the
+        //      same parity read the same candidate (shared-memory broadcast).  Hits go to the (thread, bank) buckets.
+        uint32_t cnt = 0, ng = 0;                                       // cnt: 4 x 8-bit bucket fills (bank = 2 b + u)
+        bool ovf = false, coinc = false;
         if (cmax >= 0) {
             const int wv_lo = cmin, wv_hi = cmax + 2;                   // virtual columns [tcol, tcol + 2] around each target
             for (int q = 0; q < (int)S.nranges; ++q) {
@@ -209,116 +247,154 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
                 const int4 ge = S.r_geo[q];
                 const int jlo = max(0, min(ge.y, wv_lo - ge.z)), jhi = max(0, min(ge.y, wv_hi + 1 - ge.z));
                 if (jhi <= jlo) continue;
-                const uint32_t sa = S.r_base[q] + colofs[q * (TILE_BXMAX + 4) + jlo];
-                const uint32_t sb = S.r_base[q] + colofs[q * (TILE_BXMAX + 4) + jhi];
+                const uint32_t sa = S.r_base[q] + colofs[q * COLW + jlo];
+                const uint32_t sb = S.r_base[q] + colofs[q * COLW + jhi];
 #pragma unroll 4
-                for (uint32_t s = sa; s < sb; ++s) {
+                for (uint32_t s = sa + ((sa ^ (uint32_t)u) & 1u); s < sb; s += 2) {
                     const float4 c = f4[s];
                     const float dx = fax - c.x, dy = fay - c.y, dz = faz - c.z;
                     const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                    if (r2 < fmaxf(thr_a, c.w)) {
-                        if (cnt < (uint32_t)LIST_CAPP) L[cnt * TILE_T + tid] = (uint16_t)s;
-                        ++cnt;
+                    const float Tm = fmaxf(Ta, c.w);
+                    if (r2 < fmaf(Tm, 1.00001f, Am)) {
+                        bool in_s, in_g;
+                        if (r2 < fmaf(Tm, 0.99999f, -Am) && (r2 < Ta_lo || r2 >= Ta_hi) && r2 > 0.0f) {
+                            in_s = active; in_g = active && r2 < Ta_lo;
+                        } else {                                        // near a support boundary or r = 0: exact predicate (O2/A12)
+                            const uint32_t gi = S.r_vstart[q] + (s - S.r_base[q]);
+                            const double2 xy = A.p0[gi], zh = A.p1[gi];
+                            const double ex = min_image(__dsub_rn(xa, xy.x), g.per[0], g.L[0], g.halfL[0]);
+                            const double ey = min_image(__dsub_rn(ya, xy.y), g.per[1], g.L[1], g.halfL[1]);
+                            const double ez = min_image(__dsub_rn(za, zh.x), g.per[2], g.L[2], g.halfL[2]);
+                            const double e2 = r2_exact(ex, ey, ez);
+                            in_s = active && gi != i && e2 < support2(fmax(ha, zh.y));
+                            in_g = in_s && e2 < support2(ha);
+                            if (in_s && !(e2 > 0.0)) coinc = true;      // coincident particles: left to the general kernels (A11)
+                        }
+                        if (in_s) {
+                            const int b = (int)(s >> 1) & 3;
+                            const uint32_t k = (cnt >> (8 * b)) & 0xFFu;
+                            if (k < (uint32_t)LIST_BC) B[(b * LIST_BC + k) * TILE_THREADS + tid] = (uint16_t)s;
+                            else ovf = true;
+                            cnt += (k < (uint32_t)LIST_BC) ? (1u << (8 * b)) : 0u;
+                            ng += in_g ? 1u : 0u;
+                        }
                     }
                 }
             }
         }
-        if (cnt > (uint32_t)LIST_CAPP) s_bad = 1;
-        // ---- phase 2: exact predicate (contract O2/A12) on the survivors, compacted in place
-        const double sup_a = support2(ha);
-        uint32_t m = 0, ng = 0;
-        if (active) {
-            const uint32_t nn = min(cnt, (uint32_t)LIST_CAPP);
-            const bool anysh = S.any_shift != 0;
-            for (uint32_t k = 0; k < nn; ++k) {
-                const uint32_t s = L[k * TILE_T + tid];
-                const uint32_t gq = gidx[s];
-                if ((gq & 0x07FFFFFFu) == i) continue;                  // self
-                double dx = __dsub_rn(xa, sx[s]), dy = __dsub_rn(ya, sy[s]), dz = __dsub_rn(za, sz[s]);
-                if (anysh) {
-                    dx = min_image(dx, g.per[0], g.L[0], g.halfL[0]);
-                    dy = min_image(dy, g.per[1], g.L[1], g.halfL[1]);
-                    dz = min_image(dz, g.per[2], g.L[2], g.halfL[2]);
-                }
-                const double r2 = r2_exact(dx, dy, dz);
-                const double hb = sh[s];
-                if (r2 < support2(fmax(ha, hb))) {
-                    const bool ing = r2 < sup_a;
-                    L[m * TILE_T + tid] = (uint16_t)(s | (ing ? LIST_GATHER_BIT : 0));
-                    ++m; ng += ing ? 1u : 0u;
-                }
-            }
-            if (m > (uint32_t)LIST_CAP) s_bad = 1;
+        if (ovf || coinc) s_bad = 1;
+        // ---- split every bank bucket of the target between its two threads (alternate entries)
+        const uint32_t cnt_o = __shfl_xor_sync(0xFFFFFFFFu, cnt, 1);
+        ng += __shfl_xor_sync(0xFFFFFFFFu, ng, 1);
+        unsigned long long cu = 0;                                      // 8 x 8-bit: entries of bank beta that are mine
+        uint32_t n_lane = 0, nsym = 0;
+#pragma unroll
+        for (int beta = 0; beta < 8; ++beta) {
+            const uint32_t cb = (((beta & 1) == u ? cnt : cnt_o) >> (8 * (beta >> 1))) & 0xFFu;
+            const uint32_t f = (uint32_t)(u + beta) & 1u;
+            const uint32_t mine = (cb + 1u - f) >> 1;
+            cu |= (unsigned long long)mine << (8 * beta);
+            n_lane += mine; nsym += cb;
         }
-        __syncthreads();                                                // coordinates no longer needed: L2 may alias them
+        uint32_t R = n_lane;
+#pragma unroll
+        for (int o = 16; o; o >>= 1) R = max(R, __shfl_xor_sync(0xFFFFFFFFu, R, o));
+        R = (R + 3u) & ~3u;
+        unsigned long long off = 0;
+        if (lane == 0) {
+            if (R > (uint32_t)LIST_RMAX) s_bad = 1;
+            else if (R > 0) {
+                const unsigned long long need = (unsigned long long)(R / 4) * 32;
+                off = atomicAdd(&A.ctr[CTR_POOL], need);
+                if (off + need > A.pool_cap) { s_bad = 1; atomicOr(A.status, (uint32_t)SPRAY_DEV_LIST_OVERFLOW); }
+            }
+        }
+        off = __shfl_sync(0xFFFFFFFFu, off, 0);
+        __syncthreads();
         const bool bad = s_bad != 0;
         if (!bad) {
-            // ---- phase 3: gather neighbours first, then the symmetric-only ones
-            uint32_t pos = 0;
-            for (uint32_t k = 0; k < m; ++k) { const uint16_t e = L[k * TILE_T + tid]; if (e & LIST_GATHER_BIT) L2[(pos++) * TILE_T + tid] = e & 0x7FFFu; }
-            for (uint32_t k = 0; k < m; ++k) { const uint16_t e = L[k * TILE_T + tid]; if (!(e & LIST_GATHER_BIT)) L2[(pos++) * TILE_T + tid] = e; }
-            // pad to a multiple of 4 with slot 0 (never evaluated: the sweeps stop at the counts)
-            for (uint32_t k = m; k < ((m + 3u) & ~3u); ++k) L2[k * TILE_T + tid] = 0;
-            uint32_t mx = m;
+            // ---- emit my half-list in scheduled order (see the header): phases of R/8 rounds, bank (j + t) & 7
+            unsigned long long own = 0, ovr = 0;
+            uint32_t ovtot = 0;
 #pragma unroll
-            for (int o = 16; o; o >>= 1) mx = max(mx, __shfl_xor_sync(0xFFFFFFFFu, mx, o));
-            uint2* blk = A.lists + list_block_u2(tile, warp);
-            for (uint32_t k4 = 0; k4 * 4 < mx; ++k4) {
-                uint2 v = make_uint2(0u, 0u);
-                if (k4 * 4 < m) {
-                    const uint32_t e0 = L2[(k4 * 4 + 0) * TILE_T + tid], e1 = L2[(k4 * 4 + 1) * TILE_T + tid];
-                    const uint32_t e2 = L2[(k4 * 4 + 2) * TILE_T + tid], e3 = L2[(k4 * 4 + 3) * TILE_T + tid];
-                    v = make_uint2(e0 | (e1 << 16), e2 | (e3 << 16));
-                }
-                blk[k4 * 32 + lane] = v;
+            for (int beta = 0; beta < 8; ++beta) {
+                const int t = (beta - j) & 7;
+                const uint32_t cap = (((uint32_t)(t + 1) * R) >> 3) - (((uint32_t)t * R) >> 3);
+                const uint32_t c = get8(cu, beta);
+                const uint32_t o = c > cap ? c - cap : 0u;
+                own |= (unsigned long long)(c - o) << (8 * beta);
+                ovr |= (unsigned long long)o << (8 * beta);
+                ovtot += o;
             }
-            A.lcount[(size_t)tile * TILE_T + tid] = active ? (ng | (m << 16)) : 0u;
-            if (active) A.fast[i] = 1;
+            uint2* blk = A.pool + off;
+            const int pairbase = tid & ~1;
+            int t = 0, beta = j;
+            uint32_t bnd = R >> 3, own_left = get8(own, beta), front = 0, w0 = 0, w1 = 0;
+            for (uint32_t r = 0; r < R; ++r) {
+                while (r >= bnd && t < 7) { ++t; beta = (beta + 1) & 7; bnd = ((uint32_t)(t + 1) * R) >> 3; own_left = get8(own, beta); front = 0; }
+                uint32_t item;
+                if (own_left) {
+                    const uint32_t e = ((uint32_t)(u + beta) & 1u) + 2u * front;
+                    item = B[((beta >> 1) * LIST_BC + e) * TILE_THREADS + pairbase + (beta & 1)];
+                    ++front; --own_left;
+                } else if (ovtot) {
+                    int b2 = beta;
+                    do { b2 = (b2 + 1) & 7; } while (!get8(ovr, b2));
+                    const uint32_t k = get8(cu, b2) - get8(ovr, b2);
+                    ovr -= 1ull << (8 * b2); --ovtot;
+                    const uint32_t e = ((uint32_t)(u + b2) & 1u) + 2u * k;
+                    item = B[((b2 >> 1) * LIST_BC + e) * TILE_THREADS + pairbase + (b2 & 1)];
+                } else {
+                    item = (uint32_t)(TILE_CMAX + beta);                // dummy slot of this phase's bank
+                }
+                switch (r & 3u) {
+                    case 0: w0 = item; break;
+                    case 1: w0 |= item << 16; break;
+                    case 2: w1 = item; break;
+                    default: w1 |= item << 16; blk[(size_t)(r >> 2) * 32 + lane] = make_uint2(w0, w1); break;
+                }
+            }
+            if (u == 0) A.lcount[(size_t)tile * TILE_T + tgt] = active ? (ng | (nsym << 16)) : 0u;
+            if (active && u == 0) A.fast[i] = 1;
+            if (lane == 0) A.winfo[(size_t)tile * TILE_WARPS + warp] = make_uint2((uint32_t)off, R);
         }
-        if (tid == 0) A.tile_ok[tile] = bad ? 0u : 1u;
+        if (tid == 0) {
+            A.tflags[tile] = bad ? 0u : (TILE_FLAG_OK | (s_nonuni ? 0u : TILE_FLAG_UNIH));
+            if (!bad) atomicAdd(&A.ctr[CTR_NFAST], (unsigned long long)td.nt);
+        }
     }
 }
 
-__global__ void k_count_fast(const uint8_t* __restrict__ fast, int64_t n, unsigned long long* out) {
-    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    const uint32_t b = __ballot_sync(0xFFFFFFFFu, i < n && fast[i]);
-    if ((threadIdx.x & 31) == 0 && b) atomicAdd(out, (unsigned long long)__popc(b));
-}
-
-// ------------------------------------------------------------------------------------------- launchers
-cudaError_t launch_count_fast(Ctx* c, cudaStream_t st) {
-    unsigned long long* out = reinterpret_cast<unsigned long long*>(c->hglob + 2);
-    cudaError_t e = cudaMemsetAsync(out, 0, sizeof(unsigned long long), st);
-    if (e != cudaSuccess) return e;
-    k_count_fast<<<(unsigned)((c->n + 255) / 256), 256, 0, st>>>(c->tl.fast, c->n, out);
-    return cudaGetLastError();
-}
-
+// ------------------------------------------------------------------------------------------- launcher
 cudaError_t launch_build_tiles(Ctx* c, cudaStream_t st) {
     Tiled& t = c->tl;
     t.enabled = false;
     if (c->n == 0 || !t.tiles) return cudaSuccess;
     // host-side guards: small periodic grids (a candidate row would appear twice), index width
     const spray_grid_t& gr = c->grid;
-    if (c->n >= (1ll << 27)) return cudaSuccess;
+    if (c->n >= (1ll << 31)) return cudaSuccess;
     if (gr.periodic[0] && gr.ncell[0] < 3) return cudaSuccess;
     if (gr.periodic[1] && gr.ncell[1] < 4) return cudaSuccess;
     if (gr.periodic[2] && gr.ncell[2] < 4) return cudaSuccess;
     if (gr.ncell[0] > 32000 || gr.ncell[1] > 32000 || gr.ncell[2] > 32000) return cudaSuccess;
+    const int64_t nb = (int64_t)((gr.ncell[1] + 1) / 2) * ((gr.ncell[2] + 1) / 2);
+    if (nb > t.bundle_cap) return cudaSuccess;
     cudaError_t e;
-    if ((e = cudaMemsetAsync(t.ntiles, 0, sizeof(uint32_t), st)) != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(t.ctr, 0, sizeof(unsigned long long) * CTR_COUNT, st)) != cudaSuccess) return e;
     if ((e = cudaMemsetAsync(t.fast, 0, (size_t)c->n, st)) != cudaSuccess) return e;
     CellTable ct{c->cell_start, c->cell_end};
-    const int nb = ((gr.ncell[1] + 1) / 2) * ((gr.ncell[2] + 1) / 2);
-    k_make_tiles<<<(nb + 63) / 64, 64, 0, st>>>(c->dg, ct, c->hglob, t.tiles, t.ntiles, (uint32_t)t.tile_cap, c->dev_status);
-    k_clamp_ntiles<<<1, 1, 0, st>>>(t.ntiles, (uint32_t)t.tile_cap);
+    const int blocks = (int)((nb * 32 + 255) / 256);
+    k_make_tiles<false><<<blocks, 256, 0, st>>>(c->dg, ct, c->hglob, t.bcount, t.tiles, (uint32_t)t.tile_cap, t.ctr);
+    if ((e = launch_excl_scan_u32(c, t.bcount, nb, t.bcount + t.bundle_cap, st)) != cudaSuccess) return e;
+    k_make_tiles<true><<<blocks, 256, 0, st>>>(c->dg, ct, c->hglob, t.bcount, t.tiles, (uint32_t)t.tile_cap, t.ctr);
     static bool attr_done = false;
     if (!attr_done) {
         if ((e = cudaFuncSetAttribute(k_build_lists, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BL_SMEM)) != cudaSuccess) return e;
         attr_done = true;
     }
-    ListArgs A{c->s.x, c->s.y, c->s.z, c->s.h, t.tiles, t.ntiles, t.lists, t.lcount, t.fast, t.tile_ok, c->dev_status, c->n};
-    k_build_lists<<<t.grid, TILE_T, BL_SMEM, st>>>(c->dg, ct, A);
+    ListArgs A{c->pk.p0, c->pk.p1, t.tiles, t.ctr, t.pool, (unsigned long long)t.pool_cap, t.winfo, t.lcount, t.tflags, t.fast,
+               c->hglob, c->dev_status};
+    k_build_lists<<<t.sms, TILE_THREADS, BL_SMEM, st>>>(c->dg, ct, A);
     c->launches += 3;
     t.enabled = true;
     return cudaGetLastError();

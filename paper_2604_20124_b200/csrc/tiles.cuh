@@ -6,27 +6,35 @@
 // (for cx: for row: particles of the cell), plus the candidate particles of every cell within one cell of the
 // tile's cells: (nyr + 2) x (nzr + 2) rows, x-range [cxa - 1, cxb + 1].  Each candidate row contributes one
 // contiguous range of sorted slots (two when the x-range wraps in a periodic box); the ranges are laid out
-// back-to-back in shared memory, each starting on an even global index (16-byte alignment for bulk copies), and a
-// candidate is addressed by its SLOT in that layout.  The slot numbering is a pure function of (TileDesc, cell
-// table), so the neighbour lists built once per spray_build_cells (u16 slots) stay valid for every later sweep.
+// back-to-back in shared memory and a candidate is addressed by its SLOT in that layout.  The slot numbering is a
+// pure function of (TileDesc, cell table), so the neighbour lists built once per spray_build_cells (u16 slots)
+// stay valid for every later sweep.
 //
 // Valid only when every neighbour of a target lies within one cell: 2 * h_max <= min cell edge (checked on the
 // device when the tiles are made; otherwise no tile is emitted and the general one-thread-per-particle kernels
 // serve every particle).
+//
+// Threads: TILE_TPT = 2 threads per target (thread tid serves target tid >> 1 with the half-list tid & 1), so a
+// warp holds 16 targets and an aligned group of 8 lanes (one 128-byte shared-memory wavefront of 16-byte loads)
+// holds 4 targets x 2 half-lists.  The lists are SCHEDULED per lane (tiles.cu) so that in most rounds the 8 lanes
+// of such a group read 8 different 16-byte banks.
 #pragma once
 #include "common.cuh"
 
 namespace spray {
 
-constexpr int TILE_T = 256;          // threads per CTA = max targets per tile
-constexpr int TILE_WARPS = TILE_T / 32;
-constexpr int TILE_CMAX = 2304;      // max candidate slots per tile (hydro stages 11 fp64 fields: 11*8*2304 = 198 KB)
+constexpr int TILE_T = 256;          // max targets per tile
+constexpr int TILE_TPT = 2;          // threads per target
+constexpr int TILE_THREADS = TILE_T * TILE_TPT;
+constexpr int TILE_WARPS = TILE_THREADS / 32;
+constexpr int TILE_CMAX = 2232;      // max candidate slots per tile
+constexpr int TILE_NDUMMY = 8;       // dummy slots (one per 16-byte bank) appended after the candidates
+constexpr int TILE_CMAXP = TILE_CMAX + TILE_NDUMMY;   // 2240: multiple of 8, so slot & 7 is the bank of a 16-byte record
 constexpr int TILE_MAXR = 32;        // candidate ranges: 4 x 4 rows x (1 or 2 pieces, at most 16 rows wrap)
 constexpr int TILE_BXMAX = 24;       // max columns (cells along x) of a tile
 constexpr int TILE_MAXCELL = 4 * TILE_BXMAX;
-constexpr int LIST_CAP = 128;        // neighbour-list rows per target (global storage); longer lists -> general kernel
-constexpr int LIST_CAPP = 168;       // provisional (fp32-prefiltered) rows per target in shared memory
-constexpr uint16_t LIST_GATHER_BIT = 0x8000u;
+constexpr int LIST_BC = 24;          // builder: capacity of one (thread, bank) bucket
+constexpr int LIST_RMAX = 160;       // max rounds of a warp's schedule (longer -> tile served by the general kernels)
 
 struct TileDesc {                    // 24 bytes
     int16_t y0, z0;                  // first row of the bundle
@@ -38,6 +46,9 @@ struct TileDesc {                    // 24 bytes
     uint32_t pad2;
 };
 
+constexpr uint32_t TILE_FLAG_OK = 1u;        // lists were built: the tiled kernels serve this tile
+constexpr uint32_t TILE_FLAG_UNIH = 2u;      // every target and candidate of the tile has the same h (bitwise)
+
 struct CellTable {
     const uint32_t* cell_start;
     const uint32_t* cell_end;
@@ -46,14 +57,12 @@ struct CellTable {
 // Per-CTA tile tables in shared memory (filled by tile_setup)
 struct TileS {
     // candidate ranges
-    uint32_t r_start[TILE_MAXR];     // even-aligned first global slot copied
-    uint32_t r_vstart[TILE_MAXR];    // first valid global slot
-    uint32_t r_vend[TILE_MAXR];      // one past the last valid global slot
-    uint32_t r_base[TILE_MAXR + 1];  // first shared-memory slot of the range (exclusive scan of padded lengths)
+    uint32_t r_vstart[TILE_MAXR];    // first global slot of the range
+    uint32_t r_vend[TILE_MAXR];      // one past the last global slot
+    uint32_t r_base[TILE_MAXR + 1];  // first shared-memory slot of the range (exclusive scan of the lengths)
     int8_t r_shift[TILE_MAXR][4];    // [0..2] periodic image: dx = (x_a - x_b) + shift * L (-1, 0, +1); [3] candidate row id
     int4 r_geo[TILE_MAXR];           // (first cell column, number of columns, virtual column of the first, first cell id)
     uint32_t nranges, ncand;
-    int any_shift;
     // targets
     uint32_t c_first[TILE_MAXCELL];  // global slot of the first particle of cell e (column-major enumeration)
     uint32_t c_pre[TILE_MAXCELL + 1];// exclusive scan of the cell counts
@@ -66,22 +75,22 @@ __device__ __forceinline__ uint32_t cell_id(const DevGrid& g, int cx, int cy, in
 
 // Candidate range (row, piece) of a tile: row = rz * 4 + ry enumerates the (nyr + 2) x (nzr + 2) candidate rows,
 // piece = 0/1 the two parts of an x-range that wraps in a periodic box.  Returns false when the range does not
-// exist or is empty.  [vs, ve) = valid global slots, (xlo, ncol) = its first cell column (actual index) and number
+// exist or is empty.  [vs, ve) = global slots, (xlo, ncol) = its first cell column (actual index) and number
 // of columns, vlo = position of that column in the tile's virtual column axis (0 = column cxa - 1),
 // sh = periodic image so that dx = (x_a - x_b) + sh * L.
 struct RangeGeo { uint32_t vs, ve; int xlo, ncol, vlo, cy, cz; int sh[3]; };
-__device__ __forceinline__ bool tile_range(const TileDesc& td, const DevGrid& g, const CellTable& ct, int row, int piece,
-                                           RangeGeo& R) {
-    const int nyc = td.nyr + 2, nzc = td.nzr + 2;
+__device__ __forceinline__ bool tile_range(int y0, int z0, int nyr, int nzr, int cxa, int cxb, const DevGrid& g,
+                                           const CellTable& ct, int row, int piece, RangeGeo& R) {
+    const int nyc = nyr + 2, nzc = nzr + 2;
     const int ry = row % 4, rz = row / 4;
     if (ry >= nyc || rz >= nzc) return false;
-    int cy = td.y0 - 1 + ry, cz = td.z0 - 1 + rz;
+    int cy = y0 - 1 + ry, cz = z0 - 1 + rz;
     int sy = 0, sz = 0, sx = 0;
     if (cy < 0) { if (g.per[1]) { cy += g.nc[1]; sy = 1; } else return false; }
     else if (cy >= g.nc[1]) { if (g.per[1]) { cy -= g.nc[1]; sy = -1; } else return false; }
     if (cz < 0) { if (g.per[2]) { cz += g.nc[2]; sz = 1; } else return false; }
     else if (cz >= g.nc[2]) { if (g.per[2]) { cz -= g.nc[2]; sz = -1; } else return false; }
-    int xlo = td.cxa - 1, xhi = td.cxb + 1, vlo = 0;
+    int xlo = cxa - 1, xhi = cxb + 1, vlo = 0;
     const int nx = g.nc[0];
     if (g.per[0]) {
         if (xlo < 0) {               // piece 0 = wrapped tail of the row, piece 1 = [0, xhi]
@@ -101,17 +110,19 @@ __device__ __forceinline__ bool tile_range(const TileDesc& td, const DevGrid& g,
     R.sh[0] = sx; R.sh[1] = sy; R.sh[2] = sz;
     return R.ve > R.vs;
 }
-__device__ __forceinline__ uint32_t range_padded_len(uint32_t vs, uint32_t ve) { return ((ve + 1u) & ~1u) - (vs & ~1u); }
+__device__ __forceinline__ bool tile_range(const TileDesc& td, const DevGrid& g, const CellTable& ct, int row, int piece,
+                                           RangeGeo& R) {
+    return tile_range(td.y0, td.z0, td.nyr, td.nzr, td.cxa, td.cxb, g, ct, row, piece, R);
+}
 
-// Fills S.  Must be called by all threads of the CTA; ends with __syncthreads().
+// Fills S.  Must be called by all threads of the CTA (blockDim.x >= 32 + TILE_MAXCELL); ends with __syncthreads().
 __device__ __forceinline__ void tile_setup(const TileDesc& td, const DevGrid& g, const CellTable& ct, TileS& S) {
     const int tid = threadIdx.x;
     if (tid < 32) {
         RangeGeo R;
         const bool valid = tile_range(td, g, ct, tid >> 1, tid & 1, R);
-        const uint32_t st = valid ? (R.vs & ~1u) : 0u;
-        const uint32_t len = valid ? range_padded_len(R.vs, R.ve) : 0u;
-        // compact the valid ranges to the front, keeping order (ballot + popc), and scan the padded lengths
+        const uint32_t len = valid ? R.ve - R.vs : 0u;
+        // compact the valid ranges to the front, keeping order (ballot + popc), and scan the lengths
         const uint32_t mask = __ballot_sync(0xFFFFFFFFu, valid);
         const int pos = __popc(mask & ((1u << tid) - 1u));
         uint32_t incl = len;
@@ -121,16 +132,13 @@ __device__ __forceinline__ void tile_setup(const TileDesc& td, const DevGrid& g,
             if (tid >= o) incl += v;
         }
         if (valid) {
-            S.r_start[pos] = st; S.r_vstart[pos] = R.vs; S.r_vend[pos] = R.ve; S.r_base[pos] = incl - len;
+            S.r_vstart[pos] = R.vs; S.r_vend[pos] = R.ve; S.r_base[pos] = incl - len;
             S.r_shift[pos][0] = (int8_t)R.sh[0]; S.r_shift[pos][1] = (int8_t)R.sh[1]; S.r_shift[pos][2] = (int8_t)R.sh[2];
             S.r_shift[pos][3] = (int8_t)(tid >> 1);                    // candidate row id (rz * 4 + ry)
             S.r_geo[pos] = make_int4(R.xlo, R.ncol, R.vlo, (int)cell_id(g, R.xlo, R.cy, R.cz));
         }
         const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31);
-        const uint32_t anys = __ballot_sync(0xFFFFFFFFu, valid && (R.sh[0] | R.sh[1] | R.sh[2]));
-        if (tid == 0) {
-            S.nranges = __popc(mask); S.ncand = total; S.r_base[__popc(mask)] = total; S.any_shift = anys != 0;
-        }
+        if (tid == 0) { S.nranges = __popc(mask); S.ncand = total; S.r_base[__popc(mask)] = total; }
     }
     // target cells, column-major: e = (cx - cxa) * nrows + r, r = rz * nyr + ry
     const int nrows = td.nyr * td.nzr;
@@ -164,31 +172,16 @@ __device__ __forceinline__ void tile_setup(const TileDesc& td, const DevGrid& g,
     __syncthreads();
 }
 
-// global sorted slot of target t of the tile (t < td.nt)
-__device__ __forceinline__ uint32_t tile_target(const TileDesc& td, const TileS& S, int t) {
+// global sorted slot of target t of the tile (t < td.nt); *cell_e = index of its cell in the column-major enumeration
+__device__ __forceinline__ uint32_t tile_target(const TileDesc& td, const TileS& S, int t, int* cell_e = nullptr) {
     const uint32_t p = td.skip + (uint32_t)t;
     int lo = 0, hi = (int)S.ncells;          // find e with c_pre[e] <= p < c_pre[e+1]
     while (hi - lo > 1) {
         const int mid = (lo + hi) >> 1;
         if (S.c_pre[mid] <= p) lo = mid; else hi = mid;
     }
+    if (cell_e) *cell_e = lo;
     return S.c_first[lo] + (p - S.c_pre[lo]);
-}
-
-// range index of shared-memory slot s (s < S.ncand)
-__device__ __forceinline__ int tile_slot_range(const TileS& S, uint32_t s) {
-    int lo = 0, hi = (int)S.nranges;
-    while (hi - lo > 1) {
-        const int mid = (lo + hi) >> 1;
-        if (S.r_base[mid] <= s) lo = mid; else hi = mid;
-    }
-    return lo;
-}
-
-// neighbour-list storage: per tile and warp a block of LIST_CAP rows x 32 lanes of u16 slots, stored in groups
-// of 4 rows so that one lane reads 4 consecutive entries with one 8-byte load and a warp reads 256 contiguous bytes.
-__device__ __forceinline__ size_t list_block_u2(uint32_t tile, int warp) {       // offset in uint2 units
-    return ((size_t)tile * TILE_WARPS + warp) * (size_t)(LIST_CAP / 4) * 32;
 }
 
 }  // namespace spray
