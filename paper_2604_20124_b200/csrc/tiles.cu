@@ -85,7 +85,7 @@ k_make_tiles(DevGrid g, CellTable ct, const double* __restrict__ hglob, uint32_t
     int cxa = 0;
     uint32_t skip = 0;
     while (ok && cxa < nx) {
-        if (warp_sum(row_count(row, cxa - 1, cxa + 1, nx, per)) > (uint32_t)TILE_CMAX) { ++cxa; skip = 0; continue; }   // column not tileable
+        if (warp_sum(row_count(row, cxa - 1, cxa + 1, nx, per)) > (uint32_t)(TILE_CMAX - TILE_MAXR)) { ++cxa; skip = 0; continue; }   // column not tileable
         uint32_t nt = 0;
         int cxb = cxa, next_cxa = nx;
         uint32_t next_skip = 0;
@@ -93,7 +93,7 @@ k_make_tiles(DevGrid g, CellTable ct, const double* __restrict__ hglob, uint32_t
             if (cx > cxa) {
                 const int ext = cx - cxa + 1;
                 if (ext > TILE_BXMAX || (per && ext + 2 > nx) ||
-                    warp_sum(row_count(row, cxa - 1, cx + 1, nx, per)) > (uint32_t)TILE_CMAX) {
+                    warp_sum(row_count(row, cxa - 1, cx + 1, nx, per)) > (uint32_t)(TILE_CMAX - TILE_MAXR)) {
                     next_cxa = cx; next_skip = 0; break;
                 }
             }
@@ -141,20 +141,46 @@ struct ListArgs {
 };
 
 constexpr int COLW = TILE_BXMAX + 4;
-constexpr size_t BL_OFF_F4 = 0;                                                        // float4 [CMAXP]
-constexpr size_t BL_OFF_B = BL_OFF_F4 + sizeof(float4) * TILE_CMAXP;                   // u16 [4][LIST_BC][TILE_THREADS]
-constexpr size_t BL_OFF_COL = BL_OFF_B + sizeof(uint16_t) * 4 * LIST_BC * TILE_THREADS;// u16 [MAXR][COLW]
+constexpr int LIST_LCAP = LIST_RMAX;       // builder: provisional hits per thread (flat list)
+constexpr size_t BL_OFF_XY = 0;                                                         // float4 [CMAXP/2]: (x0, x1, y0, y1) of slots 2p, 2p+1
+constexpr size_t BL_OFF_ZT = BL_OFF_XY + sizeof(float4) * (TILE_CMAXP / 2);             // float4 [CMAXP/2]: (z0, z1, T0, T1), T = (2h)^2
+constexpr size_t BL_OFF_L = BL_OFF_ZT + sizeof(float4) * (TILE_CMAXP / 2);              // u16 [LIST_LCAP][TILE_THREADS]
+constexpr size_t BL_OFF_B = BL_OFF_L + sizeof(uint16_t) * LIST_LCAP * TILE_THREADS;     // u16 [4][LIST_BC][TILE_THREADS]
+constexpr size_t BL_OFF_COL = BL_OFF_B + sizeof(uint16_t) * 4 * LIST_BC * TILE_THREADS; // u16 [MAXR][COLW]
 constexpr size_t BL_SMEM = BL_OFF_COL + sizeof(uint16_t) * TILE_MAXR * COLW;
 static_assert(BL_SMEM + sizeof(TileS) + 256 <= 227 * 1024, "list builder shared memory");
 
 __device__ __forceinline__ uint32_t get8(unsigned long long x, int b) { return (uint32_t)(x >> (8 * b)) & 0xFFu; }
+
+// packed fp32 pairs (sm_100 FADD2 / FMUL2 / FFMA2): one instruction tests two candidates
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk2(float a, float b) { f32x2 r; asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(a), "f"(b)); return r; }
+__device__ __forceinline__ void unpk2(f32x2 v, float& a, float& b) { asm("mov.b64 {%0,%1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); }
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) { f32x2 r; asm("sub.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) { f32x2 r; asm("mul.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+
+// predicated 16-bit shared-memory store + pointer bump (keeps the scan loop free of branches)
+__device__ __forceinline__ void append_if(bool hit, uint32_t& addr, uint32_t v) {
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %1, 0;\n\t@p st.shared.u16 [%0], %2;\n\t@p add.u32 %0, %0, %3;\n\t}"
+                 : "+r"(addr) : "r"((uint32_t)hit), "h"((uint16_t)v), "n"(2 * TILE_THREADS) : "memory");
+}
+
+// Which thread of a target owns bank beta in the scan (threads split the candidate PAIRS: slots 4i+2u, 4i+2u+1), and
+// the index of that bank among the owner's four buckets.
+__device__ __forceinline__ int bank_owner(int beta) { return (beta >> 1) & 1; }
+__device__ __forceinline__ int bank_local(int beta) { return ((beta >> 2) << 1) | (beta & 1); }
 
 __global__ void __launch_bounds__(TILE_THREADS, 1)
 k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
     extern __shared__ __align__(16) unsigned char smem[];
     __shared__ TileS S;
     __shared__ int s_bad, s_nonuni;
-    float4* f4 = reinterpret_cast<float4*>(smem + BL_OFF_F4);
+    float4* XY = reinterpret_cast<float4*>(smem + BL_OFF_XY);
+    float4* ZT = reinterpret_cast<float4*>(smem + BL_OFF_ZT);
+    float* XYf = reinterpret_cast<float*>(XY);
+    float* ZTf = reinterpret_cast<float*>(ZT);
+    uint16_t* Lf = reinterpret_cast<uint16_t*>(smem + BL_OFF_L);       // [k * TILE_THREADS + tid]
     uint16_t* B = reinterpret_cast<uint16_t*>(smem + BL_OFF_B);        // [(b * LIST_BC + k) * TILE_THREADS + tid]
     uint16_t* colofs = reinterpret_cast<uint16_t*>(smem + BL_OFF_COL); // [range][COLW]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -186,29 +212,33 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
                 colofs[q * COLW + jj] = (uint16_t)(gs - S.r_vstart[q]);
             }
         }
-        // ---- stage the candidates: one warp per range
+        // ---- stage the candidates as slot pairs: one warp per range; the odd pad slot of a range is put out of reach
         {
             const unsigned long long h0 = (unsigned long long)__double_as_longlong(A.p1[S.r_vstart[0]].y);
             bool nonuni = false;
             for (int q = warp; q < (int)S.nranges; q += TILE_WARPS) {
                 const uint32_t vs = S.r_vstart[q], len = S.r_vend[q] - vs, base = S.r_base[q];
                 const double shx = S.r_shift[q][0] * g.L[0], shy = S.r_shift[q][1] * g.L[1], shz = S.r_shift[q][2] * g.L[2];
-                for (uint32_t k = lane; k < len; k += 32) {
-                    const double2 xy = A.p0[vs + k], zh = A.p1[vs + k];
-                    // image position next to the tile: x_b - shift*L
-                    const float fx = (float)((xy.x - shx) - ox);
-                    const float fy = (float)((xy.y - shy) - oy);
-                    const float fz = (float)((zh.x - shz) - oz);
-                    const float Rb = 2.0f * (float)zh.y;
-                    f4[base + k] = make_float4(fx, fy, fz, Rb * Rb);
-                    nonuni |= (unsigned long long)__double_as_longlong(zh.y) != h0;
+                for (uint32_t k = lane; k < ((len + 1u) & ~1u); k += 32) {
+                    float fx = 3.0e18f, fy = 3.0e18f, fz = 3.0e18f, T = 0.0f;
+                    if (k < len) {
+                        const double2 xy = A.p0[vs + k], zh = A.p1[vs + k];
+                        fx = (float)((xy.x - shx) - ox);                // image position next to the tile: x_b - shift*L
+                        fy = (float)((xy.y - shy) - oy);
+                        fz = (float)((zh.x - shz) - oz);
+                        const float Rb = 2.0f * (float)zh.y;
+                        T = Rb * Rb;
+                        nonuni |= (unsigned long long)__double_as_longlong(zh.y) != h0;
+                    }
+                    const uint32_t s = base + k, o = (s >> 1) * 4 + (s & 1);
+                    XYf[o] = fx; XYf[o + 2] = fy; ZTf[o] = fz; ZTf[o + 2] = T;
                 }
             }
             if (nonuni) s_nonuni = 1;
         }
         // ---- this thread's target
         const bool active = tgt < (int)td.nt;
-        uint32_t i = 0;
+        uint32_t i = 0, s_self = 0xFFFFFFFFu;
         double xa = 0, ya = 0, za = 0, ha = 0;
         int tcol = 0, trow = 0;
         if (active) {
@@ -218,10 +248,13 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
             tcol = e / nrows; trow = e % nrows;
             const double2 xy = A.p0[i], zh = A.p1[i];
             xa = xy.x; ya = xy.y; za = zh.x; ha = zh.y;
+            for (int q = 0; q < (int)S.nranges; ++q)
+                if (i >= S.r_vstart[q] && i < S.r_vend[q]) s_self = S.r_base[q] + (i - S.r_vstart[q]);
         }
-        const float fax = (float)(xa - ox), fay = (float)(ya - oy), faz = (float)(za - oz);
+        // an inactive thread sits far away from everything: it never hits
+        const float fax = active ? (float)(xa - ox) : -3.0e18f, fay = (float)(ya - oy), faz = (float)(za - oz);
         const float Ra = 2.0f * (float)ha;
-        const float Ta = active ? Ra * Ra : -1.0f;
+        const float Ta = Ra * Ra;
         const float Ta_hi = fmaf(Ta, 1.00001f, Am), Ta_lo = fmaf(Ta, 0.99999f, -Am);
         // warp window in virtual columns / candidate rows
         int cmin = active ? tcol : 1 << 20, cmax = active ? tcol : -1;
@@ -234,13 +267,20 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
             zmin = min(zmin, __shfl_xor_sync(0xFFFFFFFFu, zmin, o)); zmax = max(zmax, __shfl_xor_sync(0xFFFFFFFFu, zmax, o));
         }
         __syncthreads();
+        const bool uni = s_nonuni == 0;
 
-        // ---- scan: fp32 prefilter, the even (odd) thread of a target tests the even (odd) slots; all lanes of the
-        //      same parity read the same candidate (shared-memory broadcast).  Hits go to the (thread, bank) buckets.
-        uint32_t cnt = 0, ng = 0;                                       // cnt: 4 x 8-bit bucket fills (bank = 2 b + u)
-        bool ovf = false, coinc = false;
+        // ---- scan: fp32 prefilter on slot pairs (FADD2/FFMA2: two candidates per instruction).  The two threads of a
+        //      target take alternate pairs (slots 4i+2u, 4i+2u+1); all lanes of the same parity read the same pair
+        //      (shared-memory broadcast).  A hit (r2 below the support of the larger h, error bound added) is
+        //      appended to the thread's flat list; it is classified exactly in the next phase.
+        uint32_t nl = 0;                                                // provisional hits of this thread
         if (cmax >= 0) {
             const int wv_lo = cmin, wv_hi = cmax + 2;                   // virtual columns [tcol, tcol + 2] around each target
+            const f32x2 ax2 = pk2(fax, fax), ay2 = pk2(fay, fay), az2 = pk2(faz, faz);
+            const f32x2 one_eps = pk2(1.00001f, 1.00001f), am2 = pk2(Am, Am);
+            const uint32_t lp0 = (uint32_t)__cvta_generic_to_shared(Lf + tid);
+            uint32_t lp = lp0;
+            const uint32_t lend = lp0 + 2u * (LIST_LCAP - 1) * TILE_THREADS;      // two appends per iteration at most
             for (int q = 0; q < (int)S.nranges; ++q) {
                 const int row = S.r_shift[q][3], ry = row & 3, rz = row >> 2;
                 if (ry < ymin || ry > ymax + 2 || rz < zmin || rz > zmax + 2) continue;
@@ -249,37 +289,72 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
                 if (jhi <= jlo) continue;
                 const uint32_t sa = S.r_base[q] + colofs[q * COLW + jlo];
                 const uint32_t sb = S.r_base[q] + colofs[q * COLW + jhi];
+                // pairs [sa/2, (sb+1)/2): a pair cut by a column boundary brings in a slot of the same row two or
+                // more cells away (never a neighbour, never scanned twice); a range's pad slot is out of reach
+                const uint32_t pa = sa >> 1, pb = (sb + 1u) >> 1;
+                if (uni) {
 #pragma unroll 4
-                for (uint32_t s = sa + ((sa ^ (uint32_t)u) & 1u); s < sb; s += 2) {
-                    const float4 c = f4[s];
-                    const float dx = fax - c.x, dy = fay - c.y, dz = faz - c.z;
-                    const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                    const float Tm = fmaxf(Ta, c.w);
-                    if (r2 < fmaf(Tm, 1.00001f, Am)) {
-                        bool in_s, in_g;
-                        if (r2 < fmaf(Tm, 0.99999f, -Am) && (r2 < Ta_lo || r2 >= Ta_hi) && r2 > 0.0f) {
-                            in_s = active; in_g = active && r2 < Ta_lo;
-                        } else {                                        // near a support boundary or r = 0: exact predicate (O2/A12)
-                            const uint32_t gi = S.r_vstart[q] + (s - S.r_base[q]);
-                            const double2 xy = A.p0[gi], zh = A.p1[gi];
-                            const double ex = min_image(__dsub_rn(xa, xy.x), g.per[0], g.L[0], g.halfL[0]);
-                            const double ey = min_image(__dsub_rn(ya, xy.y), g.per[1], g.L[1], g.halfL[1]);
-                            const double ez = min_image(__dsub_rn(za, zh.x), g.per[2], g.L[2], g.halfL[2]);
-                            const double e2 = r2_exact(ex, ey, ez);
-                            in_s = active && gi != i && e2 < support2(fmax(ha, zh.y));
-                            in_g = in_s && e2 < support2(ha);
-                            if (in_s && !(e2 > 0.0)) coinc = true;      // coincident particles: left to the general kernels (A11)
-                        }
-                        if (in_s) {
-                            const int b = (int)(s >> 1) & 3;
-                            const uint32_t k = (cnt >> (8 * b)) & 0xFFu;
-                            if (k < (uint32_t)LIST_BC) B[(b * LIST_BC + k) * TILE_THREADS + tid] = (uint16_t)s;
-                            else ovf = true;
-                            cnt += (k < (uint32_t)LIST_BC) ? (1u << (8 * b)) : 0u;
-                            ng += in_g ? 1u : 0u;
-                        }
+                    for (uint32_t p = pa + ((pa ^ (uint32_t)u) & 1u); p < pb; p += 2) {
+                        const float4 c0 = XY[p], c1 = ZT[p];
+                        const f32x2 dx = sub2(ax2, pk2(c0.x, c0.y)), dy = sub2(ay2, pk2(c0.z, c0.w)), dz = sub2(az2, pk2(c1.x, c1.y));
+                        float r0, r1;
+                        unpk2(fma2(dz, dz, fma2(dy, dy, mul2(dx, dx))), r0, r1);
+                        const bool room = lp < lend;
+                        append_if(r0 < Ta_hi && room, lp, 2 * p);
+                        append_if(r1 < Ta_hi && room, lp, 2 * p + 1);
+                    }
+                } else {
+#pragma unroll 4
+                    for (uint32_t p = pa + ((pa ^ (uint32_t)u) & 1u); p < pb; p += 2) {
+                        const float4 c0 = XY[p], c1 = ZT[p];
+                        const f32x2 dx = sub2(ax2, pk2(c0.x, c0.y)), dy = sub2(ay2, pk2(c0.z, c0.w)), dz = sub2(az2, pk2(c1.x, c1.y));
+                        float r0, r1, h0, h1;
+                        unpk2(fma2(dz, dz, fma2(dy, dy, mul2(dx, dx))), r0, r1);
+                        unpk2(fma2(pk2(fmaxf(Ta, c1.z), fmaxf(Ta, c1.w)), one_eps, am2), h0, h1);
+                        const bool room = lp < lend;
+                        append_if(r0 < h0 && room, lp, 2 * p);
+                        append_if(r1 < h1 && room, lp, 2 * p + 1);
                     }
                 }
+            }
+            nl = (lp - lp0) / (2u * TILE_THREADS);
+            if (lp >= lend) s_bad = 1;                                  // flat list full (it may have dropped hits)
+        }
+        // ---- classify the provisional hits and drop them into the (thread, bank) buckets.  A hit is certain when its
+        //      fp32 r2 is clear of every support boundary by more than the error bound; otherwise (and at r = 0, which
+        //      includes the target itself) the exact fp64 contract predicate decides (O2/A12).
+        uint32_t cnt = 0, ng = 0;                                       // cnt: 4 x 8-bit bucket fills
+        bool ovf = false, coinc = false;
+        for (uint32_t k = 0; k < nl; ++k) {
+            const uint32_t s = Lf[k * TILE_THREADS + tid];
+            if (s == s_self) continue;
+            const float4 c0 = XY[s >> 1], c1 = ZT[s >> 1];
+            const bool od = (s & 1u) != 0;
+            const float dx = fax - (od ? c0.y : c0.x), dy = fay - (od ? c0.w : c0.z), dz = faz - (od ? c1.y : c1.x);
+            const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+            const float Tm = fmaxf(Ta, od ? c1.w : c1.z);
+            bool in_s, in_g;
+            if (r2 < fmaf(Tm, 0.99999f, -Am) && (r2 < Ta_lo || r2 >= Ta_hi) && r2 > 0.0f) {
+                in_s = true; in_g = r2 < Ta_lo;
+            } else {
+                int q = 0;
+                while (q + 1 < (int)S.nranges && S.r_base[q + 1] <= s) ++q;
+                const uint32_t gi = S.r_vstart[q] + (s - S.r_base[q]);
+                const double2 xy = A.p0[gi], zh = A.p1[gi];
+                const double ex = min_image(__dsub_rn(xa, xy.x), g.per[0], g.L[0], g.halfL[0]);
+                const double ey = min_image(__dsub_rn(ya, xy.y), g.per[1], g.L[1], g.halfL[1]);
+                const double ez = min_image(__dsub_rn(za, zh.x), g.per[2], g.L[2], g.halfL[2]);
+                const double e2 = r2_exact(ex, ey, ez);
+                in_s = gi != i && e2 < support2(fmax(ha, zh.y));
+                in_g = in_s && e2 < support2(ha);
+                if (in_s && !(e2 > 0.0)) coinc = true;                  // coincident particles: left to the general kernels (A11)
+            }
+            if (in_s) {
+                const int b = bank_local((int)(s & 7u));
+                const uint32_t kk = (cnt >> (8 * b)) & 0xFFu;
+                if (kk < (uint32_t)LIST_BC) { B[(b * LIST_BC + kk) * TILE_THREADS + tid] = (uint16_t)s; cnt += 1u << (8 * b); }
+                else ovf = true;
+                ng += in_g ? 1u : 0u;
             }
         }
         if (ovf || coinc) s_bad = 1;
@@ -290,7 +365,7 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
         uint32_t n_lane = 0, nsym = 0;
 #pragma unroll
         for (int beta = 0; beta < 8; ++beta) {
-            const uint32_t cb = (((beta & 1) == u ? cnt : cnt_o) >> (8 * (beta >> 1))) & 0xFFu;
+            const uint32_t cb = ((bank_owner(beta) == u ? cnt : cnt_o) >> (8 * bank_local(beta))) & 0xFFu;
             const uint32_t f = (uint32_t)(u + beta) & 1u;
             const uint32_t mine = (cb + 1u - f) >> 1;
             cu |= (unsigned long long)mine << (8 * beta);
@@ -313,8 +388,9 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
         __syncthreads();
         const bool bad = s_bad != 0;
         if (!bad) {
-            // ---- emit my half-list in scheduled order (see the header): phases of R/8 rounds, bank (j + t) & 7
-            unsigned long long own = 0, ovr = 0;
+            // ---- emit my half-list in scheduled order (see the header): phase t = rounds [tR/8, (t+1)R/8) in bank
+            //      (j + t) & 7; what a phase cannot hold (overflow) fills the holes of other phases; the rest are dummies.
+            unsigned long long ovr = 0;                                 // 8 x 8-bit: overflow entries of each bank not yet placed
             uint32_t ovtot = 0;
 #pragma unroll
             for (int beta = 0; beta < 8; ++beta) {
@@ -322,37 +398,38 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
                 const uint32_t cap = (((uint32_t)(t + 1) * R) >> 3) - (((uint32_t)t * R) >> 3);
                 const uint32_t c = get8(cu, beta);
                 const uint32_t o = c > cap ? c - cap : 0u;
-                own |= (unsigned long long)(c - o) << (8 * beta);
                 ovr |= (unsigned long long)o << (8 * beta);
                 ovtot += o;
             }
-            uint2* blk = A.pool + off;
-            const int pairbase = tid & ~1;
-            int t = 0, beta = j;
-            uint32_t bnd = R >> 3, own_left = get8(own, beta), front = 0, w0 = 0, w1 = 0;
-            for (uint32_t r = 0; r < R; ++r) {
-                while (r >= bnd && t < 7) { ++t; beta = (beta + 1) & 7; bnd = ((uint32_t)(t + 1) * R) >> 3; own_left = get8(own, beta); front = 0; }
-                uint32_t item;
-                if (own_left) {
-                    const uint32_t e = ((uint32_t)(u + beta) & 1u) + 2u * front;
-                    item = B[((beta >> 1) * LIST_BC + e) * TILE_THREADS + pairbase + (beta & 1)];
-                    ++front; --own_left;
-                } else if (ovtot) {
-                    int b2 = beta;
-                    do { b2 = (b2 + 1) & 7; } while (!get8(ovr, b2));
-                    const uint32_t k = get8(cu, b2) - get8(ovr, b2);
-                    ovr -= 1ull << (8 * b2); --ovtot;
-                    const uint32_t e = ((uint32_t)(u + b2) & 1u) + 2u * k;
-                    item = B[((b2 >> 1) * LIST_BC + e) * TILE_THREADS + pairbase + (b2 & 1)];
-                } else {
-                    item = (uint32_t)(TILE_CMAX + beta);                // dummy slot of this phase's bank
+            const unsigned long long ov0 = ovr;                         // full overflow of each bank
+            // schedule into my (now free) flat-list column, then pack 4 rounds per 8-byte store
+            uint16_t* out = Lf + tid;                                   // out[r * TILE_THREADS]
+            const uint16_t* Bp = B + (tid & ~1);
+            uint32_t r = 0;
+            for (int t = 0; t < 8; ++t) {
+                const int beta = (j + t) & 7;
+                const uint32_t end = ((uint32_t)(t + 1) * R) >> 3;
+                const uint32_t own = get8(cu, beta) - get8(ov0, beta);
+                // my entries of bank beta: indices f, f+2, ... of the bucket of thread bank_owner(beta)
+                const uint16_t* bp = Bp + (bank_local(beta) * LIST_BC + ((u + beta) & 1)) * TILE_THREADS + bank_owner(beta);
+                for (uint32_t k = 0; k < own; ++k, ++r) out[r * TILE_THREADS] = bp[2 * k * TILE_THREADS];
+                for (; r < end; ++r) {
+                    uint32_t item = (uint32_t)(TILE_CMAX + beta);       // dummy slot of this phase's bank
+                    if (ovtot) {
+                        int b2 = beta;
+                        do { b2 = (b2 + 1) & 7; } while (!get8(ovr, b2));
+                        const uint32_t k = get8(cu, b2) - get8(ovr, b2);
+                        ovr -= 1ull << (8 * b2); --ovtot;
+                        item = Bp[(bank_local(b2) * LIST_BC + ((u + b2) & 1) + 2 * k) * TILE_THREADS + bank_owner(b2)];
+                    }
+                    out[r * TILE_THREADS] = (uint16_t)item;
                 }
-                switch (r & 3u) {
-                    case 0: w0 = item; break;
-                    case 1: w0 |= item << 16; break;
-                    case 2: w1 = item; break;
-                    default: w1 |= item << 16; blk[(size_t)(r >> 2) * 32 + lane] = make_uint2(w0, w1); break;
-                }
+            }
+            uint2* blk = A.pool + off + lane;
+            for (uint32_t r4 = 0; r4 < R; r4 += 4) {
+                const uint32_t e0 = out[r4 * TILE_THREADS], e1 = out[(r4 + 1) * TILE_THREADS];
+                const uint32_t e2 = out[(r4 + 2) * TILE_THREADS], e3 = out[(r4 + 3) * TILE_THREADS];
+                blk[(size_t)(r4 >> 2) * 32] = make_uint2(e0 | (e1 << 16), e2 | (e3 << 16));
             }
             if (u == 0) A.lcount[(size_t)tile * TILE_T + tgt] = active ? (ng | (nsym << 16)) : 0u;
             if (active && u == 0) A.fast[i] = 1;

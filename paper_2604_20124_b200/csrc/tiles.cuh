@@ -34,7 +34,7 @@ constexpr int TILE_MAXR = 32;        // candidate ranges: 4 x 4 rows x (1 or 2 p
 constexpr int TILE_BXMAX = 24;       // max columns (cells along x) of a tile
 constexpr int TILE_MAXCELL = 4 * TILE_BXMAX;
 constexpr int LIST_BC = 24;          // builder: capacity of one (thread, bank) bucket
-constexpr int LIST_RMAX = 160;       // max rounds of a warp's schedule (longer -> tile served by the general kernels)
+constexpr int LIST_RMAX = 80;        // max rounds of a warp's schedule = builder's flat-list rows (longer -> tile served by the general kernels)
 
 struct TileDesc {                    // 24 bytes
     int16_t y0, z0;                  // first row of the bundle
@@ -59,7 +59,7 @@ struct TileS {
     // candidate ranges
     uint32_t r_vstart[TILE_MAXR];    // first global slot of the range
     uint32_t r_vend[TILE_MAXR];      // one past the last global slot
-    uint32_t r_base[TILE_MAXR + 1];  // first shared-memory slot of the range (exclusive scan of the lengths)
+    uint32_t r_base[TILE_MAXR + 1];  // first shared-memory slot of the range (exclusive scan of the lengths rounded up to even)
     int8_t r_shift[TILE_MAXR][4];    // [0..2] periodic image: dx = (x_a - x_b) + shift * L (-1, 0, +1); [3] candidate row id
     int4 r_geo[TILE_MAXR];           // (first cell column, number of columns, virtual column of the first, first cell id)
     uint32_t nranges, ncand;
@@ -121,8 +121,8 @@ __device__ __forceinline__ void tile_setup(const TileDesc& td, const DevGrid& g,
     if (tid < 32) {
         RangeGeo R;
         const bool valid = tile_range(td, g, ct, tid >> 1, tid & 1, R);
-        const uint32_t len = valid ? R.ve - R.vs : 0u;
-        // compact the valid ranges to the front, keeping order (ballot + popc), and scan the lengths
+        const uint32_t len = valid ? ((R.ve - R.vs + 1u) & ~1u) : 0u;  // every range starts on an even slot (list builder: slot pairs)
+        // compact the valid ranges to the front, keeping order (ballot + popc), and scan the padded lengths
         const uint32_t mask = __ballot_sync(0xFFFFFFFFu, valid);
         const int pos = __popc(mask & ((1u << tid) - 1u));
         uint32_t incl = len;
