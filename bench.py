@@ -88,6 +88,23 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def max_over_ranks(seconds, world, device=None):
+    """Multi-GPU timing rule: the job's time is the MAX over ranks (one all-reduce of a scalar, outside the timed
+    region).  Replicas only: this and the barrier are the only collectives of the bench."""
+    if world <= 1:
+        return float(seconds)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([seconds], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(world, pairs_per_pass, steps, seconds):
+    """Whole-job throughput: every rank runs `steps` full passes over its own replica (weak scaling)."""
+    return world * pairs_per_pass * steps / seconds
+
+
 def oracle_sample_pass(w, targets):
     """The oracle as it stands on a bounded sample of the workload (its cell-list variant restricted to `targets`;
     rho = recipe density and mu = c/(3 rho kappa) as inputs).  Returns (seconds, pair interactions)."""
@@ -219,11 +236,8 @@ def main():
     launches = sp.launch_count() - l0
     t_total = evs[0][0].elapsed_time(evs[-1][4]) * 1e-3
     seg = np.array([[e[i].elapsed_time(e[i + 1]) for i in range(4)] for e in evs]) * 1e-3     # build, density, hydro, fld
-    if world > 1:
-        tt = torch.tensor([t_total], dtype=f64, device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        t_total = float(tt.item())
-    value = world * p_pass * args.steps / t_total
+    t_total = max_over_ranks(t_total, world, dev)
+    value = aggregate_value(world, p_pass, args.steps, t_total)
 
     # ---- e2e: pinned host buffers, H2D of every input and D2H of every output inside the timed region
     e2e = None
@@ -244,11 +258,8 @@ def main():
         e1.record()
         barrier()
         te = e0.elapsed_time(e1) * 1e-3
-        if world > 1:
-            tt = torch.tensor([te], dtype=f64, device=dev)
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            te = float(tt.item())
-        e2e = {"value": world * p_pass * ksteps / te, "unit": UNIT, "h2d_bytes_per_step": 8 * n * len(fields),
+        te = max_over_ranks(te, world, dev)
+        e2e = {"value": aggregate_value(world, p_pass, ksteps, te), "unit": UNIT, "h2d_bytes_per_step": 8 * n * len(fields),
                "d2h_bytes_per_step": 8 * n * len(out), "ms_per_step": 1e3 * te / ksteps}
 
     if rank != 0:

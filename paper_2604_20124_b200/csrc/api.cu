@@ -44,7 +44,7 @@ void free_all(Ctx* c) {
     for (double2* r : k.s) cudaFree(r);
     Tiled& t = c->tl;
     cudaFree(t.tiles); cudaFree(t.bcount); cudaFree(t.pool); cudaFree(t.ctr); cudaFree(t.winfo); cudaFree(t.lcount);
-    cudaFree(t.tflags); cudaFree(t.fast);
+    cudaFree(t.tflags); cudaFree(t.tiletab); cudaFree(t.fast);
 }
 
 // Scratch of the tiled path (tiles, neighbour lists): sized for (n, grid) at the first spray_build_cells that needs
@@ -58,17 +58,17 @@ void ensure_tiled(Ctx* c) {
     const int64_t need = (5 * ((c->n + TILE_T - 1) / TILE_T)) / 4 + 2 * nb + 64;
     const int64_t pool_need = c->n * POOL_U2_PER_PARTICLE + 4096;
     if (t.tiles && need <= t.tile_cap && nb <= t.bundle_cap && pool_need <= t.pool_cap) return;
-    cudaFree(t.tiles); cudaFree(t.bcount); cudaFree(t.pool); cudaFree(t.winfo); cudaFree(t.lcount); cudaFree(t.tflags);
-    t.tiles = nullptr; t.bcount = nullptr; t.pool = nullptr; t.winfo = nullptr; t.lcount = nullptr; t.tflags = nullptr;
+    cudaFree(t.tiles); cudaFree(t.bcount); cudaFree(t.pool); cudaFree(t.winfo); cudaFree(t.lcount); cudaFree(t.tflags); cudaFree(t.tiletab);
+    t.tiles = nullptr; t.bcount = nullptr; t.pool = nullptr; t.winfo = nullptr; t.lcount = nullptr; t.tflags = nullptr; t.tiletab = nullptr;
     t.tile_cap = 0; t.bundle_cap = 0; t.pool_cap = 0;
     bool ok = dmalloc(&t.tiles, need) && dmalloc(&t.bcount, nb + 4096 + 64) && dmalloc(&t.winfo, need * TILE_WARPS) &&
-              dmalloc(&t.lcount, need * TILE_T) && dmalloc(&t.tflags, need) && dmalloc(&t.pool, pool_need);
+              dmalloc(&t.lcount, need * TILE_T) && dmalloc(&t.tflags, need) && dmalloc(&t.tiletab, need * TILES_WORDS) && dmalloc(&t.pool, pool_need);
     if (ok && !t.ctr) ok = dmalloc(&t.ctr, CTR_COUNT);
     if (ok && !t.fast) ok = dmalloc(&t.fast, c->n_max);
     if (!ok) {
         cudaGetLastError();
-        cudaFree(t.tiles); cudaFree(t.bcount); cudaFree(t.pool); cudaFree(t.winfo); cudaFree(t.lcount); cudaFree(t.tflags);
-        t.tiles = nullptr; t.bcount = nullptr; t.pool = nullptr; t.winfo = nullptr; t.lcount = nullptr; t.tflags = nullptr;
+        cudaFree(t.tiles); cudaFree(t.bcount); cudaFree(t.pool); cudaFree(t.winfo); cudaFree(t.lcount); cudaFree(t.tflags); cudaFree(t.tiletab);
+        t.tiles = nullptr; t.bcount = nullptr; t.pool = nullptr; t.winfo = nullptr; t.lcount = nullptr; t.tflags = nullptr; t.tiletab = nullptr;
         return;
     }
     t.tile_cap = need; t.bundle_cap = nb; t.pool_cap = pool_need;

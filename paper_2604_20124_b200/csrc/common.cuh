@@ -30,6 +30,12 @@ constexpr double kWnWend = kSigmaWend;
 constexpr double kFnWend = -5.0 * kSigmaWend;
 
 __device__ __forceinline__ double dmax0(double a) { return a > 0.0 ? a : 0.0; }
+// max(a, 0) without the FP64 pipe: clamp the (signed) high word at 0.  A negative a becomes a denormal < 2.2e-308
+// (its low word survives), which is 0 at any tolerance; -0.0 and NaN handling do not matter to the callers.
+__device__ __forceinline__ double dmax0_fast(double a) {
+    const int hi = __double2hiint(a), lo = __double2loint(a);
+    return __hiloint2double(max(hi, 0), lo);
+}
 
 // ---- kernel shape functions of q = r/h, clamped so that they vanish identically for q >= 2 ("0 for q >= 2").
 // W(r;h) = sigma/h^3 * w(q);  F(r;h) = dW/dr = sigma/h^4 * f(q)

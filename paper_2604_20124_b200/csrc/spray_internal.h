@@ -44,6 +44,7 @@ struct Tiled {
     uint2* winfo = nullptr;      // [tile_cap][TILE_WARPS]: (pool offset, rounds)
     uint32_t* lcount = nullptr;  // [tile_cap][TILE_T]: n_gather | n_sym << 16
     uint32_t* tflags = nullptr;  // [tile_cap]: TILE_FLAG_*
+    uint32_t* tiletab = nullptr; // [tile_cap][TILES_WORDS]: per-tile TileS tables
     uint8_t* fast = nullptr;     // [n_max] sorted order: 1 = particle is served by the tiled kernels
 };
 enum { CTR_POOL = 0, CTR_NFAST = 1, CTR_NTILES = 2, CTR_WORK = 3, CTR_COUNT = 4 };

@@ -52,14 +52,14 @@ template <int KERNEL, bool CLAMP>
 __device__ __forceinline__ double wshape(double q) {
     if (KERNEL == 1) {                       // Wendland C2, eq. (3): (1-q/2)^4 (2q+1)
         double t = fma(-0.5, q, 1.0);
-        if (CLAMP) t = dmax0(t);
+        if (CLAMP) t = dmax0_fast(t);
         const double t2 = t * t;
         return (t2 * t2) * fma(2.0, q, 1.0);
     } else {                                 // cubic spline (A1): (2-q)^3 - 4 (1-q)_+^3
         constexpr double C = 1.5874010519681994748;      // cbrt(4)
         double t2 = 2.0 - q;
-        if (CLAMP) t2 = dmax0(t2);
-        const double t1 = dmax0(fma(-C, q, C));
+        if (CLAMP) t2 = dmax0_fast(t2);
+        const double t1 = dmax0_fast(fma(-C, q, C));
         return fma(t2 * t2, t2, -((t1 * t1) * t1));
     }
 }
@@ -67,12 +67,12 @@ template <int KERNEL, bool CLAMP>
 __device__ __forceinline__ double gshape(double q) {
     if (KERNEL == 1) {                       // q (1-q/2)^3
         double t = fma(-0.5, q, 1.0);
-        if (CLAMP) t = dmax0(t);
+        if (CLAMP) t = dmax0_fast(t);
         return (q * t) * (t * t);
     } else {                                 // (2-2q)_+^2 - (2-q)^2
         double t2 = 2.0 - q;
-        if (CLAMP) t2 = dmax0(t2);
-        const double s1 = dmax0(fma(-2.0, q, 2.0));
+        if (CLAMP) t2 = dmax0_fast(t2);
+        const double s1 = dmax0_fast(fma(-2.0, q, 2.0));
         return fma(s1, s1, -(t2 * t2));
     }
 }
@@ -97,6 +97,7 @@ struct SweepIn {
     double* mu_sorted;               // limiter: mu in sorted order for the general kernels
     const uint32_t* perm;
     const TileDesc* tiles;
+    const uint32_t* tiletab;         // [tile][TILES_WORDS]: TileS as built by tile_setup
     const unsigned long long* ctr;
     const uint2* pool;
     const uint2* winfo;
@@ -192,15 +193,14 @@ __device__ __forceinline__ void pair_body(const double2* __restrict__ F, const d
 
 template <int SWEEP, int KERNEL, bool UNI>
 __device__ __forceinline__ void pair_loop(const double2* __restrict__ F, const double* __restrict__ Ee, const uint2* __restrict__ lp,
-                                          uint32_t R, const Tgt& T, double beta, bool sym, Acc& acc) {
-    uint2 cur = R ? __ldg(lp) : make_uint2(0u, 0u);
+                                          uint32_t R, uint2 cur, uint2 nxt, const Tgt& T, double beta, bool sym, Acc& acc) {
     for (uint32_t r4 = 0; r4 < R; r4 += 4) {
-        const uint2 nxt = (r4 + 4 < R) ? __ldg(lp + (size_t)(r4 / 4 + 1) * 32) : make_uint2(0u, 0u);
+        const uint2 nx2 = (r4 + 8 < R) ? __ldg(lp + (size_t)(r4 / 4 + 2) * 32) : make_uint2(0u, 0u);
         pair_body<SWEEP, KERNEL, UNI>(F, Ee, cur.x & 0xFFFFu, T, beta, sym, acc);
         pair_body<SWEEP, KERNEL, UNI>(F, Ee, cur.x >> 16, T, beta, sym, acc);
         pair_body<SWEEP, KERNEL, UNI>(F, Ee, cur.y & 0xFFFFu, T, beta, sym, acc);
         pair_body<SWEEP, KERNEL, UNI>(F, Ee, cur.y >> 16, T, beta, sym, acc);
-        cur = nxt;
+        cur = nxt; nxt = nx2;
     }
 }
 
@@ -234,8 +234,18 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
         if (!(flags & TILE_FLAG_OK)) continue;
         const bool uni = (flags & TILE_FLAG_UNIH) != 0;
         const TileDesc td = A.tiles[tile];
+        // first two list rows: in flight while the records are staged
+        const uint2 wi = A.winfo[(size_t)tile * TILE_WARPS + warp];
+        const uint2* lp = A.pool + wi.x + lane;
+        const uint2 l0 = wi.y ? __ldg(lp) : make_uint2(0u, 0u);
+        const uint2 l1 = wi.y > 4 ? __ldg(lp + 32) : make_uint2(0u, 0u);
         __syncthreads();                                         // previous tile done with the staged records
-        tile_setup(td, g, ct, S);
+        {   // tile tables as the list builder left them
+            const uint32_t* src = A.tiletab + (size_t)tile * TILES_WORDS;
+            uint32_t* dst = reinterpret_cast<uint32_t*>(&S);
+            for (int w = tid; w < TILES_WORDS; w += TILE_THREADS) dst[w] = src[w];
+        }
+        __syncthreads();
         // ---- stage the candidate records: one warp per range
         for (int q = warp; q < (int)S.nranges; q += TILE_WARPS) {
             const uint32_t vs = S.r_vstart[q], len = S.r_vend[q] - vs, base = S.r_base[q];
@@ -270,13 +280,11 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
             if (SWEEP == SW_LIMITER) T.c0 = A.e1[i];                                         // E_a
             if (SWEEP == SW_APPLY) { const double2 me = A.rec[2][i]; T.c0 = me.y; T.c1 = me.x; T.c2 = 4.0 * me.x; }
         }
-        const uint2 wi = A.winfo[(size_t)tile * TILE_WARPS + warp];
         __syncthreads();
 
         Acc acc{0, 0, 0, 0, 0};
-        const uint2* lp = A.pool + wi.x + lane;
-        if (uni) pair_loop<SWEEP, KERNEL, true>(F, Ee, lp, wi.y, T, A.beta, sym, acc);
-        else pair_loop<SWEEP, KERNEL, false>(F, Ee, lp, wi.y, T, A.beta, sym, acc);
+        if (uni) pair_loop<SWEEP, KERNEL, true>(F, Ee, lp, wi.y, l0, l1, T, A.beta, sym, acc);
+        else pair_loop<SWEEP, KERNEL, false>(F, Ee, lp, wi.y, l0, l1, T, A.beta, sym, acc);
         // ---- add the two half-lists of the target
         acc.a0 += __shfl_xor_sync(0xFFFFFFFFu, acc.a0, 1);
         if (SWEEP != SW_DENSITY) acc.a1 += __shfl_xor_sync(0xFFFFFFFFu, acc.a1, 1);
@@ -343,7 +351,7 @@ cudaError_t launch_tiled_sweep(Ctx* c, int sweep, const TiledArgs& t, cudaStream
     SweepIn a{};
     const Packed& pk = c->pk;
     a.p1 = pk.p1; a.hh = pk.hh; a.t0 = pk.t0; a.me = pk.me; a.me_out = pk.me; a.mu_sorted = c->s.f[10]; a.e1 = pk.e1;
-    a.perm = c->perm; a.tiles = c->tl.tiles; a.ctr = c->tl.ctr; a.pool = c->tl.pool; a.winfo = c->tl.winfo;
+    a.perm = c->perm; a.tiles = c->tl.tiles; a.tiletab = c->tl.tiletab; a.ctr = c->tl.ctr; a.pool = c->tl.pool; a.winfo = c->tl.winfo;
     a.lcount = c->tl.lcount; a.tflags = c->tl.tflags; a.n = c->n;
     a.beta = t.beta; a.c_light = t.c_light; a.fld_sym = t.fld_sym;
     a.o0 = t.o0; a.o1 = t.o1; a.o2 = t.o2; a.o3 = t.o3; a.o4 = t.o4; a.ocount = t.ocount;

@@ -135,6 +135,7 @@ struct ListArgs {
     uint2* winfo;                      // [tile][warp]: (pool offset, rounds)
     uint32_t* lcount;                  // [tile][TILE_T]: n_gather | n_sym << 16
     uint32_t* tflags;                  // [tile]
+    uint32_t* tiletab;                 // [tile][TILES_WORDS]
     uint8_t* fast;                     // [n] sorted order: 1 = served by the tiled kernels
     const double* hglob;
     uint32_t* status;
@@ -193,6 +194,11 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
         __syncthreads();                                                // previous tile done with smem
         if (tid == 0) { s_bad = 0; s_nonuni = 0; }
         tile_setup(td, g, ct, S);
+        {   // keep the tables for the sweeps
+            uint32_t* dst = A.tiletab + (size_t)tile * TILES_WORDS;
+            const uint32_t* src = reinterpret_cast<const uint32_t*>(&S);
+            for (int w = tid; w < TILES_WORDS; w += TILE_THREADS) dst[w] = src[w];
+        }
         const int ncolv = td.cxb - td.cxa + 3;                          // virtual columns 0 .. ncolv-1
         // tile origin (centre of the tile's cell block) for the fp32 relative coordinates
         const double ox = g.lo[0] + (0.5 * (td.cxa + td.cxb + 1)) / g.inv[0];
@@ -469,7 +475,7 @@ cudaError_t launch_build_tiles(Ctx* c, cudaStream_t st) {
         if ((e = cudaFuncSetAttribute(k_build_lists, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BL_SMEM)) != cudaSuccess) return e;
         attr_done = true;
     }
-    ListArgs A{c->pk.p0, c->pk.p1, t.tiles, t.ctr, t.pool, (unsigned long long)t.pool_cap, t.winfo, t.lcount, t.tflags, t.fast,
+    ListArgs A{c->pk.p0, c->pk.p1, t.tiles, t.ctr, t.pool, (unsigned long long)t.pool_cap, t.winfo, t.lcount, t.tflags, t.tiletab, t.fast,
                c->hglob, c->dev_status};
     k_build_lists<<<t.sms, TILE_THREADS, BL_SMEM, st>>>(c->dg, ct, A);
     c->launches += 3;

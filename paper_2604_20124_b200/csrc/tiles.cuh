@@ -69,6 +69,9 @@ struct TileS {
     uint32_t ncells;
 };
 
+static_assert(sizeof(TileS) % 4 == 0, "TileS is copied word by word");
+constexpr int TILES_WORDS = (int)(sizeof(TileS) / 4);
+
 __device__ __forceinline__ uint32_t cell_id(const DevGrid& g, int cx, int cy, int cz) {
     return (uint32_t)((cz * g.nc[1] + cy) * g.nc[0] + cx);
 }
