@@ -195,7 +195,7 @@ template <int SWEEP, int KERNEL, bool UNI>
 __device__ __forceinline__ void pair_loop(const double2* __restrict__ F, const double* __restrict__ Ee, const uint2* __restrict__ lp,
                                           uint32_t R, uint2 cur, uint2 nxt, const Tgt& T, double beta, bool sym, Acc& acc) {
     for (uint32_t r4 = 0; r4 < R; r4 += 4) {
-        const uint2 nx2 = (r4 + 8 < R) ? __ldg(lp + (size_t)(r4 / 4 + 2) * 32) : make_uint2(0u, 0u);
+        const uint2 nx2 = (r4 + 8 < R) ? __ldcs(lp + (size_t)(r4 / 4 + 2) * 32) : make_uint2(0u, 0u);
         pair_body<SWEEP, KERNEL, UNI>(F, Ee, cur.x & 0xFFFFu, T, beta, sym, acc);
         pair_body<SWEEP, KERNEL, UNI>(F, Ee, cur.x >> 16, T, beta, sym, acc);
         pair_body<SWEEP, KERNEL, UNI>(F, Ee, cur.y & 0xFFFFu, T, beta, sym, acc);
@@ -237,8 +237,8 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
         // first two list rows: in flight while the records are staged
         const uint2 wi = A.winfo[(size_t)tile * TILE_WARPS + warp];
         const uint2* lp = A.pool + wi.x + lane;
-        const uint2 l0 = wi.y ? __ldg(lp) : make_uint2(0u, 0u);
-        const uint2 l1 = wi.y > 4 ? __ldg(lp + 32) : make_uint2(0u, 0u);
+        const uint2 l0 = wi.y ? __ldcs(lp) : make_uint2(0u, 0u);
+        const uint2 l1 = wi.y > 4 ? __ldcs(lp + 32) : make_uint2(0u, 0u);
         __syncthreads();                                         // previous tile done with the staged records
         {   // tile tables as the list builder left them
             const uint32_t* src = A.tiletab + (size_t)tile * TILES_WORDS;
