@@ -38,7 +38,7 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     headers = list(CSRC.glob("*.h")) + list(CSRC.glob("*.cuh")) + [PKG.parent / "include" / "spray.h", Path(__file__)]
     srcs = [CSRC / s for s in SOURCES if (CSRC / s).exists()]
     nvcc = _nvcc()
-    extra = ["-Xptxas", "-v"] if verbose else []
+    extra = (["-Xptxas", "-v"] if verbose else []) + os.environ.get("SPRAY_NVCC_EXTRA", "").split()
 
     def compile_one(src: Path):
         obj = OBJ / (src.stem + ".o")

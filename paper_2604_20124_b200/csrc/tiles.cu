@@ -142,6 +142,7 @@ struct ListArgs {
 };
 
 constexpr int COLW = TILE_BXMAX + 4;
+constexpr uint32_t LIST_RECHECK = 0x8000u;   // flat-list flag: classify this hit again (fp32 bounds, then exact fp64)
 constexpr int LIST_LCAP = LIST_RMAX;       // builder: provisional hits per thread (flat list)
 constexpr size_t BL_OFF_XY = 0;                                                         // float4 [CMAXP/2]: (x0, x1, y0, y1) of slots 2p, 2p+1
 constexpr size_t BL_OFF_ZT = BL_OFF_XY + sizeof(float4) * (TILE_CMAXP / 2);             // float4 [CMAXP/2]: (z0, z1, T0, T1), T = (2h)^2
@@ -284,6 +285,7 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
             const int wv_lo = cmin, wv_hi = cmax + 2;                   // virtual columns [tcol, tcol + 2] around each target
             const f32x2 ax2 = pk2(fax, fax), ay2 = pk2(fay, fay), az2 = pk2(faz, faz);
             const f32x2 one_eps = pk2(1.00001f, 1.00001f), am2 = pk2(Am, Am);
+            const float half_lo = 0.5f * Ta_lo;
             const uint32_t lp0 = (uint32_t)__cvta_generic_to_shared(Lf + tid);
             uint32_t lp = lp0;
             const uint32_t lend = lp0 + 2u * (LIST_LCAP - 1) * TILE_THREADS;      // two appends per iteration at most
@@ -306,8 +308,9 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
                         float r0, r1;
                         unpk2(fma2(dz, dz, fma2(dy, dy, mul2(dx, dx))), r0, r1);
                         const bool room = lp < lend;
-                        append_if(r0 < Ta_hi && room, lp, 2 * p);
-                        append_if(r1 < Ta_hi && room, lp, 2 * p + 1);
+                        // certain hit <=> 0 < r2 < Ta_lo <=> |r2 - Ta_lo/2| < Ta_lo/2; anything else is flagged for the exact test
+                        append_if(r0 < Ta_hi && room, lp, 2 * p + (fabsf(r0 - half_lo) < half_lo ? 0u : LIST_RECHECK));
+                        append_if(r1 < Ta_hi && room, lp, 2 * p + 1 + (fabsf(r1 - half_lo) < half_lo ? 0u : LIST_RECHECK));
                     }
                 } else {
 #pragma unroll 4
@@ -318,8 +321,8 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
                         unpk2(fma2(dz, dz, fma2(dy, dy, mul2(dx, dx))), r0, r1);
                         unpk2(fma2(pk2(fmaxf(Ta, c1.z), fmaxf(Ta, c1.w)), one_eps, am2), h0, h1);
                         const bool room = lp < lend;
-                        append_if(r0 < h0 && room, lp, 2 * p);
-                        append_if(r1 < h1 && room, lp, 2 * p + 1);
+                        append_if(r0 < h0 && room, lp, 2 * p + LIST_RECHECK);
+                        append_if(r1 < h1 && room, lp, 2 * p + 1 + LIST_RECHECK);
                     }
                 }
             }
@@ -332,28 +335,30 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
         uint32_t cnt = 0, ng = 0;                                       // cnt: 4 x 8-bit bucket fills
         bool ovf = false, coinc = false;
         for (uint32_t k = 0; k < nl; ++k) {
-            const uint32_t s = Lf[k * TILE_THREADS + tid];
+            const uint32_t v = Lf[k * TILE_THREADS + tid], s = v & 0x7FFFu;
             if (s == s_self) continue;
-            const float4 c0 = XY[s >> 1], c1 = ZT[s >> 1];
-            const bool od = (s & 1u) != 0;
-            const float dx = fax - (od ? c0.y : c0.x), dy = fay - (od ? c0.w : c0.z), dz = faz - (od ? c1.y : c1.x);
-            const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-            const float Tm = fmaxf(Ta, od ? c1.w : c1.z);
-            bool in_s, in_g;
-            if (r2 < fmaf(Tm, 0.99999f, -Am) && (r2 < Ta_lo || r2 >= Ta_hi) && r2 > 0.0f) {
-                in_s = true; in_g = r2 < Ta_lo;
-            } else {
-                int q = 0;
-                while (q + 1 < (int)S.nranges && S.r_base[q + 1] <= s) ++q;
-                const uint32_t gi = S.r_vstart[q] + (s - S.r_base[q]);
-                const double2 xy = A.p0[gi], zh = A.p1[gi];
-                const double ex = min_image(__dsub_rn(xa, xy.x), g.per[0], g.L[0], g.halfL[0]);
-                const double ey = min_image(__dsub_rn(ya, xy.y), g.per[1], g.L[1], g.halfL[1]);
-                const double ez = min_image(__dsub_rn(za, zh.x), g.per[2], g.L[2], g.halfL[2]);
-                const double e2 = r2_exact(ex, ey, ez);
-                in_s = gi != i && e2 < support2(fmax(ha, zh.y));
-                in_g = in_s && e2 < support2(ha);
-                if (in_s && !(e2 > 0.0)) coinc = true;                  // coincident particles: left to the general kernels (A11)
+            bool in_s = true, in_g = true;
+            if (v & LIST_RECHECK) {
+                const float4 c0 = XY[s >> 1], c1 = ZT[s >> 1];
+                const bool od = (s & 1u) != 0;
+                const float dx = fax - (od ? c0.y : c0.x), dy = fay - (od ? c0.w : c0.z), dz = faz - (od ? c1.y : c1.x);
+                const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                const float Tm = fmaxf(Ta, od ? c1.w : c1.z);
+                if (r2 < fmaf(Tm, 0.99999f, -Am) && (r2 < Ta_lo || r2 >= Ta_hi) && r2 > 0.0f) {
+                    in_g = r2 < Ta_lo;
+                } else {
+                    int q = 0;
+                    while (q + 1 < (int)S.nranges && S.r_base[q + 1] <= s) ++q;
+                    const uint32_t gi = S.r_vstart[q] + (s - S.r_base[q]);
+                    const double2 xy = A.p0[gi], zh = A.p1[gi];
+                    const double ex = min_image(__dsub_rn(xa, xy.x), g.per[0], g.L[0], g.halfL[0]);
+                    const double ey = min_image(__dsub_rn(ya, xy.y), g.per[1], g.L[1], g.halfL[1]);
+                    const double ez = min_image(__dsub_rn(za, zh.x), g.per[2], g.L[2], g.halfL[2]);
+                    const double e2 = r2_exact(ex, ey, ez);
+                    in_s = gi != i && e2 < support2(fmax(ha, zh.y));
+                    in_g = in_s && e2 < support2(ha);
+                    if (in_s && !(e2 > 0.0)) coinc = true;              // coincident particles: left to the general kernels (A11)
+                }
             }
             if (in_s) {
                 const int b = bank_local((int)(s & 7u));
@@ -396,7 +401,7 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
         if (!bad) {
             // ---- emit my half-list in scheduled order (see the header): phase t = rounds [tR/8, (t+1)R/8) in bank
             //      (j + t) & 7; what a phase cannot hold (overflow) fills the holes of other phases; the rest are dummies.
-            unsigned long long ovr = 0;                                 // 8 x 8-bit: overflow entries of each bank not yet placed
+            unsigned long long ovr = 0;                                 // 8 x 8-bit: entries of each bank beyond its phase
             uint32_t ovtot = 0;
 #pragma unroll
             for (int beta = 0; beta < 8; ++beta) {
@@ -411,22 +416,27 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
             // schedule into my (now free) flat-list column, then pack 4 rounds per 8-byte store
             uint16_t* out = Lf + tid;                                   // out[r * TILE_THREADS]
             const uint16_t* Bp = B + (tid & ~1);
-            uint32_t r = 0;
+            // pass 1: every phase takes its own bank's entries (up to its capacity)
             for (int t = 0; t < 8; ++t) {
                 const int beta = (j + t) & 7;
-                const uint32_t end = ((uint32_t)(t + 1) * R) >> 3;
+                const uint32_t start = ((uint32_t)t * R) >> 3;
                 const uint32_t own = get8(cu, beta) - get8(ov0, beta);
                 // my entries of bank beta: indices f, f+2, ... of the bucket of thread bank_owner(beta)
                 const uint16_t* bp = Bp + (bank_local(beta) * LIST_BC + ((u + beta) & 1)) * TILE_THREADS + bank_owner(beta);
-                for (uint32_t k = 0; k < own; ++k, ++r) out[r * TILE_THREADS] = bp[2 * k * TILE_THREADS];
-                for (; r < end; ++r) {
+                for (uint32_t k = 0; k < own; ++k) out[(start + k) * TILE_THREADS] = bp[2 * k * TILE_THREADS];
+            }
+            // pass 2: the holes take the overflow entries bank by bank, then dummies
+            int b2 = -1;
+            uint32_t k2 = 0, kend = 0;
+            for (int t = 0; t < 8; ++t) {
+                const int beta = (j + t) & 7;
+                const uint32_t end = ((uint32_t)(t + 1) * R) >> 3;
+                for (uint32_t r = (((uint32_t)t * R) >> 3) + get8(cu, beta) - get8(ov0, beta); r < end; ++r) {
                     uint32_t item = (uint32_t)(TILE_CMAX + beta);       // dummy slot of this phase's bank
                     if (ovtot) {
-                        int b2 = beta;
-                        do { b2 = (b2 + 1) & 7; } while (!get8(ovr, b2));
-                        const uint32_t k = get8(cu, b2) - get8(ovr, b2);
-                        ovr -= 1ull << (8 * b2); --ovtot;
-                        item = Bp[(bank_local(b2) * LIST_BC + ((u + b2) & 1) + 2 * k) * TILE_THREADS + bank_owner(b2)];
+                        while (k2 == kend) { ++b2; kend = get8(cu, b2); k2 = kend - get8(ov0, b2); }
+                        item = Bp[(bank_local(b2) * LIST_BC + ((u + b2) & 1) + 2 * k2) * TILE_THREADS + bank_owner(b2)];
+                        ++k2; --ovtot;
                     }
                     out[r * TILE_THREADS] = (uint16_t)item;
                 }
