@@ -143,12 +143,13 @@ struct ListArgs {
 
 constexpr int COLW = TILE_BXMAX + 4;
 constexpr uint32_t LIST_RECHECK = 0x8000u;   // flat-list flag: classify this hit again (fp32 bounds, then exact fp64)
+constexpr int LIST_BS = LIST_BC + 1;        // rows of a (thread, bank) bucket incl. the trash row
 constexpr int LIST_LCAP = LIST_RMAX;       // builder: provisional hits per thread (flat list)
 constexpr size_t BL_OFF_XY = 0;                                                         // float4 [CMAXP/2]: (x0, x1, y0, y1) of slots 2p, 2p+1
 constexpr size_t BL_OFF_ZT = BL_OFF_XY + sizeof(float4) * (TILE_CMAXP / 2);             // float4 [CMAXP/2]: (z0, z1, T0, T1), T = (2h)^2
 constexpr size_t BL_OFF_L = BL_OFF_ZT + sizeof(float4) * (TILE_CMAXP / 2);              // u16 [LIST_LCAP][TILE_THREADS]
-constexpr size_t BL_OFF_B = BL_OFF_L + sizeof(uint16_t) * LIST_LCAP * TILE_THREADS;     // u16 [4][LIST_BC][TILE_THREADS]
-constexpr size_t BL_OFF_COL = BL_OFF_B + sizeof(uint16_t) * 4 * LIST_BC * TILE_THREADS; // u16 [MAXR][COLW]
+constexpr size_t BL_OFF_B = BL_OFF_L + sizeof(uint16_t) * LIST_LCAP * TILE_THREADS;     // u16 [4][LIST_BS][TILE_THREADS]
+constexpr size_t BL_OFF_COL = BL_OFF_B + sizeof(uint16_t) * 4 * LIST_BS * TILE_THREADS; // u16 [MAXR][COLW]
 constexpr size_t BL_SMEM = BL_OFF_COL + sizeof(uint16_t) * TILE_MAXR * COLW;
 static_assert(BL_SMEM + sizeof(TileS) + 256 <= 227 * 1024, "list builder shared memory");
 
@@ -168,6 +169,21 @@ __device__ __forceinline__ void append_if(bool hit, uint32_t& addr, uint32_t v) 
                  : "+r"(addr) : "r"((uint32_t)hit), "h"((uint16_t)v), "n"(2 * TILE_THREADS) : "memory");
 }
 
+// One candidate of the scan: if r2 < hi, store (value | LIST_RECHECK unless 0 < r2 < 2 half_lo) at the bucket row pointer and
+// advance it, clamped at `end` (the bucket's trash row: a pointer that reaches it reports the overflow).  No branches.
+__device__ __forceinline__ void append_flag(float r2, float hi, float half_lo, uint32_t& addr, uint32_t end, uint32_t v) {
+    asm volatile("{\n\t.reg .pred p, s;\n\t.reg .f32 t;\n\t.reg .b32 w;\n\t"
+                 "setp.lt.f32 p, %1, %2;\n\t"
+                 "sub.f32 t, %1, %3;\n\t"
+                 "abs.f32 t, t;\n\t"
+                 "setp.lt.f32 s, t, %3;\n\t"
+                 "selp.b32 w, %5, %6, s;\n\t"
+                 "@p st.shared.u16 [%0], w;\n\t"
+                 "@p add.u32 %0, %0, %7;\n\t"
+                 "min.u32 %0, %0, %4;\n\t}"
+                 : "+r"(addr) : "f"(r2), "f"(hi), "f"(half_lo), "r"(end), "r"(v), "r"(v | LIST_RECHECK), "n"(2 * TILE_THREADS) : "memory");
+}
+
 // Which thread of a target owns bank beta in the scan (threads split the candidate PAIRS: slots 4i+2u, 4i+2u+1), and
 // the index of that bank among the owner's four buckets.
 __device__ __forceinline__ int bank_owner(int beta) { return (beta >> 1) & 1; }
@@ -183,7 +199,7 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
     float* XYf = reinterpret_cast<float*>(XY);
     float* ZTf = reinterpret_cast<float*>(ZT);
     uint16_t* Lf = reinterpret_cast<uint16_t*>(smem + BL_OFF_L);       // [k * TILE_THREADS + tid]
-    uint16_t* B = reinterpret_cast<uint16_t*>(smem + BL_OFF_B);        // [(b * LIST_BC + k) * TILE_THREADS + tid]
+    uint16_t* B = reinterpret_cast<uint16_t*>(smem + BL_OFF_B);        // [(b * LIST_BS + k) * TILE_THREADS + tid]
     uint16_t* colofs = reinterpret_cast<uint16_t*>(smem + BL_OFF_COL); // [range][COLW]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int u = tid & 1, tgt = tid >> 1, j = lane & 7;
@@ -278,17 +294,37 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
 
         // ---- scan: fp32 prefilter on slot pairs (FADD2/FFMA2: two candidates per instruction).  The two threads of a
         //      target take alternate pairs (slots 4i+2u, 4i+2u+1); all lanes of the same parity read the same pair
-        //      (shared-memory broadcast).  A hit (r2 below the support of the larger h, error bound added) is
-        //      appended to the thread's flat list; it is classified exactly in the next phase.
-        uint32_t nl = 0;                                                // provisional hits of this thread
+        //      (shared-memory broadcast).  A hit (r2 below the support of the larger h, error bound added) goes straight
+        //      to the thread's bucket of the slot's bank: pair p feeds buckets (p & 2) and (p & 2) + 1, so with the loop
+        //      unrolled by two pairs the bucket of every append is a compile-time choice.  A hit that is not certain
+        //      (0 < r2 < Ta_lo, uniform-h tiles only) carries LIST_RECHECK.
+        const uint32_t bk0 = (uint32_t)__cvta_generic_to_shared(B + tid);
+        constexpr uint32_t BROW = 2u * TILE_THREADS;                    // bytes per bucket row
+        uint32_t bp0 = bk0, bp1 = bk0 + LIST_BS * BROW, bp2 = bk0 + 2 * LIST_BS * BROW, bp3 = bk0 + 3 * LIST_BS * BROW;
+        const uint32_t e0 = bk0 + LIST_BC * BROW, e1 = e0 + LIST_BS * BROW, e2 = e1 + LIST_BS * BROW, e3 = e2 + LIST_BS * BROW;
         if (cmax >= 0) {
             const int wv_lo = cmin, wv_hi = cmax + 2;                   // virtual columns [tcol, tcol + 2] around each target
             const f32x2 ax2 = pk2(fax, fax), ay2 = pk2(fay, fay), az2 = pk2(faz, faz);
             const f32x2 one_eps = pk2(1.00001f, 1.00001f), am2 = pk2(Am, Am);
             const float half_lo = 0.5f * Ta_lo;
-            const uint32_t lp0 = (uint32_t)__cvta_generic_to_shared(Lf + tid);
-            uint32_t lp = lp0;
-            const uint32_t lend = lp0 + 2u * (LIST_LCAP - 1) * TILE_THREADS;      // two appends per iteration at most
+            // one pair: test both slots, append to buckets (pa_, pb_) whose row pointers are clamped at the trash row
+            auto pair_uni = [&](uint32_t p, uint32_t& qa, uint32_t qa_end, uint32_t& qb, uint32_t qb_end) {
+                const float4 c0 = XY[p], c1 = ZT[p];
+                const f32x2 dx = sub2(ax2, pk2(c0.x, c0.y)), dy = sub2(ay2, pk2(c0.z, c0.w)), dz = sub2(az2, pk2(c1.x, c1.y));
+                float r0, r1;
+                unpk2(fma2(dz, dz, fma2(dy, dy, mul2(dx, dx))), r0, r1);
+                append_flag(r0, Ta_hi, half_lo, qa, qa_end, 2 * p);
+                append_flag(r1, Ta_hi, half_lo, qb, qb_end, 2 * p + 1);
+            };
+            auto pair_gen = [&](uint32_t p, uint32_t& qa, uint32_t qa_end, uint32_t& qb, uint32_t qb_end) {
+                const float4 c0 = XY[p], c1 = ZT[p];
+                const f32x2 dx = sub2(ax2, pk2(c0.x, c0.y)), dy = sub2(ay2, pk2(c0.z, c0.w)), dz = sub2(az2, pk2(c1.x, c1.y));
+                float r0, r1, h0, h1;
+                unpk2(fma2(dz, dz, fma2(dy, dy, mul2(dx, dx))), r0, r1);
+                unpk2(fma2(pk2(fmaxf(Ta, c1.z), fmaxf(Ta, c1.w)), one_eps, am2), h0, h1);
+                append_flag(r0, h0, -1.0f, qa, qa_end, 2 * p);           // half_lo < 0: always flagged
+                append_flag(r1, h1, -1.0f, qb, qb_end, 2 * p + 1);
+            };
             for (int q = 0; q < (int)S.nranges; ++q) {
                 const int row = S.r_shift[q][3], ry = row & 3, rz = row >> 2;
                 if (ry < ymin || ry > ymax + 2 || rz < zmin || rz > zmax + 2) continue;
@@ -300,73 +336,64 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
                 // pairs [sa/2, (sb+1)/2): a pair cut by a column boundary brings in a slot of the same row two or
                 // more cells away (never a neighbour, never scanned twice); a range's pad slot is out of reach
                 const uint32_t pa = sa >> 1, pb = (sb + 1u) >> 1;
+                uint32_t p = pa + ((pa ^ (uint32_t)u) & 1u);
                 if (uni) {
-#pragma unroll 4
-                    for (uint32_t p = pa + ((pa ^ (uint32_t)u) & 1u); p < pb; p += 2) {
-                        const float4 c0 = XY[p], c1 = ZT[p];
-                        const f32x2 dx = sub2(ax2, pk2(c0.x, c0.y)), dy = sub2(ay2, pk2(c0.z, c0.w)), dz = sub2(az2, pk2(c1.x, c1.y));
-                        float r0, r1;
-                        unpk2(fma2(dz, dz, fma2(dy, dy, mul2(dx, dx))), r0, r1);
-                        const bool room = lp < lend;
-                        // certain hit <=> 0 < r2 < Ta_lo <=> |r2 - Ta_lo/2| < Ta_lo/2; anything else is flagged for the exact test
-                        append_if(r0 < Ta_hi && room, lp, 2 * p + (fabsf(r0 - half_lo) < half_lo ? 0u : LIST_RECHECK));
-                        append_if(r1 < Ta_hi && room, lp, 2 * p + 1 + (fabsf(r1 - half_lo) < half_lo ? 0u : LIST_RECHECK));
-                    }
+                    if ((p & 2u) && p < pb) { pair_uni(p, bp2, e2, bp3, e3); p += 2; }
+#pragma unroll 2
+                    for (; p + 2 < pb; p += 4) { pair_uni(p, bp0, e0, bp1, e1); pair_uni(p + 2, bp2, e2, bp3, e3); }
+                    if (p < pb) pair_uni(p, bp0, e0, bp1, e1);
                 } else {
-#pragma unroll 4
-                    for (uint32_t p = pa + ((pa ^ (uint32_t)u) & 1u); p < pb; p += 2) {
-                        const float4 c0 = XY[p], c1 = ZT[p];
-                        const f32x2 dx = sub2(ax2, pk2(c0.x, c0.y)), dy = sub2(ay2, pk2(c0.z, c0.w)), dz = sub2(az2, pk2(c1.x, c1.y));
-                        float r0, r1, h0, h1;
-                        unpk2(fma2(dz, dz, fma2(dy, dy, mul2(dx, dx))), r0, r1);
-                        unpk2(fma2(pk2(fmaxf(Ta, c1.z), fmaxf(Ta, c1.w)), one_eps, am2), h0, h1);
-                        const bool room = lp < lend;
-                        append_if(r0 < h0 && room, lp, 2 * p + LIST_RECHECK);
-                        append_if(r1 < h1 && room, lp, 2 * p + 1 + LIST_RECHECK);
-                    }
+                    if ((p & 2u) && p < pb) { pair_gen(p, bp2, e2, bp3, e3); p += 2; }
+#pragma unroll 2
+                    for (; p + 2 < pb; p += 4) { pair_gen(p, bp0, e0, bp1, e1); pair_gen(p + 2, bp2, e2, bp3, e3); }
+                    if (p < pb) pair_gen(p, bp0, e0, bp1, e1);
                 }
             }
-            nl = (lp - lp0) / (2u * TILE_THREADS);
-            if (lp >= lend) s_bad = 1;                                  // flat list full (it may have dropped hits)
         }
-        // ---- classify the provisional hits and drop them into the (thread, bank) buckets.  A hit is certain when its
-        //      fp32 r2 is clear of every support boundary by more than the error bound; otherwise (and at r = 0, which
-        //      includes the target itself) the exact fp64 contract predicate decides (O2/A12).
+        // ---- settle the flagged hits, bucket by bucket, in place.  Certain when the fp32 r2 is clear of every support
+        //      boundary by more than the error bound; otherwise (and at r = 0, which includes the target itself) the
+        //      exact fp64 contract predicate decides (O2/A12).
         uint32_t cnt = 0, ng = 0;                                       // cnt: 4 x 8-bit bucket fills
-        bool ovf = false, coinc = false;
-        for (uint32_t k = 0; k < nl; ++k) {
-            const uint32_t v = Lf[k * TILE_THREADS + tid], s = v & 0x7FFFu;
-            if (s == s_self) continue;
-            bool in_s = true, in_g = true;
-            if (v & LIST_RECHECK) {
-                const float4 c0 = XY[s >> 1], c1 = ZT[s >> 1];
-                const bool od = (s & 1u) != 0;
-                const float dx = fax - (od ? c0.y : c0.x), dy = fay - (od ? c0.w : c0.z), dz = faz - (od ? c1.y : c1.x);
-                const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                const float Tm = fmaxf(Ta, od ? c1.w : c1.z);
-                if (r2 < fmaf(Tm, 0.99999f, -Am) && (r2 < Ta_lo || r2 >= Ta_hi) && r2 > 0.0f) {
-                    in_g = r2 < Ta_lo;
-                } else {
-                    int q = 0;
-                    while (q + 1 < (int)S.nranges && S.r_base[q + 1] <= s) ++q;
-                    const uint32_t gi = S.r_vstart[q] + (s - S.r_base[q]);
-                    const double2 xy = A.p0[gi], zh = A.p1[gi];
-                    const double ex = min_image(__dsub_rn(xa, xy.x), g.per[0], g.L[0], g.halfL[0]);
-                    const double ey = min_image(__dsub_rn(ya, xy.y), g.per[1], g.L[1], g.halfL[1]);
-                    const double ez = min_image(__dsub_rn(za, zh.x), g.per[2], g.L[2], g.halfL[2]);
-                    const double e2 = r2_exact(ex, ey, ez);
-                    in_s = gi != i && e2 < support2(fmax(ha, zh.y));
-                    in_g = in_s && e2 < support2(ha);
-                    if (in_s && !(e2 > 0.0)) coinc = true;              // coincident particles: left to the general kernels (A11)
+        bool ovf = (bp0 >= e0) || (bp1 >= e1) || (bp2 >= e2) || (bp3 >= e3), coinc = false;
+#pragma unroll
+        for (int b = 0; b < 4; ++b) {
+            const uint32_t nb = ((b == 0 ? bp0 : b == 1 ? bp1 : b == 2 ? bp2 : bp3) - (bk0 + b * LIST_BS * BROW)) / BROW;
+            uint16_t* bb = B + (size_t)b * LIST_BS * TILE_THREADS + tid;
+            uint32_t w = 0;
+            for (uint32_t k = 0; k < nb; ++k) {
+                const uint32_t v = bb[k * TILE_THREADS], s = v & 0x7FFFu;
+                bool in_s = true, in_g = true;
+                if (v & LIST_RECHECK) {
+                    const float4 c0 = XY[s >> 1], c1 = ZT[s >> 1];
+                    const bool od = (s & 1u) != 0;
+                    const float dx = fax - (od ? c0.y : c0.x), dy = fay - (od ? c0.w : c0.z), dz = faz - (od ? c1.y : c1.x);
+                    const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                    const float Tm = fmaxf(Ta, od ? c1.w : c1.z);
+                    if (r2 < fmaf(Tm, 0.99999f, -Am) && (r2 < Ta_lo || r2 >= Ta_hi) && r2 > 0.0f) {
+                        in_g = r2 < Ta_lo;
+                    } else if (s == s_self) {
+                        in_s = false;
+                    } else {
+                        int q = 0;
+                        while (q + 1 < (int)S.nranges && S.r_base[q + 1] <= s) ++q;
+                        const uint32_t gi = S.r_vstart[q] + (s - S.r_base[q]);
+                        const double2 xy = A.p0[gi], zh = A.p1[gi];
+                        const double ex = min_image(__dsub_rn(xa, xy.x), g.per[0], g.L[0], g.halfL[0]);
+                        const double ey = min_image(__dsub_rn(ya, xy.y), g.per[1], g.L[1], g.halfL[1]);
+                        const double ez = min_image(__dsub_rn(za, zh.x), g.per[2], g.L[2], g.halfL[2]);
+                        const double e2x = r2_exact(ex, ey, ez);
+                        in_s = gi != i && e2x < support2(fmax(ha, zh.y));
+                        in_g = in_s && e2x < support2(ha);
+                        if (in_s && !(e2x > 0.0)) coinc = true;         // coincident particles: left to the general kernels (A11)
+                    }
+                    if (in_s) bb[w * TILE_THREADS] = (uint16_t)s;
+                } else if (w != k) {
+                    bb[w * TILE_THREADS] = (uint16_t)s;
                 }
+                w += in_s ? 1u : 0u;
+                ng += (in_s && in_g) ? 1u : 0u;
             }
-            if (in_s) {
-                const int b = bank_local((int)(s & 7u));
-                const uint32_t kk = (cnt >> (8 * b)) & 0xFFu;
-                if (kk < (uint32_t)LIST_BC) { B[(b * LIST_BC + kk) * TILE_THREADS + tid] = (uint16_t)s; cnt += 1u << (8 * b); }
-                else ovf = true;
-                ng += in_g ? 1u : 0u;
-            }
+            cnt |= w << (8 * b);
         }
         if (ovf || coinc) s_bad = 1;
         // ---- split every bank bucket of the target between its two threads (alternate entries)
@@ -422,7 +449,7 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
                 const uint32_t start = ((uint32_t)t * R) >> 3;
                 const uint32_t own = get8(cu, beta) - get8(ov0, beta);
                 // my entries of bank beta: indices f, f+2, ... of the bucket of thread bank_owner(beta)
-                const uint16_t* bp = Bp + (bank_local(beta) * LIST_BC + ((u + beta) & 1)) * TILE_THREADS + bank_owner(beta);
+                const uint16_t* bp = Bp + (bank_local(beta) * LIST_BS + ((u + beta) & 1)) * TILE_THREADS + bank_owner(beta);
                 for (uint32_t k = 0; k < own; ++k) out[(start + k) * TILE_THREADS] = bp[2 * k * TILE_THREADS];
             }
             // pass 2: the holes take the overflow entries bank by bank, then dummies
@@ -435,7 +462,7 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
                     uint32_t item = (uint32_t)(TILE_CMAX + beta);       // dummy slot of this phase's bank
                     if (ovtot) {
                         while (k2 == kend) { ++b2; kend = get8(cu, b2); k2 = kend - get8(ov0, b2); }
-                        item = Bp[(bank_local(b2) * LIST_BC + ((u + b2) & 1) + 2 * k2) * TILE_THREADS + bank_owner(b2)];
+                        item = Bp[(bank_local(b2) * LIST_BS + ((u + b2) & 1) + 2 * k2) * TILE_THREADS + bank_owner(b2)];
                         ++k2; --ovtot;
                     }
                     out[r * TILE_THREADS] = (uint16_t)item;
