@@ -263,12 +263,13 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
         const bool active = tgt < (int)td.nt;
         uint32_t i = 0, s_self = 0xFFFFFFFFu;
         double xa = 0, ya = 0, za = 0, ha = 0;
-        int tcol = 0, trow = 0;
+        int tcol = 0, try_ = 0, trz = 0;
         if (active) {
             int e;
             i = tile_target(td, S, tgt, &e);
-            const int nrows = td.nyr * td.nzr;
-            tcol = e / nrows; trow = e % nrows;
+            int cxe;
+            tile_cell_rc(td, e, cxe, try_, trz);
+            tcol = cxe - td.cxa;
             const double2 xy = A.p0[i], zh = A.p1[i];
             xa = xy.x; ya = xy.y; za = zh.x; ha = zh.y;
             for (int q = 0; q < (int)S.nranges; ++q)
@@ -281,8 +282,8 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
         const float Ta_hi = fmaf(Ta, 1.00001f, Am), Ta_lo = fmaf(Ta, 0.99999f, -Am);
         // warp window in virtual columns / candidate rows
         int cmin = active ? tcol : 1 << 20, cmax = active ? tcol : -1;
-        int ymin = active ? trow % td.nyr : 4, ymax = active ? trow % td.nyr : -1;
-        int zmin = active ? trow / td.nyr : 4, zmax = active ? trow / td.nyr : -1;
+        int ymin = active ? try_ : 4, ymax = active ? try_ : -1;
+        int zmin = active ? trz : 4, zmax = active ? trz : -1;
 #pragma unroll
         for (int o = 16; o; o >>= 1) {
             cmin = min(cmin, __shfl_xor_sync(0xFFFFFFFFu, cmin, o)); cmax = max(cmax, __shfl_xor_sync(0xFFFFFFFFu, cmax, o));
@@ -339,7 +340,7 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
                 uint32_t p = pa + ((pa ^ (uint32_t)u) & 1u);
                 if (uni) {
                     if ((p & 2u) && p < pb) { pair_uni(p, bp2, e2, bp3, e3); p += 2; }
-#pragma unroll 2
+#pragma unroll 4
                     for (; p + 2 < pb; p += 4) { pair_uni(p, bp0, e0, bp1, e1); pair_uni(p + 2, bp2, e2, bp3, e3); }
                     if (p < pb) pair_uni(p, bp0, e0, bp1, e1);
                 } else {
@@ -450,6 +451,7 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
                 const uint32_t own = get8(cu, beta) - get8(ov0, beta);
                 // my entries of bank beta: indices f, f+2, ... of the bucket of thread bank_owner(beta)
                 const uint16_t* bp = Bp + (bank_local(beta) * LIST_BS + ((u + beta) & 1)) * TILE_THREADS + bank_owner(beta);
+#pragma unroll 4
                 for (uint32_t k = 0; k < own; ++k) out[(start + k) * TILE_THREADS] = bp[2 * k * TILE_THREADS];
             }
             // pass 2: the holes take the overflow entries bank by bank, then dummies
@@ -469,6 +471,7 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
                 }
             }
             uint2* blk = A.pool + off + lane;
+#pragma unroll 2
             for (uint32_t r4 = 0; r4 < R; r4 += 4) {
                 const uint32_t e0 = out[r4 * TILE_THREADS], e1 = out[(r4 + 1) * TILE_THREADS];
                 const uint32_t e2 = out[(r4 + 2) * TILE_THREADS], e3 = out[(r4 + 3) * TILE_THREADS];

@@ -118,6 +118,18 @@ __device__ __forceinline__ bool tile_range(const TileDesc& td, const DevGrid& g,
     return tile_range(td.y0, td.z0, td.nyr, td.nzr, td.cxa, td.cxb, g, ct, row, piece, R);
 }
 
+// Cell e of the tile's target enumeration: column-major, and within a column the 2 x 2 rows in serpentine (Gray)
+// order, reversed in odd columns, so that consecutive cells always share a face.  A warp's 16 consecutive targets
+// then straddle two face-adjacent cells at worst and its candidate window is 36 cells instead of up to 64.
+__device__ __forceinline__ void tile_cell_rc(const TileDesc& td, int e, int& cx, int& ry, int& rz) {
+    const int nrows = td.nyr * td.nzr;
+    cx = td.cxa + e / nrows;
+    int r = e % nrows;
+    if (cx & 1) r = nrows - 1 - r;
+    rz = r / td.nyr; ry = r % td.nyr;
+    if (rz & 1) ry = td.nyr - 1 - ry;
+}
+
 // Fills S.  Must be called by all threads of the CTA (blockDim.x >= 32 + TILE_MAXCELL); ends with __syncthreads().
 __device__ __forceinline__ void tile_setup(const TileDesc& td, const DevGrid& g, const CellTable& ct, TileS& S) {
     const int tid = threadIdx.x;
@@ -143,14 +155,15 @@ __device__ __forceinline__ void tile_setup(const TileDesc& td, const DevGrid& g,
         const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31);
         if (tid == 0) { S.nranges = __popc(mask); S.ncand = total; S.r_base[__popc(mask)] = total; }
     }
-    // target cells, column-major: e = (cx - cxa) * nrows + r, r = rz * nyr + ry
+    // target cells, column-major with serpentine rows (tile_cell_rc)
     const int nrows = td.nyr * td.nzr;
     const int ncells = (td.cxb - td.cxa + 1) * nrows;
     if (tid >= 32 && tid < 32 + TILE_MAXCELL) {
         const int e = tid - 32;
         if (e < ncells) {
-            const int cx = td.cxa + e / nrows, r = e % nrows;
-            const uint32_t c = cell_id(g, cx, td.y0 + r % td.nyr, td.z0 + r / td.nyr);
+            int cx, ry, rz;
+            tile_cell_rc(td, e, cx, ry, rz);
+            const uint32_t c = cell_id(g, cx, td.y0 + ry, td.z0 + rz);
             const uint32_t a = ct.cell_start[c], b = ct.cell_end[c];
             S.c_first[e] = a;
             S.c_pre[e + 1] = b - a;          // counts, scanned below
