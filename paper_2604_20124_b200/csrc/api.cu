@@ -332,7 +332,8 @@ int spray_neighbor_counts(spray_ctx* ctx, int symmetric, uint32_t* count, void* 
     NEED_BUILT();
     Ctx* c = &ctx->c;
     if (c->n > 0 && !count) return fail(c, SPRAY_ERR_INVALID_ARG, "spray_neighbor_counts: NULL argument");
-    SweepArgs a = base_args(c);
+    CK(launch_tiled_export(c, 0, symmetric, count, nullptr, nullptr, nullptr, nullptr, (cudaStream_t)stream), "neighbour counts from the tiled lists");
+    SweepArgs a = fallback_args(c);
     a.symmetric = symmetric; a.ocount = count;
     CK(launch_ref_sweep(c, SW_COUNT, a, (cudaStream_t)stream), "neighbour count sweep");
     return SPRAY_OK;
@@ -342,7 +343,8 @@ int spray_neighbor_lists(spray_ctx* ctx, int symmetric, const uint64_t* offsets,
     NEED_BUILT();
     Ctx* c = &ctx->c;
     if (c->n > 0 && (!offsets || !nbr)) return fail(c, SPRAY_ERR_INVALID_ARG, "spray_neighbor_lists: NULL argument");
-    SweepArgs a = base_args(c);
+    CK(launch_tiled_export(c, 1, symmetric, nullptr, offsets, nbr, nullptr, nullptr, (cudaStream_t)stream), "neighbour lists from the tiled lists");
+    SweepArgs a = fallback_args(c);
     a.symmetric = symmetric; a.offsets = offsets; a.onbr = nbr;
     CK(launch_ref_sweep(c, SW_LIST, a, (cudaStream_t)stream), "neighbour list sweep");
     return SPRAY_OK;
@@ -352,7 +354,8 @@ int spray_neighbor_digest(spray_ctx* ctx, int symmetric, uint64_t* dsum, uint64_
     NEED_BUILT();
     Ctx* c = &ctx->c;
     if (c->n > 0 && (!dsum || !dxor)) return fail(c, SPRAY_ERR_INVALID_ARG, "spray_neighbor_digest: NULL argument");
-    SweepArgs a = base_args(c);
+    CK(launch_tiled_export(c, 2, symmetric, nullptr, nullptr, nullptr, dsum, dxor, (cudaStream_t)stream), "neighbour digests from the tiled lists");
+    SweepArgs a = fallback_args(c);
     a.symmetric = symmetric; a.odsum = dsum; a.odxor = dxor;
     CK(launch_ref_sweep(c, SW_DIGEST, a, (cudaStream_t)stream), "neighbour digest sweep");
     return SPRAY_OK;

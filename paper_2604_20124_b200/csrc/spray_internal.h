@@ -129,6 +129,9 @@ struct TiledArgs {
 };
 cudaError_t launch_build_tiles(Ctx* c, cudaStream_t st);
 cudaError_t launch_tiled_sweep(Ctx* c, int sweep, const TiledArgs& a, cudaStream_t st);
+// parity exports from the tiled lists: mode 0 = counts, 1 = CSR lists, 2 = digests (tiles.cu)
+cudaError_t launch_tiled_export(Ctx* c, int mode, int symmetric, uint32_t* ocount, const uint64_t* offsets, uint32_t* onbr,
+                                uint64_t* odsum, uint64_t* odxor, cudaStream_t st);
 
 // ---- probe.cu
 cudaError_t launch_fp64_probe(int blocks, int threads, int64_t iters, double* out, cudaStream_t st);

@@ -488,6 +488,124 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
     }
 }
 
+// ------------------------------------------------------------------------------------------- parity exports
+// spray_neighbor_counts / _lists / _digest served FROM THE TILED LISTS for the particles the tiled kernels serve, so
+// that the parity tests compare the very lists the sweeps run on with the oracle's sets (the general kernel does the
+// rest).  N_sym is the list itself; N_gather(a) is its subset with r2 < 4 h_a^2, decided by the exact contract
+// predicate on the fp64 coordinates (O2/A12).  Not on the hot path.
+struct ExportArgs {
+    const double2 *p0, *p1;
+    const uint32_t* perm;
+    const TileDesc* tiles;
+    const uint32_t* tiletab;
+    const unsigned long long* ctr;
+    const uint2* pool;
+    const uint2* winfo;
+    const uint32_t* tflags;
+    int symmetric;
+    uint32_t* ocount;                  // mode 0
+    const uint64_t* offsets;           // mode 1
+    uint32_t* onbr;
+    uint64_t *odsum, *odxor;           // mode 2
+};
+
+template <int MODE>
+__global__ void __launch_bounds__(TILE_THREADS, 1)
+k_tiled_export(DevGrid g, ExportArgs A) {
+    __shared__ TileS S;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int u = tid & 1, tgt = tid >> 1;
+    const uint32_t ntiles = (uint32_t)A.ctr[CTR_NTILES];
+    for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        if (!(A.tflags[tile] & TILE_FLAG_OK)) continue;
+        const TileDesc td = A.tiles[tile];
+        __syncthreads();
+        {
+            const uint32_t* src = A.tiletab + (size_t)tile * TILES_WORDS;
+            uint32_t* dst = reinterpret_cast<uint32_t*>(&S);
+            for (int w = tid; w < TILES_WORDS; w += TILE_THREADS) dst[w] = src[w];
+        }
+        __syncthreads();
+        const bool active = tgt < (int)td.nt;
+        uint32_t i = 0;
+        double xa = 0, ya = 0, za = 0, ha = 0;
+        if (active) {
+            i = tile_target(td, S, tgt);
+            const double2 xy = A.p0[i], zh = A.p1[i];
+            xa = xy.x; ya = xy.y; za = zh.x; ha = zh.y;
+        }
+        const uint2 wi = A.winfo[(size_t)tile * TILE_WARPS + warp];
+        const uint2* lp = A.pool + wi.x + lane;
+        uint32_t cnt = 0;
+        uint64_t dsum = 0, dxr = 0;
+        // mode 1 needs the first half's count before the second half writes: two passes (count, then write)
+        for (int pass = 0; pass < (MODE == 1 ? 2 : 1); ++pass) {
+            uint32_t wpos = 0;
+            if (MODE == 1 && pass == 1) {
+                const uint32_t other = __shfl_xor_sync(0xFFFFFFFFu, cnt, 1);
+                wpos = u ? other : 0u;                     // thread 1 writes after thread 0's entries
+            }
+            const uint64_t lbase = (MODE == 1 && active) ? A.offsets[A.perm[i]] : 0;
+            uint32_t c2 = 0;
+            for (uint32_t r = 0; r < wi.y; ++r) {
+                const uint2 w4 = lp[(size_t)(r >> 2) * 32];
+                const uint32_t half = (r & 2u) ? w4.y : w4.x;
+                const uint32_t s = (r & 1u) ? (half >> 16) : (half & 0xFFFFu);
+                if (s >= (uint32_t)TILE_CMAX || !active) continue;             // dummy entry
+                int q = 0;
+                while (q + 1 < (int)S.nranges && S.r_base[q + 1] <= s) ++q;
+                const uint32_t gi = S.r_vstart[q] + (s - S.r_base[q]);
+                if (!A.symmetric) {
+                    const double2 xy = A.p0[gi], zh = A.p1[gi];
+                    const double ex = min_image(__dsub_rn(xa, xy.x), g.per[0], g.L[0], g.halfL[0]);
+                    const double ey = min_image(__dsub_rn(ya, xy.y), g.per[1], g.L[1], g.halfL[1]);
+                    const double ez = min_image(__dsub_rn(za, zh.x), g.per[2], g.L[2], g.halfL[2]);
+                    if (!(r2_exact(ex, ey, ez) < support2(ha))) continue;
+                }
+                const uint32_t id = A.perm[gi];
+                if (MODE == 1 && pass == 1) A.onbr[lbase + wpos + c2] = id;
+                if (MODE == 2) { const uint64_t hsh = mix64((uint64_t)id); dsum += hsh; dxr ^= hsh; }
+                ++c2;
+            }
+            cnt = c2;
+        }
+        const uint32_t total = cnt + __shfl_xor_sync(0xFFFFFFFFu, cnt, 1);
+        if (MODE == 2) {
+            dsum += __shfl_xor_sync(0xFFFFFFFFu, dsum, 1);
+            dxr ^= __shfl_xor_sync(0xFFFFFFFFu, dxr, 1);
+        }
+        if (MODE == 1) __syncwarp();
+        if (active && u == 0) {
+            const uint32_t ia = A.perm[i];
+            if (MODE == 0) A.ocount[ia] = total;
+            if (MODE == 2) { A.odsum[ia] = dsum; A.odxor[ia] = dxr; }
+            if (MODE == 1) {               // ascending caller ids (debug export: insertion sort of this particle's segment)
+                __threadfence_block();
+                uint32_t* L = A.onbr + A.offsets[ia];
+                for (uint32_t a = 1; a < total; ++a) {
+                    uint32_t v = L[a]; int b = (int)a - 1;
+                    while (b >= 0 && L[b] > v) { L[b + 1] = L[b]; --b; }
+                    L[b + 1] = v;
+                }
+            }
+        }
+    }
+}
+
+cudaError_t launch_tiled_export(Ctx* c, int mode, int symmetric, uint32_t* ocount, const uint64_t* offsets, uint32_t* onbr,
+                                uint64_t* odsum, uint64_t* odxor, cudaStream_t st) {
+    if (c->n == 0 || !c->tl.enabled) return cudaSuccess;
+    const Tiled& t = c->tl;
+    ExportArgs A{c->pk.p0, c->pk.p1, c->perm, t.tiles, t.tiletab, t.ctr, t.pool, t.winfo, t.tflags, symmetric,
+                 ocount, offsets, onbr, odsum, odxor};
+    const int grid = t.sms * 2;
+    if (mode == 0) k_tiled_export<0><<<grid, TILE_THREADS, 0, st>>>(c->dg, A);
+    else if (mode == 1) k_tiled_export<1><<<grid, TILE_THREADS, 0, st>>>(c->dg, A);
+    else k_tiled_export<2><<<grid, TILE_THREADS, 0, st>>>(c->dg, A);
+    c->launches += 1;
+    return cudaGetLastError();
+}
+
 // ------------------------------------------------------------------------------------------- launcher
 cudaError_t launch_build_tiles(Ctx* c, cudaStream_t st) {
     Tiled& t = c->tl;
