@@ -191,15 +191,78 @@ __device__ __forceinline__ void pair_body(const double2* __restrict__ F, const d
     }
 }
 
+// Hydro pairs in groups: the branch-free part of every pair of the group first (so the compiler can interleave
+// their dependency chains), then ONE branch for the group's viscous corrections (taken only if some pair approaches),
+// then the accumulations.  Same arithmetic as pair_body<SW_HYDRO>.
+struct HydroPair { double dx, dy, dz, y, r, Ga, Gb, c, vr, Vb; uint32_t s; };
+
+template <int KERNEL, bool UNI>
+__device__ __forceinline__ void hydro_common(const double2* __restrict__ F, uint32_t s, const Tgt& T, HydroPair& h) {
+    const double2 d0 = F[s], d1 = F[TILE_CMAXP + s];
+    const double2 d2 = F[2 * TILE_CMAXP + s], d3 = F[3 * TILE_CMAXP + s];
+    h.s = s;
+    h.dx = T.x - d0.x; h.dy = T.y - d0.y; h.dz = T.z - d1.x;
+    const double r2 = fma(h.dz, h.dz, fma(h.dy, h.dy, h.dx * h.dx));
+    h.y = rsqrt_fast(r2);
+    h.r = r2 * h.y;
+    h.Vb = d1.y;
+    const double dvx = T.c3 - d2.y, dvy = T.c4 - d3.x, dvz = T.c5 - d3.y;
+    h.vr = fma(dvz, h.dz, fma(dvy, h.dy, dvx * h.dx));                   // v_ab . x_ab = w r
+    if (UNI) {
+        h.Ga = gshape<KERNEL, false>(h.r * T.hinv) * h.y;                // F / (r kFn/h^4)
+        h.Gb = h.Ga;
+        // eq. (11) P:L98 with the sign of eq. (5) (A3): -(m_b/(rho_a rho_b)) (p_a F_a + p_b F_b) x_ab / r
+        h.c = fma(h.Vb, T.c0, d2.x * T.c1);
+    } else {
+        const double2 d5 = F[5 * TILE_CMAXP + s];
+        h.Ga = (gshape<KERNEL, true>(h.r * T.hinv) * h.y) * T.fn;
+        h.Gb = (gshape<KERNEL, true>(h.r * d5.x) * h.y) * d5.y;
+        h.c = fma(h.Vb * T.c0, h.Ga, (d2.x * T.c1) * h.Gb);
+    }
+}
+template <bool UNI>
+__device__ __forceinline__ void hydro_visc(const double2* __restrict__ F, const Tgt& T, double beta, HydroPair& h, Acc& acc) {
+    // eqs. (41)-(43) P:L236-L242 (A6, A7, A8)
+    const double2 d4 = F[4 * TILE_CMAXP + h.s];
+    const double w = h.vr * h.y, hw = 0.5 * w;
+    const double vsa = fma(-beta, w, T.c2), vsb = fma(-beta, w, d4.y);
+    if (UNI) h.c = fma(-hw, fma(d4.x * T.c1, vsa, h.Vb * vsb), h.c);
+    else h.c = fma(-hw, fma((d4.x * T.c1) * vsa, h.Ga, (h.Vb * vsb) * h.Gb), h.c);
+    acc.a4 = fma((hw * w) * (d4.x * vsa), h.Ga * h.r, acc.a4);
+}
+template <bool UNI>
+__device__ __forceinline__ void hydro_accum(const HydroPair& h, Acc& acc) {
+    const double cg = UNI ? h.c * h.Ga : h.c;
+    acc.a0 = fma(cg, h.dx, acc.a0); acc.a1 = fma(cg, h.dy, acc.a1); acc.a2 = fma(cg, h.dz, acc.a2);
+    acc.a3 = fma(h.Vb * h.Ga, h.vr, acc.a3);                             // eq. (37)
+}
+template <int KERNEL, bool UNI>
+__device__ __forceinline__ void hydro_group2(const double2* __restrict__ F, uint32_t s0, uint32_t s1, const Tgt& T, double beta, Acc& acc) {
+    HydroPair h0, h1;
+    hydro_common<KERNEL, UNI>(F, s0, T, h0);
+    hydro_common<KERNEL, UNI>(F, s1, T, h1);
+    if (fmin(h0.vr, h1.vr) < 0.0) {
+        if (h0.vr < 0.0) hydro_visc<UNI>(F, T, beta, h0, acc);
+        if (h1.vr < 0.0) hydro_visc<UNI>(F, T, beta, h1, acc);
+    }
+    hydro_accum<UNI>(h0, acc);
+    hydro_accum<UNI>(h1, acc);
+}
+
 template <int SWEEP, int KERNEL, bool UNI>
 __device__ __forceinline__ void pair_loop(const double2* __restrict__ F, const double* __restrict__ Ee, const uint2* __restrict__ lp,
                                           uint32_t R, uint2 cur, uint2 nxt, const Tgt& T, double beta, bool sym, Acc& acc) {
     for (uint32_t r4 = 0; r4 < R; r4 += 4) {
         const uint2 nx2 = (r4 + 8 < R) ? __ldcs(lp + (size_t)(r4 / 4 + 2) * 32) : make_uint2(0u, 0u);
-        pair_body<SWEEP, KERNEL, UNI>(F, Ee, cur.x & 0xFFFFu, T, beta, sym, acc);
-        pair_body<SWEEP, KERNEL, UNI>(F, Ee, cur.x >> 16, T, beta, sym, acc);
-        pair_body<SWEEP, KERNEL, UNI>(F, Ee, cur.y & 0xFFFFu, T, beta, sym, acc);
-        pair_body<SWEEP, KERNEL, UNI>(F, Ee, cur.y >> 16, T, beta, sym, acc);
+        if (SWEEP == SW_HYDRO) {
+            hydro_group2<KERNEL, UNI>(F, cur.x & 0xFFFFu, cur.x >> 16, T, beta, acc);
+            hydro_group2<KERNEL, UNI>(F, cur.y & 0xFFFFu, cur.y >> 16, T, beta, acc);
+        } else {
+            pair_body<SWEEP, KERNEL, UNI>(F, Ee, cur.x & 0xFFFFu, T, beta, sym, acc);
+            pair_body<SWEEP, KERNEL, UNI>(F, Ee, cur.x >> 16, T, beta, sym, acc);
+            pair_body<SWEEP, KERNEL, UNI>(F, Ee, cur.y & 0xFFFFu, T, beta, sym, acc);
+            pair_body<SWEEP, KERNEL, UNI>(F, Ee, cur.y >> 16, T, beta, sym, acc);
+        }
         cur = nxt; nxt = nx2;
     }
 }

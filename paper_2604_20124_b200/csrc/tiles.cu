@@ -170,18 +170,23 @@ __device__ __forceinline__ void append_if(bool hit, uint32_t& addr, uint32_t v) 
 }
 
 // One candidate of the scan: if r2 < hi, store (value | LIST_RECHECK unless 0 < r2 < 2 half_lo) at the bucket row pointer and
-// advance it, clamped at `end` (the bucket's trash row: a pointer that reaches it reports the overflow).  No branches.
-__device__ __forceinline__ void append_flag(float r2, float hi, float half_lo, uint32_t& addr, uint32_t end, uint32_t v) {
-    asm volatile("{\n\t.reg .pred p, s;\n\t.reg .f32 t;\n\t.reg .b32 w;\n\t"
-                 "setp.lt.f32 p, %1, %2;\n\t"
-                 "sub.f32 t, %1, %3;\n\t"
+// advance it, clamped at `end` (the bucket's trash row: a pointer that reaches it reports the overflow); nflag counts
+// the flagged hits.  No branches.
+__device__ __forceinline__ void append_flag(float r2, float hi, float half_lo, uint32_t& addr, uint32_t end, uint32_t v, uint32_t& nflag) {
+    asm volatile("{\n\t.reg .pred p, s, q;\n\t.reg .f32 t;\n\t.reg .b32 w;\n\t"
+                 "setp.lt.f32 p, %2, %3;\n\t"
+                 "sub.f32 t, %2, %4;\n\t"
                  "abs.f32 t, t;\n\t"
-                 "setp.lt.f32 s, t, %3;\n\t"
-                 "selp.b32 w, %5, %6, s;\n\t"
+                 "setp.lt.f32 s, t, %4;\n\t"
+                 "setp.ge.and.f32 q, t, %4, p;\n\t"
+                 "selp.b32 w, %6, %7, s;\n\t"
                  "@p st.shared.u16 [%0], w;\n\t"
-                 "@p add.u32 %0, %0, %7;\n\t"
-                 "min.u32 %0, %0, %4;\n\t}"
-                 : "+r"(addr) : "f"(r2), "f"(hi), "f"(half_lo), "r"(end), "r"(v), "r"(v | LIST_RECHECK), "n"(2 * TILE_THREADS) : "memory");
+                 "@p add.u32 %0, %0, %8;\n\t"
+                 "@q add.u32 %1, %1, 1;\n\t"
+                 "min.u32 %0, %0, %5;\n\t}"
+                 : "+r"(addr), "+r"(nflag) : "f"(r2), "f"(hi), "f"(half_lo), "r"(end), "r"(v), "r"(v | LIST_RECHECK), "n"(2 * TILE_THREADS));
+    // no memory clobber: the loads of the next pairs must be free to move above the store; the buckets are read back
+    // only after the fence that follows the scan
 }
 
 // Which thread of a target owns bank beta in the scan (threads split the candidate PAIRS: slots 4i+2u, 4i+2u+1), and
@@ -301,6 +306,7 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
         //      (0 < r2 < Ta_lo, uniform-h tiles only) carries LIST_RECHECK.
         const uint32_t bk0 = (uint32_t)__cvta_generic_to_shared(B + tid);
         constexpr uint32_t BROW = 2u * TILE_THREADS;                    // bytes per bucket row
+        uint32_t nflag = 0;                                             // flagged hits of this thread
         uint32_t bp0 = bk0, bp1 = bk0 + LIST_BS * BROW, bp2 = bk0 + 2 * LIST_BS * BROW, bp3 = bk0 + 3 * LIST_BS * BROW;
         const uint32_t e0 = bk0 + LIST_BC * BROW, e1 = e0 + LIST_BS * BROW, e2 = e1 + LIST_BS * BROW, e3 = e2 + LIST_BS * BROW;
         if (cmax >= 0) {
@@ -314,8 +320,8 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
                 const f32x2 dx = sub2(ax2, pk2(c0.x, c0.y)), dy = sub2(ay2, pk2(c0.z, c0.w)), dz = sub2(az2, pk2(c1.x, c1.y));
                 float r0, r1;
                 unpk2(fma2(dz, dz, fma2(dy, dy, mul2(dx, dx))), r0, r1);
-                append_flag(r0, Ta_hi, half_lo, qa, qa_end, 2 * p);
-                append_flag(r1, Ta_hi, half_lo, qb, qb_end, 2 * p + 1);
+                append_flag(r0, Ta_hi, half_lo, qa, qa_end, 2 * p, nflag);
+                append_flag(r1, Ta_hi, half_lo, qb, qb_end, 2 * p + 1, nflag);
             };
             auto pair_gen = [&](uint32_t p, uint32_t& qa, uint32_t qa_end, uint32_t& qb, uint32_t qb_end) {
                 const float4 c0 = XY[p], c1 = ZT[p];
@@ -323,8 +329,8 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
                 float r0, r1, h0, h1;
                 unpk2(fma2(dz, dz, fma2(dy, dy, mul2(dx, dx))), r0, r1);
                 unpk2(fma2(pk2(fmaxf(Ta, c1.z), fmaxf(Ta, c1.w)), one_eps, am2), h0, h1);
-                append_flag(r0, h0, -1.0f, qa, qa_end, 2 * p);           // half_lo < 0: always flagged
-                append_flag(r1, h1, -1.0f, qb, qb_end, 2 * p + 1);
+                append_flag(r0, h0, -1.0f, qa, qa_end, 2 * p, nflag);    // half_lo < 0: always flagged
+                append_flag(r1, h1, -1.0f, qb, qb_end, 2 * p + 1, nflag);
             };
             for (int q = 0; q < (int)S.nranges; ++q) {
                 const int row = S.r_shift[q][3], ry = row & 3, rz = row >> 2;
@@ -351,11 +357,33 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
                 }
             }
         }
+        asm volatile("" ::: "memory");                                  // the appends above wrote the buckets
         // ---- settle the flagged hits, bucket by bucket, in place.  Certain when the fp32 r2 is clear of every support
         //      boundary by more than the error bound; otherwise (and at r = 0, which includes the target itself) the
         //      exact fp64 contract predicate decides (O2/A12).
         uint32_t cnt = 0, ng = 0;                                       // cnt: 4 x 8-bit bucket fills
         bool ovf = (bp0 >= e0) || (bp1 >= e1) || (bp2 >= e2) || (bp3 >= e3), coinc = false;
+        // In a uniform-h tile the target itself (r = 0) is normally the only flagged hit, met by the thread that scans its
+        // slot pair: then the settle pass is a removal of that one entry from its bucket.
+        const bool sees_self = active && (((s_self >> 1) & 1u) == (uint32_t)u);
+        const bool full_settle = __any_sync(0xFFFFFFFFu, nflag != (sees_self ? 1u : 0u));
+        if (!full_settle) {
+            const uint32_t n0 = (bp0 - bk0) / BROW, n1 = (bp1 - (bk0 + LIST_BS * BROW)) / BROW;
+            const uint32_t n2 = (bp2 - (bk0 + 2 * LIST_BS * BROW)) / BROW, n3 = (bp3 - (bk0 + 3 * LIST_BS * BROW)) / BROW;
+            cnt = n0 | (n1 << 8) | (n2 << 16) | (n3 << 24);
+            if (sees_self) {
+                const int b = bank_local((int)(s_self & 7u));
+                uint16_t* bb = B + (size_t)b * LIST_BS * TILE_THREADS + tid;
+                const uint32_t nb = (cnt >> (8 * b)) & 0xFFu;
+                uint32_t k = 0;
+                while (k < nb && (bb[k * TILE_THREADS] & 0x7FFFu) != s_self) ++k;
+                if (k < nb) {                                           // the last entry takes its place (order is free)
+                    bb[k * TILE_THREADS] = bb[(nb - 1) * TILE_THREADS];
+                    cnt -= 1u << (8 * b);
+                }
+            }
+            ng = (cnt & 0xFFu) + ((cnt >> 8) & 0xFFu) + ((cnt >> 16) & 0xFFu) + (cnt >> 24);
+        } else
 #pragma unroll
         for (int b = 0; b < 4; ++b) {
             const uint32_t nb = ((b == 0 ? bp0 : b == 1 ? bp1 : b == 2 ? bp2 : bp3) - (bk0 + b * LIST_BS * BROW)) / BROW;
@@ -444,37 +472,38 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
             // schedule into my (now free) flat-list column, then pack 4 rounds per 8-byte store
             uint16_t* out = Lf + tid;                                   // out[r * TILE_THREADS]
             const uint16_t* Bp = B + (tid & ~1);
-            // pass 1: every phase takes its own bank's entries (up to its capacity)
+            // pass 1 (lockstep, R rounds): every phase takes its own bank's entries up to its capacity; a hole gets the
+            // dummy slot of the phase's bank (any value >= TILE_CMAX marks a hole)
+#pragma unroll
             for (int t = 0; t < 8; ++t) {
                 const int beta = (j + t) & 7;
-                const uint32_t start = ((uint32_t)t * R) >> 3;
+                const uint32_t start = ((uint32_t)t * R) >> 3, cap = (((uint32_t)(t + 1) * R) >> 3) - start;
                 const uint32_t own = get8(cu, beta) - get8(ov0, beta);
                 // my entries of bank beta: indices f, f+2, ... of the bucket of thread bank_owner(beta)
                 const uint16_t* bp = Bp + (bank_local(beta) * LIST_BS + ((u + beta) & 1)) * TILE_THREADS + bank_owner(beta);
-#pragma unroll 4
-                for (uint32_t k = 0; k < own; ++k) out[(start + k) * TILE_THREADS] = bp[2 * k * TILE_THREADS];
-            }
-            // pass 2: the holes take the overflow entries bank by bank, then dummies
-            int b2 = -1;
-            uint32_t k2 = 0, kend = 0;
-            for (int t = 0; t < 8; ++t) {
-                const int beta = (j + t) & 7;
-                const uint32_t end = ((uint32_t)(t + 1) * R) >> 3;
-                for (uint32_t r = (((uint32_t)t * R) >> 3) + get8(cu, beta) - get8(ov0, beta); r < end; ++r) {
-                    uint32_t item = (uint32_t)(TILE_CMAX + beta);       // dummy slot of this phase's bank
-                    if (ovtot) {
-                        while (k2 == kend) { ++b2; kend = get8(cu, b2); k2 = kend - get8(ov0, b2); }
-                        item = Bp[(bank_local(b2) * LIST_BS + ((u + b2) & 1) + 2 * k2) * TILE_THREADS + bank_owner(b2)];
-                        ++k2; --ovtot;
-                    }
-                    out[r * TILE_THREADS] = (uint16_t)item;
+                const uint16_t dummy = (uint16_t)(TILE_CMAX + beta);
+                for (uint32_t k = 0; k < cap; ++k) {
+                    uint16_t item = dummy;
+                    if (k < own) item = bp[2 * k * TILE_THREADS];
+                    out[(start + k) * TILE_THREADS] = item;
                 }
             }
+            // pass 2: pack 4 rounds per 8-byte store; the holes take the overflow entries bank by bank while there are any
+            int b2 = -1;
+            uint32_t k2 = 0, kend = 0;
+            auto fill = [&](uint32_t e) -> uint32_t {
+                if (e >= (uint32_t)TILE_CMAX && ovtot) {
+                    while (k2 == kend) { ++b2; kend = get8(cu, b2); k2 = kend - get8(ov0, b2); }
+                    e = Bp[(bank_local(b2) * LIST_BS + ((u + b2) & 1) + 2 * k2) * TILE_THREADS + bank_owner(b2)];
+                    ++k2; --ovtot;
+                }
+                return e;
+            };
             uint2* blk = A.pool + off + lane;
-#pragma unroll 2
             for (uint32_t r4 = 0; r4 < R; r4 += 4) {
-                const uint32_t e0 = out[r4 * TILE_THREADS], e1 = out[(r4 + 1) * TILE_THREADS];
-                const uint32_t e2 = out[(r4 + 2) * TILE_THREADS], e3 = out[(r4 + 3) * TILE_THREADS];
+                uint32_t e0 = out[r4 * TILE_THREADS], e1 = out[(r4 + 1) * TILE_THREADS];
+                uint32_t e2 = out[(r4 + 2) * TILE_THREADS], e3 = out[(r4 + 3) * TILE_THREADS];
+                if (ovtot) { e0 = fill(e0); e1 = fill(e1); e2 = fill(e2); e3 = fill(e3); }
                 blk[(size_t)(r4 >> 2) * 32] = make_uint2(e0 | (e1 << 16), e2 | (e3 << 16));
             }
             if (u == 0) A.lcount[(size_t)tile * TILE_T + tgt] = active ? (ng | (nsym << 16)) : 0u;
