@@ -315,8 +315,7 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
             const f32x2 one_eps = pk2(1.00001f, 1.00001f), am2 = pk2(Am, Am);
             const float half_lo = 0.5f * Ta_lo;
             // one pair: test both slots, append to buckets (pa_, pb_) whose row pointers are clamped at the trash row
-            auto pair_uni = [&](uint32_t p, uint32_t& qa, uint32_t qa_end, uint32_t& qb, uint32_t qb_end) {
-                const float4 c0 = XY[p], c1 = ZT[p];
+            auto pair_uni = [&](uint32_t p, const float4 c0, const float4 c1, uint32_t& qa, uint32_t qa_end, uint32_t& qb, uint32_t qb_end) {
                 const f32x2 dx = sub2(ax2, pk2(c0.x, c0.y)), dy = sub2(ay2, pk2(c0.z, c0.w)), dz = sub2(az2, pk2(c1.x, c1.y));
                 float r0, r1;
                 unpk2(fma2(dz, dz, fma2(dy, dy, mul2(dx, dx))), r0, r1);
@@ -345,10 +344,20 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
                 const uint32_t pa = sa >> 1, pb = (sb + 1u) >> 1;
                 uint32_t p = pa + ((pa ^ (uint32_t)u) & 1u);
                 if (uni) {
-                    if ((p & 2u) && p < pb) { pair_uni(p, bp2, e2, bp3, e3); p += 2; }
-#pragma unroll 4
-                    for (; p + 2 < pb; p += 4) { pair_uni(p, bp0, e0, bp1, e1); pair_uni(p + 2, bp2, e2, bp3, e3); }
-                    if (p < pb) pair_uni(p, bp0, e0, bp1, e1);
+                    if ((p & 2u) && p < pb) { pair_uni(p, XY[p], ZT[p], bp2, e2, bp3, e3); p += 2; }
+                    // software pipeline: the records of the next two pairs are loaded while the current two are tested
+                    // (indices clamped to the staged arrays; a clamped load is never used)
+                    constexpr uint32_t PLAST = TILE_CMAXP / 2 - 1;
+                    float4 a0 = XY[min(p, PLAST)], a1 = ZT[min(p, PLAST)], b0 = XY[min(p + 2, PLAST)], b1 = ZT[min(p + 2, PLAST)];
+#pragma unroll 2
+                    for (; p + 2 < pb; p += 4) {
+                        const uint32_t pn = min(p + 4, PLAST), pm = min(p + 6, PLAST);
+                        const float4 na0 = XY[pn], na1 = ZT[pn], nb0 = XY[pm], nb1 = ZT[pm];
+                        pair_uni(p, a0, a1, bp0, e0, bp1, e1);
+                        pair_uni(p + 2, b0, b1, bp2, e2, bp3, e3);
+                        a0 = na0; a1 = na1; b0 = nb0; b1 = nb1;
+                    }
+                    if (p < pb) pair_uni(p, a0, a1, bp0, e0, bp1, e1);
                 } else {
                     if ((p & 2u) && p < pb) { pair_gen(p, bp2, e2, bp3, e3); p += 2; }
 #pragma unroll 2
