@@ -50,13 +50,12 @@ void free_all(Ctx* c) {
 // Scratch of the tiled path (tiles, neighbour lists): sized for (n, grid) at the first spray_build_cells that needs
 // it and kept; growing it synchronises the device (cudaFree).  Failure to allocate is not an error: the general
 // kernels then serve every particle.
-constexpr int64_t POOL_U2_PER_PARTICLE = 32;      // 128 scheduled u16 entries per particle on average
 
 void ensure_tiled(Ctx* c) {
     Tiled& t = c->tl;
     const int64_t nb = (int64_t)((c->grid.ncell[1] + 1) / 2) * ((c->grid.ncell[2] + 1) / 2);
     const int64_t need = (5 * ((c->n + TILE_T - 1) / TILE_T)) / 4 + 2 * nb + 64;
-    const int64_t pool_need = c->n * POOL_U2_PER_PARTICLE + 4096;
+    const int64_t pool_need = need * TILE_WARPS * (LIST_RMAX / 4) * 32;   // one fixed block of LIST_RMAX rounds per (tile, warp)
     if (t.tiles && need <= t.tile_cap && nb <= t.bundle_cap && pool_need <= t.pool_cap) return;
     cudaFree(t.tiles); cudaFree(t.bcount); cudaFree(t.pool); cudaFree(t.winfo); cudaFree(t.lcount); cudaFree(t.tflags); cudaFree(t.tiletab);
     t.tiles = nullptr; t.bcount = nullptr; t.pool = nullptr; t.winfo = nullptr; t.lcount = nullptr; t.tflags = nullptr; t.tiletab = nullptr;

@@ -451,16 +451,9 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
 #pragma unroll
         for (int o = 16; o; o >>= 1) R = max(R, __shfl_xor_sync(0xFFFFFFFFu, R, o));
         R = (R + 3u) & ~3u;
-        unsigned long long off = 0;
-        if (lane == 0) {
-            if (R > (uint32_t)LIST_RMAX) s_bad = 1;
-            else if (R > 0) {
-                const unsigned long long need = (unsigned long long)(R / 4) * 32;
-                off = atomicAdd(&A.ctr[CTR_POOL], need);
-                if (off + need > A.pool_cap) { s_bad = 1; atomicOr(A.status, (uint32_t)SPRAY_DEV_LIST_OVERFLOW); }
-            }
-        }
-        off = __shfl_sync(0xFFFFFFFFu, off, 0);
+        // list storage: one fixed block of LIST_RMAX rounds per (tile, warp) -- no allocation, placement is deterministic
+        const unsigned long long off = ((unsigned long long)tile * TILE_WARPS + warp) * (unsigned long long)(LIST_RMAX / 4) * 32;
+        if (lane == 0 && R > (uint32_t)LIST_RMAX) s_bad = 1;
         __syncthreads();
         const bool bad = s_bad != 0;
         if (!bad) {
