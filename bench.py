@@ -242,12 +242,43 @@ def main():
     # ---- e2e: pinned host buffers, H2D of every input and D2H of every output inside the timed region
     e2e = None
     if not args.no_e2e:
+        # The four C-ABI calls need their inputs at different times, so a caller overlaps the copies with the kernels:
+        # a copy-in stream uploads the fields in the order of need (one event per call), a copy-out stream downloads each
+        # call's results while the next call runs.  Every byte still crosses PCIe inside the timed region, every step.
+        main = torch.cuda.current_stream()
+        s_in, s_out = torch.cuda.Stream(), torch.cuda.Stream()
+        groups = [("x", "y", "z", "h"), ("m",), ("p", "cs", "vx", "vy", "vz", "alpha"), ("E", "kappa")]
+        outs = [(), ("rho",), ("ax", "ay", "az", "dudt", "divv"), ("mu", "y", "diag", "offd")]
+
         def e2e_pass():
-            for f in fields:
-                d[f].copy_(host[f], non_blocking=True)
-            one_pass(d)
-            for k in out:
-                hout[k].copy_(out[k], non_blocking=True)
+            s_in.wait_stream(main)              # the previous step's kernels are done with the device inputs
+            ev_in = []
+            with torch.cuda.stream(s_in):
+                for grp in groups:
+                    for f in grp:
+                        d[f].copy_(host[f], non_blocking=True)
+                    ev = torch.cuda.Event(); ev.record(s_in); ev_in.append(ev)
+
+            def done(k):                        # results of call k go home on the copy-out stream
+                ev = torch.cuda.Event(); ev.record(main)
+                with torch.cuda.stream(s_out):
+                    s_out.wait_event(ev)
+                    for o in outs[k]:
+                        hout[o].copy_(out[o], non_blocking=True)
+
+            main.wait_event(ev_in[0])
+            sp.build_cells(w.grid, w.kernel, d["x"], d["y"], d["z"], d["h"])
+            main.wait_event(ev_in[1])
+            sp.density(d["m"], rho=out["rho"])
+            done(1)
+            main.wait_event(ev_in[2])
+            sp.hydro_rhs(d["m"], out["rho"], d["p"], d["cs"], d["vx"], d["vy"], d["vz"], d["alpha"], w.beta,
+                         out=[out["ax"], out["ay"], out["az"], out["dudt"], out["divv"]])
+            done(2)
+            main.wait_event(ev_in[3])
+            sp.fld_apply(d["m"], out["rho"], d["kappa"], d["E"], w.c_light, mu=out["mu"], y=out["y"], diag=out["diag"], offd=out["offd"])
+            done(3)
+            main.wait_stream(s_out)             # the step ends when its last result is in host memory
         e2e_pass()
         barrier()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -292,10 +323,13 @@ def main():
     t_hbm = BYTES_PER_PARTICLE * n / (pk["hbm_gbs"] * 1e9)
     calls = {"build": seg_mean[0], "density": seg_mean[1], "hydro": seg_mean[2], "fld": seg_mean[3]}
     hydro_tflops = flops["hydro"] / calls["hydro"] / 1e12
-    roofline = {"bound": "alu", "kernel": "hydro pair sweep (spray_hydro_rhs: SoA gather + pair kernel)",
+    # dram__bytes_read.sum + dram__bytes_write.sum of k_tiled_sweep<1,0> per launch at c5, one ncu --set full capture
+    # (profiles/r01c_ncu_full_tiled_path.md); null for other workloads
+    traffic = 6.12e9 + 0.67e9 if w.name.startswith("c5") else None
+    roofline = {"bound": "alu", "kernel": "hydro pair sweep (spray_hydro_rhs: prologue k_prep_hydro + k_tiled_sweep<1>)",
                 "achieved": hydro_tflops, "peak": fp64_meas, "unit": "TFLOP/s", "frac": hydro_tflops / fp64_meas,
                 "peak_source": "DFMA-chain probe measured in this run (spray_fp64_peak_probe); nominal 148x64x2x1.965GHz = %.1f" % FP64_NOMINAL_TFLOPS,
-                "traffic": None,
+                "traffic": traffic,
                 "pass": {"flops": sum(flops.values()), "bytes": BYTES_PER_PARTICLE * n, "t_alu_ms": 1e3 * t_alu, "t_hbm_ms": 1e3 * t_hbm,
                          "t_pass_ms": 1e3 * t_step, "frac": max(t_alu, t_hbm) / t_step, "hbm_peak_gbs": pk["hbm_gbs"], "hbm_peak_source": pk_src},
                 "per_call_ms": {k: 1e3 * float(v) for k, v in calls.items()},
