@@ -45,6 +45,14 @@ __device__ __forceinline__ double rcp_fast(double x) {
 #endif
 }
 
+// 16- and 8-byte asynchronous global -> shared copies (LDGSTS)
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"((uint32_t)__cvta_generic_to_shared(smem_dst)), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async8(void* smem_dst, const void* gsrc) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" :: "r"((uint32_t)__cvta_generic_to_shared(smem_dst)), "l"(gsrc) : "memory");
+}
+
 // Rescaled shape functions (common.cuh): W = kWn / h^3 * wshape(q), F = dW/dr = kFn / h^4 * gshape(q).
 // CLAMP = false is used where every listed pair is known to be inside the support (uniform h over the tile):
 // rounding can then leave 2 - q at -1e-13 at worst, which contributes nothing at the tolerance of the pass.
@@ -309,22 +317,37 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
             for (int w = tid; w < TILES_WORDS; w += TILE_THREADS) dst[w] = src[w];
         }
         __syncthreads();
-        // ---- stage the candidate records: one warp per range
+        // ---- stage the candidate records: one warp per range.  Ranges that need no periodic shift (all but those of
+        //      tiles at a periodic face) are copied with cp.async (LDGSTS): no register round trip, every copy of the
+        //      thread in flight at once, completion awaited just before the barrier that precedes the pair loop.
         for (int q = warp; q < (int)S.nranges; q += TILE_WARPS) {
             const uint32_t vs = S.r_vstart[q], len = S.r_vend[q] - vs, base = S.r_base[q];
-            const double shx = S.r_shift[q][0] * g.L[0], shy = S.r_shift[q][1] * g.L[1], shz = S.r_shift[q][2] * g.L[2];
-            for (uint32_t k = lane; k < len; k += 32) {
+            const bool shifted = (S.r_shift[q][0] | S.r_shift[q][1] | S.r_shift[q][2]) != 0;
+            if (!shifted) {
+                for (uint32_t k = lane; k < len; k += 32) {
 #pragma unroll
-                for (int v = 0; v < NV; ++v) {
-                    if (uni && ((SWEEP == SW_HYDRO && v == 5) || (SWEEP == SW_APPLY && v == 3))) continue;
-                    double2 val = A.rec[v][vs + k];
-                    if (v == 0) { val.x -= shx; val.y -= shy; }
-                    if (v == 1) val.x -= shz;
-                    F[v * TILE_CMAXP + base + k] = val;
+                    for (int v = 0; v < NV; ++v) {
+                        if (uni && ((SWEEP == SW_HYDRO && v == 5) || (SWEEP == SW_APPLY && v == 3))) continue;
+                        cp_async16(&F[v * TILE_CMAXP + base + k], &A.rec[v][vs + k]);
+                    }
+                    if (NRec<SWEEP>::e) cp_async8(&Ee[base + k], &A.e1[vs + k]);
                 }
-                if (NRec<SWEEP>::e) Ee[base + k] = A.e1[vs + k];
+            } else {
+                const double shx = S.r_shift[q][0] * g.L[0], shy = S.r_shift[q][1] * g.L[1], shz = S.r_shift[q][2] * g.L[2];
+                for (uint32_t k = lane; k < len; k += 32) {
+#pragma unroll
+                    for (int v = 0; v < NV; ++v) {
+                        if (uni && ((SWEEP == SW_HYDRO && v == 5) || (SWEEP == SW_APPLY && v == 3))) continue;
+                        double2 val = A.rec[v][vs + k];
+                        if (v == 0) { val.x -= shx; val.y -= shy; }
+                        if (v == 1) val.x -= shz;
+                        F[v * TILE_CMAXP + base + k] = val;
+                    }
+                    if (NRec<SWEEP>::e) Ee[base + k] = A.e1[vs + k];
+                }
             }
         }
+        asm volatile("cp.async.commit_group;" ::: "memory");
         // ---- this thread's target
         const bool active = tgt < (int)td.nt;
         uint32_t i = 0;
@@ -343,6 +366,7 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
             if (SWEEP == SW_LIMITER) T.c0 = A.e1[i];                                         // E_a
             if (SWEEP == SW_APPLY) { const double2 me = A.rec[2][i]; T.c0 = me.y; T.c1 = me.x; T.c2 = 4.0 * me.x; }
         }
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
         __syncthreads();
 
         Acc acc{0, 0, 0, 0, 0};
