@@ -182,3 +182,74 @@ def fld_apply(grid, kernel, x, y, z, h, m, rho, mu, E, sym_mode=True, use_cells=
                                 int(use_cells), pt, C.c_int64(nt), *[_p(out[k]) for k in keys])
     assert rc == 0
     return out
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# Row N1 of SURVEY.md section 8(f): the implicit radiation step (section 2.3).
+# Backward-Euler energy exchange + diffusion, eqs. (49)-(50), solved by Jacobi iteration: every iteration applies the
+# FLD operator to the current iterate (eqs. (51)-(52): Lambda, Gamma), then solves the per-particle quartic eq. (57)
+# for chi (eq. (56)) in closed form (eqs. (58)-(60)) and updates E by eq. (55) and u by eq. (56).
+# TEST INFRASTRUCTURE like the rest of oracle/: plain numpy fp64 on top of fld_apply, no code shared with the CUDA path.
+# Readings (A25 ff.): the limiter is frozen during the iteration (mu is an input, A18); the resolvent
+# cubic of x^4 + b x + c = 0 is y^3 + p y + q = 0 with p = -c, q = -b^2/8, the factorisation is
+# (x^2 + s x + y - b/(2s)) (x^2 - s x + y + b/(2s)), s = sqrt(2y), so the two real roots for b > 0, c < 0 are
+# x = (-s +- sqrt(-2y + 2b/s)) / 2 (the sign pairing eq. (58) leaves open); "the root that yields a real value of u closest
+# to u^n" is then the one closest to T^n, i.e. the positive one.  That root is computed by safeguarded Newton
+# (quartic_positive_root) because the closed form is numerically unusable over part of the parameter range.
+
+def quartic_roots(b, c):
+    """Real roots of x^4 + b x + c = 0 for b > 0, c < 0 by eqs. (58)-(60): returns (x_plus, x_minus)."""
+    b = np.asarray(b, dtype=np.float64); c = np.asarray(c, dtype=np.float64)
+    p = -c
+    q = -b * b / 8.0
+    w = np.cbrt(-q / 2.0 + np.sqrt(q * q / 4.0 + p ** 3 / 27.0))          # eq. (60)
+    y = w - p / (3.0 * w)                                                  # eq. (59)
+    s = np.sqrt(2.0 * y)
+    d = np.sqrt(-2.0 * y + 2.0 * b / s)
+    return 0.5 * (-s + d), 0.5 * (-s - d)                                  # eq. (58)
+
+
+def quartic_positive_root(b, c):
+    """The unique positive root of x^4 + b x + c = 0 (b > 0, c < 0) to rounding: Newton's method from the upper bound
+    min((-c)^(1/4), -c/b) (f is convex and increasing on x > 0, so the iterates decrease monotonically to the root).
+    The closed form of eqs. (58)-(60) is the same number algebraically but cancels catastrophically when the root is
+    small (relative residuals up to 0.4, even inf/nan, on a log-uniform sweep of (b, c)); it is kept as quartic_roots
+    and pinned against this routine where it is well conditioned (tests/test_oracle_rad.py)."""
+    b = np.asarray(b, dtype=np.float64); c = np.asarray(c, dtype=np.float64)
+    x = np.minimum((-c) ** 0.25, -c / b)
+    for _ in range(100):
+        dx = (x ** 4 + b * x + c) / (4.0 * x ** 3 + b)
+        x = x - dx
+        if np.all(np.abs(dx) <= 4.0 * np.finfo(np.float64).eps * np.abs(x)):
+            break
+    return x
+
+
+def rad_jacobi(grid, kernel, x, y, z, h, m, rho, mu, kappa_p, E_n, u_n, T_n, dTdu, dt, c_light, a_rad, niter,
+               sym_mode=True, E0=None):
+    """niter Jacobi iterations of eqs. (49)-(50) from the iterate E0 (default E_n).  Returns dict(E, u, chi, resid[niter],
+    S_offd): resid[k] = max_a |lhs - rhs| / |lhs| of eq. (49) for the iterate that ENTERS iteration k, 0 for k = 0."""
+    E_n = np.asarray(E_n, np.float64); u_n = np.asarray(u_n, np.float64); T_n = np.asarray(T_n, np.float64)
+    rho = np.asarray(rho, np.float64); kp = np.asarray(kappa_p, np.float64); dTdu = np.asarray(dTdu, np.float64)
+    E = E_n.copy() if E0 is None else np.asarray(E0, np.float64).copy()
+    u = u_n.copy()
+    chi = T_n.copy()
+    resid = np.zeros(niter)
+    S_offd = None
+    K = dt * c_light * kp                                                  # denominator of eq. (55)
+    X = dt * rho * c_light * kp
+    for k in range(niter):
+        ap = fld_apply(grid, kernel, x, y, z, h, m, rho, mu, E, sym_mode=sym_mode)
+        lam, gam, S_offd = ap["diag"], ap["offd"], ap["S_offd"]
+        if k > 0:                                                          # both sides of eq. (49) for the current iterate
+            rhs = E_n + dt * (lam * E + gam) + X * (a_rad * chi ** 4 - E)
+            resid[k] = np.max(np.abs(E - rhs) / np.abs(E))
+        D = 1.0 - dt * lam
+        Bq = (D + X) / K / dTdu                                            # coefficient of chi in eq. (57)
+        Aq = D * a_rad
+        Cq = E_n + dt * gam + Bq * T_n
+        # of the two real roots the positive one is the closer to T^n > 0 (P:L309): the other is negative
+        chi = quartic_positive_root(Bq / Aq, -Cq / Aq)
+        u = u_n + (chi - T_n) / dTdu                                       # eq. (56)
+        E = (u - u_n) / K + a_rad * chi ** 4                               # eq. (55)
+    return dict(E=E, u=u, chi=chi, resid=resid, S_offd=S_offd)
