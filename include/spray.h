@@ -152,6 +152,23 @@ int spray_neighbor_lists(spray_ctx* ctx, int symmetric, const uint64_t* offsets,
  * z = (z ^ z>>30) * 0xBF58476D1CE4E5B9, z = (z ^ z>>27) * 0x94D049BB133111EB, z ^ z>>31;  id_b = caller index of b. */
 int spray_neighbor_digest(spray_ctx* ctx, int symmetric, uint64_t* dsum, uint64_t* dxor, void* stream);
 
+/* (N1) implicit radiation step by Jacobi iteration, section 2.3 P:L268-L327.
+ * Backward-Euler form of eqs. (47)-(48), i.e. eqs. (49)-(50), with the limiter frozen (mu[] given, A18).  Each of the
+ * `niter` iterations (i) applies the FLD operator to the current iterate (spray_fld_apply FROZEN: Lambda_a, Gamma_a of eqs.
+ * (51)-(52) over the neighbour lists of the last spray_build_cells), (ii) solves for every particle the quartic eq. (57)
+ *       (1 - dt Lambda) a chi^4 + B chi - [E^n + dt Gamma + B T^n] = 0,   B = (1 - dt Lambda + dt rho c kappa_P) / (dt c kappa_P) / (dT/du)
+ * for its positive root chi (eq. (56); the root "closest to u^n"; safeguarded Newton from the upper bound
+ * min(C'^(1/4), C'/B'), because the closed form eqs. (58)-(60) cancels catastrophically for small roots -- DESIGN.md A25),
+ * (iii) sets u = u^n + (chi - T^n)/(dT/du) (eq. (56)) and E = (u - u^n)/(dt c kappa_P) + a chi^4 (eq. (55)).
+ * Inputs (caller order, length n): m, rho, mu (= c lambda/(rho kappa_R)), kappa_p, E_n, u_n, T_n, dTdu.
+ * E [in/out]: the starting iterate (usually a copy of E_n) and, on return, E after niter iterations; u [out].
+ * resid (nullable, DEVICE array of niter doubles): resid[k] = max_a |lhs - rhs| / |lhs| of eq. (49) for the iterate that
+ * enters iteration k ("relative error of the difference between the two sides of equation (49)"), 0 for k = 0.
+ * Requires dt, c_light, a_rad > 0, kappa_p > 0, dTdu > 0, niter >= 1.  E, u must not alias the inputs. */
+int spray_rad_jacobi(spray_ctx* ctx, const double* m, const double* rho, const double* mu, const double* kappa_p,
+                     const double* E_n, const double* u_n, const double* T_n, const double* dTdu, double dt, double c_light,
+                     double a_rad, spray_fld_kernel_mode_t kmode, int niter, double* E, double* u, double* resid, void* stream);
+
 /* Measurement aid: runs `iters` dependent DFMA per thread on `blocks` x `threads` threads
  * with 8 independent chains; out (device, [blocks*threads]) receives the sums so the work cannot be elided.
  * Used by bench.py to measure the sustained FP64 FMA peak the roofline is quoted against. */

@@ -24,7 +24,7 @@ DEV_H_EXCEEDS_HMAX, DEV_OUTSIDE_BOX, DEV_LIST_OVERFLOW = 1, 2, 4
 # every symbol include/spray.h declares
 EXPORTS = ["spray_version", "spray_create", "spray_destroy", "spray_last_error", "spray_check", "spray_launch_count", "spray_set_path", "spray_path_stats",
            "spray_build_cells", "spray_density", "spray_hydro_rhs", "spray_fld_apply", "spray_get_cell_table",
-           "spray_neighbor_counts", "spray_neighbor_lists", "spray_neighbor_digest", "spray_fp64_peak_probe"]
+           "spray_neighbor_counts", "spray_neighbor_lists", "spray_neighbor_digest", "spray_rad_jacobi", "spray_fp64_peak_probe"]
 
 
 class SprayError(RuntimeError):
@@ -64,6 +64,7 @@ def load():
     lib.spray_density.argtypes = [vp, vp, vp, vp, vp]
     lib.spray_hydro_rhs.argtypes = [vp] + [vp] * 8 + [dbl] + [vp] * 5 + [vp]
     lib.spray_fld_apply.argtypes = [vp, vp, vp, vp, vp, dbl, i32, i32, vp, vp, vp, vp, vp, vp]
+    lib.spray_rad_jacobi.argtypes = [vp] + [vp] * 8 + [dbl, dbl, dbl, i32, i32, vp, vp, vp, vp]
     lib.spray_get_cell_table.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.spray_neighbor_counts.argtypes = [vp, i32, vp, vp]
     lib.spray_neighbor_lists.argtypes = [vp, i32, vp, vp, vp]
@@ -200,6 +201,19 @@ class Spray:
                                       _ptr(y, f64, self.n), _ptr(diag), _ptr(offd), _ptr(gradE), _stream())
         self._ck(rc, "spray_fld_apply")
         return dict(mu=mu, y=y, diag=diag, offd=offd, gradE=gradE)
+
+    def rad_jacobi(self, m, rho, mu, kappa_p, E_n, u_n, T_n, dTdu, dt, c_light=1.0, a_rad=1.0, niter=1, kmode=FLD_SYMMETRIC,
+                   E0=None, want_resid=True):
+        """Row N1: niter Jacobi iterations of the implicit radiation step (include/spray.h).  Returns dict(E, u, resid)."""
+        f64 = self.torch.float64
+        E = (E_n if E0 is None else E0).clone()
+        u = self._out(None)
+        resid = self.torch.zeros(int(niter), dtype=f64, device=self.device) if want_resid else None
+        a = [_ptr(t, f64, self.n) for t in (m, rho, mu, kappa_p, E_n, u_n, T_n, dTdu)]
+        rc = self.lib.spray_rad_jacobi(self.h, *a, float(dt), float(c_light), float(a_rad), int(kmode), int(niter),
+                                       _ptr(E, f64, self.n), _ptr(u, f64, self.n), _ptr(resid), _stream())
+        self._ck(rc, "spray_rad_jacobi")
+        return dict(E=E, u=u, resid=resid)
 
     # -- parity exports
     def get_cell_table(self):

@@ -37,6 +37,7 @@ void free_all(Ctx* c) {
     for (int k = 0; k < 2; ++k) { cudaFree(c->key[k]); cudaFree(c->idx[k]); }
     cudaFree(c->hist); cudaFree(c->cell_start); cudaFree(c->cell_end); cudaFree(c->cell_hmax);
     cudaFree(c->hglob); cudaFree(c->dev_status);
+    for (double* r : c->rad_scratch) cudaFree(r);
     cudaFree(c->s.x); cudaFree(c->s.y); cudaFree(c->s.z); cudaFree(c->s.h); cudaFree(c->s.hs);
     for (double* f : c->s.f) cudaFree(f);
     Packed& k = c->pk;
@@ -311,6 +312,47 @@ int spray_fld_apply(spray_ctx* ctx, const double* m, const double* rho, const do
     }
     a.o0 = y; a.o1 = diag; a.o2 = offd;
     CK(launch_ref_sweep(c, SW_APPLY, a, st), "apply sweep");
+    return SPRAY_OK;
+}
+
+int spray_rad_jacobi(spray_ctx* ctx, const double* m, const double* rho, const double* mu, const double* kappa_p,
+                     const double* E_n, const double* u_n, const double* T_n, const double* dTdu, double dt, double c_light,
+                     double a_rad, spray_fld_kernel_mode_t kmode, int niter, double* E, double* u, double* resid, void* stream) {
+    NEED_BUILT();
+    Ctx* c = &ctx->c;
+    if (c->n > 0 && (!m || !rho || !mu || !kappa_p || !E_n || !u_n || !T_n || !dTdu || !E || !u))
+        return fail(c, SPRAY_ERR_INVALID_ARG, "spray_rad_jacobi: NULL argument");
+    if (!(dt > 0.0) || !(c_light > 0.0) || !(a_rad > 0.0) || niter < 1 || (kmode != SPRAY_FLD_SYMMETRIC && kmode != SPRAY_FLD_GATHER))
+        return fail(c, SPRAY_ERR_INVALID_ARG, "spray_rad_jacobi: dt, c_light, a_rad must be > 0, niter >= 1, kmode valid");
+    for (double*& r : c->rad_scratch)
+        if (!r && !dmalloc(&r, c->n_max)) { cudaGetLastError(); return fail(c, SPRAY_ERR_ALLOC, "spray_rad_jacobi: scratch allocation failed"); }
+    cudaStream_t st = (cudaStream_t)stream;
+    double** f = c->s.f;
+    // sorted records of the frozen operator: (z, V), (mu, E) with E = the starting iterate
+    PrepJob pj{};
+    pj.m = m; pj.rho = rho; pj.E = E; pj.kx = mu; pj.kx_is_mu = 1;
+    pj.sm = f[F_M]; pj.srho = f[F_RHO]; pj.sE = f[F_E]; pj.skx = f[F_MU]; pj.sV = f[F_V];
+    CK(launch_prep_fld(c, pj, st), "rad prologue");
+    if (resid) CK(cudaMemsetAsync(resid, 0, sizeof(double) * (size_t)niter, st), "rad residuals");
+    double *y = c->rad_scratch[0], *lam = c->rad_scratch[1], *gam = c->rad_scratch[2], *chi = c->rad_scratch[3];
+    const int sym = (kmode == SPRAY_FLD_SYMMETRIC) ? 1 : 0;
+    for (int k = 0; k < niter; ++k) {
+        if (c->tl.enabled) {
+            TiledArgs t{};
+            t.fld_sym = sym; t.o0 = y; t.o1 = lam; t.o2 = gam;
+            CK(launch_tiled_sweep(c, SW_APPLY, t, st), "rad: tiled apply sweep");
+        }
+        SweepArgs a = fallback_args(c);
+        a.m = f[F_M]; a.rho = f[F_RHO]; a.E = f[F_E]; a.mu = f[F_MU]; a.c_light = c_light; a.fld_sym = sym;
+        a.o0 = y; a.o1 = lam; a.o2 = gam;
+        CK(launch_ref_sweep(c, SW_APPLY, a, st), "rad: apply sweep");
+        RadArgs r{};
+        r.rho = rho; r.kappa_p = kappa_p; r.E_n = E_n; r.u_n = u_n; r.T_n = T_n; r.dTdu = dTdu;
+        r.lam = lam; r.gam = gam; r.dt = dt; r.c_light = c_light; r.a_rad = a_rad;
+        r.E = E; r.u = u; r.chi = chi; r.me = c->pk.me; r.sE = f[F_E];
+        r.resid = resid ? resid + k : nullptr; r.first = (k == 0) ? 1 : 0;
+        CK(launch_rad_update(c, r, st), "rad: quartic update");
+    }
     return SPRAY_OK;
 }
 

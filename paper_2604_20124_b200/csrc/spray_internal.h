@@ -70,6 +70,7 @@ struct Ctx {
     Sorted s{};
     Packed pk{};
     Tiled tl{};
+    double* rad_scratch[4] = {nullptr, nullptr, nullptr, nullptr};   // N1: y, Lambda, Gamma, chi (caller order), allocated on first use
     int64_t launches = 0;       // kernels launched through this ctx (bench.py reports it as gpu_launches)
     std::string err;
 };
@@ -132,6 +133,20 @@ cudaError_t launch_tiled_sweep(Ctx* c, int sweep, const TiledArgs& a, cudaStream
 // parity exports from the tiled lists: mode 0 = counts, 1 = CSR lists, 2 = digests (tiles.cu)
 cudaError_t launch_tiled_export(Ctx* c, int mode, int symmetric, uint32_t* ocount, const uint64_t* offsets, uint32_t* onbr,
                                 uint64_t* odsum, uint64_t* odxor, cudaStream_t st);
+
+// ---- rad.cu : row N1, per-particle quartic solve of the Jacobi iteration (eqs. (54)-(57))
+struct RadArgs {
+    const double *rho, *kappa_p, *E_n, *u_n, *T_n, *dTdu;     // caller order
+    const double *lam, *gam;                                   // caller order: Lambda, Gamma of the current iterate
+    double dt, c_light, a_rad;
+    double *E, *u;                                             // caller order: iterate out
+    double *chi;                                               // caller order scratch: chi of the previous solve (residual)
+    double2* me;                                               // sorted (mu, E) record of the tiled apply
+    double* sE;                                                // sorted E of the general kernels
+    double* resid;                                             // nullable: slot of this iteration
+    int first;                                                 // iteration 0: no residual
+};
+cudaError_t launch_rad_update(Ctx* c, const RadArgs& a, cudaStream_t st);
 
 // ---- probe.cu
 cudaError_t launch_fp64_probe(int blocks, int threads, int64_t iters, double* out, cudaStream_t st);
