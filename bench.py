@@ -158,6 +158,7 @@ def main():
     ap.add_argument("--cpu-sample", type=int, default=200000, help="target particles per oracle step (cpu_baseline / reference arm)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-n1", action="store_true", help="skip the row-N1 measurement (Jacobi iterations of spray_rad_jacobi)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -312,6 +313,28 @@ def main():
     torch.cuda.synchronize()
     fp64_meas = 10 * 148 * 8 * 256 * iters * 64 * 2 / (p0.elapsed_time(p1) * 1e-3) / 1e12
 
+    # ---- row N1: Jacobi iterations of the implicit radiation step on the same particle set, with the
+    #      neighbour lists of the last spray_build_cells; outside the timed region of the headline metric
+    n1 = None
+    if not args.no_n1:
+        u_n = d["p"] / ((w.gamma - 1.0) * out["rho"])
+        T_n = (w.gamma - 1.0) * u_n
+        dTdu = torch.full_like(u_n, w.gamma - 1.0)
+        nit = 20
+        dt_rad = 0.3 * float(w.h.min()) ** 2 / float(out["mu"].max().item())
+        sp.rad_jacobi(d["m"], out["rho"], out["mu"], d["kappa"], d["E"], u_n, T_n, dTdu, dt_rad, w.c_light, 1.0, niter=2)
+        torch.cuda.synchronize()
+        r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        r0.record()
+        rj = sp.rad_jacobi(d["m"], out["rho"], out["mu"], d["kappa"], d["E"], u_n, T_n, dTdu, dt_rad, w.c_light, 1.0, niter=nit)
+        r1.record()
+        torch.cuda.synchronize()
+        t_it = r0.elapsed_time(r1) * 1e-3 / nit
+        n1 = {"call": "spray_rad_jacobi", "iterations": nit, "ms_per_iteration": 1e3 * t_it, "iterations_per_s": 1.0 / t_it,
+              "pair_interactions_per_s": pairs["apply"] / t_it,
+              "flop_roofline_frac": pairs["apply"] * FLOPS[w.kernel]["apply"] / t_it / (fp64_meas * 1e12),
+              "resid_last": float(rj["resid"][-1].item()), "note": "includes the one-off prologue of the call (1/%d per iteration)" % nit}
+
     # ---- roofline: pass level and dominant kernel
     fl = FLOPS[w.kernel]
     visc_frac = 0.0 if not (np.any(w.vx) or np.any(w.vy) or np.any(w.vz)) else 0.5
@@ -355,7 +378,7 @@ def main():
                        "parallelism": "replicas only" if world > 1 else "1 GPU", "path": args.path,
                        "tiles": n_tiles, "tiled_fraction": n_fast / max(n, 1)},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
-            "fp64_probe_tflops": fp64_meas}
+            "fp64_probe_tflops": fp64_meas, "next_rows": {"N1_rad_jacobi": n1}}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
