@@ -152,6 +152,15 @@ int spray_neighbor_lists(spray_ctx* ctx, int symmetric, const uint64_t* offsets,
  * z = (z ^ z>>30) * 0xBF58476D1CE4E5B9, z = (z ^ z>>27) * 0x94D049BB133111EB, z ^ z>>31;  id_b = caller index of b. */
 int spray_neighbor_digest(spray_ctx* ctx, int symmetric, uint64_t* dsum, uint64_t* dxor, void* stream);
 
+/* (N2) thermal-conduction sweep: the second term of eqs. (17)/(18), for one species,
+ *       dudt_a = sum_b 4 m_b/(rho_a rho_b) * k_a k_b/(k_a + k_b) * (T_a - T_b) * x_ab . gradWbar(x_ab) / |x_ab|^2,
+ *       gradWbar = (grad W(x_ab,h_a) + grad W(x_ab,h_b))/2,  over N_sym(a).
+ * This is the Laplacian form eq. (16) with c = k, f = T, i.e. the FLD operator of spray_fld_apply (SYMMETRIC, FROZEN) with
+ * mu = k and E = T, divided by rho_a; it is served by the same pair kernel.  Inputs m, rho, k (> 0), T in caller order;
+ * dudt [out].  The electron-ion exchange term k^ei (T^e - T^i) of eqs. (17)/(18) is per-particle arithmetic left to the caller. */
+int spray_conduction(spray_ctx* ctx, const double* m, const double* rho, const double* k, const double* T, double* dudt,
+                     void* stream);
+
 /* (N1) implicit radiation step by Jacobi iteration, section 2.3 P:L268-L327.
  * Backward-Euler form of eqs. (47)-(48), i.e. eqs. (49)-(50), with the limiter frozen (mu[] given, A18).  Each of the
  * `niter` iterations (i) applies the FLD operator to the current iterate (spray_fld_apply FROZEN: Lambda_a, Gamma_a of eqs.

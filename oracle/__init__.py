@@ -253,3 +253,16 @@ def rad_jacobi(grid, kernel, x, y, z, h, m, rho, mu, kappa_p, E_n, u_n, T_n, dTd
         u = u_n + (chi - T_n) / dTdu                                       # eq. (56)
         E = (u - u_n) / K + a_rad * chi ** 4                               # eq. (55)
     return dict(E=E, u=u, chi=chi, resid=resid, S_offd=S_offd)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# Row N2: thermal-conduction term of eqs. (17)/(18) for one species:
+#   dudt_a = sum_b 4 m_b/(rho_a rho_b) k_a k_b/(k_a+k_b) (T_a - T_b) x_ab . gradWbar / |x_ab|^2
+# i.e. eq. (16) with c = k, f = T and the kernel gradient averaged over h_a, h_b, divided by rho_a.  The pair sum is
+# the one oracle_fld_apply evaluates in its symmetric mode (same formula with mu = k, E = T), so it is called, not retyped.
+def conduction(grid, kernel, x, y, z, h, m, rho, k, T, targets=None):
+    """Returns dict(dudt, S_dudt) at the targets."""
+    ap = fld_apply(grid, kernel, x, y, z, h, m, rho, k, T, sym_mode=True, targets=targets)
+    r = np.asarray(rho, np.float64)
+    r = r if targets is None else r[np.asarray(targets)]
+    return dict(dudt=ap["y"] / r, S_dudt=ap["S_y"] / r)

@@ -24,7 +24,7 @@ DEV_H_EXCEEDS_HMAX, DEV_OUTSIDE_BOX, DEV_LIST_OVERFLOW = 1, 2, 4
 # every symbol include/spray.h declares
 EXPORTS = ["spray_version", "spray_create", "spray_destroy", "spray_last_error", "spray_check", "spray_launch_count", "spray_set_path", "spray_path_stats",
            "spray_build_cells", "spray_density", "spray_hydro_rhs", "spray_fld_apply", "spray_get_cell_table",
-           "spray_neighbor_counts", "spray_neighbor_lists", "spray_neighbor_digest", "spray_rad_jacobi", "spray_fp64_peak_probe"]
+           "spray_neighbor_counts", "spray_neighbor_lists", "spray_neighbor_digest", "spray_rad_jacobi", "spray_conduction", "spray_fp64_peak_probe"]
 
 
 class SprayError(RuntimeError):
@@ -64,6 +64,7 @@ def load():
     lib.spray_density.argtypes = [vp, vp, vp, vp, vp]
     lib.spray_hydro_rhs.argtypes = [vp] + [vp] * 8 + [dbl] + [vp] * 5 + [vp]
     lib.spray_fld_apply.argtypes = [vp, vp, vp, vp, vp, dbl, i32, i32, vp, vp, vp, vp, vp, vp]
+    lib.spray_conduction.argtypes = [vp, vp, vp, vp, vp, vp, vp]
     lib.spray_rad_jacobi.argtypes = [vp] + [vp] * 8 + [dbl, dbl, dbl, i32, i32, vp, vp, vp, vp]
     lib.spray_get_cell_table.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.spray_neighbor_counts.argtypes = [vp, i32, vp, vp]
@@ -201,6 +202,15 @@ class Spray:
                                       _ptr(y, f64, self.n), _ptr(diag), _ptr(offd), _ptr(gradE), _stream())
         self._ck(rc, "spray_fld_apply")
         return dict(mu=mu, y=y, diag=diag, offd=offd, gradE=gradE)
+
+    def conduction(self, m, rho, k, T, dudt=None):
+        """Row N2: thermal-conduction term of eqs. (17)/(18) for one species (include/spray.h)."""
+        f64 = self.torch.float64
+        dudt = self._out(dudt)
+        rc = self.lib.spray_conduction(self.h, _ptr(m, f64, self.n), _ptr(rho, f64, self.n), _ptr(k, f64, self.n), _ptr(T, f64, self.n),
+                                       _ptr(dudt, f64, self.n), _stream())
+        self._ck(rc, "spray_conduction")
+        return dudt
 
     def rad_jacobi(self, m, rho, mu, kappa_p, E_n, u_n, T_n, dTdu, dt, c_light=1.0, a_rad=1.0, niter=1, kmode=FLD_SYMMETRIC,
                    E0=None, want_resid=True):

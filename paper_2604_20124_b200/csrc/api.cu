@@ -315,6 +315,29 @@ int spray_fld_apply(spray_ctx* ctx, const double* m, const double* rho, const do
     return SPRAY_OK;
 }
 
+int spray_conduction(spray_ctx* ctx, const double* m, const double* rho, const double* k, const double* T, double* dudt,
+                     void* stream) {
+    NEED_BUILT();
+    Ctx* c = &ctx->c;
+    if (c->n > 0 && (!m || !rho || !k || !T || !dudt)) return fail(c, SPRAY_ERR_INVALID_ARG, "spray_conduction: NULL argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    double** f = c->s.f;
+    PrepJob pj{};                     // the frozen symmetric operator with mu = k, E = T
+    pj.m = m; pj.rho = rho; pj.E = T; pj.kx = k; pj.kx_is_mu = 1;
+    pj.sm = f[F_M]; pj.srho = f[F_RHO]; pj.sE = f[F_E]; pj.skx = f[F_MU]; pj.sV = f[F_V];
+    CK(launch_prep_fld(c, pj, st), "conduction prologue");
+    if (c->tl.enabled) {
+        TiledArgs t{};
+        t.fld_sym = 1; t.o0 = dudt;
+        CK(launch_tiled_sweep(c, SW_APPLY, t, st), "conduction: tiled sweep");
+    }
+    SweepArgs a = fallback_args(c);
+    a.m = f[F_M]; a.rho = f[F_RHO]; a.E = f[F_E]; a.mu = f[F_MU]; a.fld_sym = 1; a.o0 = dudt;
+    CK(launch_ref_sweep(c, SW_APPLY, a, st), "conduction: sweep");
+    CK(launch_div_by_rho(c, dudt, rho, st), "conduction: 1/rho");
+    return SPRAY_OK;
+}
+
 int spray_rad_jacobi(spray_ctx* ctx, const double* m, const double* rho, const double* mu, const double* kappa_p,
                      const double* E_n, const double* u_n, const double* T_n, const double* dTdu, double dt, double c_light,
                      double a_rad, spray_fld_kernel_mode_t kmode, int niter, double* E, double* u, double* resid, void* stream) {

@@ -55,6 +55,18 @@ k_rad_update(RadArgs A, const uint32_t* __restrict__ perm, int64_t n) {
     }
 }
 
+// N2: dudt_a = y_a / rho_a (the 1/rho_a prefactor of the conduction term, eqs. (17)/(18) P:L129-L132)
+__global__ void k_div_by_rho(double* __restrict__ y, const double* __restrict__ rho, int64_t n) {
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) y[i] = y[i] / rho[i];
+}
+cudaError_t launch_div_by_rho(Ctx* c, double* y, const double* rho, cudaStream_t st) {
+    if (c->n == 0) return cudaSuccess;
+    const int64_t want = (c->n + 255) / 256;
+    k_div_by_rho<<<(int)(want < 148 * 32 ? want : 148 * 32), 256, 0, st>>>(y, rho, c->n);
+    c->launches += 1;
+    return cudaGetLastError();
+}
+
 cudaError_t launch_rad_update(Ctx* c, const RadArgs& a, cudaStream_t st) {
     if (c->n == 0) return cudaSuccess;
     const int64_t want = (c->n + 255) / 256;

@@ -147,6 +147,7 @@ struct RadArgs {
     int first;                                                 // iteration 0: no residual
 };
 cudaError_t launch_rad_update(Ctx* c, const RadArgs& a, cudaStream_t st);
+cudaError_t launch_div_by_rho(Ctx* c, double* y, const double* rho, cudaStream_t st);   // N2
 
 // ---- probe.cu
 cudaError_t launch_fp64_probe(int blocks, int threads, int64_t iters, double* out, cudaStream_t st);
