@@ -199,16 +199,6 @@ __global__ void k_reorder_build(const uint32_t* __restrict__ perm, int64_t n, co
     hh[i] = make_double2(hinv, fnk * (h2 * h2));
 }
 
-// out[k][i] = in[k][perm[i]]; with only_if_slow the kernel does nothing when the tiled kernels serve every particle
-__global__ void k_gather(GatherJob job, const uint32_t* __restrict__ perm, int64_t n, const unsigned long long* __restrict__ nfast) {
-    if (nfast && *nfast == (unsigned long long)n) return;
-    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    uint32_t p = perm[i];
-#pragma unroll 4
-    for (int k = 0; k < job.count; ++k) job.out[k][i] = __ldg(job.in[k] + p);
-}
-
 // per-call prologues: caller order -> sorted order, with the per-particle factors of the pair formulas hoisted
 // (V = m/rho, Q = V p, alpha*c, p/rho, 1/rho): one division per particle instead of one per pair.  The packed
 // records feed the tiled kernels; the structure-of-arrays copies feed the general kernels and are written only
@@ -340,13 +330,6 @@ static const unsigned long long* nfast_ptr(Ctx* c) { return c->tl.enabled ? c->t
 static PackedOut packed_out(Ctx* c) {
     PackedOut o{c->pk.s[0], c->pk.s[1], c->pk.s[2], c->pk.s[3], c->pk.t0, c->pk.me, c->pk.e1, c->pk.p1};
     return o;
-}
-
-cudaError_t launch_gather(Ctx* c, const GatherJob& job, bool only_if_slow, cudaStream_t st) {
-    if (c->n == 0 || job.count == 0) return cudaSuccess;
-    k_gather<<<cdiv64(c->n, 256), 256, 0, st>>>(job, c->perm, c->n, only_if_slow ? nfast_ptr(c) : nullptr);
-    c->launches += 1;
-    return cudaGetLastError();
 }
 
 cudaError_t launch_prep_density(Ctx* c, const double* m, cudaStream_t st) {

@@ -38,16 +38,16 @@ struct Tiled {
     int64_t tile_cap = 0;
     uint32_t* bcount = nullptr;  // [bundle_cap + 1 + scan scratch] tiles per bundle -> exclusive scan
     int64_t bundle_cap = 0;
-    uint2* pool = nullptr;       // list storage: per warp a block of rounds/4 x 32 lanes x (4 u16 slots)
+    uint2* pool = nullptr;       // list storage: per (tile, warp) a fixed block of LIST_RMAX/4 x 32 lanes x (4 u16 slots)
     int64_t pool_cap = 0;        // in uint2 units
-    unsigned long long* ctr = nullptr;   // [0] pool cursor, [1] particles served by the tiled kernels, [2] tiles, [3] work counter
+    unsigned long long* ctr = nullptr;   // [CTR_NFAST] particles served by the tiled kernels, [CTR_NTILES] tiles
     uint2* winfo = nullptr;      // [tile_cap][TILE_WARPS]: (pool offset, rounds)
     uint32_t* lcount = nullptr;  // [tile_cap][TILE_T]: n_gather | n_sym << 16
     uint32_t* tflags = nullptr;  // [tile_cap]: TILE_FLAG_*
     uint32_t* tiletab = nullptr; // [tile_cap][TILES_WORDS]: per-tile TileS tables
     uint8_t* fast = nullptr;     // [n_max] sorted order: 1 = particle is served by the tiled kernels
 };
-enum { CTR_POOL = 0, CTR_NFAST = 1, CTR_NTILES = 2, CTR_WORK = 3, CTR_COUNT = 4 };
+enum { CTR_NFAST = 1, CTR_NTILES = 2, CTR_COUNT = 4 };
 
 struct Ctx {
     int device = 0;
@@ -75,18 +75,11 @@ struct Ctx {
     std::string err;
 };
 
-struct GatherJob {              // out[k][i] = in[k][perm[i]] for k < count
-    const double* in[12];
-    double* out[12];
-    int count;
-};
-
 // ---- build.cu
 cudaError_t launch_cell_keys(Ctx* c, const double* x, const double* y, const double* z, cudaStream_t st);
 cudaError_t launch_radix_sort(Ctx* c, cudaStream_t st);      // sets c->sorted_key / c->perm
 cudaError_t launch_cell_table(Ctx* c, cudaStream_t st);
 cudaError_t launch_reorder_build(Ctx* c, const double* x, const double* y, const double* z, const double* h, cudaStream_t st);
-cudaError_t launch_gather(Ctx* c, const GatherJob& job, bool only_if_slow, cudaStream_t st);
 cudaError_t launch_cell_hmax(Ctx* c, cudaStream_t st);
 cudaError_t launch_excl_scan_u32(Ctx* c, uint32_t* a, int64_t total, uint32_t* scratch, cudaStream_t st);
 

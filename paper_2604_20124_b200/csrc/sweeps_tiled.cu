@@ -275,12 +275,17 @@ __device__ __forceinline__ void pair_loop(const double2* __restrict__ F, const d
     }
 }
 
-template <int SWEEP> struct MinBlocks { static constexpr int v = (SWEEP == SW_DENSITY || SWEEP == SW_LIMITER) ? 2 : 1; };
+// MODE 0: every tile.  MODE 1: only the tiles with uniform h, whose pair bodies never read the (1/h, Fn) record -- the
+// apply then needs 3 records per candidate, 105 KB, and two CTAs fit an SM.  MODE 2: only the other tiles.
+template <int SWEEP, int MODE> struct NRecM { static constexpr int v = (SWEEP == SW_APPLY && MODE == 1) ? 3 : NRec<SWEEP>::v; };
+template <int SWEEP, int MODE> struct MinBlocks {
+    static constexpr int v = (SWEEP == SW_DENSITY || SWEEP == SW_LIMITER || (SWEEP == SW_APPLY && MODE == 1)) ? 2 : 1;
+};
 
-template <int SWEEP, int KERNEL>
-__global__ void __launch_bounds__(TILE_THREADS, MinBlocks<SWEEP>::v)
+template <int SWEEP, int KERNEL, int MODE>
+__global__ void __launch_bounds__(TILE_THREADS, MinBlocks<SWEEP, MODE>::v)
 k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
-    constexpr int NV = NRec<SWEEP>::v;
+    constexpr int NV = NRecM<SWEEP, MODE>::v;
     extern __shared__ __align__(16) unsigned char smem[];
     __shared__ TileS S;
     double2* F = reinterpret_cast<double2*>(smem);               // F[record * TILE_CMAXP + slot]
@@ -303,7 +308,8 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
     for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
         const uint32_t flags = A.tflags[tile];
         if (!(flags & TILE_FLAG_OK)) continue;
-        const bool uni = (flags & TILE_FLAG_UNIH) != 0;
+        const bool uni = MODE == 1 ? true : (MODE == 2 ? false : (flags & TILE_FLAG_UNIH) != 0);
+        if (MODE != 0 && ((flags & TILE_FLAG_UNIH) != 0) != (MODE == 1)) continue;
         const TileDesc td = A.tiles[tile];
         // first two list rows: in flight while the records are staged
         const uint2 wi = A.winfo[(size_t)tile * TILE_WARPS + warp];
@@ -415,22 +421,30 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
     }
 }
 
-template <int SWEEP>
-static cudaError_t launch_t(Ctx* c, const SweepIn& a, cudaStream_t st) {
-    constexpr size_t smem = sizeof(double2) * NRec<SWEEP>::v * TILE_CMAXP + sizeof(double) * NRec<SWEEP>::e * TILE_CMAXP;
+template <int SWEEP, int MODE>
+static cudaError_t launch_m(Ctx* c, const SweepIn& a, cudaStream_t st) {
+    constexpr size_t smem = sizeof(double2) * NRecM<SWEEP, MODE>::v * TILE_CMAXP + sizeof(double) * NRec<SWEEP>::e * TILE_CMAXP;
     static bool attr_done = false;
     if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(k_tiled_sweep<SWEEP, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_tiled_sweep<SWEEP, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(k_tiled_sweep<SWEEP, 0, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_tiled_sweep<SWEEP, 1, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
     CellTable ct{c->cell_start, c->cell_end};
-    const int grid = c->tl.sms * MinBlocks<SWEEP>::v;
-    if (c->kernel == SPRAY_KERNEL_WENDLAND_C2) k_tiled_sweep<SWEEP, 1><<<grid, TILE_THREADS, smem, st>>>(c->dg, ct, a);
-    else k_tiled_sweep<SWEEP, 0><<<grid, TILE_THREADS, smem, st>>>(c->dg, ct, a);
+    const int grid = c->tl.sms * MinBlocks<SWEEP, MODE>::v;
+    if (c->kernel == SPRAY_KERNEL_WENDLAND_C2) k_tiled_sweep<SWEEP, 1, MODE><<<grid, TILE_THREADS, smem, st>>>(c->dg, ct, a);
+    else k_tiled_sweep<SWEEP, 0, MODE><<<grid, TILE_THREADS, smem, st>>>(c->dg, ct, a);
     c->launches += 1;
     return cudaGetLastError();
+}
+template <int SWEEP>
+static cudaError_t launch_t(Ctx* c, const SweepIn& a, cudaStream_t st) {
+    if (SWEEP == SW_APPLY) {          // uniform-h tiles at two CTAs per SM, then whatever is left
+        cudaError_t e = launch_m<SWEEP, 1>(c, a, st);
+        return e != cudaSuccess ? e : launch_m<SWEEP, 2>(c, a, st);
+    }
+    return launch_m<SWEEP, 0>(c, a, st);
 }
 
 cudaError_t launch_tiled_sweep(Ctx* c, int sweep, const TiledArgs& t, cudaStream_t st) {

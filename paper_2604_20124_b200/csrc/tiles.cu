@@ -131,7 +131,6 @@ struct ListArgs {
     const TileDesc* tiles;
     unsigned long long* ctr;           // CTR_*
     uint2* pool;
-    unsigned long long pool_cap;       // uint2 units
     uint2* winfo;                      // [tile][warp]: (pool offset, rounds)
     uint32_t* lcount;                  // [tile][TILE_T]: n_gather | n_sym << 16
     uint32_t* tflags;                  // [tile]
@@ -144,7 +143,7 @@ struct ListArgs {
 constexpr int COLW = TILE_BXMAX + 4;
 constexpr uint32_t LIST_RECHECK = 0x8000u;   // flat-list flag: classify this hit again (fp32 bounds, then exact fp64)
 constexpr int LIST_BS = LIST_BC + 1;        // rows of a (thread, bank) bucket incl. the trash row
-constexpr int LIST_LCAP = LIST_RMAX;       // builder: provisional hits per thread (flat list)
+constexpr int LIST_LCAP = LIST_RMAX;       // builder: rows of the schedule staging area (one column per thread)
 constexpr size_t BL_OFF_XY = 0;                                                         // float4 [CMAXP/2]: (x0, x1, y0, y1) of slots 2p, 2p+1
 constexpr size_t BL_OFF_ZT = BL_OFF_XY + sizeof(float4) * (TILE_CMAXP / 2);             // float4 [CMAXP/2]: (z0, z1, T0, T1), T = (2h)^2
 constexpr size_t BL_OFF_L = BL_OFF_ZT + sizeof(float4) * (TILE_CMAXP / 2);              // u16 [LIST_LCAP][TILE_THREADS]
@@ -162,12 +161,6 @@ __device__ __forceinline__ void unpk2(f32x2 v, float& a, float& b) { asm("mov.b6
 __device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) { f32x2 r; asm("sub.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
 __device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) { f32x2 r; asm("mul.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
 __device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
-
-// predicated 16-bit shared-memory store + pointer bump (keeps the scan loop free of branches)
-__device__ __forceinline__ void append_if(bool hit, uint32_t& addr, uint32_t v) {
-    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %1, 0;\n\t@p st.shared.u16 [%0], %2;\n\t@p add.u32 %0, %0, %3;\n\t}"
-                 : "+r"(addr) : "r"((uint32_t)hit), "h"((uint16_t)v), "n"(2 * TILE_THREADS) : "memory");
-}
 
 // One candidate of the scan: if r2 < hi, store (value | LIST_RECHECK unless 0 < r2 < 2 half_lo) at the bucket row pointer and
 // advance it, clamped at `end` (the bucket's trash row: a pointer that reaches it reports the overflow); nflag counts
@@ -664,7 +657,7 @@ cudaError_t launch_build_tiles(Ctx* c, cudaStream_t st) {
         if ((e = cudaFuncSetAttribute(k_build_lists, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BL_SMEM)) != cudaSuccess) return e;
         attr_done = true;
     }
-    ListArgs A{c->pk.p0, c->pk.p1, t.tiles, t.ctr, t.pool, (unsigned long long)t.pool_cap, t.winfo, t.lcount, t.tflags, t.tiletab, t.fast,
+    ListArgs A{c->pk.p0, c->pk.p1, t.tiles, t.ctr, t.pool, t.winfo, t.lcount, t.tflags, t.tiletab, t.fast,
                c->hglob, c->dev_status};
     k_build_lists<<<t.sms, TILE_THREADS, BL_SMEM, st>>>(c->dg, ct, A);
     c->launches += 3;
