@@ -152,8 +152,6 @@ constexpr size_t BL_OFF_COL = BL_OFF_B + sizeof(uint16_t) * 4 * LIST_BS * TILE_T
 constexpr size_t BL_SMEM = BL_OFF_COL + sizeof(uint16_t) * TILE_MAXR * COLW;
 static_assert(BL_SMEM + sizeof(TileS) + 256 <= 227 * 1024, "list builder shared memory");
 
-__device__ __forceinline__ uint32_t get8(unsigned long long x, int b) { return (uint32_t)(x >> (8 * b)) & 0xFFu; }
-
 // packed fp32 pairs (sm_100 FADD2 / FMUL2 / FFMA2): one instruction tests two candidates
 typedef unsigned long long f32x2;
 __device__ __forceinline__ f32x2 pk2(float a, float b) { f32x2 r; asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(a), "f"(b)); return r; }
@@ -430,14 +428,14 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
         // ---- split every bank bucket of the target between its two threads (alternate entries)
         const uint32_t cnt_o = __shfl_xor_sync(0xFFFFFFFFu, cnt, 1);
         ng += __shfl_xor_sync(0xFFFFFFFFu, ng, 1);
-        unsigned long long cu = 0;                                      // 8 x 8-bit: entries of bank beta that are mine
+        uint32_t cu = 0;                                                // 8 x 4-bit: entries of bank beta that are mine (<= LIST_BC / 2)
         uint32_t n_lane = 0, nsym = 0;
 #pragma unroll
         for (int beta = 0; beta < 8; ++beta) {
             const uint32_t cb = ((bank_owner(beta) == u ? cnt : cnt_o) >> (8 * bank_local(beta))) & 0xFFu;
             const uint32_t f = (uint32_t)(u + beta) & 1u;
             const uint32_t mine = (cb + 1u - f) >> 1;
-            cu |= (unsigned long long)mine << (8 * beta);
+            cu |= mine << (4 * beta);
             n_lane += mine; nsym += cb;
         }
         uint32_t R = n_lane;
@@ -452,53 +450,62 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
         if (!bad) {
             // ---- emit my half-list in scheduled order (see the header): phase t = rounds [tR/8, (t+1)R/8) in bank
             //      (j + t) & 7; what a phase cannot hold (overflow) fills the holes of other phases; the rest are dummies.
-            unsigned long long ovr = 0;                                 // 8 x 8-bit: entries of each bank beyond its phase
-            uint32_t ovtot = 0;
-#pragma unroll
-            for (int beta = 0; beta < 8; ++beta) {
-                const int t = (beta - j) & 7;
-                const uint32_t cap = (((uint32_t)(t + 1) * R) >> 3) - (((uint32_t)t * R) >> 3);
-                const uint32_t c = get8(cu, beta);
-                const uint32_t o = c > cap ? c - cap : 0u;
-                ovr |= (unsigned long long)o << (8 * beta);
-                ovtot += o;
-            }
-            const unsigned long long ov0 = ovr;                         // full overflow of each bank
-            // schedule into my (now free) flat-list column, then pack 4 rounds per 8-byte store
-            uint16_t* out = Lf + tid;                                   // out[r * TILE_THREADS]
+            // R = 8 m + 4 e (e = 0, 1): phase t starts at t m + e (t >> 1) and holds m + e (t & 1) rounds.
+            const uint32_t m8 = R >> 3, e4 = (R >> 2) & 1u;
+            uint16_t* out = Lf + tid;                                   // my column of the schedule: out[r * TILE_THREADS]
             const uint16_t* Bp = B + (tid & ~1);
-            // pass 1 (lockstep, R rounds): every phase takes its own bank's entries up to its capacity; a hole gets the
-            // dummy slot of the phase's bank (any value >= TILE_CMAX marks a hole)
+            uint32_t own[8], ovr[8];                                    // per phase: entries placed in the phase / left over
+            const uint16_t* bq[8];                                      // per phase: my entries of its bank (stride 2 rows)
+            uint32_t Hw = 0;                                            // 8 x 4-bit: holes of each phase
 #pragma unroll
             for (int t = 0; t < 8; ++t) {
                 const int beta = (j + t) & 7;
-                const uint32_t start = ((uint32_t)t * R) >> 3, cap = (((uint32_t)(t + 1) * R) >> 3) - start;
-                const uint32_t own = get8(cu, beta) - get8(ov0, beta);
+                const uint32_t cap = m8 + (e4 & (uint32_t)(t & 1));
+                const uint32_t c = (cu >> (4 * beta)) & 15u;
+                own[t] = min(c, cap);
+                ovr[t] = c - own[t];
+                Hw |= (cap - own[t]) << (4 * t);
                 // my entries of bank beta: indices f, f+2, ... of the bucket of thread bank_owner(beta)
-                const uint16_t* bp = Bp + (bank_local(beta) * LIST_BS + ((u + beta) & 1)) * TILE_THREADS + bank_owner(beta);
-                const uint16_t dummy = (uint16_t)(TILE_CMAX + beta);
-                for (uint32_t k = 0; k < cap; ++k) {
-                    uint16_t item = dummy;
-                    if (k < own) item = bp[2 * k * TILE_THREADS];
-                    out[(start + k) * TILE_THREADS] = item;
+                bq[t] = Bp + (bank_local(beta) * LIST_BS + ((u + beta) & 1)) * TILE_THREADS + bank_owner(beta);
+            }
+            // pass 1 (lockstep): every phase takes its own bank's entries up to its capacity; a hole gets the dummy slot
+            // of the phase's bank
+            for (uint32_t k = 0; k < m8; ++k) {
+#pragma unroll
+                for (int t = 0; t < 8; ++t) {
+                    uint16_t item = (uint16_t)(TILE_CMAX + ((j + t) & 7));
+                    if (k < own[t]) item = bq[t][2 * k * TILE_THREADS];
+                    out[((uint32_t)t * m8 + (e4 ? (uint32_t)(t >> 1) : 0u) + k) * TILE_THREADS] = item;
                 }
             }
-            // pass 2: pack 4 rounds per 8-byte store; the holes take the overflow entries bank by bank while there are any
-            int b2 = -1;
-            uint32_t k2 = 0, kend = 0;
-            auto fill = [&](uint32_t e) -> uint32_t {
-                if (e >= (uint32_t)TILE_CMAX && ovtot) {
-                    while (k2 == kend) { ++b2; kend = get8(cu, b2); k2 = kend - get8(ov0, b2); }
-                    e = Bp[(bank_local(b2) * LIST_BS + ((u + b2) & 1) + 2 * k2) * TILE_THREADS + bank_owner(b2)];
-                    ++k2; --ovtot;
+            if (e4) {
+#pragma unroll
+                for (int t = 1; t < 8; t += 2) {
+                    uint16_t item = (uint16_t)(TILE_CMAX + ((j + t) & 7));
+                    if (m8 < own[t]) item = bq[t][2 * m8 * TILE_THREADS];
+                    out[((uint32_t)t * m8 + (uint32_t)(t >> 1) + m8) * TILE_THREADS] = item;
                 }
-                return e;
-            };
+            }
+            // the left-over entries go into the holes, phase by phase (a phase has either holes or left-overs)
+            {
+                int th = -1;
+                uint32_t hrem = 0;
+#pragma unroll
+                for (int t = 0; t < 8; ++t) {
+                    for (uint32_t e = 0; e < ovr[t]; ++e) {
+                        while (hrem == 0 && th < 7) { ++th; hrem = (Hw >> (4 * th)) & 15u; }
+                        if (hrem == 0) break;                           // cannot happen: n_lane <= R
+                        const uint32_t pos = (((uint32_t)(th + 1) * R) >> 3) - hrem;
+                        --hrem;
+                        out[pos * TILE_THREADS] = bq[t][2 * (own[t] + e) * TILE_THREADS];
+                    }
+                }
+            }
+            // pass 2: pack 4 rounds per 8-byte store
             uint2* blk = A.pool + off + lane;
             for (uint32_t r4 = 0; r4 < R; r4 += 4) {
-                uint32_t e0 = out[r4 * TILE_THREADS], e1 = out[(r4 + 1) * TILE_THREADS];
-                uint32_t e2 = out[(r4 + 2) * TILE_THREADS], e3 = out[(r4 + 3) * TILE_THREADS];
-                if (ovtot) { e0 = fill(e0); e1 = fill(e1); e2 = fill(e2); e3 = fill(e3); }
+                const uint32_t e0 = out[r4 * TILE_THREADS], e1 = out[(r4 + 1) * TILE_THREADS];
+                const uint32_t e2 = out[(r4 + 2) * TILE_THREADS], e3 = out[(r4 + 3) * TILE_THREADS];
                 blk[(size_t)(r4 >> 2) * 32] = make_uint2(e0 | (e1 << 16), e2 | (e3 << 16));
             }
             if (u == 0) A.lcount[(size_t)tile * TILE_T + tgt] = active ? (ng | (nsym << 16)) : 0u;
