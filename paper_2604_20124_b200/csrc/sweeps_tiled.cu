@@ -308,11 +308,14 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
     for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
         const uint32_t flags = A.tflags[tile];
         if (!(flags & TILE_FLAG_OK)) continue;
-        const bool uni = MODE == 1 ? true : (MODE == 2 ? false : (flags & TILE_FLAG_UNIH) != 0);
-        if (MODE != 0 && ((flags & TILE_FLAG_UNIH) != 0) != (MODE == 1)) continue;
+        const bool tile_uni = (flags & TILE_FLAG_NONUNI) == 0;
+        const bool uni = MODE == 1 ? true : (MODE == 2 ? false : tile_uni);
+        if (MODE != 0 && tile_uni != (MODE == 1)) continue;
+        const bool half_ok = ((flags >> (warp / (TILE_WARPS / 2))) & 1u) != 0;   // this warp's half of the tile has lists
         const TileDesc td = A.tiles[tile];
         // first two list rows: in flight while the records are staged
-        const uint2 wi = A.winfo[(size_t)tile * TILE_WARPS + warp];
+        uint2 wi = A.winfo[(size_t)tile * TILE_WARPS + warp];
+        if (!half_ok) wi.y = 0u;
         const uint2* lp = A.pool + wi.x + lane;
         const uint2 l0 = wi.y ? __ldcs(lp) : make_uint2(0u, 0u);
         const uint2 l1 = wi.y > 4 ? __ldcs(lp + 32) : make_uint2(0u, 0u);
@@ -355,7 +358,7 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
         // ---- this thread's target
-        const bool active = tgt < (int)td.nt;
+        const bool active = half_ok && tgt < (int)td.nt;
         uint32_t i = 0;
         Tgt T{};
         if (active) {

@@ -125,7 +125,28 @@ k_make_tiles(DevGrid g, CellTable ct, const double* __restrict__ hglob, uint32_t
     }
 }
 
+// ------------------------------------------------------------------------------------------- tile tables
+// TileS of every tile, computed once per build and kept in global memory: the list builder and every sweep copy
+// them into shared memory instead of recomputing them.
+__global__ void __launch_bounds__(128)
+k_tile_tables(DevGrid g, CellTable ct, const TileDesc* __restrict__ tiles, const unsigned long long* __restrict__ ctr,
+              uint32_t* __restrict__ tiletab) {
+    __shared__ TileS S;
+    const uint32_t ntiles = (uint32_t)ctr[CTR_NTILES];
+    for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const TileDesc td = tiles[tile];
+        __syncthreads();
+        tile_setup(td, g, ct, S);
+        uint32_t* dst = tiletab + (size_t)tile * TILES_WORDS;
+        const uint32_t* src = reinterpret_cast<const uint32_t*>(&S);
+        for (int w = threadIdx.x; w < TILES_WORDS; w += blockDim.x) dst[w] = src[w];
+    }
+}
+
 // ------------------------------------------------------------------------------------------- list builder
+// One CTA of BL_THREADS threads builds the lists of HALF a tile (targets [128 half, 128 half + 128), i.e. warps
+// 8 half .. 8 half + 7 of the sweeps' CTA), so that two CTAs fit on an SM and one's barriers and staging latencies are
+// covered by the other's scan.  Work unit w = 2 tile + half.
 struct ListArgs {
     const double2 *p0, *p1;            // sorted (x, y), (z, h)
     const TileDesc* tiles;
@@ -133,24 +154,30 @@ struct ListArgs {
     uint2* pool;
     uint2* winfo;                      // [tile][warp]: (pool offset, rounds)
     uint32_t* lcount;                  // [tile][TILE_T]: n_gather | n_sym << 16
-    uint32_t* tflags;                  // [tile]
-    uint32_t* tiletab;                 // [tile][TILES_WORDS]
+    uint32_t* tflags;                  // [tile], zeroed before the launch; each half ORs its bits in
+    const uint32_t* tiletab;           // [tile][TILES_WORDS]
     uint8_t* fast;                     // [n] sorted order: 1 = served by the tiled kernels
     const double* hglob;
     uint32_t* status;
 };
 
+constexpr int BL_THREADS = TILE_THREADS / 2;
+constexpr int BL_WARPS = BL_THREADS / 32;
+constexpr int BL_TGT = TILE_T / 2;
 constexpr int COLW = TILE_BXMAX + 4;
-constexpr uint32_t LIST_RECHECK = 0x8000u;   // flat-list flag: classify this hit again (fp32 bounds, then exact fp64)
+constexpr uint32_t LIST_RECHECK = 0x8000u;   // bucket-entry flag: classify this hit again (fp32 bounds, then exact fp64)
 constexpr int LIST_BS = LIST_BC + 1;        // rows of a (thread, bank) bucket incl. the trash row
-constexpr int LIST_LCAP = LIST_RMAX;       // builder: rows of the schedule staging area (one column per thread)
+constexpr int LIST_LCAP = LIST_RMAX;       // rows of the schedule staging area (one column per thread)
 constexpr size_t BL_OFF_XY = 0;                                                         // float4 [CMAXP/2]: (x0, x1, y0, y1) of slots 2p, 2p+1
 constexpr size_t BL_OFF_ZT = BL_OFF_XY + sizeof(float4) * (TILE_CMAXP / 2);             // float4 [CMAXP/2]: (z0, z1, T0, T1), T = (2h)^2
-constexpr size_t BL_OFF_L = BL_OFF_ZT + sizeof(float4) * (TILE_CMAXP / 2);              // u16 [LIST_LCAP][TILE_THREADS]
-constexpr size_t BL_OFF_B = BL_OFF_L + sizeof(uint16_t) * LIST_LCAP * TILE_THREADS;     // u16 [4][LIST_BS][TILE_THREADS]
-constexpr size_t BL_OFF_COL = BL_OFF_B + sizeof(uint16_t) * 4 * LIST_BS * TILE_THREADS; // u16 [MAXR][COLW]
+constexpr size_t BL_OFF_L = 0;                                                          // u16 [LIST_LCAP][BL_THREADS]: the schedule, written after
+                                                                                        // the scan is over -- shares the space of XY / ZT
+constexpr size_t BL_CAND_END = BL_OFF_ZT + sizeof(float4) * (TILE_CMAXP / 2);
+constexpr size_t BL_L_END = BL_OFF_L + sizeof(uint16_t) * LIST_LCAP * BL_THREADS;
+constexpr size_t BL_OFF_B = BL_CAND_END > BL_L_END ? BL_CAND_END : BL_L_END;             // u16 [4][LIST_BS][BL_THREADS]
+constexpr size_t BL_OFF_COL = BL_OFF_B + sizeof(uint16_t) * 4 * LIST_BS * BL_THREADS;   // u16 [MAXR][COLW]
 constexpr size_t BL_SMEM = BL_OFF_COL + sizeof(uint16_t) * TILE_MAXR * COLW;
-static_assert(BL_SMEM + sizeof(TileS) + 256 <= 227 * 1024, "list builder shared memory");
+static_assert(2 * (BL_SMEM + sizeof(TileS) + 1280) <= 228 * 1024, "list builder: two CTAs per SM");
 
 // packed fp32 pairs (sm_100 FADD2 / FMUL2 / FFMA2): one instruction tests two candidates
 typedef unsigned long long f32x2;
@@ -175,7 +202,7 @@ __device__ __forceinline__ void append_flag(float r2, float hi, float half_lo, u
                  "@p add.u32 %0, %0, %8;\n\t"
                  "@q add.u32 %1, %1, 1;\n\t"
                  "min.u32 %0, %0, %5;\n\t}"
-                 : "+r"(addr), "+r"(nflag) : "f"(r2), "f"(hi), "f"(half_lo), "r"(end), "r"(v), "r"(v | LIST_RECHECK), "n"(2 * TILE_THREADS));
+                 : "+r"(addr), "+r"(nflag) : "f"(r2), "f"(hi), "f"(half_lo), "r"(end), "r"(v), "r"(v | LIST_RECHECK), "n"(2 * BL_THREADS));
     // no memory clobber: the loads of the next pairs must be free to move above the store; the buckets are read back
     // only after the fence that follows the scan
 }
@@ -185,32 +212,43 @@ __device__ __forceinline__ void append_flag(float r2, float hi, float half_lo, u
 __device__ __forceinline__ int bank_owner(int beta) { return (beta >> 1) & 1; }
 __device__ __forceinline__ int bank_local(int beta) { return ((beta >> 2) << 1) | (beta & 1); }
 
-__global__ void __launch_bounds__(TILE_THREADS, 1)
+
+__global__ void __launch_bounds__(BL_THREADS, 2)
 k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
     extern __shared__ __align__(16) unsigned char smem[];
     __shared__ TileS S;
-    __shared__ int s_bad, s_nonuni;
+    __shared__ int s_bad, s_nonuni, s_clo, s_chi;
+    __shared__ double s_h0;
     float4* XY = reinterpret_cast<float4*>(smem + BL_OFF_XY);
     float4* ZT = reinterpret_cast<float4*>(smem + BL_OFF_ZT);
     float* XYf = reinterpret_cast<float*>(XY);
     float* ZTf = reinterpret_cast<float*>(ZT);
-    uint16_t* Lf = reinterpret_cast<uint16_t*>(smem + BL_OFF_L);       // [k * TILE_THREADS + tid]
-    uint16_t* B = reinterpret_cast<uint16_t*>(smem + BL_OFF_B);        // [(b * LIST_BS + k) * TILE_THREADS + tid]
+    uint16_t* Lf = reinterpret_cast<uint16_t*>(smem + BL_OFF_L);       // [k * BL_THREADS + tid]
+    uint16_t* B = reinterpret_cast<uint16_t*>(smem + BL_OFF_B);        // [(b * LIST_BS + k) * BL_THREADS + tid]
     uint16_t* colofs = reinterpret_cast<uint16_t*>(smem + BL_OFF_COL); // [range][COLW]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int u = tid & 1, tgt = tid >> 1, j = lane & 7;
-    const uint32_t ntiles = (uint32_t)A.ctr[CTR_NTILES];
+    const int u = tid & 1, j = lane & 7;
+    const uint32_t nunits = 2u * (uint32_t)A.ctr[CTR_NTILES];
     const float Rmax = 2.0f * (float)A.hglob[1] * 1.000001f;
 
-    for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    for (uint32_t unit = blockIdx.x; unit < nunits; unit += gridDim.x) {
+        const uint32_t tile = unit >> 1;
+        const int half = (int)(unit & 1u);
         const TileDesc td = A.tiles[tile];
-        __syncthreads();                                                // previous tile done with smem
-        if (tid == 0) { s_bad = 0; s_nonuni = 0; }
-        tile_setup(td, g, ct, S);
-        {   // keep the tables for the sweeps
-            uint32_t* dst = A.tiletab + (size_t)tile * TILES_WORDS;
-            const uint32_t* src = reinterpret_cast<const uint32_t*>(&S);
-            for (int w = tid; w < TILES_WORDS; w += TILE_THREADS) dst[w] = src[w];
+        const int tgt = half * BL_TGT + (tid >> 1);                     // target index within the tile
+        const int twarp = half * BL_WARPS + warp;                       // warp index within the tile
+        if (half * BL_TGT >= (int)td.nt) {                              // no target in this half: empty lists
+            if (lane == 0) A.winfo[(size_t)tile * TILE_WARPS + twarp] = make_uint2(0u, 0u);
+            if (u == 0) A.lcount[(size_t)tile * TILE_T + tgt] = 0u;
+            if (tid == 0) atomicOr(&A.tflags[tile], TILE_FLAG_OK0 << half);
+            continue;
+        }
+        __syncthreads();                                                // previous unit done with smem
+        if (tid == 0) { s_bad = 0; s_nonuni = 0; s_clo = 1 << 20; s_chi = -1; }
+        {   // tile tables (k_tile_tables)
+            const uint32_t* src = A.tiletab + (size_t)tile * TILES_WORDS;
+            uint32_t* dst = reinterpret_cast<uint32_t*>(&S);
+            for (int w = tid; w < TILES_WORDS; w += BL_THREADS) dst[w] = src[w];
         }
         const int ncolv = td.cxb - td.cxa + 3;                          // virtual columns 0 .. ncolv-1
         // tile origin (centre of the tile's cell block) for the fp32 relative coordinates
@@ -221,39 +259,16 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
         const float ext = (float)fmax(fmax((0.5 * ncolv + 0.5) / g.inv[0], 2.5 / g.inv[1]), 2.5 / g.inv[2]);
         const float E = ext * 2.4e-7f;                                  // 4 * 2^-24 * ext
         const float Am = 4.4f * Rmax * E + 5.0f * E * E;
+        __syncthreads();
 
         // ---- per-range column offsets (slot of the first particle of each column, relative to r_base)
-        for (int w = tid; w < (int)S.nranges * COLW; w += TILE_THREADS) {
+        for (int w = tid; w < (int)S.nranges * COLW; w += BL_THREADS) {
             const int q = w / COLW, jj = w % COLW;
             const int4 ge = S.r_geo[q];
             if (jj <= ge.y) {
                 const uint32_t gs = (jj < ge.y) ? ct.cell_start[ge.w + jj] : S.r_vend[q];
                 colofs[q * COLW + jj] = (uint16_t)(gs - S.r_vstart[q]);
             }
-        }
-        // ---- stage the candidates as slot pairs: one warp per range; the odd pad slot of a range is put out of reach
-        {
-            const unsigned long long h0 = (unsigned long long)__double_as_longlong(A.p1[S.r_vstart[0]].y);
-            bool nonuni = false;
-            for (int q = warp; q < (int)S.nranges; q += TILE_WARPS) {
-                const uint32_t vs = S.r_vstart[q], len = S.r_vend[q] - vs, base = S.r_base[q];
-                const double shx = S.r_shift[q][0] * g.L[0], shy = S.r_shift[q][1] * g.L[1], shz = S.r_shift[q][2] * g.L[2];
-                for (uint32_t k = lane; k < ((len + 1u) & ~1u); k += 32) {
-                    float fx = 3.0e18f, fy = 3.0e18f, fz = 3.0e18f, T = 0.0f;
-                    if (k < len) {
-                        const double2 xy = A.p0[vs + k], zh = A.p1[vs + k];
-                        fx = (float)((xy.x - shx) - ox);                // image position next to the tile: x_b - shift*L
-                        fy = (float)((xy.y - shy) - oy);
-                        fz = (float)((zh.x - shz) - oz);
-                        const float Rb = 2.0f * (float)zh.y;
-                        T = Rb * Rb;
-                        nonuni |= (unsigned long long)__double_as_longlong(zh.y) != h0;
-                    }
-                    const uint32_t s = base + k, o = (s >> 1) * 4 + (s & 1);
-                    XYf[o] = fx; XYf[o + 2] = fy; ZTf[o] = fz; ZTf[o + 2] = T;
-                }
-            }
-            if (nonuni) s_nonuni = 1;
         }
         // ---- this thread's target
         const bool active = tgt < (int)td.nt;
@@ -276,7 +291,7 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
         const float Ra = 2.0f * (float)ha;
         const float Ta = Ra * Ra;
         const float Ta_hi = fmaf(Ta, 1.00001f, Am), Ta_lo = fmaf(Ta, 0.99999f, -Am);
-        // warp window in virtual columns / candidate rows
+        // warp window in virtual columns / candidate rows; the union over the warps is what this CTA stages
         int cmin = active ? tcol : 1 << 20, cmax = active ? tcol : -1;
         int ymin = active ? try_ : 4, ymax = active ? try_ : -1;
         int zmin = active ? trz : 4, zmax = active ? trz : -1;
@@ -285,6 +300,40 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
             cmin = min(cmin, __shfl_xor_sync(0xFFFFFFFFu, cmin, o)); cmax = max(cmax, __shfl_xor_sync(0xFFFFFFFFu, cmax, o));
             ymin = min(ymin, __shfl_xor_sync(0xFFFFFFFFu, ymin, o)); ymax = max(ymax, __shfl_xor_sync(0xFFFFFFFFu, ymax, o));
             zmin = min(zmin, __shfl_xor_sync(0xFFFFFFFFu, zmin, o)); zmax = max(zmax, __shfl_xor_sync(0xFFFFFFFFu, zmax, o));
+        }
+        if (lane == 0 && cmax >= 0) { atomicMin(&s_clo, cmin); atomicMax(&s_chi, cmax); }
+        if (tid == 0) s_h0 = ha;                                        // the half's first target: always there
+        __syncthreads();
+
+        // ---- stage the candidates of virtual columns [s_clo, s_chi + 2] as slot pairs: one warp per range; whole pairs
+        //      only (a pair cut by the window's edge is staged in full), the odd pad slot of a range is put out of reach
+        {
+            const unsigned long long h0 = (unsigned long long)__double_as_longlong(s_h0);
+            const int clo = s_clo, chi = s_chi + 2;
+            bool nonuni = false;
+            for (int q = warp; q < (int)S.nranges; q += BL_WARPS) {
+                const int4 ge = S.r_geo[q];
+                const int jlo = max(0, min(ge.y, clo - ge.z)), jhi = max(0, min(ge.y, chi + 1 - ge.z));
+                if (jhi <= jlo) continue;
+                const uint32_t vs = S.r_vstart[q], len = S.r_vend[q] - vs, base = S.r_base[q];
+                const uint32_t ka = (uint32_t)colofs[q * COLW + jlo] & ~1u, kb = ((uint32_t)colofs[q * COLW + jhi] + 1u) & ~1u;
+                const double shx = S.r_shift[q][0] * g.L[0], shy = S.r_shift[q][1] * g.L[1], shz = S.r_shift[q][2] * g.L[2];
+                for (uint32_t k = ka + lane; k < kb; k += 32) {
+                    float fx = 3.0e18f, fy = 3.0e18f, fz = 3.0e18f, T = 0.0f;
+                    if (k < len) {
+                        const double2 xy = A.p0[vs + k], zh = A.p1[vs + k];
+                        fx = (float)((xy.x - shx) - ox);                // image position next to the tile: x_b - shift*L
+                        fy = (float)((xy.y - shy) - oy);
+                        fz = (float)((zh.x - shz) - oz);
+                        const float Rb = 2.0f * (float)zh.y;
+                        T = Rb * Rb;
+                        nonuni |= (unsigned long long)__double_as_longlong(zh.y) != h0;
+                    }
+                    const uint32_t s = base + k, o = (s >> 1) * 4 + (s & 1);
+                    XYf[o] = fx; XYf[o + 2] = fy; ZTf[o] = fz; ZTf[o + 2] = T;
+                }
+            }
+            if (nonuni) s_nonuni = 1;                                   // some staged candidate differs from the first target's h
         }
         __syncthreads();
         const bool uni = s_nonuni == 0;
@@ -296,7 +345,7 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
         //      unrolled by two pairs the bucket of every append is a compile-time choice.  A hit that is not certain
         //      (0 < r2 < Ta_lo, uniform-h tiles only) carries LIST_RECHECK.
         const uint32_t bk0 = (uint32_t)__cvta_generic_to_shared(B + tid);
-        constexpr uint32_t BROW = 2u * TILE_THREADS;                    // bytes per bucket row
+        constexpr uint32_t BROW = 2u * BL_THREADS;                    // bytes per bucket row
         uint32_t nflag = 0;                                             // flagged hits of this thread
         uint32_t bp0 = bk0, bp1 = bk0 + LIST_BS * BROW, bp2 = bk0 + 2 * LIST_BS * BROW, bp3 = bk0 + 3 * LIST_BS * BROW;
         const uint32_t e0 = bk0 + LIST_BC * BROW, e1 = e0 + LIST_BS * BROW, e2 = e1 + LIST_BS * BROW, e3 = e2 + LIST_BS * BROW;
@@ -373,12 +422,12 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
             cnt = n0 | (n1 << 8) | (n2 << 16) | (n3 << 24);
             if (sees_self) {
                 const int b = bank_local((int)(s_self & 7u));
-                uint16_t* bb = B + (size_t)b * LIST_BS * TILE_THREADS + tid;
+                uint16_t* bb = B + (size_t)b * LIST_BS * BL_THREADS + tid;
                 const uint32_t nb = (cnt >> (8 * b)) & 0xFFu;
                 uint32_t k = 0;
-                while (k < nb && (bb[k * TILE_THREADS] & 0x7FFFu) != s_self) ++k;
+                while (k < nb && (bb[k * BL_THREADS] & 0x7FFFu) != s_self) ++k;
                 if (k < nb) {                                           // the last entry takes its place (order is free)
-                    bb[k * TILE_THREADS] = bb[(nb - 1) * TILE_THREADS];
+                    bb[k * BL_THREADS] = bb[(nb - 1) * BL_THREADS];
                     cnt -= 1u << (8 * b);
                 }
             }
@@ -387,10 +436,10 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
 #pragma unroll
         for (int b = 0; b < 4; ++b) {
             const uint32_t nb = ((b == 0 ? bp0 : b == 1 ? bp1 : b == 2 ? bp2 : bp3) - (bk0 + b * LIST_BS * BROW)) / BROW;
-            uint16_t* bb = B + (size_t)b * LIST_BS * TILE_THREADS + tid;
+            uint16_t* bb = B + (size_t)b * LIST_BS * BL_THREADS + tid;
             uint32_t w = 0;
             for (uint32_t k = 0; k < nb; ++k) {
-                const uint32_t v = bb[k * TILE_THREADS], s = v & 0x7FFFu;
+                const uint32_t v = bb[k * BL_THREADS], s = v & 0x7FFFu;
                 bool in_s = true, in_g = true;
                 if (v & LIST_RECHECK) {
                     const float4 c0 = XY[s >> 1], c1 = ZT[s >> 1];
@@ -415,9 +464,9 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
                         in_g = in_s && e2x < support2(ha);
                         if (in_s && !(e2x > 0.0)) coinc = true;         // coincident particles: left to the general kernels (A11)
                     }
-                    if (in_s) bb[w * TILE_THREADS] = (uint16_t)s;
+                    if (in_s) bb[w * BL_THREADS] = (uint16_t)s;
                 } else if (w != k) {
-                    bb[w * TILE_THREADS] = (uint16_t)s;
+                    bb[w * BL_THREADS] = (uint16_t)s;
                 }
                 w += in_s ? 1u : 0u;
                 ng += (in_s && in_g) ? 1u : 0u;
@@ -443,7 +492,7 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
         for (int o = 16; o; o >>= 1) R = max(R, __shfl_xor_sync(0xFFFFFFFFu, R, o));
         R = (R + 3u) & ~3u;
         // list storage: one fixed block of LIST_RMAX rounds per (tile, warp) -- no allocation, placement is deterministic
-        const unsigned long long off = ((unsigned long long)tile * TILE_WARPS + warp) * (unsigned long long)(LIST_RMAX / 4) * 32;
+        const unsigned long long off = ((unsigned long long)tile * TILE_WARPS + twarp) * (unsigned long long)(LIST_RMAX / 4) * 32;
         if (lane == 0 && R > (uint32_t)LIST_RMAX) s_bad = 1;
         __syncthreads();
         const bool bad = s_bad != 0;
@@ -452,7 +501,7 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
             //      (j + t) & 7; what a phase cannot hold (overflow) fills the holes of other phases; the rest are dummies.
             // R = 8 m + 4 e (e = 0, 1): phase t starts at t m + e (t >> 1) and holds m + e (t & 1) rounds.
             const uint32_t m8 = R >> 3, e4 = (R >> 2) & 1u;
-            uint16_t* out = Lf + tid;                                   // my column of the schedule: out[r * TILE_THREADS]
+            uint16_t* out = Lf + tid;                                   // my column of the schedule: out[r * BL_THREADS]
             const uint16_t* Bp = B + (tid & ~1);
             uint32_t own[8], ovr[8];                                    // per phase: entries placed in the phase / left over
             const uint16_t* bq[8];                                      // per phase: my entries of its bank (stride 2 rows)
@@ -466,7 +515,7 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
                 ovr[t] = c - own[t];
                 Hw |= (cap - own[t]) << (4 * t);
                 // my entries of bank beta: indices f, f+2, ... of the bucket of thread bank_owner(beta)
-                bq[t] = Bp + (bank_local(beta) * LIST_BS + ((u + beta) & 1)) * TILE_THREADS + bank_owner(beta);
+                bq[t] = Bp + (bank_local(beta) * LIST_BS + ((u + beta) & 1)) * BL_THREADS + bank_owner(beta);
             }
             // pass 1 (lockstep): every phase takes its own bank's entries up to its capacity; a hole gets the dummy slot
             // of the phase's bank
@@ -474,16 +523,16 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
 #pragma unroll
                 for (int t = 0; t < 8; ++t) {
                     uint16_t item = (uint16_t)(TILE_CMAX + ((j + t) & 7));
-                    if (k < own[t]) item = bq[t][2 * k * TILE_THREADS];
-                    out[((uint32_t)t * m8 + (e4 ? (uint32_t)(t >> 1) : 0u) + k) * TILE_THREADS] = item;
+                    if (k < own[t]) item = bq[t][2 * k * BL_THREADS];
+                    out[((uint32_t)t * m8 + (e4 ? (uint32_t)(t >> 1) : 0u) + k) * BL_THREADS] = item;
                 }
             }
             if (e4) {
 #pragma unroll
                 for (int t = 1; t < 8; t += 2) {
                     uint16_t item = (uint16_t)(TILE_CMAX + ((j + t) & 7));
-                    if (m8 < own[t]) item = bq[t][2 * m8 * TILE_THREADS];
-                    out[((uint32_t)t * m8 + (uint32_t)(t >> 1) + m8) * TILE_THREADS] = item;
+                    if (m8 < own[t]) item = bq[t][2 * m8 * BL_THREADS];
+                    out[((uint32_t)t * m8 + (uint32_t)(t >> 1) + m8) * BL_THREADS] = item;
                 }
             }
             // the left-over entries go into the holes, phase by phase (a phase has either holes or left-overs)
@@ -497,24 +546,25 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
                         if (hrem == 0) break;                           // cannot happen: n_lane <= R
                         const uint32_t pos = (((uint32_t)(th + 1) * R) >> 3) - hrem;
                         --hrem;
-                        out[pos * TILE_THREADS] = bq[t][2 * (own[t] + e) * TILE_THREADS];
+                        out[pos * BL_THREADS] = bq[t][2 * (own[t] + e) * BL_THREADS];
                     }
                 }
             }
             // pass 2: pack 4 rounds per 8-byte store
             uint2* blk = A.pool + off + lane;
             for (uint32_t r4 = 0; r4 < R; r4 += 4) {
-                const uint32_t e0 = out[r4 * TILE_THREADS], e1 = out[(r4 + 1) * TILE_THREADS];
-                const uint32_t e2 = out[(r4 + 2) * TILE_THREADS], e3 = out[(r4 + 3) * TILE_THREADS];
+                const uint32_t e0 = out[r4 * BL_THREADS], e1 = out[(r4 + 1) * BL_THREADS];
+                const uint32_t e2 = out[(r4 + 2) * BL_THREADS], e3 = out[(r4 + 3) * BL_THREADS];
                 blk[(size_t)(r4 >> 2) * 32] = make_uint2(e0 | (e1 << 16), e2 | (e3 << 16));
             }
             if (u == 0) A.lcount[(size_t)tile * TILE_T + tgt] = active ? (ng | (nsym << 16)) : 0u;
             if (active && u == 0) A.fast[i] = 1;
-            if (lane == 0) A.winfo[(size_t)tile * TILE_WARPS + warp] = make_uint2((uint32_t)off, R);
+            if (lane == 0) A.winfo[(size_t)tile * TILE_WARPS + twarp] = make_uint2((uint32_t)off, R);
         }
         if (tid == 0) {
-            A.tflags[tile] = bad ? 0u : (TILE_FLAG_OK | (s_nonuni ? 0u : TILE_FLAG_UNIH));
-            if (!bad) atomicAdd(&A.ctr[CTR_NFAST], (unsigned long long)td.nt);
+            const uint32_t bits = (bad ? 0u : (TILE_FLAG_OK0 << half)) | (s_nonuni ? TILE_FLAG_NONUNI : 0u);
+            if (bits) atomicOr(&A.tflags[tile], bits);
+            if (!bad) atomicAdd(&A.ctr[CTR_NFAST], (unsigned long long)min((int)td.nt - half * BL_TGT, BL_TGT));
         }
     }
 }
@@ -548,7 +598,9 @@ k_tiled_export(DevGrid g, ExportArgs A) {
     const int u = tid & 1, tgt = tid >> 1;
     const uint32_t ntiles = (uint32_t)A.ctr[CTR_NTILES];
     for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-        if (!(A.tflags[tile] & TILE_FLAG_OK)) continue;
+        const uint32_t flags = A.tflags[tile];
+        if (!(flags & TILE_FLAG_OK)) continue;
+        const bool half_ok = ((flags >> (warp / (TILE_WARPS / 2))) & 1u) != 0;
         const TileDesc td = A.tiles[tile];
         __syncthreads();
         {
@@ -557,7 +609,7 @@ k_tiled_export(DevGrid g, ExportArgs A) {
             for (int w = tid; w < TILES_WORDS; w += TILE_THREADS) dst[w] = src[w];
         }
         __syncthreads();
-        const bool active = tgt < (int)td.nt;
+        const bool active = half_ok && tgt < (int)td.nt;
         uint32_t i = 0;
         double xa = 0, ya = 0, za = 0, ha = 0;
         if (active) {
@@ -565,7 +617,8 @@ k_tiled_export(DevGrid g, ExportArgs A) {
             const double2 xy = A.p0[i], zh = A.p1[i];
             xa = xy.x; ya = xy.y; za = zh.x; ha = zh.y;
         }
-        const uint2 wi = A.winfo[(size_t)tile * TILE_WARPS + warp];
+        uint2 wi = A.winfo[(size_t)tile * TILE_WARPS + warp];
+        if (!half_ok) wi.y = 0u;
         const uint2* lp = A.pool + wi.x + lane;
         uint32_t cnt = 0;
         uint64_t dsum = 0, dxr = 0;
@@ -659,6 +712,8 @@ cudaError_t launch_build_tiles(Ctx* c, cudaStream_t st) {
     k_make_tiles<false><<<blocks, 256, 0, st>>>(c->dg, ct, c->hglob, t.bcount, t.tiles, (uint32_t)t.tile_cap, t.ctr);
     if ((e = launch_excl_scan_u32(c, t.bcount, nb, t.bcount + t.bundle_cap, st)) != cudaSuccess) return e;
     k_make_tiles<true><<<blocks, 256, 0, st>>>(c->dg, ct, c->hglob, t.bcount, t.tiles, (uint32_t)t.tile_cap, t.ctr);
+    k_tile_tables<<<t.sms * 8, 128, 0, st>>>(c->dg, ct, t.tiles, t.ctr, t.tiletab);
+    if ((e = cudaMemsetAsync(t.tflags, 0, sizeof(uint32_t) * (size_t)t.tile_cap, st)) != cudaSuccess) return e;
     static bool attr_done = false;
     if (!attr_done) {
         if ((e = cudaFuncSetAttribute(k_build_lists, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BL_SMEM)) != cudaSuccess) return e;
@@ -666,8 +721,8 @@ cudaError_t launch_build_tiles(Ctx* c, cudaStream_t st) {
     }
     ListArgs A{c->pk.p0, c->pk.p1, t.tiles, t.ctr, t.pool, t.winfo, t.lcount, t.tflags, t.tiletab, t.fast,
                c->hglob, c->dev_status};
-    k_build_lists<<<t.sms, TILE_THREADS, BL_SMEM, st>>>(c->dg, ct, A);
-    c->launches += 3;
+    k_build_lists<<<t.sms * 2, BL_THREADS, BL_SMEM, st>>>(c->dg, ct, A);
+    c->launches += 4;
     t.enabled = true;
     return cudaGetLastError();
 }

@@ -46,8 +46,12 @@ struct TileDesc {                    // 24 bytes
     uint32_t pad2;
 };
 
-constexpr uint32_t TILE_FLAG_OK = 1u;        // lists were built: the tiled kernels serve this tile
-constexpr uint32_t TILE_FLAG_UNIH = 2u;      // every target and candidate of the tile has the same h (bitwise)
+// Tile flags.  The lists of a tile are built in two halves (targets [0, TILE_T/2) and [TILE_T/2, TILE_T), i.e. the
+// first and the second TILE_WARPS/2 warps of a sweep's CTA); each half reports on its own.
+constexpr uint32_t TILE_FLAG_OK0 = 1u;       // lists of the first half were built: the tiled kernels serve those targets
+constexpr uint32_t TILE_FLAG_OK1 = 2u;       // same for the second half (= TILE_FLAG_OK0 << 1)
+constexpr uint32_t TILE_FLAG_OK = 3u;        // mask: any half
+constexpr uint32_t TILE_FLAG_NONUNI = 4u;    // NOT every target and candidate of the tile has the same h (bitwise)
 
 struct CellTable {
     const uint32_t* cell_start;
