@@ -266,3 +266,23 @@ def conduction(grid, kernel, x, y, z, h, m, rho, k, T, targets=None):
     r = np.asarray(rho, np.float64)
     r = r if targets is None else r[np.asarray(targets)]
     return dict(dudt=ap["y"] / r, S_dudt=ap["S_y"] / r)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# Row N3: continuity equation eq. (37) with the kernel-gradient-correction filter of eqs. (39)-(40),
+# oracle_kgc_continuity in spray_oracle.c.  Reading A28: where the moment matrix is singular (|det| <= 1e-12) L = I.
+def kgc_continuity(grid, kernel, x, y, z, h, m, rho, vx, vy, vz, use_cells=True, targets=None):
+    """Returns dict(drhodt, drhodt_raw, M, L, S_M, S_N) at the targets; M, L, S_M, S_N have shape (nt, 3, 3)."""
+    n = len(x)
+    (x, px), (y, py), (z, pz), (h, ph), (m, pm), (rho, pr) = _d(x), _d(y), _d(z), _d(h), _d(m), _d(rho)
+    (vx, pvx), (vy, pvy), (vz, pvz) = _d(vx), _d(vy), _d(vz)
+    t, pt, nt = _targets(targets, n)
+    out = {k: np.zeros(nt) for k in ("drhodt", "drhodt_raw")}
+    mats = {k: np.zeros((nt, 3, 3)) for k in ("M", "L", "S_M", "S_N")}
+    g = _grid(grid)
+    rc = lib().oracle_kgc_continuity(C.byref(g), int(kernel), C.c_int64(n), px, py, pz, ph, pm, pr, pvx, pvy, pvz,
+                                     int(use_cells), pt, C.c_int64(nt), _p(out["drhodt"]), _p(out["drhodt_raw"]),
+                                     _p(mats["M"]), _p(mats["L"]), _p(mats["S_M"]), _p(mats["S_N"]))
+    assert rc == 0
+    out.update(mats)
+    return out

@@ -495,3 +495,113 @@ int oracle_fld_apply(const oracle_grid_t* g, int kernel, int64_t n, const double
     search_free(&s);
     return 0;
 }
+
+/* ------------------------------------------------------------------ N3: continuity equation with kernel gradient correction
+ * eq. (37) P:L213 with the KGC filter of eqs. (39)-(40) P:L222-L228, over N_gather(a)\{a}:
+ *     M_a = sum_b (m_b/rho_b) gradW(x_ab,h_a) (x) x_ba         eq. (40): row i = dW/dx_i, column j = (x_b - x_a)_j
+ *     L_a = M_a^{-1}                                           eq. (40)
+ *     drho_a/dt = rho_a sum_b (m_b/rho_b) (v_a - v_b) . (L_a gradW(x_ab,h_a))      eq. (37) with eq. (39)
+ * gradW(x_ab,h) = F(r;h) x_ab / r (A4).  The inverse is Gauss-Jordan with partial pivoting in long double.  Reading A28
+ * (the paper is silent): where M_a is singular (|det M_a| <= 1e-12; M is dimensionless, the identity for a full support)
+ * the gradient is left uncorrected, L_a = I.  Second loop over the neighbours, as the paper states it (first L, then the
+ * corrected gradient pair by pair).
+ * Outputs per target t: Mout/Lout [t*9 + 3 i + j], drhodt, drhodt_raw (eq. (37) without the filter), and the absolute sums
+ * S_M[t*9 + ..] = sum_b |(m_b/rho_b) dW/dx_i x_ba,j|, S_N[t*9 + 3 i + j] = sum_b |(m_b/rho_b) (v_a - v_b)_i dW/dx_j|.
+ */
+static int invert3(const long double M[9], long double L[9], long double* det_out) {
+    long double A[3][6];
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j) { A[i][j] = M[3 * i + j]; A[i][3 + j] = (i == j) ? 1.0L : 0.0L; }
+    long double det = 1.0L;
+    for (int c = 0; c < 3; ++c) {
+        int piv = c;
+        for (int r = c + 1; r < 3; ++r) if (fabsl(A[r][c]) > fabsl(A[piv][c])) piv = r;
+        if (A[piv][c] == 0.0L) { *det_out = 0.0L; return -1; }
+        if (piv != c) {
+            for (int j = 0; j < 6; ++j) { long double t = A[c][j]; A[c][j] = A[piv][j]; A[piv][j] = t; }
+            det = -det;
+        }
+        det *= A[c][c];
+        long double inv = 1.0L / A[c][c];
+        for (int j = 0; j < 6; ++j) A[c][j] *= inv;
+        for (int r = 0; r < 3; ++r) {
+            if (r == c) continue;
+            long double f = A[r][c];
+            for (int j = 0; j < 6; ++j) A[r][j] -= f * A[c][j];
+        }
+    }
+    for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) L[3 * i + j] = A[i][3 + j];
+    *det_out = det;
+    return 0;
+}
+
+int oracle_kgc_continuity(const oracle_grid_t* g, int kernel, int64_t n, const double* x, const double* y, const double* z,
+                          const double* h, const double* m, const double* rho, const double* vx, const double* vy,
+                          const double* vz, int use_cells, const int64_t* targets, int64_t nt,
+                          double* drhodt, double* drhodt_raw, double* Mout, double* Lout, double* S_M, double* S_N) {
+    search_t s;
+    if (search_init(&s, g, n, x, y, z, h, use_cells)) return -1;
+    if (!targets) nt = n;
+#pragma omp parallel
+    {
+        ilist_t l = {0, 0, 0};
+#pragma omp for schedule(dynamic, 64)
+        for (int64_t t = 0; t < nt; ++t) {
+            int64_t a = targets ? targets[t] : t;
+            enumerate(&s, ORACLE_GATHER, a, &l);
+            long double M[9] = {0}, SM[9] = {0}, SN[9] = {0}, L[9];
+            for (int64_t k = 0; k < l.n; ++k) {                     /* eq. (40) */
+                int64_t b = l.v[k];
+                if (b == a) continue;
+                double d[3];
+                double r2 = pair_r2(&s, a, b, &d[0], &d[1], &d[2]);
+                if (r2 == 0.0) continue;
+                double r = sqrt(r2);
+                double Vb = m[b] / rho[b], Fa = oracle_F(kernel, r, h[a]);
+                for (int i = 0; i < 3; ++i) {
+                    double gi = Fa * (d[i] / r);                    /* dW/dx_i at a */
+                    for (int j = 0; j < 3; ++j) {
+                        double term = Vb * gi * (-d[j]);            /* x_ba = -x_ab */
+                        M[3 * i + j] += term;
+                        SM[3 * i + j] += fabs(term);
+                    }
+                }
+            }
+            long double det;
+            if (invert3(M, L, &det) != 0 || fabsl(det) <= 1e-12L) {  /* A28 */
+                for (int i = 0; i < 9; ++i) L[i] = (i % 4 == 0) ? 1.0L : 0.0L;
+            }
+            double Ld[9];
+            for (int i = 0; i < 9; ++i) Ld[i] = (double)L[i];
+            long double sc = 0, sr = 0;
+            for (int64_t k = 0; k < l.n; ++k) {                     /* eq. (37) with eq. (39) */
+                int64_t b = l.v[k];
+                if (b == a) continue;
+                double d[3];
+                double r2 = pair_r2(&s, a, b, &d[0], &d[1], &d[2]);
+                if (r2 == 0.0) continue;
+                double r = sqrt(r2);
+                double Vb = m[b] / rho[b], Fa = oracle_F(kernel, r, h[a]);
+                double gw[3], gc[3];
+                for (int i = 0; i < 3; ++i) gw[i] = Fa * (d[i] / r);
+                for (int i = 0; i < 3; ++i) gc[i] = Ld[3 * i] * gw[0] + Ld[3 * i + 1] * gw[1] + Ld[3 * i + 2] * gw[2];   /* eq. (39) */
+                double dv[3] = {vx[a] - vx[b], vy[a] - vy[b], vz[a] - vz[b]};
+                sc += Vb * (dv[0] * gc[0] + dv[1] * gc[1] + dv[2] * gc[2]);
+                sr += Vb * (dv[0] * gw[0] + dv[1] * gw[1] + dv[2] * gw[2]);
+                for (int i = 0; i < 3; ++i)
+                    for (int j = 0; j < 3; ++j) SN[3 * i + j] += fabs(Vb * dv[i] * gw[j]);
+            }
+            drhodt[t] = rho[a] * (double)sc;
+            if (drhodt_raw) drhodt_raw[t] = rho[a] * (double)sr;
+            for (int i = 0; i < 9; ++i) {
+                if (Mout) Mout[t * 9 + i] = (double)M[i];
+                if (Lout) Lout[t * 9 + i] = Ld[i];
+                if (S_M) S_M[t * 9 + i] = (double)SM[i];
+                if (S_N) S_N[t * 9 + i] = (double)SN[i];
+            }
+        }
+        free(l.v);
+    }
+    search_free(&s);
+    return 0;
+}
