@@ -161,6 +161,18 @@ int spray_neighbor_digest(spray_ctx* ctx, int symmetric, uint64_t* dsum, uint64_
 int spray_conduction(spray_ctx* ctx, const double* m, const double* rho, const double* k, const double* T, double* dudt,
                      void* stream);
 
+/* (N3) continuity equation with the kernel-gradient-correction (KGC) filter, P:L207-L228:
+ *       M_a = sum_b (m_b/rho_b) gradW(x_ab,h_a) (x) x_ba          eq. (40): row i = dW/dx_i, column j = (x_b - x_a)_j
+ *       L_a = M_a^{-1}                                            eq. (40)
+ *       drhodt_a = rho_a sum_b (m_b/rho_b) (v_a - v_b) . (L_a gradW(x_ab,h_a))      eq. (37) with eq. (39)
+ * over N_gather(a) \ {a}, from the neighbour lists of the last spray_build_cells.  Since L_a does not depend on b the sum is
+ * evaluated as L_a : sum_b (m_b/rho_b) (v_a - v_b) (x) gradW in the same sweep that accumulates M_a.  Where M_a is singular
+ * (|det M_a| <= 1e-12; A28) the gradient is left uncorrected (L_a = I).
+ * Inputs m, rho, vx, vy, vz in caller order.  drhodt [out, n]; L [out, nullable, 9 n]: L[(3 i + j) n + a] = (L_a)_ij;
+ * drhodt_raw [out, nullable, n]: eq. (37) without the filter. */
+int spray_kgc_continuity(spray_ctx* ctx, const double* m, const double* rho, const double* vx, const double* vy,
+                         const double* vz, double* drhodt, double* L, double* drhodt_raw, void* stream);
+
 /* (N1) implicit radiation step by Jacobi iteration, section 2.3 P:L268-L327.
  * Backward-Euler form of eqs. (47)-(48), i.e. eqs. (49)-(50), with the limiter frozen (mu[] given, A18).  Each of the
  * `niter` iterations (i) applies the FLD operator to the current iterate (spray_fld_apply FROZEN: Lambda_a, Gamma_a of eqs.

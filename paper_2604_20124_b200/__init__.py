@@ -24,7 +24,7 @@ DEV_H_EXCEEDS_HMAX, DEV_OUTSIDE_BOX, DEV_LIST_OVERFLOW = 1, 2, 4
 # every symbol include/spray.h declares
 EXPORTS = ["spray_version", "spray_create", "spray_destroy", "spray_last_error", "spray_check", "spray_launch_count", "spray_set_path", "spray_path_stats",
            "spray_build_cells", "spray_density", "spray_hydro_rhs", "spray_fld_apply", "spray_get_cell_table",
-           "spray_neighbor_counts", "spray_neighbor_lists", "spray_neighbor_digest", "spray_rad_jacobi", "spray_conduction", "spray_fp64_peak_probe"]
+           "spray_neighbor_counts", "spray_neighbor_lists", "spray_neighbor_digest", "spray_rad_jacobi", "spray_conduction", "spray_kgc_continuity", "spray_fp64_peak_probe"]
 
 
 class SprayError(RuntimeError):
@@ -65,6 +65,7 @@ def load():
     lib.spray_hydro_rhs.argtypes = [vp] + [vp] * 8 + [dbl] + [vp] * 5 + [vp]
     lib.spray_fld_apply.argtypes = [vp, vp, vp, vp, vp, dbl, i32, i32, vp, vp, vp, vp, vp, vp]
     lib.spray_conduction.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+    lib.spray_kgc_continuity.argtypes = [vp] * 10
     lib.spray_rad_jacobi.argtypes = [vp] + [vp] * 8 + [dbl, dbl, dbl, i32, i32, vp, vp, vp, vp]
     lib.spray_get_cell_table.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.spray_neighbor_counts.argtypes = [vp, i32, vp, vp]
@@ -211,6 +212,18 @@ class Spray:
                                        _ptr(dudt, f64, self.n), _stream())
         self._ck(rc, "spray_conduction")
         return dudt
+
+    def kgc_continuity(self, m, rho, vx, vy, vz, want_L=True, want_raw=True):
+        """Row N3: continuity equation eq. (37) with the KGC filter of eqs. (39)-(40) (include/spray.h).
+        Returns dict(drhodt, L [9, n] or None, drhodt_raw or None)."""
+        f64 = self.torch.float64
+        drhodt = self._out(None)
+        L = self.torch.empty((9, self.n), dtype=f64, device=self.device) if want_L else None
+        raw = self._out(None) if want_raw else None
+        a = [_ptr(t, f64, self.n) for t in (m, rho, vx, vy, vz)]
+        rc = self.lib.spray_kgc_continuity(self.h, *a, _ptr(drhodt, f64, self.n), _ptr(L), _ptr(raw), _stream())
+        self._ck(rc, "spray_kgc_continuity")
+        return dict(drhodt=drhodt, L=L, drhodt_raw=raw)
 
     def rad_jacobi(self, m, rho, mu, kappa_p, E_n, u_n, T_n, dTdu, dt, c_light=1.0, a_rad=1.0, niter=1, kmode=FLD_SYMMETRIC,
                    E0=None, want_resid=True):

@@ -338,6 +338,30 @@ int spray_conduction(spray_ctx* ctx, const double* m, const double* rho, const d
     return SPRAY_OK;
 }
 
+int spray_kgc_continuity(spray_ctx* ctx, const double* m, const double* rho, const double* vx, const double* vy,
+                         const double* vz, double* drhodt, double* L, double* drhodt_raw, void* stream) {
+    NEED_BUILT();
+    Ctx* c = &ctx->c;
+    if (c->n > 0 && (!m || !rho || !vx || !vy || !vz || !drhodt))
+        return fail(c, SPRAY_ERR_INVALID_ARG, "spray_kgc_continuity: NULL argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    double** f = c->s.f;
+    PrepJob pj{};
+    pj.m = m; pj.rho = rho; pj.vx = vx; pj.vy = vy; pj.vz = vz;
+    pj.sm = f[F_M]; pj.srho = f[F_RHO]; pj.svx = f[F_VX]; pj.svy = f[F_VY]; pj.svz = f[F_VZ]; pj.sV = f[F_V];
+    CK(launch_prep_kgc(c, pj, st), "kgc prologue");
+    if (c->tl.enabled) {
+        TiledArgs t{};
+        t.o0 = drhodt; t.o1 = L; t.o2 = drhodt_raw;
+        CK(launch_tiled_sweep(c, SW_KGC, t, st), "kgc: tiled sweep");
+    }
+    SweepArgs a = fallback_args(c);
+    a.m = f[F_M]; a.rho = f[F_RHO]; a.vx = f[F_VX]; a.vy = f[F_VY]; a.vz = f[F_VZ];
+    a.o0 = drhodt; a.o1 = L; a.o2 = drhodt_raw;
+    CK(launch_ref_sweep(c, SW_KGC, a, st), "kgc: sweep");
+    return SPRAY_OK;
+}
+
 int spray_rad_jacobi(spray_ctx* ctx, const double* m, const double* rho, const double* mu, const double* kappa_p,
                      const double* E_n, const double* u_n, const double* T_n, const double* dTdu, double dt, double c_light,
                      double a_rad, spray_fld_kernel_mode_t kmode, int niter, double* E, double* u, double* resid, void* stream) {

@@ -250,6 +250,24 @@ __global__ void k_prep_fld(PrepJob j, const uint32_t* __restrict__ perm, int64_t
     }
 }
 
+// N3: (z, V), (vx, vy), (vz, -), target record (rho, -)
+__global__ void k_prep_kgc(PrepJob j, const uint32_t* __restrict__ perm, int64_t n, PackedOut o,
+                           const unsigned long long* __restrict__ nfast) {
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const uint32_t p = perm[i];
+    const double m = __ldg(j.m + p), rho = __ldg(j.rho + p);
+    const double vx = __ldg(j.vx + p), vy = __ldg(j.vy + p), vz = __ldg(j.vz + p);
+    const double V = m / rho;
+    o.s0[i] = make_double2(o.p1[i].x, V);
+    o.s1[i] = make_double2(vx, vy);
+    o.s2[i] = make_double2(vz, 0.0);
+    o.t0[i] = make_double2(rho, 0.0);
+    if (!nfast || *nfast != (unsigned long long)n) {
+        j.sm[i] = m; j.srho[i] = rho; j.svx[i] = vx; j.svy[i] = vy; j.svz[i] = vz; j.sV[i] = V;
+    }
+}
+
 // per-cell max h (fp64 max is exact and order independent), global min/max of h, and the h <= h_max check
 __global__ void k_init_hglob(double* hglob) { hglob[0] = __longlong_as_double(0x7FF0000000000000ll); hglob[1] = 0.0; }
 
@@ -347,6 +365,13 @@ cudaError_t launch_prep_hydro(Ctx* c, const PrepJob& j, cudaStream_t st) {
 cudaError_t launch_prep_fld(Ctx* c, const PrepJob& j, cudaStream_t st) {
     if (c->n == 0) return cudaSuccess;
     k_prep_fld<<<cdiv64(c->n, 256), 256, 0, st>>>(j, c->perm, c->n, packed_out(c), nfast_ptr(c));
+    c->launches += 1;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_prep_kgc(Ctx* c, const PrepJob& j, cudaStream_t st) {
+    if (c->n == 0) return cudaSuccess;
+    k_prep_kgc<<<cdiv64(c->n, 256), 256, 0, st>>>(j, c->perm, c->n, packed_out(c), nfast_ptr(c));
     c->launches += 1;
     return cudaGetLastError();
 }

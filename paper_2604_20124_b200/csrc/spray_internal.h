@@ -113,6 +113,7 @@ struct PrepJob {
 cudaError_t launch_prep_density(Ctx* c, const double* m, cudaStream_t st);
 cudaError_t launch_prep_hydro(Ctx* c, const PrepJob& j, cudaStream_t st);
 cudaError_t launch_prep_fld(Ctx* c, const PrepJob& j, cudaStream_t st);
+cudaError_t launch_prep_kgc(Ctx* c, const PrepJob& j, cudaStream_t st);
 
 // ---- tiles.cu / sweeps_tiled.cu : tiled path
 struct TiledArgs {

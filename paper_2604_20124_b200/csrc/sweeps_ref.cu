@@ -56,12 +56,14 @@ __device__ __forceinline__ void ref_particle(const DevGrid& g, int64_t n, const 
     uint32_t cnt = 0;
     uint64_t dsum = 0, dxr = 0;
     double rho_a = 0, p_a = 0, vxa = 0, vya = 0, vza = 0, ac_a = 0, E_a = 0, mu_a = 0, Wn = 0, Fn = 0;
+    double km[6] = {0, 0, 0, 0, 0, 0}, kq[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};   // SW_KGC: sum c x_i x_j, sum c dv_i x_j
     Wn = sigma<KERNEL>() * hinv * hinv * hinv;          // sigma / h^3
     Fn = Wn * hinv;                                      // sigma / h^4
     if (SWEEP == SW_HYDRO) {
         rho_a = A.rho[i]; p_a = A.p[i]; vxa = A.vx[i]; vya = A.vy[i]; vza = A.vz[i]; ac_a = A.alpha[i] * A.cs[i];
     }
     if (SWEEP == SW_LIMITER) { E_a = A.E[i]; }
+    if (SWEEP == SW_KGC) { rho_a = A.rho[i]; vxa = A.vx[i]; vya = A.vy[i]; vza = A.vz[i]; }
     if (SWEEP == SW_APPLY) { E_a = A.E[i]; mu_a = A.mu[i]; }
     uint64_t lbase = 0;
     if (SWEEP == SW_LIST) lbase = A.offsets[ia];
@@ -130,6 +132,18 @@ __device__ __forceinline__ void ref_particle(const DevGrid& g, int64_t n, const 
                             const double cc = (A.m[j] / A.rho[j]) * (A.E[j] - E_a) * (Fn * shape_f<KERNEL>(r * hinv)) / r;
                             acc0 += cc * dx; acc1 += cc * dy; acc2 += cc * dz;
                         }
+                    } else if (SWEEP == SW_KGC) {
+                        if (in_g && !self && r2 > 0.0) {
+                            // eqs. (37), (39), (40) P:L213-L228: moment sums over N_gather(a), h_a only
+                            const double r = sqrt(r2);
+                            const double cc = (A.m[j] / A.rho[j]) * (Fn * shape_f<KERNEL>(r * hinv)) / r;
+                            const double cx = cc * dx, cy = cc * dy, cz = cc * dz;
+                            const double dvx = vxa - A.vx[j], dvy = vya - A.vy[j], dvz = vza - A.vz[j];
+                            km[0] += cx * dx; km[1] += cx * dy; km[2] += cx * dz; km[3] += cy * dy; km[4] += cy * dz; km[5] += cz * dz;
+                            kq[0] += dvx * cx; kq[1] += dvx * cy; kq[2] += dvx * cz;
+                            kq[3] += dvy * cx; kq[4] += dvy * cy; kq[5] += dvy * cz;
+                            kq[6] += dvz * cx; kq[7] += dvz * cy; kq[8] += dvz * cz;
+                        }
                     } else if (SWEEP == SW_APPLY) {
                         if (in_set && r2 > 0.0) {
                             // eq. (47) first term P:L270 on eq. (16); Fbar as P:L134 (A17)
@@ -184,6 +198,25 @@ __device__ __forceinline__ void ref_particle(const DevGrid& g, int64_t n, const 
         A.o0[ia] = acc0;
         if (A.o1) A.o1[ia] = acc1;
         if (A.o2) A.o2[ia] = acc2;
+    } else if (SWEEP == SW_KGC) {
+        // M_a = -sum c x (x) x, L_a = M_a^-1 by cofactors; singular -> L_a = I (A28)
+        const double m00 = -km[0], m01 = -km[1], m02 = -km[2], m11 = -km[3], m12 = -km[4], m22 = -km[5];
+        const double c00 = m11 * m22 - m12 * m12, c01 = m02 * m12 - m01 * m22, c02 = m01 * m12 - m02 * m11;
+        const double det = m00 * c00 + m01 * c01 + m02 * c02;
+        double l00 = 1.0, l01 = 0.0, l02 = 0.0, l11 = 1.0, l12 = 0.0, l22 = 1.0;
+        if (fabs(det) > 1e-12) {
+            const double id = 1.0 / det;
+            l00 = c00 * id; l01 = c01 * id; l02 = c02 * id;
+            l11 = (m00 * m22 - m02 * m02) * id; l12 = (m01 * m02 - m00 * m12) * id; l22 = (m00 * m11 - m01 * m01) * id;
+        }
+        const double corr = l00 * kq[0] + l11 * kq[4] + l22 * kq[8] + l01 * (kq[1] + kq[3]) + l02 * (kq[2] + kq[6]) + l12 * (kq[5] + kq[7]);
+        A.o0[ia] = rho_a * corr;
+        if (A.o1) {
+            double* Lo = A.o1 + ia;
+            Lo[0] = l00; Lo[n] = l01; Lo[2 * n] = l02; Lo[3 * n] = l01; Lo[4 * n] = l11; Lo[5 * n] = l12;
+            Lo[6 * n] = l02; Lo[7 * n] = l12; Lo[8 * n] = l22;
+        }
+        if (A.o2) A.o2[ia] = rho_a * (kq[0] + kq[4] + kq[8]);
     }
 }
 
@@ -219,6 +252,7 @@ cudaError_t launch_ref_sweep(Ctx* c, int sweep, const SweepArgs& a, cudaStream_t
         case SW_COUNT: return launch_k<SW_COUNT>(c, a, st);
         case SW_LIST: return launch_k<SW_LIST>(c, a, st);
         case SW_DIGEST: return launch_k<SW_DIGEST>(c, a, st);
+        case SW_KGC: return launch_k<SW_KGC>(c, a, st);
     }
     return cudaErrorInvalidValue;
 }

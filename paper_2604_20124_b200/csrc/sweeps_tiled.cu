@@ -93,6 +93,7 @@ template <> struct NRec<SW_DENSITY> { static constexpr int v = 2, e = 0; };   //
 template <> struct NRec<SW_HYDRO> { static constexpr int v = 6, e = 0; };     // (x,y) (z,V) (Q,vx) (vy,vz) (m,alpha c) (1/h,Fn)
 template <> struct NRec<SW_LIMITER> { static constexpr int v = 2, e = 1; };   // (x,y) (z,V) | E
 template <> struct NRec<SW_APPLY> { static constexpr int v = 4, e = 0; };     // (x,y) (z,V) (mu,E) (1/h,Fn)
+template <> struct NRec<SW_KGC> { static constexpr int v = 4, e = 0; };       // (x,y) (z,V) (vx,vy) (vz,-)
 
 struct SweepIn {
     const double2* rec[6];           // sorted global records, in the order of NRec
@@ -118,7 +119,10 @@ struct SweepIn {
     uint32_t* ocount;
 };
 
-struct Acc { double a0, a1, a2, a3, a4; };
+struct Acc {
+    double a0, a1, a2, a3, a4;
+    double k[15];                    // SW_KGC: sum c x_i x_j (xx, xy, xz, yy, yz, zz), then sum c dv_i x_j (row-major 3 x 3)
+};
 struct Tgt {                         // per-target constants
     double x, y, z, hinv, fn;
     double c0, c1, c2, c3, c4, c5;   // per sweep (see k_tiled_sweep)
@@ -178,6 +182,18 @@ __device__ __forceinline__ void pair_body(const double2* __restrict__ F, const d
         const double G = gshape<KERNEL, !UNI>(qa) * y;
         const double cc = (d1.y * (Ee[s] - T.c0)) * G;
         acc.a0 = fma(cc, dx, acc.a0); acc.a1 = fma(cc, dy, acc.a1); acc.a2 = fma(cc, dz, acc.a2);
+    } else if (SWEEP == SW_KGC) {
+        // eq. (40): M_a = sum V_b gradW (x) x_ba = -(kFn/h_a^4) sum c x_ab (x) x_ab, c = V_b F/(r kFn/h_a^4);
+        // eq. (37) with eq. (39): L_a : sum V_b v_ab (x) gradW = (kFn/h_a^4) L_a : sum c v_ab (x) x_ab.  h_a only.
+        const double2 d2 = F[2 * TILE_CMAXP + s], d3 = F[3 * TILE_CMAXP + s];
+        const double c = d1.y * (gshape<KERNEL, !UNI>(qa) * y);
+        const double cx = c * dx, cy = c * dy, cz = c * dz;
+        const double dvx = T.c3 - d2.x, dvy = T.c4 - d2.y, dvz = T.c5 - d3.x;
+        acc.k[0] = fma(cx, dx, acc.k[0]); acc.k[1] = fma(cx, dy, acc.k[1]); acc.k[2] = fma(cx, dz, acc.k[2]);
+        acc.k[3] = fma(cy, dy, acc.k[3]); acc.k[4] = fma(cy, dz, acc.k[4]); acc.k[5] = fma(cz, dz, acc.k[5]);
+        acc.k[6] = fma(dvx, cx, acc.k[6]); acc.k[7] = fma(dvx, cy, acc.k[7]); acc.k[8] = fma(dvx, cz, acc.k[8]);
+        acc.k[9] = fma(dvy, cx, acc.k[9]); acc.k[10] = fma(dvy, cy, acc.k[10]); acc.k[11] = fma(dvy, cz, acc.k[11]);
+        acc.k[12] = fma(dvz, cx, acc.k[12]); acc.k[13] = fma(dvz, cy, acc.k[13]); acc.k[14] = fma(dvz, cz, acc.k[14]);
     } else {
         // eq. (47) first term P:L270 on eq. (16); Fbar as P:L134 (A17)
         const double2 d2 = F[2 * TILE_CMAXP + s];
@@ -374,11 +390,16 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
             }
             if (SWEEP == SW_LIMITER) T.c0 = A.e1[i];                                         // E_a
             if (SWEEP == SW_APPLY) { const double2 me = A.rec[2][i]; T.c0 = me.y; T.c1 = me.x; T.c2 = 4.0 * me.x; }
+            if (SWEEP == SW_KGC) {
+                const double2 q1 = A.rec[2][i], q2 = A.rec[3][i];
+                T.c0 = A.t0[i].x;                                                            // rho_a
+                T.c3 = q1.x; T.c4 = q1.y; T.c5 = q2.x;                                       // v_a
+            }
         }
         asm volatile("cp.async.wait_group 0;" ::: "memory");
         __syncthreads();
 
-        Acc acc{0, 0, 0, 0, 0};
+        Acc acc{};
         if (uni) pair_loop<SWEEP, KERNEL, true>(F, Ee, lp, wi.y, l0, l1, T, A.beta, sym, acc);
         else pair_loop<SWEEP, KERNEL, false>(F, Ee, lp, wi.y, l0, l1, T, A.beta, sym, acc);
         // ---- add the two half-lists of the target
@@ -388,6 +409,10 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
         if (SWEEP == SW_HYDRO) {
             acc.a3 += __shfl_xor_sync(0xFFFFFFFFu, acc.a3, 1);
             acc.a4 += __shfl_xor_sync(0xFFFFFFFFu, acc.a4, 1);
+        }
+        if (SWEEP == SW_KGC) {
+#pragma unroll
+            for (int e = 0; e < 15; ++e) acc.k[e] += __shfl_xor_sync(0xFFFFFFFFu, acc.k[e], 1);
         }
 
         if (active && u == 0) {
@@ -414,6 +439,29 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
                 A.me_out[i] = make_double2(mu, T.c0);
                 A.mu_sorted[i] = mu;
                 if (A.o1) { A.o1[ia] = gx; A.o1[A.n + ia] = gy; A.o1[2 * A.n + ia] = gz; }
+            } else if (SWEEP == SW_KGC) {
+                // M_a = -(kFn/h_a^4) sum c x (x) x (symmetric), L_a = M_a^-1 by cofactors; singular -> L_a = I (A28)
+                const double fn = T.fn;
+                const double m00 = -fn * acc.k[0], m01 = -fn * acc.k[1], m02 = -fn * acc.k[2];
+                const double m11 = -fn * acc.k[3], m12 = -fn * acc.k[4], m22 = -fn * acc.k[5];
+                const double c00 = m11 * m22 - m12 * m12, c01 = m02 * m12 - m01 * m22, c02 = m01 * m12 - m02 * m11;
+                const double det = m00 * c00 + m01 * c01 + m02 * c02;
+                double l00 = 1.0, l01 = 0.0, l02 = 0.0, l11 = 1.0, l12 = 0.0, l22 = 1.0;
+                if (fabs(det) > 1e-12) {
+                    const double id = 1.0 / det;
+                    l00 = c00 * id; l01 = c01 * id; l02 = c02 * id;
+                    l11 = (m00 * m22 - m02 * m02) * id; l12 = (m01 * m02 - m00 * m12) * id; l22 = (m00 * m11 - m01 * m01) * id;
+                }
+                const double* q = acc.k + 6;                     // q[3 i + j] = sum c dv_i x_j
+                const double corr = l00 * q[0] + l11 * q[4] + l22 * q[8] + l01 * (q[1] + q[3]) + l02 * (q[2] + q[6]) + l12 * (q[5] + q[7]);
+                A.o0[ia] = T.c0 * (fn * corr);
+                if (A.o1) {
+                    double* Lo = A.o1 + ia;
+                    Lo[0] = l00; Lo[A.n] = l01; Lo[2 * A.n] = l02;
+                    Lo[3 * A.n] = l01; Lo[4 * A.n] = l11; Lo[5 * A.n] = l12;
+                    Lo[6 * A.n] = l02; Lo[7 * A.n] = l12; Lo[8 * A.n] = l22;
+                }
+                if (A.o2) A.o2[ia] = T.c0 * (fn * (q[0] + q[4] + q[8]));
             } else {
                 const double yv = sc * acc.a0, lam = sc * acc.a1;
                 A.o0[ia] = yv;
@@ -469,6 +517,9 @@ cudaError_t launch_tiled_sweep(Ctx* c, int sweep, const TiledArgs& t, cudaStream
         case SW_APPLY:
             a.rec[2] = pk.me; a.rec[3] = pk.hh;
             return launch_t<SW_APPLY>(c, a, st);
+        case SW_KGC:
+            a.rec[2] = pk.s[1]; a.rec[3] = pk.s[2];
+            return launch_t<SW_KGC>(c, a, st);
     }
     return cudaErrorInvalidValue;
 }
