@@ -158,7 +158,7 @@ def main():
     ap.add_argument("--cpu-sample", type=int, default=200000, help="target particles per oracle step (cpu_baseline / reference arm)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--no-n1", action="store_true", help="skip the row-N1 measurement (Jacobi iterations of spray_rad_jacobi)")
+    ap.add_argument("--no-n1", action="store_true", help="skip the row-N1/N3 measurements (spray_rad_jacobi iterations, spray_kgc_continuity)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -335,6 +335,24 @@ def main():
               "flop_roofline_frac": pairs["apply"] * FLOPS[w.kernel]["apply"] / t_it / (fp64_meas * 1e12),
               "resid_last": float(rj["resid"][-1].item()), "note": "includes the one-off prologue of the call (1/%d per iteration)" % nit}
 
+    # ---- row N3: continuity equation with the KGC filter (spray_kgc_continuity), same lists; 60 flops per in-support ordered pair
+    #      over N_gather (distance 9, sqrt + 1/r + F 12, grad W and V_b 6, moment matrix 12, v_ab 3, velocity moments 18)
+    n3 = None
+    if not args.no_n1:
+        for _ in range(2):
+            sp.kgc_continuity(d["m"], out["rho"], d["vx"], d["vy"], d["vz"], want_L=False, want_raw=False)
+        torch.cuda.synchronize()
+        r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        nrep = 5
+        r0.record()
+        for _ in range(nrep):
+            sp.kgc_continuity(d["m"], out["rho"], d["vx"], d["vy"], d["vz"], want_L=False, want_raw=False)
+        r1.record()
+        torch.cuda.synchronize()
+        t_k = r0.elapsed_time(r1) * 1e-3 / nrep
+        n3 = {"call": "spray_kgc_continuity", "ms_per_call": 1e3 * t_k, "pair_interactions_per_s": pairs["limiter"] / t_k,
+              "flops_per_pair": 60, "flop_roofline_frac": pairs["limiter"] * 60 / t_k / (fp64_meas * 1e12)}
+
     # ---- roofline: pass level and dominant kernel
     fl = FLOPS[w.kernel]
     visc_frac = 0.0 if not (np.any(w.vx) or np.any(w.vy) or np.any(w.vz)) else 0.5
@@ -378,7 +396,7 @@ def main():
                        "parallelism": "replicas only" if world > 1 else "1 GPU", "path": args.path,
                        "tiles": n_tiles, "tiled_fraction": n_fast / max(n, 1)},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
-            "fp64_probe_tflops": fp64_meas, "next_rows": {"N1_rad_jacobi": n1}}
+            "fp64_probe_tflops": fp64_meas, "next_rows": {"N1_rad_jacobi": n1, "N3_kgc_continuity": n3}}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

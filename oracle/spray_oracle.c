@@ -18,7 +18,8 @@
  * closer to the exact sum than any plain fp64 order (O8).
  *
  * Parity pins: every function below is pinned by tests/test_oracle_*.py (closed forms T1/T2/T13/T14,
- * lattice constants T3/T4/T6/T7, brute force T5, invariants T8-T12, symmetries T15), except the
+ * lattice constants T3/T4/T6/T7, brute force T5, invariants T8-T12, symmetries T15; oracle_kgc_continuity by
+ * tests/test_oracle_kgc.py: lattice constant, exact linear fields, brute force, rotation, closed form), except the
  * choice "viscosity acts only for w < 0" (A6) which is PARITY UNPINNED: both readings satisfy every
  * invariant the paper states; the reading is fixed by SURVEY.md §8(c2) A6 / DESIGN.md.
  */
