@@ -9,7 +9,7 @@ from workloads import Grid
 from parity_util import compare_isolated, gpu_isolated, make_ctx, oracle_isolated, u32, upload
 
 pytestmark = pytest.mark.gpu
-PATHS = [0]
+PATHS = [0, 1]          # 0 = general kernels only, 1 = tiled kernels + general kernels for what they decline
 
 
 def test_error_codes():
@@ -81,6 +81,16 @@ def test_empty_and_single_particle(path):
         fl = sp.fld_apply(m, m, m, m)
         assert float(fl["y"][0]) == 0.0 and float(fl["diag"][0]) == 0.0
         assert float(fl["mu"][0]) == pytest.approx(1.0 / 3.0 / 4.0, rel=1e-15)      # R = 0: lambda = 1/3, mu = c/(3 rho kappa)
+        # next rows on one particle: no neighbour, so no conduction, L = I (A28) and no density change
+        assert float(sp.conduction(m, m, m, m)[0]) == 0.0
+        kg = sp.kgc_continuity(m, m, m, m, m)
+        assert float(kg["drhodt"][0]) == 0.0 and float(kg["drhodt_raw"][0]) == 0.0
+        assert kg["L"].flatten().tolist() == [1.0, 0.0, 0.0, 0.0, 1.0, 0.0, 0.0, 0.0, 1.0]
+    # ... and on the empty set
+    sp.build_cells(g, 0, e, e, e, e)
+    assert sp.conduction(e, e, e, e).numel() == 0
+    assert sp.kgc_continuity(e, e, e, e, e)["drhodt"].numel() == 0
+    assert sp.rad_jacobi(e, e, e, e, e, e, e, e, 0.1, niter=2)["E"].numel() == 0
     assert sp.check() == 0
 
 
@@ -136,6 +146,12 @@ def test_all_particles_in_one_cell_and_coincident(path):
     sp.build_cells(w.grid, w.kernel, d["x"], d["y"], d["z"], d["h"])
     mu_full = O.limiter(w.grid, w.kernel, w.x, w.y, w.z, w.h, w.m, w.rho_nom, w.kappa, w.E, w.c_light)["mu"]
     compare_isolated(gpu_isolated(sp, d, w, mu_in=mu_full), oracle_isolated(w, mu_full=mu_full))
+    # row N3 with coincident particles: pairs at r = 0 add nothing to the moment sums on either side
+    o = O.kgc_continuity(w.grid, w.kernel, w.x, w.y, w.z, w.h, w.m, w.rho_nom, w.vx, w.vy, w.vz)
+    r = sp.kgc_continuity(d["m"], d["rho_nom"], d["vx"], d["vy"], d["vz"])
+    lo = np.linalg.norm(o["L"].reshape(-1, 9), axis=1)
+    scale = w.rho_nom * lo * np.linalg.norm(o["S_N"].reshape(-1, 9), axis=1) * (1 + lo * np.linalg.norm(o["S_M"].reshape(-1, 9), axis=1))
+    assert np.all(np.abs(r["drhodt"].cpu().numpy() - o["drhodt"]) <= 1e-11 * scale)
     assert sp.check() == 0
 
 
