@@ -132,9 +132,8 @@ struct Tgt {                         // per-target constants
 // UNI: every particle of the tile has the target's h, so F(r;h_b) = F(r;h_a), the normalisation kFn/h^4 is applied
 // once per target after the loop (k_tiled_sweep) and no support clamp is needed.
 template <int SWEEP, int KERNEL, bool UNI>
-__device__ __forceinline__ void pair_body(const double2* __restrict__ F, const double* __restrict__ Ee, uint32_t s, const Tgt& T,
-                                          double beta, bool sym, Acc& acc) {
-    const double2 d0 = F[s], d1 = F[TILE_CMAXP + s];
+__device__ __forceinline__ void pair_body(const double2* __restrict__ F, const double* __restrict__ Ee, uint32_t s, const double2 d0,
+                                          const double2 d1, const Tgt& T, double beta, bool sym, Acc& acc) {
     const double dx = T.x - d0.x, dy = T.y - d0.y, dz = T.z - d1.x;
     const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
     const double y = rsqrt_fast(r2);                     // 1/r  (r2 > 0: coincident pairs never reach the tiled lists)
@@ -274,20 +273,40 @@ __device__ __forceinline__ void hydro_group2(const double2* __restrict__ F, uint
 }
 
 template <int SWEEP, int KERNEL, bool UNI>
+__device__ __forceinline__ void pair_body(const double2* __restrict__ F, const double* __restrict__ Ee, uint32_t s, const Tgt& T,
+                                          double beta, bool sym, Acc& acc) {
+    pair_body<SWEEP, KERNEL, UNI>(F, Ee, s, F[s], F[TILE_CMAXP + s], T, beta, sym, acc);
+}
+
+template <int SWEEP, int KERNEL, bool UNI>
 __device__ __forceinline__ void pair_loop(const double2* __restrict__ F, const double* __restrict__ Ee, const uint2* __restrict__ lp,
-                                          uint32_t R, uint2 cur, uint2 nxt, const Tgt& T, double beta, bool sym, Acc& acc) {
+                                          uint32_t R, uint2 cur, uint2 nxt, uint2 nx2, const Tgt& T, double beta, bool sym, Acc& acc) {
+    // list rows are read three iterations ahead of their use (the compiler sinks the load to the end of the iteration, which
+    // leaves two full iterations of this warp to cover the DRAM latency of the streamed lists)
+    // Density and limiter (two records per pair, the lightest pair bodies): the position records of the first pair of an
+    // iteration are read from shared memory during the iteration before (slot 0 when there is none: read and not used), so
+    // that the shared-memory round trip, long when the data pipe is busy, is not exposed at the top of every iteration.
+    // Measured: -5 % for these two sweeps, +1-2 % for the heavier ones, which therefore do not do it.
+    constexpr bool PIPE_FIRST = SWEEP == SW_DENSITY || SWEEP == SW_LIMITER;
+    double2 q0 = F[cur.x & 0xFFFFu], q1 = F[TILE_CMAXP + (cur.x & 0xFFFFu)];
     for (uint32_t r4 = 0; r4 < R; r4 += 4) {
-        const uint2 nx2 = (r4 + 8 < R) ? __ldcs(lp + (size_t)(r4 / 4 + 2) * 32) : make_uint2(0u, 0u);
+        const uint2 nx3 = (r4 + 12 < R) ? __ldcs(lp + (size_t)(r4 / 4 + 3) * 32) : make_uint2(0u, 0u);
+        const uint32_t sn = nxt.x & 0xFFFFu;
         if (SWEEP == SW_HYDRO) {
             hydro_group2<KERNEL, UNI>(F, cur.x & 0xFFFFu, cur.x >> 16, T, beta, acc);
             hydro_group2<KERNEL, UNI>(F, cur.y & 0xFFFFu, cur.y >> 16, T, beta, acc);
         } else {
-            pair_body<SWEEP, KERNEL, UNI>(F, Ee, cur.x & 0xFFFFu, T, beta, sym, acc);
+            if (PIPE_FIRST) {
+                pair_body<SWEEP, KERNEL, UNI>(F, Ee, cur.x & 0xFFFFu, q0, q1, T, beta, sym, acc);
+                q0 = F[sn]; q1 = F[TILE_CMAXP + sn];
+            } else {
+                pair_body<SWEEP, KERNEL, UNI>(F, Ee, cur.x & 0xFFFFu, T, beta, sym, acc);
+            }
             pair_body<SWEEP, KERNEL, UNI>(F, Ee, cur.x >> 16, T, beta, sym, acc);
             pair_body<SWEEP, KERNEL, UNI>(F, Ee, cur.y & 0xFFFFu, T, beta, sym, acc);
             pair_body<SWEEP, KERNEL, UNI>(F, Ee, cur.y >> 16, T, beta, sym, acc);
         }
-        cur = nxt; nxt = nx2;
+        cur = nxt; nxt = nx2; nx2 = nx3;
     }
 }
 
@@ -329,12 +348,13 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
         if (MODE != 0 && tile_uni != (MODE == 1)) continue;
         const bool half_ok = ((flags >> (warp / (TILE_WARPS / 2))) & 1u) != 0;   // this warp's half of the tile has lists
         const TileDesc td = A.tiles[tile];
-        // first two list rows: in flight while the records are staged
+        // first three list rows: in flight while the records are staged
         uint2 wi = A.winfo[(size_t)tile * TILE_WARPS + warp];
         if (!half_ok) wi.y = 0u;
         const uint2* lp = A.pool + wi.x + lane;
         const uint2 l0 = wi.y ? __ldcs(lp) : make_uint2(0u, 0u);
         const uint2 l1 = wi.y > 4 ? __ldcs(lp + 32) : make_uint2(0u, 0u);
+        const uint2 l2 = wi.y > 8 ? __ldcs(lp + 64) : make_uint2(0u, 0u);
         __syncthreads();                                         // previous tile done with the staged records
         {   // tile tables as the list builder left them
             const uint32_t* src = A.tiletab + (size_t)tile * TILES_WORDS;
@@ -342,6 +362,34 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
             for (int w = tid; w < TILES_WORDS; w += TILE_THREADS) dst[w] = src[w];
         }
         __syncthreads();
+        // ---- this thread's target.  Except in the hydro kernel (register pressure: measured slower) its loads go out before
+        //      the staging traffic, so they are back when the pair loop starts.
+        constexpr bool EARLY_TARGET = SWEEP != SW_HYDRO;
+        const bool active = half_ok && tgt < (int)td.nt;
+        uint32_t i = 0, ia = 0;
+        Tgt T{};
+        auto load_target = [&]() {
+            if (!active) return;
+            i = tile_target(td, S, tgt);
+            ia = A.perm[i];                                      // caller index of the target: needed only in the epilogue
+            const double2 xy = A.rec[0][i], zh = A.p1[i], hv = A.hh[i];
+            T.x = xy.x; T.y = xy.y; T.z = zh.x; T.hinv = hv.x; T.fn = hv.y;
+            if (SWEEP == SW_DENSITY) T.c0 = A.rec[1][i].y;                                   // m_a
+            if (SWEEP == SW_HYDRO) {
+                const double2 t0 = A.t0[i], q1 = A.rec[2][i], q2 = A.rec[3][i];
+                T.c0 = t0.x; T.c1 = t0.y;                                                    // p_a/rho_a, 1/rho_a
+                T.c2 = A.rec[4][i].y;                                                        // alpha_a c_a
+                T.c3 = q1.y; T.c4 = q2.x; T.c5 = q2.y;                                       // v_a
+            }
+            if (SWEEP == SW_LIMITER) T.c0 = A.e1[i];                                         // E_a
+            if (SWEEP == SW_APPLY) { const double2 me = A.rec[2][i]; T.c0 = me.y; T.c1 = me.x; T.c2 = 4.0 * me.x; }
+            if (SWEEP == SW_KGC) {
+                const double2 q1 = A.rec[2][i], q2 = A.rec[3][i];
+                T.c0 = A.t0[i].x;                                                            // rho_a
+                T.c3 = q1.x; T.c4 = q1.y; T.c5 = q2.x;                                       // v_a
+            }
+        };
+        if (EARLY_TARGET) load_target();
         // ---- stage the candidate records: one warp per range.  Ranges that need no periodic shift (all but those of
         //      tiles at a periodic face) are copied with cp.async (LDGSTS): no register round trip, every copy of the
         //      thread in flight at once, completion awaited just before the barrier that precedes the pair loop.
@@ -373,35 +421,13 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
             }
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
-        // ---- this thread's target
-        const bool active = half_ok && tgt < (int)td.nt;
-        uint32_t i = 0;
-        Tgt T{};
-        if (active) {
-            i = tile_target(td, S, tgt);
-            const double2 xy = A.rec[0][i], zh = A.p1[i], hv = A.hh[i];
-            T.x = xy.x; T.y = xy.y; T.z = zh.x; T.hinv = hv.x; T.fn = hv.y;
-            if (SWEEP == SW_DENSITY) T.c0 = A.rec[1][i].y;                                   // m_a
-            if (SWEEP == SW_HYDRO) {
-                const double2 t0 = A.t0[i], q1 = A.rec[2][i], q2 = A.rec[3][i];
-                T.c0 = t0.x; T.c1 = t0.y;                                                    // p_a/rho_a, 1/rho_a
-                T.c2 = A.rec[4][i].y;                                                        // alpha_a c_a
-                T.c3 = q1.y; T.c4 = q2.x; T.c5 = q2.y;                                       // v_a
-            }
-            if (SWEEP == SW_LIMITER) T.c0 = A.e1[i];                                         // E_a
-            if (SWEEP == SW_APPLY) { const double2 me = A.rec[2][i]; T.c0 = me.y; T.c1 = me.x; T.c2 = 4.0 * me.x; }
-            if (SWEEP == SW_KGC) {
-                const double2 q1 = A.rec[2][i], q2 = A.rec[3][i];
-                T.c0 = A.t0[i].x;                                                            // rho_a
-                T.c3 = q1.x; T.c4 = q1.y; T.c5 = q2.x;                                       // v_a
-            }
-        }
+        if (!EARLY_TARGET) load_target();
         asm volatile("cp.async.wait_group 0;" ::: "memory");
         __syncthreads();
 
         Acc acc{};
-        if (uni) pair_loop<SWEEP, KERNEL, true>(F, Ee, lp, wi.y, l0, l1, T, A.beta, sym, acc);
-        else pair_loop<SWEEP, KERNEL, false>(F, Ee, lp, wi.y, l0, l1, T, A.beta, sym, acc);
+        if (uni) pair_loop<SWEEP, KERNEL, true>(F, Ee, lp, wi.y, l0, l1, l2, T, A.beta, sym, acc);
+        else pair_loop<SWEEP, KERNEL, false>(F, Ee, lp, wi.y, l0, l1, l2, T, A.beta, sym, acc);
         // ---- add the two half-lists of the target
         acc.a0 += __shfl_xor_sync(0xFFFFFFFFu, acc.a0, 1);
         if (SWEEP != SW_DENSITY) acc.a1 += __shfl_xor_sync(0xFFFFFFFFu, acc.a1, 1);
@@ -416,7 +442,6 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
         }
 
         if (active && u == 0) {
-            const uint32_t ia = A.perm[i];
             const double sc = uni ? T.fn : 1.0;                  // kFn / h_a^4 where it was hoisted out of the loop
             if (SWEEP == SW_DENSITY) {
                 // self term m_a W(0; h_a) (A11)
