@@ -516,11 +516,12 @@ static cudaError_t launch_m(Ctx* c, const SweepIn& a, cudaStream_t st) {
 }
 template <int SWEEP>
 static cudaError_t launch_t(Ctx* c, const SweepIn& a, cudaStream_t st) {
-    if (SWEEP == SW_APPLY) {          // uniform-h tiles at two CTAs per SM, then whatever is left
+    if constexpr (SWEEP == SW_APPLY) {          // uniform-h tiles at two CTAs per SM, then whatever is left
         cudaError_t e = launch_m<SWEEP, 1>(c, a, st);
         return e != cudaSuccess ? e : launch_m<SWEEP, 2>(c, a, st);
+    } else {
+        return launch_m<SWEEP, 0>(c, a, st);
     }
-    return launch_m<SWEEP, 0>(c, a, st);
 }
 
 cudaError_t launch_tiled_sweep(Ctx* c, int sweep, const TiledArgs& t, cudaStream_t st) {
