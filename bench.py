@@ -379,7 +379,7 @@ def main():
     hydro_tflops = flops["hydro"] / calls["hydro"] / 1e12
     # dram__bytes_read.sum + dram__bytes_write.sum of k_tiled_sweep<1,0> per launch at c5, one ncu --set full capture
     # (profiles/r01d_ncu_full_tiled_path.md); null for other workloads
-    traffic = 6.14e9 + 0.67e9 if w.name.startswith("c5") else None
+    traffic = 6.01e9 + 0.67e9 if w.name.startswith("c5") else None
     roofline = {"bound": "alu", "kernel": "hydro pair sweep (spray_hydro_rhs: prologue k_prep_hydro + k_tiled_sweep<1>)",
                 "achieved": hydro_tflops, "peak": fp64_meas, "unit": "TFLOP/s", "frac": hydro_tflops / fp64_meas,
                 "peak_source": "DFMA-chain probe measured in this run (spray_fp64_peak_probe); nominal 148x64x2x1.965GHz = %.1f" % FP64_NOMINAL_TFLOPS,
