@@ -226,12 +226,19 @@ def quartic_positive_root(b, c):
 
 
 def rad_jacobi(grid, kernel, x, y, z, h, m, rho, mu, kappa_p, E_n, u_n, T_n, dTdu, dt, c_light, a_rad, niter,
-               sym_mode=True, E0=None):
+               sym_mode=True, E0=None, targets=None):
     """niter Jacobi iterations of eqs. (49)-(50) from the iterate E0 (default E_n).  Returns dict(E, u, chi, resid[niter],
-    S_offd): resid[k] = max_a |lhs - rhs| / |lhs| of eq. (49) for the iterate that ENTERS iteration k, 0 for k = 0."""
-    E_n = np.asarray(E_n, np.float64); u_n = np.asarray(u_n, np.float64); T_n = np.asarray(T_n, np.float64)
-    rho = np.asarray(rho, np.float64); kp = np.asarray(kappa_p, np.float64); dTdu = np.asarray(dTdu, np.float64)
-    E = E_n.copy() if E0 is None else np.asarray(E0, np.float64).copy()
+    S_offd): resid[k] = max_a |lhs - rhs| / |lhs| of eq. (49) for the iterate that ENTERS iteration k, 0 for k = 0.
+    targets (niter = 1 only: the first iteration needs the operator at the targets alone) restricts the outputs to a sample."""
+    E_full = np.asarray(E_n, np.float64) if E0 is None else np.asarray(E0, np.float64)
+    rho_full = np.asarray(rho, np.float64)
+    sel = slice(None)
+    if targets is not None:
+        assert niter == 1, "a sample of targets can only be followed for one iteration"
+        sel = np.asarray(targets, np.int64)
+    E_n = np.asarray(E_n, np.float64)[sel]; u_n = np.asarray(u_n, np.float64)[sel]; T_n = np.asarray(T_n, np.float64)[sel]
+    rho = rho_full[sel]; kp = np.asarray(kappa_p, np.float64)[sel]; dTdu = np.asarray(dTdu, np.float64)[sel]
+    E = E_full.copy() if targets is None else E_full
     u = u_n.copy()
     chi = T_n.copy()
     resid = np.zeros(niter)
@@ -239,7 +246,7 @@ def rad_jacobi(grid, kernel, x, y, z, h, m, rho, mu, kappa_p, E_n, u_n, T_n, dTd
     K = dt * c_light * kp                                                  # denominator of eq. (55)
     X = dt * rho * c_light * kp
     for k in range(niter):
-        ap = fld_apply(grid, kernel, x, y, z, h, m, rho, mu, E, sym_mode=sym_mode)
+        ap = fld_apply(grid, kernel, x, y, z, h, m, rho_full, mu, E, sym_mode=sym_mode, targets=targets)
         lam, gam, S_offd = ap["diag"], ap["offd"], ap["S_offd"]
         if k > 0:                                                          # both sides of eq. (49) for the current iterate
             rhs = E_n + dt * (lam * E + gam) + X * (a_rad * chi ** 4 - E)

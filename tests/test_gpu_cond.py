@@ -40,3 +40,22 @@ def test_conduction_parity(name):
     assert np.all(g0 == 0.0)
     assert sp.check() == 0
     print(name, "max normalised error", e)
+
+
+def test_conduction_full_size_sampled():
+    """Config 5 (16.7M particles), the launch configuration of bench.py: 2000 sampled targets against the oracle."""
+    import torch
+    w = W.make("c5")
+    i = np.arange(2000, dtype=np.uint64)
+    sel = np.unique((W.splitmix64(i + np.uint64(91)) % np.uint64(w.n)).astype(np.int64))
+    k = 0.2 + w.kappa / (1.0 + w.kappa)
+    T = 0.5 + w.E / np.max(w.E) + 0.1 * np.sin(9.0 * w.x)
+    o = O.conduction(w.grid, w.kernel, w.x, w.y, w.z, w.h, w.m, w.rho_nom, k, T, targets=sel)
+    d = upload(w)
+    sp = make_ctx(w)
+    sp.build_cells(w.grid, w.kernel, d["x"], d["y"], d["z"], d["h"])
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    g = sp.conduction(d["m"], d["rho_nom"], t(k), t(T)).cpu().numpy()
+    e = check("dudt", g[sel], o["dudt"], o["S_dudt"])
+    assert sp.path_stats()[1] == w.n          # every particle was served by the tiled kernels
+    print("c5 sampled: max normalised error", e)
