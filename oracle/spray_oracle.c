@@ -606,3 +606,101 @@ int oracle_kgc_continuity(const oracle_grid_t* g, int kernel, int64_t n, const d
     search_free(&s);
     return 0;
 }
+
+/* ------------------------------------------------------------------ N4: mesh-free laser ray tracing and energy deposition
+ * PAPER.md section 2.5.  f = n_e / n_c (dimensionless), kib = the absorption
+ * coefficient kappa^ib of eq. (70) per particle (an input: nu^ei and the material data it needs are not in the paper).
+ *   (1) gradient at the particles, literally as printed:  G_a = sum_b (m_b/rho_b) f_b gradW(x_ab, h_a)  over N_gather(a)\{a}
+ *   (2) each ray is a particle (x, v, P).  Per step of fixed dt ("for a fixed small dt"), at the ray's position x:
+ *         G(x)     = sum_a (m_a/rho_a) G_a W(|x - x_a|, h_a)          SPH interpolation with the particles' own h (A30)
+ *         kappa(x) = sum_a (m_a/rho_a) kib_a W(|x - x_a|, h_a)        ("gathered with standard SPH interpolation")
+ *         w_a      = (m_a/rho_a) W(|x - x_a|, h_a),  wsum = sum_a w_a
+ *         v <- v - (c^2/2) G(x) dt                                     eq. (72)
+ *         x <- x + v dt  (the new v: semi-implicit Euler, A31);  ds = |v| dt   (the discrete track length)
+ *         dE = P (1 - exp(-kappa(x) ds))                               eq. (71) P:L412 over the track with kappa held (A32)
+ *         P <- P - dE;   edep_a += dE w_a / wsum                       ("based on the kernel weight", normalised: A33)
+ *       The ray stops after nsteps, when P <= pmin, or when it has left the box in a non-periodic dimension (checked after
+ *       the move; periodic dimensions wrap the position) (A34).
+ * The ray loop is the plain definition: every particle is visited at every step (no cell list).  Sums in long double, particles
+ * in ascending caller index, rays in input order.
+ * Outputs: gradn[3n] (planes x, y, z), edep[n], rays_out[7 nrays] (planes x y z vx vy vz P), steps_out[nrays]. */
+int oracle_ray_deposit(const oracle_grid_t* g, int kernel, int64_t n, const double* x, const double* y, const double* z,
+                       const double* h, const double* m, const double* rho, const double* f, const double* kib,
+                       int use_cells, int64_t nrays, const double* rays_in, double dt, int64_t nsteps, double c_light,
+                       double pmin, double* gradn, double* edep, double* rays_out, int64_t* steps_out) {
+    search_t s;
+    if (search_init(&s, g, n, x, y, z, h, use_cells)) return -1;
+    /* (1) */
+#pragma omp parallel
+    {
+        ilist_t l = {0, 0, 0};
+#pragma omp for schedule(dynamic, 64)
+        for (int64_t a = 0; a < n; ++a) {
+            enumerate(&s, ORACLE_GATHER, a, &l);
+            long double sx = 0, sy = 0, sz = 0;
+            for (int64_t k = 0; k < l.n; ++k) {
+                int64_t b = l.v[k];
+                if (b == a) continue;
+                double dx, dy, dz;
+                double r2 = pair_r2(&s, a, b, &dx, &dy, &dz);
+                if (r2 == 0.0) continue;
+                double r = sqrt(r2);
+                double c = (m[b] / rho[b]) * f[b] * oracle_F(kernel, r, h[a]);
+                sx += c * (dx / r); sy += c * (dy / r); sz += c * (dz / r);
+            }
+            gradn[a] = (double)sx; gradn[n + a] = (double)sy; gradn[2 * n + a] = (double)sz;
+        }
+        free(l.v);
+    }
+    search_free(&s);
+    /* (2) */
+    long double* dep = (long double*)calloc((size_t)(n > 0 ? n : 1), sizeof(long double));
+    double* w = (double*)malloc(sizeof(double) * (size_t)(n > 0 ? n : 1));
+    if (!dep || !w) { free(dep); free(w); return -1; }
+    const double L[3] = {g->hi[0] - g->lo[0], g->hi[1] - g->lo[1], g->hi[2] - g->lo[2]};
+    for (int64_t q = 0; q < nrays; ++q) {
+        double p[3] = {rays_in[q], rays_in[nrays + q], rays_in[2 * nrays + q]};
+        double v[3] = {rays_in[3 * nrays + q], rays_in[4 * nrays + q], rays_in[5 * nrays + q]};
+        double P = rays_in[6 * nrays + q];
+        int64_t k = 0;
+        for (; k < nsteps && P > pmin; ++k) {
+            long double gx = 0, gy = 0, gz = 0, kap = 0, wsum = 0;
+            for (int64_t a = 0; a < n; ++a) {
+                double dx = min_image(p[0] - x[a], g->periodic[0], L[0]);
+                double dy = min_image(p[1] - y[a], g->periodic[1], L[1]);
+                double dz = min_image(p[2] - z[a], g->periodic[2], L[2]);
+                double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+                w[a] = 0.0;
+                if (!(r2 < 4.0 * (h[a] * h[a]))) continue;
+                double wa = (m[a] / rho[a]) * oracle_W(kernel, sqrt(r2), h[a]);
+                w[a] = wa;
+                gx += wa * gradn[a]; gy += wa * gradn[n + a]; gz += wa * gradn[2 * n + a];
+                kap += wa * kib[a];
+                wsum += wa;
+            }
+            const double acc = -0.5 * c_light * c_light * dt;
+            v[0] += acc * (double)gx; v[1] += acc * (double)gy; v[2] += acc * (double)gz;
+            const double ds = sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]) * dt;
+            if ((double)wsum > 0.0) {
+                const double dE = P * (1.0 - exp(-(double)kap * ds));
+                P -= dE;
+                const double sc = dE / (double)wsum;
+                for (int64_t a = 0; a < n; ++a) if (w[a] != 0.0) dep[a] += sc * w[a];
+            }
+            int out = 0;
+            for (int d = 0; d < 3; ++d) {
+                p[d] += v[d] * dt;
+                if (g->periodic[d]) {
+                    if (p[d] < g->lo[d]) p[d] += L[d]; else if (p[d] >= g->hi[d]) p[d] -= L[d];
+                } else if (p[d] < g->lo[d] || p[d] >= g->hi[d]) out = 1;
+            }
+            if (out) { ++k; break; }
+        }
+        for (int d = 0; d < 3; ++d) { rays_out[d * nrays + q] = p[d]; rays_out[(3 + d) * nrays + q] = v[d]; }
+        rays_out[6 * nrays + q] = P;
+        if (steps_out) steps_out[q] = k;
+    }
+    for (int64_t a = 0; a < n; ++a) edep[a] = (double)dep[a];
+    free(dep); free(w);
+    return 0;
+}
