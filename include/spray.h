@@ -190,6 +190,27 @@ int spray_rad_jacobi(spray_ctx* ctx, const double* m, const double* rho, const d
                      const double* E_n, const double* u_n, const double* T_n, const double* dTdu, double dt, double c_light,
                      double a_rad, spray_fld_kernel_mode_t kmode, int niter, double* E, double* u, double* resid, void* stream);
 
+/* (N4) mesh-free laser ray tracing and energy deposition, section 2.5.
+ * f = n_e/n_c (dimensionless), kib = the inverse-bremsstrahlung absorption coefficient kappa^ib of eq. (70) per particle (an
+ * input: nu^ei and the material data it needs are not in the paper).  Inputs m, rho, f, kib: [n], caller order.
+ *   (1) gradient at the particles, as printed at P:L420:  G_a = sum_b (m_b/rho_b) f_b gradW(x_ab, h_a)  over N_gather(a)\{a}
+ *       -> gradn (nullable, [3n] as x|y|z planes).
+ *   (2) every ray q is a particle (x, v, P).  rays_in [7 nrays]: planes x, y, z, vx, vy, vz, P.  Per step of the fixed
+ *       dt, with SPH interpolation at the ray's position over the particles with |x - x_a| < 2 h_a (own h, A30):
+ *         G(x) = sum_a V_a G_a W(|x-x_a|,h_a);  kappa(x) = sum_a V_a kib_a W;  w_a = V_a W;  wsum = sum_a w_a
+ *         v <- v - (c_light^2/2) G(x) dt              eq. (72)
+ *         ds = |v| dt;  dE = P (1 - exp(-kappa(x) ds)) (eq. (71), A32);  P <- P - dE  (skipped when wsum = 0)
+ *         edep_a += dE w_a / wsum                    ("based on the kernel weight", normalised: A33)
+ *         x <- x + v dt with the new v (A31); periodic dimensions wrap
+ *       A ray stops after nsteps steps, when P <= pmin, or once it has left [lo, hi) in a non-periodic dimension (A34).
+ *   Outputs: edep [n] caller order (overwritten); rays_out [7 nrays] final state; steps_out (nullable, i64[nrays]) steps taken.
+ * Uses the cell table of the last spray_build_cells (one warp per ray; rays are independent).  The deposit uses fp64
+ * atomics: its summation order, hence its last bits, may differ from run to run; everything else is reproducible.
+ * Errors: SPRAY_ERR_INVALID_ARG (NULL, nrays < 0, nsteps < 0, dt <= 0, c_light <= 0). nrays = 0 and n = 0 are valid. */
+int spray_ray_deposit(spray_ctx* ctx, const double* m, const double* rho, const double* f, const double* kib, int64_t nrays,
+                      const double* rays_in, double dt, int64_t nsteps, double c_light, double pmin, double* gradn, double* edep,
+                      double* rays_out, int64_t* steps_out, void* stream);
+
 /* Measurement aid: runs `iters` dependent DFMA per thread on `blocks` x `threads` threads
  * with 8 independent chains; out (device, [blocks*threads]) receives the sums so the work cannot be elided.
  * Used by bench.py to measure the sustained FP64 FMA peak the roofline is quoted against. */

@@ -299,16 +299,17 @@ def kgc_continuity(grid, kernel, x, y, z, h, m, rho, vx, vy, vz, use_cells=True,
 # Row N4: mesh-free laser ray tracing and inverse-bremsstrahlung deposition, section 2.5:
 # oracle_ray_deposit in spray_oracle.c (readings A29-A35 of DESIGN.md in its header).
 def ray_deposit(grid, kernel, x, y, z, h, m, rho, f, kib, rays, dt, nsteps, c_light=1.0, pmin=0.0, use_cells=True):
-    """rays: array (7, nrays) with rows x, y, z, vx, vy, vz, P.  Returns dict(gradn (3, n), edep (n), rays (7, nrays), steps)."""
+    """rays: array (7, nrays) with rows x, y, z, vx, vy, vz, P.  Returns dict(gradn (3, n), edep (n), rays (7, nrays), steps,
+    S_gradn (3, n): sums of the absolute pair contributions to gradn, the parity normaliser)."""
     n = len(x)
     (x, px), (y, py), (z, pz), (h, ph), (m, pm), (rho, pr), (f, pf), (kib, pk) = (_d(a) for a in (x, y, z, h, m, rho, f, kib))
     rays = np.ascontiguousarray(rays, dtype=np.float64)
     assert rays.ndim == 2 and rays.shape[0] == 7
     nr = rays.shape[1]
-    gradn = np.zeros((3, n)); edep = np.zeros(n); rout = np.zeros((7, nr)); steps = np.zeros(nr, np.int64)
+    gradn = np.zeros((3, n)); edep = np.zeros(n); rout = np.zeros((7, nr)); steps = np.zeros(nr, np.int64); S = np.zeros((3, n))
     g = _grid(grid)
     rc = lib().oracle_ray_deposit(C.byref(g), int(kernel), C.c_int64(n), px, py, pz, ph, pm, pr, pf, pk, int(use_cells),
                                   C.c_int64(nr), _p(rays), C.c_double(dt), C.c_int64(nsteps), C.c_double(c_light),
-                                  C.c_double(pmin), _p(gradn), _p(edep), _p(rout), _p(steps))
+                                  C.c_double(pmin), _p(gradn), _p(edep), _p(rout), _p(steps), _p(S))
     assert rc == 0
-    return dict(gradn=gradn, edep=edep, rays=rout, steps=steps)
+    return dict(gradn=gradn, edep=edep, rays=rout, steps=steps, S_gradn=S)

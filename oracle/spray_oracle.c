@@ -623,11 +623,12 @@ int oracle_kgc_continuity(const oracle_grid_t* g, int kernel, int64_t n, const d
  *       the move; periodic dimensions wrap the position) (A34).
  * The ray loop is the plain definition: every particle is visited at every step (no cell list).  Sums in long double, particles
  * in ascending caller index, rays in input order.
- * Outputs: gradn[3n] (planes x, y, z), edep[n], rays_out[7 nrays] (planes x y z vx vy vz P), steps_out[nrays]. */
+ * Outputs: gradn[3n] (planes x, y, z), edep[n], rays_out[7 nrays] (planes x y z vx vy vz P), steps_out[nrays];
+ * S_gradn[3n] (nullable): the sums of the absolute pair contributions to gradn, the normaliser of the parity tests (O8). */
 int oracle_ray_deposit(const oracle_grid_t* g, int kernel, int64_t n, const double* x, const double* y, const double* z,
                        const double* h, const double* m, const double* rho, const double* f, const double* kib,
                        int use_cells, int64_t nrays, const double* rays_in, double dt, int64_t nsteps, double c_light,
-                       double pmin, double* gradn, double* edep, double* rays_out, int64_t* steps_out) {
+                       double pmin, double* gradn, double* edep, double* rays_out, int64_t* steps_out, double* S_gradn) {
     search_t s;
     if (search_init(&s, g, n, x, y, z, h, use_cells)) return -1;
     /* (1) */
@@ -637,7 +638,7 @@ int oracle_ray_deposit(const oracle_grid_t* g, int kernel, int64_t n, const doub
 #pragma omp for schedule(dynamic, 64)
         for (int64_t a = 0; a < n; ++a) {
             enumerate(&s, ORACLE_GATHER, a, &l);
-            long double sx = 0, sy = 0, sz = 0;
+            long double sx = 0, sy = 0, sz = 0, ax = 0, ay = 0, az = 0;
             for (int64_t k = 0; k < l.n; ++k) {
                 int64_t b = l.v[k];
                 if (b == a) continue;
@@ -647,8 +648,10 @@ int oracle_ray_deposit(const oracle_grid_t* g, int kernel, int64_t n, const doub
                 double r = sqrt(r2);
                 double c = (m[b] / rho[b]) * f[b] * oracle_F(kernel, r, h[a]);
                 sx += c * (dx / r); sy += c * (dy / r); sz += c * (dz / r);
+                ax += fabs(c * (dx / r)); ay += fabs(c * (dy / r)); az += fabs(c * (dz / r));
             }
             gradn[a] = (double)sx; gradn[n + a] = (double)sy; gradn[2 * n + a] = (double)sz;
+            if (S_gradn) { S_gradn[a] = (double)ax; S_gradn[n + a] = (double)ay; S_gradn[2 * n + a] = (double)az; }
         }
         free(l.v);
     }

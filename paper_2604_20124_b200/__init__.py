@@ -24,7 +24,7 @@ DEV_H_EXCEEDS_HMAX, DEV_OUTSIDE_BOX, DEV_LIST_OVERFLOW = 1, 2, 4
 # every symbol include/spray.h declares
 EXPORTS = ["spray_version", "spray_create", "spray_destroy", "spray_last_error", "spray_check", "spray_launch_count", "spray_set_path", "spray_path_stats",
            "spray_build_cells", "spray_density", "spray_hydro_rhs", "spray_fld_apply", "spray_get_cell_table",
-           "spray_neighbor_counts", "spray_neighbor_lists", "spray_neighbor_digest", "spray_rad_jacobi", "spray_conduction", "spray_kgc_continuity", "spray_fp64_peak_probe"]
+           "spray_neighbor_counts", "spray_neighbor_lists", "spray_neighbor_digest", "spray_rad_jacobi", "spray_conduction", "spray_kgc_continuity", "spray_ray_deposit", "spray_fp64_peak_probe"]
 
 
 class SprayError(RuntimeError):
@@ -67,6 +67,7 @@ def load():
     lib.spray_conduction.argtypes = [vp, vp, vp, vp, vp, vp, vp]
     lib.spray_kgc_continuity.argtypes = [vp] * 10
     lib.spray_rad_jacobi.argtypes = [vp] + [vp] * 8 + [dbl, dbl, dbl, i32, i32, vp, vp, vp, vp]
+    lib.spray_ray_deposit.argtypes = [vp, vp, vp, vp, vp, i64, vp, dbl, i64, dbl, dbl, vp, vp, vp, vp, vp]
     lib.spray_get_cell_table.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.spray_neighbor_counts.argtypes = [vp, i32, vp, vp]
     lib.spray_neighbor_lists.argtypes = [vp, i32, vp, vp, vp]
@@ -237,6 +238,24 @@ class Spray:
                                        _ptr(E, f64, self.n), _ptr(u, f64, self.n), _ptr(resid), _stream())
         self._ck(rc, "spray_rad_jacobi")
         return dict(E=E, u=u, resid=resid)
+
+    def ray_deposit(self, m, rho, f, kib, rays, dt, nsteps, c_light=1.0, pmin=0.0, want_gradn=True):
+        """Row N4: mesh-free laser ray tracing and deposition (include/spray.h).  rays: fp64 CUDA tensor (7, nrays) with
+        rows x, y, z, vx, vy, vz, P.  Returns dict(gradn (3, n) or None, edep (n), rays (7, nrays), steps (nrays, int64))."""
+        t = self.torch
+        f64 = t.float64
+        if rays.dim() != 2 or rays.shape[0] != 7:
+            raise SprayError("rays must have shape (7, nrays)")
+        nr = int(rays.shape[1])
+        gradn = t.empty((3, self.n), dtype=f64, device=self.device) if want_gradn else None
+        edep = self._out(None)
+        rout = t.empty((7, nr), dtype=f64, device=self.device)
+        steps = t.empty(nr, dtype=t.int64, device=self.device)
+        a = [_ptr(x, f64, self.n) for x in (m, rho, f, kib)]
+        rc = self.lib.spray_ray_deposit(self.h, *a, nr, _ptr(rays, f64, 7 * nr), float(dt), int(nsteps), float(c_light), float(pmin),
+                                        _ptr(gradn), _ptr(edep, f64, self.n), _ptr(rout), _ptr(steps), _stream())
+        self._ck(rc, "spray_ray_deposit")
+        return dict(gradn=gradn, edep=edep, rays=rout, steps=steps)
 
     # -- parity exports
     def get_cell_table(self):

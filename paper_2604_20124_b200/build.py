@@ -14,7 +14,7 @@ PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 OBJ = PKG / "build"
 LIB = PKG / "libspray_b200.so"
-SOURCES = ["api.cu", "build.cu", "sweeps_ref.cu", "tiles.cu", "sweeps_tiled.cu", "rad.cu", "probe.cu"]
+SOURCES = ["api.cu", "build.cu", "sweeps_ref.cu", "tiles.cu", "sweeps_tiled.cu", "rad.cu", "ray.cu", "probe.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr", "-cudart", "static"]
 

@@ -403,6 +403,42 @@ int spray_rad_jacobi(spray_ctx* ctx, const double* m, const double* rho, const d
     return SPRAY_OK;
 }
 
+int spray_ray_deposit(spray_ctx* ctx, const double* m, const double* rho, const double* f, const double* kib, int64_t nrays,
+                      const double* rays_in, double dt, int64_t nsteps, double c_light, double pmin, double* gradn, double* edep,
+                      double* rays_out, int64_t* steps_out, void* stream) {
+    NEED_BUILT();
+    Ctx* c = &ctx->c;
+    if (c->n > 0 && (!m || !rho || !f || !kib || !edep)) return fail(c, SPRAY_ERR_INVALID_ARG, "spray_ray_deposit: NULL argument");
+    if (nrays < 0 || nsteps < 0 || (nrays > 0 && (!rays_in || !rays_out)) || !(dt > 0.0) || !(c_light > 0.0))
+        return fail(c, SPRAY_ERR_INVALID_ARG, "spray_ray_deposit: nrays, nsteps >= 0, dt, c_light > 0, ray buffers non-NULL");
+    cudaStream_t st = (cudaStream_t)stream;
+    double** fs = c->s.f;
+    // (1) G_a = sum_b V_b f_b gradW(x_ab, h_a): the limiter-type sweep without the -f_a term; sorted records
+    //     (z, V), f, (kib, f) from the FLD prologue with "mu" = kib, "E" = f
+    PrepJob pj{};
+    pj.m = m; pj.rho = rho; pj.E = f; pj.kx = kib; pj.kx_is_mu = 1;
+    pj.sm = fs[F_M]; pj.srho = fs[F_RHO]; pj.sE = fs[F_E]; pj.skx = fs[F_MU]; pj.sV = fs[F_V];
+    CK(launch_prep_fld(c, pj, st), "ray: prologue");
+    if (c->tl.enabled) {
+        TiledArgs t{};
+        t.o1 = gradn;
+        CK(launch_tiled_sweep(c, SW_GRADN, t, st), "ray: tiled gradient sweep");
+    }
+    SweepArgs a = fallback_args(c);
+    a.m = fs[F_M]; a.rho = fs[F_RHO]; a.E = fs[F_E]; a.mu = fs[F_MU];
+    a.o1 = gradn; a.me_sorted = c->pk.s[1]; a.g2_sorted = c->pk.s[2];
+    CK(launch_ref_sweep(c, SW_GRADN, a, st), "ray: gradient sweep");
+    // (2) rays: deposit into a sorted-order accumulator, then back to caller order
+    double* dep = fs[15];
+    if (c->n > 0) CK(cudaMemsetAsync(dep, 0, sizeof(double) * (size_t)c->n, st), "ray: deposit accumulator");
+    RayArgs r{};
+    r.nrays = nrays; r.rays_in = rays_in; r.dt = dt; r.c_light = c_light; r.pmin = pmin; r.nsteps = nsteps;
+    r.dep_sorted = dep; r.rays_out = rays_out; r.steps_out = steps_out;
+    CK(launch_ray_trace(c, r, st), "ray: trace");
+    CK(launch_unsort(c, dep, edep, st), "ray: deposit to caller order");
+    return SPRAY_OK;
+}
+
 int spray_get_cell_table(spray_ctx* ctx, uint32_t* sorted_key, uint32_t* perm, uint32_t* cell_start, uint32_t* cell_end,
                          void* stream) {
     NEED_BUILT();

@@ -93,7 +93,8 @@ struct SweepArgs {
     // caller-order outputs (written through perm)
     double *o0, *o1, *o2, *o3, *o4, *o5;
     double* mu_sorted;          // limiter: also keeps mu in sorted order for the apply that follows
-    double2* me_sorted;         // limiter: (mu, E) record of the tiled apply
+    double2* me_sorted;         // limiter: (mu, E) record of the tiled apply;  SW_GRADN: (G_x, G_y)
+    double2* g2_sorted;         // SW_GRADN: (G_z, kappa^ib)
     uint32_t* ocount;
     const uint64_t* offsets;
     uint32_t* onbr;
@@ -142,6 +143,19 @@ struct RadArgs {
 };
 cudaError_t launch_rad_update(Ctx* c, const RadArgs& a, cudaStream_t st);
 cudaError_t launch_div_by_rho(Ctx* c, double* y, const double* rho, cudaStream_t st);   // N2
+
+// ---- ray.cu : row N4, mesh-free laser ray tracing and deposition
+struct RayArgs {
+    int64_t nrays;
+    const double* rays_in;      // [7 nrays] planes x y z vx vy vz P
+    double dt, c_light, pmin;
+    int64_t nsteps;
+    double* dep_sorted;         // [n] sorted order, zeroed: deposited energy (fp64 atomics)
+    double* rays_out;           // [7 nrays]
+    int64_t* steps_out;         // nullable
+};
+cudaError_t launch_ray_trace(Ctx* c, const RayArgs& a, cudaStream_t st);
+cudaError_t launch_unsort(Ctx* c, const double* sorted, double* caller, cudaStream_t st);   // caller[perm[i]] = sorted[i]
 
 // ---- probe.cu
 cudaError_t launch_fp64_probe(int blocks, int threads, int64_t iters, double* out, cudaStream_t st);

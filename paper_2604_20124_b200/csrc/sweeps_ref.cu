@@ -63,6 +63,7 @@ __device__ __forceinline__ void ref_particle(const DevGrid& g, int64_t n, const 
         rho_a = A.rho[i]; p_a = A.p[i]; vxa = A.vx[i]; vya = A.vy[i]; vza = A.vz[i]; ac_a = A.alpha[i] * A.cs[i];
     }
     if (SWEEP == SW_LIMITER) { E_a = A.E[i]; }
+    if (SWEEP == SW_GRADN) { E_a = 0.0; }      // row N4: sum_b V_b f_b gradW(x_ab, h_a), no -f_a term
     if (SWEEP == SW_KGC) { rho_a = A.rho[i]; vxa = A.vx[i]; vya = A.vy[i]; vza = A.vz[i]; }
     if (SWEEP == SW_APPLY) { E_a = A.E[i]; mu_a = A.mu[i]; }
     uint64_t lbase = 0;
@@ -125,7 +126,7 @@ __device__ __forceinline__ void ref_particle(const DevGrid& g, int64_t n, const 
                             acc0 += cr * dx; acc1 += cr * dy; acc2 += cr * dz;
                             acc3 += (mb / rho_b) * w * Fa;      // eq. (37)
                         }
-                    } else if (SWEEP == SW_LIMITER) {
+                    } else if (SWEEP == SW_LIMITER || SWEEP == SW_GRADN) {
                         if (in_g && !self && r2 > 0.0) {
                             // eq. (9) phi = 1 with f = E (A19)
                             const double r = sqrt(r2);
@@ -194,6 +195,10 @@ __device__ __forceinline__ void ref_particle(const DevGrid& g, int64_t n, const 
         A.mu_sorted[i] = mu;
         if (A.me_sorted) A.me_sorted[i] = make_double2(mu, E_a);
         if (A.o1) { A.o1[ia] = acc0; A.o1[n + ia] = acc1; A.o1[2 * n + ia] = acc2; }
+    } else if (SWEEP == SW_GRADN) {
+        A.me_sorted[i] = make_double2(acc0, acc1);
+        A.g2_sorted[i] = make_double2(acc2, A.mu[i]);   // (G_z, kappa^ib)
+        if (A.o1) { A.o1[ia] = acc0; A.o1[n + ia] = acc1; A.o1[2 * n + ia] = acc2; }
     } else if (SWEEP == SW_APPLY) {
         A.o0[ia] = acc0;
         if (A.o1) A.o1[ia] = acc1;
@@ -253,6 +258,7 @@ cudaError_t launch_ref_sweep(Ctx* c, int sweep, const SweepArgs& a, cudaStream_t
         case SW_LIST: return launch_k<SW_LIST>(c, a, st);
         case SW_DIGEST: return launch_k<SW_DIGEST>(c, a, st);
         case SW_KGC: return launch_k<SW_KGC>(c, a, st);
+        case SW_GRADN: return launch_k<SW_GRADN>(c, a, st);
     }
     return cudaErrorInvalidValue;
 }

@@ -94,6 +94,7 @@ template <> struct NRec<SW_HYDRO> { static constexpr int v = 6, e = 0; };     //
 template <> struct NRec<SW_LIMITER> { static constexpr int v = 2, e = 1; };   // (x,y) (z,V) | E
 template <> struct NRec<SW_APPLY> { static constexpr int v = 4, e = 0; };     // (x,y) (z,V) (mu,E) (1/h,Fn)
 template <> struct NRec<SW_KGC> { static constexpr int v = 4, e = 0; };       // (x,y) (z,V) (vx,vy) (vz,-)
+template <> struct NRec<SW_GRADN> { static constexpr int v = 2, e = 1; };     // (x,y) (z,V) | f = n_e/n_c   (row N4)
 
 struct SweepIn {
     const double2* rec[6];           // sorted global records, in the order of NRec
@@ -103,6 +104,7 @@ struct SweepIn {
     const double2* t0;               // per-call target record
     const double2* me;               // (mu, E)
     double2* me_out;                 // limiter: (mu, E) for the apply
+    double2* g_out[2];               // SW_GRADN: (G_x, G_y), (G_z, kappa^ib) in sorted order for the ray kernel (ray.cu)
     double* mu_sorted;               // limiter: mu in sorted order for the general kernels
     const uint32_t* perm;
     const TileDesc* tiles;
@@ -176,8 +178,9 @@ __device__ __forceinline__ void pair_body(const double2* __restrict__ F, const d
             acc.a0 = fma(c, dx, acc.a0); acc.a1 = fma(c, dy, acc.a1); acc.a2 = fma(c, dz, acc.a2);
             acc.a3 = fma(Vb * Ga, vr, acc.a3);
         }
-    } else if (SWEEP == SW_LIMITER) {
-        // eq. (9) phi = 1 with f = E (A19): h_a only
+    } else if (SWEEP == SW_LIMITER || SWEEP == SW_GRADN) {
+        // eq. (9) phi = 1 with f = E (A19): h_a only.  SW_GRADN (row N4) is the same sum without
+        // the -E_a term (T.c0 = 0): G_a = sum_b V_b f_b gradW(x_ab, h_a), literally as printed.
         const double G = gshape<KERNEL, !UNI>(qa) * y;
         const double cc = (d1.y * (Ee[s] - T.c0)) * G;
         acc.a0 = fma(cc, dx, acc.a0); acc.a1 = fma(cc, dy, acc.a1); acc.a2 = fma(cc, dz, acc.a2);
@@ -287,7 +290,7 @@ __device__ __forceinline__ void pair_loop(const double2* __restrict__ F, const d
     // iteration are read from shared memory during the iteration before (slot 0 when there is none: read and not used), so
     // that the shared-memory round trip, long when the data pipe is busy, is not exposed at the top of every iteration.
     // Measured: -5 % for these two sweeps, +1-2 % for the heavier ones, which therefore do not do it.
-    constexpr bool PIPE_FIRST = SWEEP == SW_DENSITY || SWEEP == SW_LIMITER;
+    constexpr bool PIPE_FIRST = SWEEP == SW_DENSITY || SWEEP == SW_LIMITER || SWEEP == SW_GRADN;
     double2 q0 = F[cur.x & 0xFFFFu], q1 = F[TILE_CMAXP + (cur.x & 0xFFFFu)];
     for (uint32_t r4 = 0; r4 < R; r4 += 4) {
         const uint2 nx3 = (r4 + 12 < R) ? __ldcs(lp + (size_t)(r4 / 4 + 3) * 32) : make_uint2(0u, 0u);
@@ -314,7 +317,7 @@ __device__ __forceinline__ void pair_loop(const double2* __restrict__ F, const d
 // apply then needs 3 records per candidate, 105 KB, and two CTAs fit an SM.  MODE 2: only the other tiles.
 template <int SWEEP, int MODE> struct NRecM { static constexpr int v = (SWEEP == SW_APPLY && MODE == 1) ? 3 : NRec<SWEEP>::v; };
 template <int SWEEP, int MODE> struct MinBlocks {
-    static constexpr int v = (SWEEP == SW_DENSITY || SWEEP == SW_LIMITER || (SWEEP == SW_APPLY && MODE == 1)) ? 2 : 1;
+    static constexpr int v = (SWEEP == SW_DENSITY || SWEEP == SW_LIMITER || SWEEP == SW_GRADN || (SWEEP == SW_APPLY && MODE == 1)) ? 2 : 1;
 };
 
 template <int SWEEP, int KERNEL, int MODE>
@@ -382,6 +385,7 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
                 T.c3 = q1.y; T.c4 = q2.x; T.c5 = q2.y;                                       // v_a
             }
             if (SWEEP == SW_LIMITER) T.c0 = A.e1[i];                                         // E_a
+            if (SWEEP == SW_GRADN) T.c0 = 0.0;
             if (SWEEP == SW_APPLY) { const double2 me = A.rec[2][i]; T.c0 = me.y; T.c1 = me.x; T.c2 = 4.0 * me.x; }
             if (SWEEP == SW_KGC) {
                 const double2 q1 = A.rec[2][i], q2 = A.rec[3][i];
@@ -431,7 +435,7 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
         // ---- add the two half-lists of the target
         acc.a0 += __shfl_xor_sync(0xFFFFFFFFu, acc.a0, 1);
         if (SWEEP != SW_DENSITY) acc.a1 += __shfl_xor_sync(0xFFFFFFFFu, acc.a1, 1);
-        if (SWEEP == SW_HYDRO || SWEEP == SW_LIMITER) acc.a2 += __shfl_xor_sync(0xFFFFFFFFu, acc.a2, 1);
+        if (SWEEP == SW_HYDRO || SWEEP == SW_LIMITER || SWEEP == SW_GRADN) acc.a2 += __shfl_xor_sync(0xFFFFFFFFu, acc.a2, 1);
         if (SWEEP == SW_HYDRO) {
             acc.a3 += __shfl_xor_sync(0xFFFFFFFFu, acc.a3, 1);
             acc.a4 += __shfl_xor_sync(0xFFFFFFFFu, acc.a4, 1);
@@ -463,6 +467,12 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
                 A.o0[ia] = mu;
                 A.me_out[i] = make_double2(mu, T.c0);
                 A.mu_sorted[i] = mu;
+                if (A.o1) { A.o1[ia] = gx; A.o1[A.n + ia] = gy; A.o1[2 * A.n + ia] = gz; }
+            } else if (SWEEP == SW_GRADN) {
+                // row N4: gradient of n_e/n_c at the particle, caller order (nullable) + the sorted records the ray kernel gathers
+                const double gx = T.fn * acc.a0, gy = T.fn * acc.a1, gz = T.fn * acc.a2;
+                A.g_out[0][i] = make_double2(gx, gy);
+                A.g_out[1][i] = make_double2(gz, A.me[i].x);     // (G_z, kappa^ib)
                 if (A.o1) { A.o1[ia] = gx; A.o1[A.n + ia] = gy; A.o1[2 * A.n + ia] = gz; }
             } else if (SWEEP == SW_KGC) {
                 // M_a = -(kFn/h_a^4) sum c x (x) x (symmetric), L_a = M_a^-1 by cofactors; singular -> L_a = I (A28)
@@ -540,6 +550,9 @@ cudaError_t launch_tiled_sweep(Ctx* c, int sweep, const TiledArgs& t, cudaStream
             a.rec[2] = pk.s[1]; a.rec[3] = pk.s[2]; a.rec[4] = pk.s[3]; a.rec[5] = pk.hh;
             return launch_t<SW_HYDRO>(c, a, st);
         case SW_LIMITER: return launch_t<SW_LIMITER>(c, a, st);
+        case SW_GRADN:
+            a.g_out[0] = pk.s[1]; a.g_out[1] = pk.s[2];
+            return launch_t<SW_GRADN>(c, a, st);
         case SW_APPLY:
             a.rec[2] = pk.me; a.rec[3] = pk.hh;
             return launch_t<SW_APPLY>(c, a, st);
