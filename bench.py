@@ -366,6 +366,38 @@ def main():
         n3 = {"call": "spray_kgc_continuity", "ms_per_call": 1e3 * t_k, "pair_interactions_per_s": pairs["limiter"] / t_k,
               "flops_per_pair": 60, "flop_roofline_frac": pairs["limiter"] * 60 / t_k / (fp64_meas * 1e12)}
 
+    # ---- row N4: mesh-free laser ray tracing and deposition (spray_ray_deposit) on the same particle set and cell table: a beam
+    #      of 65 536 rays entering at the low-z face with a small divergence, 128 steps of one lattice spacing; f = n_e/n_c
+    #      proportional to rho (0.8 in the densest fluid), kib proportional to f^2.  Counted: ray steps, and in-support
+    #      ray-particle interactions (neighbour count of a particle = particles within 2h = interactions per ray step, uniform h).
+    n4 = None
+    if not args.no_n1:
+        nr, nst = 65536, 128
+        gen = torch.Generator(device=dev); gen.manual_seed(1234)
+        lo = [float(v) for v in w.grid.lo]
+        Lb = [float(b) - float(a) for a, b in zip(w.grid.lo, w.grid.hi)]
+        u = torch.rand((5, nr), generator=gen, device=dev, dtype=f64)
+        rays = torch.stack([lo[0] + Lb[0] * u[0], lo[1] + Lb[1] * u[1], torch.full((nr,), lo[2] + 0.05 * Lb[2], dtype=f64, device=dev),
+                            0.1 * (u[2] - 0.5), 0.1 * (u[3] - 0.5), torch.ones(nr, dtype=f64, device=dev), 1.0 + u[4]]).contiguous()
+        fq = 0.8 * out["rho"] / out["rho"].max()
+        kib = 20.0 * (0.05 + fq * fq)
+        dt_ray = Lb[2] / round(n ** (1.0 / 3.0))
+        sp.ray_deposit(d["m"], out["rho"], fq, kib, rays, dt_ray, 4, c_light=1.0, want_gradn=False)
+        torch.cuda.synchronize()
+        r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        r0.record()
+        rr = sp.ray_deposit(d["m"], out["rho"], fq, kib, rays, dt_ray, nst, c_light=1.0, want_gradn=False)
+        r1.record()
+        torch.cuda.synchronize()
+        t_r = r0.elapsed_time(r1) * 1e-3
+        steps_taken = int(rr["steps"].sum().item())
+        nb_mean = pairs["limiter"] / n + 1.0
+        n4 = {"call": "spray_ray_deposit", "rays": nr, "max_steps": nst, "ray_steps": steps_taken, "ms_per_call": 1e3 * t_r,
+              "ray_steps_per_s": steps_taken / t_r, "ray_particle_interactions_per_s": steps_taken * nb_mean / t_r,
+              "energy_balance_rel": float(abs(rr["edep"].sum() + rr["rays"][6].sum() - rays[6].sum()) / rays[6].sum()),
+              "absorbed_fraction": float(rr["edep"].sum() / rays[6].sum()),
+              "note": "includes the gradient sweep over all particles (prologue + SW_GRADN) and the deposit scatter"}
+
     # ---- roofline: pass level and dominant kernel
     fl = FLOPS[w.kernel]
     visc_frac = 0.0 if not (np.any(w.vx) or np.any(w.vy) or np.any(w.vz)) else 0.5
@@ -409,7 +441,7 @@ def main():
                        "parallelism": "replicas only" if world > 1 else "1 GPU", "path": args.path,
                        "tiles": n_tiles, "tiled_fraction": n_fast / max(n, 1)},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
-            "fp64_probe_tflops": fp64_meas, "next_rows": {"N1_rad_jacobi": n1, "N3_kgc_continuity": n3}}
+            "fp64_probe_tflops": fp64_meas, "next_rows": {"N1_rad_jacobi": n1, "N3_kgc_continuity": n3, "N4_ray_deposit": n4}}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -6,7 +6,8 @@
 //         spray_build_cells, reach 2 max(h) (device scalar hglob[1]), rows (cy, cz) culled by their distance to the ray
 //         and the x-range of a row narrowed to the chord of the reach sphere; after the sort the cells of a row are
 //         one contiguous range of sorted slots (two when the range wraps in a periodic box);
-//   (ii)  strides its 32 lanes over those slots: 16-byte records (x,y) (z,h) for the test r^2 < 4 h_a^2 in the contract
+//   (ii)  numbers the candidates of up to 32 rows consecutively (one lane per row reads the cell table, warp scan) and
+//         strides its 32 lanes over that numbering: 16-byte records (x,y) (z,h) for the test r^2 < 4 h_a^2 in the contract
 //         form (common.cuh), and for the accepted ones (z,V) (G_x,G_y) (G_z,kappa^ib) -- the last two written by the
 //         SW_GRADN sweep -- to accumulate  G(x) = sum V_a G_a W,  kappa(x) = sum V_a kib_a W,  wsum = sum V_a W
 //         (standard SPH interpolation with the particles' own h; reading A30);
@@ -68,69 +69,108 @@ __device__ __forceinline__ int wrap_mod(int c, int nc) { c %= nc; return c < 0 ?
 
 struct RaySums { double gx, gy, gz, kap, wsum; };
 
+// Per-warp table of the rows of one chunk (32 rows, one per lane): up to two contiguous pieces of sorted slots per row and
+// the row's offset in the chunk's flattened candidate numbering.
+struct RowTab {
+    uint32_t jb0[32], len0[32], jb1[32], off[33];
+};
+
 // One traversal of the particles around the ray at (px, py, pz).  PASS 0: accumulate the sums, cache (slot, weight);
 // returns the number of accepted particles with nonzero weight.  PASS 1: deposit sc * w_a by recomputation.
+// The rows (cy, cz) in reach are taken 32 at a time: lane l works out the slot ranges of row l (cell-table reads of all
+// rows in flight together), a warp scan numbers the candidates of the chunk consecutively, and the lanes then stride over
+// that numbering, so all 32 lanes stay busy whatever the row lengths, with the next candidate's records loaded before the
+// current one is evaluated.
 template <int KERNEL, int PASS>
 __device__ __forceinline__ uint32_t ray_visit(const DevGrid& g, const RayIn& A, double px, double py, double pz, double reach, int lane,
-                                              RaySums& S, uint32_t* __restrict__ c_idx, double* __restrict__ c_w, double sc,
+                                              RaySums& S, RowTab& RT, uint32_t* __restrict__ c_idx, double* __restrict__ c_w, double sc,
                                               double* __restrict__ dep) {
     uint32_t cnt = 0;
     const double reach2 = reach * reach;
     const RSpan sy = ray_span(g, 1, py, reach), sz = ray_span(g, 2, pz, reach);
-    for (int kz = 0; kz < sz.cnt; ++kz) {
-        const int czu = sz.start + kz;
-        const double dz0 = slab_dist(g, 2, czu, pz, sz.all);
-        const int czz = g.per[2] ? wrap_mod(czu, g.nc[2]) : czu;
-        for (int ky = 0; ky < sy.cnt; ++ky) {
-            const int cyu = sy.start + ky;
-            const double dy0 = slab_dist(g, 1, cyu, py, sy.all);
+    const int nrows = sy.cnt * sz.cnt;
+    for (int r0 = 0; r0 < nrows; r0 += 32) {
+        // ---- this lane's row
+        uint32_t jb0 = 0, len0 = 0, jb1 = 0, len1 = 0;
+        const int rr = r0 + lane;
+        if (rr < nrows) {
+            const int kz = rr / sy.cnt, ky = rr - kz * sy.cnt;
+            const int czu = sz.start + kz, cyu = sy.start + ky;
+            const double dz0 = slab_dist(g, 2, czu, pz, sz.all), dy0 = slab_dist(g, 1, cyu, py, sy.all);
             const double rem = reach2 - (dy0 * dy0 + dz0 * dz0);
-            if (!(rem > 0.0)) continue;                       // the row is out of reach
-            const int cyy = g.per[1] ? wrap_mod(cyu, g.nc[1]) : cyu;
-            const RSpan sx = ray_span(g, 0, px, sqrt(rem));
-            const uint32_t row = (uint32_t)((czz * g.nc[1] + cyy) * g.nc[0]);
-            // one or two contiguous pieces of cells
-            int c0 = g.per[0] ? wrap_mod(sx.start, g.nc[0]) : sx.start;
-            int left = sx.cnt;
-            while (left > 0) {
-                const int take = min(left, g.nc[0] - c0);
-                const uint32_t jb = __ldg(A.cell_start + row + c0), je = __ldg(A.cell_end + row + c0 + take - 1);
-                for (uint32_t base = jb; base < je; base += 32) {
-                    const uint32_t j = base + lane;
-                    bool hit = false;
-                    double wa = 0.0;
-                    if (j < je) {
-                        const double2 a0 = __ldg(A.p0 + j), a1 = __ldg(A.p1 + j);
-                        const double dx = min_image(__dsub_rn(px, a0.x), g.per[0], g.L[0], g.halfL[0]);
-                        const double dy = min_image(__dsub_rn(py, a0.y), g.per[1], g.L[1], g.halfL[1]);
-                        const double dz = min_image(__dsub_rn(pz, a1.x), g.per[2], g.L[2], g.halfL[2]);
-                        const double r2 = r2_exact(dx, dy, dz);
-                        const double ha = a1.y;
-                        if (r2 < support2(ha)) {
-                            const double hinv = 1.0 / ha;
-                            wa = __ldg(A.s0 + j).y * ((sigma<KERNEL>() * hinv * hinv * hinv) * shape_w<KERNEL>(sqrt(r2) * hinv));
-                            hit = wa != 0.0;
-                        }
-                    }
-                    if (PASS == 0) {
-                        if (hit) {
-                            const double2 ga = __ldg(A.gA + j), gb = __ldg(A.gB + j);
-                            S.gx = fma(wa, ga.x, S.gx); S.gy = fma(wa, ga.y, S.gy); S.gz = fma(wa, gb.x, S.gz);
-                            S.kap = fma(wa, gb.y, S.kap);
-                            S.wsum += wa;
-                        }
-                        const uint32_t mask = __ballot_sync(0xFFFFFFFFu, hit);
-                        if (hit) {
-                            const uint32_t pos = cnt + __popc(mask & ((1u << lane) - 1u));
-                            if (pos < (uint32_t)RAY_CAP) { c_idx[pos] = j; c_w[pos] = wa; }
-                        }
-                        cnt += __popc(mask);
-                    } else {
-                        if (hit) atomicAdd(dep + j, sc * wa);
-                    }
+            if (rem > 0.0) {                                   // else the row is out of reach
+                const int czz = g.per[2] ? wrap_mod(czu, g.nc[2]) : czu;
+                const int cyy = g.per[1] ? wrap_mod(cyu, g.nc[1]) : cyu;
+                const RSpan sx = ray_span(g, 0, px, sqrt(rem));
+                const uint32_t row = (uint32_t)((czz * g.nc[1] + cyy) * g.nc[0]);
+                const int c0 = g.per[0] ? wrap_mod(sx.start, g.nc[0]) : sx.start;
+                const int take = min(sx.cnt, g.nc[0] - c0);
+                jb0 = __ldg(A.cell_start + row + c0);
+                len0 = __ldg(A.cell_end + row + c0 + take - 1) - jb0;
+                if (take < sx.cnt) {                           // the range wraps: second piece from column 0
+                    jb1 = __ldg(A.cell_start + row);
+                    len1 = __ldg(A.cell_end + row + (sx.cnt - take) - 1) - jb1;
                 }
-                left -= take;
-                c0 = 0;
+            }
+        }
+        // ---- number the candidates of the chunk
+        const uint32_t len = len0 + len1;
+        uint32_t inc = len;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t v = __shfl_up_sync(0xFFFFFFFFu, inc, o);
+            if (lane >= o) inc += v;
+        }
+        const uint32_t total = __shfl_sync(0xFFFFFFFFu, inc, 31);
+        __syncwarp();
+        RT.jb0[lane] = jb0; RT.len0[lane] = len0; RT.jb1[lane] = jb1; RT.off[lane] = inc - len;
+        if (lane == 31) RT.off[32] = total;
+        __syncwarp();
+        // ---- stride over them
+        int row = 0;
+        auto slot_of = [&](uint32_t t) -> uint32_t {
+            while (RT.off[row + 1] <= t) ++row;                // t < total = off[32]: terminates; rows of length 0 are skipped
+            const uint32_t k = t - RT.off[row], l0 = RT.len0[row];
+            return k < l0 ? RT.jb0[row] + k : RT.jb1[row] + (k - l0);
+        };
+        uint32_t j = 0;
+        double2 a0 = make_double2(0.0, 0.0), a1 = a0;
+        if ((uint32_t)lane < total) { j = slot_of(lane); a0 = __ldg(A.p0 + j); a1 = __ldg(A.p1 + j); }
+        for (uint32_t base = 0; base < total; base += 32) {
+            const uint32_t t = base + lane;
+            const bool valid = t < total;
+            const uint32_t jc = j;
+            const double2 b0 = a0, b1 = a1;
+            if (t + 32 < total) { j = slot_of(t + 32); a0 = __ldg(A.p0 + j); a1 = __ldg(A.p1 + j); }
+            bool hit = false;
+            double wa = 0.0;
+            if (valid) {
+                const double dx = min_image(__dsub_rn(px, b0.x), g.per[0], g.L[0], g.halfL[0]);
+                const double dy = min_image(__dsub_rn(py, b0.y), g.per[1], g.L[1], g.halfL[1]);
+                const double dz = min_image(__dsub_rn(pz, b1.x), g.per[2], g.L[2], g.halfL[2]);
+                const double r2 = r2_exact(dx, dy, dz);
+                const double ha = b1.y;
+                if (r2 < support2(ha)) {
+                    const double hinv = 1.0 / ha;
+                    wa = __ldg(A.s0 + jc).y * ((sigma<KERNEL>() * hinv * hinv * hinv) * shape_w<KERNEL>(sqrt(r2) * hinv));
+                    hit = wa != 0.0;
+                }
+            }
+            if (PASS == 0) {
+                if (hit) {
+                    const double2 ga = __ldg(A.gA + jc), gb = __ldg(A.gB + jc);
+                    S.gx = fma(wa, ga.x, S.gx); S.gy = fma(wa, ga.y, S.gy); S.gz = fma(wa, gb.x, S.gz);
+                    S.kap = fma(wa, gb.y, S.kap);
+                    S.wsum += wa;
+                }
+                const uint32_t mask = __ballot_sync(0xFFFFFFFFu, hit);
+                if (hit) {
+                    const uint32_t pos = cnt + __popc(mask & ((1u << lane) - 1u));
+                    if (pos < (uint32_t)RAY_CAP) { c_idx[pos] = jc; c_w[pos] = wa; }
+                }
+                cnt += __popc(mask);
+            } else {
+                if (hit) atomicAdd(dep + jc, sc * wa);
             }
         }
     }
@@ -148,6 +188,7 @@ __global__ void __launch_bounds__(32 * RAY_WARPS)
 k_ray_trace(DevGrid g, RayIn A, RayArgs R) {
     __shared__ uint32_t s_idx[RAY_WARPS][RAY_CAP];
     __shared__ double s_w[RAY_WARPS][RAY_CAP];
+    __shared__ RowTab s_rt[RAY_WARPS];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int64_t q = (int64_t)blockIdx.x * RAY_WARPS + warp;
     if (q >= R.nrays) return;                                   // warp-uniform; no CTA-wide barrier below
@@ -162,7 +203,7 @@ k_ray_trace(DevGrid g, RayIn A, RayArgs R) {
     int64_t k = 0;
     for (; k < R.nsteps && P > R.pmin; ++k) {
         RaySums S{0.0, 0.0, 0.0, 0.0, 0.0};
-        const uint32_t cnt = ray_visit<KERNEL, 0>(g, A, p[0], p[1], p[2], reach, lane, S, c_idx, c_w, 0.0, nullptr);
+        const uint32_t cnt = ray_visit<KERNEL, 0>(g, A, p[0], p[1], p[2], reach, lane, S, s_rt[warp], c_idx, c_w, 0.0, nullptr);
         S.gx = warp_sum(S.gx); S.gy = warp_sum(S.gy); S.gz = warp_sum(S.gz); S.kap = warp_sum(S.kap); S.wsum = warp_sum(S.wsum);
         // eq. (72), then the track length of this step with the new v (A31)
         v[0] = fma(acc, S.gx, v[0]); v[1] = fma(acc, S.gy, v[1]); v[2] = fma(acc, S.gz, v[2]);
@@ -177,7 +218,7 @@ k_ray_trace(DevGrid g, RayIn A, RayArgs R) {
                 __syncwarp();
             } else {
                 RaySums dummy{};
-                ray_visit<KERNEL, 1>(g, A, p[0], p[1], p[2], reach, lane, dummy, nullptr, nullptr, sc, R.dep_sorted);
+                ray_visit<KERNEL, 1>(g, A, p[0], p[1], p[2], reach, lane, dummy, s_rt[warp], nullptr, nullptr, sc, R.dep_sorted);
             }
         }
         bool out = false;

@@ -144,3 +144,40 @@ def test_ray_edge_cases_empty_sets():
     gg = run_gpu(w, f, kib, np.zeros((7, 0)), 0.01, 10, 1.0)
     oo = O.ray_deposit(w.grid, w.kernel, w.x, w.y, w.z, w.h, w.m, w.rho_nom, f, kib, np.zeros((7, 0)), 0.01, 10)
     assert np.all(gg["edep"] == 0.0) and np.all(np.abs(gg["gradn"] - oo["gradn"]) <= TOL * oo["S_gradn"])
+
+
+def test_ray_full_size_c5_tube():
+    """BJ configs[4] (16.7M particles), the launch configuration bench.py times.  The oracle visits every particle at every
+    step, so it runs on a TUBE around the rays instead: a ray step at x reads the particles within 2 h_max of x and, through
+    G_a, their gather neighbours (2 h_max further).  Every particle a ray reads receives a deposit > 0 (kib > 0 everywhere), so
+    the touched set is {edep > 0}; if every touched particle lies at least 4 h_max inside the tube's faces, every ray position
+    was at least 2 h_max inside, every particle within reach of a ray was in the tube, and so were all its gather neighbours:
+    the tube then determines the result completely (checked on the oracle's own output), and taking its particles in ascending
+    caller order leaves even the oracle's summation order unchanged.  The GPU runs on the full set; outside the tube it must
+    deposit nothing."""
+    w = W.make("c5")
+    hmax = float(w.h.max())
+    x0, x1, half = 0.49, 0.51, 0.07
+    nrays, nsteps, c = 12, 60, 1.0
+    i = np.arange(nrays, dtype=np.int64)
+    rays = np.vstack([x0 + (x1 - x0) * W.u01(7, i, 0), x0 + (x1 - x0) * W.u01(7, i, 1), 0.36 + 0.02 * W.u01(7, i, 2),
+                      0.1 * (W.u01(7, i, 3) - 0.5), 0.1 * (W.u01(7, i, 4) - 0.5), np.ones(nrays), 1.0 + W.u01(7, i, 5)])
+    dt = 1.0 / 256.0                                                        # one lattice spacing per step: crosses the interface at z ~ 0.5
+    f = 0.8 * w.rho_nom / w.rho_nom.max()
+    kib = 20.0 * (0.05 + f * f)
+    tube = np.flatnonzero((np.abs(w.x - 0.5) < half) & (np.abs(w.y - 0.5) < half))
+    o = O.ray_deposit(w.grid, w.kernel, w.x[tube], w.y[tube], w.z[tube], w.h[tube], w.m[tube], w.rho_nom[tube], f[tube], kib[tube],
+                      rays, dt, nsteps, c)
+    touched = o["edep"] > 0
+    depth = half - np.maximum(np.abs(w.x[tube] - 0.5), np.abs(w.y[tube] - 0.5))      # distance to the nearest face of the tube
+    assert touched.sum() > 1000 and np.min(depth[touched]) > 4.0 * hmax + 1e-6
+    assert np.sum(o["edep"]) > 0.05 * np.sum(rays[6])
+    g = run_gpu(w, f, kib, rays, dt, nsteps, c)
+    outside = np.ones(w.n, bool); outside[tube] = False
+    assert np.all(g["edep"][outside] == 0.0)
+    # gradn is compared where the tube holds the particle's whole neighbourhood
+    inner = depth > 2.0 * hmax + 1e-6
+    gt = dict(g, edep=g["edep"][tube], gradn=g["gradn"][:, tube][:, inner])
+    ot = dict(o, gradn=o["gradn"][:, inner], S_gradn=o["S_gradn"][:, inner])
+    e = compare(w, gt, ot, rays, dt, nsteps, c)
+    print("c5 tube", tube.size, "of", w.n, "touched", int(touched.sum()), "worst edep error / tolerance", e)
