@@ -390,9 +390,17 @@ def main():
         r1.record()
         torch.cuda.synchronize()
         t_r = r0.elapsed_time(r1) * 1e-3
+        # the same call without rays: the gradient sweep over all particles (prologue + SW_GRADN) and the deposit scatter alone
+        g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        g0.record()
+        sp.ray_deposit(d["m"], out["rho"], fq, kib, rays[:, :0].contiguous(), dt_ray, nst, c_light=1.0, want_gradn=False)
+        g1.record()
+        torch.cuda.synchronize()
+        t_g = g0.elapsed_time(g1) * 1e-3
         steps_taken = int(rr["steps"].sum().item())
         nb_mean = pairs["limiter"] / n + 1.0
         n4 = {"call": "spray_ray_deposit", "rays": nr, "max_steps": nst, "ray_steps": steps_taken, "ms_per_call": 1e3 * t_r,
+              "ms_gradient_sweep_and_scatter": 1e3 * t_g, "ms_ray_kernel": 1e3 * (t_r - t_g),
               "ray_steps_per_s": steps_taken / t_r, "ray_particle_interactions_per_s": steps_taken * nb_mean / t_r,
               "energy_balance_rel": float(abs(rr["edep"].sum() + rr["rays"][6].sum() - rays[6].sum()) / rays[6].sum()),
               "absorbed_fraction": float(rr["edep"].sum() / rays[6].sum()),

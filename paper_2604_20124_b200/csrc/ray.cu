@@ -11,12 +11,13 @@
 //         form (common.cuh), and for the accepted ones (z,V) (G_x,G_y) (G_z,kappa^ib) -- the last two written by the
 //         SW_GRADN sweep -- to accumulate  G(x) = sum V_a G_a W,  kappa(x) = sum V_a kib_a W,  wsum = sum V_a W
 //         (standard SPH interpolation with the particles' own h; reading A30);
-//   (iii) keeps (slot, weight) of the accepted particles in a per-warp shared-memory cache, reduces the five sums with
+//   (iii) compacts the accepted candidates into a per-warp hit list (slot, r^2) in shared memory and evaluates that list
+//         densely (all lanes busy with accepted particles, their four records loaded together), reduces the five sums with
 //         a shuffle butterfly (every lane ends with the same bits), and every lane advances the ray redundantly:
 //         v <- v - (c^2/2) G dt (eq. (72)), ds = |v| dt, dE = P (1 - exp(-kappa ds)) (eq. (71)), P <- P - dE,
 //         x <- x + v dt (semi-implicit Euler, A31), periodic wrap / exit test (A34);
 //   (iv)  deposits dE w_a / wsum ("based on the kernel weight", A33) with fp64 atomics into a SORTED-order
-//         accumulator (neighbouring rays hit neighbouring slots), from the cache -- or by a second traversal in the
+//         accumulator (neighbouring rays hit neighbouring slots), from the hit list -- or by a second traversal in the
 //         rare step whose support holds more than RAY_CAP particles.
 // The atomics make the deposit's summation order, hence its last bits, vary from run to run.
 #include "spray_internal.h"
@@ -75,8 +76,36 @@ struct RowTab {
     uint32_t jb0[32], len0[32], jb1[32], off[33];
 };
 
-// One traversal of the particles around the ray at (px, py, pz).  PASS 0: accumulate the sums, cache (slot, weight);
-// returns the number of accepted particles with nonzero weight.  PASS 1: deposit sc * w_a by recomputation.
+// Dense evaluation of a hit list (slot, r^2): lanes stride over it, the four records of a hit are loaded together.
+// PASS 0: w_a = V_a W(r; h_a) replaces r^2 in the list and the interpolation sums are accumulated.
+// PASS 1: deposit sc * w_a (second traversal of a step whose hits did not fit one list).
+template <int KERNEL, int PASS>
+__device__ __forceinline__ void ray_eval(const RayIn& A, int lane, uint32_t cnt, const uint32_t* __restrict__ c_idx, double* __restrict__ c_w,
+                                         RaySums& S, double sc, double* __restrict__ dep) {
+    __syncwarp();
+    for (uint32_t t = lane; t < cnt; t += 32) {
+        const uint32_t j = c_idx[t];
+        const double r2 = c_w[t];
+        const double ha = __ldg(A.p1 + j).y, V = __ldg(A.s0 + j).y;
+        const double hinv = 1.0 / ha;
+        const double wa = V * ((sigma<KERNEL>() * hinv * hinv * hinv) * shape_w<KERNEL>(sqrt(r2) * hinv));
+        if (PASS == 0) {
+            const double2 ga = __ldg(A.gA + j), gb = __ldg(A.gB + j);
+            S.gx = fma(wa, ga.x, S.gx); S.gy = fma(wa, ga.y, S.gy); S.gz = fma(wa, gb.x, S.gz);
+            S.kap = fma(wa, gb.y, S.kap);
+            S.wsum += wa;
+            c_w[t] = wa;
+        } else {
+            if (wa != 0.0) atomicAdd(dep + j, sc * wa);
+        }
+    }
+    __syncwarp();
+}
+
+// One traversal of the particles around the ray at (px, py, pz): tests every candidate and compacts the accepted ones into
+// the hit list (slot, r^2); returns the number of hits left in the list for the caller to evaluate (ray_eval).  When the list
+// fills up it is evaluated on the spot and `overflow` is set: the list then no longer holds the whole step, and the
+// deposit needs a second traversal (PASS 1, which evaluates with the deposit scale sc instead of accumulating).
 // The rows (cy, cz) in reach are taken 32 at a time: lane l works out the slot ranges of row l (cell-table reads of all
 // rows in flight together), a warp scan numbers the candidates of the chunk consecutively, and the lanes then stride over
 // that numbering, so all 32 lanes stay busy whatever the row lengths, with the next candidate's records loaded before the
@@ -84,7 +113,7 @@ struct RowTab {
 template <int KERNEL, int PASS>
 __device__ __forceinline__ uint32_t ray_visit(const DevGrid& g, const RayIn& A, double px, double py, double pz, double reach, int lane,
                                               RaySums& S, RowTab& RT, uint32_t* __restrict__ c_idx, double* __restrict__ c_w, double sc,
-                                              double* __restrict__ dep) {
+                                              double* __restrict__ dep, bool& overflow) {
     uint32_t cnt = 0;
     const double reach2 = reach * reach;
     const RSpan sy = ray_span(g, 1, py, reach), sz = ray_span(g, 2, pz, reach);
@@ -126,7 +155,7 @@ __device__ __forceinline__ uint32_t ray_visit(const DevGrid& g, const RayIn& A, 
         RT.jb0[lane] = jb0; RT.len0[lane] = len0; RT.jb1[lane] = jb1; RT.off[lane] = inc - len;
         if (lane == 31) RT.off[32] = total;
         __syncwarp();
-        // ---- stride over them
+        // ---- stride over them: the test only (contract predicate); accepted candidates are compacted into the hit list
         int row = 0;
         auto slot_of = [&](uint32_t t) -> uint32_t {
             while (RT.off[row + 1] <= t) ++row;                // t < total = off[32]: terminates; rows of length 0 are skipped
@@ -138,40 +167,29 @@ __device__ __forceinline__ uint32_t ray_visit(const DevGrid& g, const RayIn& A, 
         if ((uint32_t)lane < total) { j = slot_of(lane); a0 = __ldg(A.p0 + j); a1 = __ldg(A.p1 + j); }
         for (uint32_t base = 0; base < total; base += 32) {
             const uint32_t t = base + lane;
-            const bool valid = t < total;
             const uint32_t jc = j;
             const double2 b0 = a0, b1 = a1;
             if (t + 32 < total) { j = slot_of(t + 32); a0 = __ldg(A.p0 + j); a1 = __ldg(A.p1 + j); }
             bool hit = false;
-            double wa = 0.0;
-            if (valid) {
+            double r2 = 0.0;
+            if (t < total) {
                 const double dx = min_image(__dsub_rn(px, b0.x), g.per[0], g.L[0], g.halfL[0]);
                 const double dy = min_image(__dsub_rn(py, b0.y), g.per[1], g.L[1], g.halfL[1]);
                 const double dz = min_image(__dsub_rn(pz, b1.x), g.per[2], g.L[2], g.halfL[2]);
-                const double r2 = r2_exact(dx, dy, dz);
-                const double ha = b1.y;
-                if (r2 < support2(ha)) {
-                    const double hinv = 1.0 / ha;
-                    wa = __ldg(A.s0 + jc).y * ((sigma<KERNEL>() * hinv * hinv * hinv) * shape_w<KERNEL>(sqrt(r2) * hinv));
-                    hit = wa != 0.0;
-                }
+                r2 = r2_exact(dx, dy, dz);
+                hit = r2 < support2(b1.y);
             }
-            if (PASS == 0) {
-                if (hit) {
-                    const double2 ga = __ldg(A.gA + jc), gb = __ldg(A.gB + jc);
-                    S.gx = fma(wa, ga.x, S.gx); S.gy = fma(wa, ga.y, S.gy); S.gz = fma(wa, gb.x, S.gz);
-                    S.kap = fma(wa, gb.y, S.kap);
-                    S.wsum += wa;
-                }
-                const uint32_t mask = __ballot_sync(0xFFFFFFFFu, hit);
-                if (hit) {
-                    const uint32_t pos = cnt + __popc(mask & ((1u << lane) - 1u));
-                    if (pos < (uint32_t)RAY_CAP) { c_idx[pos] = jc; c_w[pos] = wa; }
-                }
-                cnt += __popc(mask);
-            } else {
-                if (hit) atomicAdd(dep + jc, sc * wa);
+            if (cnt > (uint32_t)(RAY_CAP - 32)) {              // warp-uniform: the list may not take 32 more -- evaluate it now
+                ray_eval<KERNEL, PASS>(A, lane, cnt, c_idx, c_w, S, sc, dep);
+                overflow = true;
+                cnt = 0;
             }
+            const uint32_t mask = __ballot_sync(0xFFFFFFFFu, hit);
+            if (hit) {
+                const uint32_t pos = cnt + __popc(mask & ((1u << lane) - 1u));
+                c_idx[pos] = jc; c_w[pos] = r2;
+            }
+            cnt += __popc(mask);
         }
     }
     return cnt;
@@ -203,7 +221,9 @@ k_ray_trace(DevGrid g, RayIn A, RayArgs R) {
     int64_t k = 0;
     for (; k < R.nsteps && P > R.pmin; ++k) {
         RaySums S{0.0, 0.0, 0.0, 0.0, 0.0};
-        const uint32_t cnt = ray_visit<KERNEL, 0>(g, A, p[0], p[1], p[2], reach, lane, S, s_rt[warp], c_idx, c_w, 0.0, nullptr);
+        bool overflow = false;
+        const uint32_t cnt = ray_visit<KERNEL, 0>(g, A, p[0], p[1], p[2], reach, lane, S, s_rt[warp], c_idx, c_w, 0.0, nullptr, overflow);
+        ray_eval<KERNEL, 0>(A, lane, cnt, c_idx, c_w, S, 0.0, nullptr);
         S.gx = warp_sum(S.gx); S.gy = warp_sum(S.gy); S.gz = warp_sum(S.gz); S.kap = warp_sum(S.kap); S.wsum = warp_sum(S.wsum);
         // eq. (72), then the track length of this step with the new v (A31)
         v[0] = fma(acc, S.gx, v[0]); v[1] = fma(acc, S.gy, v[1]); v[2] = fma(acc, S.gz, v[2]);
@@ -212,13 +232,17 @@ k_ray_trace(DevGrid g, RayIn A, RayArgs R) {
             const double dE = P * (1.0 - exp(-S.kap * ds));     // eq. (71), kappa held over the step (A32)
             P -= dE;
             const double sc = dE / S.wsum;                      // normalised kernel weights (A33)
-            if (cnt <= (uint32_t)RAY_CAP) {
-                __syncwarp();
-                for (uint32_t t = lane; t < cnt; t += 32) atomicAdd(R.dep_sorted + c_idx[t], sc * c_w[t]);
+            if (!overflow) {
+                for (uint32_t t = lane; t < cnt; t += 32) {
+                    const double wa = c_w[t];
+                    if (wa != 0.0) atomicAdd(R.dep_sorted + c_idx[t], sc * wa);
+                }
                 __syncwarp();
             } else {
                 RaySums dummy{};
-                ray_visit<KERNEL, 1>(g, A, p[0], p[1], p[2], reach, lane, dummy, s_rt[warp], nullptr, nullptr, sc, R.dep_sorted);
+                bool o2 = false;
+                const uint32_t c2 = ray_visit<KERNEL, 1>(g, A, p[0], p[1], p[2], reach, lane, dummy, s_rt[warp], c_idx, c_w, sc, R.dep_sorted, o2);
+                ray_eval<KERNEL, 1>(A, lane, c2, c_idx, c_w, dummy, sc, R.dep_sorted);
             }
         }
         bool out = false;
