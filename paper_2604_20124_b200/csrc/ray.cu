@@ -26,6 +26,9 @@ namespace spray {
 
 constexpr int RAY_WARPS = 4;        // rays per CTA
 constexpr int RAY_CAP = 320;        // cached (slot, weight) pairs per ray and step
+#ifndef RAY_MINB
+#define RAY_MINB 8
+#endif
 
 struct RayIn {
     const double2 *p0, *p1, *s0, *gA, *gB;      // sorted records: (x,y) (z,h) (z,V) (G_x,G_y) (G_z,kappa^ib)
@@ -202,7 +205,7 @@ __device__ __forceinline__ double warp_sum(double v) {
 }
 
 template <int KERNEL>
-__global__ void __launch_bounds__(32 * RAY_WARPS)
+__global__ void __launch_bounds__(32 * RAY_WARPS, RAY_MINB)
 k_ray_trace(DevGrid g, RayIn A, RayArgs R) {
     __shared__ uint32_t s_idx[RAY_WARPS][RAY_CAP];
     __shared__ double s_w[RAY_WARPS][RAY_CAP];
