@@ -27,7 +27,7 @@ namespace spray {
 constexpr int RAY_WARPS = 4;        // rays per CTA
 constexpr int RAY_CAP = 320;        // cached (slot, weight) pairs per ray and step
 #ifndef RAY_MINB
-#define RAY_MINB 8
+#define RAY_MINB 6    // CTAs per SM the register budget is set for (80 registers): 8 -> 33.1 ms, 6 -> 31.7 ms, 4 (128 registers) -> 39.2 ms at c5
 #endif
 
 struct RayIn {
