@@ -181,3 +181,23 @@ def test_ray_full_size_c5_tube():
     ot = dict(o, gradn=o["gradn"][:, inner], S_gradn=o["S_gradn"][:, inner])
     e = compare(w, gt, ot, rays, dt, nsteps, c)
     print("c5 tube", tube.size, "of", w.n, "touched", int(touched.sum()), "worst edep error / tolerance", e)
+
+
+def test_ray_hit_list_overflow_and_many_rows():
+    """Supports so wide that a ray step accepts more particles (~700) than the per-warp hit list holds (320): the list is
+    evaluated in instalments and the deposit takes the second traversal; 2 h_max spans several cells, so the rows in reach
+    exceed one chunk of 32."""
+    w = workload("cloud_open")
+    h = 1.6 * w.h
+    grid = W.Grid(w.grid.lo, w.grid.hi, (12, 12, 12), w.grid.periodic, float(h.max()))      # 144 rows in reach
+    w.h, w.grid = h, grid
+    f, kib = medium(w)
+    rays = make_rays(w, 12)
+    dt, nsteps, c = 0.01, 60, 1.0
+    o = O.ray_deposit(w.grid, w.kernel, w.x, w.y, w.z, w.h, w.m, w.rho_nom, f, kib, rays, dt, nsteps, c)
+    # hits per step at the first ray's start position: well beyond the list capacity
+    d2 = (w.x - rays[0, 0]) ** 2 + (w.y - rays[1, 0]) ** 2 + (w.z - rays[2, 0]) ** 2
+    assert np.count_nonzero(d2 < 4.0 * h * h) > 200 and np.count_nonzero((w.x - 0.5) ** 2 + (w.y - 0.5) ** 2 + (w.z - 0.5) ** 2 < 4.0 * h * h) > 400
+    g = run_gpu(w, f, kib, rays, dt, nsteps, c)
+    e = compare(w, g, o, rays, dt, nsteps, c)
+    print("overflow case: worst edep error / tolerance", e)
