@@ -276,6 +276,49 @@ def conduction(grid, kernel, x, y, z, h, m, rho, k, T, targets=None):
 
 
 # ---------------------------------------------------------------------------------------------------------------
+# Row N2, second half: the implicit (backward-Euler) two-temperature heat-transport system of eqs. (26)-(34), P:L166-L192,
+# as a MATRIX-FREE operator: cond_implicit returns the left-hand sides of eqs. (28)/(29) applied to a given (u^i, u^e) and the
+# right-hand sides b^i + c, b^e - c of eqs. (33)/(34), assembled term by term in the paper's notation from the pair sums of
+# oracle_fld_apply in its symmetric mode with mu = k^s (called, not retyped: with E = g it returns diag_a = sum_b c_ab and
+# offd_a = -sum_b c_ab g_b, c_ab = (m_b/rho_b) 4 k_a k_b/(k_a+k_b) x_ab.gradWbar/|x_ab|^2, so that sum_b [4 m_b/(rho_a rho_b) ...] g_b =
+# -offd_a/rho_a).  tau^s = dT^s/du^s.
+#   Lambda^s_a = 1 - dt tau_a D_a + dt kei_a tau_a,  D_a = diag_a/rho_a                                  eq. (30)
+#   sum_b chi^s_ab u_b = dt sum_b [..]_ab tau_b u_b = -dt offd_a[g = tau u]/rho_a                        eq. (31)
+#   Gamma^s_a u_a = dt kei_a tau_a u_a                                                                  eq. (32)
+#   b^s_a = u_a + dt sum_b [..]_ab [T_a - T_b - tau_a u_a + tau_b u_b] = u_a + dt y_a[g = T - tau u]/rho_a   eq. (33)
+#   c_a = dt kei_a [T^e_a - T^i_a - tau^e_a u^e_a + tau^i_a u^i_a]                                       eq. (34)
+#   lhs^i = Lambda^i u^i + sum_b chi^i_ab u^i_b - Gamma^e u^e                                            eq. (28)
+#   lhs^e = Lambda^e u^e + sum_b chi^e_ab u^e_b - Gamma^i u^i                                            eq. (29), reading A37
+# Reading A37: eq. (29) prints "+ Gamma^i u^i"; substituting T^{N+1} = T^N + tau (u^{N+1} - u^N) into eq. (27), whose
+# exchange term is -k^ei (T^e - T^i), gives -Gamma^i u^i (the mirror image of eq. (28)); with the printed sign the exchange
+# would not conserve energy.  Pinned by substitution into eqs. (26)/(27) and by energy conservation (tests/test_oracle_cond.py).
+# Sign note: the paper's sums carry x_ab.gradWbar/|x_ab|^2 <= 0, and eqs. (26)/(27) are used exactly as printed (the same
+# expression oracle.conduction evaluates for eqs. (17)/(18)).
+def cond_implicit(grid, kernel, x, y, z, h, m, rho, k_i, k_e, kei, tau_i, tau_e, T_i, T_e, u_i, u_e, dt):
+    """Returns dict(lhs_i, lhs_e, rhs_i, rhs_e, S_i, S_e): lhs = operator of eqs. (28)/(29) applied to (u_i, u_e); rhs = b^i + c,
+    b^e - c of eqs. (33)/(34) for (u, T) taken as the time-level-N state; S = sums of absolute contributions (parity normaliser)."""
+    rho = np.asarray(rho, np.float64); kei = np.asarray(kei, np.float64)
+    out = {}
+    gam = {}
+    S = {}
+    for s, k, tau, T, u in (("i", k_i, tau_i, T_i, u_i), ("e", k_e, tau_e, T_e, u_e)):
+        k = np.asarray(k, np.float64); tau = np.asarray(tau, np.float64); T = np.asarray(T, np.float64); u = np.asarray(u, np.float64)
+        a1 = fld_apply(grid, kernel, x, y, z, h, m, rho, k, tau * u, sym_mode=True)
+        D = a1["diag"] / rho
+        Lam = 1.0 - dt * tau * D + dt * kei * tau                         # eq. (30)
+        chi = -dt * a1["offd"] / rho                                      # eq. (31)
+        gam[s] = dt * kei * tau * u                                       # eq. (32)
+        a2 = fld_apply(grid, kernel, x, y, z, h, m, rho, k, T - tau * u, sym_mode=True)
+        out["b_" + s] = u + dt * a2["y"] / rho                            # eq. (33)
+        out["lu_" + s] = Lam * u + chi
+        S[s] = np.abs(u) + dt * (a1["S_y"] + a2["S_y"] + a1["S_offd"]) / rho + dt * kei * (np.abs(tau * u) + np.abs(T))
+    c = dt * kei * (np.asarray(T_e) - np.asarray(T_i) - np.asarray(tau_e) * np.asarray(u_e) + np.asarray(tau_i) * np.asarray(u_i))   # eq. (34)
+    Sx = dt * kei * (np.abs(T_e) + np.abs(T_i) + np.abs(np.asarray(tau_e) * u_e) + np.abs(np.asarray(tau_i) * u_i))
+    return dict(lhs_i=out["lu_i"] - gam["e"], lhs_e=out["lu_e"] - gam["i"],          # eqs. (28), (29) (A37)
+                rhs_i=out["b_i"] + c, rhs_e=out["b_e"] - c, S_i=S["i"] + Sx, S_e=S["e"] + Sx)
+
+
+# ---------------------------------------------------------------------------------------------------------------
 # Row N3: continuity equation eq. (37) (P:L213) with the kernel-gradient-correction filter of eqs. (39)-(40) (P:L222-L228),
 # oracle_kgc_continuity in spray_oracle.c.  Reading A28: where the moment matrix is singular (|det| <= 1e-12) L = I.
 def kgc_continuity(grid, kernel, x, y, z, h, m, rho, vx, vy, vz, use_cells=True, targets=None):

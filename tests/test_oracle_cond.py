@@ -54,3 +54,105 @@ def test_quadratic_temperature_gives_the_laplacian(kname, hfac):
     k0 = 0.37
     r = O.conduction(g, KID[kname], x, y, z, h, m, rho, np.full(x.size, k0), T, targets=ctr)
     assert r["dudt"][0] == pytest.approx(k0 * np.trace(H) * s2 / rho[ctr[0]], rel=1e-11)
+
+
+# ---------------------------------------------------------------- implicit two-temperature system, eqs. (26)-(34) (oracle.cond_implicit)
+def _two_temperature_state(w, seed=3):
+    i = np.arange(w.n, dtype=np.int64)
+    k_i = 0.05 + 0.2 * W.u01(seed, i, 0)
+    k_e = 0.3 + w.kappa / (1.0 + w.kappa)
+    kei = 0.5 + 2.0 * W.u01(seed, i, 1)
+    tau_i = 0.6 + 0.3 * W.u01(seed, i, 2)
+    tau_e = 1.2 + 0.5 * W.u01(seed, i, 3)
+    u_i = 0.8 + 0.4 * W.u01(seed, i, 4)
+    u_e = 1.5 + w.E / np.max(w.E)
+    T_i = tau_i * u_i + 0.05 * W.u01(seed, i, 5)          # T need not be tau u (a general equation of state)
+    T_e = tau_e * u_e - 0.03 * W.u01(seed, i, 6)
+    return k_i, k_e, kei, tau_i, tau_e, T_i, T_e, u_i, u_e
+
+
+def _geom(w):
+    return (w.grid, w.kernel, w.x, w.y, w.z, w.h, w.m, w.rho_nom)
+
+
+def test_implicit_system_is_eqs_26_27_with_extrapolated_temperature():
+    """Substitution: for ANY trial state u^{N+1}, lhs(u^{N+1}) - rhs(u^N, T^N) must equal the residual of the backward-Euler
+    eqs. (26)/(27) with T^{N+1} = T^N + tau (u^{N+1} - u^N), evaluated independently with the pinned explicit
+    conduction term (oracle.conduction) and the exchange term written out.  A wrong sign or a dropped term anywhere in
+    eqs. (28)-(34) -- in particular the sign of Gamma in eq. (29) (A37) -- fails this."""
+    w = W.random_cloud(2500, seed=31, periodic=(1, 0, 1), hvar=1.8)
+    k_i, k_e, kei, tau_i, tau_e, T_i, T_e, u_i, u_e = _two_temperature_state(w)
+    i = np.arange(w.n, dtype=np.int64)
+    v_i = u_i * (1.0 + 0.2 * (W.u01(8, i, 0) - 0.5))      # trial u^{N+1}
+    v_e = u_e * (1.0 + 0.2 * (W.u01(8, i, 1) - 0.5))
+    dt = 0.37
+    g = _geom(w)
+    rhs = O.cond_implicit(*g, k_i, k_e, kei, tau_i, tau_e, T_i, T_e, u_i, u_e, dt)
+    lhs = O.cond_implicit(*g, k_i, k_e, kei, tau_i, tau_e, T_i, T_e, v_i, v_e, dt)
+    Tn_i = T_i + tau_i * (v_i - u_i)
+    Tn_e = T_e + tau_e * (v_e - u_e)
+    ci = O.conduction(*g, k_i, Tn_i); ce = O.conduction(*g, k_e, Tn_e)
+    res_i = (v_i - u_i) - dt * (ci["dudt"] + kei * (Tn_e - Tn_i))          # eq. (26)
+    res_e = (v_e - u_e) - dt * (ce["dudt"] - kei * (Tn_e - Tn_i))          # eq. (27)
+    assert np.max(np.abs(res_i)) > 1e-3
+    assert np.all(np.abs((lhs["lhs_i"] - rhs["rhs_i"]) - res_i) <= 1e-13 * (rhs["S_i"] + lhs["S_i"]))
+    assert np.all(np.abs((lhs["lhs_e"] - rhs["rhs_e"]) - res_e) <= 1e-13 * (rhs["S_e"] + lhs["S_e"]))
+
+
+def test_implicit_system_conserves_total_energy():
+    """Conduction is symmetric in (a, b) and the exchange terms of the two species cancel, so for any u:
+    sum_a m_a [lhs^i + lhs^e - u^i - u^e] = 0 and sum_a m_a [rhs^i + rhs^e - u^i - u^e] = 0: a solution of lhs = rhs has the
+    total energy of the old state."""
+    w = W.random_cloud(3000, seed=32, periodic=(1, 1, 1), hvar=2.0)
+    st = _two_temperature_state(w)
+    r = O.cond_implicit(*_geom(w), *st, 0.2)
+    u_i, u_e = st[7], st[8]
+    scale = np.sum(w.m * (r["S_i"] + r["S_e"]))
+    assert abs(np.sum(w.m * (r["lhs_i"] + r["lhs_e"] - u_i - u_e))) <= 1e-13 * scale
+    assert abs(np.sum(w.m * (r["rhs_i"] + r["rhs_e"] - u_i - u_e))) <= 1e-13 * scale
+    assert np.max(np.abs(r["lhs_i"] - u_i)) > 1e-3 and np.max(np.abs(r["rhs_e"] - u_e)) > 1e-3
+
+
+def test_implicit_system_equilibrium_and_identity_rows():
+    """Uniform, equal temperatures with T = tau u: nothing conducts or is exchanged, so rhs = u^N; and with uniform tau the
+    operator maps a uniform u (same for both species) to itself (row sums of A are 1)."""
+    w = W.random_cloud(900, seed=33, periodic=(0, 0, 0), hvar=1.6)
+    k_i, k_e, kei, *_ = _two_temperature_state(w)
+    tau = np.full(w.n, 0.7)
+    u = np.full(w.n, 2.0)
+    r = O.cond_implicit(*_geom(w), k_i, k_e, kei, tau, tau, tau * u, tau * u, u, u, 0.5)
+    for key in ("rhs_i", "rhs_e", "lhs_i", "lhs_e"):
+        assert np.allclose(r[key], u, rtol=0, atol=1e-12 * np.max(r["S_i"] + r["S_e"])), key
+
+
+def test_dense_solve_of_the_operator_satisfies_backward_euler():
+    """40 particles: the 2n x 2n matrix of eqs. (28)/(29) assembled column by column from the matrix-free operator (it is
+    linear: lhs(u) is applied to unit vectors), solved with numpy; the solution satisfies eqs. (26)/(27) with the extrapolated
+    temperature (independent evaluation through oracle.conduction), conserves energy, and the matrix is strictly diagonally
+    dominant by columns in the mass-weighted sense (Lambda >= 1)."""
+    n = 40
+    w = W.random_cloud(n, seed=34, periodic=(0, 0, 0), hvar=1.5)
+    h = 1.6 * w.h
+    grid = W.Grid((0.0, 0.0, 0.0), (1.0, 1.0, 1.0), (1, 1, 1), (0, 0, 0), float(h.max()))
+    geom = (grid, w.kernel, w.x, w.y, w.z, h, w.m, w.rho_nom)
+    k_i, k_e, kei, tau_i, tau_e, T_i, T_e, u_i, u_e = _two_temperature_state(w)
+    dt = 0.8
+    args = (k_i, k_e, kei, tau_i, tau_e, T_i, T_e)
+    base = O.cond_implicit(*geom, *args, u_i, u_e, dt)
+    A = np.zeros((2 * n, 2 * n))
+    z = np.zeros(n)
+    for j in range(2 * n):
+        e = np.zeros(2 * n); e[j] = 1.0
+        r = O.cond_implicit(*geom, *args, e[:n], e[n:], dt)
+        A[:n, j], A[n:, j] = r["lhs_i"], r["lhs_e"]
+    assert np.all(np.diag(A) >= 1.0)
+    sol = np.linalg.solve(A, np.concatenate([base["rhs_i"], base["rhs_e"]]))
+    v_i, v_e = sol[:n], sol[n:]
+    Tn_i = T_i + tau_i * (v_i - u_i); Tn_e = T_e + tau_e * (v_e - u_e)
+    ci = O.conduction(*geom, k_i, Tn_i)["dudt"]; ce = O.conduction(*geom, k_e, Tn_e)["dudt"]
+    assert np.allclose(v_i - u_i, dt * (ci + kei * (Tn_e - Tn_i)), rtol=1e-9, atol=1e-12)
+    assert np.allclose(v_e - u_e, dt * (ce - kei * (Tn_e - Tn_i)), rtol=1e-9, atol=1e-12)
+    assert abs(np.sum(w.m * (v_i + v_e - u_i - u_e))) <= 1e-12 * np.sum(w.m * (u_i + u_e))
+    assert np.max(np.abs(v_e - u_e)) > 1e-2                                # something happened
+    # relaxation: the species' temperatures move towards each other
+    assert np.mean(np.abs(Tn_e - Tn_i)) < np.mean(np.abs(T_e - T_i))
