@@ -161,6 +161,24 @@ int spray_neighbor_digest(spray_ctx* ctx, int symmetric, uint64_t* dsum, uint64_
 int spray_conduction(spray_ctx* ctx, const double* m, const double* rho, const double* k, const double* T, double* dudt,
                      void* stream);
 
+/* (N2, second half) implicit two-temperature heat transport: the backward-Euler system eqs. (28)-(29) as a
+ * MATRIX-FREE operator (the paper assembles it for cuSPARSE ILU-BiCGSTAB; here it is applied, never stored), and its
+ * right-hand side eqs. (33)-(34).  With C^s[g]_a = sum_b 4 m_b/(rho_a rho_b) k^s_a k^s_b/(k^s_a+k^s_b) (g_a - g_b) x_ab.gradWbar/|x_ab|^2
+ * (the pair sum of spray_conduction over N_sym(a)), tau^s = dT^s/du^s and X_a = kei_a (g^e_a - g^i_a):
+ *   which = SPRAY_COND_OPERATOR:  g^s = tau^s u^s,            out^i = u^i - dt (C^i[g^i] + X),  out^e = u^e - dt (C^e[g^e] - X)
+ *        = Lambda^i u^i + sum_b chi^i_ab u^i_b - Gamma^e u^e  and  Lambda^e u^e + sum_b chi^e_ab u^e_b - Gamma^i u^i, eqs. (28)-(32)
+ *        (eq. (29) prints + Gamma^i: DESIGN.md A37).  T_i, T_e are not read (may be NULL).
+ *   which = SPRAY_COND_RHS:       g^s = T^s - tau^s u^s,      out^i = u^i + dt (C^i[g^i] + X) = b^i + c,  out^e = u^e + dt (C^e[g^e] - X) = b^e - c,
+ *        eqs. (33)-(34), with (u, T) the state at time level N.
+ * A Krylov or Jacobi solve of out_OPERATOR(u) = out_RHS is caller-side (two sweeps per application).
+ * Inputs [n], caller order: m, rho, k_i, k_e (> 0), kei, dTdu_i, dTdu_e, T_i, T_e, u_i, u_e.  Outputs out_i, out_e [n], must not
+ * alias inputs.  Errors: SPRAY_ERR_INVALID_ARG (NULL, unknown `which`, dt <= 0), SPRAY_ERR_ALLOC (scratch, first call). */
+typedef enum { SPRAY_COND_OPERATOR = 0, SPRAY_COND_RHS = 1 } spray_cond_which_t;
+int spray_conduction_implicit(spray_ctx* ctx, const double* m, const double* rho, const double* k_i, const double* k_e,
+                              const double* kei, const double* dTdu_i, const double* dTdu_e, const double* T_i, const double* T_e,
+                              const double* u_i, const double* u_e, double dt, spray_cond_which_t which, double* out_i, double* out_e,
+                              void* stream);
+
 /* (N3) continuity equation with the kernel-gradient-correction (KGC) filter, P:L207-L228:
  *       M_a = sum_b (m_b/rho_b) gradW(x_ab,h_a) (x) x_ba          eq. (40): row i = dW/dx_i, column j = (x_b - x_a)_j
  *       L_a = M_a^{-1}                                            eq. (40)

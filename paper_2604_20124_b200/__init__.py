@@ -19,12 +19,13 @@ _LIBPATH = Path(__file__).resolve().parent / "libspray_b200.so"
 KERNEL_CUBIC_SPLINE, KERNEL_WENDLAND_C2 = 0, 1
 FLD_SYMMETRIC, FLD_GATHER = 0, 1
 FLD_UPDATE_LIMITER, FLD_FROZEN = 0, 1
+COND_OPERATOR, COND_RHS = 0, 1
 DEV_H_EXCEEDS_HMAX, DEV_OUTSIDE_BOX, DEV_LIST_OVERFLOW = 1, 2, 4
 
 # every symbol include/spray.h declares
 EXPORTS = ["spray_version", "spray_create", "spray_destroy", "spray_last_error", "spray_check", "spray_launch_count", "spray_set_path", "spray_path_stats",
            "spray_build_cells", "spray_density", "spray_hydro_rhs", "spray_fld_apply", "spray_get_cell_table",
-           "spray_neighbor_counts", "spray_neighbor_lists", "spray_neighbor_digest", "spray_rad_jacobi", "spray_conduction", "spray_kgc_continuity", "spray_ray_deposit", "spray_fp64_peak_probe"]
+           "spray_neighbor_counts", "spray_neighbor_lists", "spray_neighbor_digest", "spray_rad_jacobi", "spray_conduction", "spray_kgc_continuity", "spray_ray_deposit", "spray_conduction_implicit", "spray_fp64_peak_probe"]
 
 
 class SprayError(RuntimeError):
@@ -66,6 +67,7 @@ def load():
     lib.spray_fld_apply.argtypes = [vp, vp, vp, vp, vp, dbl, i32, i32, vp, vp, vp, vp, vp, vp]
     lib.spray_conduction.argtypes = [vp, vp, vp, vp, vp, vp, vp]
     lib.spray_kgc_continuity.argtypes = [vp] * 10
+    lib.spray_conduction_implicit.argtypes = [vp] + [vp] * 11 + [dbl, i32, vp, vp, vp]
     lib.spray_rad_jacobi.argtypes = [vp] + [vp] * 8 + [dbl, dbl, dbl, i32, i32, vp, vp, vp, vp]
     lib.spray_ray_deposit.argtypes = [vp, vp, vp, vp, vp, i64, vp, dbl, i64, dbl, dbl, vp, vp, vp, vp, vp]
     lib.spray_get_cell_table.argtypes = [vp, vp, vp, vp, vp, vp]
@@ -213,6 +215,16 @@ class Spray:
                                        _ptr(dudt, f64, self.n), _stream())
         self._ck(rc, "spray_conduction")
         return dudt
+
+    def conduction_implicit(self, m, rho, k_i, k_e, kei, dTdu_i, dTdu_e, T_i, T_e, u_i, u_e, dt, which):
+        """Row N2, implicit two-temperature system eqs. (28)-(34): which = COND_OPERATOR (left-hand sides applied to (u_i, u_e);
+        T_i, T_e may be None) or COND_RHS (b^i + c, b^e - c).  Returns (out_i, out_e)."""
+        f64 = self.torch.float64
+        out_i, out_e = self._out(None), self._out(None)
+        a = [_ptr(t, f64, self.n) for t in (m, rho, k_i, k_e, kei, dTdu_i, dTdu_e, T_i, T_e, u_i, u_e)]
+        rc = self.lib.spray_conduction_implicit(self.h, *a, float(dt), int(which), _ptr(out_i, f64, self.n), _ptr(out_e, f64, self.n), _stream())
+        self._ck(rc, "spray_conduction_implicit")
+        return out_i, out_e
 
     def kgc_continuity(self, m, rho, vx, vy, vz, want_L=True, want_raw=True):
         """Row N3: continuity equation eq. (37) with the KGC filter of eqs. (39)-(40) (include/spray.h).

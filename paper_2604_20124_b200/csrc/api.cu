@@ -338,6 +338,51 @@ int spray_conduction(spray_ctx* ctx, const double* m, const double* rho, const d
     return SPRAY_OK;
 }
 
+// pair sum of the conduction operator for one species: y_a = sum_b V_b 4 k_a k_b/(k_a+k_b) (g_a - g_b) Fbar/r (not yet divided by rho_a)
+static int cond_pair_sum(Ctx* c, const double* m, const double* rho, const double* k, const double* g, double* y, cudaStream_t st) {
+    double** f = c->s.f;
+    PrepJob pj{};
+    pj.m = m; pj.rho = rho; pj.E = g; pj.kx = k; pj.kx_is_mu = 1;
+    pj.sm = f[F_M]; pj.srho = f[F_RHO]; pj.sE = f[F_E]; pj.skx = f[F_MU]; pj.sV = f[F_V];
+    CK(launch_prep_fld(c, pj, st), "implicit conduction: prologue");
+    if (c->tl.enabled) {
+        TiledArgs t{};
+        t.fld_sym = 1; t.o0 = y;
+        CK(launch_tiled_sweep(c, SW_APPLY, t, st), "implicit conduction: tiled sweep");
+    }
+    SweepArgs a = fallback_args(c);
+    a.m = f[F_M]; a.rho = f[F_RHO]; a.E = f[F_E]; a.mu = f[F_MU]; a.fld_sym = 1; a.o0 = y;
+    CK(launch_ref_sweep(c, SW_APPLY, a, st), "implicit conduction: sweep");
+    return SPRAY_OK;
+}
+
+int spray_conduction_implicit(spray_ctx* ctx, const double* m, const double* rho, const double* k_i, const double* k_e,
+                              const double* kei, const double* dTdu_i, const double* dTdu_e, const double* T_i, const double* T_e,
+                              const double* u_i, const double* u_e, double dt, spray_cond_which_t which, double* out_i, double* out_e,
+                              void* stream) {
+    NEED_BUILT();
+    Ctx* c = &ctx->c;
+    if (which != SPRAY_COND_OPERATOR && which != SPRAY_COND_RHS) return fail(c, SPRAY_ERR_INVALID_ARG, "spray_conduction_implicit: unknown `which`");
+    const bool rhs = which == SPRAY_COND_RHS;
+    if (c->n > 0 && (!m || !rho || !k_i || !k_e || !kei || !dTdu_i || !dTdu_e || !u_i || !u_e || !out_i || !out_e || (rhs && (!T_i || !T_e))))
+        return fail(c, SPRAY_ERR_INVALID_ARG, "spray_conduction_implicit: NULL argument");
+    if (!(dt > 0.0)) return fail(c, SPRAY_ERR_INVALID_ARG, "spray_conduction_implicit: dt must be > 0");
+    for (double*& r : c->rad_scratch)
+        if (!r && !dmalloc(&r, c->n_max)) { cudaGetLastError(); return fail(c, SPRAY_ERR_ALLOC, "spray_conduction_implicit: scratch allocation failed"); }
+    cudaStream_t st = (cudaStream_t)stream;
+    CondArgs a{};
+    a.rho = rho; a.kei = kei; a.tau_i = dTdu_i; a.tau_e = dTdu_e; a.T_i = T_i; a.T_e = T_e; a.u_i = u_i; a.u_e = u_e;
+    a.g_i = c->rad_scratch[0]; a.g_e = c->rad_scratch[1]; a.y_i = c->rad_scratch[2]; a.y_e = c->rad_scratch[3];
+    a.dt = dt; a.rhs = rhs ? 1 : 0; a.out_i = out_i; a.out_e = out_e;
+    CK(launch_cond_form(c, a, st), "implicit conduction: g");
+    int rc = cond_pair_sum(c, m, rho, k_i, a.g_i, c->rad_scratch[2], st);
+    if (rc != SPRAY_OK) return rc;
+    rc = cond_pair_sum(c, m, rho, k_e, a.g_e, c->rad_scratch[3], st);
+    if (rc != SPRAY_OK) return rc;
+    CK(launch_cond_combine(c, a, st), "implicit conduction: combine");
+    return SPRAY_OK;
+}
+
 int spray_kgc_continuity(spray_ctx* ctx, const double* m, const double* rho, const double* vx, const double* vy,
                          const double* vz, double* drhodt, double* L, double* drhodt_raw, void* stream) {
     NEED_BUILT();

@@ -67,6 +67,37 @@ cudaError_t launch_div_by_rho(Ctx* c, double* y, const double* rho, cudaStream_t
     return cudaGetLastError();
 }
 
+// N2, implicit two-temperature system: per-particle parts of eqs. (28)-(34)
+__global__ void k_cond_form(CondArgs a, int64_t n) {
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const double gi = a.tau_i[i] * a.u_i[i], ge = a.tau_e[i] * a.u_e[i];
+        a.g_i[i] = a.rhs ? a.T_i[i] - gi : gi;
+        a.g_e[i] = a.rhs ? a.T_e[i] - ge : ge;
+    }
+}
+__global__ void k_cond_combine(CondArgs a, int64_t n) {
+    const double sdt = a.rhs ? a.dt : -a.dt;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const double rinv = 1.0 / a.rho[i];
+        const double X = a.kei[i] * (a.g_e[i] - a.g_i[i]);       // exchange term of eqs. (26)/(27) on g
+        a.out_i[i] = fma(sdt, fma(a.y_i[i], rinv, X), a.u_i[i]);
+        a.out_e[i] = fma(sdt, fma(a.y_e[i], rinv, -X), a.u_e[i]);
+    }
+}
+static int cond_blocks(int64_t n) { const int64_t want = (n + 255) / 256; return (int)(want < 148 * 32 ? want : 148 * 32); }
+cudaError_t launch_cond_form(Ctx* c, const CondArgs& a, cudaStream_t st) {
+    if (c->n == 0) return cudaSuccess;
+    k_cond_form<<<cond_blocks(c->n), 256, 0, st>>>(a, c->n);
+    c->launches += 1;
+    return cudaGetLastError();
+}
+cudaError_t launch_cond_combine(Ctx* c, const CondArgs& a, cudaStream_t st) {
+    if (c->n == 0) return cudaSuccess;
+    k_cond_combine<<<cond_blocks(c->n), 256, 0, st>>>(a, c->n);
+    c->launches += 1;
+    return cudaGetLastError();
+}
+
 cudaError_t launch_rad_update(Ctx* c, const RadArgs& a, cudaStream_t st) {
     if (c->n == 0) return cudaSuccess;
     const int64_t want = (c->n + 255) / 256;

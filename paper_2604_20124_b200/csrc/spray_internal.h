@@ -143,6 +143,18 @@ struct RadArgs {
 };
 cudaError_t launch_rad_update(Ctx* c, const RadArgs& a, cudaStream_t st);
 cudaError_t launch_div_by_rho(Ctx* c, double* y, const double* rho, cudaStream_t st);   // N2
+// N2 implicit system (eqs. (28)-(34)): g = tau u (rhs = 0) or T - tau u (rhs = 1) for both species; then
+// out^i = u^i + s dt (y^i/rho + X), out^e = u^e + s dt (y^e/rho - X), X = kei (g^e - g^i), s = -1 (operator) or +1 (rhs)
+struct CondArgs {
+    const double *rho, *kei, *tau_i, *tau_e, *T_i, *T_e, *u_i, *u_e;   // caller order
+    double *g_i, *g_e;                                                 // caller-order scratch
+    const double *y_i, *y_e;                                           // caller-order pair sums of the two species
+    double dt;
+    int rhs;
+    double *out_i, *out_e;
+};
+cudaError_t launch_cond_form(Ctx* c, const CondArgs& a, cudaStream_t st);
+cudaError_t launch_cond_combine(Ctx* c, const CondArgs& a, cudaStream_t st);
 
 // ---- ray.cu : row N4, mesh-free laser ray tracing and deposition
 struct RayArgs {
