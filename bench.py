@@ -348,6 +348,41 @@ def main():
               "flop_roofline_frac": pairs["apply"] * FLOPS[w.kernel]["apply"] / t_it / (fp64_meas * 1e12),
               "resid_last": float(rj["resid"][-1].item()), "note": "includes the one-off prologue of the call (1/%d per iteration)" % nit}
 
+    # ---- row N2: thermal conduction (spray_conduction: one symmetric frozen sweep of the apply kernel with mu = k, E = T) and the
+    #      matrix-free operator of the implicit two-temperature system, eqs. (28)-(34) (spray_conduction_implicit: two sweeps, one
+    #      per species); k proportional to T^(5/2) (Spitzer-like), same lists; apply flops per ordered pair
+    n2 = None
+    if not args.no_n1:
+        u_g = d["p"] / ((w.gamma - 1.0) * out["rho"])
+        T_g = (w.gamma - 1.0) * u_g
+        T_e = 1.1 * T_g
+        k_i = 0.02 * (T_g / T_g.mean()) ** 2.5 + 1e-3
+        k_e = 0.05 * (T_e / T_e.mean()) ** 2.5 + 1e-3
+        kei = torch.full_like(u_g, 0.5)
+        tau = torch.full_like(u_g, w.gamma - 1.0)
+        u_e = T_e / (w.gamma - 1.0)
+        dt_c = 0.3 * float(w.h.min()) ** 2 / float(k_e.max().item())
+        def _time(fn, nrep=5):
+            fn(); fn()
+            torch.cuda.synchronize()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            for _ in range(nrep):
+                fn()
+            b.record()
+            torch.cuda.synchronize()
+            return a.elapsed_time(b) * 1e-3 / nrep
+        t_c = _time(lambda: sp.conduction(d["m"], out["rho"], k_i, T_g))
+        t_o = _time(lambda: sp.conduction_implicit(d["m"], out["rho"], k_i, k_e, kei, tau, tau, None, None, u_g, u_e, dt_c, 0))
+        fa = FLOPS[w.kernel]["apply"]
+        n2 = {"call": "spray_conduction", "ms_per_call": 1e3 * t_c, "pair_interactions_per_s": pairs["apply"] / t_c,
+              "flop_roofline_frac": pairs["apply"] * fa / t_c / (fp64_meas * 1e12),
+              "implicit_operator": {"call": "spray_conduction_implicit(SPRAY_COND_OPERATOR)", "ms_per_application": 1e3 * t_o,
+                                    "pair_interactions_per_s": 2 * pairs["apply"] / t_o,
+                                    "flop_roofline_frac": 2 * pairs["apply"] * fa / t_o / (fp64_meas * 1e12),
+                                    "note": "two symmetric frozen sweeps (ions, electrons) + per-particle form/combine kernels"}}
+        del u_g, T_g, T_e, k_i, k_e, kei, tau, u_e
+
     # ---- row N3: continuity equation with the KGC filter (spray_kgc_continuity), same lists; 60 flops per in-support ordered pair
     #      over N_gather (distance 9, sqrt + 1/r + F 12, grad W and V_b 6, moment matrix 12, v_ab 3, velocity moments 18)
     n3 = None
@@ -453,7 +488,7 @@ def main():
                        "parallelism": "replicas only" if world > 1 else "1 GPU", "path": args.path,
                        "tiles": n_tiles, "tiled_fraction": n_fast / max(n, 1)},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
-            "fp64_probe_tflops": fp64_meas, "next_rows": {"N1_rad_jacobi": n1, "N3_kgc_continuity": n3, "N4_ray_deposit": n4}}
+            "fp64_probe_tflops": fp64_meas, "next_rows": {"N1_rad_jacobi": n1, "N2_conduction": n2, "N3_kgc_continuity": n3, "N4_ray_deposit": n4}}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -294,26 +294,33 @@ def conduction(grid, kernel, x, y, z, h, m, rho, k, T, targets=None):
 # would not conserve energy.  Pinned by substitution into eqs. (26)/(27) and by energy conservation (tests/test_oracle_cond.py).
 # Sign note: the paper's sums carry x_ab.gradWbar/|x_ab|^2 <= 0, and eqs. (26)/(27) are used exactly as printed (the same
 # expression oracle.conduction evaluates for eqs. (17)/(18)).
-def cond_implicit(grid, kernel, x, y, z, h, m, rho, k_i, k_e, kei, tau_i, tau_e, T_i, T_e, u_i, u_e, dt):
+def cond_implicit(grid, kernel, x, y, z, h, m, rho, k_i, k_e, kei, tau_i, tau_e, T_i, T_e, u_i, u_e, dt, targets=None):
     """Returns dict(lhs_i, lhs_e, rhs_i, rhs_e, S_i, S_e): lhs = operator of eqs. (28)/(29) applied to (u_i, u_e); rhs = b^i + c,
-    b^e - c of eqs. (33)/(34) for (u, T) taken as the time-level-N state; S = sums of absolute contributions (parity normaliser)."""
-    rho = np.asarray(rho, np.float64); kei = np.asarray(kei, np.float64)
+    b^e - c of eqs. (33)/(34) for (u, T) taken as the time-level-N state; S = sums of absolute contributions (parity normaliser).  `targets` (indices)
+    restricts the rows that are evaluated (full-size sampled parity); the arithmetic of a row does not depend on it."""
+    rho_all = np.asarray(rho, np.float64)
+    sel = slice(None) if targets is None else np.asarray(targets, np.int64)
+    rho = rho_all[sel]; kei = np.asarray(kei, np.float64)[sel]
+    T_i, T_e, tau_i, tau_e, u_i, u_e = (np.asarray(a, np.float64) for a in (T_i, T_e, tau_i, tau_e, u_i, u_e))
     out = {}
     gam = {}
     S = {}
     for s, k, tau, T, u in (("i", k_i, tau_i, T_i, u_i), ("e", k_e, tau_e, T_e, u_e)):
-        k = np.asarray(k, np.float64); tau = np.asarray(tau, np.float64); T = np.asarray(T, np.float64); u = np.asarray(u, np.float64)
-        a1 = fld_apply(grid, kernel, x, y, z, h, m, rho, k, tau * u, sym_mode=True)
+        k = np.asarray(k, np.float64)
+        a1 = fld_apply(grid, kernel, x, y, z, h, m, rho_all, k, tau * u, sym_mode=True, targets=targets)
+        g2 = T - tau * u
+        tau = tau[sel]; T = T[sel]; u = u[sel]
         D = a1["diag"] / rho
         Lam = 1.0 - dt * tau * D + dt * kei * tau                         # eq. (30)
         chi = -dt * a1["offd"] / rho                                      # eq. (31)
         gam[s] = dt * kei * tau * u                                       # eq. (32)
-        a2 = fld_apply(grid, kernel, x, y, z, h, m, rho, k, T - tau * u, sym_mode=True)
+        a2 = fld_apply(grid, kernel, x, y, z, h, m, rho_all, k, g2, sym_mode=True, targets=targets)
         out["b_" + s] = u + dt * a2["y"] / rho                            # eq. (33)
         out["lu_" + s] = Lam * u + chi
         S[s] = np.abs(u) + dt * (a1["S_y"] + a2["S_y"] + a1["S_offd"]) / rho + dt * kei * (np.abs(tau * u) + np.abs(T))
-    c = dt * kei * (np.asarray(T_e) - np.asarray(T_i) - np.asarray(tau_e) * np.asarray(u_e) + np.asarray(tau_i) * np.asarray(u_i))   # eq. (34)
-    Sx = dt * kei * (np.abs(T_e) + np.abs(T_i) + np.abs(np.asarray(tau_e) * u_e) + np.abs(np.asarray(tau_i) * u_i))
+    T_i, T_e, tau_i, tau_e, u_i, u_e = T_i[sel], T_e[sel], tau_i[sel], tau_e[sel], u_i[sel], u_e[sel]
+    c = dt * kei * (T_e - T_i - tau_e * u_e + tau_i * u_i)   # eq. (34)
+    Sx = dt * kei * (np.abs(T_e) + np.abs(T_i) + np.abs(tau_e * u_e) + np.abs(tau_i * u_i))
     return dict(lhs_i=out["lu_i"] - gam["e"], lhs_e=out["lu_e"] - gam["i"],          # eqs. (28), (29) (A37)
                 rhs_i=out["b_i"] + c, rhs_e=out["b_e"] - c, S_i=S["i"] + Sx, S_e=S["e"] + Sx)
 

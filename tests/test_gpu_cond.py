@@ -104,6 +104,34 @@ def test_conduction_implicit_parity(name):
     print(name, "max normalised error", e)
 
 
+def test_conduction_implicit_full_size_sampled():
+    """Config 5 (16.7M particles), the launch configuration of bench.py: operator and right-hand side of eqs. (28)-(34) at 1500
+    sampled rows against oracle.cond_implicit (which evaluates those rows only)."""
+    import torch
+    from paper_2604_20124_b200 import COND_OPERATOR, COND_RHS
+    w = W.make("c5")
+    i = np.arange(1500, dtype=np.uint64)
+    sel = np.unique((W.splitmix64(i + np.uint64(177)) % np.uint64(w.n)).astype(np.int64))
+    st = _state(w, seed=5)
+    dt = 0.3 * float(w.h.min()) ** 2 / 0.5
+    o = O.cond_implicit(w.grid, w.kernel, w.x, w.y, w.z, w.h, w.m, w.rho_nom, *st, dt, targets=sel)
+    d = upload(w)
+    sp = make_ctx(w)
+    sp.build_cells(w.grid, w.kernel, d["x"], d["y"], d["z"], d["h"])
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    ts = [t(a) for a in st]
+    li, le = sp.conduction_implicit(d["m"], d["rho_nom"], *ts[:5], None, None, ts[7], ts[8], dt, COND_OPERATOR)
+    ri, re = sp.conduction_implicit(d["m"], d["rho_nom"], *ts, dt, COND_RHS)
+    torch.cuda.synchronize()
+    g = lambda a: a.cpu().numpy()[sel]
+    e = max(check("lhs_i", g(li), o["lhs_i"], o["S_i"]), check("lhs_e", g(le), o["lhs_e"], o["S_e"]),
+            check("rhs_i", g(ri), o["rhs_i"], o["S_i"]), check("rhs_e", g(re), o["rhs_e"], o["S_e"]))
+    assert np.max(np.abs(o["lhs_e"] - st[8][sel])) > 1e-6 * np.max(st[8])
+    assert sp.path_stats()[1] == w.n          # every particle was served by the tiled kernels
+    assert sp.check() == 0
+    print("c5 sampled: max normalised error", e)
+
+
 def test_conduction_implicit_jacobi_solve_converges_to_backward_euler():
     """The operator in use: a damped Jacobi iteration u <- u + (rhs - A u) / Lambda-bound on the GPU operator converges, and the
     fixed point satisfies eqs. (26)/(27) with the extrapolated temperature evaluated by the oracle's explicit conduction term."""

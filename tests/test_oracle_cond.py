@@ -156,3 +156,18 @@ def test_dense_solve_of_the_operator_satisfies_backward_euler():
     assert np.max(np.abs(v_e - u_e)) > 1e-2                                # something happened
     # relaxation: the species' temperatures move towards each other
     assert np.mean(np.abs(Tn_e - Tn_i)) < np.mean(np.abs(T_e - T_i))
+
+
+def test_cond_implicit_targets_select_rows():
+    """`targets` only selects the rows that are evaluated: the sampled rows are bitwise those of the full evaluation."""
+    w = W.random_cloud(3000, seed=21, periodic=(1, 0, 1), hvar=1.8)
+    i = np.arange(w.n, dtype=np.int64)
+    f = lambda c, a, b: a + b * W.u01(9, i, c)
+    st = (f(0, 0.05, 0.2), f(1, 0.3, 0.5), f(2, 0.5, 2.0), f(3, 0.6, 0.3), f(4, 1.2, 0.5), f(5, 0.7, 0.4), f(6, 1.9, 0.6),
+          f(7, 0.8, 0.4), f(8, 1.5, 0.5))
+    dt = 0.3 * float(w.h.min()) ** 2 / 0.5
+    full = O.cond_implicit(w.grid, w.kernel, w.x, w.y, w.z, w.h, w.m, w.rho_nom, *st, dt)
+    sel = np.array([0, 7, 2999, 123, 300], dtype=np.int64)
+    part = O.cond_implicit(w.grid, w.kernel, w.x, w.y, w.z, w.h, w.m, w.rho_nom, *st, dt, targets=sel)
+    for k in full:
+        assert np.array_equal(part[k], full[k][sel]), k
