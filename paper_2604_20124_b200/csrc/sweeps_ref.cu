@@ -29,6 +29,23 @@ __device__ __forceinline__ Span cell_span(const DevGrid& g, int d, int c, double
 }
 __device__ __forceinline__ int wrap_cell(int c, int nc) { return c < 0 ? c + nc : (c >= nc ? c - nc : c); }
 
+// Cell culling.  t = (x_a - lo_d) * inv_d as k_cell_key computes it (cell units), ca = the target's cell, o = the (unwrapped)
+// offset of a visited cell: every particle b of that cell has (x_b - lo_d) * inv_d in [ca + o, ca + o + 1) (or beyond the outer
+// face when it was clamped into a boundary cell), so |x_a - x_b| >= gap / inv_d with gap = o - f (o > 0), f + |o| - 1 (o < 0),
+// 0 (o = 0), f = t - ca.  In a periodic dimension the image at offset o is the nearest one as long as the span does not cover
+// the whole dimension (2R + 1 < nc); when it does, `full` switches the bound off.  1e-9 cell units cover the rounding of t.
+// A cell farther than the reach in this bound holds no neighbour and is skipped: the neighbour sets do not change.
+__device__ __forceinline__ double cell_gap2(int o, double f, bool full, double edge) {
+    double gp = 0.0;
+    if (!full) {
+        if (o > 0) gp = (double)o - f;
+        else if (o < 0) gp = f - (double)(o + 1);
+    }
+    gp = gp - 1e-9;
+    gp = gp > 0.0 ? gp * edge : 0.0;
+    return gp * gp;
+}
+
 template <int SWEEP, int KERNEL>
 __device__ __forceinline__ void ref_particle(const DevGrid& g, int64_t n, const CellTabs& T, const SweepArgs& A, int64_t i) {
     if (A.skip && A.skip[i]) return;        // served by the tiled kernels
@@ -49,6 +66,12 @@ __device__ __forceinline__ void ref_particle(const DevGrid& g, int64_t n, const 
     const uint32_t key = T.sorted_key[i];
     const int cx = key % g.nc[0], cy = (key / g.nc[0]) % g.nc[1], cz = key / (g.nc[0] * g.nc[1]);
     const Span sx = cell_span(g, 0, cx, reach), sy = cell_span(g, 1, cy, reach), sz = cell_span(g, 2, cz, reach);
+    const double fcx = __dmul_rn(__dsub_rn(xa, g.lo[0]), g.inv[0]) - (double)cx;
+    const double fcy = __dmul_rn(__dsub_rn(ya, g.lo[1]), g.inv[1]) - (double)cy;
+    const double fcz = __dmul_rn(__dsub_rn(za, g.lo[2]), g.inv[2]) - (double)cz;
+    const double ex = 1.0 / g.inv[0], ey = 1.0 / g.inv[1], ez = 1.0 / g.inv[2];
+    const bool fullx = sx.cnt == g.nc[0] && g.per[0], fully = sy.cnt == g.nc[1] && g.per[1], fullz = sz.cnt == g.nc[2] && g.per[2];
+    const double reach2 = (reach * reach) * (1.0 + 1e-9);
 
     // per-particle constants
     const double hinv = 1.0 / ha;
@@ -71,10 +94,15 @@ __device__ __forceinline__ void ref_particle(const DevGrid& g, int64_t n, const 
 
     for (int kz = 0; kz < sz.cnt; ++kz) {
         const int czz = g.per[2] ? wrap_cell(sz.start + kz, g.nc[2]) : sz.start + kz;
+        const double gz2 = cell_gap2(sz.start + kz - cz, fcz, fullz, ez);
+        if (gz2 > reach2) continue;
         for (int ky = 0; ky < sy.cnt; ++ky) {
             const int cyy = g.per[1] ? wrap_cell(sy.start + ky, g.nc[1]) : sy.start + ky;
+            const double gyz2 = gz2 + cell_gap2(sy.start + ky - cy, fcy, fully, ey);
+            if (gyz2 > reach2) continue;
             for (int kx = 0; kx < sx.cnt; ++kx) {
                 const int cxx = g.per[0] ? wrap_cell(sx.start + kx, g.nc[0]) : sx.start + kx;
+                if (gyz2 + cell_gap2(sx.start + kx - cx, fcx, fullx, ex) > reach2) continue;
                 const uint32_t c = (uint32_t)((czz * g.nc[1] + cyy) * g.nc[0] + cxx);
                 const uint32_t jb = __ldg(T.cell_start + c), je = __ldg(T.cell_end + c);
                 for (uint32_t j = jb; j < je; ++j) {
