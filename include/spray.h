@@ -122,6 +122,20 @@ int spray_hydro_rhs(spray_ctx* ctx, const double* m, const double* rho, const do
                     const double* vx, const double* vy, const double* vz, const double* alpha, double beta,
                     double* ax, double* ay, double* az, double* dudt, double* divv_sum, void* stream);
 
+/* (a6) + (a7) in one sweep: the hydro right-hand sides of spray_hydro_rhs AND the flux-limiter pre-sweep of spray_fld_apply
+ * (P:L275 with grad E by eq. (9), phi = 1:  gradE_a = sum_{b in N_gather(a)} V_b (E_b - E_a) gradW(x_ab, h_a),  R_a = |gradE_a| /
+ * (rho_a kappa_a E_a),  lambda_a = 1/sqrt(9 + R_a^2),  mu_a = c lambda_a / (rho_a kappa_a)).  Both sums need rho and nothing of each
+ * other, and where h is uniform over a tile N_gather = N_sym, so the limiter's pair term reuses x_ab, 1/r and F/r of the hydro
+ * pair: results are BITWISE those of spray_hydro_rhs followed by spray_fld_apply(SPRAY_FLD_UPDATE_LIMITER)'s mu / gradE (same
+ * pair terms, same summation order; tiles with variable h and the particles of the general path run the two sweeps one after
+ * the other inside this call).  Follow it with spray_fld_apply(..., SPRAY_FLD_FROZEN, mu, ...) for y, Lambda, Gamma.
+ * Inputs [n] caller order as in the two calls; outputs ax, ay, az, dudt, mu [n]; divv_sum [n] and gradE [3n] nullable.
+ * Errors: SPRAY_ERR_INVALID_ARG (NULL). */
+int spray_hydro_rhs_limiter(spray_ctx* ctx, const double* m, const double* rho, const double* p, const double* cs,
+                            const double* vx, const double* vy, const double* vz, const double* alpha, double beta,
+                            const double* E, const double* kappa, double c_light,
+                            double* ax, double* ay, double* az, double* dudt, double* divv_sum, double* mu, double* gradE, void* stream);
+
 /* (a7)+(a8) matrix-free apply of the SPH flux-limited-diffusion operator.
  *   limiter pre-sweep (UPDATE_LIMITER only), P:L275 with grad E by eq. (9), phi = 1 (A19), over N_gather(a)\{a}:
  *       gradE_a = sum_b V_b (E_b - E_a) F(r;h_a) xhat_ab;   R = |gradE|/(rho kappa E);

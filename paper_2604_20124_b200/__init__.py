@@ -24,7 +24,7 @@ DEV_H_EXCEEDS_HMAX, DEV_OUTSIDE_BOX, DEV_LIST_OVERFLOW = 1, 2, 4
 
 # every symbol include/spray.h declares
 EXPORTS = ["spray_version", "spray_create", "spray_destroy", "spray_last_error", "spray_check", "spray_launch_count", "spray_set_path", "spray_path_stats",
-           "spray_build_cells", "spray_density", "spray_hydro_rhs", "spray_fld_apply", "spray_get_cell_table",
+           "spray_build_cells", "spray_density", "spray_hydro_rhs", "spray_hydro_rhs_limiter", "spray_fld_apply", "spray_get_cell_table",
            "spray_neighbor_counts", "spray_neighbor_lists", "spray_neighbor_digest", "spray_rad_jacobi", "spray_conduction", "spray_kgc_continuity", "spray_ray_deposit", "spray_conduction_implicit", "spray_fp64_peak_probe"]
 
 
@@ -64,6 +64,7 @@ def load():
     lib.spray_build_cells.argtypes = [vp, C.POINTER(Grid), i32, i64, vp, vp, vp, vp, vp]
     lib.spray_density.argtypes = [vp, vp, vp, vp, vp]
     lib.spray_hydro_rhs.argtypes = [vp] + [vp] * 8 + [dbl] + [vp] * 5 + [vp]
+    lib.spray_hydro_rhs_limiter.argtypes = [vp] + [vp] * 8 + [dbl] + [vp, vp, dbl] + [vp] * 7 + [vp]
     lib.spray_fld_apply.argtypes = [vp, vp, vp, vp, vp, dbl, i32, i32, vp, vp, vp, vp, vp, vp]
     lib.spray_conduction.argtypes = [vp, vp, vp, vp, vp, vp, vp]
     lib.spray_kgc_continuity.argtypes = [vp] * 10
@@ -190,6 +191,24 @@ class Spray:
         outs = [_ptr(t, f64, self.n) for t in out]
         self._ck(self.lib.spray_hydro_rhs(self.h, *ins, float(beta), *outs, _stream()), "spray_hydro_rhs")
         return out   # ax, ay, az, dudt, divv_sum
+
+    # -- spray_hydro_rhs_limiter
+    def hydro_rhs_limiter(self, m, rho, p, cs, vx, vy, vz, alpha, E, kappa, beta=2.0, c_light=1.0, out=None, mu=None, gradE=None,
+                          want_gradE=False):
+        """Hydro right-hand sides and the FLD limiter pre-sweep in one sweep (include/spray.h).
+        Returns ([ax, ay, az, dudt, divv_sum], mu, gradE or None)."""
+        f64 = self.torch.float64
+        if out is None:
+            out = [self._out(None) for _ in range(5)]
+        mu = self._out(mu)
+        if want_gradE:
+            gradE = self._out(gradE, n=3 * self.n)
+        ins = [_ptr(t, f64, self.n) for t in (m, rho, p, cs, vx, vy, vz, alpha)]
+        outs = [_ptr(t, f64, self.n) for t in out]
+        rc = self.lib.spray_hydro_rhs_limiter(self.h, *ins, float(beta), _ptr(E, f64, self.n), _ptr(kappa, f64, self.n), float(c_light),
+                                              *outs, _ptr(mu, f64, self.n), _ptr(gradE), _stream())
+        self._ck(rc, "spray_hydro_rhs_limiter")
+        return out, mu, gradE
 
     # -- spray_fld_apply
     def fld_apply(self, m, rho, kappa, E, c_light=1.0, kmode=FLD_SYMMETRIC, lmode=FLD_UPDATE_LIMITER, mu=None, y=None,

@@ -273,6 +273,45 @@ int spray_hydro_rhs(spray_ctx* ctx, const double* m, const double* rho, const do
     return SPRAY_OK;
 }
 
+int spray_hydro_rhs_limiter(spray_ctx* ctx, const double* m, const double* rho, const double* p, const double* cs,
+                            const double* vx, const double* vy, const double* vz, const double* alpha, double beta,
+                            const double* E, const double* kappa, double c_light,
+                            double* ax, double* ay, double* az, double* dudt, double* divv_sum, double* mu, double* gradE, void* stream) {
+    NEED_BUILT();
+    Ctx* c = &ctx->c;
+    if (c->n > 0 && (!m || !rho || !p || !cs || !vx || !vy || !vz || !alpha || !E || !kappa || !ax || !ay || !az || !dudt || !mu))
+        return fail(c, SPRAY_ERR_INVALID_ARG, "spray_hydro_rhs_limiter: NULL argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    double** f = c->s.f;
+    PrepJob pj{};
+    pj.m = m; pj.rho = rho; pj.p = p; pj.cs = cs; pj.vx = vx; pj.vy = vy; pj.vz = vz; pj.alpha = alpha;
+    pj.sm = f[F_M]; pj.srho = f[F_RHO]; pj.sp = f[F_P]; pj.scs = f[F_CS]; pj.svx = f[F_VX]; pj.svy = f[F_VY]; pj.svz = f[F_VZ];
+    pj.salpha = f[F_ALPHA]; pj.sV = f[F_V]; pj.sQ = f[F_Q]; pj.sAC = f[F_AC];
+    CK(launch_prep_hydro(c, pj, st), "hydro prologue");
+    PrepJob pl{};                     // limiter prologue; rho kappa goes to the (mu, E) record so that t0 stays the hydro's
+    pl.m = m; pl.rho = rho; pl.E = E; pl.kx = kappa; pl.kx_is_mu = 0; pl.rk_to_me = 1;
+    pl.sm = f[F_M]; pl.srho = f[F_RHO]; pl.sE = f[F_E]; pl.skx = f[F_KAPPA]; pl.sV = f[F_V];
+    CK(launch_prep_fld(c, pl, st), "limiter prologue");
+    if (c->tl.enabled) {
+        TiledArgs t{};
+        t.beta = beta; t.c_light = c_light;
+        t.o0 = ax; t.o1 = ay; t.o2 = az; t.o3 = dudt; t.o4 = divv_sum; t.o5 = mu; t.o6 = gradE;
+        CK(launch_tiled_sweep(c, SW_HYDLIM, t, st), "tiled hydro + limiter sweep");
+    }
+    SweepArgs a = fallback_args(c);
+    a.m = f[F_M]; a.rho = f[F_RHO]; a.p = f[F_P]; a.cs = f[F_CS];
+    a.vx = f[F_VX]; a.vy = f[F_VY]; a.vz = f[F_VZ]; a.alpha = f[F_ALPHA];
+    a.beta = beta;
+    a.o0 = ax; a.o1 = ay; a.o2 = az; a.o3 = dudt; a.o4 = divv_sum;
+    CK(launch_ref_sweep(c, SW_HYDRO, a, st), "hydro sweep");
+    SweepArgs l = fallback_args(c);
+    l.m = f[F_M]; l.rho = f[F_RHO]; l.E = f[F_E]; l.kappa = f[F_KAPPA]; l.mu = f[F_MU];
+    l.c_light = c_light;
+    l.o0 = mu; l.o1 = gradE; l.mu_sorted = f[F_MU]; l.me_sorted = c->pk.me;
+    CK(launch_ref_sweep(c, SW_LIMITER, l, st), "limiter sweep");
+    return SPRAY_OK;
+}
+
 int spray_fld_apply(spray_ctx* ctx, const double* m, const double* rho, const double* kappa, const double* E,
                     double c_light, spray_fld_kernel_mode_t kmode, spray_fld_limiter_mode_t lmode, double* mu, double* y,
                     double* diag, double* offd, double* gradE, void* stream) {

@@ -243,6 +243,7 @@ __global__ void k_prep_fld(PrepJob j, const uint32_t* __restrict__ perm, int64_t
     o.s0[i] = make_double2(o.p1[i].x, V);
     o.e1[i] = E;
     if (j.kx_is_mu) o.me[i] = make_double2(kx, E);
+    else if (j.rk_to_me) o.me[i] = make_double2(rho * kx, E);
     else o.t0[i] = make_double2(rho * kx, 0.0);
     if (!nfast || *nfast != (unsigned long long)n) {
         j.sm[i] = m; j.srho[i] = rho; j.sE[i] = E; j.skx[i] = kx;

@@ -15,7 +15,7 @@ struct DevGrid {
     int per[3];
 };
 
-enum SweepId { SW_DENSITY = 0, SW_HYDRO = 1, SW_LIMITER = 2, SW_APPLY = 3, SW_HSEARCH = 4, SW_COUNT = 5, SW_LIST = 6, SW_DIGEST = 7, SW_KGC = 8, SW_GRADN = 9 };
+enum SweepId { SW_DENSITY = 0, SW_HYDRO = 1, SW_LIMITER = 2, SW_APPLY = 3, SW_HSEARCH = 4, SW_COUNT = 5, SW_LIST = 6, SW_DIGEST = 7, SW_KGC = 8, SW_GRADN = 9, SW_HYDLIM = 10 };
 
 constexpr double kPi = 3.14159265358979323846264338327950288;
 constexpr double kSigmaCubic = 1.0 / kPi;            // M4 cubic spline, 3-D (A1)

@@ -110,6 +110,7 @@ struct PrepJob {
     const double *m, *rho, *p, *cs, *vx, *vy, *vz, *alpha, *E, *kx;   // caller order (kx = kappa or mu)
     double *sm, *srho, *sp, *scs, *svx, *svy, *svz, *salpha, *sE, *skx, *sV, *sQ, *sAC;   // sorted order (general kernels)
     int kx_is_mu;
+    int rk_to_me;               // limiter prologue of the fused hydro + limiter call: (rho kappa, E) goes to me[], t0 stays the hydro's
 };
 cudaError_t launch_prep_density(Ctx* c, const double* m, cudaStream_t st);
 cudaError_t launch_prep_hydro(Ctx* c, const PrepJob& j, cudaStream_t st);
@@ -121,6 +122,7 @@ struct TiledArgs {
     double beta, c_light;
     int fld_sym;
     double *o0, *o1, *o2, *o3, *o4;              // caller-order outputs
+    double *o5 = nullptr, *o6 = nullptr;         // SW_HYDLIM: mu, gradE
     uint32_t* ocount;
 };
 cudaError_t launch_build_tiles(Ctx* c, cudaStream_t st);

@@ -95,6 +95,9 @@ template <> struct NRec<SW_LIMITER> { static constexpr int v = 2, e = 1; };   //
 template <> struct NRec<SW_APPLY> { static constexpr int v = 4, e = 0; };     // (x,y) (z,V) (mu,E) (1/h,Fn)
 template <> struct NRec<SW_KGC> { static constexpr int v = 4, e = 0; };       // (x,y) (z,V) (vx,vy) (vz,-)
 template <> struct NRec<SW_GRADN> { static constexpr int v = 2, e = 1; };     // (x,y) (z,V) | f = n_e/n_c   (row N4)
+// hydro RHS + FLD limiter sum in one sweep (spray_hydro_rhs_limiter): the hydro records and the limiter's E.  Launched on
+// uniform-h tiles only (MODE 1: no (1/h,Fn) record, 5 records + E = 197 KB); there N_gather = N_sym, so both sums walk the same list.
+template <> struct NRec<SW_HYDLIM> { static constexpr int v = 6, e = 1; };    // (x,y) (z,V) (Q,vx) (vy,vz) (m,alpha c) (1/h,Fn) | E
 
 struct SweepIn {
     const double2* rec[6];           // sorted global records, in the order of NRec
@@ -102,7 +105,7 @@ struct SweepIn {
     const double2* p1;               // (z, h)
     const double2* hh;               // (1/h, Fn)
     const double2* t0;               // per-call target record
-    const double2* me;               // (mu, E)
+    const double2* me;               // (mu, E); limiter with rk_in_me: (rho kappa, E) on entry
     double2* me_out;                 // limiter: (mu, E) for the apply
     double2* g_out[2];               // SW_GRADN: (G_x, G_y), (G_z, kappa^ib) in sorted order for the ray kernel (ray.cu)
     double* mu_sorted;               // limiter: mu in sorted order for the general kernels
@@ -118,6 +121,8 @@ struct SweepIn {
     double beta, c_light;
     int fld_sym;
     double *o0, *o1, *o2, *o3, *o4;
+    double *o5, *o6;                 // SW_HYDLIM: mu, gradE (nullable)
+    int rk_in_me;                    // limiter epilogue reads rho_a kappa_a from me[i].x instead of t0[i].x
     uint32_t* ocount;
 };
 
@@ -128,6 +133,7 @@ struct Acc {
 struct Tgt {                         // per-target constants
     double x, y, z, hinv, fn;
     double c0, c1, c2, c3, c4, c5;   // per sweep (see k_tiled_sweep)
+    double e;                        // SW_HYDLIM: E_a
 };
 
 // One pair (target, slot s).  F = staged records ([record][TILE_CMAXP] double2), Ee = staged E (limiter).
@@ -220,10 +226,11 @@ __device__ __forceinline__ void pair_body(const double2* __restrict__ F, const d
 // Hydro pairs in groups: the branch-free part of every pair of the group first (so the compiler can interleave
 // their dependency chains), then ONE branch for the group's viscous corrections (taken only if some pair approaches),
 // then the accumulations.  Same arithmetic as pair_body<SW_HYDRO>.
-struct HydroPair { double dx, dy, dz, y, r, Ga, Gb, c, vr, Vb; uint32_t s; };
+struct HydroPair { double dx, dy, dz, y, r, Ga, Gb, c, vr, Vb, dE; uint32_t s; };
 
-template <int KERNEL, bool UNI>
-__device__ __forceinline__ void hydro_common(const double2* __restrict__ F, uint32_t s, const Tgt& T, HydroPair& h) {
+template <int KERNEL, bool UNI, bool LIM>
+__device__ __forceinline__ void hydro_common(const double2* __restrict__ F, const double* __restrict__ Ee, uint32_t s, const Tgt& T, HydroPair& h) {
+    if (LIM) h.dE = Ee[s] - T.e;
     const double2 d0 = F[s], d1 = F[TILE_CMAXP + s];
     const double2 d2 = F[2 * TILE_CMAXP + s], d3 = F[3 * TILE_CMAXP + s];
     h.s = s;
@@ -256,23 +263,27 @@ __device__ __forceinline__ void hydro_visc(const double2* __restrict__ F, const 
     else h.c = fma(-hw, fma((d4.x * T.c1) * vsa, h.Ga, (h.Vb * vsb) * h.Gb), h.c);
     acc.a4 = fma((hw * w) * (d4.x * vsa), h.Ga * h.r, acc.a4);
 }
-template <bool UNI>
+template <bool UNI, bool LIM>
 __device__ __forceinline__ void hydro_accum(const HydroPair& h, Acc& acc) {
     const double cg = UNI ? h.c * h.Ga : h.c;
     acc.a0 = fma(cg, h.dx, acc.a0); acc.a1 = fma(cg, h.dy, acc.a1); acc.a2 = fma(cg, h.dz, acc.a2);
     acc.a3 = fma(h.Vb * h.Ga, h.vr, acc.a3);                             // eq. (37)
+    if (LIM) {                           // eq. (9) phi = 1 with f = E: the pair term of pair_body<SW_LIMITER>, same order (uniform h)
+        const double cc = (h.Vb * h.dE) * h.Ga;
+        acc.k[0] = fma(cc, h.dx, acc.k[0]); acc.k[1] = fma(cc, h.dy, acc.k[1]); acc.k[2] = fma(cc, h.dz, acc.k[2]);
+    }
 }
-template <int KERNEL, bool UNI>
-__device__ __forceinline__ void hydro_group2(const double2* __restrict__ F, uint32_t s0, uint32_t s1, const Tgt& T, double beta, Acc& acc) {
+template <int KERNEL, bool UNI, bool LIM>
+__device__ __forceinline__ void hydro_group2(const double2* __restrict__ F, const double* __restrict__ Ee, uint32_t s0, uint32_t s1, const Tgt& T, double beta, Acc& acc) {
     HydroPair h0, h1;
-    hydro_common<KERNEL, UNI>(F, s0, T, h0);
-    hydro_common<KERNEL, UNI>(F, s1, T, h1);
+    hydro_common<KERNEL, UNI, LIM>(F, Ee, s0, T, h0);
+    hydro_common<KERNEL, UNI, LIM>(F, Ee, s1, T, h1);
     if (fmin(h0.vr, h1.vr) < 0.0) {
         if (h0.vr < 0.0) hydro_visc<UNI>(F, T, beta, h0, acc);
         if (h1.vr < 0.0) hydro_visc<UNI>(F, T, beta, h1, acc);
     }
-    hydro_accum<UNI>(h0, acc);
-    hydro_accum<UNI>(h1, acc);
+    hydro_accum<UNI, LIM>(h0, acc);
+    hydro_accum<UNI, LIM>(h1, acc);
 }
 
 template <int SWEEP, int KERNEL, bool UNI>
@@ -295,9 +306,9 @@ __device__ __forceinline__ void pair_loop(const double2* __restrict__ F, const d
     for (uint32_t r4 = 0; r4 < R; r4 += 4) {
         const uint2 nx3 = (r4 + 12 < R) ? __ldcs(lp + (size_t)(r4 / 4 + 3) * 32) : make_uint2(0u, 0u);
         const uint32_t sn = nxt.x & 0xFFFFu;
-        if (SWEEP == SW_HYDRO) {
-            hydro_group2<KERNEL, UNI>(F, cur.x & 0xFFFFu, cur.x >> 16, T, beta, acc);
-            hydro_group2<KERNEL, UNI>(F, cur.y & 0xFFFFu, cur.y >> 16, T, beta, acc);
+        if (SWEEP == SW_HYDRO || SWEEP == SW_HYDLIM) {
+            hydro_group2<KERNEL, UNI, SWEEP == SW_HYDLIM>(F, Ee, cur.x & 0xFFFFu, cur.x >> 16, T, beta, acc);
+            hydro_group2<KERNEL, UNI, SWEEP == SW_HYDLIM>(F, Ee, cur.y & 0xFFFFu, cur.y >> 16, T, beta, acc);
         } else {
             if (PIPE_FIRST) {
                 pair_body<SWEEP, KERNEL, UNI>(F, Ee, cur.x & 0xFFFFu, q0, q1, T, beta, sym, acc);
@@ -315,7 +326,9 @@ __device__ __forceinline__ void pair_loop(const double2* __restrict__ F, const d
 
 // MODE 0: every tile.  MODE 1: only the tiles with uniform h, whose pair bodies never read the (1/h, Fn) record -- the
 // apply then needs 3 records per candidate, 105 KB, and two CTAs fit an SM.  MODE 2: only the other tiles.
-template <int SWEEP, int MODE> struct NRecM { static constexpr int v = (SWEEP == SW_APPLY && MODE == 1) ? 3 : NRec<SWEEP>::v; };
+template <int SWEEP, int MODE> struct NRecM {
+    static constexpr int v = (SWEEP == SW_APPLY && MODE == 1) ? 3 : ((SWEEP == SW_HYDLIM && MODE == 1) ? 5 : NRec<SWEEP>::v);
+};
 template <int SWEEP, int MODE> struct MinBlocks {
     static constexpr int v = (SWEEP == SW_DENSITY || SWEEP == SW_LIMITER || SWEEP == SW_GRADN || (SWEEP == SW_APPLY && MODE == 1)) ? 2 : 1;
 };
@@ -331,7 +344,8 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int u = tid & 1, tgt = tid >> 1;
     const uint32_t ntiles = (uint32_t)A.ctr[CTR_NTILES];
-    const bool sym = (SWEEP == SW_HYDRO) || (SWEEP == SW_APPLY && A.fld_sym != 0);
+    constexpr bool HYD = SWEEP == SW_HYDRO || SWEEP == SW_HYDLIM;
+    const bool sym = HYD || (SWEEP == SW_APPLY && A.fld_sym != 0);
     // dummy slots: far away, every weight zero, so that a padded list entry adds exactly nothing
     if (tid < TILE_NDUMMY) {
         const double far = g.lo[0] - 1.0e4 * g.L[0];
@@ -367,7 +381,7 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
         __syncthreads();
         // ---- this thread's target.  Except in the hydro kernel (register pressure: measured slower) its loads go out before
         //      the staging traffic, so they are back when the pair loop starts.
-        constexpr bool EARLY_TARGET = SWEEP != SW_HYDRO;
+        constexpr bool EARLY_TARGET = !HYD;
         const bool active = half_ok && tgt < (int)td.nt;
         uint32_t i = 0, ia = 0;
         Tgt T{};
@@ -378,7 +392,8 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
             const double2 xy = A.rec[0][i], zh = A.p1[i], hv = A.hh[i];
             T.x = xy.x; T.y = xy.y; T.z = zh.x; T.hinv = hv.x; T.fn = hv.y;
             if (SWEEP == SW_DENSITY) T.c0 = A.rec[1][i].y;                                   // m_a
-            if (SWEEP == SW_HYDRO) {
+            if (SWEEP == SW_HYDLIM) T.e = A.e1[i];                                           // E_a
+            if (HYD) {
                 const double2 t0 = A.t0[i], q1 = A.rec[2][i], q2 = A.rec[3][i];
                 T.c0 = t0.x; T.c1 = t0.y;                                                    // p_a/rho_a, 1/rho_a
                 T.c2 = A.rec[4][i].y;                                                        // alpha_a c_a
@@ -404,7 +419,7 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
                 for (uint32_t k = lane; k < len; k += 32) {
 #pragma unroll
                     for (int v = 0; v < NV; ++v) {
-                        if (uni && ((SWEEP == SW_HYDRO && v == 5) || (SWEEP == SW_APPLY && v == 3))) continue;
+                        if (uni && ((HYD && v == 5) || (SWEEP == SW_APPLY && v == 3))) continue;
                         cp_async16(&F[v * TILE_CMAXP + base + k], &A.rec[v][vs + k]);
                     }
                     if (NRec<SWEEP>::e) cp_async8(&Ee[base + k], &A.e1[vs + k]);
@@ -414,7 +429,7 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
                 for (uint32_t k = lane; k < len; k += 32) {
 #pragma unroll
                     for (int v = 0; v < NV; ++v) {
-                        if (uni && ((SWEEP == SW_HYDRO && v == 5) || (SWEEP == SW_APPLY && v == 3))) continue;
+                        if (uni && ((HYD && v == 5) || (SWEEP == SW_APPLY && v == 3))) continue;
                         double2 val = A.rec[v][vs + k];
                         if (v == 0) { val.x -= shx; val.y -= shy; }
                         if (v == 1) val.x -= shz;
@@ -435,8 +450,12 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
         // ---- add the two half-lists of the target
         acc.a0 += __shfl_xor_sync(0xFFFFFFFFu, acc.a0, 1);
         if (SWEEP != SW_DENSITY) acc.a1 += __shfl_xor_sync(0xFFFFFFFFu, acc.a1, 1);
-        if (SWEEP == SW_HYDRO || SWEEP == SW_LIMITER || SWEEP == SW_GRADN) acc.a2 += __shfl_xor_sync(0xFFFFFFFFu, acc.a2, 1);
-        if (SWEEP == SW_HYDRO) {
+        if (HYD || SWEEP == SW_LIMITER || SWEEP == SW_GRADN) acc.a2 += __shfl_xor_sync(0xFFFFFFFFu, acc.a2, 1);
+        if (SWEEP == SW_HYDLIM) {
+#pragma unroll
+            for (int e = 0; e < 3; ++e) acc.k[e] += __shfl_xor_sync(0xFFFFFFFFu, acc.k[e], 1);
+        }
+        if (HYD) {
             acc.a3 += __shfl_xor_sync(0xFFFFFFFFu, acc.a3, 1);
             acc.a4 += __shfl_xor_sync(0xFFFFFFFFu, acc.a4, 1);
         }
@@ -452,15 +471,27 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
                 const double wn = wn_k<KERNEL>() * (T.hinv * T.hinv) * T.hinv;
                 A.o0[ia] = wn * fma(T.c0, w0_k<KERNEL>(), acc.a0);
                 if (A.ocount) A.ocount[ia] = A.lcount[(size_t)tile * TILE_T + tgt] & 0xFFFFu;
-            } else if (SWEEP == SW_HYDRO) {
+            } else if (HYD) {
                 A.o0[ia] = -(sc * acc.a0); A.o1[ia] = -(sc * acc.a1); A.o2[ia] = -(sc * acc.a2);
                 const double D = sc * acc.a3;
                 A.o3[ia] = T.c0 * D - (sc * acc.a4) * T.c1;      // eq. (17) 1st term P:L129 + eq. (42)
                 if (A.o4) A.o4[ia] = D;
+                if (SWEEP == SW_HYDLIM) {
+                    // the limiter epilogue of SW_LIMITER below, on the sums of the same pair terms
+                    const double gx = T.fn * acc.k[0], gy = T.fn * acc.k[1], gz = T.fn * acc.k[2];
+                    const double rk = A.me[i].x;                 // rho_a kappa_a (k_prep_fld, rk_to_me)
+                    const double gn = sqrt(gx * gx + gy * gy + gz * gz);
+                    const double Rl = gn / (rk * T.e);
+                    const double mu = A.c_light * (1.0 / sqrt(9.0 + Rl * Rl)) / rk;
+                    A.o5[ia] = mu;
+                    A.me_out[i] = make_double2(mu, T.e);
+                    A.mu_sorted[i] = mu;
+                    if (A.o6) { A.o6[ia] = gx; A.o6[A.n + ia] = gy; A.o6[2 * A.n + ia] = gz; }
+                }
             } else if (SWEEP == SW_LIMITER) {
                 // Larsen limiter, k = 2 (A20); the limiter sum always carries kFn/h_a^4 outside
                 const double gx = T.fn * acc.a0, gy = T.fn * acc.a1, gz = T.fn * acc.a2;
-                const double rk = A.t0[i].x;                     // rho_a kappa_a
+                const double rk = A.rk_in_me ? A.me[i].x : A.t0[i].x;   // rho_a kappa_a
                 const double gn = sqrt(gx * gx + gy * gy + gz * gz);
                 const double Rl = gn / (rk * T.c0);
                 const double mu = A.c_light * (1.0 / sqrt(9.0 + Rl * Rl)) / rk;
@@ -529,6 +560,13 @@ static cudaError_t launch_t(Ctx* c, const SweepIn& a, cudaStream_t st) {
     if constexpr (SWEEP == SW_APPLY) {          // uniform-h tiles at two CTAs per SM, then whatever is left
         cudaError_t e = launch_m<SWEEP, 1>(c, a, st);
         return e != cudaSuccess ? e : launch_m<SWEEP, 2>(c, a, st);
+    } else if constexpr (SWEEP == SW_HYDLIM) {  // fused sweep on the uniform-h tiles; the other tiles run the two sweeps one after the other
+        cudaError_t e = launch_m<SW_HYDLIM, 1>(c, a, st);
+        if (e == cudaSuccess) e = launch_m<SW_HYDRO, 2>(c, a, st);
+        if (e != cudaSuccess) return e;
+        SweepIn l = a;                          // limiter view of the same job: its outputs are o0 (mu), o1 (gradE)
+        l.o0 = a.o5; l.o1 = a.o6; l.rk_in_me = 1;
+        return launch_m<SW_LIMITER, 2>(c, l, st);
     } else {
         return launch_m<SWEEP, 0>(c, a, st);
     }
@@ -542,7 +580,7 @@ cudaError_t launch_tiled_sweep(Ctx* c, int sweep, const TiledArgs& t, cudaStream
     a.perm = c->perm; a.tiles = c->tl.tiles; a.tiletab = c->tl.tiletab; a.ctr = c->tl.ctr; a.pool = c->tl.pool; a.winfo = c->tl.winfo;
     a.lcount = c->tl.lcount; a.tflags = c->tl.tflags; a.n = c->n;
     a.beta = t.beta; a.c_light = t.c_light; a.fld_sym = t.fld_sym;
-    a.o0 = t.o0; a.o1 = t.o1; a.o2 = t.o2; a.o3 = t.o3; a.o4 = t.o4; a.ocount = t.ocount;
+    a.o0 = t.o0; a.o1 = t.o1; a.o2 = t.o2; a.o3 = t.o3; a.o4 = t.o4; a.o5 = t.o5; a.o6 = t.o6; a.ocount = t.ocount;
     a.rec[0] = pk.p0; a.rec[1] = pk.s[0];
     switch (sweep) {
         case SW_DENSITY: return launch_t<SW_DENSITY>(c, a, st);
@@ -550,6 +588,9 @@ cudaError_t launch_tiled_sweep(Ctx* c, int sweep, const TiledArgs& t, cudaStream
             a.rec[2] = pk.s[1]; a.rec[3] = pk.s[2]; a.rec[4] = pk.s[3]; a.rec[5] = pk.hh;
             return launch_t<SW_HYDRO>(c, a, st);
         case SW_LIMITER: return launch_t<SW_LIMITER>(c, a, st);
+        case SW_HYDLIM:
+            a.rec[2] = pk.s[1]; a.rec[3] = pk.s[2]; a.rec[4] = pk.s[3]; a.rec[5] = pk.hh;
+            return launch_t<SW_HYDLIM>(c, a, st);
         case SW_GRADN:
             a.g_out[0] = pk.s[1]; a.g_out[1] = pk.s[2];
             return launch_t<SW_GRADN>(c, a, st);
