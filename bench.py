@@ -3,8 +3,10 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c5] [--impl ours|reference]
 
-A step = one pass of the whole hot path: spray_build_cells -> spray_density -> spray_hydro_rhs
--> spray_fld_apply(UPDATE_LIMITER) over one synthetic particle set (BASELINE.json configs, workloads/).
+A step = one pass of the whole hot path over one synthetic particle set (BASELINE.json configs, workloads/):
+spray_build_cells -> spray_density -> spray_hydro_rhs_limiter (hydro right-hand sides + limiter pre-sweep in one sweep) ->
+spray_fld_apply(FROZEN) (operator apply); --separate-calls runs spray_hydro_rhs -> spray_fld_apply(UPDATE_LIMITER) instead
+(the same outputs bit for bit, tests/test_gpu_fused.py).
 `value` = pair interactions per second with inputs resident in HBM; `e2e` = the same through the C-ABI with pinned
 HOST buffers (H2D of every input and D2H of every output inside the timed region).  Multi-GPU: the path does not
 shard (BASELINE.json: one GPU, no collectives) -> N independent replicas, "weak" scaling, no data-path collective.
@@ -158,6 +160,9 @@ def main():
     ap.add_argument("--cpu-sample", type=int, default=200000, help="target particles per oracle step (cpu_baseline / reference arm)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--separate-calls", action="store_true",
+                    help="pass = build, density, spray_hydro_rhs, spray_fld_apply(UPDATE_LIMITER) (two sweeps) instead of the default "
+                         "build, density, spray_hydro_rhs_limiter (hydro + limiter in one sweep), spray_fld_apply(FROZEN): same outputs, bitwise")
     ap.add_argument("--no-n1", action="store_true", help="skip the row-N1/N3 measurements (spray_rad_jacobi iterations, spray_kgc_continuity)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
@@ -197,15 +202,27 @@ def main():
     out = {k: torch.empty(n, dtype=f64, device=dev) for k in ("rho", "ax", "ay", "az", "dudt", "divv", "mu", "y", "diag", "offd")}
     hout = {k: torch.empty(n, dtype=f64).pin_memory() for k in out}
 
+    fused = not args.separate_calls
+
+    def hydro_and_fld(src, o, between=None):
+        """rows (a6)-(a8): hydro right-hand sides, limiter pre-sweep, operator apply -- as two calls either way"""
+        hy = [o["ax"], o["ay"], o["az"], o["dudt"], o["divv"]]
+        if fused:
+            sp.hydro_rhs_limiter(src["m"], o["rho"], src["p"], src["cs"], src["vx"], src["vy"], src["vz"], src["alpha"], src["E"], src["kappa"],
+                                 beta=w.beta, c_light=w.c_light, out=hy, mu=o["mu"])
+            if between: between()
+            sp.fld_apply(src["m"], o["rho"], None, src["E"], w.c_light, lmode=P.FLD_FROZEN, mu=o["mu"], y=o["y"], diag=o["diag"], offd=o["offd"])
+        else:
+            sp.hydro_rhs(src["m"], o["rho"], src["p"], src["cs"], src["vx"], src["vy"], src["vz"], src["alpha"], w.beta, out=hy)
+            if between: between()
+            sp.fld_apply(src["m"], o["rho"], src["kappa"], src["E"], w.c_light, mu=o["mu"], y=o["y"], diag=o["diag"], offd=o["offd"])
+
     def one_pass(src, ev=None):
         sp.build_cells(w.grid, w.kernel, src["x"], src["y"], src["z"], src["h"])
         if ev: ev[1].record()
         sp.density(src["m"], rho=out["rho"])
         if ev: ev[2].record()
-        sp.hydro_rhs(src["m"], out["rho"], src["p"], src["cs"], src["vx"], src["vy"], src["vz"], src["alpha"], w.beta,
-                     out=[out["ax"], out["ay"], out["az"], out["dudt"], out["divv"]])
-        if ev: ev[3].record()
-        sp.fld_apply(src["m"], out["rho"], src["kappa"], src["E"], w.c_light, mu=out["mu"], y=out["y"], diag=out["diag"], offd=out["offd"])
+        hydro_and_fld(src, out, (lambda: ev[3].record()) if ev else None)
         if ev: ev[4].record()
 
     def barrier():
@@ -250,8 +267,12 @@ def main():
         # Every byte still crosses PCIe inside the timed region, every step.
         main = torch.cuda.current_stream()
         s_in, s_out = torch.cuda.Stream(), torch.cuda.Stream()
-        groups = [("x", "y", "z", "h"), ("m",), ("p", "cs", "vx", "vy", "vz", "alpha"), ("E", "kappa")]
-        outs = [(), ("rho",), ("ax", "ay", "az", "dudt", "divv"), ("mu", "y", "diag", "offd")]
+        if fused:
+            groups = [("x", "y", "z", "h"), ("m",), ("p", "cs", "vx", "vy", "vz", "alpha", "E", "kappa"), ()]
+            outs = [(), ("rho",), ("ax", "ay", "az", "dudt", "divv", "mu"), ("y", "diag", "offd")]
+        else:
+            groups = [("x", "y", "z", "h"), ("m",), ("p", "cs", "vx", "vy", "vz", "alpha"), ("E", "kappa")]
+            outs = [(), ("rho",), ("ax", "ay", "az", "dudt", "divv"), ("mu", "y", "diag", "offd")]
         dbuf = [d, {f: torch.empty_like(d[f]) for f in fields}]
         obuf = [out, {o: torch.empty_like(out[o]) for o in out}]
         in_free = [torch.cuda.Event(), torch.cuda.Event()]     # kernels of the step that last read dbuf[b] are done
@@ -281,11 +302,11 @@ def main():
             sp.density(dd["m"], rho=oo["rho"])
             done(1)
             main.wait_event(ev_in[2])
-            sp.hydro_rhs(dd["m"], oo["rho"], dd["p"], dd["cs"], dd["vx"], dd["vy"], dd["vz"], dd["alpha"], w.beta,
-                         out=[oo["ax"], oo["ay"], oo["az"], oo["dudt"], oo["divv"]])
-            done(2)
-            main.wait_event(ev_in[3])
-            sp.fld_apply(dd["m"], oo["rho"], dd["kappa"], dd["E"], w.c_light, mu=oo["mu"], y=oo["y"], diag=oo["diag"], offd=oo["offd"])
+
+            def between():
+                done(2)
+                main.wait_event(ev_in[3])
+            hydro_and_fld(dd, oo, between)
             done(3)
             in_free[b].record(main)
             out_free[b].record(s_out)
@@ -455,11 +476,16 @@ def main():
     t_alu = sum(flops.values()) / (fp64_meas * 1e12)
     t_hbm = BYTES_PER_PARTICLE * n / (pk["hbm_gbs"] * 1e9)
     calls = {"build": seg_mean[0], "density": seg_mean[1], "hydro": seg_mean[2], "fld": seg_mean[3]}
-    hydro_tflops = flops["hydro"] / calls["hydro"] / 1e12
+    # dominant kernel: the hydro sweep; in the default pass it also carries the limiter sums, so its algorithmic work is both rows
+    hyd_flops = flops["hydro"] + (flops["limiter"] if fused else 0.0)
+    fld_flops = flops["apply"] + (0.0 if fused else flops["limiter"])
+    hydro_tflops = hyd_flops / calls["hydro"] / 1e12
     # dram__bytes_read.sum + dram__bytes_write.sum of k_tiled_sweep<1,0> per launch at c5, one ncu --set full capture
     # (profiles/r01d_ncu_full_tiled_path.md); null for other workloads
     traffic = 6.01e9 + 0.67e9 if w.name.startswith("c5") else None
-    roofline = {"bound": "alu", "kernel": "hydro pair sweep (spray_hydro_rhs: prologue k_prep_hydro + k_tiled_sweep<1>)",
+    kname = ("hydro + limiter pair sweep (spray_hydro_rhs_limiter: prologues k_prep_hydro, k_prep_fld + k_tiled_sweep<10>; algorithmic flops of rows a6 + a7)"
+             if fused else "hydro pair sweep (spray_hydro_rhs: prologue k_prep_hydro + k_tiled_sweep<1>)")
+    roofline = {"bound": "alu", "kernel": kname,
                 "achieved": hydro_tflops, "peak": fp64_meas, "unit": "TFLOP/s", "frac": hydro_tflops / fp64_meas,
                 "peak_source": "DFMA-chain probe measured in this run (spray_fp64_peak_probe); nominal 148x64x2x1.965GHz = %.1f" % FP64_NOMINAL_TFLOPS,
                 "traffic": traffic,
@@ -467,7 +493,9 @@ def main():
                          "t_pass_ms": 1e3 * t_step, "frac": max(t_alu, t_hbm) / t_step, "hbm_peak_gbs": pk["hbm_gbs"], "hbm_peak_source": pk_src},
                 "per_call_ms": {k: 1e3 * float(v) for k, v in calls.items()},
                 "per_call_tflops": {"density": flops["density"] / calls["density"] / 1e12, "hydro": hydro_tflops,
-                                    "fld": (flops["limiter"] + flops["apply"]) / calls["fld"] / 1e12}}
+                                    "fld": fld_flops / calls["fld"] / 1e12},
+                "calls": (["spray_build_cells", "spray_density", "spray_hydro_rhs_limiter", "spray_fld_apply(FROZEN)"] if fused else
+                          ["spray_build_cells", "spray_density", "spray_hydro_rhs", "spray_fld_apply(UPDATE_LIMITER)"])}
 
     cpu = None
     if not args.no_cpu_baseline:
