@@ -40,14 +40,14 @@ struct Tiled {
     int64_t bundle_cap = 0;
     uint2* pool = nullptr;       // list storage: per (tile, warp) a fixed block of LIST_RMAX/4 x 32 lanes x (4 u16 slots)
     int64_t pool_cap = 0;        // in uint2 units
-    unsigned long long* ctr = nullptr;   // [CTR_NFAST] particles served by the tiled kernels, [CTR_NTILES] tiles
+    unsigned long long* ctr = nullptr;   // [CTR_NFAST] particles served by the tiled kernels, [CTR_NTILES] tiles, [CTR_NNONUNI]
     uint2* winfo = nullptr;      // [tile_cap][TILE_WARPS]: (pool offset, rounds)
     uint32_t* lcount = nullptr;  // [tile_cap][TILE_T]: n_gather | n_sym << 16
     uint32_t* tflags = nullptr;  // [tile_cap]: TILE_FLAG_*
     uint32_t* tiletab = nullptr; // [tile_cap][TILES_WORDS]: per-tile TileS tables
     uint8_t* fast = nullptr;     // [n_max] sorted order: 1 = particle is served by the tiled kernels
 };
-enum { CTR_NFAST = 1, CTR_NTILES = 2, CTR_COUNT = 4 };
+enum { CTR_NFAST = 1, CTR_NTILES = 2, CTR_NNONUNI = 3, CTR_COUNT = 4 };   // CTR_NNONUNI: half-tile units that found non-uniform h
 
 struct Ctx {
     int device = 0;

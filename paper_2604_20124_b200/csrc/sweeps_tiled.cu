@@ -344,6 +344,7 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int u = tid & 1, tgt = tid >> 1;
     const uint32_t ntiles = (uint32_t)A.ctr[CTR_NTILES];
+    if (MODE == 2 && A.ctr[CTR_NNONUNI] == 0) return;          // no tile with variable h (the usual case): nothing for this launch
     constexpr bool HYD = SWEEP == SW_HYDRO || SWEEP == SW_HYDLIM;
     const bool sym = HYD || (SWEEP == SW_APPLY && A.fld_sym != 0);
     // dummy slots: far away, every weight zero, so that a padded list entry adds exactly nothing

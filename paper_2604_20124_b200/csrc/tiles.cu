@@ -564,6 +564,7 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
         if (tid == 0) {
             const uint32_t bits = (bad ? 0u : (TILE_FLAG_OK0 << half)) | (s_nonuni ? TILE_FLAG_NONUNI : 0u);
             if (bits) atomicOr(&A.tflags[tile], bits);
+            if (s_nonuni) atomicAdd(&A.ctr[CTR_NNONUNI], 1ull);
             if (!bad) atomicAdd(&A.ctr[CTR_NFAST], (unsigned long long)min((int)td.nt - half * BL_TGT, BL_TGT));
         }
     }
