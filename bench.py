@@ -482,7 +482,8 @@ def main():
     hydro_tflops = hyd_flops / calls["hydro"] / 1e12
     # dram__bytes_read.sum + dram__bytes_write.sum of k_tiled_sweep<1,0> per launch at c5, one ncu --set full capture
     # (profiles/r01d_ncu_full_tiled_path.md); null for other workloads
-    traffic = 6.01e9 + 0.67e9 if w.name.startswith("c5") else None
+    # (fused sweep k_tiled_sweep<10,0,1>: profiles/r01h_ncu_full_fused_pass.md)
+    traffic = ((6.87e9 + 1.20e9) if fused else (6.01e9 + 0.67e9)) if w.name.startswith("c5") else None
     kname = ("hydro + limiter pair sweep (spray_hydro_rhs_limiter: prologues k_prep_hydro, k_prep_fld + k_tiled_sweep<10>; algorithmic flops of rows a6 + a7)"
              if fused else "hydro pair sweep (spray_hydro_rhs: prologue k_prep_hydro + k_tiled_sweep<1>)")
     roofline = {"bound": "alu", "kernel": kname,
