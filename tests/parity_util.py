@@ -73,6 +73,12 @@ def gpu_isolated(sp, d, w, targets=None, mu_in=None, kmode=0):
     rho, nn = sp.density(d["m"], want_nnbr=True)
     ax, ay, az, dudt, divv = sp.hydro_rhs(d["m"], d["rho_nom"], d["p"], d["cs"], d["vx"], d["vy"], d["vz"], d["alpha"], w.beta)
     up = sp.fld_apply(d["m"], d["rho_nom"], d["kappa"], d["E"], w.c_light, kmode=kmode, lmode=0, want_gradE=True)
+    # spray_hydro_rhs_limiter promises the results of the two calls above bit for bit, on every path and particle set
+    fy, fmu, fg = sp.hydro_rhs_limiter(d["m"], d["rho_nom"], d["p"], d["cs"], d["vx"], d["vy"], d["vz"], d["alpha"], d["E"], d["kappa"],
+                                       beta=w.beta, c_light=w.c_light, want_gradE=True)
+    for k, a, b in zip(("ax", "ay", "az", "dudt", "divv"), (ax, ay, az, dudt, divv), fy):
+        assert torch.equal(a, b), "fused " + k
+    assert torch.equal(up["mu"], fmu) and torch.equal(up["gradE"], fg), "fused limiter"
     out = dict(rho=rho, nnbr=nn, ax=ax, ay=ay, az=az, dudt=dudt, divv=divv, mu=up["mu"], y_upd=up["y"],
                gradE=up["gradE"])
     if mu_in is not None:

@@ -38,6 +38,8 @@ def test_error_codes():
     x = torch.linspace(0.05, 0.95, 10, dtype=torch.float64, device="cuda")
     sp.build_cells(g, 0, x, x, x, h)
     assert sp.density(h).shape[0] == 10
+    with pytest.raises(P.SprayError, match=r"\(-1\)"):          # INVALID_ARG: NULL input of the fused call
+        sp.hydro_rhs_limiter(h, h, h, h, h, h, h, h, None, h)
     assert sp.check() == 0
 
 
@@ -66,6 +68,7 @@ def test_empty_and_single_particle(path):
     assert sp.density(e).numel() == 0
     assert len(sp.hydro_rhs(e, e, e, e, e, e, e, e)) == 5
     assert sp.fld_apply(e, e, e, e)["y"].numel() == 0
+    assert sp.hydro_rhs_limiter(e, e, e, e, e, e, e, e, e, e)[1].numel() == 0
     t = sp.get_cell_table()
     assert (u32(t["cell_start"]) == 0).all() and (u32(t["cell_end"]) == 0).all()
     one = torch.tensor([0.4], dtype=torch.float64, device="cuda")
@@ -81,6 +84,8 @@ def test_empty_and_single_particle(path):
         fl = sp.fld_apply(m, m, m, m)
         assert float(fl["y"][0]) == 0.0 and float(fl["diag"][0]) == 0.0
         assert float(fl["mu"][0]) == pytest.approx(1.0 / 3.0 / 4.0, rel=1e-15)      # R = 0: lambda = 1/3, mu = c/(3 rho kappa)
+        fy, fmu, _ = sp.hydro_rhs_limiter(m, m, m, m, m, m, m, m, m, m)
+        assert all(float(t[0]) == 0.0 for t in fy) and float(fmu[0]) == float(fl["mu"][0])
         # next rows on one particle: no neighbour, so no conduction, L = I (A28) and no density change
         assert float(sp.conduction(m, m, m, m)[0]) == 0.0
         kg = sp.kgc_continuity(m, m, m, m, m)
