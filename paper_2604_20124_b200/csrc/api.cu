@@ -287,11 +287,9 @@ int spray_hydro_rhs_limiter(spray_ctx* ctx, const double* m, const double* rho, 
     pj.m = m; pj.rho = rho; pj.p = p; pj.cs = cs; pj.vx = vx; pj.vy = vy; pj.vz = vz; pj.alpha = alpha;
     pj.sm = f[F_M]; pj.srho = f[F_RHO]; pj.sp = f[F_P]; pj.scs = f[F_CS]; pj.svx = f[F_VX]; pj.svy = f[F_VY]; pj.svz = f[F_VZ];
     pj.salpha = f[F_ALPHA]; pj.sV = f[F_V]; pj.sQ = f[F_Q]; pj.sAC = f[F_AC];
-    CK(launch_prep_hydro(c, pj, st), "hydro prologue");
-    PrepJob pl{};                     // limiter prologue; rho kappa goes to the (mu, E) record so that t0 stays the hydro's
-    pl.m = m; pl.rho = rho; pl.E = E; pl.kx = kappa; pl.kx_is_mu = 0; pl.rk_to_me = 1;
-    pl.sm = f[F_M]; pl.srho = f[F_RHO]; pl.sE = f[F_E]; pl.skx = f[F_KAPPA]; pl.sV = f[F_V];
-    CK(launch_prep_fld(c, pl, st), "limiter prologue");
+    // the limiter's prologue rides along: E, and rho kappa parked in the (mu, E) record so that t0 stays the hydro's
+    pj.E = E; pj.kx = kappa; pj.sE = f[F_E]; pj.skx = f[F_KAPPA];
+    CK(launch_prep_hydro(c, pj, st), "hydro + limiter prologue");
     if (c->tl.enabled) {
         TiledArgs t{};
         t.beta = beta; t.c_light = c_light;

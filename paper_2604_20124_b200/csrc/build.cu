@@ -227,10 +227,17 @@ __global__ void k_prep_hydro(PrepJob j, const uint32_t* __restrict__ perm, int64
     o.s2[i] = make_double2(vy, vz);
     o.s3[i] = make_double2(m, al * cs);
     o.t0[i] = make_double2(pr * ia, ia);
-    if (!nfast || *nfast != (unsigned long long)n) {
+    const bool soa = !nfast || *nfast != (unsigned long long)n;
+    if (soa) {
         j.sm[i] = m; j.srho[i] = rho; j.sp[i] = pr; j.scs[i] = cs; j.salpha[i] = al;
         j.svx[i] = vx; j.svy[i] = vy; j.svz[i] = vz;
         j.sV[i] = V; j.sQ[i] = V * pr; j.sAC[i] = al * cs;
+    }
+    if (j.E) {   // spray_hydro_rhs_limiter: the limiter's prologue in the same pass over the particles
+        const double E = __ldg(j.E + p), kx = __ldg(j.kx + p);
+        o.e1[i] = E;
+        o.me[i] = make_double2(rho * kx, E);
+        if (soa) { j.sE[i] = E; j.skx[i] = kx; }
     }
 }
 __global__ void k_prep_fld(PrepJob j, const uint32_t* __restrict__ perm, int64_t n, PackedOut o,
@@ -243,7 +250,6 @@ __global__ void k_prep_fld(PrepJob j, const uint32_t* __restrict__ perm, int64_t
     o.s0[i] = make_double2(o.p1[i].x, V);
     o.e1[i] = E;
     if (j.kx_is_mu) o.me[i] = make_double2(kx, E);
-    else if (j.rk_to_me) o.me[i] = make_double2(rho * kx, E);
     else o.t0[i] = make_double2(rho * kx, 0.0);
     if (!nfast || *nfast != (unsigned long long)n) {
         j.sm[i] = m; j.srho[i] = rho; j.sE[i] = E; j.skx[i] = kx;

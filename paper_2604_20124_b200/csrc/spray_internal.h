@@ -110,7 +110,6 @@ struct PrepJob {
     const double *m, *rho, *p, *cs, *vx, *vy, *vz, *alpha, *E, *kx;   // caller order (kx = kappa or mu)
     double *sm, *srho, *sp, *scs, *svx, *svy, *svz, *salpha, *sE, *skx, *sV, *sQ, *sAC;   // sorted order (general kernels)
     int kx_is_mu;
-    int rk_to_me;               // limiter prologue of the fused hydro + limiter call: (rho kappa, E) goes to me[], t0 stays the hydro's
 };
 cudaError_t launch_prep_density(Ctx* c, const double* m, cudaStream_t st);
 cudaError_t launch_prep_hydro(Ctx* c, const PrepJob& j, cudaStream_t st);

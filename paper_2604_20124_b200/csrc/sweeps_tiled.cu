@@ -480,7 +480,7 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
                 if (SWEEP == SW_HYDLIM) {
                     // the limiter epilogue of SW_LIMITER below, on the sums of the same pair terms
                     const double gx = T.fn * acc.k[0], gy = T.fn * acc.k[1], gz = T.fn * acc.k[2];
-                    const double rk = A.me[i].x;                 // rho_a kappa_a (k_prep_fld, rk_to_me)
+                    const double rk = A.me[i].x;                 // rho_a kappa_a, parked there by k_prep_hydro
                     const double gn = sqrt(gx * gx + gy * gy + gz * gz);
                     const double Rl = gn / (rk * T.e);
                     const double mu = A.c_light * (1.0 / sqrt(9.0 + Rl * Rl)) / rk;
