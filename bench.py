@@ -484,7 +484,7 @@ def main():
     # (profiles/r01d_ncu_full_tiled_path.md); null for other workloads
     # (fused sweep k_tiled_sweep<10,0,1>: profiles/r01h_ncu_full_fused_pass.md)
     traffic = ((6.87e9 + 1.20e9) if fused else (6.01e9 + 0.67e9)) if w.name.startswith("c5") else None
-    kname = ("hydro + limiter pair sweep (spray_hydro_rhs_limiter: prologues k_prep_hydro, k_prep_fld + k_tiled_sweep<10>; algorithmic flops of rows a6 + a7)"
+    kname = ("hydro + limiter pair sweep (spray_hydro_rhs_limiter: prologue k_prep_hydro + k_tiled_sweep<10>; algorithmic flops of rows a6 + a7)"
              if fused else "hydro pair sweep (spray_hydro_rhs: prologue k_prep_hydro + k_tiled_sweep<1>)")
     roofline = {"bound": "alu", "kernel": kname,
                 "achieved": hydro_tflops, "peak": fp64_meas, "unit": "TFLOP/s", "frac": hydro_tflops / fp64_meas,
