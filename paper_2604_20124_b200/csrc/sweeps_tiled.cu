@@ -133,7 +133,7 @@ struct Acc {
 struct Tgt {                         // per-target constants
     double x, y, z, hinv, fn;
     double c0, c1, c2, c3, c4, c5;   // per sweep (see k_tiled_sweep)
-    double e;                        // SW_HYDLIM: E_a
+    double e, rk;                    // SW_HYDLIM: E_a, rho_a kappa_a
 };
 
 // One pair (target, slot s).  F = staged records ([record][TILE_CMAXP] double2), Ee = staged E (limiter).
@@ -393,7 +393,7 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
             const double2 xy = A.rec[0][i], zh = A.p1[i], hv = A.hh[i];
             T.x = xy.x; T.y = xy.y; T.z = zh.x; T.hinv = hv.x; T.fn = hv.y;
             if (SWEEP == SW_DENSITY) T.c0 = A.rec[1][i].y;                                   // m_a
-            if (SWEEP == SW_HYDLIM) T.e = A.e1[i];                                           // E_a
+            if (SWEEP == SW_HYDLIM) { const double2 re = A.me[i]; T.rk = re.x; T.e = re.y; }  // (rho_a kappa_a, E_a), parked there by k_prep_hydro
             if (HYD) {
                 const double2 t0 = A.t0[i], q1 = A.rec[2][i], q2 = A.rec[3][i];
                 T.c0 = t0.x; T.c1 = t0.y;                                                    // p_a/rho_a, 1/rho_a
@@ -480,7 +480,7 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
                 if (SWEEP == SW_HYDLIM) {
                     // the limiter epilogue of SW_LIMITER below, on the sums of the same pair terms
                     const double gx = T.fn * acc.k[0], gy = T.fn * acc.k[1], gz = T.fn * acc.k[2];
-                    const double rk = A.me[i].x;                 // rho_a kappa_a, parked there by k_prep_hydro
+                    const double rk = T.rk;
                     const double gn = sqrt(gx * gx + gy * gy + gz * gz);
                     const double Rl = gn / (rk * T.e);
                     const double mu = A.c_light * (1.0 / sqrt(9.0 + Rl * Rl)) / rk;
