@@ -93,8 +93,12 @@ int64_t spray_launch_count(const spray_ctx* ctx);
 int spray_set_path(spray_ctx* ctx, int path);
 
 /* Debug/measurement: synchronises `stream`; *n_tiles = tiles of the tiled path built by the last spray_build_cells,
- * *n_fast = particles served by the tiled kernels (the rest, n - n_fast, by the general kernels). Both nullable. */
-int spray_path_stats(spray_ctx* ctx, void* stream, int64_t* n_tiles, int64_t* n_fast);
+ * *n_fast = particles served by the tiled kernels (the rest, n - n_fast, by the general kernels),
+ * *n_nonuniform = list-builder work units (half tiles) whose particles do not all share one h (they run the
+ * variable-h pair bodies), *scratch_bytes = device memory the context holds (allocated at spray_create).
+ * All host pointers, all nullable. */
+int spray_path_stats(spray_ctx* ctx, void* stream, int64_t* n_tiles, int64_t* n_fast, int64_t* n_nonuniform,
+                     int64_t* scratch_bytes);
 
 /* (a1)-(a4) NNPS: cell index per particle  c_d = floor((x_d - lo_d) * ncell_d / L_d) clamped,
  * key = (c_z*ncell_y + c_y)*ncell_x + c_x;  STABLE sort of (key, caller index);  cell_start[c] = #{key < c},

@@ -129,6 +129,18 @@ def neighbor_lists(grid, x, y, z, h, mode, use_cells=True, targets=None):
     return off, nbr[: int(off[-1])]
 
 
+def neighbor_digest(grid, x, y, z, h, mode, use_cells=True):
+    """Full-population (count uint32, sum uint64, xor uint64) of splitmix64(caller id) over each particle's neighbour set
+    (self excluded); SYM is built from the gather sets by transposition (see oracle_neighbor_digest)."""
+    n = len(x)
+    (x, px), (y, py), (z, pz), (h, ph) = _d(x), _d(y), _d(z), _d(h)
+    cnt = np.zeros(n, np.uint32); ds = np.zeros(n, np.uint64); dx = np.zeros(n, np.uint64)
+    g = _grid(grid)
+    rc = lib().oracle_neighbor_digest(C.byref(g), C.c_int64(n), px, py, pz, ph, int(use_cells), int(mode), _p(cnt), _p(ds), _p(dx))
+    assert rc == 0
+    return cnt, ds, dx
+
+
 def density(grid, kernel, x, y, z, h, m, use_cells=True, targets=None):
     """O4, eq. (35).  Returns dict(rho, nnbr, S_rho) at the targets."""
     n = len(x)

@@ -293,6 +293,71 @@ int oracle_neighbor_lists(const oracle_grid_t* g, int64_t n, const double* x, co
     return 0;
 }
 
+/* ------------------------------------------------------------------ K9: neighbour-set digests
+ * Order-independent digest of a neighbour set: (count, sum over b of H(b) mod 2^64, xor over b of H(b)), H = the
+ * splitmix64 finaliser of the caller index, so that full-population set comparisons need 20 bytes per particle
+ * instead of the CSR lists.  Self excluded in both modes.
+ * GATHER: the set is enumerated directly.
+ * SYM: r2 < 4 max(h_a,h_b)^2  <=>  r2 < 4 h_a^2  or  r2 < 4 h_b^2, and r2(a,b) = r2(b,a) bit for bit (the
+ * displacement, its minimum image and the squares are odd/even in the exchange), hence
+ *   N_sym(b) = (N_gather(b) \ {b})  U  { a : b in N_gather(a), a not in N_gather(b) }.
+ * Every a therefore adds H(b) to its own digest for each b it sees, and H(a) to the digest of each b it sees that
+ * does not see it (integer sums and xors commute, so the order of the scattered updates is immaterial).  This only
+ * needs the gather reach 2 h_a, not 2 max(h): it is what makes the full-population comparison at BASELINE.json's
+ * config 4 feasible.  Pinned against the direct enumeration (oracle_neighbor_lists) in tests/test_oracle_pins.py.
+ */
+static uint64_t digest_hash(uint64_t x) {
+    x += 0x9E3779B97F4A7C15ull;
+    x = (x ^ (x >> 30)) * 0xBF58476D1CE4E5B9ull;
+    x = (x ^ (x >> 27)) * 0x94D049BB133111EBull;
+    return x ^ (x >> 31);
+}
+
+int oracle_neighbor_digest(const oracle_grid_t* g, int64_t n, const double* x, const double* y, const double* z,
+                           const double* h, int use_cells, int mode, uint32_t* count, uint64_t* dsum, uint64_t* dxor /* [n] each */) {
+    search_t s;
+    if (search_init(&s, g, n, x, y, z, h, use_cells)) return -1;
+    for (int64_t a = 0; a < n; ++a) { count[a] = 0; dsum[a] = 0; dxor[a] = 0; }
+#pragma omp parallel
+    {
+        ilist_t l = {0, 0, 0};
+#pragma omp for schedule(dynamic, 64)
+        for (int64_t a = 0; a < n; ++a) {
+            enumerate(&s, ORACLE_GATHER, a, &l);
+            uint32_t c = 0;
+            uint64_t sm = 0, xr = 0;
+            const uint64_t ha = digest_hash((uint64_t)a);
+            for (int64_t k = 0; k < l.n; ++k) {
+                const int64_t b = l.v[k];
+                if (b == a) continue;
+                const uint64_t hb = digest_hash((uint64_t)b);
+                c += 1; sm += hb; xr ^= hb;
+                if (mode == ORACLE_SYM) {
+                    double dx, dy, dz;
+                    const double r2 = pair_r2(&s, b, a, &dx, &dy, &dz);
+                    if (!(r2 < 4.0 * (s.h[b] * s.h[b]))) {      /* b does not see a: a is b's neighbour through h_a only */
+#pragma omp atomic
+                        count[b] += 1;
+#pragma omp atomic
+                        dsum[b] += ha;
+#pragma omp atomic
+                        dxor[b] ^= ha;
+                    }
+                }
+            }
+#pragma omp atomic
+            count[a] += c;
+#pragma omp atomic
+            dsum[a] += sm;
+#pragma omp atomic
+            dxor[a] ^= xr;
+        }
+        free(l.v);
+    }
+    search_free(&s);
+    return 0;
+}
+
 /* ------------------------------------------------------------------ O4: density, eq. (35)
  * rho_a = sum_{b in N_gather(a)} m_b W(r_ab; h_a), self term included (A11).
  * S_rho = the same sum of absolute values (O8).  nnbr = |N_gather(a)| - 1.

@@ -60,7 +60,7 @@ def load():
     lib.spray_check.argtypes = [vp, vp, C.POINTER(C.c_uint32)]
     lib.spray_set_path.argtypes = [vp, i32]
     lib.spray_launch_count.argtypes = [vp]
-    lib.spray_path_stats.argtypes = [vp, vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+    lib.spray_path_stats.argtypes = [vp, vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
     lib.spray_build_cells.argtypes = [vp, C.POINTER(Grid), i32, i64, vp, vp, vp, vp, vp]
     lib.spray_density.argtypes = [vp, vp, vp, vp, vp]
     lib.spray_hydro_rhs.argtypes = [vp] + [vp] * 8 + [dbl] + [vp] * 5 + [vp]
@@ -150,11 +150,17 @@ class Spray:
     def launch_count(self) -> int:
         return int(self.lib.spray_launch_count(self.h))
 
+    def path_stats_full(self):
+        """Statistics of the last build_cells (synchronises): tiles, particles served by the tiled kernels, list-builder
+        work units (half tiles) that found non-uniform h, bytes of device scratch the context holds."""
+        nt, nf, nn, nb = C.c_int64(0), C.c_int64(0), C.c_int64(0), C.c_int64(0)
+        self._ck(self.lib.spray_path_stats(self.h, _stream(), C.byref(nt), C.byref(nf), C.byref(nn), C.byref(nb)), "spray_path_stats")
+        return {"tiles": int(nt.value), "n_fast": int(nf.value), "nonuniform_units": int(nn.value), "scratch_bytes": int(nb.value)}
+
     def path_stats(self):
         """(tiles, particles served by the tiled kernels) of the last build_cells; synchronises."""
-        nt, nf = C.c_int64(0), C.c_int64(0)
-        self._ck(self.lib.spray_path_stats(self.h, _stream(), C.byref(nt), C.byref(nf)), "spray_path_stats")
-        return int(nt.value), int(nf.value)
+        st = self.path_stats_full()
+        return st["tiles"], st["n_fast"]
 
     def check(self) -> int:
         st = C.c_uint32(0)

@@ -28,9 +28,11 @@ int cuda_fail(Ctx* c, cudaError_t e, const char* where) {
 }
 
 template <class T>
-bool dmalloc(T** p, int64_t count) {
+bool dmalloc(T** p, int64_t count, Ctx* c = nullptr) {
     if (count < 1) count = 1;
-    return cudaMalloc((void**)p, sizeof(T) * (size_t)count) == cudaSuccess;
+    if (cudaMalloc((void**)p, sizeof(T) * (size_t)count) != cudaSuccess) return false;
+    if (c) c->scratch_bytes += (int64_t)(sizeof(T) * (size_t)count);
+    return true;
 }
 
 void free_all(Ctx* c) {
@@ -165,7 +167,8 @@ int spray_set_path(spray_ctx* ctx, int path) {
     return SPRAY_OK;
 }
 
-int spray_path_stats(spray_ctx* ctx, void* stream, int64_t* n_tiles, int64_t* n_fast) {
+int spray_path_stats(spray_ctx* ctx, void* stream, int64_t* n_tiles, int64_t* n_fast, int64_t* n_nonuniform,
+                     int64_t* scratch_bytes) {
     NEED_BUILT();
     Ctx* c = &ctx->c;
     cudaStream_t st = (cudaStream_t)stream;
@@ -176,6 +179,8 @@ int spray_path_stats(spray_ctx* ctx, void* stream, int64_t* n_tiles, int64_t* n_
     }
     if (n_tiles) *n_tiles = (int64_t)v[CTR_NTILES];
     if (n_fast) *n_fast = (int64_t)v[CTR_NFAST];
+    if (n_nonuniform) *n_nonuniform = (int64_t)v[CTR_NNONUNI];
+    if (scratch_bytes) *scratch_bytes = c->scratch_bytes;
     return SPRAY_OK;
 }
 

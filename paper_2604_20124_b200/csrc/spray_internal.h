@@ -72,6 +72,7 @@ struct Ctx {
     Tiled tl{};
     double* rad_scratch[4] = {nullptr, nullptr, nullptr, nullptr};   // N1: y, Lambda, Gamma, chi (caller order), allocated on first use
     int64_t launches = 0;       // kernels launched through this ctx (bench.py reports it as gpu_launches)
+    int64_t scratch_bytes = 0;  // device memory held by this ctx
     std::string err;
 };
 

@@ -67,3 +67,52 @@ def test_full_size_sampled(name):
     assert abs(float((V * fl["y"]).sum())) <= 1e-11 * float((V * fl["y"]).abs().sum()) + 1e-300
     assert bool((fl["diag"] <= 0).all()) and bool(torch.isfinite(fl["y"]).all())
     assert sp.check() == 0
+
+
+@pytest.mark.parametrize("name", ["c2", "c3", "c4", "c5"])
+def test_full_population_neighbour_digests(name):
+    """the neighbour sets of EVERY particle at full size, both set kinds, as (count, sum, xor) digests of the
+    hashed caller ids -- the GPU's come from the lists the sweeps run on (and from the general kernels for what the tiled
+    path declines), the oracle's from oracle_neighbor_digest (pinned in tests/test_oracle_pins.py)."""
+    w = W.make(name)
+    d = upload(w)
+    sp = make_ctx(w)
+    sp.build_cells(w.grid, w.kernel, d["x"], d["y"], d["z"], d["h"])
+    uniform = float(w.h.min()) == float(w.h.max())
+    ref = {}
+    for sym, mode in ((False, O.GATHER), (True, O.SYM)):
+        if sym and uniform:
+            ref[mode] = ref[O.GATHER]          # one h: N_sym(a) = N_gather(a) minus a, nothing to transpose
+        else:
+            ref[mode] = O.neighbor_digest(w.grid, w.x, w.y, w.z, w.h, mode)
+        cnt, ds, dx = ref[mode]
+        assert np.array_equal(u32(sp.neighbor_counts(sym)), cnt), (name, sym, "counts")
+        gs, gx = sp.neighbor_digest(sym)
+        assert np.array_equal(u64(gs), ds), (name, sym, "sum digests")
+        assert np.array_equal(u64(gx), dx), (name, sym, "xor digests")
+    assert sp.check() == 0
+
+
+@pytest.mark.parametrize("name", ["c2", "c3", "c4", "c5", "c5_v"])
+def test_full_size_outputs(name):
+    """Every fp64 output of every sweep: ALL particles at c2 and c3, 200 000 sampled targets at c4, c5 and c5_v (the c5
+    variant with v ~ N(0, 0.01^2): the viscous branch of eqs. (41)-(43) at full size on the tiled path).  The frozen apply
+    takes mu = c / (3 rho kappa) (the diffusion limit, computed here from the inputs) on both sides, so no closure of the
+    sample is needed; the limiter sweep (UPDATE mode) is compared on its own."""
+    w = W.make(name)
+    d = upload(w)
+    sp = make_ctx(w)
+    sp.build_cells(w.grid, w.kernel, d["x"], d["y"], d["z"], d["h"])
+    if name in ("c2", "c3"):
+        tg = None
+    else:
+        rng = np.random.default_rng(5)
+        tg = np.sort(rng.choice(w.n, size=200000, replace=False)).astype(np.int64)
+    mu_full = w.c_light / (3.0 * w.rho_nom * w.kappa)
+    g = gpu_isolated(sp, d, w, targets=tg, mu_in=mu_full)
+    o = oracle_isolated(w, targets=tg, mu_full=mu_full)
+    errs = compare_isolated(g, o)
+    if name == "c5_v":
+        assert np.abs(o["dudt"]).max() > 0 and (o["S_dudt"] > 0).all()
+    assert sp.check() == 0
+    print(name, w.n, "all" if tg is None else tg.size, {k: f"{v:.1e}" for k, v in errs.items()})

@@ -102,9 +102,22 @@ def test_chained_pass(case, path):
         check(k, t.cpu().numpy(), oh[k], oh["S_" + k])
     check_mu(fl["mu"].cpu().numpy(), ol)
     # y depends on mu_a, mu_b with the relative perturbation allowed for mu: widen by that factor
+    # c_ab is homogeneous of degree one in (mu_a, mu_b), so its relative perturbation is at most the larger of the two
+    # particles' allowed relative perturbation of mu: widen PER PARTICLE by the worst factor over a and its own
+    # symmetric neighbours (not by the global worst).
     from parity_util import mu_tolerance
-    widen = float(np.max(mu_tolerance(ol)) / 1e-11)
-    check("y", fl["y"].cpu().numpy(), oa["y"], oa["S_y"], tol=1e-11 * max(1.0, 2 * widen))
+    tol_mu = mu_tolerance(ol)
+    off, nbr = O.neighbor_lists(w.grid, w.x, w.y, w.z, w.h, O.SYM)
+    worst = tol_mu.copy()
+    if nbr.size:
+        rows = np.repeat(np.arange(w.n), np.diff(off).astype(np.int64))
+        np.maximum.at(worst, rows, tol_mu[nbr])
+    gy, S = fl["y"].cpu().numpy(), oa["S_y"]
+    bound = (1e-11 + 2.0 * worst) * S
+    z = S == 0
+    assert np.array_equal(gy[z], oa["y"][z]) and np.isfinite(gy).all()
+    bad = np.abs(gy - oa["y"]) > bound
+    assert not bad.any(), f"y: {bad.sum()} particles beyond the per-particle bound, worst {float((np.abs(gy - oa['y'])[~z] / bound[~z]).max()):.2e} x"
     assert sp.check() == 0
 
 

@@ -148,6 +148,24 @@ def test_T5_sets_vs_independent_numpy_search(periodic):
         assert (msym == msym.T).all()          # "all neighbours are mutual"
 
 
+@pytest.mark.parametrize("periodic", [(1, 1, 1), (0, 0, 0), (1, 0, 1)])
+def test_T5_digests_vs_independent_numpy_search(periodic):
+    """oracle_neighbor_digest (full-population set digests; SYM built from the gather sets by transposition) against the
+    vectorised all-pairs masks of this file and numpy's own splitmix64 (workloads module): count, sum, xor per particle."""
+    w = W.random_cloud(2400, seed=9, periodic=periodic, hvar=2.0)
+    hsh = W.splitmix64(np.arange(w.n, dtype=np.uint64))
+    for mode in (O.GATHER, O.SYM):
+        mask = numpy_allpairs_sets(w, mode)
+        want_cnt = mask.sum(axis=1).astype(np.uint32)
+        with np.errstate(over="ignore"):
+            want_sum = (mask * hsh[None, :]).sum(axis=1, dtype=np.uint64)
+        want_xor = np.bitwise_xor.reduce(np.where(mask, hsh[None, :], np.uint64(0)), axis=1)
+        for cells in (False, True):
+            cnt, ds, dx = O.neighbor_digest(w.grid, w.x, w.y, w.z, w.h, mode, use_cells=cells)
+            assert np.array_equal(cnt, want_cnt) and np.array_equal(ds, want_sum) and np.array_equal(dx, want_xor)
+    assert not np.array_equal(numpy_allpairs_sets(w, O.GATHER), numpy_allpairs_sets(w, O.SYM))   # the case is not degenerate
+
+
 TINY = ["c1_tiny", "c2_tiny", "c3_tiny", "c4_tiny", "c5_tiny"]
 
 
@@ -399,3 +417,14 @@ def test_T15_permutation_translation_mirror():
     assert np.allclose(rm["ay"], base["ay"], rtol=0, atol=1e-11 * base["S_ay"].max())
     assert np.allclose(rm["dudt"], base["dudt"], rtol=0, atol=1e-11 * base["S_dudt"].max())
     assert np.allclose(rm["y"], base["y"], rtol=0, atol=1e-11 * base["S_y"].max())
+
+
+def test_golden_lattice_constants_reproduce_by_direct_summation():
+    """tests/golden/lattice_constants.txt is reproduced (to 2 units of the 15th decimal) by the committed generator, which
+    sums the retyped kernel formulas over the lattice and imports neither oracle/ nor the CUDA package."""
+    import subprocess
+    import sys
+    gen = os.path.join(os.path.dirname(GOLD), "make_lattice_constants.py")
+    src = open(gen).read()
+    assert "import oracle" not in src and "paper_2604_20124_b200" not in src
+    assert subprocess.run([sys.executable, gen, "--check"]).returncode == 0

@@ -155,6 +155,35 @@ def config1(nside: int = 16, seed: int = SEEDS[1], jitter: float = 0.05) -> Work
     return _finish(f"c1_cube{nside}", KERNEL_CUBIC_SPLINE, grid, 5.0 / 3.0, x, y, z, h, m, rho, u, vx, vy, vz, E, kappa)
 
 
+def lattice_hjitter(nside: int = 40, kernel: int = KERNEL_WENDLAND_C2, periodic=(1, 1, 1), seed: int = 2604201250,
+                    hjit: float = 0.05, jitter: float = 0.05) -> Workload:
+    """Jittered lattice in the unit cube with h = 1.2 dx (1 +- hjit) drawn per particle, on a grid with cell edge >= 2 max(h):
+    every neighbourhood mixes different h, so the tiled path (which needs 2 h_max <= cell edge) runs its VARIABLE-h tile
+    kernels on every tile (tests/test_gpu_edges.py).  Fields as config 1, unequal masses, variable rho and kappa."""
+    dx = 1.0 / nside
+    i, ix, iy, iz = _lattice(nside, nside, nside)
+    n = i.size
+    jit = lambda ch: (2.0 * u01(seed, i, ch) - 1.0) * jitter * dx
+    pos = []
+    for d, (c, ch) in enumerate(((ix, 0), (iy, 1), (iz, 2))):
+        v = (c + 0.5) * dx + jit(ch)
+        pos.append(_wrap(v, 0.0, 1.0) if periodic[d] else np.clip(v, 0.0, np.nextafter(1.0, 0.0)))
+    x, y, z = pos
+    h = 1.2 * dx * (1.0 + hjit * (2.0 * u01(seed, i, 3) - 1.0))
+    hmax = 1.2 * dx * (1.0 + hjit)
+    m = (0.8 + 0.4 * u01(seed, i, 10)) / n
+    rho = 0.8 + 0.4 * u01(seed, i, 11)
+    u = 0.9 + 0.2 * u01(seed, i, 12)
+    vx, vy, vz = (0.1 * normal(seed, i, ch) for ch in (4, 6, 8))
+    d2 = sum((np.abs(c - 0.5)) ** 2 for c in (x, y, z))
+    E = 1.0 + 0.5 * np.exp(-d2 / 0.02)
+    kappa = 0.5 + 2.0 * u01(seed, i, 13)
+    grid = _uniform_grid((0, 0, 0), (1, 1, 1), tuple(periodic), hmax)
+    w = _finish(f"hjit{nside}", kernel, grid, 5.0 / 3.0, x, y, z, h, m, rho, u, vx, vy, vz, E, kappa)
+    w.alpha = 0.5 + u01(seed, i, 14)
+    return w
+
+
 # --------------------------------------------------------------------------- config 2
 def config2(nl: int = 160, seed: int = SEEDS[2], jitter: float = 0.02, ly: float = 0.25) -> Workload:
     """Sod-style tube, periodic [0,2]x[0,.25]x[0,.25] (BJ config 2; Table 1).
@@ -350,6 +379,9 @@ PRESETS = {
     "c3_mid": lambda: config3(40),
     "c4_mid": lambda: config4(48, rho_min=0.01),
     "c5_mid": lambda: config5(48, vsigma=0.01),
+    # every tile of the tiled path has variable h (h jittered +-5 % on a grid with edge >= 2 max h)
+    "hjit_w": lambda: lattice_hjitter(40, KERNEL_WENDLAND_C2, (1, 1, 1)),
+    "hjit_c": lambda: lattice_hjitter(36, KERNEL_CUBIC_SPLINE, (1, 0, 1)),
 }
 
 
