@@ -1,6 +1,7 @@
 // api.cu -- the C-ABI of include/spray.h: argument checks, scratch ownership, kernel sequencing.
 // Every step of the path runs in CUDA kernels enqueued on the caller's stream; nothing here touches particle
 // data on the host and there is no CPU fallback.
+#include <cmath>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -47,34 +48,51 @@ void free_all(Ctx* c) {
     for (double2* r : k.s) cudaFree(r);
     Tiled& t = c->tl;
     cudaFree(t.tiles); cudaFree(t.bcount); cudaFree(t.pool); cudaFree(t.ctr); cudaFree(t.winfo); cudaFree(t.lcount);
-    cudaFree(t.tflags); cudaFree(t.tiletab); cudaFree(t.fast);
+    cudaFree(t.tflags); cudaFree(t.tiletab); cudaFree(t.fast); cudaFree(t.coinc);
 }
 
-// Scratch of the tiled path (tiles, neighbour lists): sized for (n, grid) at the first spray_build_cells that needs
-// it and kept; growing it synchronises the device (cudaFree).  Failure to allocate is not an error: the general
-// kernels then serve every particle.
-
-void ensure_tiled(Ctx* c) {
+// Scratch of the tiled path (tiles, tile tables, neighbour-list pool), allocated once by spray_create from n_max and
+// ncell_max -- spray_build_cells never allocates, frees or synchronises.  Capacities: a bundle is a 2 x 2 block of cell
+// rows, so a grid has ceil(ny/2) ceil(nz/2) of them: room for 4 ncell_max^(2/3) (at least 4096), which covers every
+// grid whose x extent is not much shorter than the other two; tiles: n_max / TILE_T plus the partial tiles at bundle
+// ends and column cuts; list pool: 208 bytes per particle (two bytes per neighbour and list padding; ~100 neighbours).
+// A build that needs more than this is served by the general kernels (whole grid or, for the pool, unit by unit).
+// Failure to allocate is not an error either: the general kernels then serve every particle.
+void alloc_tiled(Ctx* c) {
     Tiled& t = c->tl;
-    const int64_t nb = (int64_t)((c->grid.ncell[1] + 1) / 2) * ((c->grid.ncell[2] + 1) / 2);
-    const int64_t need = (5 * ((c->n + TILE_T - 1) / TILE_T)) / 4 + 2 * nb + 64;
-    const int64_t pool_need = need * TILE_WARPS * (LIST_RMAX / 4) * 32;   // one fixed block of LIST_RMAX rounds per (tile, warp)
-    if (t.tiles && need <= t.tile_cap && nb <= t.bundle_cap && pool_need <= t.pool_cap) return;
-    cudaFree(t.tiles); cudaFree(t.bcount); cudaFree(t.pool); cudaFree(t.winfo); cudaFree(t.lcount); cudaFree(t.tflags); cudaFree(t.tiletab);
-    t.tiles = nullptr; t.bcount = nullptr; t.pool = nullptr; t.winfo = nullptr; t.lcount = nullptr; t.tflags = nullptr; t.tiletab = nullptr;
-    t.tile_cap = 0; t.bundle_cap = 0; t.pool_cap = 0;
-    bool ok = dmalloc(&t.tiles, need) && dmalloc(&t.bcount, nb + 4096 + 64) && dmalloc(&t.winfo, need * TILE_WARPS) &&
-              dmalloc(&t.lcount, need * TILE_T) && dmalloc(&t.tflags, need) && dmalloc(&t.tiletab, need * TILES_WORDS) && dmalloc(&t.pool, pool_need);
-    if (ok && !t.ctr) ok = dmalloc(&t.ctr, CTR_COUNT);
-    if (ok && !t.fast) ok = dmalloc(&t.fast, c->n_max);
+    const int64_t n = c->n_max;
+    int64_t nb = 4 * (int64_t)ceil(pow((double)c->ncell_max, 2.0 / 3.0));
+    nb = nb < 4096 ? 4096 : nb;
+    nb = nb > c->ncell_max ? c->ncell_max : nb;
+    const int64_t tiles = (5 * ((n + TILE_T - 1) / TILE_T)) / 4 + 2 * nb + c->ncell_max / 64 + 64;
+    const int64_t rows = (n * 208) / 256 + 4096;
+    bool ok = dmalloc(&t.tiles, tiles, c) && dmalloc(&t.bcount, nb + 4096 + 64, c) && dmalloc(&t.winfo, tiles * TILE_WARPS, c) &&
+              dmalloc(&t.lcount, tiles * TILE_T, c) && dmalloc(&t.tflags, tiles, c) && dmalloc(&t.tiletab, tiles * TILES_WORDS, c) &&
+              dmalloc(&t.pool, rows * 32, c) && dmalloc(&t.ctr, CTR_COUNT, c) && dmalloc(&t.fast, n, c) && dmalloc(&t.coinc, n, c);
+    if (ok) ok = tiled_set_attributes(c) == cudaSuccess;
     if (!ok) {
         cudaGetLastError();
         cudaFree(t.tiles); cudaFree(t.bcount); cudaFree(t.pool); cudaFree(t.winfo); cudaFree(t.lcount); cudaFree(t.tflags); cudaFree(t.tiletab);
-        t.tiles = nullptr; t.bcount = nullptr; t.pool = nullptr; t.winfo = nullptr; t.lcount = nullptr; t.tflags = nullptr; t.tiletab = nullptr;
+        cudaFree(t.ctr); cudaFree(t.fast); cudaFree(t.coinc);
+        t = Tiled{};
+        int sms = 0;
+        if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device) == cudaSuccess && sms > 0) t.sms = sms;
         return;
     }
-    t.tile_cap = need; t.bundle_cap = nb; t.pool_cap = pool_need;
+    t.tile_cap = tiles; t.bundle_cap = nb; t.pool_rows = rows > 0xFFFFFFF0ll ? 0xFFFFFFF0ll : rows;
 }
+
+// every entry point runs on the context's device and leaves the caller's current device as it found it
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = true;
+    explicit DeviceGuard(int dev) {
+        if (cudaGetDevice(&prev) != cudaSuccess) { prev = -1; cudaGetLastError(); }
+        if (prev != dev) ok = cudaSetDevice(dev) == cudaSuccess;
+        if (prev == dev) prev = -1;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
 
 SweepArgs base_args(Ctx* c) {
     SweepArgs a;
@@ -91,7 +109,10 @@ SweepArgs fallback_args(Ctx* c) {
 }
 
 #define CK(call, where) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) return cuda_fail(c, e__, where); } while (0)
-#define NEED_BUILT() do { if (!ctx) return SPRAY_ERR_INVALID_ARG; if (!ctx->c.built) return fail(&ctx->c, SPRAY_ERR_NOT_BUILT, "spray_build_cells has not succeeded on this context"); } while (0)
+#define NEED_BUILT() if (!ctx) return SPRAY_ERR_INVALID_ARG; \
+    if (!ctx->c.built) return fail(&ctx->c, SPRAY_ERR_NOT_BUILT, "spray_build_cells has not succeeded on this context"); \
+    DeviceGuard dev_guard__(ctx->c.device); \
+    if (!dev_guard__.ok) { cudaGetLastError(); return fail(&ctx->c, SPRAY_ERR_CUDA, "cudaSetDevice failed"); }
 
 enum { F_M = 0, F_RHO, F_P, F_CS, F_VX, F_VY, F_VZ, F_ALPHA, F_E, F_KAPPA, F_MU, F_V, F_Q, F_AC };
 
@@ -102,9 +123,11 @@ extern "C" {
 const char* spray_version(void) { return "spray-b200 0.1 sm_100a"; }
 
 int spray_create(spray_ctx** out, int64_t n_max, int64_t ncell_max, int device) {
-    if (!out || n_max < 0 || ncell_max < 1 || n_max > 0xFFFFFFF0ll || ncell_max > 0x7FFFFFFFll)
-        return fail(nullptr, SPRAY_ERR_INVALID_ARG, "spray_create: bad arguments");
-    if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return fail(nullptr, SPRAY_ERR_CUDA, "spray_create: cudaSetDevice failed"); }
+    // n_max <= 2^28: the radix sort scans its digit histograms in two levels of 4096 (build.cu), which covers 2^28 keys
+    if (!out || n_max < 0 || ncell_max < 1 || n_max > (1ll << 28) || ncell_max > 0x7FFFFFFFll)
+        return fail(nullptr, SPRAY_ERR_INVALID_ARG, "spray_create: bad arguments (n_max <= 2^28, 1 <= ncell_max < 2^31)");
+    DeviceGuard dg(device);
+    if (!dg.ok) { cudaGetLastError(); return fail(nullptr, SPRAY_ERR_CUDA, "spray_create: cudaSetDevice failed"); }
     spray_ctx* h = new (std::nothrow) spray_ctx();
     if (!h) return SPRAY_ERR_ALLOC;
     Ctx* c = &h->c;
@@ -114,15 +137,16 @@ int spray_create(spray_ctx** out, int64_t n_max, int64_t ncell_max, int device) 
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) == cudaSuccess && sms > 0) c->tl.sms = sms;
     c->hist_cap = 256 * ((n_max + 4095) / 4096 + 1) + 4096;   // radix histograms + block totals of their scan
     bool ok = true;
-    for (int k = 0; k < 2; ++k) ok = ok && dmalloc(&c->key[k], n_max) && dmalloc(&c->idx[k], n_max);
-    ok = ok && dmalloc(&c->hist, c->hist_cap) && dmalloc(&c->cell_start, ncell_max) && dmalloc(&c->cell_end, ncell_max) &&
-         dmalloc(&c->cell_hmax, ncell_max) && dmalloc(&c->hglob, 4) && dmalloc(&c->dev_status, 1) && dmalloc(&c->s.x, n_max) &&
-         dmalloc(&c->s.y, n_max) && dmalloc(&c->s.z, n_max) && dmalloc(&c->s.h, n_max) && dmalloc(&c->s.hs, n_max);
-    for (double*& f : c->s.f) ok = ok && dmalloc(&f, n_max);
+    for (int k = 0; k < 2; ++k) ok = ok && dmalloc(&c->key[k], n_max, c) && dmalloc(&c->idx[k], n_max, c);
+    ok = ok && dmalloc(&c->hist, c->hist_cap, c) && dmalloc(&c->cell_start, ncell_max, c) && dmalloc(&c->cell_end, ncell_max, c) &&
+         dmalloc(&c->cell_hmax, ncell_max, c) && dmalloc(&c->hglob, 4, c) && dmalloc(&c->dev_status, 1, c) && dmalloc(&c->s.x, n_max, c) &&
+         dmalloc(&c->s.y, n_max, c) && dmalloc(&c->s.z, n_max, c) && dmalloc(&c->s.h, n_max, c) && dmalloc(&c->s.hs, n_max, c);
+    for (double*& f : c->s.f) ok = ok && dmalloc(&f, n_max, c);
     Packed& k = c->pk;
-    ok = ok && dmalloc(&k.p0, n_max) && dmalloc(&k.p1, n_max) && dmalloc(&k.hh, n_max) && dmalloc(&k.t0, n_max) &&
-         dmalloc(&k.me, n_max) && dmalloc(&k.e1, n_max);
-    for (double2*& r : k.s) ok = ok && dmalloc(&r, n_max);
+    ok = ok && dmalloc(&k.p0, n_max, c) && dmalloc(&k.p1, n_max, c) && dmalloc(&k.hh, n_max, c) && dmalloc(&k.t0, n_max, c) &&
+         dmalloc(&k.me, n_max, c) && dmalloc(&k.e1, n_max, c);
+    for (double2*& r : k.s) ok = ok && dmalloc(&r, n_max, c);
+    for (double*& r : c->rad_scratch) ok = ok && dmalloc(&r, n_max, c);     // rows N1, N2: y, Lambda, Gamma, chi / g, y of two species
     if (ok) ok = cudaMemset(c->dev_status, 0, sizeof(uint32_t)) == cudaSuccess;
     if (!ok) {
         cudaGetLastError();
@@ -130,13 +154,14 @@ int spray_create(spray_ctx** out, int64_t n_max, int64_t ncell_max, int device) 
         delete h;
         return fail(nullptr, SPRAY_ERR_ALLOC, "spray_create: device allocation failed");
     }
+    alloc_tiled(c);
     *out = h;
     return SPRAY_OK;
 }
 
 int spray_destroy(spray_ctx* ctx) {
     if (!ctx) return SPRAY_OK;
-    cudaSetDevice(ctx->c.device);
+    DeviceGuard dg(ctx->c.device);
     cudaDeviceSynchronize();
     free_all(&ctx->c);
     delete ctx;
@@ -148,6 +173,7 @@ const char* spray_last_error(const spray_ctx* ctx) { return ctx ? ctx->c.err.c_s
 int spray_check(spray_ctx* ctx, void* stream, uint32_t* dev_status) {
     if (!ctx) return SPRAY_ERR_INVALID_ARG;
     Ctx* c = &ctx->c;
+    DeviceGuard dg(c->device);
     cudaStream_t st = (cudaStream_t)stream;
     CK(cudaStreamSynchronize(st), "spray_check (a kernel enqueued earlier faulted)");
     uint32_t v = 0;
@@ -172,7 +198,7 @@ int spray_path_stats(spray_ctx* ctx, void* stream, int64_t* n_tiles, int64_t* n_
     NEED_BUILT();
     Ctx* c = &ctx->c;
     cudaStream_t st = (cudaStream_t)stream;
-    unsigned long long v[CTR_COUNT] = {0, 0, 0, 0};
+    unsigned long long v[CTR_COUNT] = {};
     if (c->tl.enabled && c->n > 0) {
         CK(cudaStreamSynchronize(st), "spray_path_stats");
         CK(cudaMemcpy(v, c->tl.ctr, sizeof v, cudaMemcpyDeviceToHost), "spray_path_stats");
@@ -189,6 +215,8 @@ int spray_build_cells(spray_ctx* ctx, const spray_grid_t* g, spray_kernel_t kern
     if (!ctx) return SPRAY_ERR_INVALID_ARG;
     Ctx* c = &ctx->c;
     c->built = false;
+    DeviceGuard dg(c->device);
+    if (!dg.ok) { cudaGetLastError(); return fail(c, SPRAY_ERR_CUDA, "cudaSetDevice failed"); }
     if (!g || n < 0 || (n > 0 && (!x || !y || !z || !h))) return fail(c, SPRAY_ERR_INVALID_ARG, "spray_build_cells: NULL argument or n < 0");
     if (kernel != SPRAY_KERNEL_CUBIC_SPLINE && kernel != SPRAY_KERNEL_WENDLAND_C2)
         return fail(c, SPRAY_ERR_INVALID_ARG, "spray_build_cells: unknown kernel id");
@@ -224,10 +252,7 @@ int spray_build_cells(spray_ctx* ctx, const spray_grid_t* g, spray_kernel_t kern
     SweepArgs a = base_args(c);
     a.o0 = c->s.hs;
     CK(launch_ref_sweep(c, SW_HSEARCH, a, st), "search-length sweep");
-    if (c->path == 1) {
-        ensure_tiled(c);
-        CK(launch_build_tiles(c, st), "tiles + neighbour lists");
-    }
+    if (c->path == 1) CK(launch_build_tiles(c, st), "tiles + neighbour lists");
     c->built = true;
     return SPRAY_OK;
 }
@@ -409,8 +434,6 @@ int spray_conduction_implicit(spray_ctx* ctx, const double* m, const double* rho
     if (c->n > 0 && (!m || !rho || !k_i || !k_e || !kei || !dTdu_i || !dTdu_e || !u_i || !u_e || !out_i || !out_e || (rhs && (!T_i || !T_e))))
         return fail(c, SPRAY_ERR_INVALID_ARG, "spray_conduction_implicit: NULL argument");
     if (!(dt > 0.0)) return fail(c, SPRAY_ERR_INVALID_ARG, "spray_conduction_implicit: dt must be > 0");
-    for (double*& r : c->rad_scratch)
-        if (!r && !dmalloc(&r, c->n_max)) { cudaGetLastError(); return fail(c, SPRAY_ERR_ALLOC, "spray_conduction_implicit: scratch allocation failed"); }
     cudaStream_t st = (cudaStream_t)stream;
     CondArgs a{};
     a.rho = rho; a.kei = kei; a.tau_i = dTdu_i; a.tau_e = dTdu_e; a.T_i = T_i; a.T_e = T_e; a.u_i = u_i; a.u_e = u_e;
@@ -458,8 +481,6 @@ int spray_rad_jacobi(spray_ctx* ctx, const double* m, const double* rho, const d
         return fail(c, SPRAY_ERR_INVALID_ARG, "spray_rad_jacobi: NULL argument");
     if (!(dt > 0.0) || !(c_light > 0.0) || !(a_rad > 0.0) || niter < 1 || (kmode != SPRAY_FLD_SYMMETRIC && kmode != SPRAY_FLD_GATHER))
         return fail(c, SPRAY_ERR_INVALID_ARG, "spray_rad_jacobi: dt, c_light, a_rad must be > 0, niter >= 1, kmode valid");
-    for (double*& r : c->rad_scratch)
-        if (!r && !dmalloc(&r, c->n_max)) { cudaGetLastError(); return fail(c, SPRAY_ERR_ALLOC, "spray_rad_jacobi: scratch allocation failed"); }
     cudaStream_t st = (cudaStream_t)stream;
     double** f = c->s.f;
     // sorted records of the frozen operator: (z, V), (mu, E) with E = the starting iterate
@@ -574,7 +595,8 @@ int spray_neighbor_digest(spray_ctx* ctx, int symmetric, uint64_t* dsum, uint64_
 
 int spray_fp64_peak_probe(int device, int blocks, int threads, int64_t iters, double* out, void* stream) {
     if (!out || blocks < 1 || threads < 1 || threads > 256 || iters < 0) return SPRAY_ERR_INVALID_ARG;
-    if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return SPRAY_ERR_CUDA; }
+    DeviceGuard dg(device);
+    if (!dg.ok) { cudaGetLastError(); return SPRAY_ERR_CUDA; }
     return launch_fp64_probe(blocks, threads, iters, out, (cudaStream_t)stream) == cudaSuccess ? SPRAY_OK : SPRAY_ERR_CUDA;
 }
 

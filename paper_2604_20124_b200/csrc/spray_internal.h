@@ -38,16 +38,21 @@ struct Tiled {
     int64_t tile_cap = 0;
     uint32_t* bcount = nullptr;  // [bundle_cap + 1 + scan scratch] tiles per bundle -> exclusive scan
     int64_t bundle_cap = 0;
-    uint2* pool = nullptr;       // list storage: per (tile, warp) a fixed block of LIST_RMAX/4 x 32 lanes x (4 u16 slots)
-    int64_t pool_cap = 0;        // in uint2 units
-    unsigned long long* ctr = nullptr;   // [CTR_NFAST] particles served by the tiled kernels, [CTR_NTILES] tiles, [CTR_NNONUNI]
-    uint2* winfo = nullptr;      // [tile_cap][TILE_WARPS]: (pool offset, rounds)
+    uint2* pool = nullptr;       // list storage: rows of 32 lanes x (4 u16 slots); a unit's warps take R/4 rows each, allocated
+                                 // by the list builder from ctr[CTR_POOL]
+    int64_t pool_rows = 0;       // capacity in rows (256 bytes each)
+    unsigned long long* ctr = nullptr;   // CTR_*
+    uint2* winfo = nullptr;      // [tile_cap][TILE_WARPS]: (first pool row, rounds)
     uint32_t* lcount = nullptr;  // [tile_cap][TILE_T]: n_gather | n_sym << 16
     uint32_t* tflags = nullptr;  // [tile_cap]: TILE_FLAG_*
     uint32_t* tiletab = nullptr; // [tile_cap][TILES_WORDS]: per-tile TileS tables
     uint8_t* fast = nullptr;     // [n_max] sorted order: 1 = particle is served by the tiled kernels
+    uint8_t* coinc = nullptr;    // [n_max] sorted order: 1 = particle has a twin at distance 0 (general kernels, A11)
+    int attr_device = -1;        // device on which the dynamic shared-memory opt-in of the tiled kernels was set
 };
-enum { CTR_NFAST = 1, CTR_NTILES = 2, CTR_NNONUNI = 3, CTR_COUNT = 4 };   // CTR_NNONUNI: half-tile units that found non-uniform h
+// CTR_NFAST: particles served by the tiled kernels; CTR_NTILES: tiles; CTR_NNONUNI: half-tile units that found non-uniform h;
+// CTR_POOL: list-pool rows handed out
+enum { CTR_NFAST = 1, CTR_NTILES = 2, CTR_NNONUNI = 3, CTR_POOL = 4, CTR_COUNT = 8 };
 
 struct Ctx {
     int device = 0;
@@ -126,6 +131,9 @@ struct TiledArgs {
     uint32_t* ocount;
 };
 cudaError_t launch_build_tiles(Ctx* c, cudaStream_t st);
+cudaError_t tiled_set_attributes(Ctx* c);      // dynamic shared-memory opt-in of the tiled kernels, on the ctx's device (spray_create)
+cudaError_t sweeps_set_attributes();
+cudaError_t launch_mark_coincident(Ctx* c, cudaStream_t st);   // build.cu
 cudaError_t launch_tiled_sweep(Ctx* c, int sweep, const TiledArgs& a, cudaStream_t st);
 // parity exports from the tiled lists: mode 0 = counts, 1 = CSR lists, 2 = digests (tiles.cu)
 cudaError_t launch_tiled_export(Ctx* c, int mode, int symmetric, uint32_t* ocount, const uint64_t* offsets, uint32_t* onbr,

@@ -369,7 +369,7 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
         // first three list rows: in flight while the records are staged
         uint2 wi = A.winfo[(size_t)tile * TILE_WARPS + warp];
         if (!half_ok) wi.y = 0u;
-        const uint2* lp = A.pool + wi.x + lane;
+        const uint2* lp = A.pool + (size_t)wi.x * 32 + lane;
         const uint2 l0 = wi.y ? __ldcs(lp) : make_uint2(0u, 0u);
         const uint2 l1 = wi.y > 4 ? __ldcs(lp + 32) : make_uint2(0u, 0u);
         const uint2 l2 = wi.y > 8 ? __ldcs(lp + 64) : make_uint2(0u, 0u);
@@ -540,15 +540,34 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
 }
 
 template <int SWEEP, int MODE>
+constexpr size_t sweep_smem() {
+    return sizeof(double2) * NRecM<SWEEP, MODE>::v * TILE_CMAXP + sizeof(double) * NRec<SWEEP>::e * TILE_CMAXP;
+}
+// The opt-in to more than 48 KB of dynamic shared memory is a per-device function attribute: set for every instantiation
+// that is launched, on the current device (spray_create calls this after cudaSetDevice).
+template <int SWEEP, int MODE>
+static cudaError_t set_attr() {
+    cudaError_t e = cudaFuncSetAttribute(k_tiled_sweep<SWEEP, 0, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sweep_smem<SWEEP, MODE>());
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_tiled_sweep<SWEEP, 1, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sweep_smem<SWEEP, MODE>());
+    return e;
+}
+cudaError_t sweeps_set_attributes() {
+    cudaError_t e = set_attr<SW_DENSITY, 0>();
+    if (e == cudaSuccess) e = set_attr<SW_HYDRO, 0>();
+    if (e == cudaSuccess) e = set_attr<SW_HYDRO, 2>();
+    if (e == cudaSuccess) e = set_attr<SW_LIMITER, 0>();
+    if (e == cudaSuccess) e = set_attr<SW_LIMITER, 2>();
+    if (e == cudaSuccess) e = set_attr<SW_HYDLIM, 1>();
+    if (e == cudaSuccess) e = set_attr<SW_GRADN, 0>();
+    if (e == cudaSuccess) e = set_attr<SW_APPLY, 1>();
+    if (e == cudaSuccess) e = set_attr<SW_APPLY, 2>();
+    if (e == cudaSuccess) e = set_attr<SW_KGC, 0>();
+    return e;
+}
+
+template <int SWEEP, int MODE>
 static cudaError_t launch_m(Ctx* c, const SweepIn& a, cudaStream_t st) {
-    constexpr size_t smem = sizeof(double2) * NRecM<SWEEP, MODE>::v * TILE_CMAXP + sizeof(double) * NRec<SWEEP>::e * TILE_CMAXP;
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(k_tiled_sweep<SWEEP, 0, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_tiled_sweep<SWEEP, 1, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        attr_done = true;
-    }
+    constexpr size_t smem = sweep_smem<SWEEP, MODE>();
     CellTable ct{c->cell_start, c->cell_end};
     const int grid = c->tl.sms * MinBlocks<SWEEP, MODE>::v;
     if (c->kernel == SPRAY_KERNEL_WENDLAND_C2) k_tiled_sweep<SWEEP, 1, MODE><<<grid, TILE_THREADS, smem, st>>>(c->dg, ct, a);

@@ -33,16 +33,19 @@ struct RowRef {                      // one candidate row of a bundle
     bool valid;
     bool target;                     // the row is one of the bundle's own rows
 };
+// slots the candidates of columns [xlo, xhi] of the row take in a tile's layout: every contiguous piece is padded to a
+// multiple of 8 slots (tile_setup)
+__device__ __forceinline__ uint32_t pad8(uint32_t c) { return (c + 7u) & ~7u; }
 __device__ __forceinline__ uint32_t row_count(const RowRef& r, int xlo, int xhi, int nx, bool per) {
     if (!r.valid) return 0u;
     if (per) {
-        if (xlo < 0) return (r.ce[nx - 1] - r.cs[xlo + nx]) + (r.ce[xhi] - r.cs[0]);
-        if (xhi >= nx) return (r.ce[nx - 1] - r.cs[xlo]) + (r.ce[xhi - nx] - r.cs[0]);
+        if (xlo < 0) return pad8(r.ce[nx - 1] - r.cs[xlo + nx]) + pad8(r.ce[xhi] - r.cs[0]);
+        if (xhi >= nx) return pad8(r.ce[nx - 1] - r.cs[xlo]) + pad8(r.ce[xhi - nx] - r.cs[0]);
     } else {
         xlo = xlo < 0 ? 0 : xlo;
         xhi = xhi > nx - 1 ? nx - 1 : xhi;
     }
-    return r.ce[xhi] - r.cs[xlo];
+    return pad8(r.ce[xhi] - r.cs[xlo]);
 }
 __device__ __forceinline__ uint32_t warp_sum(uint32_t v) {
 #pragma unroll
@@ -85,7 +88,7 @@ k_make_tiles(DevGrid g, CellTable ct, const double* __restrict__ hglob, uint32_t
     int cxa = 0;
     uint32_t skip = 0;
     while (ok && cxa < nx) {
-        if (warp_sum(row_count(row, cxa - 1, cxa + 1, nx, per)) > (uint32_t)(TILE_CMAX - TILE_MAXR)) { ++cxa; skip = 0; continue; }   // column not tileable
+        if (warp_sum(row_count(row, cxa - 1, cxa + 1, nx, per)) > (uint32_t)TILE_CMAX) { ++cxa; skip = 0; continue; }   // column not tileable
         uint32_t nt = 0;
         int cxb = cxa, next_cxa = nx;
         uint32_t next_skip = 0;
@@ -93,7 +96,7 @@ k_make_tiles(DevGrid g, CellTable ct, const double* __restrict__ hglob, uint32_t
             if (cx > cxa) {
                 const int ext = cx - cxa + 1;
                 if (ext > TILE_BXMAX || (per && ext + 2 > nx) ||
-                    warp_sum(row_count(row, cxa - 1, cx + 1, nx, per)) > (uint32_t)(TILE_CMAX - TILE_MAXR)) {
+                    warp_sum(row_count(row, cxa - 1, cx + 1, nx, per)) > (uint32_t)TILE_CMAX) {
                     next_cxa = cx; next_skip = 0; break;
                 }
             }
@@ -147,16 +150,30 @@ k_tile_tables(DevGrid g, CellTable ct, const TileDesc* __restrict__ tiles, const
 // One CTA of BL_THREADS threads builds the lists of HALF a tile (targets [128 half, 128 half + 128), i.e. warps
 // 8 half .. 8 half + 7 of the sweeps' CTA), so that two CTAs fit on an SM and one's barriers and staging latencies are
 // covered by the other's scan.  Work unit w = 2 tile + half.
+//
+// THE SCAN.  Candidates are staged as fp32 coordinates relative to the tile centre, one array per component, indexed
+// by slot; candidate ranges start on multiples of 8 slots, so an aligned BLOCK of 8 slots holds one slot of every
+// shared-memory bank of the sweeps (slot & 7).  The two threads of a target split the banks: thread u tests slots
+// 8 b + 4 u .. 8 b + 4 u + 3 of every block b of its warp's window with two packed (sm_100 FADD2/FFMA2) chains,
+//     t = dz^2 + (dy^2 + (dx^2 - T_hi)),   T_hi = (2 h)^2 (1 + 1e-5) + Am   (error bound Am below),
+// and a candidate with t < 0 is appended -- one predicated 16-bit store of the block number and one predicated
+// pointer increment -- to the thread's bucket of the candidate's bank.  The thread keeps min |t| over everything
+// it tested: if that stays above the width of the uncertainty band, every decision of the fp32 test was certain
+// and the buckets are final (only the target itself has to be taken out); otherwise, and in tiles with variable h,
+// every bucket entry is classified again (fp32 bounds first, then the exact fp64 contract predicate, O2/A12), so the
+// sets are bit-identical to the definition.  A hit is never lost: t < 0 is a superset of the support.
 struct ListArgs {
     const double2 *p0, *p1;            // sorted (x, y), (z, h)
     const TileDesc* tiles;
     unsigned long long* ctr;           // CTR_*
-    uint2* pool;
-    uint2* winfo;                      // [tile][warp]: (pool offset, rounds)
+    uint2* pool;                       // list storage, rows of 32 lanes x 4 u16 slots, allocated from ctr[CTR_POOL]
+    uint32_t pool_rows;                // capacity in rows
+    uint2* winfo;                      // [tile][warp]: (first pool row, rounds)
     uint32_t* lcount;                  // [tile][TILE_T]: n_gather | n_sym << 16
     uint32_t* tflags;                  // [tile], zeroed before the launch; each half ORs its bits in
     const uint32_t* tiletab;           // [tile][TILES_WORDS]
     uint8_t* fast;                     // [n] sorted order: 1 = served by the tiled kernels
+    const uint8_t* coinc;              // [n] sorted order: 1 = the particle has a twin at distance 0 (k_mark_coincident)
     const double* hglob;
     uint32_t* status;
 };
@@ -165,52 +182,46 @@ constexpr int BL_THREADS = TILE_THREADS / 2;
 constexpr int BL_WARPS = BL_THREADS / 32;
 constexpr int BL_TGT = TILE_T / 2;
 constexpr int COLW = TILE_BXMAX + 4;
-constexpr uint32_t LIST_RECHECK = 0x8000u;   // bucket-entry flag: classify this hit again (fp32 bounds, then exact fp64)
-constexpr int LIST_BS = LIST_BC + 1;        // rows of a (thread, bank) bucket incl. the trash row
-constexpr int LIST_LCAP = LIST_RMAX;       // rows of the schedule staging area (one column per thread)
-constexpr size_t BL_OFF_XY = 0;                                                         // float4 [CMAXP/2]: (x0, x1, y0, y1) of slots 2p, 2p+1
-constexpr size_t BL_OFF_ZT = BL_OFF_XY + sizeof(float4) * (TILE_CMAXP / 2);             // float4 [CMAXP/2]: (z0, z1, T0, T1), T = (2h)^2
+constexpr int LIST_TRASH = 4;                // trash rows of a bucket: the scan clamps its row pointers once per 4 blocks
+constexpr int LIST_BS = LIST_BC + LIST_TRASH;
+constexpr int LIST_LCAP = LIST_RMAX;         // rows of the schedule staging area (one column per thread)
+constexpr size_t BL_OFF_X = 0;                                                          // float [CMAXP] each: x, y, z relative to the
+constexpr size_t BL_OFF_Y = BL_OFF_X + sizeof(float) * TILE_CMAXP;                      // tile centre, T = (2 h)^2
+constexpr size_t BL_OFF_Z = BL_OFF_Y + sizeof(float) * TILE_CMAXP;
+constexpr size_t BL_OFF_T = BL_OFF_Z + sizeof(float) * TILE_CMAXP;
+constexpr size_t BL_CAND_END = BL_OFF_T + sizeof(float) * TILE_CMAXP;
 constexpr size_t BL_OFF_L = 0;                                                          // u16 [LIST_LCAP][BL_THREADS]: the schedule, written after
-                                                                                        // the scan is over -- shares the space of XY / ZT
-constexpr size_t BL_CAND_END = BL_OFF_ZT + sizeof(float4) * (TILE_CMAXP / 2);
+                                                                                        // the scan is over -- shares the space of the candidates
 constexpr size_t BL_L_END = BL_OFF_L + sizeof(uint16_t) * LIST_LCAP * BL_THREADS;
 constexpr size_t BL_OFF_B = BL_CAND_END > BL_L_END ? BL_CAND_END : BL_L_END;             // u16 [4][LIST_BS][BL_THREADS]
 constexpr size_t BL_OFF_COL = BL_OFF_B + sizeof(uint16_t) * 4 * LIST_BS * BL_THREADS;   // u16 [MAXR][COLW]
 constexpr size_t BL_SMEM = BL_OFF_COL + sizeof(uint16_t) * TILE_MAXR * COLW;
 static_assert(2 * (BL_SMEM + sizeof(TileS) + 1280) <= 228 * 1024, "list builder: two CTAs per SM");
+static_assert(TILE_CMAXP % 8 == 0 && TILE_CMAX % 8 == 0, "blocks of 8 slots");
 
 // packed fp32 pairs (sm_100 FADD2 / FMUL2 / FFMA2): one instruction tests two candidates
 typedef unsigned long long f32x2;
 __device__ __forceinline__ f32x2 pk2(float a, float b) { f32x2 r; asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(a), "f"(b)); return r; }
 __device__ __forceinline__ void unpk2(f32x2 v, float& a, float& b) { asm("mov.b64 {%0,%1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); }
 __device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) { f32x2 r; asm("sub.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
-__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) { f32x2 r; asm("mul.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
 __device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
 
-// One candidate of the scan: if r2 < hi, store (value | LIST_RECHECK unless 0 < r2 < 2 half_lo) at the bucket row pointer and
-// advance it, clamped at `end` (the bucket's trash row: a pointer that reaches it reports the overflow); nflag counts
-// the flagged hits.  No branches.
-__device__ __forceinline__ void append_flag(float r2, float hi, float half_lo, uint32_t& addr, uint32_t end, uint32_t v, uint32_t& nflag) {
-    asm volatile("{\n\t.reg .pred p, s, q;\n\t.reg .f32 t;\n\t.reg .b32 w;\n\t"
-                 "setp.lt.f32 p, %2, %3;\n\t"
-                 "sub.f32 t, %2, %4;\n\t"
-                 "abs.f32 t, t;\n\t"
-                 "setp.lt.f32 s, t, %4;\n\t"
-                 "setp.ge.and.f32 q, t, %4, p;\n\t"
-                 "selp.b32 w, %6, %7, s;\n\t"
-                 "@p st.shared.u16 [%0], w;\n\t"
-                 "@p add.u32 %0, %0, %8;\n\t"
-                 "@q add.u32 %1, %1, 1;\n\t"
-                 "min.u32 %0, %0, %5;\n\t}"
-                 : "+r"(addr), "+r"(nflag) : "f"(r2), "f"(hi), "f"(half_lo), "r"(end), "r"(v), "r"(v | LIST_RECHECK), "n"(2 * BL_THREADS));
-    // no memory clobber: the loads of the next pairs must be free to move above the store; the buckets are read back
+// One candidate of the scan: if t < 0 store the block number at the bucket row pointer and advance it.  No branches; the
+// caller clamps the pointer at the first trash row of the bucket once per LIST_TRASH blocks.
+__device__ __forceinline__ void append_if_neg(float t, uint32_t& addr, uint32_t blk) {
+    asm volatile("{\n\t.reg .pred p;\n\t"
+                 "setp.lt.f32 p, %1, 0f00000000;\n\t"
+                 "@p st.shared.u16 [%0], %2;\n\t"
+                 "@p add.u32 %0, %0, %3;\n\t}"
+                 : "+r"(addr) : "f"(t), "r"(blk), "n"(2 * BL_THREADS));
+    // no memory clobber: the loads of the next blocks must be free to move above the store; the buckets are read back
     // only after the fence that follows the scan
 }
 
-// Which thread of a target owns bank beta in the scan (threads split the candidate PAIRS: slots 4i+2u, 4i+2u+1), and
-// the index of that bank among the owner's four buckets.
-__device__ __forceinline__ int bank_owner(int beta) { return (beta >> 1) & 1; }
-__device__ __forceinline__ int bank_local(int beta) { return ((beta >> 2) << 1) | (beta & 1); }
+// Which thread of a target owns bank beta in the scan (thread u tests slots 8 b + 4 u .. 8 b + 4 u + 3), and the index
+// of that bank among the owner's four buckets.
+__device__ __forceinline__ int bank_owner(int beta) { return beta >> 2; }
+__device__ __forceinline__ int bank_local(int beta) { return beta & 3; }
 
 
 __global__ void __launch_bounds__(BL_THREADS, 2)
@@ -218,11 +229,12 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
     extern __shared__ __align__(16) unsigned char smem[];
     __shared__ TileS S;
     __shared__ int s_bad, s_nonuni, s_clo, s_chi;
+    __shared__ uint32_t s_rows[BL_WARPS], s_row0;
     __shared__ double s_h0;
-    float4* XY = reinterpret_cast<float4*>(smem + BL_OFF_XY);
-    float4* ZT = reinterpret_cast<float4*>(smem + BL_OFF_ZT);
-    float* XYf = reinterpret_cast<float*>(XY);
-    float* ZTf = reinterpret_cast<float*>(ZT);
+    float* X = reinterpret_cast<float*>(smem + BL_OFF_X);
+    float* Y = reinterpret_cast<float*>(smem + BL_OFF_Y);
+    float* Z = reinterpret_cast<float*>(smem + BL_OFF_Z);
+    float* Tc = reinterpret_cast<float*>(smem + BL_OFF_T);
     uint16_t* Lf = reinterpret_cast<uint16_t*>(smem + BL_OFF_L);       // [k * BL_THREADS + tid]
     uint16_t* B = reinterpret_cast<uint16_t*>(smem + BL_OFF_B);        // [(b * LIST_BS + k) * BL_THREADS + tid]
     uint16_t* colofs = reinterpret_cast<uint16_t*>(smem + BL_OFF_COL); // [range][COLW]
@@ -252,12 +264,20 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
         }
         const int ncolv = td.cxb - td.cxa + 3;                          // virtual columns 0 .. ncolv-1
         // tile origin (centre of the tile's cell block) for the fp32 relative coordinates
-        const double ox = g.lo[0] + (0.5 * (td.cxa + td.cxb + 1)) / g.inv[0];
-        const double oy = g.lo[1] + (td.y0 + 0.5 * td.nyr) / g.inv[1];
-        const double oz = g.lo[2] + (td.z0 + 0.5 * td.nzr) / g.inv[2];
-        // bound on the absolute error of an fp32 relative coordinate difference: 2 roundings of magnitude <= ext
-        const float ext = (float)fmax(fmax((0.5 * ncolv + 0.5) / g.inv[0], 2.5 / g.inv[1]), 2.5 / g.inv[2]);
+        const double ex = g.L[0] / g.nc[0], ey = g.L[1] / g.nc[1], ez = g.L[2] / g.nc[2];
+        const double ox = g.lo[0] + (0.5 * (td.cxa + td.cxb + 1)) * ex;
+        const double oy = g.lo[1] + (td.y0 + 0.5 * td.nyr) * ey;
+        const double oz = g.lo[2] + (td.z0 + 0.5 * td.nzr) * ez;
+        // Bound on the absolute error of an fp32 relative coordinate difference: every staged coordinate lies within
+        // ext of the origin (checked while staging: particles clamped into an edge cell from outside an open box do not,
+        // and send the unit to the general kernels), so each of the two operands carries one rounding <= 2^-24 ext and
+        // the difference another one: 3 x 2^-24 ext < E.
+        const float ext = (float)fmax(fmax((0.5 * ncolv + 0.5) * ex, 2.5 * ey), 2.5 * ez);
+        const float extc = ext * 1.0001f;
         const float E = ext * 2.4e-7f;                                  // 4 * 2^-24 * ext
+        // |r2_fp32 - r2| <= 2 (|dx| + |dy| + |dz|) E + 3 E^2 + the roundings of the three fused steps (relative 2^-24 each,
+        // of max(r2, T) <= 1.1 T: covered by the relative margin 1e-5 of the thresholds) <= 2 sqrt(3) Rmax' E + 3 E^2 near a
+        // support boundary (r <= Rmax (1 + 1e-5) + ...)
         const float Am = 4.4f * Rmax * E + 5.0f * E * E;
         __syncthreads();
 
@@ -275,6 +295,7 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
         uint32_t i = 0, s_self = 0xFFFFFFFFu;
         double xa = 0, ya = 0, za = 0, ha = 0;
         int tcol = 0, try_ = 0, trz = 0;
+        bool tbad = false;
         if (active) {
             int e;
             i = tile_target(td, S, tgt, &e);
@@ -285,9 +306,12 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
             xa = xy.x; ya = xy.y; za = zh.x; ha = zh.y;
             for (int q = 0; q < (int)S.nranges; ++q)
                 if (i >= S.r_vstart[q] && i < S.r_vend[q]) s_self = S.r_base[q] + (i - S.r_vstart[q]);
+            tbad = A.coinc[i] != 0;                                     // a twin at distance 0: left to the general kernels (A11)
         }
         // an inactive thread sits far away from everything: it never hits
         const float fax = active ? (float)(xa - ox) : -3.0e18f, fay = (float)(ya - oy), faz = (float)(za - oz);
+        if (active && !(fabsf(fax) <= extc && fabsf(fay) <= extc && fabsf(faz) <= extc)) tbad = true;
+        if (tbad) s_bad = 1;
         const float Ra = 2.0f * (float)ha;
         const float Ta = Ra * Ra;
         const float Ta_hi = fmaf(Ta, 1.00001f, Am), Ta_lo = fmaf(Ta, 0.99999f, -Am);
@@ -305,18 +329,20 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
         if (tid == 0) s_h0 = ha;                                        // the half's first target: always there
         __syncthreads();
 
-        // ---- stage the candidates of virtual columns [s_clo, s_chi + 2] as slot pairs: one warp per range; whole pairs
-        //      only (a pair cut by the window's edge is staged in full), the odd pad slot of a range is put out of reach
+        // ---- stage the candidates of virtual columns [s_clo, s_chi + 2], whole blocks of 8 slots: one warp per range;
+        //      the pad slots of a range and the slots of a block that lie outside the window's columns but inside the
+        //      range are real particles two or more cells away from every target that can reach the block (never a
+        //      neighbour); slots past the end of the range are put out of reach
         {
             const unsigned long long h0 = (unsigned long long)__double_as_longlong(s_h0);
             const int clo = s_clo, chi = s_chi + 2;
-            bool nonuni = false;
+            bool nonuni = false, far = false;
             for (int q = warp; q < (int)S.nranges; q += BL_WARPS) {
                 const int4 ge = S.r_geo[q];
                 const int jlo = max(0, min(ge.y, clo - ge.z)), jhi = max(0, min(ge.y, chi + 1 - ge.z));
                 if (jhi <= jlo) continue;
                 const uint32_t vs = S.r_vstart[q], len = S.r_vend[q] - vs, base = S.r_base[q];
-                const uint32_t ka = (uint32_t)colofs[q * COLW + jlo] & ~1u, kb = ((uint32_t)colofs[q * COLW + jhi] + 1u) & ~1u;
+                const uint32_t ka = (uint32_t)colofs[q * COLW + jlo] & ~7u, kb = ((uint32_t)colofs[q * COLW + jhi] + 7u) & ~7u;
                 const double shx = S.r_shift[q][0] * g.L[0], shy = S.r_shift[q][1] * g.L[1], shz = S.r_shift[q][2] * g.L[2];
                 for (uint32_t k = ka + lane; k < kb; k += 32) {
                     float fx = 3.0e18f, fy = 3.0e18f, fz = 3.0e18f, T = 0.0f;
@@ -328,49 +354,55 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
                         const float Rb = 2.0f * (float)zh.y;
                         T = Rb * Rb;
                         nonuni |= (unsigned long long)__double_as_longlong(zh.y) != h0;
+                        far |= !(fabsf(fx) <= extc && fabsf(fy) <= extc && fabsf(fz) <= extc);
                     }
-                    const uint32_t s = base + k, o = (s >> 1) * 4 + (s & 1);
-                    XYf[o] = fx; XYf[o + 2] = fy; ZTf[o] = fz; ZTf[o + 2] = T;
+                    const uint32_t s = base + k;
+                    X[s] = fx; Y[s] = fy; Z[s] = fz; Tc[s] = T;
                 }
             }
             if (nonuni) s_nonuni = 1;                                   // some staged candidate differs from the first target's h
+            if (far) s_bad = 1;                                         // the error bound does not hold: general kernels
         }
         __syncthreads();
         const bool uni = s_nonuni == 0;
 
-        // ---- scan: fp32 prefilter on slot pairs (FADD2/FFMA2: two candidates per instruction).  The two threads of a
-        //      target take alternate pairs (slots 4i+2u, 4i+2u+1); all lanes of the same parity read the same pair
-        //      (shared-memory broadcast).  A hit (r2 below the support of the larger h, error bound added) goes straight
-        //      to the thread's bucket of the slot's bank: pair p feeds buckets (p & 2) and (p & 2) + 1, so with the loop
-        //      unrolled by two pairs the bucket of every append is a compile-time choice.  A hit that is not certain
-        //      (0 < r2 < Ta_lo, uniform-h tiles only) carries LIST_RECHECK.
+        // ---- scan (see the header).  All lanes of one parity read the same 16 bytes (shared-memory broadcast).
         const uint32_t bk0 = (uint32_t)__cvta_generic_to_shared(B + tid);
         constexpr uint32_t BROW = 2u * BL_THREADS;                    // bytes per bucket row
-        uint32_t nflag = 0;                                             // flagged hits of this thread
         uint32_t bp0 = bk0, bp1 = bk0 + LIST_BS * BROW, bp2 = bk0 + 2 * LIST_BS * BROW, bp3 = bk0 + 3 * LIST_BS * BROW;
         const uint32_t e0 = bk0 + LIST_BC * BROW, e1 = e0 + LIST_BS * BROW, e2 = e1 + LIST_BS * BROW, e3 = e2 + LIST_BS * BROW;
+        float tmin = 3.0e38f;                                           // min |t| over the tested candidates
         if (cmax >= 0) {
             const int wv_lo = cmin, wv_hi = cmax + 2;                   // virtual columns [tcol, tcol + 2] around each target
             const f32x2 ax2 = pk2(fax, fax), ay2 = pk2(fay, fay), az2 = pk2(faz, faz);
-            const f32x2 one_eps = pk2(1.00001f, 1.00001f), am2 = pk2(Am, Am);
-            const float half_lo = 0.5f * Ta_lo;
-            // one pair: test both slots, append to buckets (pa_, pb_) whose row pointers are clamped at the trash row
-            auto pair_uni = [&](uint32_t p, const float4 c0, const float4 c1, uint32_t& qa, uint32_t qa_end, uint32_t& qb, uint32_t qb_end) {
-                const f32x2 dx = sub2(ax2, pk2(c0.x, c0.y)), dy = sub2(ay2, pk2(c0.z, c0.w)), dz = sub2(az2, pk2(c1.x, c1.y));
-                float r0, r1;
-                unpk2(fma2(dz, dz, fma2(dy, dy, mul2(dx, dx))), r0, r1);
-                append_flag(r0, Ta_hi, half_lo, qa, qa_end, 2 * p, nflag);
-                append_flag(r1, Ta_hi, half_lo, qb, qb_end, 2 * p + 1, nflag);
+            const f32x2 nT2 = pk2(-Ta_hi, -Ta_hi);
+            const float4* X4 = reinterpret_cast<const float4*>(X) + u;   // [2 b]: slots 8 b + 4 u ..
+            const float4* Y4 = reinterpret_cast<const float4*>(Y) + u;
+            const float4* Z4 = reinterpret_cast<const float4*>(Z) + u;
+            const float4* T4 = reinterpret_cast<const float4*>(Tc) + u;
+            auto block_uni = [&](uint32_t b) {
+                const float4 x = X4[2 * b], y = Y4[2 * b], z = Z4[2 * b];
+                const f32x2 dx0 = sub2(ax2, pk2(x.x, x.y)), dy0 = sub2(ay2, pk2(y.x, y.y)), dz0 = sub2(az2, pk2(z.x, z.y));
+                const f32x2 dx1 = sub2(ax2, pk2(x.z, x.w)), dy1 = sub2(ay2, pk2(y.z, y.w)), dz1 = sub2(az2, pk2(z.z, z.w));
+                float t0, t1, t2, t3;
+                unpk2(fma2(dz0, dz0, fma2(dy0, dy0, fma2(dx0, dx0, nT2))), t0, t1);
+                unpk2(fma2(dz1, dz1, fma2(dy1, dy1, fma2(dx1, dx1, nT2))), t2, t3);
+                append_if_neg(t0, bp0, b); append_if_neg(t1, bp1, b); append_if_neg(t2, bp2, b); append_if_neg(t3, bp3, b);
+                tmin = fminf(fminf(tmin, fabsf(t0)), fminf(fabsf(t1), fminf(fabsf(t2), fabsf(t3))));
             };
-            auto pair_gen = [&](uint32_t p, uint32_t& qa, uint32_t qa_end, uint32_t& qb, uint32_t qb_end) {
-                const float4 c0 = XY[p], c1 = ZT[p];
-                const f32x2 dx = sub2(ax2, pk2(c0.x, c0.y)), dy = sub2(ay2, pk2(c0.z, c0.w)), dz = sub2(az2, pk2(c1.x, c1.y));
-                float r0, r1, h0, h1;
-                unpk2(fma2(dz, dz, fma2(dy, dy, mul2(dx, dx))), r0, r1);
-                unpk2(fma2(pk2(fmaxf(Ta, c1.z), fmaxf(Ta, c1.w)), one_eps, am2), h0, h1);
-                append_flag(r0, h0, -1.0f, qa, qa_end, 2 * p, nflag);    // half_lo < 0: always flagged
-                append_flag(r1, h1, -1.0f, qb, qb_end, 2 * p + 1, nflag);
+            auto block_gen = [&](uint32_t b) {
+                const float4 x = X4[2 * b], y = Y4[2 * b], z = Z4[2 * b], T = T4[2 * b];
+                const f32x2 dx0 = sub2(ax2, pk2(x.x, x.y)), dy0 = sub2(ay2, pk2(y.x, y.y)), dz0 = sub2(az2, pk2(z.x, z.y));
+                const f32x2 dx1 = sub2(ax2, pk2(x.z, x.w)), dy1 = sub2(ay2, pk2(y.z, y.w)), dz1 = sub2(az2, pk2(z.z, z.w));
+                // support of the larger h, error bound added
+                const float n0 = -fmaf(fmaxf(Ta, T.x), 1.00001f, Am), n1 = -fmaf(fmaxf(Ta, T.y), 1.00001f, Am);
+                const float n2 = -fmaf(fmaxf(Ta, T.z), 1.00001f, Am), n3 = -fmaf(fmaxf(Ta, T.w), 1.00001f, Am);
+                float t0, t1, t2, t3;
+                unpk2(fma2(dz0, dz0, fma2(dy0, dy0, fma2(dx0, dx0, pk2(n0, n1)))), t0, t1);
+                unpk2(fma2(dz1, dz1, fma2(dy1, dy1, fma2(dx1, dx1, pk2(n2, n3)))), t2, t3);
+                append_if_neg(t0, bp0, b); append_if_neg(t1, bp1, b); append_if_neg(t2, bp2, b); append_if_neg(t3, bp3, b);
             };
+            auto clamp = [&]() { bp0 = min(bp0, e0); bp1 = min(bp1, e1); bp2 = min(bp2, e2); bp3 = min(bp3, e3); };
             for (int q = 0; q < (int)S.nranges; ++q) {
                 const int row = S.r_shift[q][3], ry = row & 3, rz = row >> 2;
                 if (ry < ymin || ry > ymax + 2 || rz < zmin || rz > zmax + 2) continue;
@@ -379,99 +411,93 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
                 if (jhi <= jlo) continue;
                 const uint32_t sa = S.r_base[q] + colofs[q * COLW + jlo];
                 const uint32_t sb = S.r_base[q] + colofs[q * COLW + jhi];
-                // pairs [sa/2, (sb+1)/2): a pair cut by a column boundary brings in a slot of the same row two or
-                // more cells away (never a neighbour, never scanned twice); a range's pad slot is out of reach
-                const uint32_t pa = sa >> 1, pb = (sb + 1u) >> 1;
-                uint32_t p = pa + ((pa ^ (uint32_t)u) & 1u);
+                uint32_t b = sa >> 3;
+                const uint32_t b1 = (sb + 7u) >> 3;                     // blocks [b, b1): all staged (the unit's window contains the warp's)
                 if (uni) {
-                    if ((p & 2u) && p < pb) { pair_uni(p, XY[p], ZT[p], bp2, e2, bp3, e3); p += 2; }
-                    // software pipeline: the records of the next two pairs are loaded while the current two are tested
-                    // (indices clamped to the staged arrays; a clamped load is never used)
-                    constexpr uint32_t PLAST = TILE_CMAXP / 2 - 1;
-                    float4 a0 = XY[min(p, PLAST)], a1 = ZT[min(p, PLAST)], b0 = XY[min(p + 2, PLAST)], b1 = ZT[min(p + 2, PLAST)];
-#pragma unroll 2
-                    for (; p + 2 < pb; p += 4) {
-                        const uint32_t pn = min(p + 4, PLAST), pm = min(p + 6, PLAST);
-                        const float4 na0 = XY[pn], na1 = ZT[pn], nb0 = XY[pm], nb1 = ZT[pm];
-                        pair_uni(p, a0, a1, bp0, e0, bp1, e1);
-                        pair_uni(p + 2, b0, b1, bp2, e2, bp3, e3);
-                        a0 = na0; a1 = na1; b0 = nb0; b1 = nb1;
+                    for (; b + LIST_TRASH <= b1; b += LIST_TRASH) {
+#pragma unroll
+                        for (int k = 0; k < LIST_TRASH; ++k) block_uni(b + k);
+                        clamp();
                     }
-                    if (p < pb) pair_uni(p, a0, a1, bp0, e0, bp1, e1);
+                    for (; b < b1; ++b) block_uni(b);
+                    clamp();
                 } else {
-                    if ((p & 2u) && p < pb) { pair_gen(p, bp2, e2, bp3, e3); p += 2; }
-#pragma unroll 2
-                    for (; p + 2 < pb; p += 4) { pair_gen(p, bp0, e0, bp1, e1); pair_gen(p + 2, bp2, e2, bp3, e3); }
-                    if (p < pb) pair_gen(p, bp0, e0, bp1, e1);
+                    for (; b + LIST_TRASH <= b1; b += LIST_TRASH) {
+#pragma unroll
+                        for (int k = 0; k < LIST_TRASH; ++k) block_gen(b + k);
+                        clamp();
+                    }
+                    for (; b < b1; ++b) block_gen(b);
+                    clamp();
                 }
             }
         }
         asm volatile("" ::: "memory");                                  // the appends above wrote the buckets
-        // ---- settle the flagged hits, bucket by bucket, in place.  Certain when the fp32 r2 is clear of every support
-        //      boundary by more than the error bound; otherwise (and at r = 0, which includes the target itself) the
-        //      exact fp64 contract predicate decides (O2/A12).
+        // ---- settle.  An entry is the block number of a hit of the fp32 test; its slot is 8 block + 4 u + bucket.
         uint32_t cnt = 0, ng = 0;                                       // cnt: 4 x 8-bit bucket fills
         bool ovf = (bp0 >= e0) || (bp1 >= e1) || (bp2 >= e2) || (bp3 >= e3), coinc = false;
-        // In a uniform-h tile the target itself (r = 0) is normally the only flagged hit, met by the thread that scans its
-        // slot pair: then the settle pass is a removal of that one entry from its bucket.
-        const bool sees_self = active && (((s_self >> 1) & 1u) == (uint32_t)u);
-        const bool full_settle = __any_sync(0xFFFFFFFFu, nflag != (sees_self ? 1u : 0u));
+        // Certain scan: no tested candidate within the uncertainty band of the support boundary, i.e. every fp32 decision
+        // holds for the exact predicate too.  |t| >= band  <=>  r2_fp32 outside [T_lo, T_hi + (T_hi - T_lo)).
+        const bool certain = uni && tmin >= (Ta_hi - Ta_lo);
+        const bool sees_self = active && ((s_self >> 2) & 1u) == (uint32_t)u;
+        const bool full_settle = __any_sync(0xFFFFFFFFu, !certain && !ovf);
         if (!full_settle) {
+            // the target itself (r = 0) is met by the thread that owns its bank: take that one entry out of its bucket
             const uint32_t n0 = (bp0 - bk0) / BROW, n1 = (bp1 - (bk0 + LIST_BS * BROW)) / BROW;
             const uint32_t n2 = (bp2 - (bk0 + 2 * LIST_BS * BROW)) / BROW, n3 = (bp3 - (bk0 + 3 * LIST_BS * BROW)) / BROW;
             cnt = n0 | (n1 << 8) | (n2 << 16) | (n3 << 24);
-            if (sees_self) {
-                const int b = bank_local((int)(s_self & 7u));
+            if (sees_self && !ovf) {
+                const int b = (int)(s_self & 3u);
                 uint16_t* bb = B + (size_t)b * LIST_BS * BL_THREADS + tid;
-                const uint32_t nb = (cnt >> (8 * b)) & 0xFFu;
+                const uint32_t nb = (cnt >> (8 * b)) & 0xFFu, want = s_self >> 3;
                 uint32_t k = 0;
-                while (k < nb && (bb[k * BL_THREADS] & 0x7FFFu) != s_self) ++k;
+                while (k < nb && bb[k * BL_THREADS] != want) ++k;
                 if (k < nb) {                                           // the last entry takes its place (order is free)
                     bb[k * BL_THREADS] = bb[(nb - 1) * BL_THREADS];
                     cnt -= 1u << (8 * b);
                 }
             }
             ng = (cnt & 0xFFu) + ((cnt >> 8) & 0xFFu) + ((cnt >> 16) & 0xFFu) + (cnt >> 24);
-        } else
+        } else if (!ovf) {
 #pragma unroll
-        for (int b = 0; b < 4; ++b) {
-            const uint32_t nb = ((b == 0 ? bp0 : b == 1 ? bp1 : b == 2 ? bp2 : bp3) - (bk0 + b * LIST_BS * BROW)) / BROW;
-            uint16_t* bb = B + (size_t)b * LIST_BS * BL_THREADS + tid;
-            uint32_t w = 0;
-            for (uint32_t k = 0; k < nb; ++k) {
-                const uint32_t v = bb[k * BL_THREADS], s = v & 0x7FFFu;
-                bool in_s = true, in_g = true;
-                if (v & LIST_RECHECK) {
-                    const float4 c0 = XY[s >> 1], c1 = ZT[s >> 1];
-                    const bool od = (s & 1u) != 0;
-                    const float dx = fax - (od ? c0.y : c0.x), dy = fay - (od ? c0.w : c0.z), dz = faz - (od ? c1.y : c1.x);
+            for (int b = 0; b < 4; ++b) {
+                const uint32_t nb = ((b == 0 ? bp0 : b == 1 ? bp1 : b == 2 ? bp2 : bp3) - (bk0 + b * LIST_BS * BROW)) / BROW;
+                uint16_t* bb = B + (size_t)b * LIST_BS * BL_THREADS + tid;
+                uint32_t w = 0;
+                for (uint32_t k = 0; k < nb; ++k) {
+                    const uint32_t blk = bb[k * BL_THREADS], s = (blk << 3) + 4u * (uint32_t)u + (uint32_t)b;
+                    bool in_s = true, in_g = true;
+                    const float dx = fax - X[s], dy = fay - Y[s], dz = faz - Z[s];
                     const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                    const float Tm = fmaxf(Ta, od ? c1.w : c1.z);
+                    const float Tm = fmaxf(Ta, Tc[s]);
                     if (r2 < fmaf(Tm, 0.99999f, -Am) && (r2 < Ta_lo || r2 >= Ta_hi) && r2 > 0.0f) {
-                        in_g = r2 < Ta_lo;
+                        in_g = r2 < Ta_lo;                              // certain member of N_sym; N_gather decided with the same margin
                     } else if (s == s_self) {
                         in_s = false;
                     } else {
                         int q = 0;
                         while (q + 1 < (int)S.nranges && S.r_base[q + 1] <= s) ++q;
-                        const uint32_t gi = S.r_vstart[q] + (s - S.r_base[q]);
-                        const double2 xy = A.p0[gi], zh = A.p1[gi];
-                        const double ex = min_image(__dsub_rn(xa, xy.x), g.per[0], g.L[0], g.halfL[0]);
-                        const double ey = min_image(__dsub_rn(ya, xy.y), g.per[1], g.L[1], g.halfL[1]);
-                        const double ez = min_image(__dsub_rn(za, zh.x), g.per[2], g.L[2], g.halfL[2]);
-                        const double e2x = r2_exact(ex, ey, ez);
-                        in_s = gi != i && e2x < support2(fmax(ha, zh.y));
-                        in_g = in_s && e2x < support2(ha);
-                        if (in_s && !(e2x > 0.0)) coinc = true;         // coincident particles: left to the general kernels (A11)
+                        const uint32_t k2 = s - S.r_base[q];
+                        if (k2 >= S.r_vend[q] - S.r_vstart[q]) {
+                            in_s = false;                               // pad slot (cannot hit; kept for safety)
+                        } else {
+                            const uint32_t gi = S.r_vstart[q] + k2;
+                            const double2 xy = A.p0[gi], zh = A.p1[gi];
+                            const double ex2 = min_image(__dsub_rn(xa, xy.x), g.per[0], g.L[0], g.halfL[0]);
+                            const double ey2 = min_image(__dsub_rn(ya, xy.y), g.per[1], g.L[1], g.halfL[1]);
+                            const double ez2 = min_image(__dsub_rn(za, zh.x), g.per[2], g.L[2], g.halfL[2]);
+                            const double e2x = r2_exact(ex2, ey2, ez2);
+                            in_s = gi != i && e2x < support2(fmax(ha, zh.y));
+                            in_g = in_s && e2x < support2(ha);
+                            if (in_s && !(e2x > 1.0e-290)) coinc = true;    // (near-)coincident particles: left to the general kernels (A11)
+                        }
                     }
-                    if (in_s) bb[w * BL_THREADS] = (uint16_t)s;
-                } else if (w != k) {
-                    bb[w * BL_THREADS] = (uint16_t)s;
+                    if (in_s) bb[w * BL_THREADS] = (uint16_t)blk;
+                    w += in_s ? 1u : 0u;
+                    ng += (in_s && in_g) ? 1u : 0u;
                 }
-                w += in_s ? 1u : 0u;
-                ng += (in_s && in_g) ? 1u : 0u;
+                cnt |= w << (8 * b);
             }
-            cnt |= w << (8 * b);
         }
         if (ovf || coinc) s_bad = 1;
         // ---- split every bank bucket of the target between its two threads (alternate entries)
@@ -491,12 +517,26 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
 #pragma unroll
         for (int o = 16; o; o >>= 1) R = max(R, __shfl_xor_sync(0xFFFFFFFFu, R, o));
         R = (R + 3u) & ~3u;
-        // list storage: one fixed block of LIST_RMAX rounds per (tile, warp) -- no allocation, placement is deterministic
-        const unsigned long long off = ((unsigned long long)tile * TILE_WARPS + twarp) * (unsigned long long)(LIST_RMAX / 4) * 32;
-        if (lane == 0 && R > (uint32_t)LIST_RMAX) s_bad = 1;
+        if (lane == 0) {
+            if (R > (uint32_t)LIST_RMAX) s_bad = 1;
+            s_rows[warp] = R >> 2;
+        }
+        __syncthreads();
+        // list storage: rows of 32 lanes x 4 slots, one allocation per unit (its warps back to back) from the pool counter.
+        // Placement depends on the order in which units get there; the contents of a warp's rows do not.
+        if (tid == 0 && s_bad == 0) {
+            uint32_t tot = 0;
+#pragma unroll
+            for (int w = 0; w < BL_WARPS; ++w) tot += s_rows[w];
+            const unsigned long long r0 = atomicAdd(&A.ctr[CTR_POOL], (unsigned long long)tot);
+            if (r0 + tot > (unsigned long long)A.pool_rows) s_bad = 1;  // pool exhausted: general kernels
+            s_row0 = (uint32_t)r0;
+        }
         __syncthreads();
         const bool bad = s_bad != 0;
         if (!bad) {
+            uint32_t row0 = s_row0;
+            for (int w = 0; w < warp; ++w) row0 += s_rows[w];
             // ---- emit my half-list in scheduled order (see the header): phase t = rounds [tR/8, (t+1)R/8) in bank
             //      (j + t) & 7; what a phase cannot hold (overflow) fills the holes of other phases; the rest are dummies.
             // R = 8 m + 4 e (e = 0, 1): phase t starts at t m + e (t >> 1) and holds m + e (t & 1) rounds.
@@ -517,22 +557,24 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
                 // my entries of bank beta: indices f, f+2, ... of the bucket of thread bank_owner(beta)
                 bq[t] = Bp + (bank_local(beta) * LIST_BS + ((u + beta) & 1)) * BL_THREADS + bank_owner(beta);
             }
-            // pass 1 (lockstep): every phase takes its own bank's entries up to its capacity; a hole gets the dummy slot
-            // of the phase's bank
+            // pass 1 (lockstep): every phase takes its own bank's entries up to its capacity (an entry is a block number:
+            // slot = 8 block + bank); a hole gets the dummy slot of the phase's bank
             for (uint32_t k = 0; k < m8; ++k) {
 #pragma unroll
                 for (int t = 0; t < 8; ++t) {
-                    uint16_t item = (uint16_t)(TILE_CMAX + ((j + t) & 7));
-                    if (k < own[t]) item = bq[t][2 * k * BL_THREADS];
-                    out[((uint32_t)t * m8 + (e4 ? (uint32_t)(t >> 1) : 0u) + k) * BL_THREADS] = item;
+                    const uint32_t beta = (uint32_t)(j + t) & 7u;
+                    uint32_t item = (uint32_t)TILE_CMAX + beta;
+                    if (k < own[t]) item = ((uint32_t)bq[t][2 * k * BL_THREADS] << 3) + beta;
+                    out[((uint32_t)t * m8 + (e4 ? (uint32_t)(t >> 1) : 0u) + k) * BL_THREADS] = (uint16_t)item;
                 }
             }
             if (e4) {
 #pragma unroll
                 for (int t = 1; t < 8; t += 2) {
-                    uint16_t item = (uint16_t)(TILE_CMAX + ((j + t) & 7));
-                    if (m8 < own[t]) item = bq[t][2 * m8 * BL_THREADS];
-                    out[((uint32_t)t * m8 + (uint32_t)(t >> 1) + m8) * BL_THREADS] = item;
+                    const uint32_t beta = (uint32_t)(j + t) & 7u;
+                    uint32_t item = (uint32_t)TILE_CMAX + beta;
+                    if (m8 < own[t]) item = ((uint32_t)bq[t][2 * m8 * BL_THREADS] << 3) + beta;
+                    out[((uint32_t)t * m8 + (uint32_t)(t >> 1) + m8) * BL_THREADS] = (uint16_t)item;
                 }
             }
             // the left-over entries go into the holes, phase by phase (a phase has either holes or left-overs)
@@ -541,17 +583,18 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
                 uint32_t hrem = 0;
 #pragma unroll
                 for (int t = 0; t < 8; ++t) {
+                    const uint32_t beta = (uint32_t)(j + t) & 7u;
                     for (uint32_t e = 0; e < ovr[t]; ++e) {
                         while (hrem == 0 && th < 7) { ++th; hrem = (Hw >> (4 * th)) & 15u; }
                         if (hrem == 0) break;                           // cannot happen: n_lane <= R
                         const uint32_t pos = (((uint32_t)(th + 1) * R) >> 3) - hrem;
                         --hrem;
-                        out[pos * BL_THREADS] = bq[t][2 * (own[t] + e) * BL_THREADS];
+                        out[pos * BL_THREADS] = (uint16_t)(((uint32_t)bq[t][2 * (own[t] + e) * BL_THREADS] << 3) + beta);
                     }
                 }
             }
             // pass 2: pack 4 rounds per 8-byte store
-            uint2* blk = A.pool + off + lane;
+            uint2* blk = A.pool + (size_t)row0 * 32 + lane;
             for (uint32_t r4 = 0; r4 < R; r4 += 4) {
                 const uint32_t e0 = out[r4 * BL_THREADS], e1 = out[(r4 + 1) * BL_THREADS];
                 const uint32_t e2 = out[(r4 + 2) * BL_THREADS], e3 = out[(r4 + 3) * BL_THREADS];
@@ -559,7 +602,7 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
             }
             if (u == 0) A.lcount[(size_t)tile * TILE_T + tgt] = active ? (ng | (nsym << 16)) : 0u;
             if (active && u == 0) A.fast[i] = 1;
-            if (lane == 0) A.winfo[(size_t)tile * TILE_WARPS + twarp] = make_uint2((uint32_t)off, R);
+            if (lane == 0) A.winfo[(size_t)tile * TILE_WARPS + twarp] = make_uint2(row0, R);
         }
         if (tid == 0) {
             const uint32_t bits = (bad ? 0u : (TILE_FLAG_OK0 << half)) | (s_nonuni ? TILE_FLAG_NONUNI : 0u);
@@ -620,7 +663,7 @@ k_tiled_export(DevGrid g, ExportArgs A) {
         }
         uint2 wi = A.winfo[(size_t)tile * TILE_WARPS + warp];
         if (!half_ok) wi.y = 0u;
-        const uint2* lp = A.pool + wi.x + lane;
+        const uint2* lp = A.pool + (size_t)wi.x * 32 + lane;
         uint32_t cnt = 0;
         uint64_t dsum = 0, dxr = 0;
         // mode 1 needs the first half's count before the second half writes: two passes (count, then write)
@@ -692,6 +735,13 @@ cudaError_t launch_tiled_export(Ctx* c, int mode, int symmetric, uint32_t* ocoun
 }
 
 // ------------------------------------------------------------------------------------------- launcher
+cudaError_t tiled_set_attributes(Ctx* c) {
+    cudaError_t e = cudaFuncSetAttribute(k_build_lists, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BL_SMEM);
+    if (e == cudaSuccess) e = sweeps_set_attributes();
+    if (e == cudaSuccess) c->tl.attr_device = c->device;
+    return e;
+}
+
 cudaError_t launch_build_tiles(Ctx* c, cudaStream_t st) {
     Tiled& t = c->tl;
     t.enabled = false;
@@ -708,6 +758,7 @@ cudaError_t launch_build_tiles(Ctx* c, cudaStream_t st) {
     cudaError_t e;
     if ((e = cudaMemsetAsync(t.ctr, 0, sizeof(unsigned long long) * CTR_COUNT, st)) != cudaSuccess) return e;
     if ((e = cudaMemsetAsync(t.fast, 0, (size_t)c->n, st)) != cudaSuccess) return e;
+    if ((e = launch_mark_coincident(c, st)) != cudaSuccess) return e;
     CellTable ct{c->cell_start, c->cell_end};
     const int blocks = (int)((nb * 32 + 255) / 256);
     k_make_tiles<false><<<blocks, 256, 0, st>>>(c->dg, ct, c->hglob, t.bcount, t.tiles, (uint32_t)t.tile_cap, t.ctr);
@@ -715,13 +766,8 @@ cudaError_t launch_build_tiles(Ctx* c, cudaStream_t st) {
     k_make_tiles<true><<<blocks, 256, 0, st>>>(c->dg, ct, c->hglob, t.bcount, t.tiles, (uint32_t)t.tile_cap, t.ctr);
     k_tile_tables<<<t.sms * 8, 128, 0, st>>>(c->dg, ct, t.tiles, t.ctr, t.tiletab);
     if ((e = cudaMemsetAsync(t.tflags, 0, sizeof(uint32_t) * (size_t)t.tile_cap, st)) != cudaSuccess) return e;
-    static bool attr_done = false;
-    if (!attr_done) {
-        if ((e = cudaFuncSetAttribute(k_build_lists, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BL_SMEM)) != cudaSuccess) return e;
-        attr_done = true;
-    }
-    ListArgs A{c->pk.p0, c->pk.p1, t.tiles, t.ctr, t.pool, t.winfo, t.lcount, t.tflags, t.tiletab, t.fast,
-               c->hglob, c->dev_status};
+    ListArgs A{c->pk.p0, c->pk.p1, t.tiles, t.ctr, t.pool, (uint32_t)t.pool_rows, t.winfo, t.lcount, t.tflags, t.tiletab, t.fast,
+               t.coinc, c->hglob, c->dev_status};
     k_build_lists<<<t.sms * 2, BL_THREADS, BL_SMEM, st>>>(c->dg, ct, A);
     c->launches += 4;
     t.enabled = true;

@@ -33,7 +33,7 @@ constexpr int TILE_CMAXP = TILE_CMAX + TILE_NDUMMY;   // 2240: multiple of 8, so
 constexpr int TILE_MAXR = 32;        // candidate ranges: 4 x 4 rows x (1 or 2 pieces, at most 16 rows wrap)
 constexpr int TILE_BXMAX = 24;       // max columns (cells along x) of a tile
 constexpr int TILE_MAXCELL = 4 * TILE_BXMAX;
-constexpr int LIST_BC = 24;          // builder: capacity of one (thread, bank) bucket
+constexpr int LIST_BC = 24;          // builder: capacity of one (target, bank) bucket
 constexpr int LIST_RMAX = 80;        // max rounds of a warp's schedule = builder's flat-list rows (longer -> tile served by the general kernels)
 
 struct TileDesc {                    // 24 bytes
@@ -140,7 +140,7 @@ __device__ __forceinline__ void tile_setup(const TileDesc& td, const DevGrid& g,
     if (tid < 32) {
         RangeGeo R;
         const bool valid = tile_range(td, g, ct, tid >> 1, tid & 1, R);
-        const uint32_t len = valid ? ((R.ve - R.vs + 1u) & ~1u) : 0u;  // every range starts on an even slot (list builder: slot pairs)
+        const uint32_t len = valid ? ((R.ve - R.vs + 7u) & ~7u) : 0u;  // every range starts on a slot that is a multiple of 8 (list builder: blocks of 8 slots = the 8 banks)
         // compact the valid ranges to the front, keeping order (ballot + popc), and scan the padded lengths
         const uint32_t mask = __ballot_sync(0xFFFFFFFFu, valid);
         const int pos = __popc(mask & ((1u << tid) - 1u));
