@@ -236,6 +236,7 @@ int spray_build_cells(spray_ctx* ctx, const spray_grid_t* g, spray_kernel_t kern
         c->dg.lo[d] = g->lo[d];
         c->dg.L[d] = g->hi[d] - g->lo[d];
         c->dg.halfL[d] = 0.5 * c->dg.L[d];
+        c->dg.edge[d] = c->dg.L[d] / (double)g->ncell[d];
         c->dg.inv[d] = (double)g->ncell[d] / c->dg.L[d];
         c->dg.nc[d] = g->ncell[d];
         c->dg.per[d] = g->periodic[d] ? 1 : 0;

@@ -11,6 +11,7 @@ struct DevGrid {
     double inv[3];    // ncell_d / L_d  (one fp64 division on the host, same as the contract O1)
     double L[3];      // hi_d - lo_d
     double halfL[3];  // 0.5 * L_d
+    double edge[3];   // L_d / ncell_d: cell edge (tile geometry only, never in a set decision)
     int nc[3];
     int per[3];
 };

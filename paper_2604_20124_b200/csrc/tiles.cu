@@ -184,20 +184,26 @@ constexpr int BL_TGT = TILE_T / 2;
 constexpr int COLW = TILE_BXMAX + 4;
 constexpr int LIST_TRASH = 4;                // trash rows of a bucket: the scan clamps its row pointers once per 4 blocks
 constexpr int LIST_BS = LIST_BC + LIST_TRASH;
-constexpr int LIST_LCAP = LIST_RMAX;         // rows of the schedule staging area (one column per thread)
+constexpr int LIST_LCAP = LIST_RMAX;         // rounds of the schedule staging area
+constexpr int WBLK_CAP = TILE_CMAXP / 8 + 8; // a warp's block list: every staged block at most, padded to a multiple of 4
 constexpr size_t BL_OFF_X = 0;                                                          // float [CMAXP] each: x, y, z relative to the
 constexpr size_t BL_OFF_Y = BL_OFF_X + sizeof(float) * TILE_CMAXP;                      // tile centre, T = (2 h)^2
 constexpr size_t BL_OFF_Z = BL_OFF_Y + sizeof(float) * TILE_CMAXP;
 constexpr size_t BL_OFF_T = BL_OFF_Z + sizeof(float) * TILE_CMAXP;
 constexpr size_t BL_CAND_END = BL_OFF_T + sizeof(float) * TILE_CMAXP;
-constexpr size_t BL_OFF_L = 0;                                                          // u16 [LIST_LCAP][BL_THREADS]: the schedule, written after
-                                                                                        // the scan is over -- shares the space of the candidates
+constexpr size_t BL_OFF_L = 0;                                                          // uint2 [LIST_LCAP / 4][BL_THREADS]: the schedule, 4 rounds per
+                                                                                        // word pair, written after the scan is over -- shares the
+                                                                                        // space of the candidates
 constexpr size_t BL_L_END = BL_OFF_L + sizeof(uint16_t) * LIST_LCAP * BL_THREADS;
 constexpr size_t BL_OFF_B = BL_CAND_END > BL_L_END ? BL_CAND_END : BL_L_END;             // u16 [4][LIST_BS][BL_THREADS]
 constexpr size_t BL_OFF_COL = BL_OFF_B + sizeof(uint16_t) * 4 * LIST_BS * BL_THREADS;   // u16 [MAXR][COLW]
-constexpr size_t BL_SMEM = BL_OFF_COL + sizeof(uint16_t) * TILE_MAXR * COLW;
-static_assert(2 * (BL_SMEM + sizeof(TileS) + 1280) <= 228 * 1024, "list builder: two CTAs per SM");
+constexpr size_t BL_OFF_WB = BL_OFF_COL + sizeof(uint16_t) * TILE_MAXR * COLW;          // u16 [BL_WARPS][WBLK_CAP]
+constexpr size_t BL_SMEM = BL_OFF_WB + sizeof(uint16_t) * BL_WARPS * WBLK_CAP;
+static_assert(2 * (BL_SMEM + 2 * sizeof(TileS) + 1280) <= 228 * 1024, "list builder: two CTAs per SM");
 static_assert(TILE_CMAXP % 8 == 0 && TILE_CMAX % 8 == 0, "blocks of 8 slots");
+static_assert(TILES_WORDS <= 2 * BL_THREADS, "tile table prefetch: two words per thread");
+static_assert(sizeof(TileDesc) == 24, "tile descriptor prefetch: six words");
+static_assert(BL_OFF_WB % 8 == 0 && WBLK_CAP % 4 == 0, "block list rows are read four entries at a time");
 
 // packed fp32 pairs (sm_100 FADD2 / FMUL2 / FFMA2): one instruction tests two candidates
 typedef unsigned long long f32x2;
@@ -217,6 +223,8 @@ __device__ __forceinline__ void append_if_neg(float t, uint32_t& addr, uint32_t 
     // no memory clobber: the loads of the next blocks must be free to move above the store; the buckets are read back
     // only after the fence that follows the scan
 }
+__device__ __forceinline__ uint32_t lds_u16(uint32_t addr) { uint32_t v; asm volatile("ld.shared.u16 %0, [%1];" : "=r"(v) : "r"(addr)); return v; }
+__device__ __forceinline__ void sts_u16(uint32_t addr, uint32_t v) { asm volatile("st.shared.u16 [%0], %1;" :: "r"(addr), "r"(v)); }
 
 // Which thread of a target owns bank beta in the scan (thread u tests slots 8 b + 4 u .. 8 b + 4 u + 3), and the index
 // of that bank among the owner's four buckets.
@@ -227,59 +235,76 @@ __device__ __forceinline__ int bank_local(int beta) { return beta & 3; }
 __global__ void __launch_bounds__(BL_THREADS, 2)
 k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
     extern __shared__ __align__(16) unsigned char smem[];
-    __shared__ TileS S;
+    __shared__ TileS Sb[2];                                             // this unit's tile table / the next unit's, prefetched
+    __shared__ uint32_t s_td[2][6];
     __shared__ int s_bad, s_nonuni, s_clo, s_chi;
-    __shared__ uint32_t s_rows[BL_WARPS], s_row0;
     __shared__ double s_h0;
     float* X = reinterpret_cast<float*>(smem + BL_OFF_X);
     float* Y = reinterpret_cast<float*>(smem + BL_OFF_Y);
     float* Z = reinterpret_cast<float*>(smem + BL_OFF_Z);
     float* Tc = reinterpret_cast<float*>(smem + BL_OFF_T);
-    uint16_t* Lf = reinterpret_cast<uint16_t*>(smem + BL_OFF_L);       // [k * BL_THREADS + tid]
     uint16_t* B = reinterpret_cast<uint16_t*>(smem + BL_OFF_B);        // [(b * LIST_BS + k) * BL_THREADS + tid]
     uint16_t* colofs = reinterpret_cast<uint16_t*>(smem + BL_OFF_COL); // [range][COLW]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    uint16_t* wblk = reinterpret_cast<uint16_t*>(smem + BL_OFF_WB) + warp * WBLK_CAP;
     const int u = tid & 1, j = lane & 7;
     const uint32_t nunits = 2u * (uint32_t)A.ctr[CTR_NTILES];
     const float Rmax = 2.0f * (float)A.hglob[1] * 1.000001f;
+    constexpr uint32_t BROW = 2u * BL_THREADS;                        // bytes per bucket row
 
-    for (uint32_t unit = blockIdx.x; unit < nunits; unit += gridDim.x) {
+    // tile table and descriptor of the first unit; afterwards each unit prefetches the next one's while it works
+    if (blockIdx.x < nunits) {
+        const uint32_t tile = blockIdx.x >> 1;
+        const uint32_t* src = A.tiletab + (size_t)tile * TILES_WORDS;
+        uint32_t* dst = reinterpret_cast<uint32_t*>(&Sb[0]);
+        for (int w = tid; w < TILES_WORDS; w += BL_THREADS) dst[w] = src[w];
+        if (tid < 6) s_td[0][tid] = reinterpret_cast<const uint32_t*>(A.tiles + tile)[tid];
+    }
+    int buf = 0;
+    for (uint32_t unit = blockIdx.x; unit < nunits; unit += gridDim.x, buf ^= 1) {
+        __syncthreads();                                                // previous unit done with smem; this unit's table is in place
+        const TileS& S = Sb[buf];
         const uint32_t tile = unit >> 1;
         const int half = (int)(unit & 1u);
-        const TileDesc td = A.tiles[tile];
+        TileDesc td;
+        {
+            uint32_t* w = reinterpret_cast<uint32_t*>(&td);
+#pragma unroll
+            for (int k = 0; k < 6; ++k) w[k] = s_td[buf][k];
+        }
+        // prefetch: two table words (and one descriptor word) per thread, parked in registers until the end of the unit
+        const uint32_t nunit = unit + gridDim.x;
+        uint32_t pf0 = 0, pf1 = 0, pfd = 0;
+        if (nunit < nunits) {
+            const uint32_t* src = A.tiletab + (size_t)(nunit >> 1) * TILES_WORDS;
+            pf0 = __ldg(src + tid);
+            if (tid + BL_THREADS < TILES_WORDS) pf1 = __ldg(src + tid + BL_THREADS);
+            if (tid < 6) pfd = __ldg(reinterpret_cast<const uint32_t*>(A.tiles + (nunit >> 1)) + tid);
+        }
         const int tgt = half * BL_TGT + (tid >> 1);                     // target index within the tile
         const int twarp = half * BL_WARPS + warp;                       // warp index within the tile
         if (half * BL_TGT >= (int)td.nt) {                              // no target in this half: empty lists
             if (lane == 0) A.winfo[(size_t)tile * TILE_WARPS + twarp] = make_uint2(0u, 0u);
             if (u == 0) A.lcount[(size_t)tile * TILE_T + tgt] = 0u;
             if (tid == 0) atomicOr(&A.tflags[tile], TILE_FLAG_OK0 << half);
-            continue;
-        }
-        __syncthreads();                                                // previous unit done with smem
+        } else {
         if (tid == 0) { s_bad = 0; s_nonuni = 0; s_clo = 1 << 20; s_chi = -1; }
-        {   // tile tables (k_tile_tables)
-            const uint32_t* src = A.tiletab + (size_t)tile * TILES_WORDS;
-            uint32_t* dst = reinterpret_cast<uint32_t*>(&S);
-            for (int w = tid; w < TILES_WORDS; w += BL_THREADS) dst[w] = src[w];
-        }
         const int ncolv = td.cxb - td.cxa + 3;                          // virtual columns 0 .. ncolv-1
         // tile origin (centre of the tile's cell block) for the fp32 relative coordinates
-        const double ex = g.L[0] / g.nc[0], ey = g.L[1] / g.nc[1], ez = g.L[2] / g.nc[2];
-        const double ox = g.lo[0] + (0.5 * (td.cxa + td.cxb + 1)) * ex;
-        const double oy = g.lo[1] + (td.y0 + 0.5 * td.nyr) * ey;
-        const double oz = g.lo[2] + (td.z0 + 0.5 * td.nzr) * ez;
+        const double ox = g.lo[0] + (0.5 * (td.cxa + td.cxb + 1)) * g.edge[0];
+        const double oy = g.lo[1] + (td.y0 + 0.5 * td.nyr) * g.edge[1];
+        const double oz = g.lo[2] + (td.z0 + 0.5 * td.nzr) * g.edge[2];
         // Bound on the absolute error of an fp32 relative coordinate difference: every staged coordinate lies within
         // ext of the origin (checked while staging: particles clamped into an edge cell from outside an open box do not,
         // and send the unit to the general kernels), so each of the two operands carries one rounding <= 2^-24 ext and
         // the difference another one: 3 x 2^-24 ext < E.
-        const float ext = (float)fmax(fmax((0.5 * ncolv + 0.5) * ex, 2.5 * ey), 2.5 * ez);
+        const float ext = (float)fmax(fmax((0.5 * ncolv + 0.5) * g.edge[0], 2.5 * g.edge[1]), 2.5 * g.edge[2]);
         const float extc = ext * 1.0001f;
         const float E = ext * 2.4e-7f;                                  // 4 * 2^-24 * ext
         // |r2_fp32 - r2| <= 2 (|dx| + |dy| + |dz|) E + 3 E^2 + the roundings of the three fused steps (relative 2^-24 each,
         // of max(r2, T) <= 1.1 T: covered by the relative margin 1e-5 of the thresholds) <= 2 sqrt(3) Rmax' E + 3 E^2 near a
-        // support boundary (r <= Rmax (1 + 1e-5) + ...)
+        // support boundary
         const float Am = 4.4f * Rmax * E + 5.0f * E * E;
-        __syncthreads();
 
         // ---- per-range column offsets (slot of the first particle of each column, relative to r_base)
         for (int w = tid; w < (int)S.nranges * COLW; w += BL_THREADS) {
@@ -304,14 +329,19 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
             tcol = cxe - td.cxa;
             const double2 xy = A.p0[i], zh = A.p1[i];
             xa = xy.x; ya = xy.y; za = zh.x; ha = zh.y;
-            for (int q = 0; q < (int)S.nranges; ++q)
+            // the target's own slot: its row is candidate row (trz + 1, try_ + 1), one or two (wrapped x-range) pieces
+            const int row = (trz + 1) * 4 + (try_ + 1);
+            int q = S.r_row[row];
+            if (q != 0xFF) {
+                if (!(i >= S.r_vstart[q] && i < S.r_vend[q]) && q + 1 < (int)S.nranges && S.r_shift[q + 1][3] == row) ++q;
                 if (i >= S.r_vstart[q] && i < S.r_vend[q]) s_self = S.r_base[q] + (i - S.r_vstart[q]);
+            }
             tbad = A.coinc[i] != 0;                                     // a twin at distance 0: left to the general kernels (A11)
         }
         // an inactive thread sits far away from everything: it never hits
         const float fax = active ? (float)(xa - ox) : -3.0e18f, fay = (float)(ya - oy), faz = (float)(za - oz);
         if (active && !(fabsf(fax) <= extc && fabsf(fay) <= extc && fabsf(faz) <= extc)) tbad = true;
-        if (tbad) s_bad = 1;
+        if (active && s_self == 0xFFFFFFFFu) tbad = true;               // cannot happen: the target's cell is among the candidates
         const float Ra = 2.0f * (float)ha;
         const float Ta = Ra * Ra;
         const float Ta_hi = fmaf(Ta, 1.00001f, Am), Ta_lo = fmaf(Ta, 0.99999f, -Am);
@@ -325,14 +355,43 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
             ymin = min(ymin, __shfl_xor_sync(0xFFFFFFFFu, ymin, o)); ymax = max(ymax, __shfl_xor_sync(0xFFFFFFFFu, ymax, o));
             zmin = min(zmin, __shfl_xor_sync(0xFFFFFFFFu, zmin, o)); zmax = max(zmax, __shfl_xor_sync(0xFFFFFFFFu, zmax, o));
         }
+        __syncthreads();                                                // flags reset by thread 0 above; column offsets written
+        if (tbad) s_bad = 1;
         if (lane == 0 && cmax >= 0) { atomicMin(&s_clo, cmin); atomicMax(&s_chi, cmax); }
         if (tid == 0) s_h0 = ha;                                        // the half's first target: always there
+        // ---- the warp's block list: lane q takes candidate range q, its blocks inside the warp's window (rows
+        //      [ymin, ymax + 2] x [zmin, zmax + 2], virtual columns [cmin, cmax + 2]: one cell around every target), whole
+        //      blocks of 8 slots; the list is padded to a multiple of 4 entries with the block of the dummy slots, which
+        //      is staged out of reach.  A block that reaches over the window's columns brings in slots of the same row
+        //      two or more cells away (never a neighbour); slots past the end of a range are put out of reach.
+        uint32_t nwb = 0;
+        {
+            uint32_t b0 = 0, nb = 0;
+            if (lane < (int)S.nranges && cmax >= 0) {
+                const int row = S.r_shift[lane][3], ry = row & 3, rz = row >> 2;
+                if (!(ry < ymin || ry > ymax + 2 || rz < zmin || rz > zmax + 2)) {
+                    const int4 ge = S.r_geo[lane];
+                    const int jlo = max(0, min(ge.y, cmin - ge.z)), jhi = max(0, min(ge.y, cmax + 3 - ge.z));
+                    if (jhi > jlo) {
+                        const uint32_t sa = S.r_base[lane] + colofs[lane * COLW + jlo];
+                        const uint32_t sb = S.r_base[lane] + colofs[lane * COLW + jhi];
+                        b0 = sa >> 3; nb = ((sb + 7u) >> 3) - b0;
+                    }
+                }
+            }
+            uint32_t incl = nb;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+                if (lane >= o) incl += v;
+            }
+            nwb = __shfl_sync(0xFFFFFFFFu, incl, 31);
+            for (uint32_t k = 0, at = incl - nb; k < nb; ++k) wblk[at + k] = (uint16_t)(b0 + k);
+            if (lane < 4) wblk[nwb + lane] = (uint16_t)(TILE_CMAX / 8);  // pad (up to 3 used)
+        }
         __syncthreads();
 
-        // ---- stage the candidates of virtual columns [s_clo, s_chi + 2], whole blocks of 8 slots: one warp per range;
-        //      the pad slots of a range and the slots of a block that lie outside the window's columns but inside the
-        //      range are real particles two or more cells away from every target that can reach the block (never a
-        //      neighbour); slots past the end of the range are put out of reach
+        // ---- stage the candidates of virtual columns [s_clo, s_chi + 2], whole blocks of 8 slots: one warp per range
         {
             const unsigned long long h0 = (unsigned long long)__double_as_longlong(s_h0);
             const int clo = s_clo, chi = s_chi + 2;
@@ -360,6 +419,7 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
                     X[s] = fx; Y[s] = fy; Z[s] = fz; Tc[s] = T;
                 }
             }
+            if (tid < TILE_NDUMMY) { X[TILE_CMAX + tid] = 3.0e18f; Y[TILE_CMAX + tid] = 3.0e18f; Z[TILE_CMAX + tid] = 3.0e18f; Tc[TILE_CMAX + tid] = 0.0f; }
             if (nonuni) s_nonuni = 1;                                   // some staged candidate differs from the first target's h
             if (far) s_bad = 1;                                         // the error bound does not hold: general kernels
         }
@@ -368,12 +428,10 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
 
         // ---- scan (see the header).  All lanes of one parity read the same 16 bytes (shared-memory broadcast).
         const uint32_t bk0 = (uint32_t)__cvta_generic_to_shared(B + tid);
-        constexpr uint32_t BROW = 2u * BL_THREADS;                    // bytes per bucket row
         uint32_t bp0 = bk0, bp1 = bk0 + LIST_BS * BROW, bp2 = bk0 + 2 * LIST_BS * BROW, bp3 = bk0 + 3 * LIST_BS * BROW;
         const uint32_t e0 = bk0 + LIST_BC * BROW, e1 = e0 + LIST_BS * BROW, e2 = e1 + LIST_BS * BROW, e3 = e2 + LIST_BS * BROW;
         float tmin = 3.0e38f;                                           // min |t| over the tested candidates
-        if (cmax >= 0) {
-            const int wv_lo = cmin, wv_hi = cmax + 2;                   // virtual columns [tcol, tcol + 2] around each target
+        {
             const f32x2 ax2 = pk2(fax, fax), ay2 = pk2(fay, fay), az2 = pk2(faz, faz);
             const f32x2 nT2 = pk2(-Ta_hi, -Ta_hi);
             const float4* X4 = reinterpret_cast<const float4*>(X) + u;   // [2 b]: slots 8 b + 4 u ..
@@ -402,33 +460,18 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
                 unpk2(fma2(dz1, dz1, fma2(dy1, dy1, fma2(dx1, dx1, pk2(n2, n3)))), t2, t3);
                 append_if_neg(t0, bp0, b); append_if_neg(t1, bp1, b); append_if_neg(t2, bp2, b); append_if_neg(t3, bp3, b);
             };
-            auto clamp = [&]() { bp0 = min(bp0, e0); bp1 = min(bp1, e1); bp2 = min(bp2, e2); bp3 = min(bp3, e3); };
-            for (int q = 0; q < (int)S.nranges; ++q) {
-                const int row = S.r_shift[q][3], ry = row & 3, rz = row >> 2;
-                if (ry < ymin || ry > ymax + 2 || rz < zmin || rz > zmax + 2) continue;
-                const int4 ge = S.r_geo[q];
-                const int jlo = max(0, min(ge.y, wv_lo - ge.z)), jhi = max(0, min(ge.y, wv_hi + 1 - ge.z));
-                if (jhi <= jlo) continue;
-                const uint32_t sa = S.r_base[q] + colofs[q * COLW + jlo];
-                const uint32_t sb = S.r_base[q] + colofs[q * COLW + jhi];
-                uint32_t b = sa >> 3;
-                const uint32_t b1 = (sb + 7u) >> 3;                     // blocks [b, b1): all staged (the unit's window contains the warp's)
-                if (uni) {
-                    for (; b + LIST_TRASH <= b1; b += LIST_TRASH) {
-#pragma unroll
-                        for (int k = 0; k < LIST_TRASH; ++k) block_uni(b + k);
-                        clamp();
-                    }
-                    for (; b < b1; ++b) block_uni(b);
-                    clamp();
-                } else {
-                    for (; b + LIST_TRASH <= b1; b += LIST_TRASH) {
-#pragma unroll
-                        for (int k = 0; k < LIST_TRASH; ++k) block_gen(b + k);
-                        clamp();
-                    }
-                    for (; b < b1; ++b) block_gen(b);
-                    clamp();
+            const uint2* wb4 = reinterpret_cast<const uint2*>(wblk);
+            if (uni) {
+                for (uint32_t k = 0; k < nwb; k += 4) {
+                    const uint2 w = wb4[k >> 2];
+                    block_uni(w.x & 0xFFFFu); block_uni(w.x >> 16); block_uni(w.y & 0xFFFFu); block_uni(w.y >> 16);
+                    bp0 = min(bp0, e0); bp1 = min(bp1, e1); bp2 = min(bp2, e2); bp3 = min(bp3, e3);
+                }
+            } else {
+                for (uint32_t k = 0; k < nwb; k += 4) {
+                    const uint2 w = wb4[k >> 2];
+                    block_gen(w.x & 0xFFFFu); block_gen(w.x >> 16); block_gen(w.y & 0xFFFFu); block_gen(w.y >> 16);
+                    bp0 = min(bp0, e0); bp1 = min(bp1, e1); bp2 = min(bp2, e2); bp3 = min(bp3, e3);
                 }
             }
         }
@@ -517,98 +560,96 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
 #pragma unroll
         for (int o = 16; o; o >>= 1) R = max(R, __shfl_xor_sync(0xFFFFFFFFu, R, o));
         R = (R + 3u) & ~3u;
-        if (lane == 0) {
-            if (R > (uint32_t)LIST_RMAX) s_bad = 1;
-            s_rows[warp] = R >> 2;
+        __syncthreads();                                                // every warp is done with the staged candidates: the schedule
+                                                                        // staging area below shares their space
+        // list storage: rows of 32 lanes x 4 slots, R / 4 rows per warp, taken from the pool counter.  Placement depends on
+        // the order in which warps get there; the contents of the rows do not.  If another warp sends the unit to the general
+        // kernels after this one has emitted (list too long, pool exhausted), the rows stay unused.
+        uint32_t row0 = 0;
+        bool wbad = R > (uint32_t)LIST_RMAX || s_bad != 0;
+        if (lane == 0 && !wbad && R) {
+            const unsigned long long r0 = atomicAdd(&A.ctr[CTR_POOL], (unsigned long long)(R >> 2));
+            if (r0 + (R >> 2) > (unsigned long long)A.pool_rows) wbad = true;   // pool exhausted: general kernels
+            row0 = (uint32_t)r0;
         }
-        __syncthreads();
-        // list storage: rows of 32 lanes x 4 slots, one allocation per unit (its warps back to back) from the pool counter.
-        // Placement depends on the order in which units get there; the contents of a warp's rows do not.
-        if (tid == 0 && s_bad == 0) {
-            uint32_t tot = 0;
-#pragma unroll
-            for (int w = 0; w < BL_WARPS; ++w) tot += s_rows[w];
-            const unsigned long long r0 = atomicAdd(&A.ctr[CTR_POOL], (unsigned long long)tot);
-            if (r0 + tot > (unsigned long long)A.pool_rows) s_bad = 1;  // pool exhausted: general kernels
-            s_row0 = (uint32_t)r0;
-        }
-        __syncthreads();
-        const bool bad = s_bad != 0;
-        if (!bad) {
-            uint32_t row0 = s_row0;
-            for (int w = 0; w < warp; ++w) row0 += s_rows[w];
+        wbad = __shfl_sync(0xFFFFFFFFu, (int)wbad, 0) != 0;
+        row0 = __shfl_sync(0xFFFFFFFFu, row0, 0);
+        if (wbad) {
+            if (lane == 0) s_bad = 1;
+        } else {
             // ---- emit my half-list in scheduled order (see the header): phase t = rounds [tR/8, (t+1)R/8) in bank
             //      (j + t) & 7; what a phase cannot hold (overflow) fills the holes of other phases; the rest are dummies.
             // R = 8 m + 4 e (e = 0, 1): phase t starts at t m + e (t >> 1) and holds m + e (t & 1) rounds.
+            // The schedule is laid out [round / 4][thread][round & 3] (u16), so that four rounds leave as one 8-byte word.
             const uint32_t m8 = R >> 3, e4 = (R >> 2) & 1u;
-            uint16_t* out = Lf + tid;                                   // my column of the schedule: out[r * BL_THREADS]
-            const uint16_t* Bp = B + (tid & ~1);
-            uint32_t own[8], ovr[8];                                    // per phase: entries placed in the phase / left over
-            const uint16_t* bq[8];                                      // per phase: my entries of its bank (stride 2 rows)
+            const uint32_t Lb = (uint32_t)__cvta_generic_to_shared(smem + BL_OFF_L) + 8u * (uint32_t)tid;
+            const uint32_t Bb = (uint32_t)__cvta_generic_to_shared(B + (tid & ~1));
+            auto out_addr = [&](uint32_t r) { return Lb + (r >> 2) * (8u * BL_THREADS) + (r & 3u) * 2u; };
+            // my entries of bank beta: indices f, f + 2, ... (f = (u + beta) & 1) of the bucket of thread bank_owner(beta)
+            auto src_addr = [&](uint32_t beta) {
+                return Bb + 2u * (((beta & 3u) * LIST_BS + ((u + beta) & 1u)) * BL_THREADS + (beta >> 2));
+            };
             uint32_t Hw = 0;                                            // 8 x 4-bit: holes of each phase
-#pragma unroll
-            for (int t = 0; t < 8; ++t) {
-                const int beta = (j + t) & 7;
-                const uint32_t cap = m8 + (e4 & (uint32_t)(t & 1));
-                const uint32_t c = (cu >> (4 * beta)) & 15u;
-                own[t] = min(c, cap);
-                ovr[t] = c - own[t];
-                Hw |= (cap - own[t]) << (4 * t);
-                // my entries of bank beta: indices f, f+2, ... of the bucket of thread bank_owner(beta)
-                bq[t] = Bp + (bank_local(beta) * LIST_BS + ((u + beta) & 1)) * BL_THREADS + bank_owner(beta);
-            }
-            // pass 1 (lockstep): every phase takes its own bank's entries up to its capacity (an entry is a block number:
-            // slot = 8 block + bank); a hole gets the dummy slot of the phase's bank
-            for (uint32_t k = 0; k < m8; ++k) {
-#pragma unroll
-                for (int t = 0; t < 8; ++t) {
-                    const uint32_t beta = (uint32_t)(j + t) & 7u;
-                    uint32_t item = (uint32_t)TILE_CMAX + beta;
-                    if (k < own[t]) item = ((uint32_t)bq[t][2 * k * BL_THREADS] << 3) + beta;
-                    out[((uint32_t)t * m8 + (e4 ? (uint32_t)(t >> 1) : 0u) + k) * BL_THREADS] = (uint16_t)item;
-                }
-            }
-            if (e4) {
-#pragma unroll
-                for (int t = 1; t < 8; t += 2) {
-                    const uint32_t beta = (uint32_t)(j + t) & 7u;
-                    uint32_t item = (uint32_t)TILE_CMAX + beta;
-                    if (m8 < own[t]) item = ((uint32_t)bq[t][2 * m8 * BL_THREADS] << 3) + beta;
-                    out[((uint32_t)t * m8 + (uint32_t)(t >> 1) + m8) * BL_THREADS] = (uint16_t)item;
-                }
+            // pass 1: every phase takes its own bank's entries up to its capacity (an entry is a block number: slot = 8 block
+            // + bank); a hole gets the dummy slot of the phase's bank
+#pragma unroll 1
+            for (uint32_t t = 0; t < 8; ++t) {
+                const uint32_t beta = (uint32_t)(j + t) & 7u;
+                const uint32_t cap = m8 + (e4 & (t & 1u));
+                const uint32_t own = min((cu >> (4 * beta)) & 15u, cap);
+                Hw |= (cap - own) << (4 * t);
+                const uint32_t r0 = t * m8 + (e4 ? (t >> 1) : 0u);
+                uint32_t src = src_addr(beta);
+                for (uint32_t k = 0; k < own; ++k, src += 2u * BROW) sts_u16(out_addr(r0 + k), (lds_u16(src) << 3) + beta);
+                for (uint32_t k = own; k < cap; ++k) sts_u16(out_addr(r0 + k), (uint32_t)TILE_CMAX + beta);
             }
             // the left-over entries go into the holes, phase by phase (a phase has either holes or left-overs)
             {
-                int th = -1;
-                uint32_t hrem = 0;
-#pragma unroll
-                for (int t = 0; t < 8; ++t) {
+                uint32_t th = 0;
+#pragma unroll 1
+                for (uint32_t t = 0; t < 8; ++t) {
                     const uint32_t beta = (uint32_t)(j + t) & 7u;
-                    for (uint32_t e = 0; e < ovr[t]; ++e) {
-                        while (hrem == 0 && th < 7) { ++th; hrem = (Hw >> (4 * th)) & 15u; }
-                        if (hrem == 0) break;                           // cannot happen: n_lane <= R
-                        const uint32_t pos = (((uint32_t)(th + 1) * R) >> 3) - hrem;
-                        --hrem;
-                        out[pos * BL_THREADS] = (uint16_t)(((uint32_t)bq[t][2 * (own[t] + e) * BL_THREADS] << 3) + beta);
+                    const uint32_t cap = m8 + (e4 & (t & 1u));
+                    const uint32_t c = (cu >> (4 * beta)) & 15u;
+                    if (c <= cap) continue;
+                    uint32_t src = src_addr(beta) + cap * 2u * BROW;
+                    for (uint32_t e = cap; e < c; ++e, src += 2u * BROW) {
+                        while (th < 8 && ((Hw >> (4 * th)) & 15u) == 0u) ++th;
+                        if (th >= 8) break;                             // cannot happen: n_lane <= R
+                        const uint32_t hrem = (Hw >> (4 * th)) & 15u;
+                        const uint32_t pos = (((th + 1u) * R) >> 3) - hrem;
+                        Hw -= 1u << (4 * th);
+                        sts_u16(out_addr(pos), (lds_u16(src) << 3) + beta);
                     }
                 }
             }
-            // pass 2: pack 4 rounds per 8-byte store
+            // pass 2: four rounds per 8-byte store
             uint2* blk = A.pool + (size_t)row0 * 32 + lane;
-            for (uint32_t r4 = 0; r4 < R; r4 += 4) {
-                const uint32_t e0 = out[r4 * BL_THREADS], e1 = out[(r4 + 1) * BL_THREADS];
-                const uint32_t e2 = out[(r4 + 2) * BL_THREADS], e3 = out[(r4 + 3) * BL_THREADS];
-                blk[(size_t)(r4 >> 2) * 32] = make_uint2(e0 | (e1 << 16), e2 | (e3 << 16));
+            const uint32_t nr4 = R >> 2;
+            for (uint32_t r4 = 0; r4 < nr4; ++r4) {
+                uint2 v;
+                asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(Lb + r4 * (8u * BL_THREADS)));
+                blk[(size_t)r4 * 32] = v;
             }
             if (u == 0) A.lcount[(size_t)tile * TILE_T + tgt] = active ? (ng | (nsym << 16)) : 0u;
-            if (active && u == 0) A.fast[i] = 1;
             if (lane == 0) A.winfo[(size_t)tile * TILE_WARPS + twarp] = make_uint2(row0, R);
         }
+        __syncthreads();
+        const bool bad = s_bad != 0;
+        if (!bad && active && u == 0) A.fast[i] = 1;
         if (tid == 0) {
             const uint32_t bits = (bad ? 0u : (TILE_FLAG_OK0 << half)) | (s_nonuni ? TILE_FLAG_NONUNI : 0u);
             if (bits) atomicOr(&A.tflags[tile], bits);
             if (s_nonuni) atomicAdd(&A.ctr[CTR_NNONUNI], 1ull);
             if (!bad) atomicAdd(&A.ctr[CTR_NFAST], (unsigned long long)min((int)td.nt - half * BL_TGT, BL_TGT));
+        }
+        }
+        // the next unit's table goes into the other buffer (read after the barrier at the top of the loop)
+        if (nunit < nunits) {
+            uint32_t* dst = reinterpret_cast<uint32_t*>(&Sb[buf ^ 1]);
+            dst[tid] = pf0;
+            if (tid + BL_THREADS < TILES_WORDS) dst[tid + BL_THREADS] = pf1;
+            if (tid < 6) s_td[buf ^ 1][tid] = pfd;
         }
     }
 }

@@ -66,6 +66,7 @@ struct TileS {
     uint32_t r_base[TILE_MAXR + 1];  // first shared-memory slot of the range (exclusive scan of the lengths rounded up to even)
     int8_t r_shift[TILE_MAXR][4];    // [0..2] periodic image: dx = (x_a - x_b) + shift * L (-1, 0, +1); [3] candidate row id
     int4 r_geo[TILE_MAXR];           // (first cell column, number of columns, virtual column of the first, first cell id)
+    uint8_t r_row[16];               // candidate row id (rz * 4 + ry) -> index of its first range, 0xFF when the row has none
     uint32_t nranges, ncand;
     // targets
     uint32_t c_first[TILE_MAXCELL];  // global slot of the first particle of cell e (column-major enumeration)
@@ -158,6 +159,10 @@ __device__ __forceinline__ void tile_setup(const TileDesc& td, const DevGrid& g,
         }
         const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31);
         if (tid == 0) { S.nranges = __popc(mask); S.ncand = total; S.r_base[__popc(mask)] = total; }
+        if ((tid & 1) == 0) {                                          // first valid piece of candidate row tid >> 1
+            const bool v1 = (mask >> (tid + 1)) & 1u;
+            S.r_row[tid >> 1] = valid ? (uint8_t)pos : (v1 ? (uint8_t)__popc(mask & ((2u << tid) - 1u)) : (uint8_t)0xFF);
+        }
     }
     // target cells, column-major with serpentine rows (tile_cell_rc)
     const int nrows = td.nyr * td.nzr;
