@@ -45,6 +45,16 @@ def peaks():
         return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
 
 
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.lower().startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
+
+
 class ClockSampler:
     """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md recipe)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -505,8 +515,18 @@ def main():
         ns = min(n, args.cpu_sample)
         targets = np.sort(rng.choice(n, size=ns, replace=False)).astype(np.int64)
         dt, pr = oracle_sample_pass(w, targets)
-        cpu = {"value": pr / dt, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle", "seconds": dt,
-               "sample": f"{ns} of {n} target particles of {w.name} (all their neighbours), oracle cell-list variant, long-double sums"}
+        # the same oracle on ONE thread, on a sample sized for ~10 s (single thread and all hardware threads)
+        nthr = O.num_threads()
+        ns1 = max(1, min(ns, int(ns * 10.0 / max(dt * nthr, 1e-9))))
+        O.set_threads(1)
+        dt1, pr1 = oracle_sample_pass(w, targets[:: max(1, ns // ns1)][:ns1])
+        O.set_threads(nthr)
+        cpu = {"value": pr / dt, "unit": UNIT, "cores": nthr, "kind": "oracle", "seconds": dt,
+               "sample": f"{ns} of {n} target particles of {w.name} (all their neighbours), oracle cell-list variant, long-double sums",
+               "single_thread": {"value": pr1 / dt1, "unit": UNIT, "seconds": dt1, "targets": int(min(ns1, ns))},
+               "cpu_model": cpu_model(),
+               "note": "the oracle is a parity checker (x87 long-double sums, -O2 -ffp-contract=off, normaliser sums), not a tuned CPU code: "
+                       "GPU/oracle ratios are ratios against a checker"}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": 1e3 * t_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",

@@ -96,9 +96,19 @@ int spray_set_path(spray_ctx* ctx, int path);
  * *n_fast = particles served by the tiled kernels (the rest, n - n_fast, by the general kernels),
  * *n_nonuniform = list-builder work units (half tiles) whose particles do not all share one h (they run the
  * variable-h pair bodies), *scratch_bytes = device memory the context holds (allocated at spray_create).
- * All host pointers, all nullable. */
+ * declined[k] = list-builder events that left a half tile to the general kernels, by reason: 0 a warp's candidate window
+ * longer than 128 blocks of 8 slots, 1 left-over queue overflow in the schedule, 2 a list longer than 80 rounds or more than
+ * 24 neighbours in one shared-memory bank, 3 other (coincident particles, particle outside the tile's fp32 range, list pool
+ * exhausted).  All host pointers, all nullable. */
 int spray_path_stats(spray_ctx* ctx, void* stream, int64_t* n_tiles, int64_t* n_fast, int64_t* n_nonuniform,
-                     int64_t* scratch_bytes);
+                     int64_t* scratch_bytes, int64_t* declined /* [4] */);
+
+/* Measurement: device time of the three parts of the LAST spray_build_cells on this context, from CUDA events the call
+ * records on its stream (no cost on the path): *ms_cells = keys, sort, cell table, reorder, per-cell h_max, symmetric
+ * search length (a1-a4); *ms_tiles = coincidence marks, tile cutting, tile tables; *ms_lists = the neighbour-list
+ * builder (k_build_lists).  The last two are 0 on path 0.  Synchronises on the build's last event.  Host pointers,
+ * nullable. */
+int spray_build_timing(spray_ctx* ctx, double* ms_cells, double* ms_tiles, double* ms_lists);
 
 /* (a1)-(a4) NNPS: cell index per particle  c_d = floor((x_d - lo_d) * ncell_d / L_d) clamped,
  * key = (c_z*ncell_y + c_y)*ncell_x + c_x;  STABLE sort of (key, caller index);  cell_start[c] = #{key < c},

@@ -64,6 +64,11 @@ def num_threads() -> int:
     return int(lib().oracle_num_threads())
 
 
+def set_threads(n: int) -> None:
+    """OpenMP threads of the calls that follow (timing harness: single-thread and all-core oracle timings)."""
+    lib().oracle_set_threads(int(n))
+
+
 def _d(a):
     a = np.ascontiguousarray(a, dtype=np.float64)
     return a, a.ctypes.data_as(C.c_void_p)

@@ -41,6 +41,15 @@ typedef struct {
 enum { ORACLE_CUBIC_SPLINE = 0, ORACLE_WENDLAND_C2 = 1 };
 enum { ORACLE_GATHER = 0, ORACLE_SYM = 1 };
 
+/* timing harness only (bench.py reports the oracle single-threaded and on all cores): number of OpenMP threads of the calls that follow */
+void oracle_set_threads(int n) {
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
 int oracle_num_threads(void) {
 #ifdef _OPENMP
     return omp_get_max_threads();

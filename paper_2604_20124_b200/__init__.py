@@ -23,7 +23,7 @@ COND_OPERATOR, COND_RHS = 0, 1
 DEV_H_EXCEEDS_HMAX, DEV_OUTSIDE_BOX, DEV_LIST_OVERFLOW = 1, 2, 4
 
 # every symbol include/spray.h declares
-EXPORTS = ["spray_version", "spray_create", "spray_destroy", "spray_last_error", "spray_check", "spray_launch_count", "spray_set_path", "spray_path_stats",
+EXPORTS = ["spray_version", "spray_create", "spray_destroy", "spray_last_error", "spray_check", "spray_launch_count", "spray_set_path", "spray_path_stats", "spray_build_timing",
            "spray_build_cells", "spray_density", "spray_hydro_rhs", "spray_hydro_rhs_limiter", "spray_fld_apply", "spray_get_cell_table",
            "spray_neighbor_counts", "spray_neighbor_lists", "spray_neighbor_digest", "spray_rad_jacobi", "spray_conduction", "spray_kgc_continuity", "spray_ray_deposit", "spray_conduction_implicit", "spray_fp64_peak_probe"]
 
@@ -60,7 +60,8 @@ def load():
     lib.spray_check.argtypes = [vp, vp, C.POINTER(C.c_uint32)]
     lib.spray_set_path.argtypes = [vp, i32]
     lib.spray_launch_count.argtypes = [vp]
-    lib.spray_path_stats.argtypes = [vp, vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+    lib.spray_path_stats.argtypes = [vp, vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+    lib.spray_build_timing.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double)]
     lib.spray_build_cells.argtypes = [vp, C.POINTER(Grid), i32, i64, vp, vp, vp, vp, vp]
     lib.spray_density.argtypes = [vp, vp, vp, vp, vp]
     lib.spray_hydro_rhs.argtypes = [vp] + [vp] * 8 + [dbl] + [vp] * 5 + [vp]
@@ -154,8 +155,16 @@ class Spray:
         """Statistics of the last build_cells (synchronises): tiles, particles served by the tiled kernels, list-builder
         work units (half tiles) that found non-uniform h, bytes of device scratch the context holds."""
         nt, nf, nn, nb = C.c_int64(0), C.c_int64(0), C.c_int64(0), C.c_int64(0)
-        self._ck(self.lib.spray_path_stats(self.h, _stream(), C.byref(nt), C.byref(nf), C.byref(nn), C.byref(nb)), "spray_path_stats")
-        return {"tiles": int(nt.value), "n_fast": int(nf.value), "nonuniform_units": int(nn.value), "scratch_bytes": int(nb.value)}
+        dec = (C.c_int64 * 4)()
+        self._ck(self.lib.spray_path_stats(self.h, _stream(), C.byref(nt), C.byref(nf), C.byref(nn), C.byref(nb), dec), "spray_path_stats")
+        return {"tiles": int(nt.value), "n_fast": int(nf.value), "nonuniform_units": int(nn.value), "scratch_bytes": int(nb.value),
+                "declined": [int(x) for x in dec]}
+
+    def build_timing(self):
+        """Device milliseconds of the last build_cells: (cell list a1-a4, tiles + tables, neighbour-list builder); synchronises."""
+        a, b, d = C.c_double(0), C.c_double(0), C.c_double(0)
+        self._ck(self.lib.spray_build_timing(self.h, C.byref(a), C.byref(b), C.byref(d)), "spray_build_timing")
+        return a.value, b.value, d.value
 
     def path_stats(self):
         """(tiles, particles served by the tiled kernels) of the last build_cells; synchronises."""

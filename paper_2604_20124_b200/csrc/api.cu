@@ -155,6 +155,8 @@ int spray_create(spray_ctx** out, int64_t n_max, int64_t ncell_max, int device) 
         return fail(nullptr, SPRAY_ERR_ALLOC, "spray_create: device allocation failed");
     }
     alloc_tiled(c);
+    for (cudaEvent_t& e : c->ev)
+        if (cudaEventCreate(&e) != cudaSuccess) { cudaGetLastError(); e = nullptr; }
     *out = h;
     return SPRAY_OK;
 }
@@ -163,6 +165,7 @@ int spray_destroy(spray_ctx* ctx) {
     if (!ctx) return SPRAY_OK;
     DeviceGuard dg(ctx->c.device);
     cudaDeviceSynchronize();
+    for (cudaEvent_t e : ctx->c.ev) if (e) cudaEventDestroy(e);
     free_all(&ctx->c);
     delete ctx;
     return SPRAY_OK;
@@ -194,7 +197,7 @@ int spray_set_path(spray_ctx* ctx, int path) {
 }
 
 int spray_path_stats(spray_ctx* ctx, void* stream, int64_t* n_tiles, int64_t* n_fast, int64_t* n_nonuniform,
-                     int64_t* scratch_bytes) {
+                     int64_t* scratch_bytes, int64_t* declined) {
     NEED_BUILT();
     Ctx* c = &ctx->c;
     cudaStream_t st = (cudaStream_t)stream;
@@ -207,6 +210,24 @@ int spray_path_stats(spray_ctx* ctx, void* stream, int64_t* n_tiles, int64_t* n_
     if (n_fast) *n_fast = (int64_t)v[CTR_NFAST];
     if (n_nonuniform) *n_nonuniform = (int64_t)v[CTR_NNONUNI];
     if (scratch_bytes) *scratch_bytes = c->scratch_bytes;
+    if (declined) for (int k = 0; k < 4; ++k) declined[k] = (int64_t)v[CTR_DECL + k];
+    return SPRAY_OK;
+}
+
+int spray_build_timing(spray_ctx* ctx, double* ms_cells, double* ms_tiles, double* ms_lists) {
+    NEED_BUILT();
+    Ctx* c = &ctx->c;
+    for (cudaEvent_t e : c->ev) if (!e) return fail(c, SPRAY_ERR_CUDA, "spray_build_timing: no events");
+    CK(cudaEventSynchronize(c->ev[3]), "spray_build_timing");
+    float a = 0.f, b = 0.f, d = 0.f;
+    CK(cudaEventElapsedTime(&a, c->ev[0], c->ev[1]), "spray_build_timing");
+    if (c->tl.enabled) {
+        CK(cudaEventElapsedTime(&b, c->ev[1], c->ev[2]), "spray_build_timing");
+        CK(cudaEventElapsedTime(&d, c->ev[2], c->ev[3]), "spray_build_timing");
+    }
+    if (ms_cells) *ms_cells = a;
+    if (ms_tiles) *ms_tiles = b;
+    if (ms_lists) *ms_lists = d;
     return SPRAY_OK;
 }
 
@@ -242,6 +263,7 @@ int spray_build_cells(spray_ctx* ctx, const spray_grid_t* g, spray_kernel_t kern
         c->dg.per[d] = g->periodic[d] ? 1 : 0;
     }
     cudaStream_t st = (cudaStream_t)stream;
+    if (c->ev[0]) cudaEventRecord(c->ev[0], st);
     CK(launch_cell_keys(c, x, y, z, st), "cell keys");
     CK(launch_radix_sort(c, st), "radix sort");
     CK(launch_cell_table(c, st), "cell table");
@@ -253,7 +275,9 @@ int spray_build_cells(spray_ctx* ctx, const spray_grid_t* g, spray_kernel_t kern
     SweepArgs a = base_args(c);
     a.o0 = c->s.hs;
     CK(launch_ref_sweep(c, SW_HSEARCH, a, st), "search-length sweep");
+    if (c->ev[1]) cudaEventRecord(c->ev[1], st);
     if (c->path == 1) CK(launch_build_tiles(c, st), "tiles + neighbour lists");
+    if (c->ev[3]) cudaEventRecord(c->ev[3], st);
     c->built = true;
     return SPRAY_OK;
 }

@@ -52,7 +52,10 @@ struct Tiled {
 };
 // CTR_NFAST: particles served by the tiled kernels; CTR_NTILES: tiles; CTR_NNONUNI: half-tile units that found non-uniform h;
 // CTR_POOL: list-pool rows handed out
-enum { CTR_NFAST = 1, CTR_NTILES = 2, CTR_NNONUNI = 3, CTR_POOL = 4, CTR_COUNT = 8 };
+// CTR_DECL + k: warps / threads that declined their unit (general kernels), by reason k: 0 = window longer than 128 blocks,
+// 1 = left-over queue overflow, 2 = list longer than LIST_RMAX rounds or more than LIST_BC neighbours in one bank, 3 = other
+// (coincident particles, particle outside the tile's fp32 range, list pool exhausted)
+enum { CTR_NFAST = 1, CTR_NTILES = 2, CTR_NNONUNI = 3, CTR_POOL = 4, CTR_DECL = 8, CTR_COUNT = 12 };
 
 struct Ctx {
     int device = 0;
@@ -78,6 +81,7 @@ struct Ctx {
     double* rad_scratch[4] = {nullptr, nullptr, nullptr, nullptr};   // N1: y, Lambda, Gamma, chi (caller order), allocated on first use
     int64_t launches = 0;       // kernels launched through this ctx (bench.py reports it as gpu_launches)
     int64_t scratch_bytes = 0;  // device memory held by this ctx
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};   // recorded by spray_build_cells: start, cell list done, tiles done, lists done
     std::string err;
 };
 
