@@ -149,26 +149,19 @@ k_tile_tables(DevGrid g, CellTable ct, const TileDesc* __restrict__ tiles, const
 // ------------------------------------------------------------------------------------------- list builder
 // One CTA of BL_THREADS threads builds the lists of HALF a tile (targets [128 half, 128 half + 128), i.e. warps
 // 8 half .. 8 half + 7 of the sweeps' CTA), so that two CTAs fit on an SM and one's barriers and staging latencies are
-// covered by the other's work.  Work unit w = 2 tile + half.  A warp serves 16 targets, as in the sweeps.
+// covered by the other's scan.  Work unit w = 2 tile + half.
 //
 // THE SCAN.  Candidates are staged as fp32 coordinates relative to the tile centre, one array per component, indexed
 // by slot; candidate ranges start on multiples of 8 slots, so an aligned BLOCK of 8 slots holds one slot of every
-// shared-memory bank of the sweeps (slot & 7).  A warp's window (the cells within one cell of its targets) is a list of
-// such blocks.  In the scan the LANES HOLD THE CANDIDATES and the 16 TARGETS SIT IN REGISTERS: per iteration lane l
-// loads one candidate (ordinal 32 n + l of the window, bank l & 7: three conflict-light 4-byte loads) and tests it
-// against the 8 target pairs with packed fp32 arithmetic (sm_100 FADD2 / FFMA2),
+// shared-memory bank of the sweeps (slot & 7).  The two threads of a target split the banks: thread u tests slots
+// 8 b + 4 u .. 8 b + 4 u + 3 of every block b of its warp's window with two packed (sm_100 FADD2/FFMA2) chains,
 //     t = dz^2 + (dy^2 + (dx^2 - T_hi)),   T_hi = (2 h)^2 (1 + 1e-5) + Am   (error bound Am below),
-// shifting the sign of t into the target's hit mask (one SHF per test): 4 instructions per test and no shared-memory
-// traffic in the inner loop (the previous layout -- lanes = targets, candidates broadcast from shared memory, hits
-// appended by predicated stores -- was bound by shared-memory wavefronts: profiles/r02b).  The lane keeps min |t| over
-// everything it tested: if that stays above the width of the uncertainty band for every lane of the warp, every
-// decision of the fp32 test was certain and the masks are final (only the target itself has to be taken out);
-// otherwise, and in tiles with variable h, every hit is classified again (fp32 bounds first, then the exact fp64
-// contract predicate, O2/A12), so the sets are bit-identical to the definition.  A hit is never lost: t < 0 is a
-// superset of the support.
-// The masks are transposed through shared memory (word [target][lane] = the target's hits among that lane's
-// candidates, all of one bank), and each thread of a target then walks the hits of the four banks of its parity,
-// dealing them alternately to the two half-lists of the target, straight into their scheduled positions.
+// and a candidate with t < 0 is appended -- one predicated 16-bit store of the block number and one predicated
+// pointer increment -- to the thread's bucket of the candidate's bank.  The thread keeps min |t| over everything
+// it tested: if that stays above the width of the uncertainty band, every decision of the fp32 test was certain
+// and the buckets are final (only the target itself has to be taken out); otherwise, and in tiles with variable h,
+// every bucket entry is classified again (fp32 bounds first, then the exact fp64 contract predicate, O2/A12), so the
+// sets are bit-identical to the definition.  A hit is never lost: t < 0 is a superset of the support.
 struct ListArgs {
     const double2 *p0, *p1;            // sorted (x, y), (z, h)
     const TileDesc* tiles;
@@ -189,13 +182,10 @@ constexpr int BL_THREADS = TILE_THREADS / 2;
 constexpr int BL_WARPS = BL_THREADS / 32;
 constexpr int BL_TGT = TILE_T / 2;
 constexpr int COLW = TILE_BXMAX + 4;
+constexpr int LIST_TRASH = 4;                // trash rows of a bucket: the scan clamps its row pointers once per 4 blocks
+constexpr int LIST_BS = LIST_BC + LIST_TRASH;
 constexpr int LIST_LCAP = LIST_RMAX;         // rounds of the schedule staging area
-constexpr int TS_NMAX = 32;                  // scan iterations of a lane per chunk = bits of a hit mask (128 blocks of the window)
-constexpr int TS_CHUNKS = 2;                 // chunks of a window: at most 256 blocks = 2048 slots (longer: general kernels)
-constexpr int WBLK_CAP = 4 * TS_NMAX * TS_CHUNKS + 8;   // a warp's block list (padded to a multiple of 4 entries)
-constexpr int MS_STRIDE = 33;                // words per target row of the transposed masks (33: the 16 targets of a warp read
-                                             // the same column in 16 different banks)
-constexpr int LQ_CAP = 16;                   // left-over queue of one (half-list, source thread)
+constexpr int WBLK_CAP = TILE_CMAXP / 8 + 8; // a warp's block list: every staged block at most, padded to a multiple of 4
 constexpr size_t BL_OFF_X = 0;                                                          // float [CMAXP] each: x, y, z relative to the
 constexpr size_t BL_OFF_Y = BL_OFF_X + sizeof(float) * TILE_CMAXP;                      // tile centre, T = (2 h)^2
 constexpr size_t BL_OFF_Z = BL_OFF_Y + sizeof(float) * TILE_CMAXP;
@@ -205,34 +195,41 @@ constexpr size_t BL_OFF_L = 0;                                                  
                                                                                         // word pair, written after the scan is over -- shares the
                                                                                         // space of the candidates
 constexpr size_t BL_L_END = BL_OFF_L + sizeof(uint16_t) * LIST_LCAP * BL_THREADS;
-constexpr size_t BL_OFF_MS = BL_CAND_END > BL_L_END ? BL_CAND_END : BL_L_END;            // u32 [BL_WARPS][TS_CHUNKS][16][MS_STRIDE]: transposed hit masks
-constexpr size_t BL_OFF_LQ = BL_OFF_MS + sizeof(uint32_t) * BL_WARPS * TS_CHUNKS * 16 * MS_STRIDE;  // u16 [BL_THREADS][2][LQ_CAP]: left-over queues
-constexpr size_t BL_OFF_TG = BL_OFF_LQ + sizeof(uint16_t) * BL_THREADS * 2 * LQ_CAP;    // float [BL_WARPS][4][16]: x, y, z, -T_hi of a warp's targets
-constexpr size_t BL_OFF_COL = BL_OFF_TG + sizeof(float) * BL_WARPS * 4 * 16;            // u16 [MAXR][COLW]
+constexpr size_t BL_OFF_B = BL_CAND_END > BL_L_END ? BL_CAND_END : BL_L_END;             // u16 [4][LIST_BS][BL_THREADS]
+constexpr size_t BL_OFF_COL = BL_OFF_B + sizeof(uint16_t) * 4 * LIST_BS * BL_THREADS;   // u16 [MAXR][COLW]
 constexpr size_t BL_OFF_WB = BL_OFF_COL + sizeof(uint16_t) * TILE_MAXR * COLW;          // u16 [BL_WARPS][WBLK_CAP]
 constexpr size_t BL_SMEM = BL_OFF_WB + sizeof(uint16_t) * BL_WARPS * WBLK_CAP;
 static_assert(2 * (BL_SMEM + 2 * sizeof(TileS) + 1280) <= 228 * 1024, "list builder: two CTAs per SM");
 static_assert(TILE_CMAXP % 8 == 0 && TILE_CMAX % 8 == 0, "blocks of 8 slots");
 static_assert(TILES_WORDS <= 2 * BL_THREADS, "tile table prefetch: two words per thread");
 static_assert(sizeof(TileDesc) == 24, "tile descriptor prefetch: six words");
-static_assert(BL_OFF_TG % 16 == 0 && BL_OFF_MS % 4 == 0 && BL_OFF_WB % 2 == 0, "alignment");
+static_assert(BL_OFF_WB % 8 == 0 && WBLK_CAP % 4 == 0, "block list rows are read four entries at a time");
 
-// packed fp32 pairs (sm_100 FADD2 / FMUL2 / FFMA2): one instruction tests two targets
+// packed fp32 pairs (sm_100 FADD2 / FMUL2 / FFMA2): one instruction tests two candidates
 typedef unsigned long long f32x2;
 __device__ __forceinline__ f32x2 pk2(float a, float b) { f32x2 r; asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(a), "f"(b)); return r; }
 __device__ __forceinline__ void unpk2(f32x2 v, float& a, float& b) { asm("mov.b64 {%0,%1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); }
 __device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) { f32x2 r; asm("sub.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
-__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) { f32x2 r; asm("add.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
-__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) { f32x2 r; asm("mul.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
 __device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
-// mask = (mask << 1) | sign bit of t
-__device__ __forceinline__ uint32_t shift_in_sign(uint32_t mask, float t) {
-    uint32_t r;
-    asm("shf.l.wrap.b32 %0, %1, %2, 1;" : "=r"(r) : "r"(__float_as_uint(t)), "r"(mask));
-    return r;
+
+// One candidate of the scan: if t < 0 store the block number at the bucket row pointer and advance it.  No branches; the
+// caller clamps the pointer at the first trash row of the bucket once per LIST_TRASH blocks.
+__device__ __forceinline__ void append_if_neg(float t, uint32_t& addr, uint32_t blk) {
+    asm volatile("{\n\t.reg .pred p;\n\t"
+                 "setp.lt.f32 p, %1, 0f00000000;\n\t"
+                 "@p st.shared.u16 [%0], %2;\n\t"
+                 "@p add.u32 %0, %0, %3;\n\t}"
+                 : "+r"(addr) : "f"(t), "r"(blk), "n"(2 * BL_THREADS));
+    // no memory clobber: the loads of the next blocks must be free to move above the store; the buckets are read back
+    // only after the fence that follows the scan
 }
-__device__ __forceinline__ void sts_u16(uint32_t addr, uint32_t v) { asm volatile("st.shared.u16 [%0], %1;" :: "r"(addr), "r"(v) : "memory"); }
-__device__ __forceinline__ uint32_t lds_u16(uint32_t addr) { uint32_t v; asm volatile("ld.shared.u16 %0, [%1];" : "=r"(v) : "r"(addr) : "memory"); return v; }
+__device__ __forceinline__ uint32_t lds_u16(uint32_t addr) { uint32_t v; asm volatile("ld.shared.u16 %0, [%1];" : "=r"(v) : "r"(addr)); return v; }
+__device__ __forceinline__ void sts_u16(uint32_t addr, uint32_t v) { asm volatile("st.shared.u16 [%0], %1;" :: "r"(addr), "r"(v)); }
+
+// Which thread of a target owns bank beta in the scan (thread u tests slots 8 b + 4 u .. 8 b + 4 u + 3), and the index
+// of that bank among the owner's four buckets.
+__device__ __forceinline__ int bank_owner(int beta) { return beta >> 2; }
+__device__ __forceinline__ int bank_local(int beta) { return beta & 3; }
 
 
 __global__ void __launch_bounds__(BL_THREADS, 2)
@@ -246,15 +243,15 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
     float* Y = reinterpret_cast<float*>(smem + BL_OFF_Y);
     float* Z = reinterpret_cast<float*>(smem + BL_OFF_Z);
     float* Tc = reinterpret_cast<float*>(smem + BL_OFF_T);
+    uint16_t* Lf = reinterpret_cast<uint16_t*>(smem + BL_OFF_L);       // [k * BL_THREADS + tid]
+    uint16_t* B = reinterpret_cast<uint16_t*>(smem + BL_OFF_B);        // [(b * LIST_BS + k) * BL_THREADS + tid]
     uint16_t* colofs = reinterpret_cast<uint16_t*>(smem + BL_OFF_COL); // [range][COLW]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     uint16_t* wblk = reinterpret_cast<uint16_t*>(smem + BL_OFF_WB) + warp * WBLK_CAP;
-    uint32_t* MS = reinterpret_cast<uint32_t*>(smem + BL_OFF_MS) + warp * TS_CHUNKS * 16 * MS_STRIDE;
-    float* TG = reinterpret_cast<float*>(smem + BL_OFF_TG) + warp * 64;
-    uint16_t* LQ = reinterpret_cast<uint16_t*>(smem + BL_OFF_LQ);      // [list column][source thread parity][LQ_CAP]
-    const int u = tid & 1, j = lane & 7, it = lane >> 1;               // it: my target among the warp's 16
+    const int u = tid & 1, j = lane & 7;
     const uint32_t nunits = 2u * (uint32_t)A.ctr[CTR_NTILES];
     const float Rmax = 2.0f * (float)A.hglob[1] * 1.000001f;
+    constexpr uint32_t BROW = 2u * BL_THREADS;                        // bytes per bucket row
 
     // tile table and descriptor of the first unit; afterwards each unit prefetches the next one's while it works
     if (blockIdx.x < nunits) {
@@ -322,7 +319,6 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
         // ---- this thread's target
         const bool active = tgt < (int)td.nt;
         uint32_t i = 0, s_self = 0xFFFFFFFFu;
-        int q_self = 0;
         double xa = 0, ya = 0, za = 0, ha = 0;
         int tcol = 0, try_ = 0, trz = 0;
         bool tbad = false;
@@ -339,18 +335,17 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
             int q = S.r_row[row];
             if (q != 0xFF) {
                 if (!(i >= S.r_vstart[q] && i < S.r_vend[q]) && q + 1 < (int)S.nranges && S.r_shift[q + 1][3] == row) ++q;
-                if (i >= S.r_vstart[q] && i < S.r_vend[q]) { s_self = S.r_base[q] + (i - S.r_vstart[q]); q_self = q; }
+                if (i >= S.r_vstart[q] && i < S.r_vend[q]) s_self = S.r_base[q] + (i - S.r_vstart[q]);
             }
             tbad = A.coinc[i] != 0;                                     // a twin at distance 0: left to the general kernels (A11)
         }
-        // an inactive thread's target sits far away from everything: it never hits
+        // an inactive thread sits far away from everything: it never hits
         const float fax = active ? (float)(xa - ox) : -3.0e18f, fay = (float)(ya - oy), faz = (float)(za - oz);
         if (active && !(fabsf(fax) <= extc && fabsf(fay) <= extc && fabsf(faz) <= extc)) tbad = true;
         if (active && s_self == 0xFFFFFFFFu) tbad = true;               // cannot happen: the target's cell is among the candidates
         const float Ra = 2.0f * (float)ha;
         const float Ta = Ra * Ra;
         const float Ta_hi = fmaf(Ta, 1.00001f, Am), Ta_lo = fmaf(Ta, 0.99999f, -Am);
-        if (u == 0) { TG[it] = fax; TG[16 + it] = fay; TG[32 + it] = faz; TG[48 + it] = -Ta_hi; }
         // warp window in virtual columns / candidate rows; the union over the warps is what this CTA stages
         int cmin = active ? tcol : 1 << 20, cmax = active ? tcol : -1;
         int ymin = active ? try_ : 4, ymax = active ? try_ : -1;
@@ -362,7 +357,7 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
             zmin = min(zmin, __shfl_xor_sync(0xFFFFFFFFu, zmin, o)); zmax = max(zmax, __shfl_xor_sync(0xFFFFFFFFu, zmax, o));
         }
         __syncthreads();                                                // flags reset by thread 0 above; column offsets written
-        if (tbad) { s_bad = 1; atomicAdd(&A.ctr[CTR_DECL + 3], 1ull); }
+        if (tbad) s_bad = 1;
         if (lane == 0 && cmax >= 0) { atomicMin(&s_clo, cmin); atomicMax(&s_chi, cmax); }
         if (tid == 0) s_h0 = ha;                                        // the half's first target: always there
         // ---- the warp's block list: lane q takes candidate range q, its blocks inside the warp's window (rows
@@ -370,8 +365,7 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
         //      blocks of 8 slots; the list is padded to a multiple of 4 entries with the block of the dummy slots, which
         //      is staged out of reach.  A block that reaches over the window's columns brings in slots of the same row
         //      two or more cells away (never a neighbour); slots past the end of a range are put out of reach.
-        //      Window ordinal o = 8 (position in the list) + (slot & 7); lane l scans the ordinals 32 n + l.
-        uint32_t nwb = 0, o_self = 0;
+        uint32_t nwb = 0;
         {
             uint32_t b0 = 0, nb = 0;
             if (lane < (int)S.nranges && cmax >= 0) {
@@ -393,22 +387,9 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
                 if (lane >= o) incl += v;
             }
             nwb = __shfl_sync(0xFFFFFFFFu, incl, 31);
-            const uint32_t at = incl - nb;
-            if (nwb > 4u * TS_NMAX * TS_CHUNKS) {                       // window too long for the hit masks: general kernels
-                if (lane == 0) { s_bad = 1; atomicAdd(&A.ctr[CTR_DECL + 0], 1ull); }
-                nwb = 0; nb = 0;
-            }
-            for (uint32_t k = 0; k < nb; ++k) wblk[at + k] = (uint16_t)(b0 + k);
+            for (uint32_t k = 0, at = incl - nb; k < nb; ++k) wblk[at + k] = (uint16_t)(b0 + k);
             if (lane < 4) wblk[nwb + lane] = (uint16_t)(TILE_CMAX / 8);  // pad (up to 3 used)
-            // ordinal of the target's own slot: its block is in the list part of range q_self
-            const uint32_t at_s = __shfl_sync(0xFFFFFFFFu, at, q_self), b0_s = __shfl_sync(0xFFFFFFFFu, b0, q_self);
-            o_self = 8u * (at_s + ((s_self >> 3) - b0_s)) + (s_self & 7u);
         }
-        const uint32_t NT = (nwb + 3u) >> 2;                            // scan iterations of a lane, in chunks of 32 (= bits of a hit mask)
-        const uint32_t NCH = (NT + 31u) >> 5;
-        // Hit-mask words of (target, bank beta): word kk = 4 c + k is chunk c, lane beta + 8 k; its bit p is iteration
-        // n = 32 c + N_c - 1 - p of that lane (N_c = iterations of the chunk), i.e. the slot of bank beta in block 4 n + k of the list.
-        auto chunk_n = [&](uint32_t c) { return min(32u, NT - 32u * c); };
         __syncthreads();
 
         // ---- stage the candidates of virtual columns [s_clo, s_chi + 2], whole blocks of 8 slots: one warp per range
@@ -441,156 +422,139 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
             }
             if (tid < TILE_NDUMMY) { X[TILE_CMAX + tid] = 3.0e18f; Y[TILE_CMAX + tid] = 3.0e18f; Z[TILE_CMAX + tid] = 3.0e18f; Tc[TILE_CMAX + tid] = 0.0f; }
             if (nonuni) s_nonuni = 1;                                   // some staged candidate differs from the first target's h
-            if (far) { s_bad = 1; atomicAdd(&A.ctr[CTR_DECL + 3], 1ull); }   // the error bound does not hold: general kernels
+            if (far) s_bad = 1;                                         // the error bound does not hold: general kernels
         }
         __syncthreads();
         const bool uni = s_nonuni == 0;
 
-        // ---- scan (see the header): lane l holds candidate 32 n + l of the window, the 16 targets sit in registers as 8 pairs
-        float tmin = 3.0e38f;                                           // min |t| over the tests of this lane
+        // ---- scan (see the header).  All lanes of one parity read the same 16 bytes (shared-memory broadcast).
+        const uint32_t bk0 = (uint32_t)__cvta_generic_to_shared(B + tid);
+        uint32_t bp0 = bk0, bp1 = bk0 + LIST_BS * BROW, bp2 = bk0 + 2 * LIST_BS * BROW, bp3 = bk0 + 3 * LIST_BS * BROW;
+        const uint32_t e0 = bk0 + LIST_BC * BROW, e1 = e0 + LIST_BS * BROW, e2 = e1 + LIST_BS * BROW, e3 = e2 + LIST_BS * BROW;
+        float tmin = 3.0e38f;                                           // min |t| over the tested candidates
         {
-            f32x2 tx[8], ty[8], tz[8];
-            {
-                const float2* t2 = reinterpret_cast<const float2*>(TG);
-#pragma unroll
-                for (int p = 0; p < 8; ++p) {
-                    const float2 a = t2[p], b = t2[8 + p], c = t2[16 + p];
-                    tx[p] = pk2(a.x, a.y); ty[p] = pk2(b.x, b.y); tz[p] = pk2(c.x, c.y);
-                }
-            }
-            const uint32_t sub = (uint32_t)lane >> 3, bank = (uint32_t)lane & 7u;
-#pragma unroll 1
-            for (uint32_t c = 0; c < NCH; ++c) {
-            const uint32_t n0 = 32u * c, n1 = n0 + chunk_n(c);
-            uint32_t m[16];
-#pragma unroll
-            for (int k = 0; k < 16; ++k) m[k] = 0u;
+            const f32x2 ax2 = pk2(fax, fax), ay2 = pk2(fay, fay), az2 = pk2(faz, faz);
+            const f32x2 nT2 = pk2(-Ta_hi, -Ta_hi);
+            const float4* X4 = reinterpret_cast<const float4*>(X) + u;   // [2 b]: slots 8 b + 4 u ..
+            const float4* Y4 = reinterpret_cast<const float4*>(Y) + u;
+            const float4* Z4 = reinterpret_cast<const float4*>(Z) + u;
+            const float4* T4 = reinterpret_cast<const float4*>(Tc) + u;
+            auto block_uni = [&](uint32_t b) {
+                const float4 x = X4[2 * b], y = Y4[2 * b], z = Z4[2 * b];
+                const f32x2 dx0 = sub2(ax2, pk2(x.x, x.y)), dy0 = sub2(ay2, pk2(y.x, y.y)), dz0 = sub2(az2, pk2(z.x, z.y));
+                const f32x2 dx1 = sub2(ax2, pk2(x.z, x.w)), dy1 = sub2(ay2, pk2(y.z, y.w)), dz1 = sub2(az2, pk2(z.z, z.w));
+                float t0, t1, t2, t3;
+                unpk2(fma2(dz0, dz0, fma2(dy0, dy0, fma2(dx0, dx0, nT2))), t0, t1);
+                unpk2(fma2(dz1, dz1, fma2(dy1, dy1, fma2(dx1, dx1, nT2))), t2, t3);
+                append_if_neg(t0, bp0, b); append_if_neg(t1, bp1, b); append_if_neg(t2, bp2, b); append_if_neg(t3, bp3, b);
+                tmin = fminf(fminf(tmin, fabsf(t0)), fminf(fabsf(t1), fminf(fabsf(t2), fabsf(t3))));
+            };
+            auto block_gen = [&](uint32_t b) {
+                const float4 x = X4[2 * b], y = Y4[2 * b], z = Z4[2 * b], T = T4[2 * b];
+                const f32x2 dx0 = sub2(ax2, pk2(x.x, x.y)), dy0 = sub2(ay2, pk2(y.x, y.y)), dz0 = sub2(az2, pk2(z.x, z.y));
+                const f32x2 dx1 = sub2(ax2, pk2(x.z, x.w)), dy1 = sub2(ay2, pk2(y.z, y.w)), dz1 = sub2(az2, pk2(z.z, z.w));
+                // support of the larger h, error bound added
+                const float n0 = -fmaf(fmaxf(Ta, T.x), 1.00001f, Am), n1 = -fmaf(fmaxf(Ta, T.y), 1.00001f, Am);
+                const float n2 = -fmaf(fmaxf(Ta, T.z), 1.00001f, Am), n3 = -fmaf(fmaxf(Ta, T.w), 1.00001f, Am);
+                float t0, t1, t2, t3;
+                unpk2(fma2(dz0, dz0, fma2(dy0, dy0, fma2(dx0, dx0, pk2(n0, n1)))), t0, t1);
+                unpk2(fma2(dz1, dz1, fma2(dy1, dy1, fma2(dx1, dx1, pk2(n2, n3)))), t2, t3);
+                append_if_neg(t0, bp0, b); append_if_neg(t1, bp1, b); append_if_neg(t2, bp2, b); append_if_neg(t3, bp3, b);
+            };
+            const uint2* wb4 = reinterpret_cast<const uint2*>(wblk);
             if (uni) {
-                const float nT = TG[48];                                // one h in the whole unit: one threshold (the warp's first target:
-                const f32x2 nT2 = pk2(nT, nT);                          // a lane whose own target slot is empty must not use its own)
-                for (uint32_t n = n0; n < n1; ++n) {
-                    const uint32_t s = 8u * (uint32_t)wblk[4u * n + sub] + bank;
-                    const float cx = X[s], cy = Y[s], cz = Z[s];
-                    const f32x2 cx2 = pk2(cx, cx), cy2 = pk2(cy, cy), cz2 = pk2(cz, cz);
-#pragma unroll
-                    for (int p = 0; p < 8; ++p) {
-                        const f32x2 dx = sub2(tx[p], cx2), dy = sub2(ty[p], cy2), dz = sub2(tz[p], cz2);
-                        float t0, t1;
-                        unpk2(fma2(dz, dz, fma2(dy, dy, fma2(dx, dx, nT2))), t0, t1);
-                        m[2 * p] = shift_in_sign(m[2 * p], t0);
-                        m[2 * p + 1] = shift_in_sign(m[2 * p + 1], t1);
-                        tmin = fminf(tmin, fminf(fabsf(t0), fabsf(t1)));
-                    }
+                for (uint32_t k = 0; k < nwb; k += 4) {
+                    const uint2 w = wb4[k >> 2];
+                    block_uni(w.x & 0xFFFFu); block_uni(w.x >> 16); block_uni(w.y & 0xFFFFu); block_uni(w.y >> 16);
+                    bp0 = min(bp0, e0); bp1 = min(bp1, e1); bp2 = min(bp2, e2); bp3 = min(bp3, e3);
                 }
             } else {
-                // variable h: support of the larger h of the pair, t = r2 - max(T_hi(a), T_hi(b)) < 0  <=>  r2 - T_hi(a) < 0 or
-                // r2 - T_hi(b) < 0; every hit is classified again below
-                const float2* nt2 = reinterpret_cast<const float2*>(TG) + 24;
-                for (uint32_t n = n0; n < n1; ++n) {
-                    const uint32_t s = 8u * (uint32_t)wblk[4u * n + sub] + bank;
-                    const float cx = X[s], cy = Y[s], cz = Z[s], nTb = -fmaf(Tc[s], 1.00001f, Am);
-                    const f32x2 cx2 = pk2(cx, cx), cy2 = pk2(cy, cy), cz2 = pk2(cz, cz), nTb2 = pk2(nTb, nTb);
-#pragma unroll
-                    for (int p = 0; p < 8; ++p) {
-                        const f32x2 dx = sub2(tx[p], cx2), dy = sub2(ty[p], cy2), dz = sub2(tz[p], cz2);
-                        const f32x2 r2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
-                        const float2 na = nt2[p];
-                        float a0, a1, b0, b1;
-                        unpk2(add2(r2, pk2(na.x, na.y)), a0, a1);
-                        unpk2(add2(r2, nTb2), b0, b1);
-                        m[2 * p] = shift_in_sign(m[2 * p], __uint_as_float(__float_as_uint(a0) | __float_as_uint(b0)));
-                        m[2 * p + 1] = shift_in_sign(m[2 * p + 1], __uint_as_float(__float_as_uint(a1) | __float_as_uint(b1)));
-                    }
+                for (uint32_t k = 0; k < nwb; k += 4) {
+                    const uint2 w = wb4[k >> 2];
+                    block_gen(w.x & 0xFFFFu); block_gen(w.x >> 16); block_gen(w.y & 0xFFFFu); block_gen(w.y >> 16);
+                    bp0 = min(bp0, e0); bp1 = min(bp1, e1); bp2 = min(bp2, e2); bp3 = min(bp3, e3);
                 }
             }
-            // transpose: word [chunk][target][lane] = the target's hits among this lane's candidates of the chunk
-#pragma unroll
-            for (int k = 0; k < 16; ++k) MS[(c * 16 + k) * MS_STRIDE + lane] = m[k];
-            }
         }
-        __syncwarp();
-        // Certain scan: no test of the warp within the uncertainty band of the support boundary, i.e. every fp32 decision
+        asm volatile("" ::: "memory");                                  // the appends above wrote the buckets
+        // ---- settle.  An entry is the block number of a hit of the fp32 test; its slot is 8 block + 4 u + bucket.
+        uint32_t cnt = 0, ng = 0;                                       // cnt: 4 x 8-bit bucket fills
+        bool ovf = (bp0 >= e0) || (bp1 >= e1) || (bp2 >= e2) || (bp3 >= e3), coinc = false;
+        // Certain scan: no tested candidate within the uncertainty band of the support boundary, i.e. every fp32 decision
         // holds for the exact predicate too.  |t| >= band  <=>  r2_fp32 outside [T_lo, T_hi + (T_hi - T_lo)).
-        const float band = __shfl_sync(0xFFFFFFFFu, Ta_hi - Ta_lo, 0);
-        const bool certain = uni && !__any_sync(0xFFFFFFFFu, tmin < band);
-        // ---- my four banks (beta = u, u + 2, u + 4, u + 6) of my target: take the target itself out, settle if needed, count
-        uint32_t* Mt = MS + it * MS_STRIDE;                             // word kk of bank beta: Mt[(kk >> 2) * 16 * MS_STRIDE + beta + 8 (kk & 3)]
-        auto mword = [&](uint32_t beta, uint32_t kk) -> uint32_t& { return Mt[(kk >> 2) * (16 * MS_STRIDE) + beta + 8u * (kk & 3u)]; };
-        auto bit_slot = [&](uint32_t beta, uint32_t kk, uint32_t p) {
-            const uint32_t c = kk >> 2, n = 32u * c + chunk_n(c) - 1u - p;
-            return 8u * (uint32_t)wblk[4u * n + (kk & 3u)] + beta;
-        };
-        uint32_t cnt = 0, ng = 0;                                       // cnt: 4 x 8-bit hit counts of my banks
-        bool coinc = false;
-        if (active && NT > 0 && (o_self & 1u) == (uint32_t)u) {
-            // the target itself (r = 0) is among the hits of bank o_self & 7: lane o_self & 31, iteration o_self >> 5
-            const uint32_t n = o_self >> 5, c = n >> 5;
-            Mt[c * (16 * MS_STRIDE) + (o_self & 31u)] &= ~(1u << (chunk_n(c) - 1u - (n & 31u)));
-        }
-        __syncwarp();
-#pragma unroll
-        for (int bb = 0; bb < 4; ++bb) {
-            const uint32_t beta = (uint32_t)u + 2u * bb;
-            uint32_t c = 0;
-#pragma unroll 1
-            for (uint32_t k = 0; k < 4u * NCH; ++k) {
-                uint32_t w = mword(beta, k);
-                if (!certain && active) {
-                    // classify every hit again: certain by the fp32 bounds, else the exact fp64 contract predicate (O2/A12)
-                    uint32_t keep = w;
-                    while (w) {
-                        const uint32_t p = 31u - (uint32_t)__clz(w);
-                        w ^= 1u << p;
-                        const uint32_t s = bit_slot(beta, k, p);
-                        bool in_s = true, in_g = true;
-                        const float dx = fax - X[s], dy = fay - Y[s], dz = faz - Z[s];
-                        const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                        const float Tm = fmaxf(Ta, Tc[s]);
-                        if (r2 < fmaf(Tm, 0.99999f, -Am) && (r2 < Ta_lo || r2 >= Ta_hi) && r2 > 0.0f) {
-                            in_g = r2 < Ta_lo;                          // certain member of N_sym; N_gather decided with the same margin
-                        } else {
-                            int q = 0;
-                            while (q + 1 < (int)S.nranges && S.r_base[q + 1] <= s) ++q;
-                            const uint32_t k2 = s - S.r_base[q];
-                            if (k2 >= S.r_vend[q] - S.r_vstart[q]) {
-                                in_s = false;                           // pad slot (cannot hit; kept for safety)
-                            } else {
-                                const uint32_t gi = S.r_vstart[q] + k2;
-                                const double2 xy = A.p0[gi], zh = A.p1[gi];
-                                const double ex2 = min_image(__dsub_rn(xa, xy.x), g.per[0], g.L[0], g.halfL[0]);
-                                const double ey2 = min_image(__dsub_rn(ya, xy.y), g.per[1], g.L[1], g.halfL[1]);
-                                const double ez2 = min_image(__dsub_rn(za, zh.x), g.per[2], g.L[2], g.halfL[2]);
-                                const double e2x = r2_exact(ex2, ey2, ez2);
-                                in_s = gi != i && e2x < support2(fmax(ha, zh.y));
-                                in_g = in_s && e2x < support2(ha);
-                                if (in_s && !(e2x > 1.0e-290)) coinc = true;   // (near-)coincident particles: general kernels (A11)
-                            }
-                        }
-                        if (!in_s) keep ^= 1u << p;
-                        ng += (in_s && in_g) ? 1u : 0u;
-                    }
-                    mword(beta, k) = keep;
-                    w = keep;
+        const bool certain = uni && tmin >= (Ta_hi - Ta_lo);
+        const bool sees_self = active && ((s_self >> 2) & 1u) == (uint32_t)u;
+        const bool full_settle = __any_sync(0xFFFFFFFFu, !certain && !ovf);
+        if (!full_settle) {
+            // the target itself (r = 0) is met by the thread that owns its bank: take that one entry out of its bucket
+            const uint32_t n0 = (bp0 - bk0) / BROW, n1 = (bp1 - (bk0 + LIST_BS * BROW)) / BROW;
+            const uint32_t n2 = (bp2 - (bk0 + 2 * LIST_BS * BROW)) / BROW, n3 = (bp3 - (bk0 + 3 * LIST_BS * BROW)) / BROW;
+            cnt = n0 | (n1 << 8) | (n2 << 16) | (n3 << 24);
+            if (sees_self && !ovf) {
+                const int b = (int)(s_self & 3u);
+                uint16_t* bb = B + (size_t)b * LIST_BS * BL_THREADS + tid;
+                const uint32_t nb = (cnt >> (8 * b)) & 0xFFu, want = s_self >> 3;
+                uint32_t k = 0;
+                while (k < nb && bb[k * BL_THREADS] != want) ++k;
+                if (k < nb) {                                           // the last entry takes its place (order is free)
+                    bb[k * BL_THREADS] = bb[(nb - 1) * BL_THREADS];
+                    cnt -= 1u << (8 * b);
                 }
-                c += (uint32_t)__popc(w);
             }
-            cnt |= min(c, 255u) << (8 * bb);
-            if (c > (uint32_t)LIST_BC) { coinc = true; atomicAdd(&A.ctr[CTR_DECL + 2], 1ull); }   // more than 24 neighbours in one bank: general kernels
+            ng = (cnt & 0xFFu) + ((cnt >> 8) & 0xFFu) + ((cnt >> 16) & 0xFFu) + (cnt >> 24);
+        } else if (!ovf) {
+#pragma unroll
+            for (int b = 0; b < 4; ++b) {
+                const uint32_t nb = ((b == 0 ? bp0 : b == 1 ? bp1 : b == 2 ? bp2 : bp3) - (bk0 + b * LIST_BS * BROW)) / BROW;
+                uint16_t* bb = B + (size_t)b * LIST_BS * BL_THREADS + tid;
+                uint32_t w = 0;
+                for (uint32_t k = 0; k < nb; ++k) {
+                    const uint32_t blk = bb[k * BL_THREADS], s = (blk << 3) + 4u * (uint32_t)u + (uint32_t)b;
+                    bool in_s = true, in_g = true;
+                    const float dx = fax - X[s], dy = fay - Y[s], dz = faz - Z[s];
+                    const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                    const float Tm = fmaxf(Ta, Tc[s]);
+                    if (r2 < fmaf(Tm, 0.99999f, -Am) && (r2 < Ta_lo || r2 >= Ta_hi) && r2 > 0.0f) {
+                        in_g = r2 < Ta_lo;                              // certain member of N_sym; N_gather decided with the same margin
+                    } else if (s == s_self) {
+                        in_s = false;
+                    } else {
+                        int q = 0;
+                        while (q + 1 < (int)S.nranges && S.r_base[q + 1] <= s) ++q;
+                        const uint32_t k2 = s - S.r_base[q];
+                        if (k2 >= S.r_vend[q] - S.r_vstart[q]) {
+                            in_s = false;                               // pad slot (cannot hit; kept for safety)
+                        } else {
+                            const uint32_t gi = S.r_vstart[q] + k2;
+                            const double2 xy = A.p0[gi], zh = A.p1[gi];
+                            const double ex2 = min_image(__dsub_rn(xa, xy.x), g.per[0], g.L[0], g.halfL[0]);
+                            const double ey2 = min_image(__dsub_rn(ya, xy.y), g.per[1], g.L[1], g.halfL[1]);
+                            const double ez2 = min_image(__dsub_rn(za, zh.x), g.per[2], g.L[2], g.halfL[2]);
+                            const double e2x = r2_exact(ex2, ey2, ez2);
+                            in_s = gi != i && e2x < support2(fmax(ha, zh.y));
+                            in_g = in_s && e2x < support2(ha);
+                            if (in_s && !(e2x > 1.0e-290)) coinc = true;    // (near-)coincident particles: left to the general kernels (A11)
+                        }
+                    }
+                    if (in_s) bb[w * BL_THREADS] = (uint16_t)blk;
+                    w += in_s ? 1u : 0u;
+                    ng += (in_s && in_g) ? 1u : 0u;
+                }
+                cnt |= w << (8 * b);
+            }
         }
-        if (certain) ng = (cnt & 0xFFu) + ((cnt >> 8) & 0xFFu) + ((cnt >> 16) & 0xFFu) + (cnt >> 24);
-        if (coinc) s_bad = 1;
-        __syncwarp();
-        // ---- split every bank of the target between its two half-lists (alternate hits)
+        if (ovf || coinc) s_bad = 1;
+        // ---- split every bank bucket of the target between its two threads (alternate entries)
         const uint32_t cnt_o = __shfl_xor_sync(0xFFFFFFFFu, cnt, 1);
         ng += __shfl_xor_sync(0xFFFFFFFFu, ng, 1);
-        uint32_t cu = 0;                                                // 8 x 4-bit: hits of bank beta that go to MY half-list
+        uint32_t cu = 0;                                                // 8 x 4-bit: entries of bank beta that are mine (<= LIST_BC / 2)
         uint32_t n_lane = 0, nsym = 0;
 #pragma unroll
         for (int beta = 0; beta < 8; ++beta) {
-            const uint32_t cb = (((beta & 1) == u ? cnt : cnt_o) >> (8 * (beta >> 1))) & 0xFFu;
+            const uint32_t cb = ((bank_owner(beta) == u ? cnt : cnt_o) >> (8 * bank_local(beta))) & 0xFFu;
             const uint32_t f = (uint32_t)(u + beta) & 1u;
             const uint32_t mine = (cb + 1u - f) >> 1;
-            cu |= min(mine, 15u) << (4 * beta);
+            cu |= mine << (4 * beta);
             n_lane += mine; nsym += cb;
         }
         uint32_t R = n_lane;
@@ -604,10 +568,9 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
         // kernels after this one has emitted (list too long, pool exhausted), the rows stay unused.
         uint32_t row0 = 0;
         bool wbad = R > (uint32_t)LIST_RMAX || s_bad != 0;
-        if (lane == 0 && R > (uint32_t)LIST_RMAX) atomicAdd(&A.ctr[CTR_DECL + 2], 1ull);
         if (lane == 0 && !wbad && R) {
             const unsigned long long r0 = atomicAdd(&A.ctr[CTR_POOL], (unsigned long long)(R >> 2));
-            if (r0 + (R >> 2) > (unsigned long long)A.pool_rows) { wbad = true; atomicAdd(&A.ctr[CTR_DECL + 3], 1ull); }   // pool exhausted: general kernels
+            if (r0 + (R >> 2) > (unsigned long long)A.pool_rows) wbad = true;   // pool exhausted: general kernels
             row0 = (uint32_t)r0;
         }
         wbad = __shfl_sync(0xFFFFFFFFu, (int)wbad, 0) != 0;
@@ -615,81 +578,71 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
         if (wbad) {
             if (lane == 0) s_bad = 1;
         } else {
-            // ---- emit the half-lists in scheduled order: lane jj of an 8-lane group spends phase t = rounds [tR/8, (t+1)R/8)
-            //      in bank (jj + t) & 7; what a phase cannot hold fills the holes of other phases; the rest are dummies.
+            // ---- emit my half-list in scheduled order (see the header): phase t = rounds [tR/8, (t+1)R/8) in bank
+            //      (j + t) & 7; what a phase cannot hold (overflow) fills the holes of other phases; the rest are dummies.
             // R = 8 m + 4 e (e = 0, 1): phase t starts at t m + e (t >> 1) and holds m + e (t & 1) rounds.
-            // The schedule is laid out [round / 4][list column][round & 3] (u16), so that four rounds leave as one 8-byte word.
             const uint32_t m8 = R >> 3, e4 = (R >> 2) & 1u;
-            const uint32_t Lb = (uint32_t)__cvta_generic_to_shared(smem + BL_OFF_L);
-            const uint32_t Qb = (uint32_t)__cvta_generic_to_shared(LQ);
-            auto out_addr = [&](uint32_t col, uint32_t r) { return Lb + ((r >> 2) * BL_THREADS + col) * 8u + (r & 3u) * 2u; };
-            uint32_t nq0 = 0, nq1 = 0;                                  // left-overs I queued for half-list 0 / 1 of my target
-            // pass 1: I deal the hits of my four banks alternately to the two half-lists of my target (the first hit of bank
-            // beta goes to half-list beta & 1): hit number e of a half-list's share goes to round (phase start) + e, or to that
-            // half-list's left-over queue when the phase is full
-#pragma unroll 1
-            for (int bb = 0; bb < 4; ++bb) {
-                const uint32_t beta = (uint32_t)u + 2u * bb;
-                uint32_t st[2], cp[2];
+            uint16_t* out = Lf + tid;                                   // my column of the schedule: out[r * BL_THREADS]
+            const uint16_t* Bp = B + (tid & ~1);
+            uint32_t own[8], ovr[8];                                    // per phase: entries placed in the phase / left over
+            const uint16_t* bq[8];                                      // per phase: my entries of its bank (stride 2 rows)
+            uint32_t Hw = 0;                                            // 8 x 4-bit: holes of each phase
 #pragma unroll
-                for (int v = 0; v < 2; ++v) {
-                    const uint32_t t = (beta - (((uint32_t)j & 6u) | (uint32_t)v)) & 7u;   // phase in which half-list v visits bank beta
-                    cp[v] = m8 + (e4 & t & 1u);
-                    st[v] = t * m8 + (e4 ? (t >> 1) : 0u);
-                }
-                uint32_t r = 0;
-#pragma unroll 1
-                for (uint32_t k = 0; k < 4u * NCH; ++k) {
-                    uint32_t w = mword(beta, k);
-                    while (w) {
-                        const uint32_t p = 31u - (uint32_t)__clz(w);
-                        w ^= 1u << p;
-                        const uint32_t slot = bit_slot(beta, k, p);
-                        const uint32_t v = (r + beta) & 1u, e = r >> 1;
-                        ++r;
-                        const uint32_t col = ((uint32_t)tid & ~1u) | v;
-                        if (e < cp[v]) {
-                            sts_u16(out_addr(col, st[v] + e), slot);
-                        } else {
-                            const uint32_t nq = v ? nq1 : nq0;
-                            if (nq < (uint32_t)LQ_CAP) sts_u16(Qb + ((col * 2u + (uint32_t)u) * LQ_CAP + nq) * 2u, slot);
-                            if (v) ++nq1; else ++nq0;
-                        }
-                    }
-                }
+            for (int t = 0; t < 8; ++t) {
+                const int beta = (j + t) & 7;
+                const uint32_t cap = m8 + (e4 & (uint32_t)(t & 1));
+                const uint32_t c = (cu >> (4 * beta)) & 15u;
+                own[t] = min(c, cap);
+                ovr[t] = c - own[t];
+                Hw |= (cap - own[t]) << (4 * t);
+                // my entries of bank beta: indices f, f+2, ... of the bucket of thread bank_owner(beta)
+                bq[t] = Bp + (bank_local(beta) * LIST_BS + ((u + beta) & 1)) * BL_THREADS + bank_owner(beta);
             }
-            __syncwarp();
-            // pass 2: the holes of MY half-list take its left-overs (queued by me, then by my partner), then dummy slots of the
-            // phase's bank
-            {
-                const uint32_t mine_q = u ? nq1 : nq0;                                 // queued by me for my own half-list
-                const uint32_t part_q = __shfl_xor_sync(0xFFFFFFFFu, u ? nq0 : nq1, 1);  // queued by my partner for my half-list
-                if (nq0 > (uint32_t)LQ_CAP || nq1 > (uint32_t)LQ_CAP) { s_bad = 1; atomicAdd(&A.ctr[CTR_DECL + 1], 1ull); }   // queue overflow: general kernels
-                uint32_t taken = 0;
-                const uint32_t qa = Qb + (((uint32_t)tid * 2u + (uint32_t)u) * LQ_CAP) * 2u, qb = Qb + (((uint32_t)tid * 2u + (uint32_t)(u ^ 1)) * LQ_CAP) * 2u;
-#pragma unroll 1
-                for (uint32_t t = 0; t < 8; ++t) {
+            // pass 1 (lockstep): every phase takes its own bank's entries up to its capacity (an entry is a block number:
+            // slot = 8 block + bank); a hole gets the dummy slot of the phase's bank
+            for (uint32_t k = 0; k < m8; ++k) {
+#pragma unroll
+                for (int t = 0; t < 8; ++t) {
                     const uint32_t beta = (uint32_t)(j + t) & 7u;
-                    const uint32_t cap = m8 + (e4 & t & 1u);
-                    const uint32_t own = min((cu >> (4 * beta)) & 15u, cap);
-                    const uint32_t r0 = t * m8 + (e4 ? (t >> 1) : 0u);
-                    for (uint32_t k = own; k < cap; ++k) {
-                        uint32_t item = (uint32_t)TILE_CMAX + beta;
-                        if (taken < mine_q) item = lds_u16(qa + 2u * min(taken, (uint32_t)LQ_CAP - 1u));
-                        else if (taken < mine_q + part_q) item = lds_u16(qb + 2u * min(taken - mine_q, (uint32_t)LQ_CAP - 1u));
-                        ++taken;
-                        sts_u16(out_addr((uint32_t)tid, r0 + k), item);
-                    }
+                    uint32_t item = (uint32_t)TILE_CMAX + beta;
+                    if (k < own[t]) item = ((uint32_t)bq[t][2 * k * BL_THREADS] << 3) + beta;
+                    out[((uint32_t)t * m8 + (e4 ? (uint32_t)(t >> 1) : 0u) + k) * BL_THREADS] = (uint16_t)item;
                 }
             }
-            __syncwarp();
-            // pass 3: four rounds per 8-byte store
+            if (e4) {
+#pragma unroll
+                for (int t = 1; t < 8; t += 2) {
+                    const uint32_t beta = (uint32_t)(j + t) & 7u;
+                    uint32_t item = (uint32_t)TILE_CMAX + beta;
+                    if (m8 < own[t]) item = ((uint32_t)bq[t][2 * m8 * BL_THREADS] << 3) + beta;
+                    out[((uint32_t)t * m8 + (uint32_t)(t >> 1) + m8) * BL_THREADS] = (uint16_t)item;
+                }
+            }
+            // the left-over entries go into the holes (a phase has either holes or left-overs): one left-over per iteration,
+            // its phase and the phase of the next hole are the first non-zero 4-bit fields
+            {
+                uint32_t Ov = 0;
+#pragma unroll
+                for (int t = 0; t < 8; ++t) Ov |= ovr[t] << (4 * t);
+                const uint32_t Ov0 = Ov;
+                while (Ov != 0u && Hw != 0u) {                          // Hw runs out only after Ov: n_lane <= R
+                    const uint32_t ts = (uint32_t)(__ffs((int)Ov) - 1) >> 2, th = (uint32_t)(__ffs((int)Hw) - 1) >> 2;
+                    const uint32_t beta = ((uint32_t)j + ts) & 7u;
+                    const uint32_t cap_s = m8 + (e4 & ts & 1u);         // a phase with left-overs is full: own = cap
+                    const uint32_t taken = ((Ov0 >> (4 * ts)) & 15u) - ((Ov >> (4 * ts)) & 15u);
+                    const uint16_t* src = Bp + (bank_local((int)beta) * LIST_BS + ((u + (int)beta) & 1)) * BL_THREADS + bank_owner((int)beta);
+                    const uint32_t hrem = (Hw >> (4 * th)) & 15u;
+                    const uint32_t pos = (((th + 1u) * R) >> 3) - hrem;
+                    out[pos * BL_THREADS] = (uint16_t)(((uint32_t)src[2 * (cap_s + taken) * BL_THREADS] << 3) + beta);
+                    Ov -= 1u << (4 * ts); Hw -= 1u << (4 * th);
+                }
+            }
+            // pass 2: pack 4 rounds per 8-byte store
             uint2* blk = A.pool + (size_t)row0 * 32 + lane;
-            const uint32_t nr4 = R >> 2;
-            for (uint32_t r4 = 0; r4 < nr4; ++r4) {
-                uint2 v;
-                asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(Lb + (r4 * BL_THREADS + (uint32_t)tid) * 8u) : "memory");
-                blk[(size_t)r4 * 32] = v;
+            for (uint32_t r4 = 0; r4 < R; r4 += 4) {
+                const uint32_t e0 = out[r4 * BL_THREADS], e1 = out[(r4 + 1) * BL_THREADS];
+                const uint32_t e2 = out[(r4 + 2) * BL_THREADS], e3 = out[(r4 + 3) * BL_THREADS];
+                blk[(size_t)(r4 >> 2) * 32] = make_uint2(e0 | (e1 << 16), e2 | (e3 << 16));
             }
             if (u == 0) A.lcount[(size_t)tile * TILE_T + tgt] = active ? (ng | (nsym << 16)) : 0u;
             if (lane == 0) A.winfo[(size_t)tile * TILE_WARPS + twarp] = make_uint2(row0, R);
