@@ -45,6 +45,47 @@ def peaks():
         return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
 
 
+def traffic_table(workload):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture of this workload
+    (profiles/r02_traffic.csv: workload, kernel, read bytes, written bytes, commit).  Empty when there is no capture."""
+    out = {}
+    try:
+        for line in open(os.path.join(ROOT, "profiles", "r02_traffic.csv")):
+            f = [c.strip() for c in line.split(",")]
+            if len(f) >= 4 and f[0] == workload:
+                out[f[1]] = float(f[2]) + float(f[3])
+    except Exception:
+        pass
+    return out
+
+
+def approaching_fraction(workload):
+    """Fraction of ordered neighbour pairs with v_ab . x_ab < 0 (the pairs that take the viscous branch, eqs. (41)-(43)), MEASURED
+    on the reduced-size preset of the same recipe (same lattice, jitter and velocity law, so the same fraction): the neighbour
+    lists of the 48^3 set from the library's own export, the dot products in torch."""
+    import numpy as np
+    import torch
+    import workloads as W
+    import paper_2604_20124_b200 as P
+    small = {"c5_v": "c5_mid", "c5": "c5_mid", "c4": "c4_mid", "c3": "c3_mid", "c2": "c2_mid", "c1": "c1"}.get(workload, workload)
+    w = W.make(small)
+    dev = torch.device("cuda", torch.cuda.current_device())
+    t = {f: torch.from_numpy(np.ascontiguousarray(getattr(w, f))).to(dev) for f in ("x", "y", "z", "h", "vx", "vy", "vz")}
+    sp = P.Spray(w.n, w.grid.ncell_total, device=dev.index or 0)
+    sp.build_cells(w.grid, w.kernel, t["x"], t["y"], t["z"], t["h"])
+    off, nbr = sp.neighbor_lists(True)
+    a = torch.repeat_interleave(torch.arange(w.n, device=dev), (off[1:] - off[:-1]).to(torch.int64))
+    b = nbr.to(torch.int64)
+    dot = torch.zeros(a.shape[0], dtype=torch.float64, device=dev)
+    for k, (c, v) in enumerate((("x", "vx"), ("y", "vy"), ("z", "vz"))):
+        dx = t[c][a] - t[c][b]
+        if w.grid.periodic[k]:
+            L = float(w.grid.hi[k]) - float(w.grid.lo[k])
+            dx = dx - L * torch.round(dx / L)
+        dot += dx * (t[v][a] - t[v][b])
+    return float((dot < 0).double().mean().item())
+
+
 def cpu_model():
     try:
         for line in open("/proc/cpuinfo"):
@@ -174,8 +215,15 @@ def main():
                     help="pass = build, density, spray_hydro_rhs, spray_fld_apply(UPDATE_LIMITER) (two sweeps) instead of the default "
                          "build, density, spray_hydro_rhs_limiter (hydro + limiter in one sweep), spray_fld_apply(FROZEN): same outputs, bitwise")
     ap.add_argument("--no-n1", action="store_true", help="skip the row-N1/N3 measurements (spray_rad_jacobi iterations, spray_kgc_continuity)")
+    ap.add_argument("--no-variants", action="store_true", help="skip the c5_v variant (v ~ N(0, 0.01^2): the viscous branch at full size)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    # --gpus N without a launcher: start the N replica ranks ourselves (one process per GPU, torchrun on 127.0.0.1)
+    if args.impl == "ours" and args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        port = 29500 + os.getpid() % 2000
+        os.execv(sys.executable, [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+                                  "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:])
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -245,7 +293,8 @@ def main():
     cg = int(sp.neighbor_counts(False).to(torch.int64).sum().item())
     cs = int(sp.neighbor_counts(True).to(torch.int64).sum().item())
     assert sp.check() == 0, "device status flags set"
-    n_tiles, n_fast = sp.path_stats()
+    pstats = sp.path_stats_full()
+    n_tiles, n_fast = pstats["tiles"], pstats["n_fast"]
     pairs = {"density": cg + n, "hydro": cs, "limiter": cg, "apply": cs}
     p_pass = sum(pairs.values())
 
@@ -476,9 +525,39 @@ def main():
               "absorbed_fraction": float(rr["edep"].sum() / rays[6].sum()),
               "note": "includes the gradient sweep over all particles (prologue + SW_GRADN) and the deposit scatter"}
 
-    # ---- roofline: pass level and dominant kernel
+    # ---- variant of SURVEY 8(d) config 5: the same particle set with v ~ N(0, 0.01^2), so that about half of the pairs take the
+    #      viscous branch of eqs. (41)-(43); same pass, timed the same way (headline stays the literal v = 0 config)
+    variants = None
+    if w.name.startswith("c5") and not (np.any(w.vx) or np.any(w.vy) or np.any(w.vz)) and not args.no_variants and not args.no_n1:
+        wv = W.make("c5_v")
+        dv = dict(d)
+        for f in ("vx", "vy", "vz"):
+            dv[f] = torch.from_numpy(np.ascontiguousarray(getattr(wv, f))).to(dev)
+        for _ in range(3):
+            one_pass(dv)
+        torch.cuda.synchronize()
+        v0, v1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        nv = max(3, min(args.steps, 10))
+        v0.record()
+        for _ in range(nv):
+            one_pass(dv)
+        v1.record()
+        torch.cuda.synchronize()
+        t_v = v0.elapsed_time(v1) * 1e-3 / nv
+        fv = approaching_fraction("c5_v")
+        flv = FLOPS[w.kernel]
+        flops_v = (pairs["density"] * flv["density"] + pairs["hydro"] * (flv["hydro"] + fv * flv["hydro_visc"]) +
+                   pairs["limiter"] * flv["limiter"] + pairs["apply"] * flv["apply"])
+        variants = {"c5_v": {"workload": wv.name, "ms_per_pass": 1e3 * t_v, "pair_interactions_per_s": p_pass / t_v,
+                             "approaching_pair_fraction": fv, "flops": flops_v, "frac": flops_v / (fp64_meas * 1e12) / t_v,
+                             "note": "v ~ N(0, 0.01^2): the +25-flop viscous term weighted by the measured fraction of approaching pairs"}}
+        del wv, dv
+
+    # ---- roofline.  Top level = the WHOLE PASS, the quantity BASELINE.json's north_star targets;
+    #      `kernels` lists every part of the pass with its measured time, share, algorithmic work and fraction of its own bound.
     fl = FLOPS[w.kernel]
-    visc_frac = 0.0 if not (np.any(w.vx) or np.any(w.vy) or np.any(w.vz)) else 0.5
+    moving = bool(np.any(w.vx) or np.any(w.vy) or np.any(w.vz))
+    visc_frac = approaching_fraction(args.workload) if moving else 0.0
     flops = {"density": pairs["density"] * fl["density"], "hydro": pairs["hydro"] * (fl["hydro"] + visc_frac * fl["hydro_visc"]),
              "limiter": pairs["limiter"] * fl["limiter"], "apply": pairs["apply"] * fl["apply"]}
     seg_mean = seg.mean(axis=0)
@@ -486,24 +565,48 @@ def main():
     t_alu = sum(flops.values()) / (fp64_meas * 1e12)
     t_hbm = BYTES_PER_PARTICLE * n / (pk["hbm_gbs"] * 1e9)
     calls = {"build": seg_mean[0], "density": seg_mean[1], "hydro": seg_mean[2], "fld": seg_mean[3]}
-    # dominant kernel: the hydro sweep; in the default pass it also carries the limiter sums, so its algorithmic work is both rows
     hyd_flops = flops["hydro"] + (flops["limiter"] if fused else 0.0)
     fld_flops = flops["apply"] + (0.0 if fused else flops["limiter"])
-    hydro_tflops = hyd_flops / calls["hydro"] / 1e12
-    # dram__bytes_read.sum + dram__bytes_write.sum of k_tiled_sweep<1,0> per launch at c5, one ncu --set full capture
-    # (profiles/r01d_ncu_full_tiled_path.md); null for other workloads
-    # (fused sweep k_tiled_sweep<10,0,1>: profiles/r01h_ncu_full_fused_pass.md)
-    traffic = ((6.87e9 + 1.20e9) if fused else (6.01e9 + 0.67e9)) if w.name.startswith("c5") else None
-    kname = ("hydro + limiter pair sweep (spray_hydro_rhs_limiter: prologue k_prep_hydro + k_tiled_sweep<10>; algorithmic flops of rows a6 + a7)"
-             if fused else "hydro pair sweep (spray_hydro_rhs: prologue k_prep_hydro + k_tiled_sweep<1>)")
-    roofline = {"bound": "alu", "kernel": kname,
-                "achieved": hydro_tflops, "peak": fp64_meas, "unit": "TFLOP/s", "frac": hydro_tflops / fp64_meas,
+    # parts of spray_build_cells from the events the call records on its stream (spray_build_timing), a few extra passes
+    bt = np.zeros(3)
+    for _ in range(3):
+        sp.build_cells(w.grid, w.kernel, d["x"], d["y"], d["z"], d["h"])
+        bt += np.array(sp.build_timing())
+    bt *= 1e-3 / 3
+    hbm = pk["hbm_gbs"] * 1e9
+    pk64 = fp64_meas * 1e12
+    b_cells = (32 + 48 + 64) * n                       # keys, three sort passes, reorder
+    b_lists = (2 * 32 + 2 * (pairs["hydro"] / max(n, 1))) * n      # candidates read once per tile row (32 B twice) + 2 B per neighbour written
+    tr = traffic_table(w.name)
+    def part(name, kernel, sec, bound, work, peak, extra=None):
+        e = {"part": name, "kernel": kernel, "ms": 1e3 * float(sec), "share": float(sec) / t_step, "bound": bound,
+             "algorithmic": work, "unit": "flop" if bound == "alu" else "B",
+             "frac": (work / max(float(sec), 1e-12)) / peak if work else 0.0, "traffic": tr.get(kernel)}
+        if extra:
+            e.update(extra)
+        return e
+    kernels = [
+        part("cell list (a1-a4)", "k_cell_key..k_ref_sweep<4>", bt[0], "hbm", b_cells, hbm),
+        part("tiles + tables", "k_mark_coincident..k_tile_tables", bt[1], "hbm", 0, hbm, {"note": "index work only"}),
+        part("neighbour lists", "k_build_lists", bt[2], "hbm", b_lists, hbm,
+             {"note": "a search: zero algorithmic flops; bound in practice by shared-memory wavefronts and issue (profiles/r02*)"}),
+        part("density (a5)", "k_prep_density + k_tiled_sweep<0>", calls["density"], "alu", flops["density"], pk64),
+        part("hydro + limiter (a6, a7)" if fused else "hydro (a6)", "k_prep_hydro + k_tiled_sweep<10>" if fused else "k_prep_hydro + k_tiled_sweep<1>",
+             calls["hydro"], "alu", hyd_flops, pk64),
+        part("apply (a8)" if fused else "limiter + apply (a7, a8)", "k_prep_fld + k_tiled_sweep<3>", calls["fld"], "alu", fld_flops, pk64),
+    ]
+    dom = max(kernels, key=lambda e: e["ms"])
+    roofline = {"bound": "alu", "kernel": "whole pass (density + hydro + FLD incl. the cell-list and neighbour-list build): north_star's target quantity",
+                "achieved": sum(flops.values()) / t_step / 1e12, "peak": fp64_meas, "unit": "TFLOP/s",
+                "frac": max(t_alu, t_hbm) / t_step,
                 "peak_source": "DFMA-chain probe measured in this run (spray_fp64_peak_probe); nominal 148x64x2x1.965GHz = %.1f" % FP64_NOMINAL_TFLOPS,
-                "traffic": traffic,
+                "traffic": dom["traffic"], "dominant": dom["part"] + " (" + dom["kernel"] + ")",
+                "kernels": kernels,
                 "pass": {"flops": sum(flops.values()), "bytes": BYTES_PER_PARTICLE * n, "t_alu_ms": 1e3 * t_alu, "t_hbm_ms": 1e3 * t_hbm,
-                         "t_pass_ms": 1e3 * t_step, "frac": max(t_alu, t_hbm) / t_step, "hbm_peak_gbs": pk["hbm_gbs"], "hbm_peak_source": pk_src},
+                         "t_pass_ms": 1e3 * t_step, "frac": max(t_alu, t_hbm) / t_step, "hbm_peak_gbs": pk["hbm_gbs"], "hbm_peak_source": pk_src,
+                         "approaching_pair_fraction": visc_frac},
                 "per_call_ms": {k: 1e3 * float(v) for k, v in calls.items()},
-                "per_call_tflops": {"density": flops["density"] / calls["density"] / 1e12, "hydro": hydro_tflops,
+                "per_call_tflops": {"density": flops["density"] / calls["density"] / 1e12, "hydro": hyd_flops / calls["hydro"] / 1e12,
                                     "fld": fld_flops / calls["fld"] / 1e12},
                 "calls": (["spray_build_cells", "spray_density", "spray_hydro_rhs_limiter", "spray_fld_apply(FROZEN)"] if fused else
                           ["spray_build_cells", "spray_density", "spray_hydro_rhs", "spray_fld_apply(UPDATE_LIMITER)"])}
@@ -533,11 +636,13 @@ def main():
             "data": "synthetic",
             "config": {"workload": w.name, "n_particles": n, "kernel": ["cubic_spline", "wendland_c2"][w.kernel], "grid": list(w.grid.ncell),
                        "pairs_per_pass": p_pass, "unique_ordered_pairs": cs, "unique_pairs_per_s": world * cs * args.steps / t_total,
-                       "l2": "inputs larger than L2 (%.1f GB resident per replica)" % (8e-9 * n * (len(fields) + len(out))),
+                       "l2": "inputs larger than L2 (%.1f GB of caller arrays + %.1f GB of library scratch resident per replica)"
+                             % (8e-9 * n * (len(fields) + len(out)), 1e-9 * pstats["scratch_bytes"]),
+                       "scratch_bytes": pstats["scratch_bytes"], "declined": pstats["declined"],
                        "parallelism": "replicas only" if world > 1 else "1 GPU", "path": args.path,
                        "tiles": n_tiles, "tiled_fraction": n_fast / max(n, 1)},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
-            "fp64_probe_tflops": fp64_meas, "next_rows": {"N1_rad_jacobi": n1, "N2_conduction": n2, "N3_kgc_continuity": n3, "N4_ray_deposit": n4}}
+            "fp64_probe_tflops": fp64_meas, "variants": variants, "next_rows": {"N1_rad_jacobi": n1, "N2_conduction": n2, "N3_kgc_continuity": n3, "N4_ray_deposit": n4}}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
