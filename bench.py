@@ -215,6 +215,7 @@ def main():
                     help="pass = build, density, spray_hydro_rhs, spray_fld_apply(UPDATE_LIMITER) (two sweeps) instead of the default "
                          "build, density, spray_hydro_rhs_limiter (hydro + limiter in one sweep), spray_fld_apply(FROZEN): same outputs, bitwise")
     ap.add_argument("--no-n1", action="store_true", help="skip the row-N1/N3 measurements (spray_rad_jacobi iterations, spray_kgc_continuity)")
+    ap.add_argument("--no-levels", action="store_true", help="do not set up the internal levels of the tiled path for variable-h workloads")
     ap.add_argument("--no-variants", action="store_true", help="skip the c5_v variant (v ~ N(0, 0.01^2): the viscous branch at full size)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
@@ -256,6 +257,11 @@ def main():
     sp = P.Spray(n, w.grid.ncell_total, device=local_rank)
     if args.path is not None:
         sp.set_path(args.path)
+    levels = []
+    if float(w.h.min()) != float(w.h.max()) and not args.no_levels:
+        # variable h (BASELINE.json configs 2 and 4): internal levels of the tiled path, cell edges from the h range (workloads.level_edges)
+        levels = W.level_edges(w.h)
+        sp.set_levels(w.grid, levels)
     f64 = torch.float64
     out = {k: torch.empty(n, dtype=f64, device=dev) for k in ("rho", "ax", "ay", "az", "dudt", "divv", "mu", "y", "diag", "offd")}
     hout = {k: torch.empty(n, dtype=f64).pin_memory() for k in out}
@@ -638,7 +644,7 @@ def main():
                        "pairs_per_pass": p_pass, "unique_ordered_pairs": cs, "unique_pairs_per_s": world * cs * args.steps / t_total,
                        "l2": "inputs larger than L2 (%.1f GB of caller arrays + %.1f GB of library scratch resident per replica)"
                              % (8e-9 * n * (len(fields) + len(out)), 1e-9 * pstats["scratch_bytes"]),
-                       "scratch_bytes": pstats["scratch_bytes"], "declined": pstats["declined"],
+                       "scratch_bytes": pstats["scratch_bytes"], "declined": pstats["declined"], "level_edges": levels,
                        "parallelism": "replicas only" if world > 1 else "1 GPU", "path": args.path,
                        "tiles": n_tiles, "tiled_fraction": n_fast / max(n, 1)},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,

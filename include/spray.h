@@ -96,12 +96,26 @@ int spray_set_path(spray_ctx* ctx, int path);
  * *n_fast = particles served by the tiled kernels (the rest, n - n_fast, by the general kernels),
  * *n_nonuniform = list-builder work units (half tiles) whose particles do not all share one h (they run the
  * variable-h pair bodies), *scratch_bytes = device memory the context holds (allocated at spray_create).
- * declined[k] = list-builder events that left a half tile to the general kernels, by reason: 0 a warp's candidate window
- * longer than 128 blocks of 8 slots, 1 left-over queue overflow in the schedule, 2 a list longer than 80 rounds or more than
- * 24 neighbours in one shared-memory bank, 3 other (coincident particles, particle outside the tile's fp32 range, list pool
- * exhausted).  All host pointers, all nullable. */
+ * declined[k] = list-builder events that left a half tile to the general kernels, by reason: 0 unused, 1 list pool
+ * exhausted, 2 a list longer than 80 rounds or more than 24 neighbours in one shared-memory bank, 3 other (coincident
+ * particles, particle outside the tile's fp32 range).  All host pointers, all nullable. */
 int spray_path_stats(spray_ctx* ctx, void* stream, int64_t* n_tiles, int64_t* n_fast, int64_t* n_nonuniform,
                      int64_t* scratch_bytes, int64_t* declined /* [4] */);
+
+/* Internal levels of the tiled path, for particle sets whose smoothing lengths do not fit one grid (the search
+ * range of a particle follows from the ratio of its smoothing length to the cell size, and neighbours are made mutual).
+ * The tiled kernels need every mutual neighbour of a particle within one cell of the grid they work on; where the caller's
+ * grid (an input, A14) does not give that -- cell edge below 2 h for some particles, or cells holding far more particles
+ * than a tile can stage for others -- the library sorts the particles a second, third, ... time on grids of its own over
+ * the same box: level k has ncell_d = floor(L_d / edges[k]) cells and serves the particles a with 2 hs_a (hs = symmetric
+ * search length: max of h_a and the h of every particle that sees a) above the cell edge of level k - 1 and not above that
+ * of level k; what no level can take (2 hs above the last edge, a tile's candidates over the staging budget) stays with the
+ * general kernels, so results are complete and identical either way.  edges: host, [nlevels], ascending, > 0 (a good
+ * choice: a geometric sequence of ratio ~1.5 from 2 min(h) to 2 max(h)); ncell_max: host, [nlevels], cell capacity of each
+ * level (>= prod floor(L_d / edges[k])).  Allocates the levels' scratch (synchronises the device; call it once, before
+ * spray_build_cells); nlevels = 0 removes them.  Returns SPRAY_ERR_ALLOC when a level cannot be allocated (none is kept).
+ * The cell table, the sort permutation and every output are those of the caller's grid regardless. */
+int spray_set_levels(spray_ctx* ctx, int nlevels, const double* edges, const int64_t* ncell_max);
 
 /* Measurement: device time of the three parts of the LAST spray_build_cells on this context, from CUDA events the call
  * records on its stream (no cost on the path): *ms_cells = keys, sort, cell table, reorder, per-cell h_max, symmetric

@@ -23,7 +23,7 @@ COND_OPERATOR, COND_RHS = 0, 1
 DEV_H_EXCEEDS_HMAX, DEV_OUTSIDE_BOX, DEV_LIST_OVERFLOW = 1, 2, 4
 
 # every symbol include/spray.h declares
-EXPORTS = ["spray_version", "spray_create", "spray_destroy", "spray_last_error", "spray_check", "spray_launch_count", "spray_set_path", "spray_path_stats", "spray_build_timing",
+EXPORTS = ["spray_version", "spray_create", "spray_destroy", "spray_last_error", "spray_check", "spray_launch_count", "spray_set_path", "spray_set_levels", "spray_path_stats", "spray_build_timing",
            "spray_build_cells", "spray_density", "spray_hydro_rhs", "spray_hydro_rhs_limiter", "spray_fld_apply", "spray_get_cell_table",
            "spray_neighbor_counts", "spray_neighbor_lists", "spray_neighbor_digest", "spray_rad_jacobi", "spray_conduction", "spray_kgc_continuity", "spray_ray_deposit", "spray_conduction_implicit", "spray_fp64_peak_probe"]
 
@@ -61,6 +61,7 @@ def load():
     lib.spray_set_path.argtypes = [vp, i32]
     lib.spray_launch_count.argtypes = [vp]
     lib.spray_path_stats.argtypes = [vp, vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+    lib.spray_set_levels.argtypes = [vp, i32, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
     lib.spray_build_timing.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double)]
     lib.spray_build_cells.argtypes = [vp, C.POINTER(Grid), i32, i64, vp, vp, vp, vp, vp]
     lib.spray_density.argtypes = [vp, vp, vp, vp, vp]
@@ -159,6 +160,19 @@ class Spray:
         self._ck(self.lib.spray_path_stats(self.h, _stream(), C.byref(nt), C.byref(nf), C.byref(nn), C.byref(nb), dec), "spray_path_stats")
         return {"tiles": int(nt.value), "n_fast": int(nf.value), "nonuniform_units": int(nn.value), "scratch_bytes": int(nb.value),
                 "declined": [int(x) for x in dec]}
+
+    def set_levels(self, grid, edges):
+        """Internal levels of the tiled path on the box of `grid`: one grid of cell edge >= edges[k] each (ascending)."""
+        edges = [float(e) for e in edges]
+        nc = []
+        for e in edges:
+            m = 1
+            for d in range(3):
+                m *= max(1, int((float(grid.hi[d]) - float(grid.lo[d])) / e * (1.0 + 1e-12)))
+            nc.append(m)
+        ea = (C.c_double * max(len(edges), 1))(*edges)
+        na = (C.c_int64 * max(len(edges), 1))(*nc)
+        self._ck(self.lib.spray_set_levels(self.h, len(edges), ea, na), "spray_set_levels")
 
     def build_timing(self):
         """Device milliseconds of the last build_cells: (cell list a1-a4, tiles + tables, neighbour-list builder); synchronises."""

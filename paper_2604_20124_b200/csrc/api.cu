@@ -3,6 +3,7 @@
 // data on the host and there is no CPU fallback.
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -39,7 +40,7 @@ bool dmalloc(T** p, int64_t count, Ctx* c = nullptr) {
 void free_all(Ctx* c) {
     for (int k = 0; k < 2; ++k) { cudaFree(c->key[k]); cudaFree(c->idx[k]); }
     cudaFree(c->hist); cudaFree(c->cell_start); cudaFree(c->cell_end); cudaFree(c->cell_hmax);
-    cudaFree(c->hglob); cudaFree(c->dev_status);
+    cudaFree(c->hglob); cudaFree(c->dev_status); cudaFree(c->cell_tend); cudaFree(c->cell_hmin); cudaFree(c->left); cudaFree(c->hs_c); cudaFree(c->fast_c); cudaFree(c->fast_all);
     for (double* r : c->rad_scratch) cudaFree(r);
     cudaFree(c->s.x); cudaFree(c->s.y); cudaFree(c->s.z); cudaFree(c->s.h); cudaFree(c->s.hs);
     for (double* f : c->s.f) cudaFree(f);
@@ -101,11 +102,49 @@ SweepArgs base_args(Ctx* c) {
     return a;
 }
 
-// general-kernel arguments of a sweep that the tiled kernels ran first: skip what they served
-SweepArgs fallback_args(Ctx* c) {
+// general-kernel arguments of a sweep that the tiled kernels ran first: skip what they served (levels = the call also ran the
+// tiled kernels of the internal levels)
+SweepArgs fallback_args(Ctx* c, bool levels = false) {
     SweepArgs a = base_args(c);
-    if (c->tl.enabled) { a.skip = c->tl.fast; a.nfast = c->tl.ctr + CTR_NFAST; }
+    if (levels && c->levels_on) { a.skip = c->fast_all; a.nfast = c->tl.ctr + CTR_NFAST_ALL; a.left = c->left; a.nleft = c->tl.ctr + CTR_NLEFT; }
+    else if (c->tl.enabled) {
+        a.skip = c->tl.fast; a.nfast = c->tl.ctr + CTR_NFAST;
+        if (!c->levels_on) { a.left = c->left; a.nleft = c->tl.ctr + CTR_NLEFT; }   // (with levels the list holds what is left after them)
+    }
     return a;
+}
+
+enum { F_M = 0, F_RHO, F_P, F_CS, F_VX, F_VY, F_VZ, F_ALPHA, F_E, F_KAPPA, F_MU, F_V, F_Q, F_AC };
+
+// the per-call prologue of a level context: same caller arrays, the level's own sorted scratch
+PrepJob level_job(const PrepJob& j, Ctx* v) {
+    PrepJob r = j;
+    double** f = v->s.f;
+    if (j.sm) r.sm = f[F_M];
+    if (j.srho) r.srho = f[F_RHO];
+    if (j.sp) r.sp = f[F_P];
+    if (j.scs) r.scs = f[F_CS];
+    if (j.svx) r.svx = f[F_VX];
+    if (j.svy) r.svy = f[F_VY];
+    if (j.svz) r.svz = f[F_VZ];
+    if (j.salpha) r.salpha = f[F_ALPHA];
+    if (j.sE) r.sE = f[F_E];
+    if (j.skx) r.skx = j.kx_is_mu ? f[F_MU] : f[F_KAPPA];
+    if (j.sV) r.sV = f[F_V];
+    if (j.sQ) r.sQ = f[F_Q];
+    if (j.sAC) r.sAC = f[F_AC];
+    return r;
+}
+
+// the contexts whose tiled kernels serve particles of this one: itself and its levels
+struct TiledSet { Ctx* v[1 + SPRAY_MAX_LEVELS]; int n = 0; };
+TiledSet tiled_set(Ctx* c) {
+    TiledSet s;
+    if (c->tl.enabled) s.v[s.n++] = c;
+    if (c->levels_on)
+        for (int k = 0; k < c->nlevels; ++k)
+            if (c->child[k] && c->child[k]->built && c->child[k]->tl.enabled) s.v[s.n++] = c->child[k];
+    return s;
 }
 
 #define CK(call, where) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) return cuda_fail(c, e__, where); } while (0)
@@ -114,7 +153,6 @@ SweepArgs fallback_args(Ctx* c) {
     DeviceGuard dev_guard__(ctx->c.device); \
     if (!dev_guard__.ok) { cudaGetLastError(); return fail(&ctx->c, SPRAY_ERR_CUDA, "cudaSetDevice failed"); }
 
-enum { F_M = 0, F_RHO, F_P, F_CS, F_VX, F_VY, F_VZ, F_ALPHA, F_E, F_KAPPA, F_MU, F_V, F_Q, F_AC };
 
 }  // namespace
 
@@ -139,7 +177,9 @@ int spray_create(spray_ctx** out, int64_t n_max, int64_t ncell_max, int device) 
     bool ok = true;
     for (int k = 0; k < 2; ++k) ok = ok && dmalloc(&c->key[k], n_max, c) && dmalloc(&c->idx[k], n_max, c);
     ok = ok && dmalloc(&c->hist, c->hist_cap, c) && dmalloc(&c->cell_start, ncell_max, c) && dmalloc(&c->cell_end, ncell_max, c) &&
-         dmalloc(&c->cell_hmax, ncell_max, c) && dmalloc(&c->hglob, 4, c) && dmalloc(&c->dev_status, 1, c) && dmalloc(&c->s.x, n_max, c) &&
+         dmalloc(&c->cell_hmax, ncell_max, c) && dmalloc(&c->cell_tend, ncell_max, c) && dmalloc(&c->cell_hmin, ncell_max, c) && dmalloc(&c->left, n_max, c) &&
+         dmalloc(&c->hs_c, n_max, c) &&
+         dmalloc(&c->fast_c, n_max, c) && dmalloc(&c->fast_all, n_max, c) && dmalloc(&c->hglob, 4, c) && dmalloc(&c->dev_status, 1, c) && dmalloc(&c->s.x, n_max, c) &&
          dmalloc(&c->s.y, n_max, c) && dmalloc(&c->s.z, n_max, c) && dmalloc(&c->s.h, n_max, c) && dmalloc(&c->s.hs, n_max, c);
     for (double*& f : c->s.f) ok = ok && dmalloc(&f, n_max, c);
     Packed& k = c->pk;
@@ -161,10 +201,51 @@ int spray_create(spray_ctx** out, int64_t n_max, int64_t ncell_max, int device) 
     return SPRAY_OK;
 }
 
+static void destroy_levels(Ctx* c) {
+    for (int k = 0; k < c->nlevels; ++k) {
+        if (!c->child[k]) continue;
+        spray_ctx* h = reinterpret_cast<spray_ctx*>(c->child[k]);     // Ctx is the first (only) member of spray_ctx
+        for (cudaEvent_t e : h->c.ev) if (e) cudaEventDestroy(e);
+        c->scratch_bytes -= h->c.scratch_bytes;
+        free_all(&h->c);
+        delete h;
+        c->child[k] = nullptr;
+    }
+    c->nlevels = 0;
+    c->levels_on = false;
+}
+
+int spray_set_levels(spray_ctx* ctx, int nlevels, const double* edges, const int64_t* ncell_max) {
+    if (!ctx) return SPRAY_ERR_INVALID_ARG;
+    Ctx* c = &ctx->c;
+    if (nlevels < 0 || nlevels > SPRAY_MAX_LEVELS || (nlevels > 0 && (!edges || !ncell_max)))
+        return fail(c, SPRAY_ERR_INVALID_ARG, "spray_set_levels: 0 <= nlevels <= 16, edges and ncell_max non-NULL");
+    for (int k = 0; k < nlevels; ++k)
+        if (!(edges[k] > 0.0) || (k > 0 && !(edges[k] > edges[k - 1])) || ncell_max[k] < 1)
+            return fail(c, SPRAY_ERR_INVALID_ARG, "spray_set_levels: edges must be positive and ascending, ncell_max >= 1");
+    DeviceGuard dg(c->device);
+    if (!dg.ok) { cudaGetLastError(); return fail(c, SPRAY_ERR_CUDA, "cudaSetDevice failed"); }
+    cudaDeviceSynchronize();
+    destroy_levels(c);
+    c->built = false;
+    for (int k = 0; k < nlevels; ++k) {
+        spray_ctx* h = nullptr;
+        const int rc = spray_create(&h, c->n_max, ncell_max[k], c->device);
+        if (rc != SPRAY_OK) { destroy_levels(c); return fail(c, rc, "spray_set_levels: allocation of a level failed"); }
+        h->c.is_level = true;
+        c->child[k] = &h->c;
+        c->level_edge[k] = edges[k];
+        c->nlevels = k + 1;
+        c->scratch_bytes += h->c.scratch_bytes;
+    }
+    return SPRAY_OK;
+}
+
 int spray_destroy(spray_ctx* ctx) {
     if (!ctx) return SPRAY_OK;
     DeviceGuard dg(ctx->c.device);
     cudaDeviceSynchronize();
+    destroy_levels(&ctx->c);
     for (cudaEvent_t e : ctx->c.ev) if (e) cudaEventDestroy(e);
     free_all(&ctx->c);
     delete ctx;
@@ -202,15 +283,87 @@ int spray_path_stats(spray_ctx* ctx, void* stream, int64_t* n_tiles, int64_t* n_
     Ctx* c = &ctx->c;
     cudaStream_t st = (cudaStream_t)stream;
     unsigned long long v[CTR_COUNT] = {};
-    if (c->tl.enabled && c->n > 0) {
+    int64_t tiles = 0, nonuni = 0, dec[4] = {0, 0, 0, 0}, nfast = 0;
+    if (c->n > 0 && (c->tl.enabled || c->levels_on)) {
         CK(cudaStreamSynchronize(st), "spray_path_stats");
-        CK(cudaMemcpy(v, c->tl.ctr, sizeof v, cudaMemcpyDeviceToHost), "spray_path_stats");
+        const TiledSet ts = tiled_set(c);
+        for (int k = 0; k < ts.n; ++k) {
+            CK(cudaMemcpy(v, ts.v[k]->tl.ctr, sizeof v, cudaMemcpyDeviceToHost), "spray_path_stats");
+            tiles += (int64_t)v[CTR_NTILES]; nonuni += (int64_t)v[CTR_NNONUNI];
+            if (getenv("SPRAY_DEBUG"))
+                fprintf(stderr, "[spray] %s grid %d x %d x %d  2hs in (%.4g, %.4g]  tiles %llu  served %llu  nonuniform units %llu  declined %llu %llu %llu\n",
+                        ts.v[k] == c ? "caller grid" : "level", ts.v[k]->grid.ncell[0], ts.v[k]->grid.ncell[1], ts.v[k]->grid.ncell[2],
+                        ts.v[k]->level_lo, ts.v[k]->level_hi, v[CTR_NTILES], v[CTR_NFAST], v[CTR_NNONUNI], v[CTR_DECL + 1], v[CTR_DECL + 2], v[CTR_DECL + 3]);
+            for (int r = 0; r < 4; ++r) dec[r] += (int64_t)v[CTR_DECL + r];
+            if (!c->levels_on) nfast += (int64_t)v[CTR_NFAST];
+        }
+        if (c->levels_on) {
+            CK(cudaMemcpy(v, c->tl.ctr, sizeof v, cudaMemcpyDeviceToHost), "spray_path_stats");
+            nfast = (int64_t)v[CTR_NFAST_ALL];
+        }
     }
-    if (n_tiles) *n_tiles = (int64_t)v[CTR_NTILES];
-    if (n_fast) *n_fast = (int64_t)v[CTR_NFAST];
-    if (n_nonuniform) *n_nonuniform = (int64_t)v[CTR_NNONUNI];
+    if (n_tiles) *n_tiles = tiles;
+    if (n_fast) *n_fast = nfast;
+    if (n_nonuniform) *n_nonuniform = nonuni;
     if (scratch_bytes) *scratch_bytes = c->scratch_bytes;
-    if (declined) for (int k = 0; k < 4; ++k) declined[k] = (int64_t)v[CTR_DECL + k];
+    if (declined) for (int k = 0; k < 4; ++k) declined[k] = dec[k];
+    return SPRAY_OK;
+}
+
+// Internal levels of the tiled path (spray_set_levels; the search range follows from the ratio of a
+// particle's smoothing length to the cell size, neighbours are mutual).  Level k is a grid over the caller's box with
+// ncell_d = floor(L_d / edge_k) cells; it serves the particles a that nobody served yet with hi_(k-1) < 2 hs_a <= hi_k, where
+// hs_a is the symmetric search length (max of h_a and of the h of everyone who sees a) and hi_k the smallest cell edge of
+// the level: every mutual neighbour of such a particle lies within one cell of its own.  The level sorts ALL particles by
+// (cell, served-here bit), so the targets of a cell come first and every particle is a candidate; tiles, lists and sweeps
+// are those of tiles.cu / sweeps_tiled.cu unchanged.  What no level takes stays with the general kernels of this context.
+static int build_levels(Ctx* c, const double* x, const double* y, const double* z, const double* h, cudaStream_t st) {
+    CK(launch_to_caller_order(c, st), "levels: search lengths to caller order");
+    double lo = 0.0;
+    for (int k = 0; k < c->nlevels; ++k) {
+        Ctx* v = c->child[k];
+        v->built = false; v->tl.enabled = false;
+        spray_grid_t g = c->grid;
+        int64_t nc = 1;
+        double emin = 1e300, emax = 0.0;
+        bool ok = true;
+        for (int d = 0; d < 3; ++d) {
+            const double L = g.hi[d] - g.lo[d];
+            int64_t m = (int64_t)floor(L / c->level_edge[k] * (1.0 + 1e-12));
+            m = m < 1 ? 1 : (m > 32000 ? 32000 : m);
+            g.ncell[d] = (int32_t)m;
+            nc *= m;
+            emin = fmin(emin, L / (double)m); emax = fmax(emax, L / (double)m);
+        }
+        if (nc > v->ncell_max) ok = false;
+        const double hi = emin / (1.0 + 1e-9);
+        if (!ok || !(hi > lo)) continue;                  // the level cannot be built on this box: its particles stay unserved
+        v->grid = g; v->kernel = c->kernel; v->n = c->n; v->ncell = nc; v->path = 1;
+        for (int d = 0; d < 3; ++d) {
+            v->dg.lo[d] = g.lo[d]; v->dg.L[d] = g.hi[d] - g.lo[d]; v->dg.halfL[d] = 0.5 * v->dg.L[d];
+            v->dg.inv[d] = (double)g.ncell[d] / v->dg.L[d]; v->dg.edge[d] = v->dg.L[d] / (double)g.ncell[d];
+            v->dg.nc[d] = g.ncell[d]; v->dg.per[d] = g.periodic[d] ? 1 : 0;
+        }
+        v->level_lo = lo; v->level_hi = hi;
+        v->level_rmax = (float)(3.5 * emax * (1.0 + 1e-6));   // every candidate of a window lies within 2 cells per dimension
+        v->hs_caller = c->hs_c; v->fast_caller = c->fast_c;
+        Ctx* keep = c;
+        {
+            Ctx* c = v;                                   // CK reports into the level's context
+            CK(launch_cell_keys(c, x, y, z, st), "level: cell keys");
+            CK(launch_radix_sort(c, st), "level: radix sort");
+            CK(launch_cell_table(c, st), "level: cell table");
+            CK(launch_reorder_build(c, x, y, z, h, st), "level: reorder");
+            CK(launch_build_tiles(c, st), "level: tiles + neighbour lists");
+            c->built = true;
+        }
+        c = keep;
+        CK(launch_merge_served(c, v, st), "levels: served flags");
+        lo = hi;
+    }
+    CK(launch_fast_from_caller(c, st), "levels: served flags to sorted order");
+    CK(launch_compact_left(c, c->fast_all, st), "levels: list of the particles left to the general kernels");
+    c->levels_on = true;
     return SPRAY_OK;
 }
 
@@ -277,6 +430,12 @@ int spray_build_cells(spray_ctx* ctx, const spray_grid_t* g, spray_kernel_t kern
     CK(launch_ref_sweep(c, SW_HSEARCH, a, st), "search-length sweep");
     if (c->ev[1]) cudaEventRecord(c->ev[1], st);
     if (c->path == 1) CK(launch_build_tiles(c, st), "tiles + neighbour lists");
+    if (c->tl.enabled) CK(launch_compact_left(c, c->tl.fast, st), "list of the particles left to the general kernels");
+    c->levels_on = false;
+    if (c->path == 1 && c->nlevels > 0 && n > 0) {
+        const int rc = build_levels(c, x, y, z, h, st);
+        if (rc != SPRAY_OK) return rc;
+    }
     if (c->ev[3]) cudaEventRecord(c->ev[3], st);
     c->built = true;
     return SPRAY_OK;
@@ -288,12 +447,14 @@ int spray_density(spray_ctx* ctx, const double* m, double* rho, uint32_t* nnbr, 
     if (c->n > 0 && (!m || !rho)) return fail(c, SPRAY_ERR_INVALID_ARG, "spray_density: NULL argument");
     cudaStream_t st = (cudaStream_t)stream;
     CK(launch_prep_density(c, m, st), "density prologue");
-    if (c->tl.enabled) {
+    const TiledSet ts = tiled_set(c);
+    for (int k = 0; k < ts.n; ++k) {
+        if (ts.v[k] != c) CK(launch_prep_density(ts.v[k], m, st), "density prologue (level)");
         TiledArgs t{};
         t.o0 = rho; t.ocount = nnbr;
-        CK(launch_tiled_sweep(c, SW_DENSITY, t, st), "tiled density sweep");
+        CK(launch_tiled_sweep(ts.v[k], SW_DENSITY, t, st), "tiled density sweep");
     }
-    SweepArgs a = fallback_args(c);
+    SweepArgs a = fallback_args(c, true);
     a.m = c->s.f[F_M]; a.o0 = rho; a.ocount = nnbr;
     CK(launch_ref_sweep(c, SW_DENSITY, a, st), "density sweep");
     return SPRAY_OK;
@@ -313,13 +474,15 @@ int spray_hydro_rhs(spray_ctx* ctx, const double* m, const double* rho, const do
     pj.sm = f[F_M]; pj.srho = f[F_RHO]; pj.sp = f[F_P]; pj.scs = f[F_CS]; pj.svx = f[F_VX]; pj.svy = f[F_VY]; pj.svz = f[F_VZ];
     pj.salpha = f[F_ALPHA]; pj.sV = f[F_V]; pj.sQ = f[F_Q]; pj.sAC = f[F_AC];
     CK(launch_prep_hydro(c, pj, st), "hydro prologue");
-    if (c->tl.enabled) {
+    const TiledSet ts = tiled_set(c);
+    for (int k = 0; k < ts.n; ++k) {
+        if (ts.v[k] != c) CK(launch_prep_hydro(ts.v[k], level_job(pj, ts.v[k]), st), "hydro prologue (level)");
         TiledArgs t{};
         t.beta = beta;
         t.o0 = ax; t.o1 = ay; t.o2 = az; t.o3 = dudt; t.o4 = divv_sum;
-        CK(launch_tiled_sweep(c, SW_HYDRO, t, st), "tiled hydro sweep");
+        CK(launch_tiled_sweep(ts.v[k], SW_HYDRO, t, st), "tiled hydro sweep");
     }
-    SweepArgs a = fallback_args(c);
+    SweepArgs a = fallback_args(c, true);
     a.m = f[F_M]; a.rho = f[F_RHO]; a.p = f[F_P]; a.cs = f[F_CS];
     a.vx = f[F_VX]; a.vy = f[F_VY]; a.vz = f[F_VZ]; a.alpha = f[F_ALPHA];
     a.beta = beta;
@@ -345,19 +508,21 @@ int spray_hydro_rhs_limiter(spray_ctx* ctx, const double* m, const double* rho, 
     // the limiter's prologue rides along: E, and rho kappa parked in the (mu, E) record so that t0 stays the hydro's
     pj.E = E; pj.kx = kappa; pj.sE = f[F_E]; pj.skx = f[F_KAPPA];
     CK(launch_prep_hydro(c, pj, st), "hydro + limiter prologue");
-    if (c->tl.enabled) {
+    const TiledSet ts = tiled_set(c);
+    for (int k = 0; k < ts.n; ++k) {
+        if (ts.v[k] != c) CK(launch_prep_hydro(ts.v[k], level_job(pj, ts.v[k]), st), "hydro + limiter prologue (level)");
         TiledArgs t{};
         t.beta = beta; t.c_light = c_light;
         t.o0 = ax; t.o1 = ay; t.o2 = az; t.o3 = dudt; t.o4 = divv_sum; t.o5 = mu; t.o6 = gradE;
-        CK(launch_tiled_sweep(c, SW_HYDLIM, t, st), "tiled hydro + limiter sweep");
+        CK(launch_tiled_sweep(ts.v[k], SW_HYDLIM, t, st), "tiled hydro + limiter sweep");
     }
-    SweepArgs a = fallback_args(c);
+    SweepArgs a = fallback_args(c, true);
     a.m = f[F_M]; a.rho = f[F_RHO]; a.p = f[F_P]; a.cs = f[F_CS];
     a.vx = f[F_VX]; a.vy = f[F_VY]; a.vz = f[F_VZ]; a.alpha = f[F_ALPHA];
     a.beta = beta;
     a.o0 = ax; a.o1 = ay; a.o2 = az; a.o3 = dudt; a.o4 = divv_sum;
     CK(launch_ref_sweep(c, SW_HYDRO, a, st), "hydro sweep");
-    SweepArgs l = fallback_args(c);
+    SweepArgs l = fallback_args(c, true);
     l.m = f[F_M]; l.rho = f[F_RHO]; l.E = f[F_E]; l.kappa = f[F_KAPPA]; l.mu = f[F_MU];
     l.c_light = c_light;
     l.o0 = mu; l.o1 = gradE; l.mu_sorted = f[F_MU]; l.me_sorted = c->pk.me;
@@ -381,26 +546,37 @@ int spray_fld_apply(spray_ctx* ctx, const double* m, const double* rho, const do
     pj.m = m; pj.rho = rho; pj.E = E; pj.kx = update ? kappa : mu; pj.kx_is_mu = update ? 0 : 1;
     pj.sm = f[F_M]; pj.srho = f[F_RHO]; pj.sE = f[F_E]; pj.skx = update ? f[F_KAPPA] : f[F_MU]; pj.sV = f[F_V];
     CK(launch_prep_fld(c, pj, st), "fld prologue");
-    const bool tiled = c->tl.enabled;
-    SweepArgs a = fallback_args(c);
+    const TiledSet ts = tiled_set(c);
+    for (int k = 0; k < ts.n; ++k)
+        if (ts.v[k] != c) CK(launch_prep_fld(ts.v[k], level_job(pj, ts.v[k]), st), "fld prologue (level)");
+    SweepArgs a = fallback_args(c, true);
     a.m = f[F_M]; a.rho = f[F_RHO]; a.E = f[F_E]; a.kappa = f[F_KAPPA]; a.mu = f[F_MU];
     a.c_light = c_light;
     if (update) {
-        if (tiled) {
+        for (int k = 0; k < ts.n; ++k) {
             TiledArgs t{};
             t.c_light = c_light; t.o0 = mu; t.o1 = gradE;
-            CK(launch_tiled_sweep(c, SW_LIMITER, t, st), "tiled limiter sweep");
+            CK(launch_tiled_sweep(ts.v[k], SW_LIMITER, t, st), "tiled limiter sweep");
         }
         SweepArgs l = a;
         l.o0 = mu; l.o1 = gradE; l.mu_sorted = f[F_MU]; l.me_sorted = c->pk.me;
         CK(launch_ref_sweep(c, SW_LIMITER, l, st), "limiter sweep");
+        if (c->levels_on) {
+            // every context computed mu for the particles it serves only: the (mu, E) records and the sorted mu of all of them
+            // are re-packed from the caller-order mu (as in FROZEN mode) before the apply
+            PrepJob pm = pj;
+            pm.kx = mu; pm.kx_is_mu = 1; pm.skx = f[F_MU];
+            CK(launch_prep_fld(c, pm, st), "fld prologue (mu)");
+            for (int k = 0; k < ts.n; ++k)
+                if (ts.v[k] != c) CK(launch_prep_fld(ts.v[k], level_job(pm, ts.v[k]), st), "fld prologue (mu, level)");
+        }
     }
     a.fld_sym = (kmode == SPRAY_FLD_SYMMETRIC) ? 1 : 0;
-    if (tiled) {
+    for (int k = 0; k < ts.n; ++k) {
         TiledArgs t{};
         t.fld_sym = a.fld_sym;
         t.o0 = y; t.o1 = diag; t.o2 = offd;
-        CK(launch_tiled_sweep(c, SW_APPLY, t, st), "tiled apply sweep");
+        CK(launch_tiled_sweep(ts.v[k], SW_APPLY, t, st), "tiled apply sweep");
     }
     a.o0 = y; a.o1 = diag; a.o2 = offd;
     CK(launch_ref_sweep(c, SW_APPLY, a, st), "apply sweep");
@@ -589,8 +765,10 @@ int spray_neighbor_counts(spray_ctx* ctx, int symmetric, uint32_t* count, void* 
     NEED_BUILT();
     Ctx* c = &ctx->c;
     if (c->n > 0 && !count) return fail(c, SPRAY_ERR_INVALID_ARG, "spray_neighbor_counts: NULL argument");
-    CK(launch_tiled_export(c, 0, symmetric, count, nullptr, nullptr, nullptr, nullptr, (cudaStream_t)stream), "neighbour counts from the tiled lists");
-    SweepArgs a = fallback_args(c);
+    const TiledSet ts = tiled_set(c);
+    for (int k = 0; k < ts.n; ++k)
+        CK(launch_tiled_export(ts.v[k], 0, symmetric, count, nullptr, nullptr, nullptr, nullptr, (cudaStream_t)stream), "neighbour counts from the tiled lists");
+    SweepArgs a = fallback_args(c, true);
     a.symmetric = symmetric; a.ocount = count;
     CK(launch_ref_sweep(c, SW_COUNT, a, (cudaStream_t)stream), "neighbour count sweep");
     return SPRAY_OK;
@@ -600,8 +778,10 @@ int spray_neighbor_lists(spray_ctx* ctx, int symmetric, const uint64_t* offsets,
     NEED_BUILT();
     Ctx* c = &ctx->c;
     if (c->n > 0 && (!offsets || !nbr)) return fail(c, SPRAY_ERR_INVALID_ARG, "spray_neighbor_lists: NULL argument");
-    CK(launch_tiled_export(c, 1, symmetric, nullptr, offsets, nbr, nullptr, nullptr, (cudaStream_t)stream), "neighbour lists from the tiled lists");
-    SweepArgs a = fallback_args(c);
+    const TiledSet ts = tiled_set(c);
+    for (int k = 0; k < ts.n; ++k)
+        CK(launch_tiled_export(ts.v[k], 1, symmetric, nullptr, offsets, nbr, nullptr, nullptr, (cudaStream_t)stream), "neighbour lists from the tiled lists");
+    SweepArgs a = fallback_args(c, true);
     a.symmetric = symmetric; a.offsets = offsets; a.onbr = nbr;
     CK(launch_ref_sweep(c, SW_LIST, a, (cudaStream_t)stream), "neighbour list sweep");
     return SPRAY_OK;
@@ -611,8 +791,10 @@ int spray_neighbor_digest(spray_ctx* ctx, int symmetric, uint64_t* dsum, uint64_
     NEED_BUILT();
     Ctx* c = &ctx->c;
     if (c->n > 0 && (!dsum || !dxor)) return fail(c, SPRAY_ERR_INVALID_ARG, "spray_neighbor_digest: NULL argument");
-    CK(launch_tiled_export(c, 2, symmetric, nullptr, nullptr, nullptr, dsum, dxor, (cudaStream_t)stream), "neighbour digests from the tiled lists");
-    SweepArgs a = fallback_args(c);
+    const TiledSet ts = tiled_set(c);
+    for (int k = 0; k < ts.n; ++k)
+        CK(launch_tiled_export(ts.v[k], 2, symmetric, nullptr, nullptr, nullptr, dsum, dxor, (cudaStream_t)stream), "neighbour digests from the tiled lists");
+    SweepArgs a = fallback_args(c, true);
     a.symmetric = symmetric; a.odsum = dsum; a.odxor = dxor;
     CK(launch_ref_sweep(c, SW_DIGEST, a, (cudaStream_t)stream), "neighbour digest sweep");
     return SPRAY_OK;

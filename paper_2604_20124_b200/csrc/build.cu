@@ -9,9 +9,12 @@ namespace spray {
 // ------------------------------------------------------------------------------------------- K1: cell key
 // c_d = (int) floor((x_d - lo_d) * inv_d) clamped to [0, nc_d-1]; key = (c_z*nc_y + c_y)*nc_x + c_x.
 // Subtract then multiply (two roundings, nothing to contract).  24 B read + 8 B written per particle.
+// Level contexts (api.cu) append one bit: 0 for the particles the level serves (2 hs in (lvl_lo, lvl_hi], not served before),
+// 1 for the others, so that the sort puts the targets of a cell in front of its other particles.
 __global__ void k_cell_key(DevGrid g, int64_t n, const double* __restrict__ x, const double* __restrict__ y,
                            const double* __restrict__ z, uint32_t* __restrict__ key, uint32_t* __restrict__ idx,
-                           uint32_t* __restrict__ status) {
+                           uint32_t* __restrict__ status, const double* __restrict__ hs_caller, const uint8_t* __restrict__ fast_caller,
+                           double lvl_lo, double lvl_hi) {
     int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (i >= n) return;
     double p[3] = {x[i], y[i], z[i]};
@@ -25,7 +28,13 @@ __global__ void k_cell_key(DevGrid g, int64_t n, const double* __restrict__ x, c
         if (g.per[d] && !(p[d] >= g.lo[d] && p[d] < g.lo[d] + g.L[d])) bad = true;
         c[d] = ci;
     }
-    key[i] = (uint32_t)((c[2] * g.nc[1] + c[1]) * g.nc[0] + c[0]);
+    uint32_t k = (uint32_t)((c[2] * g.nc[1] + c[1]) * g.nc[0] + c[0]);
+    if (hs_caller) {
+        const double r = 2.0 * hs_caller[i];
+        const bool target = !fast_caller[i] && r > lvl_lo && r <= lvl_hi && !bad;
+        k = (k << 1) | (target ? 0u : 1u);
+    }
+    key[i] = k;
     idx[i] = (uint32_t)i;
     if (bad) atomicOr(status, (uint32_t)SPRAY_DEV_OUTSIDE_BOX);
 }
@@ -180,6 +189,16 @@ __global__ void k_cell_table(const uint32_t* __restrict__ sorted_key, uint32_t n
     if (c < ncell) cell_start[c] = lb;
     if (c > 0) cell_end[c - 1] = lb;
 }
+// level contexts: keys are 2 cell + (0 target | 1 other)
+__global__ void k_cell_table_level(const uint32_t* __restrict__ sorted_key, uint32_t n, uint32_t ncell, uint32_t* __restrict__ cell_start,
+                                   uint32_t* __restrict__ cell_tend, uint32_t* __restrict__ cell_end) {
+    uint32_t v = blockIdx.x * blockDim.x + threadIdx.x;
+    if (v > 2u * ncell) return;
+    uint32_t lb = lower_bound_u32(sorted_key, n, v);
+    if (v & 1u) { cell_tend[v >> 1] = lb; return; }
+    if (v < 2u * ncell) cell_start[v >> 1] = lb;
+    if (v > 0) cell_end[(v >> 1) - 1] = lb;
+}
 
 // ------------------------------------------------------------------------------------------- K4: reorder by cell
 // Sorted copies of (x, y, z, h): structure-of-arrays for the general kernels and 16-byte records (x,y), (z,h),
@@ -280,12 +299,13 @@ __global__ void k_init_hglob(double* hglob) { hglob[0] = __longlong_as_double(0x
 
 __global__ void k_cell_hmax(const uint32_t* __restrict__ cell_start, const uint32_t* __restrict__ cell_end,
                             const double* __restrict__ h, uint32_t ncell, double hmax_decl,
-                            double* __restrict__ cell_hmax, double* __restrict__ hglob, uint32_t* __restrict__ status) {
+                            double* __restrict__ cell_hmax, double* __restrict__ cell_hmin, double* __restrict__ hglob, uint32_t* __restrict__ status) {
     uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
     double mx = 0.0, mn = __longlong_as_double(0x7FF0000000000000ll);
     if (c < ncell) {
         for (uint32_t j = cell_start[c]; j < cell_end[c]; ++j) { double v = h[j]; mx = fmax(mx, v); mn = fmin(mn, v); }
         cell_hmax[c] = mx;
+        cell_hmin[c] = mn;
     }
     // warp reduce, then one atomic per warp on the bit patterns (positive doubles order like integers)
     for (int o = 16; o; o >>= 1) {
@@ -308,10 +328,10 @@ __global__ void k_cell_hmax(const uint32_t* __restrict__ cell_start, const uint3
 // such a cell anyway).
 __global__ void k_mark_coincident(DevGrid g, int64_t n, const uint32_t* __restrict__ sorted_key, const uint32_t* __restrict__ cell_start,
                                   const uint32_t* __restrict__ cell_end, const double* __restrict__ x, const double* __restrict__ y,
-                                  const double* __restrict__ z, uint8_t* __restrict__ coinc) {
+                                  const double* __restrict__ z, uint8_t* __restrict__ coinc, int key_shift) {
     const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (i >= n) return;
-    const uint32_t key = sorted_key[i];
+    const uint32_t key = sorted_key[i] >> key_shift;
     const uint32_t cs = cell_start[key], ce = cell_end[key];
     const double xi = x[i], yi = y[i], zi = z[i];
     constexpr double TINY = 1.0e-140, R2MIN = 1.0e-290;
@@ -350,29 +370,103 @@ __global__ void k_mark_coincident(DevGrid g, int64_t n, const uint32_t* __restri
     if (hit) coinc[i] = 1;
 }
 
+// ---- levels (api.cu): per-particle data between the parent (sorted order) and the level contexts (caller order)
+__global__ void k_to_caller(const uint32_t* __restrict__ perm, int64_t n, const double* __restrict__ hs, const uint8_t* __restrict__ fast,
+                            double* __restrict__ hs_c, uint8_t* __restrict__ fast_c) {
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const uint32_t p = perm[i];
+    hs_c[p] = hs[i];
+    fast_c[p] = fast ? fast[i] : (uint8_t)0;
+}
+__global__ void k_merge_served(const uint32_t* __restrict__ perm_child, int64_t n, const uint8_t* __restrict__ fast_child,
+                               uint8_t* __restrict__ fast_c) {
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    if (fast_child[i]) fast_c[perm_child[i]] = 1;
+}
+__global__ void k_fast_from_caller(const uint32_t* __restrict__ perm, int64_t n, const uint8_t* __restrict__ fast_c, uint8_t* __restrict__ fast,
+                                   unsigned long long* __restrict__ nfast) {
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    const bool f = i < n && fast_c[perm[i]] != 0;
+    if (i < n) fast[i] = f ? 1 : 0;
+    const unsigned m = __ballot_sync(0xFFFFFFFFu, f);
+    if ((threadIdx.x & 31) == 0 && m) atomicAdd(nfast, (unsigned long long)__popc(m));
+}
+
 // ------------------------------------------------------------------------------------------- launchers
 static inline int cdiv64(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
+
+// the particles the tiled kernels do not serve, compacted in ascending sorted order within a block's 256 (blocks in the order
+// they get to the counter: the order of the list changes nothing in the results, each particle's sums are its own)
+__global__ void k_compact_left(const uint8_t* __restrict__ fast, int64_t n, uint32_t* __restrict__ left, unsigned long long* __restrict__ nleft) {
+    __shared__ uint32_t wbase[8];
+    __shared__ unsigned long long base;
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    const bool keep = i < n && fast[i] == 0;
+    const unsigned m = __ballot_sync(0xFFFFFFFFu, keep);
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (lane == 0) wbase[w] = __popc(m);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        uint32_t run = 0;
+        for (int k = 0; k < 8; ++k) { const uint32_t t = wbase[k]; wbase[k] = run; run += t; }
+        base = run ? atomicAdd(nleft, (unsigned long long)run) : 0ull;
+    }
+    __syncthreads();
+    if (keep) left[base + wbase[w] + __popc(m & ((1u << lane) - 1u))] = (uint32_t)i;
+}
+cudaError_t launch_compact_left(Ctx* c, const uint8_t* fast, cudaStream_t st) {
+    if (c->n == 0 || !c->left) return cudaSuccess;
+    cudaError_t e = cudaMemsetAsync(c->tl.ctr + CTR_NLEFT, 0, sizeof(unsigned long long), st);
+    if (e != cudaSuccess) return e;
+    k_compact_left<<<cdiv64(c->n, 256), 256, 0, st>>>(fast, c->n, c->left, c->tl.ctr + CTR_NLEFT);
+    c->launches += 1;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_to_caller_order(Ctx* c, cudaStream_t st) {
+    if (c->n == 0) return cudaSuccess;
+    k_to_caller<<<cdiv64(c->n, 256), 256, 0, st>>>(c->perm, c->n, c->s.hs, c->tl.enabled ? c->tl.fast : nullptr, c->hs_c, c->fast_c);
+    c->launches += 1;
+    return cudaGetLastError();
+}
+cudaError_t launch_merge_served(Ctx* parent, Ctx* child, cudaStream_t st) {
+    if (child->n == 0 || !child->tl.enabled) return cudaSuccess;
+    k_merge_served<<<cdiv64(child->n, 256), 256, 0, st>>>(child->perm, child->n, child->tl.fast, parent->fast_c);
+    parent->launches += 1;
+    return cudaGetLastError();
+}
+cudaError_t launch_fast_from_caller(Ctx* c, cudaStream_t st) {
+    if (c->n == 0) return cudaSuccess;
+    cudaError_t e = cudaMemsetAsync(c->tl.ctr + CTR_NFAST_ALL, 0, sizeof(unsigned long long), st);
+    if (e != cudaSuccess) return e;
+    k_fast_from_caller<<<cdiv64(c->n, 256), 256, 0, st>>>(c->perm, c->n, c->fast_c, c->fast_all, c->tl.ctr + CTR_NFAST_ALL);
+    c->launches += 1;
+    return cudaGetLastError();
+}
 
 cudaError_t launch_mark_coincident(Ctx* c, cudaStream_t st) {
     if (c->n == 0 || !c->tl.coinc) return cudaSuccess;
     cudaError_t e = cudaMemsetAsync(c->tl.coinc, 0, (size_t)c->n, st);
     if (e != cudaSuccess) return e;
     k_mark_coincident<<<cdiv64(c->n, 256), 256, 0, st>>>(c->dg, c->n, c->sorted_key, c->cell_start, c->cell_end, c->s.x, c->s.y, c->s.z,
-                                                        c->tl.coinc);
+                                                        c->tl.coinc, c->is_level ? 1 : 0);
     c->launches += 1;
     return cudaGetLastError();
 }
 
 cudaError_t launch_cell_keys(Ctx* c, const double* x, const double* y, const double* z, cudaStream_t st) {
     if (c->n == 0) return cudaSuccess;
-    k_cell_key<<<cdiv64(c->n, 256), 256, 0, st>>>(c->dg, c->n, x, y, z, c->key[0], c->idx[0], c->dev_status);
+    k_cell_key<<<cdiv64(c->n, 256), 256, 0, st>>>(c->dg, c->n, x, y, z, c->key[0], c->idx[0], c->dev_status,
+                                                 c->is_level ? c->hs_caller : nullptr, c->fast_caller, c->level_lo, c->level_hi);
     c->launches += 1;
     return cudaGetLastError();
 }
 
 cudaError_t launch_radix_sort(Ctx* c, cudaStream_t st) {
     int bits = 0;
-    while (((int64_t)1 << bits) < c->ncell) ++bits;
+    while (((int64_t)1 << bits) < c->ncell * (c->is_level ? 2 : 1)) ++bits;
     int passes = (bits + 7) / 8;
     int cur = 0;
     int nblk = cdiv64(c->n, RS_TILE);
@@ -398,8 +492,12 @@ cudaError_t launch_radix_sort(Ctx* c, cudaStream_t st) {
 }
 
 cudaError_t launch_cell_table(Ctx* c, cudaStream_t st) {
-    k_cell_table<<<cdiv64(c->ncell + 1, 256), 256, 0, st>>>(c->sorted_key, (uint32_t)c->n, (uint32_t)c->ncell, c->cell_start,
-                                                           c->cell_end);
+    if (c->is_level)
+        k_cell_table_level<<<cdiv64(2 * c->ncell + 1, 256), 256, 0, st>>>(c->sorted_key, (uint32_t)c->n, (uint32_t)c->ncell, c->cell_start,
+                                                                         c->cell_tend, c->cell_end);
+    else
+        k_cell_table<<<cdiv64(c->ncell + 1, 256), 256, 0, st>>>(c->sorted_key, (uint32_t)c->n, (uint32_t)c->ncell, c->cell_start,
+                                                               c->cell_end);
     c->launches += 1;
     return cudaGetLastError();
 }
@@ -412,7 +510,12 @@ cudaError_t launch_reorder_build(Ctx* c, const double* x, const double* y, const
     return cudaGetLastError();
 }
 
-static const unsigned long long* nfast_ptr(Ctx* c) { return c->tl.enabled ? c->tl.ctr + CTR_NFAST : nullptr; }
+// device word the prologues compare with n: equal = nobody needs the structure-of-arrays copies (general kernels idle).
+// A level context never runs general kernels: its word is CTR_NALL = n.
+static const unsigned long long* nfast_ptr(Ctx* c) {
+    if (c->is_level) return c->tl.ctr + CTR_NALL;
+    return c->tl.enabled ? c->tl.ctr + CTR_NFAST : nullptr;
+}
 static PackedOut packed_out(Ctx* c) {
     PackedOut o{c->pk.s[0], c->pk.s[1], c->pk.s[2], c->pk.s[3], c->pk.t0, c->pk.me, c->pk.e1, c->pk.p1};
     return o;
@@ -457,7 +560,7 @@ cudaError_t launch_excl_scan_u32(Ctx* c, uint32_t* a, int64_t total, uint32_t* s
 cudaError_t launch_cell_hmax(Ctx* c, cudaStream_t st) {
     k_init_hglob<<<1, 1, 0, st>>>(c->hglob);
     k_cell_hmax<<<cdiv64(c->ncell, 256), 256, 0, st>>>(c->cell_start, c->cell_end, c->s.h, (uint32_t)c->ncell, c->grid.h_max,
-                                                      c->cell_hmax, c->hglob, c->dev_status);
+                                                      c->cell_hmax, c->cell_hmin, c->hglob, c->dev_status);
     c->launches += 2;
     return cudaGetLastError();
 }

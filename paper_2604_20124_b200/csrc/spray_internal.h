@@ -8,6 +8,8 @@
 #include "common.cuh"
 #include "tiles.cuh"
 
+constexpr int SPRAY_MAX_LEVELS = 16;
+
 namespace spray {
 
 // Particle store in SORTED order, structure-of-arrays (BASELINE.json "reordered by cell after the sort"): used by
@@ -52,10 +54,12 @@ struct Tiled {
 };
 // CTR_NFAST: particles served by the tiled kernels; CTR_NTILES: tiles; CTR_NNONUNI: half-tile units that found non-uniform h;
 // CTR_POOL: list-pool rows handed out
-// CTR_DECL + k: warps / threads that declined their unit (general kernels), by reason k: 0 = window longer than 128 blocks,
-// 1 = left-over queue overflow, 2 = list longer than LIST_RMAX rounds or more than LIST_BC neighbours in one bank, 3 = other
-// (coincident particles, particle outside the tile's fp32 range, list pool exhausted)
-enum { CTR_NFAST = 1, CTR_NTILES = 2, CTR_NNONUNI = 3, CTR_POOL = 4, CTR_DECL = 8, CTR_COUNT = 12 };
+// CTR_DECL + k: warps / threads that declined their unit (general kernels), by reason k: 1 = list pool exhausted, 2 = list
+// longer than LIST_RMAX rounds or more than LIST_BC neighbours in one bank, 3 = other (coincident particles, particle
+// outside the tile's fp32 range)
+// CTR_NALL: n (level contexts: the per-call prologues compare it with n and skip the structure-of-arrays copies)
+// CTR_NFAST_ALL: particles served by the tiled kernels of the context or of one of its levels
+enum { CTR_NFAST = 1, CTR_NTILES = 2, CTR_NNONUNI = 3, CTR_POOL = 4, CTR_NALL = 5, CTR_NFAST_ALL = 6, CTR_NLEFT = 7, CTR_DECL = 8, CTR_COUNT = 12 };
 
 struct Ctx {
     int device = 0;
@@ -72,7 +76,11 @@ struct Ctx {
     int64_t hist_cap = 0;
     uint32_t *sorted_key = nullptr, *perm = nullptr;   // aliases into key[]/idx[] after the last pass
     uint32_t *cell_start = nullptr, *cell_end = nullptr;
+    uint32_t* cell_tend = nullptr;  // level contexts: end of the targets of a cell (they are sorted to the front of the cell)
     double* cell_hmax = nullptr;
+    double* cell_hmin = nullptr;    // per-cell min h (search-length pre-pass: a cell whose particles all have h >= h_b cannot be raised by b)
+    uint32_t* left = nullptr;       // sorted indices of the particles the tiled kernels (own + levels) do not serve: the general
+                                    // kernels run over this compact list at full lane occupancy; count in tl.ctr[CTR_NLEFT]
     double* hglob = nullptr;    // [0] = min h, [1] = max h (device scalars)
     uint32_t* dev_status = nullptr;
     Sorted s{};
@@ -81,16 +89,35 @@ struct Ctx {
     double* rad_scratch[4] = {nullptr, nullptr, nullptr, nullptr};   // N1: y, Lambda, Gamma, chi (caller order), allocated on first use
     int64_t launches = 0;       // kernels launched through this ctx (bench.py reports it as gpu_launches)
     int64_t scratch_bytes = 0;  // device memory held by this ctx
+    // ---- internal levels of the tiled path (spray_set_levels): a level is a context of its own on a grid of the library's
+    //      choosing (same box, cell edge >= level_edge), built from the same particles; it serves (tiles, lists, sweeps) only
+    //      the particles a with level_lo < 2 hs_a <= level_hi that nobody served before; the parent keeps the general kernels
+    int nlevels = 0;
+    Ctx* child[SPRAY_MAX_LEVELS] = {};
+    double level_edge[SPRAY_MAX_LEVELS] = {};
+    bool is_level = false;
+    double level_lo = 0.0, level_hi = 0.0;      // of a level context: its range of 2 hs
+    float level_rmax = 0.f;                     // of a level context: largest support radius it can meet (error bound of the fp32 prefilter)
+    const double* hs_caller = nullptr;          // level context: the parent's arrays below
+    const uint8_t* fast_caller = nullptr;
+    double* hs_c = nullptr;                     // parent: hs in caller order
+    uint8_t* fast_c = nullptr;                  // parent: 1 = served by the tiled kernels of the parent or of a level (caller order)
+    uint8_t* fast_all = nullptr;                // parent: the same in the parent's sorted order (skip flags of its general kernels)
+    bool levels_on = false;                     // the last build used the levels: fast_all / ctr[CTR_NFAST_ALL] are valid
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};   // recorded by spray_build_cells: start, cell list done, tiles done, lists done
     std::string err;
 };
 
 // ---- build.cu
 cudaError_t launch_cell_keys(Ctx* c, const double* x, const double* y, const double* z, cudaStream_t st);
+cudaError_t launch_to_caller_order(Ctx* c, cudaStream_t st);           // hs_c, fast_c from the sorted hs / fast of the parent
+cudaError_t launch_merge_served(Ctx* parent, Ctx* child, cudaStream_t st);   // fast_c |= the child's served targets
+cudaError_t launch_fast_from_caller(Ctx* c, cudaStream_t st);          // parent: fast_all[i] = fast_c[perm[i]], ctr[CTR_NFAST_ALL] = count
 cudaError_t launch_radix_sort(Ctx* c, cudaStream_t st);      // sets c->sorted_key / c->perm
 cudaError_t launch_cell_table(Ctx* c, cudaStream_t st);
 cudaError_t launch_reorder_build(Ctx* c, const double* x, const double* y, const double* z, const double* h, cudaStream_t st);
 cudaError_t launch_cell_hmax(Ctx* c, cudaStream_t st);
+cudaError_t launch_compact_left(Ctx* c, const uint8_t* fast, cudaStream_t st);   // c->left, ctr[CTR_NLEFT] from the served flags
 cudaError_t launch_excl_scan_u32(Ctx* c, uint32_t* a, int64_t total, uint32_t* scratch, cudaStream_t st);
 
 // ---- sweeps_ref.cu : general pair kernels (one thread per particle)
@@ -111,6 +138,8 @@ struct SweepArgs {
     uint64_t *odsum, *odxor;
     int symmetric;              // count / list / digest: which set
     const uint8_t* skip;        // nullable: particles with skip[i] != 0 are served by the tiled kernels
+    const uint32_t* left;       // nullable: the particles with skip[i] == 0, compacted (then the kernel runs over this list)
+    const unsigned long long* nleft;
     const unsigned long long* nfast;   // nullable: device count of such particles (== n: nothing to do)
 };
 cudaError_t launch_ref_sweep(Ctx* c, int sweep, const SweepArgs& a, cudaStream_t st);

@@ -9,6 +9,8 @@ namespace spray {
 struct CellTabs {
     const uint32_t *sorted_key, *perm, *cell_start, *cell_end;
     const double* hglob;
+    const double* cell_hmin;
+    const double* cell_hmax;      // per-cell max h: a cell farther from the target than 2 max(h_a, cell_hmax) holds no mutual neighbour
 };
 
 // cells to visit along one dimension: `cnt` cells starting at `start` (wrapped when periodic)
@@ -46,8 +48,19 @@ __device__ __forceinline__ double cell_gap2(int o, double f, bool full, double e
     return gp * gp;
 }
 
-template <int SWEEP, int KERNEL>
+// WARP = false: one thread per particle (the paper's scheme).  WARP = true: one WARP per particle -- the lanes share the
+// particle and split the candidates of every cell it visits; the partial sums are added by a fixed shuffle butterfly (so the
+// result does not depend on the launch) and lane 0 writes.  Used for the compact list of particles the tiled kernels leave
+// over, which are few and expensive (long search ranges through dense cells): 32 times the parallelism, coalesced candidates.
+template <class V>
+__device__ __forceinline__ V warp_add(V v) {
+#pragma unroll
+    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
+    return v;
+}
+template <int SWEEP, int KERNEL, bool WARP>
 __device__ __forceinline__ void ref_particle(const DevGrid& g, int64_t n, const CellTabs& T, const SweepArgs& A, int64_t i) {
+    const uint32_t j_lo = WARP ? (threadIdx.x & 31u) : 0u, j_st = WARP ? 32u : 1u;
     if (A.skip && A.skip[i]) return;        // served by the tiled kernels
     const double xa = A.x[i], ya = A.y[i], za = A.z[i], ha = A.h[i];
     const uint32_t ia = T.perm[i];
@@ -102,10 +115,17 @@ __device__ __forceinline__ void ref_particle(const DevGrid& g, int64_t n, const 
             if (gyz2 > reach2) continue;
             for (int kx = 0; kx < sx.cnt; ++kx) {
                 const int cxx = g.per[0] ? wrap_cell(sx.start + kx, g.nc[0]) : sx.start + kx;
-                if (gyz2 + cell_gap2(sx.start + kx - cx, fcx, fullx, ex) > reach2) continue;
+                const double gap2 = gyz2 + cell_gap2(sx.start + kx - cx, fcx, fullx, ex);
+                if (gap2 > reach2) continue;
                 const uint32_t c = (uint32_t)((czz * g.nc[1] + cyy) * g.nc[0] + cxx);
+                if (SWEEP == SW_HSEARCH && !(__ldg(T.cell_hmin + c) < ha)) continue;   // nobody in the cell has a smaller h
+                if (sym) {
+                    // symmetric sets: b in N_sym(a) needs r < 2 max(h_a, h_b) <= 2 max(h_a, max h of b's cell), and r >= the gap
+                    const double rc = 2.0 * fmax(ha, __ldg(T.cell_hmax + c));
+                    if (gap2 > (rc * rc) * (1.0 + 1e-9)) continue;
+                }
                 const uint32_t jb = __ldg(T.cell_start + c), je = __ldg(T.cell_end + c);
-                for (uint32_t j = jb; j < je; ++j) {
+                for (uint32_t j = jb + j_lo; j < je; j += j_st) {
                     const double dx = min_image(__dsub_rn(xa, __ldg(A.x + j)), g.per[0], g.L[0], g.halfL[0]);
                     const double dy = min_image(__dsub_rn(ya, __ldg(A.y + j)), g.per[1], g.L[1], g.halfL[1]);
                     const double dz = min_image(__dsub_rn(za, __ldg(A.z + j)), g.per[2], g.L[2], g.halfL[2]);
@@ -194,6 +214,22 @@ __device__ __forceinline__ void ref_particle(const DevGrid& g, int64_t n, const 
         }
     }
 
+    if (WARP) {
+        acc0 = warp_add(acc0); acc1 = warp_add(acc1); acc2 = warp_add(acc2); acc3 = warp_add(acc3); acc4 = warp_add(acc4);
+        cnt = warp_add(cnt);
+        if (SWEEP == SW_DIGEST) {
+            dsum = warp_add(dsum);
+#pragma unroll
+            for (int o = 16; o; o >>= 1) dxr ^= __shfl_xor_sync(0xFFFFFFFFu, dxr, o);
+        }
+        if (SWEEP == SW_KGC) {
+#pragma unroll
+            for (int e = 0; e < 6; ++e) km[e] = warp_add(km[e]);
+#pragma unroll
+            for (int e = 0; e < 9; ++e) kq[e] = warp_add(kq[e]);
+        }
+        if ((threadIdx.x & 31u) != 0u) return;
+    }
     if (SWEEP == SW_DENSITY) {
         A.o0[ia] = Wn * acc0;
         if (A.ocount) A.ocount[ia] = cnt;
@@ -259,14 +295,26 @@ template <int SWEEP, int KERNEL>
 __global__ void __launch_bounds__(128)
 k_ref_sweep(DevGrid g, int64_t n, CellTabs T, SweepArgs A) {
     if (A.nfast && *A.nfast == (unsigned long long)n) return;   // the tiled kernels serve every particle
+    if (A.left) {                                               // the rest, compacted: one warp per particle (SW_LIST: one thread)
+        const int64_t nl = (int64_t)*A.nleft;
+        if (SWEEP == SW_LIST) {
+            for (int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; t < nl; t += (int64_t)gridDim.x * blockDim.x)
+                ref_particle<SWEEP, KERNEL, false>(g, n, T, A, (int64_t)A.left[t]);
+        } else {
+            const int64_t nw = ((int64_t)gridDim.x * blockDim.x) >> 5;
+            for (int64_t t = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5; t < nl; t += nw)
+                ref_particle<SWEEP, KERNEL, true>(g, n, T, A, (int64_t)A.left[t]);
+        }
+        return;
+    }
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
-        ref_particle<SWEEP, KERNEL>(g, n, T, A, i);
+        ref_particle<SWEEP, KERNEL, false>(g, n, T, A, i);
 }
 
 template <int SWEEP>
 static cudaError_t launch_k(Ctx* c, const SweepArgs& a, cudaStream_t st) {
     if (c->n == 0) return cudaSuccess;
-    CellTabs T{c->sorted_key, c->perm, c->cell_start, c->cell_end, c->hglob};
+    CellTabs T{c->sorted_key, c->perm, c->cell_start, c->cell_end, c->hglob, c->cell_hmin, c->cell_hmax};
     const int64_t want = (c->n + 127) / 128;
     const int blocks = (int)(want < 148 * 64 ? want : 148 * 64);
     if (c->kernel == SPRAY_KERNEL_WENDLAND_C2) k_ref_sweep<SWEEP, 1><<<blocks, 128, 0, st>>>(c->dg, c->n, T, a);

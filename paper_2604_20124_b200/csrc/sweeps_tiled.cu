@@ -568,7 +568,7 @@ cudaError_t sweeps_set_attributes() {
 template <int SWEEP, int MODE>
 static cudaError_t launch_m(Ctx* c, const SweepIn& a, cudaStream_t st) {
     constexpr size_t smem = sweep_smem<SWEEP, MODE>();
-    CellTable ct{c->cell_start, c->cell_end};
+    CellTable ct{c->cell_start, c->cell_end, c->is_level ? c->cell_tend : c->cell_end};
     const int grid = c->tl.sms * MinBlocks<SWEEP, MODE>::v;
     if (c->kernel == SPRAY_KERNEL_WENDLAND_C2) k_tiled_sweep<SWEEP, 1, MODE><<<grid, TILE_THREADS, smem, st>>>(c->dg, ct, a);
     else k_tiled_sweep<SWEEP, 0, MODE><<<grid, TILE_THREADS, smem, st>>>(c->dg, ct, a);

@@ -29,7 +29,7 @@ namespace spray {
 // of every bundle, EMIT = true writes them at the scanned offsets, so the tile order is deterministic and follows
 // the grid (consecutive tiles share candidate rows in L2).
 struct RowRef {                      // one candidate row of a bundle
-    const uint32_t *cs, *ce;         // cell_start / cell_end of the row (indexed by column)
+    const uint32_t *cs, *ce, *te;    // cell_start / cell_end / cell_tend of the row (indexed by column)
     bool valid;
     bool target;                     // the row is one of the bundle's own rows
 };
@@ -56,19 +56,22 @@ __device__ __forceinline__ uint32_t warp_sum(uint32_t v) {
 template <bool EMIT>
 __global__ void __launch_bounds__(256)
 k_make_tiles(DevGrid g, CellTable ct, const double* __restrict__ hglob, uint32_t* __restrict__ bcount,
-             TileDesc* __restrict__ tiles, uint32_t cap, unsigned long long* __restrict__ ctr) {
-    const int nby = (g.nc[1] + 1) / 2, nbz = (g.nc[2] + 1) / 2;
+             TileDesc* __restrict__ tiles, uint32_t cap, unsigned long long* __restrict__ ctr, int level, unsigned long long n_all, int brows) {
+    // a bundle is brows x brows cell rows: 2 x 2 on the caller's grid (cells of ~18 particles: 4 x 4 candidate rows), 1 x 1 on the
+    // internal levels, whose cells hold up to ~60 particles (3 x 3 candidate rows fit the staging budget)
+    const int nby = (g.nc[1] + brows - 1) / brows, nbz = (g.nc[2] + brows - 1) / brows;
     const int b = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
     if (b >= nby * nbz) return;
     // every neighbour within one cell: 2 h_max <= cell edge in every dimension (tiny safety margin)
-    const double hmax = hglob[1];
+    // (a level context serves only particles whose 2 hs fits its cells: api.cu)
+    const double hmax = level ? 0.0 : hglob[1];
     bool ok = true;
     for (int d = 0; d < 3; ++d)
         if (!(2.0 * hmax * g.inv[d] * (1.0 + 1e-9) <= 1.0)) ok = false;
     const int nx = g.nc[0];
-    const int y0 = 2 * (b % nby), z0 = 2 * (b / nby);
-    const int nyr = min(2, g.nc[1] - y0), nzr = min(2, g.nc[2] - z0);
+    const int y0 = brows * (b % nby), z0 = brows * (b / nby);
+    const int nyr = min(brows, g.nc[1] - y0), nzr = min(brows, g.nc[2] - z0);
     RowRef row;
     {
         const int ry = lane & 3, rz = (lane >> 2) & 3;
@@ -80,7 +83,7 @@ k_make_tiles(DevGrid g, CellTable ct, const double* __restrict__ hglob, uint32_t
         else if (cz >= g.nc[2]) { if (g.per[2]) cz -= g.nc[2]; else row.valid = false; }
         row.target = row.valid && ry >= 1 && ry <= nyr && rz >= 1 && rz <= nzr;
         const uint32_t base = row.valid ? cell_id(g, 0, cy, cz) : 0u;
-        row.cs = ct.cell_start + base; row.ce = ct.cell_end + base;
+        row.cs = ct.cell_start + base; row.ce = ct.cell_end + base; row.te = ct.cell_tend + base;
     }
     const bool per = g.per[0] != 0;
     uint32_t ntl = 0;
@@ -100,7 +103,7 @@ k_make_tiles(DevGrid g, CellTable ct, const double* __restrict__ hglob, uint32_t
                     next_cxa = cx; next_skip = 0; break;
                 }
             }
-            uint32_t c = warp_sum(row.target ? row.ce[cx] - row.cs[cx] : 0u);
+            uint32_t c = warp_sum(row.target ? row.te[cx] - row.cs[cx] : 0u);
             if (cx == cxa) c -= skip;
             const uint32_t take = min(c, (uint32_t)TILE_T - nt);
             nt += take;
@@ -125,6 +128,7 @@ k_make_tiles(DevGrid g, CellTable ct, const double* __restrict__ hglob, uint32_t
         const uint32_t total = obase + ntl;
         ctr[CTR_NTILES] = total < cap ? total : cap;
         if (total > cap) ctr[CTR_NTILES] = cap;      // dropped tiles: their particles use the general kernels
+        ctr[CTR_NALL] = n_all;
     }
 }
 
@@ -176,6 +180,7 @@ struct ListArgs {
     const uint8_t* coinc;              // [n] sorted order: 1 = the particle has a twin at distance 0 (k_mark_coincident)
     const double* hglob;
     uint32_t* status;
+    float rmax;                        // > 0: largest support radius the unit can meet (level contexts); else 2 max h from hglob
 };
 
 constexpr int BL_THREADS = TILE_THREADS / 2;
@@ -250,7 +255,7 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
     uint16_t* wblk = reinterpret_cast<uint16_t*>(smem + BL_OFF_WB) + warp * WBLK_CAP;
     const int u = tid & 1, j = lane & 7;
     const uint32_t nunits = 2u * (uint32_t)A.ctr[CTR_NTILES];
-    const float Rmax = 2.0f * (float)A.hglob[1] * 1.000001f;
+    const float Rmax = A.rmax > 0.f ? A.rmax : 2.0f * (float)A.hglob[1] * 1.000001f;
     constexpr uint32_t BROW = 2u * BL_THREADS;                        // bytes per bucket row
 
     // tile table and descriptor of the first unit; afterwards each unit prefetches the next one's while it works
@@ -357,7 +362,8 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
             zmin = min(zmin, __shfl_xor_sync(0xFFFFFFFFu, zmin, o)); zmax = max(zmax, __shfl_xor_sync(0xFFFFFFFFu, zmax, o));
         }
         __syncthreads();                                                // flags reset by thread 0 above; column offsets written
-        if (tbad) s_bad = 1;
+        // (a target that cannot be served -- tbad here, bucket overflow or a list that is too long below -- is declined on its
+        //  own: empty lists, fast[i] stays 0, the general kernels compute it after the tiled sweeps and overwrite what they wrote)
         if (lane == 0 && cmax >= 0) { atomicMin(&s_clo, cmin); atomicMax(&s_chi, cmax); }
         if (tid == 0) s_h0 = ha;                                        // the half's first target: always there
         // ---- the warp's block list: lane q takes candidate range q, its blocks inside the warp's window (rows
@@ -422,7 +428,7 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
             }
             if (tid < TILE_NDUMMY) { X[TILE_CMAX + tid] = 3.0e18f; Y[TILE_CMAX + tid] = 3.0e18f; Z[TILE_CMAX + tid] = 3.0e18f; Tc[TILE_CMAX + tid] = 0.0f; }
             if (nonuni) s_nonuni = 1;                                   // some staged candidate differs from the first target's h
-            if (far) s_bad = 1;                                         // the error bound does not hold: general kernels
+            if (far) { s_bad = 1; atomicAdd(&A.ctr[CTR_DECL + 3], 1ull); }   // the error bound does not hold: general kernels
         }
         __syncthreads();
         const bool uni = s_nonuni == 0;
@@ -543,7 +549,10 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
                 cnt |= w << (8 * b);
             }
         }
-        if (ovf || coinc) s_bad = 1;
+        if (active && (ovf || coinc || (tbad && u == 0))) atomicAdd(&A.ctr[CTR_DECL + (ovf ? 2 : 3)], 1ull);
+        bool tdecl = ovf || coinc || tbad;                              // decline this target (both of its threads agree below)
+        tdecl = __shfl_xor_sync(0xFFFFFFFFu, (int)tdecl, 1) != 0 || tdecl;
+        if (tdecl) { cnt = 0; ng = 0; }
         // ---- split every bank bucket of the target between its two threads (alternate entries)
         const uint32_t cnt_o = __shfl_xor_sync(0xFFFFFFFFu, cnt, 1);
         ng += __shfl_xor_sync(0xFFFFFFFFu, ng, 1);
@@ -557,6 +566,14 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
             cu |= mine << (4 * beta);
             n_lane += mine; nsym += cb;
         }
+        {   // a list longer than the schedule can hold: decline the target
+            bool toolong = n_lane > (uint32_t)LIST_RMAX;
+            toolong = __shfl_xor_sync(0xFFFFFFFFu, (int)toolong, 1) != 0 || toolong;
+            if (toolong) {
+                if (active && u == 0) atomicAdd(&A.ctr[CTR_DECL + 2], 1ull);
+                tdecl = true; cu = 0; n_lane = 0; nsym = 0; ng = 0;
+            }
+        }
         uint32_t R = n_lane;
 #pragma unroll
         for (int o = 16; o; o >>= 1) R = max(R, __shfl_xor_sync(0xFFFFFFFFu, R, o));
@@ -567,10 +584,10 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
         // the order in which warps get there; the contents of the rows do not.  If another warp sends the unit to the general
         // kernels after this one has emitted (list too long, pool exhausted), the rows stay unused.
         uint32_t row0 = 0;
-        bool wbad = R > (uint32_t)LIST_RMAX || s_bad != 0;
+        bool wbad = s_bad != 0;
         if (lane == 0 && !wbad && R) {
             const unsigned long long r0 = atomicAdd(&A.ctr[CTR_POOL], (unsigned long long)(R >> 2));
-            if (r0 + (R >> 2) > (unsigned long long)A.pool_rows) wbad = true;   // pool exhausted: general kernels
+            if (r0 + (R >> 2) > (unsigned long long)A.pool_rows) { wbad = true; atomicAdd(&A.ctr[CTR_DECL + 1], 1ull); }   // pool exhausted
             row0 = (uint32_t)r0;
         }
         wbad = __shfl_sync(0xFFFFFFFFu, (int)wbad, 0) != 0;
@@ -644,17 +661,17 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
                 const uint32_t e2 = out[(r4 + 2) * BL_THREADS], e3 = out[(r4 + 3) * BL_THREADS];
                 blk[(size_t)(r4 >> 2) * 32] = make_uint2(e0 | (e1 << 16), e2 | (e3 << 16));
             }
-            if (u == 0) A.lcount[(size_t)tile * TILE_T + tgt] = active ? (ng | (nsym << 16)) : 0u;
+            if (u == 0) A.lcount[(size_t)tile * TILE_T + tgt] = (active && !tdecl) ? (ng | (nsym << 16)) : 0u;
             if (lane == 0) A.winfo[(size_t)tile * TILE_WARPS + twarp] = make_uint2(row0, R);
         }
-        __syncthreads();
+        const int served = __syncthreads_count(active && u == 0 && !tdecl);
         const bool bad = s_bad != 0;
-        if (!bad && active && u == 0) A.fast[i] = 1;
+        if (!bad && active && u == 0 && !tdecl) A.fast[i] = 1;
         if (tid == 0) {
             const uint32_t bits = (bad ? 0u : (TILE_FLAG_OK0 << half)) | (s_nonuni ? TILE_FLAG_NONUNI : 0u);
             if (bits) atomicOr(&A.tflags[tile], bits);
             if (s_nonuni) atomicAdd(&A.ctr[CTR_NNONUNI], 1ull);
-            if (!bad) atomicAdd(&A.ctr[CTR_NFAST], (unsigned long long)min((int)td.nt - half * BL_TGT, BL_TGT));
+            if (!bad) atomicAdd(&A.ctr[CTR_NFAST], (unsigned long long)served);
         }
         }
         // the next unit's table goes into the other buffer (read after the barrier at the top of the loop)
@@ -807,22 +824,24 @@ cudaError_t launch_build_tiles(Ctx* c, cudaStream_t st) {
     if (gr.periodic[1] && gr.ncell[1] < 4) return cudaSuccess;
     if (gr.periodic[2] && gr.ncell[2] < 4) return cudaSuccess;
     if (gr.ncell[0] > 32000 || gr.ncell[1] > 32000 || gr.ncell[2] > 32000) return cudaSuccess;
-    const int64_t nb = (int64_t)((gr.ncell[1] + 1) / 2) * ((gr.ncell[2] + 1) / 2);
+    const int brows = c->is_level ? 1 : 2;
+    const int64_t nb = (int64_t)((gr.ncell[1] + brows - 1) / brows) * ((gr.ncell[2] + brows - 1) / brows);
     if (nb > t.bundle_cap) return cudaSuccess;
     cudaError_t e;
     if ((e = cudaMemsetAsync(t.ctr, 0, sizeof(unsigned long long) * CTR_COUNT, st)) != cudaSuccess) return e;
     if ((e = cudaMemsetAsync(t.fast, 0, (size_t)c->n, st)) != cudaSuccess) return e;
     if ((e = launch_mark_coincident(c, st)) != cudaSuccess) return e;
-    CellTable ct{c->cell_start, c->cell_end};
+    CellTable ct{c->cell_start, c->cell_end, c->is_level ? c->cell_tend : c->cell_end};
     const int blocks = (int)((nb * 32 + 255) / 256);
-    k_make_tiles<false><<<blocks, 256, 0, st>>>(c->dg, ct, c->hglob, t.bcount, t.tiles, (uint32_t)t.tile_cap, t.ctr);
+    const int lvl = c->is_level ? 1 : 0;
+    k_make_tiles<false><<<blocks, 256, 0, st>>>(c->dg, ct, c->hglob, t.bcount, t.tiles, (uint32_t)t.tile_cap, t.ctr, lvl, (unsigned long long)c->n, brows);
     if ((e = launch_excl_scan_u32(c, t.bcount, nb, t.bcount + t.bundle_cap, st)) != cudaSuccess) return e;
-    k_make_tiles<true><<<blocks, 256, 0, st>>>(c->dg, ct, c->hglob, t.bcount, t.tiles, (uint32_t)t.tile_cap, t.ctr);
+    k_make_tiles<true><<<blocks, 256, 0, st>>>(c->dg, ct, c->hglob, t.bcount, t.tiles, (uint32_t)t.tile_cap, t.ctr, lvl, (unsigned long long)c->n, brows);
     k_tile_tables<<<t.sms * 8, 128, 0, st>>>(c->dg, ct, t.tiles, t.ctr, t.tiletab);
     if ((e = cudaMemsetAsync(t.tflags, 0, sizeof(uint32_t) * (size_t)t.tile_cap, st)) != cudaSuccess) return e;
     if (c->ev[2]) cudaEventRecord(c->ev[2], st);
     ListArgs A{c->pk.p0, c->pk.p1, t.tiles, t.ctr, t.pool, (uint32_t)t.pool_rows, t.winfo, t.lcount, t.tflags, t.tiletab, t.fast,
-               t.coinc, c->hglob, c->dev_status};
+               t.coinc, c->hglob, c->dev_status, c->is_level ? c->level_rmax : 0.f};
     k_build_lists<<<t.sms * 2, BL_THREADS, BL_SMEM, st>>>(c->dg, ct, A);
     c->launches += 4;
     t.enabled = true;

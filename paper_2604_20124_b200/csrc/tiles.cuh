@@ -56,6 +56,8 @@ constexpr uint32_t TILE_FLAG_NONUNI = 4u;    // NOT every target and candidate o
 struct CellTable {
     const uint32_t* cell_start;
     const uint32_t* cell_end;
+    const uint32_t* cell_tend;       // the TARGETS of a cell are the slots [cell_start, cell_tend); = cell_end unless the grid is an
+                                     // internal level of the tiled path, which serves only the particles of its h range (api.cu)
 };
 
 // Per-CTA tile tables in shared memory (filled by tile_setup)
@@ -173,7 +175,7 @@ __device__ __forceinline__ void tile_setup(const TileDesc& td, const DevGrid& g,
             int cx, ry, rz;
             tile_cell_rc(td, e, cx, ry, rz);
             const uint32_t c = cell_id(g, cx, td.y0 + ry, td.z0 + rz);
-            const uint32_t a = ct.cell_start[c], b = ct.cell_end[c];
+            const uint32_t a = ct.cell_start[c], b = ct.cell_tend[c];
             S.c_first[e] = a;
             S.c_pre[e + 1] = b - a;          // counts, scanned below
         }

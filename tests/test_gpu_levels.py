@@ -1,0 +1,68 @@
+"""The internal levels of the tiled path (spray_set_levels): particle sets whose smoothing lengths do not fit the caller's grid
+(BASELINE.json configs 2 and 4: cell edge 2 mean(h)) are served by the tiled kernels on grids of the
+library's own, with the same bit-exact neighbour sets and the same sums as the oracle."""
+import numpy as np
+import pytest
+
+import oracle as O
+import workloads as W
+from parity_util import compare_isolated, gpu_isolated, make_ctx, oracle_isolated, u32, u64, upload
+
+pytestmark = pytest.mark.gpu
+
+
+def get(name):
+    if name == "cloud":
+        return W.random_cloud(6000, seed=21, periodic=(1, 0, 1), hvar=2.5)
+    return W.make(name)
+
+
+@pytest.mark.parametrize("name", ["c2_tiny", "c4_tiny", "c2_mid", "c4_mid", "cloud"])
+@pytest.mark.parametrize("kmode", [0, 1])
+def test_levels_parity(name, kmode):
+    w = get(name)
+    d = upload(w)
+    sp = make_ctx(w)
+    sp.set_levels(w.grid, W.level_edges(w.h))
+    sp.build_cells(w.grid, w.kernel, d["x"], d["y"], d["z"], d["h"])
+    st = sp.path_stats_full()
+    # the cell table is the caller's grid's, whatever the levels do
+    ref = O.build_cells(w.grid, w.x, w.y, w.z)
+    t = sp.get_cell_table()
+    for k in ("sorted_key", "perm", "cell_start", "cell_end"):
+        assert np.array_equal(u32(t[k]), ref[k]), k
+    for sym, mode in ((False, O.GATHER), (True, O.SYM)):
+        cnt, ds, dx = O.neighbor_digest(w.grid, w.x, w.y, w.z, w.h, mode)
+        assert np.array_equal(u32(sp.neighbor_counts(sym)), cnt), (name, sym)
+        gs, gx = sp.neighbor_digest(sym)
+        assert np.array_equal(u64(gs), ds) and np.array_equal(u64(gx), dx), (name, sym)
+        off, nbr = sp.neighbor_lists(sym)
+        ooff, onbr = O.neighbor_lists(w.grid, w.x, w.y, w.z, w.h, mode)
+        assert np.array_equal(off.cpu().numpy().astype(np.uint64), ooff) and np.array_equal(u32(nbr), onbr)
+    mu_full = O.limiter(w.grid, w.kernel, w.x, w.y, w.z, w.h, w.m, w.rho_nom, w.kappa, w.E, w.c_light)["mu"]
+    g = gpu_isolated(sp, d, w, mu_in=mu_full, kmode=kmode)
+    o = oracle_isolated(w, sym_mode=(kmode == 0), mu_full=mu_full)
+    errs = compare_isolated(g, o)
+    assert sp.check() == 0
+    print(name, "kmode", kmode, st, {k: f"{v:.1e}" for k, v in errs.items()})
+    if name in ("c2_mid", "c4_mid"):
+        assert st["n_fast"] >= 0.7 * w.n, st           # most of the set is on the tiled path now
+
+
+def test_levels_are_optional_and_removable():
+    w = W.make("c4_tiny")
+    d = upload(w)
+    sp = make_ctx(w)
+    sp.build_cells(w.grid, w.kernel, d["x"], d["y"], d["z"], d["h"])
+    r0 = sp.density(d["m"]).clone()
+    f0 = sp.path_stats_full()["n_fast"]
+    sp.set_levels(w.grid, W.level_edges(w.h))
+    sp.build_cells(w.grid, w.kernel, d["x"], d["y"], d["z"], d["h"])
+    r1 = sp.density(d["m"]).clone()
+    f1 = sp.path_stats_full()["n_fast"]
+    sp.set_levels(w.grid, [])
+    sp.build_cells(w.grid, w.kernel, d["x"], d["y"], d["z"], d["h"])
+    r2 = sp.density(d["m"])
+    assert f1 > f0 and sp.path_stats_full()["n_fast"] == f0
+    S = O.density(w.grid, w.kernel, w.x, w.y, w.z, w.h, w.m)["S_rho"]
+    assert np.all(np.abs((r1 - r0).cpu().numpy()) <= 1e-11 * S) and bool((r2 == r0).all())

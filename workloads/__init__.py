@@ -417,3 +417,15 @@ def random_cloud(n: int, seed: int = 12345, kernel: int = KERNEL_WENDLAND_C2, pe
     w = _finish(f"cloud{n}", kernel, grid, 5.0 / 3.0, x, y, z, h, m, rho, u, vx, vy, vz, E, kappa)
     w.alpha = 0.2 + u01(seed, i, 15)
     return w
+
+
+def level_edges(h: np.ndarray, ratio: float = 1.5, max_levels: int = 16):
+    """Cell edges for the internal levels of the tiled path (spray_set_levels): a geometric sequence from 2 min(h) up to
+    2 max(h), the last one exactly 2 max(h) (all with a 1e-6 margin), at most `max_levels` values.  A grid choice like
+    `_uniform_grid` (A14): no SPH arithmetic."""
+    lo, hi = 2.0 * float(np.min(h)) * (1.0 + 1e-6), 2.0 * float(np.max(h)) * (1.0 + 1e-6)
+    if hi <= lo * (1.0 + 1e-9):
+        return [hi]
+    k = max(1, min(max_levels - 1, int(math.ceil(math.log(hi / lo) / math.log(ratio)))))
+    r = (hi / lo) ** (1.0 / k)
+    return [lo * r ** i for i in range(k)] + [hi]
