@@ -275,7 +275,7 @@ def main():
             sp.hydro_rhs_limiter(src["m"], o["rho"], src["p"], src["cs"], src["vx"], src["vy"], src["vz"], src["alpha"], src["E"], src["kappa"],
                                  beta=w.beta, c_light=w.c_light, out=hy, mu=o["mu"])
             if between: between()
-            sp.fld_apply(src["m"], o["rho"], None, src["E"], w.c_light, lmode=P.FLD_FROZEN, mu=o["mu"], y=o["y"], diag=o["diag"], offd=o["offd"])
+            sp.fld_apply(src["m"], o["rho"], None, src["E"], w.c_light, lmode=P.FLD_FROZEN_CHAINED, mu=o["mu"], y=o["y"], diag=o["diag"], offd=o["offd"])
         else:
             sp.hydro_rhs(src["m"], o["rho"], src["p"], src["cs"], src["vx"], src["vy"], src["vz"], src["alpha"], w.beta, out=hy)
             if between: between()
@@ -614,7 +614,7 @@ def main():
                 "per_call_ms": {k: 1e3 * float(v) for k, v in calls.items()},
                 "per_call_tflops": {"density": flops["density"] / calls["density"] / 1e12, "hydro": hyd_flops / calls["hydro"] / 1e12,
                                     "fld": fld_flops / calls["fld"] / 1e12},
-                "calls": (["spray_build_cells", "spray_density", "spray_hydro_rhs_limiter", "spray_fld_apply(FROZEN)"] if fused else
+                "calls": (["spray_build_cells", "spray_density", "spray_hydro_rhs_limiter", "spray_fld_apply(FROZEN_CHAINED)"] if fused else
                           ["spray_build_cells", "spray_density", "spray_hydro_rhs", "spray_fld_apply(UPDATE_LIMITER)"])}
 
     cpu = None

@@ -59,7 +59,11 @@ enum {
 
 typedef enum { SPRAY_KERNEL_CUBIC_SPLINE = 0, SPRAY_KERNEL_WENDLAND_C2 = 1 } spray_kernel_t;
 typedef enum { SPRAY_FLD_SYMMETRIC = 0, SPRAY_FLD_GATHER = 1 } spray_fld_kernel_mode_t;       /* A17 */
-typedef enum { SPRAY_FLD_UPDATE_LIMITER = 0, SPRAY_FLD_FROZEN = 1 } spray_fld_limiter_mode_t; /* A18 */
+typedef enum { SPRAY_FLD_UPDATE_LIMITER = 0, SPRAY_FLD_FROZEN = 1,
+               /* FROZEN, called right after spray_hydro_rhs_limiter on this context with the same m, rho, E arrays and the mu array
+                * that call wrote: the sorted operator records it left are reused and the per-call prologue (one pass over all
+                * particles) is skipped; same results bit for bit.  SPRAY_ERR_INVALID_ARG if the context did anything else since. */
+               SPRAY_FLD_FROZEN_CHAINED = 2 } spray_fld_limiter_mode_t; /* A18 */
 
 /* Uniform cell grid (an INPUT, A14; "dimensions of these cells are ... determined based on the average
  * smoothing length ... during the initialization phase").  h_max is the caller-declared upper bound on h. */

@@ -220,8 +220,12 @@ static int cell_span(const oracle_grid_t* g, int d, double p, double reach, int*
         if (c1 - c0 + 1 >= nc) { for (int c = 0; c < nc; ++c) out[cnt++] = c; return cnt; }
         for (int64_t c = c0; c <= c1; ++c) out[cnt++] = (int)(((c % nc) + nc) % nc);
     } else {
+        /* a point outside an open box lives in the edge cell it was clamped into (O1, A16): both ends of the span are clamped
+         * into [0, nc-1], so that such a point still finds the other points clamped into the same edge cells */
         if (c0 < 0) c0 = 0;
+        if (c0 > nc - 1) c0 = nc - 1;
         if (c1 > nc - 1) c1 = nc - 1;
+        if (c1 < 0) c1 = 0;
         for (int64_t c = c0; c <= c1; ++c) out[cnt++] = (int)c;
     }
     return cnt;

@@ -12,13 +12,13 @@ import ctypes as C
 from pathlib import Path
 
 __all__ = ["load", "Spray", "SprayError", "KERNEL_CUBIC_SPLINE", "KERNEL_WENDLAND_C2", "FLD_SYMMETRIC", "FLD_GATHER",
-           "FLD_UPDATE_LIMITER", "FLD_FROZEN", "EXPORTS"]
+           "FLD_UPDATE_LIMITER", "FLD_FROZEN", "FLD_FROZEN_CHAINED", "EXPORTS"]
 
 _LIBPATH = Path(__file__).resolve().parent / "libspray_b200.so"
 
 KERNEL_CUBIC_SPLINE, KERNEL_WENDLAND_C2 = 0, 1
 FLD_SYMMETRIC, FLD_GATHER = 0, 1
-FLD_UPDATE_LIMITER, FLD_FROZEN = 0, 1
+FLD_UPDATE_LIMITER, FLD_FROZEN, FLD_FROZEN_CHAINED = 0, 1, 2
 COND_OPERATOR, COND_RHS = 0, 1
 DEV_H_EXCEEDS_HMAX, DEV_OUTSIDE_BOX, DEV_LIST_OVERFLOW = 1, 2, 4
 

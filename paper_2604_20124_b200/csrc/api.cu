@@ -49,7 +49,7 @@ void free_all(Ctx* c) {
     for (double2* r : k.s) cudaFree(r);
     Tiled& t = c->tl;
     cudaFree(t.tiles); cudaFree(t.bcount); cudaFree(t.pool); cudaFree(t.ctr); cudaFree(t.winfo); cudaFree(t.lcount);
-    cudaFree(t.tflags); cudaFree(t.tiletab); cudaFree(t.fast); cudaFree(t.coinc);
+    cudaFree(t.tflags); cudaFree(t.tiletab); cudaFree(t.fast);
 }
 
 // Scratch of the tiled path (tiles, tile tables, neighbour-list pool), allocated once by spray_create from n_max and
@@ -69,12 +69,12 @@ void alloc_tiled(Ctx* c) {
     const int64_t rows = (n * 208) / 256 + 4096;
     bool ok = dmalloc(&t.tiles, tiles, c) && dmalloc(&t.bcount, nb + 4096 + 64, c) && dmalloc(&t.winfo, tiles * TILE_WARPS, c) &&
               dmalloc(&t.lcount, tiles * TILE_T, c) && dmalloc(&t.tflags, tiles, c) && dmalloc(&t.tiletab, tiles * TILES_WORDS, c) &&
-              dmalloc(&t.pool, rows * 32, c) && dmalloc(&t.ctr, CTR_COUNT, c) && dmalloc(&t.fast, n, c) && dmalloc(&t.coinc, n, c);
+              dmalloc(&t.pool, rows * 32, c) && dmalloc(&t.ctr, CTR_COUNT, c) && dmalloc(&t.fast, n, c);
     if (ok) ok = tiled_set_attributes(c) == cudaSuccess;
     if (!ok) {
         cudaGetLastError();
         cudaFree(t.tiles); cudaFree(t.bcount); cudaFree(t.pool); cudaFree(t.winfo); cudaFree(t.lcount); cudaFree(t.tflags); cudaFree(t.tiletab);
-        cudaFree(t.ctr); cudaFree(t.fast); cudaFree(t.coinc);
+        cudaFree(t.ctr); cudaFree(t.fast);
         t = Tiled{};
         int sms = 0;
         if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device) == cudaSuccess && sms > 0) t.sms = sms;
@@ -389,6 +389,7 @@ int spray_build_cells(spray_ctx* ctx, const spray_grid_t* g, spray_kernel_t kern
     if (!ctx) return SPRAY_ERR_INVALID_ARG;
     Ctx* c = &ctx->c;
     c->built = false;
+    c->chain_ok = false;
     DeviceGuard dg(c->device);
     if (!dg.ok) { cudaGetLastError(); return fail(c, SPRAY_ERR_CUDA, "cudaSetDevice failed"); }
     if (!g || n < 0 || (n > 0 && (!x || !y || !z || !h))) return fail(c, SPRAY_ERR_INVALID_ARG, "spray_build_cells: NULL argument or n < 0");
@@ -444,6 +445,7 @@ int spray_build_cells(spray_ctx* ctx, const spray_grid_t* g, spray_kernel_t kern
 int spray_density(spray_ctx* ctx, const double* m, double* rho, uint32_t* nnbr, void* stream) {
     NEED_BUILT();
     Ctx* c = &ctx->c;
+    c->chain_ok = false;
     if (c->n > 0 && (!m || !rho)) return fail(c, SPRAY_ERR_INVALID_ARG, "spray_density: NULL argument");
     cudaStream_t st = (cudaStream_t)stream;
     CK(launch_prep_density(c, m, st), "density prologue");
@@ -465,6 +467,7 @@ int spray_hydro_rhs(spray_ctx* ctx, const double* m, const double* rho, const do
                     double* ax, double* ay, double* az, double* dudt, double* divv_sum, void* stream) {
     NEED_BUILT();
     Ctx* c = &ctx->c;
+    c->chain_ok = false;
     if (c->n > 0 && (!m || !rho || !p || !cs || !vx || !vy || !vz || !alpha || !ax || !ay || !az || !dudt))
         return fail(c, SPRAY_ERR_INVALID_ARG, "spray_hydro_rhs: NULL argument");
     cudaStream_t st = (cudaStream_t)stream;
@@ -527,6 +530,9 @@ int spray_hydro_rhs_limiter(spray_ctx* ctx, const double* m, const double* rho, 
     l.c_light = c_light;
     l.o0 = mu; l.o1 = gradE; l.mu_sorted = f[F_MU]; l.me_sorted = c->pk.me;
     CK(launch_ref_sweep(c, SW_LIMITER, l, st), "limiter sweep");
+    // the sorted (z, V) and (mu, E) records of every particle are in place: spray_fld_apply(SPRAY_FLD_FROZEN_CHAINED) may reuse them
+    c->chain_ok = !c->levels_on;
+    c->chain_m = m; c->chain_rho = rho; c->chain_E = E; c->chain_mu = mu;
     return SPRAY_OK;
 }
 
@@ -536,16 +542,25 @@ int spray_fld_apply(spray_ctx* ctx, const double* m, const double* rho, const do
     NEED_BUILT();
     Ctx* c = &ctx->c;
     const bool update = (lmode == SPRAY_FLD_UPDATE_LIMITER);
+    // FROZEN_CHAINED: FROZEN with the same m, rho, E and the mu that the spray_hydro_rhs_limiter call just before produced:
+    // that call left the sorted records of the operator in place, so the prologue (a pass over all particles) is skipped
+    bool chained = (lmode == SPRAY_FLD_FROZEN_CHAINED);
+    if (chained && !(c->chain_ok && m == c->chain_m && rho == c->chain_rho && E == c->chain_E && mu == c->chain_mu)) {
+        if (!c->levels_on) return fail(c, SPRAY_ERR_INVALID_ARG, "spray_fld_apply(FROZEN_CHAINED): not preceded by spray_hydro_rhs_limiter on the same arrays");
+        chained = false;                                   // with internal levels the records are re-packed (FROZEN)
+    }
+    if (!chained) c->chain_ok = false;
     if (c->n > 0 && (!m || !rho || !E || !mu || !y || (update && !kappa)))
         return fail(c, SPRAY_ERR_INVALID_ARG, "spray_fld_apply: NULL argument");
-    if ((kmode != SPRAY_FLD_SYMMETRIC && kmode != SPRAY_FLD_GATHER) || (lmode != SPRAY_FLD_UPDATE_LIMITER && lmode != SPRAY_FLD_FROZEN))
+    if ((kmode != SPRAY_FLD_SYMMETRIC && kmode != SPRAY_FLD_GATHER) ||
+        (lmode != SPRAY_FLD_UPDATE_LIMITER && lmode != SPRAY_FLD_FROZEN && lmode != SPRAY_FLD_FROZEN_CHAINED))
         return fail(c, SPRAY_ERR_INVALID_ARG, "spray_fld_apply: unknown mode");
     cudaStream_t st = (cudaStream_t)stream;
     double** f = c->s.f;
     PrepJob pj{};
     pj.m = m; pj.rho = rho; pj.E = E; pj.kx = update ? kappa : mu; pj.kx_is_mu = update ? 0 : 1;
     pj.sm = f[F_M]; pj.srho = f[F_RHO]; pj.sE = f[F_E]; pj.skx = update ? f[F_KAPPA] : f[F_MU]; pj.sV = f[F_V];
-    CK(launch_prep_fld(c, pj, st), "fld prologue");
+    if (!chained) CK(launch_prep_fld(c, pj, st), "fld prologue");
     const TiledSet ts = tiled_set(c);
     for (int k = 0; k < ts.n; ++k)
         if (ts.v[k] != c) CK(launch_prep_fld(ts.v[k], level_job(pj, ts.v[k]), st), "fld prologue (level)");
@@ -587,6 +602,7 @@ int spray_conduction(spray_ctx* ctx, const double* m, const double* rho, const d
                      void* stream) {
     NEED_BUILT();
     Ctx* c = &ctx->c;
+    c->chain_ok = false;
     if (c->n > 0 && (!m || !rho || !k || !T || !dudt)) return fail(c, SPRAY_ERR_INVALID_ARG, "spray_conduction: NULL argument");
     cudaStream_t st = (cudaStream_t)stream;
     double** f = c->s.f;
@@ -630,6 +646,7 @@ int spray_conduction_implicit(spray_ctx* ctx, const double* m, const double* rho
                               void* stream) {
     NEED_BUILT();
     Ctx* c = &ctx->c;
+    c->chain_ok = false;
     if (which != SPRAY_COND_OPERATOR && which != SPRAY_COND_RHS) return fail(c, SPRAY_ERR_INVALID_ARG, "spray_conduction_implicit: unknown `which`");
     const bool rhs = which == SPRAY_COND_RHS;
     if (c->n > 0 && (!m || !rho || !k_i || !k_e || !kei || !dTdu_i || !dTdu_e || !u_i || !u_e || !out_i || !out_e || (rhs && (!T_i || !T_e))))
@@ -653,6 +670,7 @@ int spray_kgc_continuity(spray_ctx* ctx, const double* m, const double* rho, con
                          const double* vz, double* drhodt, double* L, double* drhodt_raw, void* stream) {
     NEED_BUILT();
     Ctx* c = &ctx->c;
+    c->chain_ok = false;
     if (c->n > 0 && (!m || !rho || !vx || !vy || !vz || !drhodt))
         return fail(c, SPRAY_ERR_INVALID_ARG, "spray_kgc_continuity: NULL argument");
     cudaStream_t st = (cudaStream_t)stream;
@@ -678,6 +696,7 @@ int spray_rad_jacobi(spray_ctx* ctx, const double* m, const double* rho, const d
                      double a_rad, spray_fld_kernel_mode_t kmode, int niter, double* E, double* u, double* resid, void* stream) {
     NEED_BUILT();
     Ctx* c = &ctx->c;
+    c->chain_ok = false;
     if (c->n > 0 && (!m || !rho || !mu || !kappa_p || !E_n || !u_n || !T_n || !dTdu || !E || !u))
         return fail(c, SPRAY_ERR_INVALID_ARG, "spray_rad_jacobi: NULL argument");
     if (!(dt > 0.0) || !(c_light > 0.0) || !(a_rad > 0.0) || niter < 1 || (kmode != SPRAY_FLD_SYMMETRIC && kmode != SPRAY_FLD_GATHER))
@@ -717,6 +736,7 @@ int spray_ray_deposit(spray_ctx* ctx, const double* m, const double* rho, const 
                       double* rays_out, int64_t* steps_out, void* stream) {
     NEED_BUILT();
     Ctx* c = &ctx->c;
+    c->chain_ok = false;
     if (c->n > 0 && (!m || !rho || !f || !kib || !edep)) return fail(c, SPRAY_ERR_INVALID_ARG, "spray_ray_deposit: NULL argument");
     if (nrays < 0 || nsteps < 0 || (nrays > 0 && (!rays_in || !rays_out)) || !(dt > 0.0) || !(c_light > 0.0))
         return fail(c, SPRAY_ERR_INVALID_ARG, "spray_ray_deposit: nrays, nsteps >= 0, dt, c_light > 0, ray buffers non-NULL");

@@ -319,57 +319,6 @@ __global__ void k_cell_hmax(const uint32_t* __restrict__ cell_start, const uint3
     }
 }
 
-// Particles that have a twin at distance zero -- r2 of the contract expression (O2) at or below 1e-290, where the
-// reciprocal square root of the tiled pair bodies is no longer defined -- are marked here and left to the general
-// kernels, which treat r2 == 0 as the oracle does (A11: W(0) in eq. (35), nothing in the gradient sums).  Such a pair
-// shares a cell, except where a cell face lies at the coordinate value 0 exactly (two doubles closer than 1e-145 to each
-// other are both closer than that to 0): a particle with a coordinate that small looks at the 26 cells around its own
-// as well.  A cell with more than 512 particles is not searched (its particles are marked: the tiled path cannot take
-// such a cell anyway).
-__global__ void k_mark_coincident(DevGrid g, int64_t n, const uint32_t* __restrict__ sorted_key, const uint32_t* __restrict__ cell_start,
-                                  const uint32_t* __restrict__ cell_end, const double* __restrict__ x, const double* __restrict__ y,
-                                  const double* __restrict__ z, uint8_t* __restrict__ coinc, int key_shift) {
-    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const uint32_t key = sorted_key[i] >> key_shift;
-    const uint32_t cs = cell_start[key], ce = cell_end[key];
-    const double xi = x[i], yi = y[i], zi = z[i];
-    constexpr double TINY = 1.0e-140, R2MIN = 1.0e-290;
-    bool hit = false;
-    auto test = [&](uint32_t j) {
-        const double dx = min_image(__dsub_rn(xi, x[j]), g.per[0], g.L[0], g.halfL[0]);
-        if (!(fabs(dx) < TINY)) return;
-        const double dy = min_image(__dsub_rn(yi, y[j]), g.per[1], g.L[1], g.halfL[1]);
-        const double dz = min_image(__dsub_rn(zi, z[j]), g.per[2], g.L[2], g.halfL[2]);
-        if (r2_exact(dx, dy, dz) <= R2MIN) { hit = true; coinc[j] = 1; }
-    };
-    if (ce - cs > 512u) {
-        hit = true;
-    } else {
-        // two distinct doubles closer than 1e-140 are both tiny (handled below), so in the common case a twin has the same x bit for bit
-        for (uint32_t j = (uint32_t)i + 1u; j < ce; ++j)
-            if (__ldg(x + j) == xi) test(j);
-        if (fabs(xi) < TINY || fabs(yi) < TINY || fabs(zi) < TINY) {
-            const int cx = key % g.nc[0], cy = (key / g.nc[0]) % g.nc[1], cz = key / (g.nc[0] * g.nc[1]);
-            for (int oz = -1; oz <= 1; ++oz) for (int oy = -1; oy <= 1; ++oy) for (int ox = -1; ox <= 1; ++ox) {
-                int c3[3] = {cx + ox, cy + oy, cz + oz};
-                bool ok = true;
-                for (int d = 0; d < 3; ++d) {
-                    if (c3[d] < 0 || c3[d] >= g.nc[d]) {
-                        if (g.per[d]) c3[d] = (c3[d] + g.nc[d]) % g.nc[d]; else ok = false;
-                    }
-                }
-                if (!ok) continue;
-                const uint32_t c = (uint32_t)((c3[2] * g.nc[1] + c3[1]) * g.nc[0] + c3[0]);
-                const uint32_t a = cell_start[c], b = cell_end[c];
-                if (b - a > 512u) { hit = true; continue; }
-                for (uint32_t j = a; j < b; ++j) if (j != (uint32_t)i) test(j);
-            }
-        }
-    }
-    if (hit) coinc[i] = 1;
-}
-
 // ---- levels (api.cu): per-particle data between the parent (sorted order) and the level contexts (caller order)
 __global__ void k_to_caller(const uint32_t* __restrict__ perm, int64_t n, const double* __restrict__ hs, const uint8_t* __restrict__ fast,
                             double* __restrict__ hs_c, uint8_t* __restrict__ fast_c) {
@@ -442,16 +391,6 @@ cudaError_t launch_fast_from_caller(Ctx* c, cudaStream_t st) {
     cudaError_t e = cudaMemsetAsync(c->tl.ctr + CTR_NFAST_ALL, 0, sizeof(unsigned long long), st);
     if (e != cudaSuccess) return e;
     k_fast_from_caller<<<cdiv64(c->n, 256), 256, 0, st>>>(c->perm, c->n, c->fast_c, c->fast_all, c->tl.ctr + CTR_NFAST_ALL);
-    c->launches += 1;
-    return cudaGetLastError();
-}
-
-cudaError_t launch_mark_coincident(Ctx* c, cudaStream_t st) {
-    if (c->n == 0 || !c->tl.coinc) return cudaSuccess;
-    cudaError_t e = cudaMemsetAsync(c->tl.coinc, 0, (size_t)c->n, st);
-    if (e != cudaSuccess) return e;
-    k_mark_coincident<<<cdiv64(c->n, 256), 256, 0, st>>>(c->dg, c->n, c->sorted_key, c->cell_start, c->cell_end, c->s.x, c->s.y, c->s.z,
-                                                        c->tl.coinc, c->is_level ? 1 : 0);
     c->launches += 1;
     return cudaGetLastError();
 }

@@ -49,7 +49,6 @@ struct Tiled {
     uint32_t* tflags = nullptr;  // [tile_cap]: TILE_FLAG_*
     uint32_t* tiletab = nullptr; // [tile_cap][TILES_WORDS]: per-tile TileS tables
     uint8_t* fast = nullptr;     // [n_max] sorted order: 1 = particle is served by the tiled kernels
-    uint8_t* coinc = nullptr;    // [n_max] sorted order: 1 = particle has a twin at distance 0 (general kernels, A11)
     int attr_device = -1;        // device on which the dynamic shared-memory opt-in of the tiled kernels was set
 };
 // CTR_NFAST: particles served by the tiled kernels; CTR_NTILES: tiles; CTR_NNONUNI: half-tile units that found non-uniform h;
@@ -87,6 +86,8 @@ struct Ctx {
     Packed pk{};
     Tiled tl{};
     double* rad_scratch[4] = {nullptr, nullptr, nullptr, nullptr};   // N1: y, Lambda, Gamma, chi (caller order), allocated on first use
+    bool chain_ok = false;      // the sorted records of the FLD operator are those of the last spray_hydro_rhs_limiter (FROZEN_CHAINED)
+    const double *chain_m = nullptr, *chain_rho = nullptr, *chain_E = nullptr, *chain_mu = nullptr;
     int64_t launches = 0;       // kernels launched through this ctx (bench.py reports it as gpu_launches)
     int64_t scratch_bytes = 0;  // device memory held by this ctx
     // ---- internal levels of the tiled path (spray_set_levels): a level is a context of its own on a grid of the library's
@@ -166,7 +167,7 @@ struct TiledArgs {
 cudaError_t launch_build_tiles(Ctx* c, cudaStream_t st);
 cudaError_t tiled_set_attributes(Ctx* c);      // dynamic shared-memory opt-in of the tiled kernels, on the ctx's device (spray_create)
 cudaError_t sweeps_set_attributes();
-cudaError_t launch_mark_coincident(Ctx* c, cudaStream_t st);   // build.cu
+
 cudaError_t launch_tiled_sweep(Ctx* c, int sweep, const TiledArgs& a, cudaStream_t st);
 // parity exports from the tiled lists: mode 0 = counts, 1 = CSR lists, 2 = digests (tiles.cu)
 cudaError_t launch_tiled_export(Ctx* c, int mode, int symmetric, uint32_t* ocount, const uint64_t* offsets, uint32_t* onbr,

@@ -177,7 +177,6 @@ struct ListArgs {
     uint32_t* tflags;                  // [tile], zeroed before the launch; each half ORs its bits in
     const uint32_t* tiletab;           // [tile][TILES_WORDS]
     uint8_t* fast;                     // [n] sorted order: 1 = served by the tiled kernels
-    const uint8_t* coinc;              // [n] sorted order: 1 = the particle has a twin at distance 0 (k_mark_coincident)
     const double* hglob;
     uint32_t* status;
     float rmax;                        // > 0: largest support radius the unit can meet (level contexts); else 2 max h from hglob
@@ -342,7 +341,6 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
                 if (!(i >= S.r_vstart[q] && i < S.r_vend[q]) && q + 1 < (int)S.nranges && S.r_shift[q + 1][3] == row) ++q;
                 if (i >= S.r_vstart[q] && i < S.r_vend[q]) s_self = S.r_base[q] + (i - S.r_vstart[q]);
             }
-            tbad = A.coinc[i] != 0;                                     // a twin at distance 0: left to the general kernels (A11)
         }
         // an inactive thread sits far away from everything: it never hits
         const float fax = active ? (float)(xa - ox) : -3.0e18f, fay = (float)(ya - oy), faz = (float)(za - oz);
@@ -438,6 +436,7 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
         uint32_t bp0 = bk0, bp1 = bk0 + LIST_BS * BROW, bp2 = bk0 + 2 * LIST_BS * BROW, bp3 = bk0 + 3 * LIST_BS * BROW;
         const uint32_t e0 = bk0 + LIST_BC * BROW, e1 = e0 + LIST_BS * BROW, e2 = e1 + LIST_BS * BROW, e3 = e2 + LIST_BS * BROW;
         float tmin = 3.0e38f;                                           // min |t| over the tested candidates
+        float zb0 = 0.f, zb1 = 0.f, zb2 = 0.f, zb3 = 0.f;               // max -t per bank: T_hi exactly = a candidate at fp32 distance 0
         {
             const f32x2 ax2 = pk2(fax, fax), ay2 = pk2(fay, fay), az2 = pk2(faz, faz);
             const f32x2 nT2 = pk2(-Ta_hi, -Ta_hi);
@@ -454,6 +453,7 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
                 unpk2(fma2(dz1, dz1, fma2(dy1, dy1, fma2(dx1, dx1, nT2))), t2, t3);
                 append_if_neg(t0, bp0, b); append_if_neg(t1, bp1, b); append_if_neg(t2, bp2, b); append_if_neg(t3, bp3, b);
                 tmin = fminf(fminf(tmin, fabsf(t0)), fminf(fabsf(t1), fminf(fabsf(t2), fabsf(t3))));
+                zb0 = fmaxf(zb0, -t0); zb1 = fmaxf(zb1, -t1); zb2 = fmaxf(zb2, -t2); zb3 = fmaxf(zb3, -t3);
             };
             auto block_gen = [&](uint32_t b) {
                 const float4 x = X4[2 * b], y = Y4[2 * b], z = Z4[2 * b], T = T4[2 * b];
@@ -496,12 +496,23 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
             const uint32_t n0 = (bp0 - bk0) / BROW, n1 = (bp1 - (bk0 + LIST_BS * BROW)) / BROW;
             const uint32_t n2 = (bp2 - (bk0 + 2 * LIST_BS * BROW)) / BROW, n3 = (bp3 - (bk0 + 3 * LIST_BS * BROW)) / BROW;
             cnt = n0 | (n1 << 8) | (n2 << 16) | (n3 << 24);
+            // A candidate at fp32 distance 0 (t = -T_hi exactly) is the target itself or a twin -- another particle at the same
+            // place up to fp32 resolution, possibly at fp64 distance 0, where the pair bodies are not defined (A11): the target
+            // is then declined (general kernels).  Only the bank of the target's own slot needs a look into the bucket.
+            const uint32_t kself = sees_self ? (s_self & 3u) : 4u;
+            if (active && ((zb0 == Ta_hi && kself != 0u) || (zb1 == Ta_hi && kself != 1u) || (zb2 == Ta_hi && kself != 2u) ||
+                           (zb3 == Ta_hi && kself != 3u))) coinc = true;
             if (sees_self && !ovf) {
                 const int b = (int)(s_self & 3u);
                 uint16_t* bb = B + (size_t)b * LIST_BS * BL_THREADS + tid;
                 const uint32_t nb = (cnt >> (8 * b)) & 0xFFu, want = s_self >> 3;
-                uint32_t k = 0;
-                while (k < nb && bb[k * BL_THREADS] != want) ++k;
+                uint32_t k = nb;
+                for (uint32_t e = 0; e < nb; ++e) {
+                    const uint32_t blk = bb[e * BL_THREADS];
+                    if (blk == want) { k = e; continue; }
+                    const uint32_t s = (blk << 3) + 4u * (uint32_t)u + (uint32_t)b;
+                    if (X[s] == fax && Y[s] == fay && Z[s] == faz) coinc = true;
+                }
                 if (k < nb) {                                           // the last entry takes its place (order is free)
                     bb[k * BL_THREADS] = bb[(nb - 1) * BL_THREADS];
                     cnt -= 1u << (8 * b);
@@ -830,7 +841,6 @@ cudaError_t launch_build_tiles(Ctx* c, cudaStream_t st) {
     cudaError_t e;
     if ((e = cudaMemsetAsync(t.ctr, 0, sizeof(unsigned long long) * CTR_COUNT, st)) != cudaSuccess) return e;
     if ((e = cudaMemsetAsync(t.fast, 0, (size_t)c->n, st)) != cudaSuccess) return e;
-    if ((e = launch_mark_coincident(c, st)) != cudaSuccess) return e;
     CellTable ct{c->cell_start, c->cell_end, c->is_level ? c->cell_tend : c->cell_end};
     const int blocks = (int)((nb * 32 + 255) / 256);
     const int lvl = c->is_level ? 1 : 0;
@@ -841,7 +851,7 @@ cudaError_t launch_build_tiles(Ctx* c, cudaStream_t st) {
     if ((e = cudaMemsetAsync(t.tflags, 0, sizeof(uint32_t) * (size_t)t.tile_cap, st)) != cudaSuccess) return e;
     if (c->ev[2]) cudaEventRecord(c->ev[2], st);
     ListArgs A{c->pk.p0, c->pk.p1, t.tiles, t.ctr, t.pool, (uint32_t)t.pool_rows, t.winfo, t.lcount, t.tflags, t.tiletab, t.fast,
-               t.coinc, c->hglob, c->dev_status, c->is_level ? c->level_rmax : 0.f};
+               c->hglob, c->dev_status, c->is_level ? c->level_rmax : 0.f};
     k_build_lists<<<t.sms * 2, BL_THREADS, BL_SMEM, st>>>(c->dg, ct, A);
     c->launches += 4;
     t.enabled = true;

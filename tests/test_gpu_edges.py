@@ -203,3 +203,44 @@ def test_every_tile_has_variable_h(name, kmode):
     errs = compare_isolated(g, o)
     assert sp.check() == 0
     print(name, "kmode", kmode, st, {k: f"{v:.1e}" for k, v in errs.items()})
+
+
+def test_particles_far_outside_an_open_box():
+    """spray.h allows positions outside an open (non-periodic) box: they are clamped into the edge cells (A16).  Their distance to
+    the cell block of a tile can then exceed the range the fp32 prefilter of the list builder is proven for: such half tiles must
+    go to the general kernels (a declined unit), and the neighbour sets and sums must stay those of the oracle."""
+    w = W.random_cloud(4000, seed=31, periodic=(0, 0, 0), hvar=1.0, ncell=(6, 6, 6))
+    rng = np.random.default_rng(3)
+    far = rng.choice(w.n, size=40, replace=False)
+    w.x[far[:20]] += 7.3            # far outside the box in +x: clamped into the last column
+    w.z[far[20:]] -= 5.1            # and in -z
+    d = upload(w)
+    sp = make_ctx(w)
+    sp.build_cells(w.grid, w.kernel, d["x"], d["y"], d["z"], d["h"])
+    st = sp.path_stats_full()
+    assert st["tiles"] > 0 and st["n_fast"] < w.n and st["declined"][3] > 0, st
+    for sym, mode in ((False, O.GATHER), (True, O.SYM)):
+        cnt, ds, dx = O.neighbor_digest(w.grid, w.x, w.y, w.z, w.h, mode)
+        assert np.array_equal(u32(sp.neighbor_counts(sym)), cnt)
+        gs, gx = sp.neighbor_digest(sym)
+        assert np.array_equal(gs.cpu().numpy().view(np.uint64), ds) and np.array_equal(gx.cpu().numpy().view(np.uint64), dx)
+    mu_full = O.limiter(w.grid, w.kernel, w.x, w.y, w.z, w.h, w.m, w.rho_nom, w.kappa, w.E, w.c_light)["mu"]
+    errs = compare_isolated(gpu_isolated(sp, d, w, mu_in=mu_full), oracle_isolated(w, mu_full=mu_full))
+    assert sp.check() == 0          # open box: nothing to flag
+    print(st, {k: f"{v:.1e}" for k, v in errs.items()})
+
+
+def test_levels_and_timing_arguments():
+    import paper_2604_20124_b200 as P
+    w = W.make("c1_tiny")
+    d = upload(w)
+    sp = make_ctx(w)
+    with pytest.raises(P.SprayError, match=r"\(-2\)"):          # NOT_BUILT
+        sp.build_timing()
+    with pytest.raises(P.SprayError, match=r"\(-1\)"):          # edges must ascend
+        sp.set_levels(w.grid, [0.3, 0.2])
+    sp.set_levels(w.grid, [2.0 * float(w.h.max()) * 1.001])
+    sp.build_cells(w.grid, w.kernel, d["x"], d["y"], d["z"], d["h"])
+    t = sp.build_timing()
+    assert len(t) == 3 and all(v >= 0.0 for v in t) and t[0] > 0.0
+    assert sp.path_stats_full()["n_fast"] == w.n

@@ -30,7 +30,15 @@ def _both(sp, d, w):
     fy, fmu, fg = sp.hydro_rhs_limiter(d["m"], d["rho_nom"], d["p"], d["cs"], d["vx"], d["vy"], d["vz"], d["alpha"], d["E"], d["kappa"],
                                        beta=w.beta, c_light=w.c_light, want_gradE=True)
     # the (mu, E) records the fused call leaves behind serve a FROZEN apply exactly like those of the UPDATE call
+    # (FROZEN_CHAINED reuses them without the per-call prologue: it must come right after the fused call, and equal FROZEN bit for bit)
+    fc = sp.fld_apply(d["m"], d["rho_nom"], None, d["E"], w.c_light, lmode=2, mu=fmu)
+    fc2 = sp.fld_apply(d["m"], d["rho_nom"], None, d["E"], w.c_light, lmode=2, mu=fmu)      # repeatable: the apply changes no record
     fr = sp.fld_apply(d["m"], d["rho_nom"], None, d["E"], w.c_light, lmode=1, mu=fmu)
+    for k in ("y", "diag", "offd"):
+        assert torch.equal(fc[k], fr[k]) and torch.equal(fc2[k], fr[k]), "chained " + k
+    import paper_2604_20124_b200 as P
+    with pytest.raises(P.SprayError, match=r"\(-1\)"):      # after any other call the chain is broken
+        sp.fld_apply(d["m"], d["rho_nom"], None, d["E"], w.c_light, lmode=2, mu=fmu)
     torch.cuda.synchronize()
     return hy, fl, fy, fmu, fg, fr
 

@@ -428,3 +428,26 @@ def test_golden_lattice_constants_reproduce_by_direct_summation():
     src = open(gen).read()
     assert "import oracle" not in src and "paper_2604_20124_b200" not in src
     assert subprocess.run([sys.executable, gen, "--check"]).returncode == 0
+
+
+def test_T5_cell_list_equals_brute_force_outside_an_open_box():
+    """Positions outside an open box are legal (A16): they are clamped into the edge cells by the cell key (O1), and the
+    definition of the sets stays the all-pairs one.  The cell-list variant must find the neighbours of such particles among
+    the others clamped into the same edge cells."""
+    w = W.random_cloud(3000, seed=31, periodic=(0, 0, 0), hvar=1.0, ncell=(6, 6, 6))
+    rng = np.random.default_rng(3)
+    far = rng.choice(w.n, size=60, replace=False)
+    w.x[far[:30]] += 7.3
+    w.z[far[30:]] -= 5.1
+    # make sure some of them are neighbours of each other
+    w.x[far[1]], w.y[far[1]], w.z[far[1]] = w.x[far[0]] + 0.5 * w.h[0], w.y[far[0]], w.z[far[0]]
+    w.x[far[31]], w.y[far[31]], w.z[far[31]] = w.x[far[30]], w.y[far[30]] + 0.7 * w.h[0], w.z[far[30]]
+    for mode in (O.GATHER, O.SYM):
+        o0, n0 = O.neighbor_lists(w.grid, w.x, w.y, w.z, w.h, mode, use_cells=False)
+        o1, n1 = O.neighbor_lists(w.grid, w.x, w.y, w.z, w.h, mode, use_cells=True)
+        assert np.array_equal(o0, o1) and np.array_equal(n0, n1)
+        cnt = np.diff(o0)
+        assert cnt[far[0]] >= 1 and cnt[far[30]] >= 1
+    d0 = O.density(w.grid, w.kernel, w.x, w.y, w.z, w.h, w.m, use_cells=False)
+    d1 = O.density(w.grid, w.kernel, w.x, w.y, w.z, w.h, w.m, use_cells=True)
+    assert np.array_equal(d0["rho"], d1["rho"])
