@@ -338,7 +338,10 @@ __global__ void __launch_bounds__(TILE_THREADS, MinBlocks<SWEEP, MODE>::v)
 k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
     constexpr int NV = NRecM<SWEEP, MODE>::v;
     extern __shared__ __align__(16) unsigned char smem[];
-    __shared__ TileS S;
+    // this tile's tables / the next tile's, fetched under the pair loop: ranges and target cells, the warps' list rows, descriptor, flags
+    struct TileHdr { uint2 winfo[TILE_WARPS]; TileDesc td; uint32_t flags, pad; };
+    __shared__ __align__(16) TileS Sb[2];
+    __shared__ __align__(16) TileHdr Hb[2];
     double2* F = reinterpret_cast<double2*>(smem);               // F[record * TILE_CMAXP + slot]
     double* Ee = reinterpret_cast<double*>(F + (size_t)NV * TILE_CMAXP);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -358,28 +361,41 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
         if (NRec<SWEEP>::e) Ee[TILE_CMAX + tid] = 0.0;
     }
 
+    auto fetch_tables = [&](uint32_t t, int b) {
+        if (t < ntiles) {
+            if (tid < TILES_WORDS / 4)
+                cp_async16(reinterpret_cast<uint4*>(&Sb[b]) + tid, reinterpret_cast<const uint4*>(A.tiletab + (size_t)t * TILES_WORDS) + tid);
+            else if (tid >= 128 && tid < 128 + TILE_WARPS / 2)
+                cp_async16(reinterpret_cast<uint4*>(Hb[b].winfo) + (tid - 128), reinterpret_cast<const uint4*>(A.winfo + (size_t)t * TILE_WARPS) + (tid - 128));
+            else if (tid >= 160 && tid < 163)
+                cp_async8(reinterpret_cast<uint2*>(&Hb[b].td) + (tid - 160), reinterpret_cast<const uint2*>(A.tiles + t) + (tid - 160));
+            else if (tid == 192)
+                asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" :: "r"((uint32_t)__cvta_generic_to_shared(&Hb[b].flags)), "l"(A.tflags + t) : "memory");
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    fetch_tables(blockIdx.x, 0);
+    int buf = 1;
     for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-        const uint32_t flags = A.tflags[tile];
+        buf ^= 1;
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        __syncthreads();                                         // tables in place; previous tile done with the staged records
+        fetch_tables(tile + gridDim.x, buf ^ 1);
+        const TileS& S = Sb[buf];
+        const uint32_t flags = Hb[buf].flags;
         if (!(flags & TILE_FLAG_OK)) continue;
         const bool tile_uni = (flags & TILE_FLAG_NONUNI) == 0;
         const bool uni = MODE == 1 ? true : (MODE == 2 ? false : tile_uni);
         if (MODE != 0 && tile_uni != (MODE == 1)) continue;
         const bool half_ok = ((flags >> (warp / (TILE_WARPS / 2))) & 1u) != 0;   // this warp's half of the tile has lists
-        const TileDesc td = A.tiles[tile];
+        const TileDesc td = Hb[buf].td;
         // first three list rows: in flight while the records are staged
-        uint2 wi = A.winfo[(size_t)tile * TILE_WARPS + warp];
+        uint2 wi = Hb[buf].winfo[warp];
         if (!half_ok) wi.y = 0u;
         const uint2* lp = A.pool + (size_t)wi.x * 32 + lane;
         const uint2 l0 = wi.y ? __ldcs(lp) : make_uint2(0u, 0u);
         const uint2 l1 = wi.y > 4 ? __ldcs(lp + 32) : make_uint2(0u, 0u);
         const uint2 l2 = wi.y > 8 ? __ldcs(lp + 64) : make_uint2(0u, 0u);
-        __syncthreads();                                         // previous tile done with the staged records
-        {   // tile tables as the list builder left them
-            const uint32_t* src = A.tiletab + (size_t)tile * TILES_WORDS;
-            uint32_t* dst = reinterpret_cast<uint32_t*>(&S);
-            for (int w = tid; w < TILES_WORDS; w += TILE_THREADS) dst[w] = src[w];
-        }
-        __syncthreads();
         // ---- this thread's target.  Except in the hydro kernel (register pressure: measured slower) its loads go out before
         //      the staging traffic, so they are back when the pair loop starts.
         constexpr bool EARLY_TARGET = !HYD;
@@ -444,7 +460,6 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
         if (!EARLY_TARGET) load_target();
         asm volatile("cp.async.wait_group 0;" ::: "memory");
         __syncthreads();
-
         Acc acc{};
         if (uni) pair_loop<SWEEP, KERNEL, true>(F, Ee, lp, wi.y, l0, l1, l2, T, A.beta, sym, acc);
         else pair_loop<SWEEP, KERNEL, false>(F, Ee, lp, wi.y, l0, l1, l2, T, A.beta, sym, acc);

@@ -76,7 +76,7 @@ struct TileS {
     uint32_t ncells;
 };
 
-static_assert(sizeof(TileS) % 4 == 0, "TileS is copied word by word");
+static_assert(sizeof(TileS) % 16 == 0, "TileS is copied in 16-byte pieces");
 constexpr int TILES_WORDS = (int)(sizeof(TileS) / 4);
 
 __device__ __forceinline__ uint32_t cell_id(const DevGrid& g, int cx, int cy, int cz) {
