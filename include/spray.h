@@ -137,6 +137,30 @@ int spray_build_timing(spray_ctx* ctx, double* ms_cells, double* ms_tiles, doubl
 int spray_build_cells(spray_ctx* ctx, const spray_grid_t* grid, spray_kernel_t kernel, int64_t n,
                       const double* x, const double* y, const double* z, const double* h, void* stream);
 
+/* (a1)-(a3) WITHOUT A CONTEXT AND WITHOUT ANY ALLOCATION: cell key, stable sort of (key, caller index) and the cell table of
+ * P:L438, exactly as spray_build_cells computes them (same kernels and pass order: results are bit-identical to
+ * spray_build_cells + spray_get_cell_table), for callers that cannot call cudaMalloc -- code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid it.  The call makes no cudaMalloc / cudaFree and uses no allocating library routine:
+ * the sort's scratch (two key/index buffers, radix histograms, a status word) is a file-scope device array of
+ * SPRAY_STATIC_SCRATCH_BYTES that every GPU loading the library holds until the process exits.
+ *   grid: host (h_max is not used);  x, y, z: device, [n], read only;  outputs, all device, caller-allocated, must not alias
+ *   the inputs: sorted_key[n], perm[n] (perm[i] = caller index of the particle in sorted slot i), cell_start[ncell],
+ *   cell_end[ncell];  dev_status: device, one word, nullable: receives the SPRAY_DEV_* bits of this call (OUTSIDE_BOX).
+ *   Works on the CURRENT device (cudaGetDevice), to which stream and pointers must belong.  Only enqueues.
+ * Limits: n <= SPRAY_STATIC_NMAX (SPRAY_ERR_CAPACITY beyond, nothing is launched), prod ncell_d <= SPRAY_STATIC_NCELL_MAX
+ * (SPRAY_ERR_GRID).  n = 0 is valid (empty cell table).  SPRAY_ERR_INVALID_ARG for NULL pointers / n < 0.
+ * spray_static_last_error() returns the calling thread's description of its last failure of this call.
+ * SHARED STATE: every call on a device uses the same array, which keeps the previous call's contents (the call clears what
+ * must start at zero).  Two calls that overlap on the GPU -- different streams, or different host threads -- RACE on it
+ * and give wrong results: serialise them (one stream, or events). */
+#define SPRAY_STATIC_NMAX 262144
+#define SPRAY_STATIC_NCELL_MAX 16777216
+#define SPRAY_STATIC_SCRATCH_BYTES (4 * 1024 * 1024 + 128 * 1024)
+int spray_cell_list_static(const spray_grid_t* grid, int64_t n, const double* x, const double* y, const double* z,
+                           uint32_t* sorted_key, uint32_t* perm, uint32_t* cell_start, uint32_t* cell_end,
+                           uint32_t* dev_status, void* stream);
+const char* spray_static_last_error(void);
+
 /* (a5) density by summation, eq. (35):  rho_a = sum_{b in N_gather(a)} m_b W(r_ab; h_a), self included (A11).
  * nnbr (nullable, u32[n]) = |N_gather(a)| - 1. */
 int spray_density(spray_ctx* ctx, const double* m, double* rho, uint32_t* nnbr, void* stream);

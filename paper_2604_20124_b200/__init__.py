@@ -12,7 +12,7 @@ import ctypes as C
 from pathlib import Path
 
 __all__ = ["load", "Spray", "SprayError", "KERNEL_CUBIC_SPLINE", "KERNEL_WENDLAND_C2", "FLD_SYMMETRIC", "FLD_GATHER",
-           "FLD_UPDATE_LIMITER", "FLD_FROZEN", "FLD_FROZEN_CHAINED", "EXPORTS"]
+           "FLD_UPDATE_LIMITER", "FLD_FROZEN", "FLD_FROZEN_CHAINED", "EXPORTS", "cell_list_static", "STATIC_NMAX", "STATIC_NCELL_MAX"]
 
 _LIBPATH = Path(__file__).resolve().parent / "libspray_b200.so"
 
@@ -25,7 +25,8 @@ DEV_H_EXCEEDS_HMAX, DEV_OUTSIDE_BOX, DEV_LIST_OVERFLOW = 1, 2, 4
 # every symbol include/spray.h declares
 EXPORTS = ["spray_version", "spray_create", "spray_destroy", "spray_last_error", "spray_check", "spray_launch_count", "spray_set_path", "spray_set_levels", "spray_path_stats", "spray_build_timing",
            "spray_build_cells", "spray_density", "spray_hydro_rhs", "spray_hydro_rhs_limiter", "spray_fld_apply", "spray_get_cell_table",
-           "spray_neighbor_counts", "spray_neighbor_lists", "spray_neighbor_digest", "spray_rad_jacobi", "spray_conduction", "spray_kgc_continuity", "spray_ray_deposit", "spray_conduction_implicit", "spray_fp64_peak_probe"]
+           "spray_neighbor_counts", "spray_neighbor_lists", "spray_neighbor_digest", "spray_rad_jacobi", "spray_conduction", "spray_kgc_continuity", "spray_ray_deposit", "spray_conduction_implicit", "spray_fp64_peak_probe",
+           "spray_cell_list_static", "spray_static_last_error"]
 
 
 class SprayError(RuntimeError):
@@ -78,8 +79,11 @@ def load():
     lib.spray_neighbor_lists.argtypes = [vp, i32, vp, vp, vp]
     lib.spray_neighbor_digest.argtypes = [vp, i32, vp, vp, vp]
     lib.spray_fp64_peak_probe.argtypes = [i32, i32, i32, i64, vp, vp]
+    lib.spray_cell_list_static.argtypes = [C.POINTER(Grid), i64, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.spray_static_last_error.argtypes = []
+    lib.spray_static_last_error.restype = C.c_char_p
     for name in EXPORTS:
-        if name not in ("spray_version", "spray_last_error"):
+        if name not in ("spray_version", "spray_last_error", "spray_static_last_error"):
             getattr(lib, name).restype = C.c_int
     lib.spray_launch_count.restype = C.c_int64
     _lib = lib
@@ -102,6 +106,34 @@ def _ptr(t, dtype=None, n=None):
 def _stream():
     import torch
     return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+STATIC_NMAX, STATIC_NCELL_MAX = 262144, 16777216
+
+
+def cell_list_static(grid, x, y, z, sorted_key=None, perm=None, cell_start=None, cell_end=None, dev_status=None):
+    """spray_cell_list_static: cell key, stable sort and cell table without a context and without any allocation inside
+    the library (its scratch is a static device array; calls that overlap on the GPU race on it).  Works on the current
+    device.  Output tensors not supplied are allocated HERE with torch (a caller that must not allocate passes them)."""
+    import torch
+    lib = load()
+    n = int(x.numel())
+    ncell = int(grid.ncell[0]) * int(grid.ncell[1]) * int(grid.ncell[2])
+    i32 = torch.int32   # u32 payloads viewed as int32 tensors
+    dev = x.device
+    sorted_key = torch.empty(n, dtype=i32, device=dev) if sorted_key is None else sorted_key
+    perm = torch.empty(n, dtype=i32, device=dev) if perm is None else perm
+    cell_start = torch.empty(ncell, dtype=i32, device=dev) if cell_start is None else cell_start
+    cell_end = torch.empty(ncell, dtype=i32, device=dev) if cell_end is None else cell_end
+    g = Grid((C.c_double * 3)(*grid.lo), (C.c_double * 3)(*grid.hi), (C.c_int32 * 3)(*grid.ncell),
+             (C.c_int32 * 3)(*grid.periodic), float(grid.h_max))
+    f64 = torch.float64
+    rc = lib.spray_cell_list_static(C.byref(g), n, _ptr(x, f64, n), _ptr(y, f64, n), _ptr(z, f64, n), _ptr(sorted_key, i32, n),
+                                    _ptr(perm, i32, n), _ptr(cell_start, i32, ncell), _ptr(cell_end, i32, ncell),
+                                    _ptr(dev_status, i32, 1), _stream())
+    if rc != 0:
+        raise SprayError(f"spray_cell_list_static failed ({rc}): {lib.spray_static_last_error().decode()}")
+    return dict(sorted_key=sorted_key, perm=perm, cell_start=cell_start, cell_end=cell_end)
 
 
 class Spray:

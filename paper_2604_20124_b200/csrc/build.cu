@@ -4,6 +4,9 @@
 // can be identified directly".
 #include "spray_internal.h"
 
+#include <cstdio>
+#include <mutex>
+
 namespace spray {
 
 // ------------------------------------------------------------------------------------------- K1: cell key
@@ -505,3 +508,124 @@ cudaError_t launch_cell_hmax(Ctx* c, cudaStream_t st) {
 }
 
 }  // namespace spray
+
+// ------------------------------------------------------------------------------------------- spray_cell_list_static
+// Rows a1-a3 (cell key, stable radix sort, cell table) for callers that cannot allocate: no context, no
+// cudaMalloc / cudaFree / allocating library routine.  The sort's scratch -- two (key, index) buffers and the radix
+// histograms -- lives in the file-scope device array below, which every GPU that loads the library holds until the process
+// exits.  Same kernels, launch order and pass count as spray_build_cells, so the results are bit-identical to
+// spray_build_cells + spray_get_cell_table.  The last radix pass scatters straight into the caller's sorted_key / perm.
+namespace spray {
+constexpr int64_t STATIC_NMAX = SPRAY_STATIC_NMAX;
+constexpr int64_t STATIC_HIST = 256 * (STATIC_NMAX / RS_TILE + 1) + SC_TILE;   // [digit][tile] counters + block totals of their scan
+constexpr int64_t STATIC_OFF_KEY0 = 0, STATIC_OFF_IDX0 = STATIC_NMAX, STATIC_OFF_KEY1 = 2 * STATIC_NMAX, STATIC_OFF_IDX1 = 3 * STATIC_NMAX;
+constexpr int64_t STATIC_OFF_HIST = 4 * STATIC_NMAX, STATIC_OFF_STATUS = STATIC_OFF_HIST + STATIC_HIST;
+constexpr int64_t STATIC_WORDS = STATIC_OFF_STATUS + 64;
+static_assert(STATIC_NMAX % RS_TILE == 0, "whole sort tiles");
+static_assert(STATIC_WORDS * 4 <= (int64_t)SPRAY_STATIC_SCRATCH_BYTES, "spray.h states the size of the static scratch");
+
+// In host code this name is a host-side stand-in, not a device address: kernels get the pointer cudaGetSymbolAddress returns.
+static __device__ __align__(256) uint32_t g_static_scratch[STATIC_WORDS];
+
+constexpr int STATIC_MAX_DEVICES = 64;
+static uint32_t* g_static_ptr[STATIC_MAX_DEVICES] = {};     // per device, set once with that device current
+static std::mutex g_static_mu;
+static thread_local char g_static_err[256] = "";
+
+static int static_fail(int code, const char* what, cudaError_t e = cudaSuccess) {
+    if (e != cudaSuccess) snprintf(g_static_err, sizeof g_static_err, "%s: %s", what, cudaGetErrorString(e));
+    else snprintf(g_static_err, sizeof g_static_err, "%s", what);
+    return code;
+}
+}  // namespace spray
+
+extern "C" const char* spray_static_last_error(void) { return spray::g_static_err; }
+
+extern "C" int spray_cell_list_static(const spray_grid_t* grid, int64_t n, const double* x, const double* y, const double* z,
+                                      uint32_t* sorted_key, uint32_t* perm, uint32_t* cell_start, uint32_t* cell_end,
+                                      uint32_t* dev_status, void* stream) {
+    using namespace spray;
+    g_static_err[0] = 0;
+    if (!grid || n < 0 || !cell_start || !cell_end || (n > 0 && (!x || !y || !z || !sorted_key || !perm)))
+        return static_fail(SPRAY_ERR_INVALID_ARG, "spray_cell_list_static: NULL argument or n < 0");
+    if (n > STATIC_NMAX) {
+        snprintf(g_static_err, sizeof g_static_err, "spray_cell_list_static: n = %lld exceeds SPRAY_STATIC_NMAX = %lld (the static scratch "
+                 "holds no more; use spray_create + spray_build_cells)", (long long)n, (long long)STATIC_NMAX);
+        return SPRAY_ERR_CAPACITY;
+    }
+    DevGrid dg;
+    int64_t ncell = 1;
+    for (int d = 0; d < 3; ++d) {
+        if (grid->ncell[d] < 1) return static_fail(SPRAY_ERR_GRID, "spray_cell_list_static: grid: ncell_d < 1");
+        if (!(grid->hi[d] > grid->lo[d])) return static_fail(SPRAY_ERR_GRID, "spray_cell_list_static: grid: hi <= lo");
+        ncell *= grid->ncell[d];
+        if (ncell > (int64_t)SPRAY_STATIC_NCELL_MAX) return static_fail(SPRAY_ERR_GRID, "spray_cell_list_static: grid: prod ncell_d > SPRAY_STATIC_NCELL_MAX");
+        dg.lo[d] = grid->lo[d];
+        dg.L[d] = grid->hi[d] - grid->lo[d];
+        dg.halfL[d] = 0.5 * dg.L[d];
+        dg.edge[d] = dg.L[d] / (double)grid->ncell[d];
+        dg.inv[d] = (double)grid->ncell[d] / dg.L[d];
+        dg.nc[d] = grid->ncell[d];
+        dg.per[d] = grid->periodic[d] != 0;
+    }
+    // the scratch's device address: once per device, with that device current (the caller's current device is the one whose
+    // stream and pointers it passes)
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return static_fail(SPRAY_ERR_CUDA, "spray_cell_list_static: cudaGetDevice", e);
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) return static_fail(SPRAY_ERR_INVALID_ARG, "spray_cell_list_static: device index out of range");
+    uint32_t* S = nullptr;
+    {
+        std::lock_guard<std::mutex> lk(g_static_mu);
+        if (!g_static_ptr[dev]) {
+            void* p = nullptr;
+            e = cudaGetSymbolAddress(&p, g_static_scratch);
+            if (e != cudaSuccess || !p) return static_fail(SPRAY_ERR_CUDA, "spray_cell_list_static: cudaGetSymbolAddress", e);
+            g_static_ptr[dev] = static_cast<uint32_t*>(p);
+        }
+        S = g_static_ptr[dev];
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    uint32_t* status = S + STATIC_OFF_STATUS;
+    uint32_t* hist = S + STATIC_OFF_HIST;
+    // the array keeps the last call's contents: the status word must start at zero (the histograms and block totals are
+    // overwritten in full by every pass, the key / index buffers by the key kernel and the scatters)
+    e = cudaMemsetAsync(status, 0, sizeof(uint32_t), st);
+    if (e != cudaSuccess) return static_fail(SPRAY_ERR_CUDA, "spray_cell_list_static: clearing the status word", e);
+    if (n > 0) {
+        int bits = 0;
+        while (((int64_t)1 << bits) < ncell) ++bits;
+        const int passes = (bits + 7) / 8;                              // as launch_radix_sort; 0 when the grid has one cell
+        uint32_t* kbuf[2] = {S + STATIC_OFF_KEY0, S + STATIC_OFF_KEY1};
+        uint32_t* ibuf[2] = {S + STATIC_OFF_IDX0, S + STATIC_OFF_IDX1};
+        // with no pass to run the keys (all 0) and the identity permutation are the result
+        uint32_t* k0 = passes ? kbuf[0] : sorted_key;
+        uint32_t* i0 = passes ? ibuf[0] : perm;
+        k_cell_key<<<cdiv64(n, 256), 256, 0, st>>>(dg, n, x, y, z, k0, i0, status, nullptr, nullptr, 0.0, 0.0);
+        const int nblk = cdiv64(n, RS_TILE);
+        int cur = 0;
+        for (int p = 0; p < passes; ++p) {
+            const int shift = 8 * p;
+            const bool last = p == passes - 1;
+            uint32_t* kd = last ? sorted_key : kbuf[cur ^ 1];
+            uint32_t* id = last ? perm : ibuf[cur ^ 1];
+            k_rs_hist<<<nblk, RS_THREADS, 0, st>>>(kbuf[cur], n, shift, hist, nblk);
+            const int64_t total = (int64_t)256 * nblk;
+            const int nb = cdiv64(total, SC_TILE);
+            uint32_t* btot = hist + total;
+            k_scan_blocks<<<nb, SC_THREADS, 0, st>>>(hist, total, btot);
+            k_scan_totals<<<1, SC_THREADS, 0, st>>>(btot, nb);
+            k_scan_add<<<nb, SC_THREADS, 0, st>>>(hist, total, btot);
+            k_rs_scatter<<<nblk, RS_THREADS, 0, st>>>(kbuf[cur], ibuf[cur], kd, id, n, shift, hist, nblk);
+            cur ^= 1;
+        }
+    }
+    k_cell_table<<<cdiv64(ncell + 1, 256), 256, 0, st>>>(sorted_key, (uint32_t)n, (uint32_t)ncell, cell_start, cell_end);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return static_fail(SPRAY_ERR_CUDA, "spray_cell_list_static: kernel launch", e);
+    if (dev_status) {
+        e = cudaMemcpyAsync(dev_status, status, sizeof(uint32_t), cudaMemcpyDeviceToDevice, st);
+        if (e != cudaSuccess) return static_fail(SPRAY_ERR_CUDA, "spray_cell_list_static: status copy", e);
+    }
+    return SPRAY_OK;
+}
