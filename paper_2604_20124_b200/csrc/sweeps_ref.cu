@@ -60,7 +60,6 @@ __device__ __forceinline__ V warp_add(V v) {
 }
 template <int SWEEP, int KERNEL, bool WARP>
 __device__ __forceinline__ void ref_particle(const DevGrid& g, int64_t n, const CellTabs& T, const SweepArgs& A, int64_t i) {
-    const uint32_t j_lo = WARP ? (threadIdx.x & 31u) : 0u, j_st = WARP ? 32u : 1u;
     if (A.skip && A.skip[i]) return;        // served by the tiled kernels
     const double xa = A.x[i], ya = A.y[i], za = A.z[i], ha = A.h[i];
     const uint32_t ia = T.perm[i];
@@ -105,115 +104,219 @@ __device__ __forceinline__ void ref_particle(const DevGrid& g, int64_t n, const 
     uint64_t lbase = 0;
     if (SWEEP == SW_LIST) lbase = A.offsets[ia];
 
-    for (int kz = 0; kz < sz.cnt; ++kz) {
-        const int czz = g.per[2] ? wrap_cell(sz.start + kz, g.nc[2]) : sz.start + kz;
-        const double gz2 = cell_gap2(sz.start + kz - cz, fcz, fullz, ez);
-        if (gz2 > reach2) continue;
-        for (int ky = 0; ky < sy.cnt; ++ky) {
-            const int cyy = g.per[1] ? wrap_cell(sy.start + ky, g.nc[1]) : sy.start + ky;
-            const double gyz2 = gz2 + cell_gap2(sy.start + ky - cy, fcy, fully, ey);
-            if (gyz2 > reach2) continue;
-            for (int kx = 0; kx < sx.cnt; ++kx) {
-                const int cxx = g.per[0] ? wrap_cell(sx.start + kx, g.nc[0]) : sx.start + kx;
-                const double gap2 = gyz2 + cell_gap2(sx.start + kx - cx, fcx, fullx, ex);
-                if (gap2 > reach2) continue;
-                const uint32_t c = (uint32_t)((czz * g.nc[1] + cyy) * g.nc[0] + cxx);
-                if (SWEEP == SW_HSEARCH && !(__ldg(T.cell_hmin + c) < ha)) continue;   // nobody in the cell has a smaller h
-                if (sym) {
-                    // symmetric sets: b in N_sym(a) needs r < 2 max(h_a, h_b) <= 2 max(h_a, max h of b's cell), and r >= the gap
-                    const double rc = 2.0 * fmax(ha, __ldg(T.cell_hmax + c));
-                    if (gap2 > (rc * rc) * (1.0 + 1e-9)) continue;
-                }
-                const uint32_t jb = __ldg(T.cell_start + c), je = __ldg(T.cell_end + c);
-                for (uint32_t j = jb + j_lo; j < je; j += j_st) {
-                    const double dx = min_image(__dsub_rn(xa, __ldg(A.x + j)), g.per[0], g.L[0], g.halfL[0]);
-                    const double dy = min_image(__dsub_rn(ya, __ldg(A.y + j)), g.per[1], g.L[1], g.halfL[1]);
-                    const double dz = min_image(__dsub_rn(za, __ldg(A.z + j)), g.per[2], g.L[2], g.halfL[2]);
-                    const double r2 = r2_exact(dx, dy, dz);
-                    const double hb = __ldg(A.h + j);
-                    const bool self = (j == (uint32_t)i);
-                    const bool in_g = r2 < sup_a;
-                    const bool in_s = !self && (r2 < support2(fmax(ha, hb)));
-                    const bool in_set = sym ? in_s : (in_g && !self);
+    // One candidate j: geometry and set membership (contract expressions), then the pair term of the sweep.
+    struct Pair { double dx, dy, dz, r2, hb; bool self, in_g, in_s, in_set; };
+    auto geometry = [&](uint32_t j) {
+        Pair P;
+        P.dx = min_image(__dsub_rn(xa, __ldg(A.x + j)), g.per[0], g.L[0], g.halfL[0]);
+        P.dy = min_image(__dsub_rn(ya, __ldg(A.y + j)), g.per[1], g.L[1], g.halfL[1]);
+        P.dz = min_image(__dsub_rn(za, __ldg(A.z + j)), g.per[2], g.L[2], g.halfL[2]);
+        P.r2 = r2_exact(P.dx, P.dy, P.dz);
+        P.hb = __ldg(A.h + j);
+        P.self = (j == (uint32_t)i);
+        P.in_g = P.r2 < sup_a;
+        P.in_s = !P.self && (P.r2 < support2(fmax(ha, P.hb)));
+        P.in_set = sym ? P.in_s : (P.in_g && !P.self);
+        return P;
+    };
+    // does candidate j contribute anything to this sweep?  (the conditions of the pair terms below)
+    auto contributes = [&](const Pair& P) {
+        if (SWEEP == SW_DENSITY) return P.in_g;
+        if (SWEEP == SW_HYDRO) return P.in_s && P.r2 > 0.0;
+        if (SWEEP == SW_LIMITER || SWEEP == SW_GRADN || SWEEP == SW_KGC) return P.in_g && !P.self && P.r2 > 0.0;
+        if (SWEEP == SW_APPLY) return P.in_set && P.r2 > 0.0;
+        return true;
+    };
+    auto pair_term = [&](uint32_t j, const Pair& P) {
+        const double dx = P.dx, dy = P.dy, dz = P.dz, r2 = P.r2, hb = P.hb;
+        const bool self = P.self, in_g = P.in_g, in_s = P.in_s, in_set = P.in_set;
+        (void)in_s; (void)in_set; (void)self; (void)hb; (void)dx; (void)dy; (void)dz;
 
-                    if (SWEEP == SW_DENSITY) {
-                        // eq. (35), self term included (A11)
-                        if (in_g) {
-                            double q = sqrt(r2) * hinv;
-                            acc0 += A.m[j] * shape_w<KERNEL>(q);
-                            cnt += self ? 0u : 1u;
-                        }
-                    } else if (SWEEP == SW_HSEARCH) {
-                        // make neighbours mutual -- raise the search length of every a that I see but that may not see me
-                        if (in_g && !self && hb < ha)
-                            atomicMax((unsigned long long*)(A.o0 + j), (unsigned long long)__double_as_longlong(ha));
-                    } else if (SWEEP == SW_COUNT) {
-                        cnt += in_set ? 1u : 0u;
-                    } else if (SWEEP == SW_LIST) {
-                        if (in_set) A.onbr[lbase + cnt++] = T.perm[j];
-                    } else if (SWEEP == SW_DIGEST) {
-                        if (in_set) { uint64_t hsh = mix64((uint64_t)T.perm[j]); dsum += hsh; dxr ^= hsh; }
-                    } else if (SWEEP == SW_HYDRO) {
-                        if (in_s && r2 > 0.0) {
-                            const double r = sqrt(r2), rinv = 1.0 / r;
-                            const double hbinv = 1.0 / hb;
-                            const double Fa = Fn * shape_f<KERNEL>(r * hinv);
-                            const double Fb = sigma<KERNEL>() * (hbinv * hbinv) * (hbinv * hbinv) * shape_f<KERNEL>(r * hbinv);
-                            const double mb = A.m[j], rho_b = A.rho[j], p_b = A.p[j];
-                            const double w = ((vxa - A.vx[j]) * dx + (vya - A.vy[j]) * dy + (vza - A.vz[j]) * dz) * rinv;
-                            // eq. (11) P:L98 with the sign of eq. (5) (A3)
-                            double coef = -(mb / (rho_a * rho_b)) * (p_a * Fa + p_b * Fb);
-                            if (w < 0.0) {   // eqs. (41)-(43) P:L236-L242 (A6, A7, A8)
-                                const double aw = -w;
-                                const double vsa = ac_a + A.beta * aw;
-                                const double vsb = A.alpha[j] * A.cs[j] + A.beta * aw;
-                                coef += 0.5 * mb * (vsa * Fa / rho_a + vsb * Fb / rho_b) * w;
-                                acc4 += 0.5 * mb * vsa * (w * w) * Fa;
-                            }
-                            const double cr = coef * rinv;
-                            acc0 += cr * dx; acc1 += cr * dy; acc2 += cr * dz;
-                            acc3 += (mb / rho_b) * w * Fa;      // eq. (37)
-                        }
-                    } else if (SWEEP == SW_LIMITER || SWEEP == SW_GRADN) {
-                        if (in_g && !self && r2 > 0.0) {
-                            // eq. (9) phi = 1 with f = E (A19)
-                            const double r = sqrt(r2);
-                            const double cc = (A.m[j] / A.rho[j]) * (A.E[j] - E_a) * (Fn * shape_f<KERNEL>(r * hinv)) / r;
-                            acc0 += cc * dx; acc1 += cc * dy; acc2 += cc * dz;
-                        }
-                    } else if (SWEEP == SW_KGC) {
-                        if (in_g && !self && r2 > 0.0) {
-                            // eqs. (37), (39), (40) P:L213-L228: moment sums over N_gather(a), h_a only
-                            const double r = sqrt(r2);
-                            const double cc = (A.m[j] / A.rho[j]) * (Fn * shape_f<KERNEL>(r * hinv)) / r;
-                            const double cx = cc * dx, cy = cc * dy, cz = cc * dz;
-                            const double dvx = vxa - A.vx[j], dvy = vya - A.vy[j], dvz = vza - A.vz[j];
-                            km[0] += cx * dx; km[1] += cx * dy; km[2] += cx * dz; km[3] += cy * dy; km[4] += cy * dz; km[5] += cz * dz;
-                            kq[0] += dvx * cx; kq[1] += dvx * cy; kq[2] += dvx * cz;
-                            kq[3] += dvy * cx; kq[4] += dvy * cy; kq[5] += dvy * cz;
-                            kq[6] += dvz * cx; kq[7] += dvz * cy; kq[8] += dvz * cz;
-                        }
-                    } else if (SWEEP == SW_APPLY) {
-                        if (in_set && r2 > 0.0) {
-                            // eq. (47) first term P:L270 on eq. (16); Fbar as P:L134 (A17)
-                            const double r = sqrt(r2);
-                            double Fbar = Fn * shape_f<KERNEL>(r * hinv);
-                            if (sym) {
-                                const double hbinv = 1.0 / hb;
-                                Fbar = 0.5 * (Fbar + sigma<KERNEL>() * (hbinv * hbinv) * (hbinv * hbinv) * shape_f<KERNEL>(r * hbinv));
-                            }
-                            const double mu_b = A.mu[j], E_b = A.E[j];
-                            const double cab = (A.m[j] / A.rho[j]) * (4.0 * mu_a * mu_b / (mu_a + mu_b)) * (Fbar / r);
-                            acc0 += cab * (E_a - E_b);
-                            acc1 += cab;
-                            acc2 -= cab * E_b;
-                        }
+            if (SWEEP == SW_DENSITY) {
+                // eq. (35), self term included (A11)
+                if (in_g) {
+                    double q = sqrt(r2) * hinv;
+                    acc0 += A.m[j] * shape_w<KERNEL>(q);
+                    cnt += self ? 0u : 1u;
+                }
+            } else if (SWEEP == SW_HSEARCH) {
+                // make neighbours mutual -- raise the search length of every a that I see but that may not see me
+                if (in_g && !self && hb < ha)
+                    atomicMax((unsigned long long*)(A.o0 + j), (unsigned long long)__double_as_longlong(ha));
+            } else if (SWEEP == SW_COUNT) {
+                cnt += in_set ? 1u : 0u;
+            } else if (SWEEP == SW_LIST) {
+                if (in_set) A.onbr[lbase + cnt++] = T.perm[j];
+            } else if (SWEEP == SW_DIGEST) {
+                if (in_set) { uint64_t hsh = mix64((uint64_t)T.perm[j]); dsum += hsh; dxr ^= hsh; }
+            } else if (SWEEP == SW_HYDRO) {
+                if (in_s && r2 > 0.0) {
+                    const double r = sqrt(r2), rinv = 1.0 / r;
+                    const double hbinv = 1.0 / hb;
+                    const double Fa = Fn * shape_f<KERNEL>(r * hinv);
+                    const double Fb = sigma<KERNEL>() * (hbinv * hbinv) * (hbinv * hbinv) * shape_f<KERNEL>(r * hbinv);
+                    const double mb = A.m[j], rho_b = A.rho[j], p_b = A.p[j];
+                    const double w = ((vxa - A.vx[j]) * dx + (vya - A.vy[j]) * dy + (vza - A.vz[j]) * dz) * rinv;
+                    // eq. (11) P:L98 with the sign of eq. (5) (A3)
+                    double coef = -(mb / (rho_a * rho_b)) * (p_a * Fa + p_b * Fb);
+                    if (w < 0.0) {   // eqs. (41)-(43) P:L236-L242 (A6, A7, A8)
+                        const double aw = -w;
+                        const double vsa = ac_a + A.beta * aw;
+                        const double vsb = A.alpha[j] * A.cs[j] + A.beta * aw;
+                        coef += 0.5 * mb * (vsa * Fa / rho_a + vsb * Fb / rho_b) * w;
+                        acc4 += 0.5 * mb * vsa * (w * w) * Fa;
                     }
+                    const double cr = coef * rinv;
+                    acc0 += cr * dx; acc1 += cr * dy; acc2 += cr * dz;
+                    acc3 += (mb / rho_b) * w * Fa;      // eq. (37)
+                }
+            } else if (SWEEP == SW_LIMITER || SWEEP == SW_GRADN) {
+                if (in_g && !self && r2 > 0.0) {
+                    // eq. (9) phi = 1 with f = E (A19)
+                    const double r = sqrt(r2);
+                    const double cc = (A.m[j] / A.rho[j]) * (A.E[j] - E_a) * (Fn * shape_f<KERNEL>(r * hinv)) / r;
+                    acc0 += cc * dx; acc1 += cc * dy; acc2 += cc * dz;
+                }
+            } else if (SWEEP == SW_KGC) {
+                if (in_g && !self && r2 > 0.0) {
+                    // eqs. (37), (39), (40) P:L213-L228: moment sums over N_gather(a), h_a only
+                    const double r = sqrt(r2);
+                    const double cc = (A.m[j] / A.rho[j]) * (Fn * shape_f<KERNEL>(r * hinv)) / r;
+                    const double cx = cc * dx, cy = cc * dy, cz = cc * dz;
+                    const double dvx = vxa - A.vx[j], dvy = vya - A.vy[j], dvz = vza - A.vz[j];
+                    km[0] += cx * dx; km[1] += cx * dy; km[2] += cx * dz; km[3] += cy * dy; km[4] += cy * dz; km[5] += cz * dz;
+                    kq[0] += dvx * cx; kq[1] += dvx * cy; kq[2] += dvx * cz;
+                    kq[3] += dvy * cx; kq[4] += dvy * cy; kq[5] += dvy * cz;
+                    kq[6] += dvz * cx; kq[7] += dvz * cy; kq[8] += dvz * cz;
+                }
+            } else if (SWEEP == SW_APPLY) {
+                if (in_set && r2 > 0.0) {
+                    // eq. (47) first term P:L270 on eq. (16); Fbar as P:L134 (A17)
+                    const double r = sqrt(r2);
+                    double Fbar = Fn * shape_f<KERNEL>(r * hinv);
+                    if (sym) {
+                        const double hbinv = 1.0 / hb;
+                        Fbar = 0.5 * (Fbar + sigma<KERNEL>() * (hbinv * hbinv) * (hbinv * hbinv) * shape_f<KERNEL>(r * hbinv));
+                    }
+                    const double mu_b = A.mu[j], E_b = A.E[j];
+                    const double cab = (A.m[j] / A.rho[j]) * (4.0 * mu_a * mu_b / (mu_a + mu_b)) * (Fbar / r);
+                    acc0 += cab * (E_a - E_b);
+                    acc1 += cab;
+                    acc2 -= cab * E_b;
+                }
+            }
+    };
+    // One warp per particle: the lanes test 32 candidates at a time and QUEUE the contributing ones (ballot compaction into
+    // a per-warp shared-memory queue, in candidate order: deterministic); a pair term is evaluated only when 32 are waiting,
+    // so its long fp64 body (divisions, square roots) runs with every lane busy instead of the few per cent that hit.
+    constexpr bool QUEUED = WARP && (SWEEP == SW_DENSITY || SWEEP == SW_HYDRO || SWEEP == SW_LIMITER || SWEEP == SW_GRADN ||
+                                     SWEEP == SW_KGC || SWEEP == SW_APPLY);
+    __shared__ uint32_t s_queue[QUEUED ? 4 : 1][64];
+    uint32_t* queue = s_queue[QUEUED ? (threadIdx.x >> 5) : 0];
+    uint32_t qn = 0;
+    const uint32_t lane = threadIdx.x & 31u;
+    auto drain = [&](uint32_t count) {                                  // the first `count` (<= 32) queued candidates
+        __syncwarp();
+        const uint32_t j = queue[lane < count ? lane : 0u];
+        const uint32_t moved = queue[32u + lane];
+        if (lane < count) pair_term(j, geometry(j));
+        __syncwarp();
+        queue[lane] = moved;
+        __syncwarp();
+    };
+
+    // does cell c (gap2 = squared distance bound between the target and the cell) have to be visited?
+    auto cell_wanted = [&](uint32_t c, double gap2) {
+        if (gap2 > reach2) return false;
+        if (SWEEP == SW_HSEARCH && !(__ldg(T.cell_hmin + c) < ha)) return false;   // nobody in the cell has a smaller h
+        if (sym) {
+            // symmetric sets: b in N_sym(a) needs r < 2 max(h_a, h_b) <= 2 max(h_a, max h of b's cell), and r >= the gap
+            const double rc = 2.0 * fmax(ha, __ldg(T.cell_hmax + c));
+            if (gap2 > (rc * rc) * (1.0 + 1e-9)) return false;
+        }
+        return true;
+    };
+    if (WARP) {
+        // The lanes take one cell ROW (fixed y, z; the cells of a row are consecutive ranges of sorted slots) each and cull
+        // its cells in parallel -- the per-cell loads of the culling are then 32 wide instead of one dependent chain per
+        // cell -- and leave the slot range from the first to the last cell wanted, per unwrapped piece of the row (two when
+        // the x-span crosses a periodic face), in a per-warp list; the warp then runs through the listed ranges together.
+        __shared__ uint2 s_ranges[4][64];
+        uint2* ranges = s_ranges[threadIdx.x >> 5];
+        const int nrows = sy.cnt * sz.cnt;
+        for (int r0 = 0; r0 < nrows; r0 += 32) {
+            uint2 ra = make_uint2(0u, 0u), rb = make_uint2(0u, 0u);
+            const int r = r0 + (int)lane;
+            if (r < nrows) {
+                const int kz = r / sy.cnt, ky = r - kz * sy.cnt;
+                const int czz = g.per[2] ? wrap_cell(sz.start + kz, g.nc[2]) : sz.start + kz;
+                const int cyy = g.per[1] ? wrap_cell(sy.start + ky, g.nc[1]) : sy.start + ky;
+                const double gyz2 = cell_gap2(sz.start + kz - cz, fcz, fullz, ez) + cell_gap2(sy.start + ky - cy, fcy, fully, ey);
+                if (!(gyz2 > reach2)) {
+                    const uint32_t crow = (uint32_t)((czz * g.nc[1] + cyy) * g.nc[0]);
+                    int fa = -1, la = -1, fb = -1, lb = -1;              // first / last wanted cell of the two pieces (wrapped x index)
+                    for (int kx = 0; kx < sx.cnt; ++kx) {
+                        const int ox = sx.start + kx;
+                        const int cxx = g.per[0] ? wrap_cell(ox, g.nc[0]) : ox;
+                        if (!cell_wanted(crow + (uint32_t)cxx, gyz2 + cell_gap2(ox - cx, fcx, fullx, ex))) continue;
+                        if (ox == cxx) { if (fa < 0) fa = cxx; la = cxx; }     // the piece inside [0, nc)
+                        else { if (fb < 0) fb = cxx; lb = cxx; }               // the piece beyond a periodic face
+                    }
+                    if (fa >= 0) ra = make_uint2(__ldg(T.cell_start + crow + fa), __ldg(T.cell_end + crow + la));
+                    if (fb >= 0) rb = make_uint2(__ldg(T.cell_start + crow + fb), __ldg(T.cell_end + crow + lb));
+                }
+            }
+            const uint32_t ma = __ballot_sync(0xFFFFFFFFu, ra.y > ra.x), mb = __ballot_sync(0xFFFFFFFFu, rb.y > rb.x);
+            const uint32_t lt = (1u << lane) - 1u;
+            __syncwarp();
+            if (ra.y > ra.x) ranges[__popc(ma & lt)] = ra;
+            if (rb.y > rb.x) ranges[__popc(ma) + __popc(mb & lt)] = rb;
+            const uint32_t nr = __popc(ma) + __popc(mb);
+            __syncwarp();
+            for (uint32_t q = 0; q < nr; ++q) {
+                const uint32_t jb = ranges[q].x, je = ranges[q].y;
+                if (QUEUED) {
+                    for (uint32_t j0 = jb; j0 < je; j0 += 64u) {            // two candidates per lane in flight
+                        const uint32_t j1 = j0 + lane, j2 = j1 + 32u;
+                        bool hit1 = false, hit2 = false;
+                        if (j1 < je) hit1 = contributes(geometry(j1));
+                        if (j2 < je) hit2 = contributes(geometry(j2));
+                        const uint32_t m1 = __ballot_sync(0xFFFFFFFFu, hit1), m2 = __ballot_sync(0xFFFFFFFFu, hit2);
+                        if (hit1) queue[qn + __popc(m1 & lt)] = j1;
+                        qn += __popc(m1);
+                        if (qn >= 32u) { drain(32u); qn -= 32u; }
+                        if (hit2) queue[qn + __popc(m2 & lt)] = j2;
+                        qn += __popc(m2);
+                        if (qn >= 32u) { drain(32u); qn -= 32u; }
+                    }
+                } else {
+                    for (uint32_t j = jb + lane; j < je; j += 32u) pair_term(j, geometry(j));
                 }
             }
         }
+    } else {
+        for (int kz = 0; kz < sz.cnt; ++kz) {
+            const int czz = g.per[2] ? wrap_cell(sz.start + kz, g.nc[2]) : sz.start + kz;
+            const double gz2 = cell_gap2(sz.start + kz - cz, fcz, fullz, ez);
+            if (gz2 > reach2) continue;
+            for (int ky = 0; ky < sy.cnt; ++ky) {
+                const int cyy = g.per[1] ? wrap_cell(sy.start + ky, g.nc[1]) : sy.start + ky;
+                const double gyz2 = gz2 + cell_gap2(sy.start + ky - cy, fcy, fully, ey);
+                if (gyz2 > reach2) continue;
+                for (int kx = 0; kx < sx.cnt; ++kx) {
+                    const int cxx = g.per[0] ? wrap_cell(sx.start + kx, g.nc[0]) : sx.start + kx;
+                    const double gap2 = gyz2 + cell_gap2(sx.start + kx - cx, fcx, fullx, ex);
+                    const uint32_t c = (uint32_t)((czz * g.nc[1] + cyy) * g.nc[0] + cxx);
+                    if (!cell_wanted(c, gap2)) continue;
+                    const uint32_t jb = __ldg(T.cell_start + c), je = __ldg(T.cell_end + c);
+                    for (uint32_t j = jb; j < je; ++j) pair_term(j, geometry(j));
+                }
+            }
+        }
+
     }
 
+    if (QUEUED && qn) drain(qn);
     if (WARP) {
         acc0 = warp_add(acc0); acc1 = warp_add(acc1); acc2 = warp_add(acc2); acc3 = warp_add(acc3); acc4 = warp_add(acc4);
         cnt = warp_add(cnt);
