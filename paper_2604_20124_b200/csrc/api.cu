@@ -104,7 +104,17 @@ SweepArgs base_args(Ctx* c) {
 
 // general-kernel arguments of a sweep that the tiled kernels ran first: skip what they served (levels = the call also ran the
 // tiled kernels of the internal levels)
+// the context whose grid and sorted copies the general kernels of a level-aware call use: with levels on, the finest level
+// that was built (build_levels), else the context itself
+Ctx* general_ctx(Ctx* c) { return (c->levels_on && c->general) ? c->general : c; }
+
 SweepArgs fallback_args(Ctx* c, bool levels = false) {
+    if (levels && c->levels_on && c->general) {
+        Ctx* g = c->general;
+        SweepArgs a = base_args(g);
+        a.skip = g->fast_all; a.nfast = c->tl.ctr + CTR_NFAST_ALL; a.left = g->left; a.nleft = g->tl.ctr + CTR_NLEFT;
+        return a;
+    }
     SweepArgs a = base_args(c);
     if (levels && c->levels_on) { a.skip = c->fast_all; a.nfast = c->tl.ctr + CTR_NFAST_ALL; a.left = c->left; a.nleft = c->tl.ctr + CTR_NLEFT; }
     else if (c->tl.enabled) {
@@ -213,6 +223,7 @@ static void destroy_levels(Ctx* c) {
     }
     c->nlevels = 0;
     c->levels_on = false;
+    c->general = nullptr;
 }
 
 int spray_set_levels(spray_ctx* ctx, int nlevels, const double* edges, const int64_t* ncell_max) {
@@ -322,7 +333,7 @@ static int build_levels(Ctx* c, const double* x, const double* y, const double* 
     double lo = 0.0;
     for (int k = 0; k < c->nlevels; ++k) {
         Ctx* v = c->child[k];
-        v->built = false; v->tl.enabled = false;
+        v->built = false; v->tl.enabled = false; v->soa_ctr = nullptr;
         spray_grid_t g = c->grid;
         int64_t nc = 1;
         double emin = 1e300, emax = 0.0;
@@ -363,6 +374,20 @@ static int build_levels(Ctx* c, const double* x, const double* y, const double* 
     }
     CK(launch_fast_from_caller(c, st), "levels: served flags to sorted order");
     CK(launch_compact_left(c, c->fast_all, st), "levels: list of the particles left to the general kernels");
+    // The general kernels of the level-aware calls run on the finest level that was built: where particles are left over they
+    // are dense for their search length (that is why no level could tile them), and the caller's grid (A14: 2 mean(h)) holds
+    // ~140 of them per cell at config 4 against ~18 on the finest level's.  That context gets what the general kernels need on
+    // top of a level's own: per-cell h_max / h_min, hs and the served flags in its sorted order, the list of the left-overs.
+    c->general = nullptr;
+    for (int k = 0; k < c->nlevels && !c->general; ++k) {
+        Ctx* v = c->child[k];
+        if (!v || !v->built || !v->tl.enabled) continue;
+        CK(launch_cell_hmax(v, st), "levels: per-cell h_max of the general kernels' grid");
+        CK(launch_general_from_parent(v, c, st), "levels: search lengths and served flags on the general kernels' grid");
+        CK(launch_compact_left(v, v->fast_all, st), "levels: left-over list on the general kernels' grid");
+        v->soa_ctr = c->tl.ctr + CTR_NFAST_ALL;
+        c->general = v;
+    }
     c->levels_on = true;
     return SPRAY_OK;
 }
@@ -456,9 +481,10 @@ int spray_density(spray_ctx* ctx, const double* m, double* rho, uint32_t* nnbr, 
         t.o0 = rho; t.ocount = nnbr;
         CK(launch_tiled_sweep(ts.v[k], SW_DENSITY, t, st), "tiled density sweep");
     }
+    Ctx* gc = general_ctx(c);
     SweepArgs a = fallback_args(c, true);
-    a.m = c->s.f[F_M]; a.o0 = rho; a.ocount = nnbr;
-    CK(launch_ref_sweep(c, SW_DENSITY, a, st), "density sweep");
+    a.m = gc->s.f[F_M]; a.o0 = rho; a.ocount = nnbr;
+    CK(launch_ref_sweep(gc, SW_DENSITY, a, st), "density sweep");
     return SPRAY_OK;
 }
 
@@ -485,12 +511,14 @@ int spray_hydro_rhs(spray_ctx* ctx, const double* m, const double* rho, const do
         t.o0 = ax; t.o1 = ay; t.o2 = az; t.o3 = dudt; t.o4 = divv_sum;
         CK(launch_tiled_sweep(ts.v[k], SW_HYDRO, t, st), "tiled hydro sweep");
     }
+    Ctx* gc = general_ctx(c);
+    f = gc->s.f;
     SweepArgs a = fallback_args(c, true);
     a.m = f[F_M]; a.rho = f[F_RHO]; a.p = f[F_P]; a.cs = f[F_CS];
     a.vx = f[F_VX]; a.vy = f[F_VY]; a.vz = f[F_VZ]; a.alpha = f[F_ALPHA];
     a.beta = beta;
     a.o0 = ax; a.o1 = ay; a.o2 = az; a.o3 = dudt; a.o4 = divv_sum;
-    CK(launch_ref_sweep(c, SW_HYDRO, a, st), "hydro sweep");
+    CK(launch_ref_sweep(gc, SW_HYDRO, a, st), "hydro sweep");
     return SPRAY_OK;
 }
 
@@ -519,17 +547,19 @@ int spray_hydro_rhs_limiter(spray_ctx* ctx, const double* m, const double* rho, 
         t.o0 = ax; t.o1 = ay; t.o2 = az; t.o3 = dudt; t.o4 = divv_sum; t.o5 = mu; t.o6 = gradE;
         CK(launch_tiled_sweep(ts.v[k], SW_HYDLIM, t, st), "tiled hydro + limiter sweep");
     }
+    Ctx* gc = general_ctx(c);
+    f = gc->s.f;
     SweepArgs a = fallback_args(c, true);
     a.m = f[F_M]; a.rho = f[F_RHO]; a.p = f[F_P]; a.cs = f[F_CS];
     a.vx = f[F_VX]; a.vy = f[F_VY]; a.vz = f[F_VZ]; a.alpha = f[F_ALPHA];
     a.beta = beta;
     a.o0 = ax; a.o1 = ay; a.o2 = az; a.o3 = dudt; a.o4 = divv_sum;
-    CK(launch_ref_sweep(c, SW_HYDRO, a, st), "hydro sweep");
+    CK(launch_ref_sweep(gc, SW_HYDRO, a, st), "hydro sweep");
     SweepArgs l = fallback_args(c, true);
     l.m = f[F_M]; l.rho = f[F_RHO]; l.E = f[F_E]; l.kappa = f[F_KAPPA]; l.mu = f[F_MU];
     l.c_light = c_light;
-    l.o0 = mu; l.o1 = gradE; l.mu_sorted = f[F_MU]; l.me_sorted = c->pk.me;
-    CK(launch_ref_sweep(c, SW_LIMITER, l, st), "limiter sweep");
+    l.o0 = mu; l.o1 = gradE; l.mu_sorted = f[F_MU]; l.me_sorted = gc->pk.me;
+    CK(launch_ref_sweep(gc, SW_LIMITER, l, st), "limiter sweep");
     // the sorted (z, V) and (mu, E) records of every particle are in place: spray_fld_apply(SPRAY_FLD_FROZEN_CHAINED) may reuse them
     c->chain_ok = !c->levels_on;
     c->chain_m = m; c->chain_rho = rho; c->chain_E = E; c->chain_mu = mu;
@@ -564,8 +594,10 @@ int spray_fld_apply(spray_ctx* ctx, const double* m, const double* rho, const do
     const TiledSet ts = tiled_set(c);
     for (int k = 0; k < ts.n; ++k)
         if (ts.v[k] != c) CK(launch_prep_fld(ts.v[k], level_job(pj, ts.v[k]), st), "fld prologue (level)");
+    Ctx* gc = general_ctx(c);
+    double** gf = gc->s.f;
     SweepArgs a = fallback_args(c, true);
-    a.m = f[F_M]; a.rho = f[F_RHO]; a.E = f[F_E]; a.kappa = f[F_KAPPA]; a.mu = f[F_MU];
+    a.m = gf[F_M]; a.rho = gf[F_RHO]; a.E = gf[F_E]; a.kappa = gf[F_KAPPA]; a.mu = gf[F_MU];
     a.c_light = c_light;
     if (update) {
         for (int k = 0; k < ts.n; ++k) {
@@ -574,8 +606,8 @@ int spray_fld_apply(spray_ctx* ctx, const double* m, const double* rho, const do
             CK(launch_tiled_sweep(ts.v[k], SW_LIMITER, t, st), "tiled limiter sweep");
         }
         SweepArgs l = a;
-        l.o0 = mu; l.o1 = gradE; l.mu_sorted = f[F_MU]; l.me_sorted = c->pk.me;
-        CK(launch_ref_sweep(c, SW_LIMITER, l, st), "limiter sweep");
+        l.o0 = mu; l.o1 = gradE; l.mu_sorted = gf[F_MU]; l.me_sorted = gc->pk.me;
+        CK(launch_ref_sweep(gc, SW_LIMITER, l, st), "limiter sweep");
         if (c->levels_on) {
             // every context computed mu for the particles it serves only: the (mu, E) records and the sorted mu of all of them
             // are re-packed from the caller-order mu (as in FROZEN mode) before the apply
@@ -594,7 +626,7 @@ int spray_fld_apply(spray_ctx* ctx, const double* m, const double* rho, const do
         CK(launch_tiled_sweep(ts.v[k], SW_APPLY, t, st), "tiled apply sweep");
     }
     a.o0 = y; a.o1 = diag; a.o2 = offd;
-    CK(launch_ref_sweep(c, SW_APPLY, a, st), "apply sweep");
+    CK(launch_ref_sweep(gc, SW_APPLY, a, st), "apply sweep");
     return SPRAY_OK;
 }
 
@@ -790,7 +822,7 @@ int spray_neighbor_counts(spray_ctx* ctx, int symmetric, uint32_t* count, void* 
         CK(launch_tiled_export(ts.v[k], 0, symmetric, count, nullptr, nullptr, nullptr, nullptr, (cudaStream_t)stream), "neighbour counts from the tiled lists");
     SweepArgs a = fallback_args(c, true);
     a.symmetric = symmetric; a.ocount = count;
-    CK(launch_ref_sweep(c, SW_COUNT, a, (cudaStream_t)stream), "neighbour count sweep");
+    CK(launch_ref_sweep(general_ctx(c), SW_COUNT, a, (cudaStream_t)stream), "neighbour count sweep");
     return SPRAY_OK;
 }
 
@@ -803,7 +835,7 @@ int spray_neighbor_lists(spray_ctx* ctx, int symmetric, const uint64_t* offsets,
         CK(launch_tiled_export(ts.v[k], 1, symmetric, nullptr, offsets, nbr, nullptr, nullptr, (cudaStream_t)stream), "neighbour lists from the tiled lists");
     SweepArgs a = fallback_args(c, true);
     a.symmetric = symmetric; a.offsets = offsets; a.onbr = nbr;
-    CK(launch_ref_sweep(c, SW_LIST, a, (cudaStream_t)stream), "neighbour list sweep");
+    CK(launch_ref_sweep(general_ctx(c), SW_LIST, a, (cudaStream_t)stream), "neighbour list sweep");
     return SPRAY_OK;
 }
 
@@ -816,7 +848,7 @@ int spray_neighbor_digest(spray_ctx* ctx, int symmetric, uint64_t* dsum, uint64_
         CK(launch_tiled_export(ts.v[k], 2, symmetric, nullptr, nullptr, nullptr, dsum, dxor, (cudaStream_t)stream), "neighbour digests from the tiled lists");
     SweepArgs a = fallback_args(c, true);
     a.symmetric = symmetric; a.odsum = dsum; a.odxor = dxor;
-    CK(launch_ref_sweep(c, SW_DIGEST, a, (cudaStream_t)stream), "neighbour digest sweep");
+    CK(launch_ref_sweep(general_ctx(c), SW_DIGEST, a, (cudaStream_t)stream), "neighbour digest sweep");
     return SPRAY_OK;
 }
 

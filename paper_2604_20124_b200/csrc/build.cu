@@ -346,6 +346,15 @@ __global__ void k_fast_from_caller(const uint32_t* __restrict__ perm, int64_t n,
     if ((threadIdx.x & 31) == 0 && m) atomicAdd(nfast, (unsigned long long)__popc(m));
 }
 
+__global__ void k_general_from_parent(const uint32_t* __restrict__ perm, int64_t n, const double* __restrict__ hs_c, const uint8_t* __restrict__ fast_c,
+                                      double* __restrict__ hs, uint8_t* __restrict__ fast) {
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const uint32_t p = perm[i];
+    hs[i] = hs_c[p];
+    fast[i] = fast_c[p] ? 1 : 0;
+}
+
 // ------------------------------------------------------------------------------------------- launchers
 static inline int cdiv64(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
 
@@ -395,6 +404,13 @@ cudaError_t launch_fast_from_caller(Ctx* c, cudaStream_t st) {
     if (e != cudaSuccess) return e;
     k_fast_from_caller<<<cdiv64(c->n, 256), 256, 0, st>>>(c->perm, c->n, c->fast_c, c->fast_all, c->tl.ctr + CTR_NFAST_ALL);
     c->launches += 1;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_general_from_parent(Ctx* v, Ctx* parent, cudaStream_t st) {
+    if (v->n == 0) return cudaSuccess;
+    k_general_from_parent<<<cdiv64(v->n, 256), 256, 0, st>>>(v->perm, v->n, parent->hs_c, parent->fast_c, v->s.hs, v->fast_all);
+    v->launches += 1;
     return cudaGetLastError();
 }
 
@@ -455,6 +471,7 @@ cudaError_t launch_reorder_build(Ctx* c, const double* x, const double* y, const
 // device word the prologues compare with n: equal = nobody needs the structure-of-arrays copies (general kernels idle).
 // A level context never runs general kernels: its word is CTR_NALL = n.
 static const unsigned long long* nfast_ptr(Ctx* c) {
+    if (c->soa_ctr) return c->soa_ctr;               // the level context that runs the parent's general kernels
     if (c->is_level) return c->tl.ctr + CTR_NALL;
     return c->tl.enabled ? c->tl.ctr + CTR_NFAST : nullptr;
 }

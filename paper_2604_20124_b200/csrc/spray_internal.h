@@ -97,6 +97,9 @@ struct Ctx {
     Ctx* child[SPRAY_MAX_LEVELS] = {};
     double level_edge[SPRAY_MAX_LEVELS] = {};
     bool is_level = false;
+    Ctx* general = nullptr;                     // parent, levels on: the level context (finest built one) whose grid the general kernels use for
+                                                // the particles no level serves -- the caller's grid may be far too coarse where they are dense
+    const unsigned long long* soa_ctr = nullptr;// that level context: device word the prologues compare with n (parent's count of served particles)
     double level_lo = 0.0, level_hi = 0.0;      // of a level context: its range of 2 hs
     float level_rmax = 0.f;                     // of a level context: largest support radius it can meet (error bound of the fp32 prefilter)
     const double* hs_caller = nullptr;          // level context: the parent's arrays below
@@ -113,6 +116,7 @@ struct Ctx {
 cudaError_t launch_cell_keys(Ctx* c, const double* x, const double* y, const double* z, cudaStream_t st);
 cudaError_t launch_to_caller_order(Ctx* c, cudaStream_t st);           // hs_c, fast_c from the sorted hs / fast of the parent
 cudaError_t launch_merge_served(Ctx* parent, Ctx* child, cudaStream_t st);   // fast_c |= the child's served targets
+cudaError_t launch_general_from_parent(Ctx* v, Ctx* parent, cudaStream_t st);   // level v: s.hs and fast_all in v's sorted order from the parent's caller-order arrays
 cudaError_t launch_fast_from_caller(Ctx* c, cudaStream_t st);          // parent: fast_all[i] = fast_c[perm[i]], ctr[CTR_NFAST_ALL] = count
 cudaError_t launch_radix_sort(Ctx* c, cudaStream_t st);      // sets c->sorted_key / c->perm
 cudaError_t launch_cell_table(Ctx* c, cudaStream_t st);

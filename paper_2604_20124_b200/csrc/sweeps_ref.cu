@@ -10,6 +10,7 @@ struct CellTabs {
     const uint32_t *sorted_key, *perm, *cell_start, *cell_end;
     const double* hglob;
     const double* cell_hmin;
+    int key_shift;                // 1 on a level context, whose sort keys carry a served-here bit below the cell index
     const double* cell_hmax;      // per-cell max h: a cell farther from the target than 2 max(h_a, cell_hmax) holds no mutual neighbour
 };
 
@@ -75,7 +76,7 @@ __device__ __forceinline__ void ref_particle(const DevGrid& g, int64_t n, const 
     const double reach = 2.0 * (sym ? A.hs[i] : ha);
     const double sup_a = support2(ha);
 
-    const uint32_t key = T.sorted_key[i];
+    const uint32_t key = T.sorted_key[i] >> T.key_shift;
     const int cx = key % g.nc[0], cy = (key / g.nc[0]) % g.nc[1], cz = key / (g.nc[0] * g.nc[1]);
     const Span sx = cell_span(g, 0, cx, reach), sy = cell_span(g, 1, cy, reach), sz = cell_span(g, 2, cz, reach);
     const double fcx = __dmul_rn(__dsub_rn(xa, g.lo[0]), g.inv[0]) - (double)cx;
@@ -242,7 +243,9 @@ __device__ __forceinline__ void ref_particle(const DevGrid& g, int64_t n, const 
         // cell -- and leave the slot range from the first to the last cell wanted, per unwrapped piece of the row (two when
         // the x-span crosses a periodic face), in a per-warp list; the warp then runs through the listed ranges together.
         __shared__ uint2 s_ranges[4][64];
+        __shared__ uint32_t s_rstart[4][64];
         uint2* ranges = s_ranges[threadIdx.x >> 5];
+        uint32_t* rstart = s_rstart[threadIdx.x >> 5];
         const int nrows = sy.cnt * sz.cnt;
         for (int r0 = 0; r0 < nrows; r0 += 32) {
             uint2 ra = make_uint2(0u, 0u), rb = make_uint2(0u, 0u);
@@ -273,25 +276,53 @@ __device__ __forceinline__ void ref_particle(const DevGrid& g, int64_t n, const 
             if (rb.y > rb.x) ranges[__popc(ma) + __popc(mb & lt)] = rb;
             const uint32_t nr = __popc(ma) + __popc(mb);
             __syncwarp();
-            for (uint32_t q = 0; q < nr; ++q) {
-                const uint32_t jb = ranges[q].x, je = ranges[q].y;
+            // The listed ranges are walked as ONE stream of candidates (exclusive prefix sums of their lengths; a lane finds
+            // the range of its flat index by bisection), 128 candidates per step: short ranges -- a row of a fine grid holds a
+            // few dozen particles -- would otherwise leave most lanes idle, and every step costs a full memory round trip.
+            {
+                const uint32_t l0 = lane < nr ? ranges[lane].y - ranges[lane].x : 0u;
+                const uint32_t l1 = lane + 32u < nr ? ranges[lane + 32u].y - ranges[lane + 32u].x : 0u;
+                uint32_t i0 = l0, i1 = l1;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const uint32_t v0 = __shfl_up_sync(0xFFFFFFFFu, i0, o), v1 = __shfl_up_sync(0xFFFFFFFFu, i1, o);
+                    if ((int)lane >= o) { i0 += v0; i1 += v1; }
+                }
+                const uint32_t t0 = __shfl_sync(0xFFFFFFFFu, i0, 31), total = t0 + __shfl_sync(0xFFFFFFFFu, i1, 31);
+                rstart[lane] = i0 - l0;
+                rstart[lane + 32u] = t0 + i1 - l1;
+                __syncwarp();
+                auto candidate = [&](uint32_t fidx) {                   // flat index -> sorted slot
+                    uint32_t lo = 0u, hi = nr;                          // largest q with rstart[q] <= fidx
+                    while (hi - lo > 1u) {
+                        const uint32_t mid = (lo + hi) >> 1;
+                        if (rstart[mid] <= fidx) lo = mid; else hi = mid;
+                    }
+                    return ranges[lo].x + (fidx - rstart[lo]);
+                };
                 if (QUEUED) {
-                    for (uint32_t j0 = jb; j0 < je; j0 += 64u) {            // two candidates per lane in flight
-                        const uint32_t j1 = j0 + lane, j2 = j1 + 32u;
-                        bool hit1 = false, hit2 = false;
-                        if (j1 < je) hit1 = contributes(geometry(j1));
-                        if (j2 < je) hit2 = contributes(geometry(j2));
-                        const uint32_t m1 = __ballot_sync(0xFFFFFFFFu, hit1), m2 = __ballot_sync(0xFFFFFFFFu, hit2);
-                        if (hit1) queue[qn + __popc(m1 & lt)] = j1;
-                        qn += __popc(m1);
-                        if (qn >= 32u) { drain(32u); qn -= 32u; }
-                        if (hit2) queue[qn + __popc(m2 & lt)] = j2;
-                        qn += __popc(m2);
-                        if (qn >= 32u) { drain(32u); qn -= 32u; }
+                    for (uint32_t f0 = 0; f0 < total; f0 += 128u) {
+                        uint32_t jc[4];
+                        bool hit[4];
+#pragma unroll
+                        for (int e = 0; e < 4; ++e) {
+                            const uint32_t fidx = f0 + 32u * e + lane;
+                            hit[e] = false;
+                            jc[e] = 0u;
+                            if (fidx < total) { jc[e] = candidate(fidx); hit[e] = contributes(geometry(jc[e])); }
+                        }
+#pragma unroll
+                        for (int e = 0; e < 4; ++e) {
+                            const uint32_t m = __ballot_sync(0xFFFFFFFFu, hit[e]);
+                            if (hit[e]) queue[qn + __popc(m & lt)] = jc[e];
+                            qn += __popc(m);
+                            if (qn >= 32u) { drain(32u); qn -= 32u; }
+                        }
                     }
                 } else {
-                    for (uint32_t j = jb + lane; j < je; j += 32u) pair_term(j, geometry(j));
+                    for (uint32_t fidx = lane; fidx < total; fidx += 32u) { const uint32_t j = candidate(fidx); pair_term(j, geometry(j)); }
                 }
+                __syncwarp();
             }
         }
     } else {
@@ -417,7 +448,7 @@ k_ref_sweep(DevGrid g, int64_t n, CellTabs T, SweepArgs A) {
 template <int SWEEP>
 static cudaError_t launch_k(Ctx* c, const SweepArgs& a, cudaStream_t st) {
     if (c->n == 0) return cudaSuccess;
-    CellTabs T{c->sorted_key, c->perm, c->cell_start, c->cell_end, c->hglob, c->cell_hmin, c->cell_hmax};
+    CellTabs T{c->sorted_key, c->perm, c->cell_start, c->cell_end, c->hglob, c->cell_hmin, c->is_level ? 1 : 0, c->cell_hmax};
     const int64_t want = (c->n + 127) / 128;
     const int blocks = (int)(want < 148 * 64 ? want : 148 * 64);
     if (c->kernel == SPRAY_KERNEL_WENDLAND_C2) k_ref_sweep<SWEEP, 1><<<blocks, 128, 0, st>>>(c->dg, c->n, T, a);
