@@ -100,9 +100,10 @@ int spray_set_path(spray_ctx* ctx, int path);
  * *n_fast = particles served by the tiled kernels (the rest, n - n_fast, by the general kernels),
  * *n_nonuniform = list-builder work units (half tiles) whose particles do not all share one h (they run the
  * variable-h pair bodies), *scratch_bytes = device memory the context holds (allocated at spray_create).
- * declined[k] = list-builder events that left a half tile to the general kernels, by reason: 0 unused, 1 list pool
- * exhausted, 2 a list longer than 80 rounds or more than 24 neighbours in one shared-memory bank, 3 other (coincident
- * particles, particle outside the tile's fp32 range).  All host pointers, all nullable. */
+ * declined[k] = targets (k = 1: warps) the list builder left to the general kernels, by reason: 0 unused, 1 list pool
+ * exhausted (per warp of 16 targets), 2 a list longer than 160 neighbours or more than 24 neighbours in one shared-memory
+ * bank, 3 other (coincident particles, particle outside the tile's fp32 range).  With internal levels the counts are summed
+ * over the levels.  All host pointers, all nullable. */
 int spray_path_stats(spray_ctx* ctx, void* stream, int64_t* n_tiles, int64_t* n_fast, int64_t* n_nonuniform,
                      int64_t* scratch_bytes, int64_t* declined /* [4] */);
 
