@@ -6,6 +6,9 @@
 
 namespace spray {
 
+constexpr int REF_THREADS = 128;                 // threads per CTA of k_ref_sweep: the per-warp shared-memory areas below are sized for it
+constexpr int REF_WARPS = REF_THREADS / 32;
+
 struct CellTabs {
     const uint32_t *sorted_key, *perm, *cell_start, *cell_end;
     const double* hglob;
@@ -212,7 +215,7 @@ __device__ __forceinline__ void ref_particle(const DevGrid& g, int64_t n, const 
     // so its long fp64 body (divisions, square roots) runs with every lane busy instead of the few per cent that hit.
     constexpr bool QUEUED = WARP && (SWEEP == SW_DENSITY || SWEEP == SW_HYDRO || SWEEP == SW_LIMITER || SWEEP == SW_GRADN ||
                                      SWEEP == SW_KGC || SWEEP == SW_APPLY);
-    __shared__ uint32_t s_queue[QUEUED ? 4 : 1][64];
+    __shared__ uint32_t s_queue[QUEUED ? REF_WARPS : 1][64];
     uint32_t* queue = s_queue[QUEUED ? (threadIdx.x >> 5) : 0];
     uint32_t qn = 0;
     const uint32_t lane = threadIdx.x & 31u;
@@ -242,8 +245,8 @@ __device__ __forceinline__ void ref_particle(const DevGrid& g, int64_t n, const 
         // its cells in parallel -- the per-cell loads of the culling are then 32 wide instead of one dependent chain per
         // cell -- and leave the slot range from the first to the last cell wanted, per unwrapped piece of the row (two when
         // the x-span crosses a periodic face), in a per-warp list; the warp then runs through the listed ranges together.
-        __shared__ uint2 s_ranges[4][64];
-        __shared__ uint32_t s_rstart[4][64];
+        __shared__ uint2 s_ranges[REF_WARPS][64];
+        __shared__ uint32_t s_rstart[REF_WARPS][64];
         uint2* ranges = s_ranges[threadIdx.x >> 5];
         uint32_t* rstart = s_rstart[threadIdx.x >> 5];
         const int nrows = sy.cnt * sz.cnt;
@@ -426,7 +429,7 @@ __device__ __forceinline__ void ref_particle(const DevGrid& g, int64_t n, const 
 // Grid-stride over the particles with a bounded grid: when the tiled kernels served every particle (the usual
 // case) the launch costs a few microseconds instead of n/128 empty blocks.
 template <int SWEEP, int KERNEL>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(REF_THREADS)
 k_ref_sweep(DevGrid g, int64_t n, CellTabs T, SweepArgs A) {
     if (A.nfast && *A.nfast == (unsigned long long)n) return;   // the tiled kernels serve every particle
     if (A.left) {                                               // the rest, compacted: one warp per particle (SW_LIST: one thread)
@@ -449,10 +452,10 @@ template <int SWEEP>
 static cudaError_t launch_k(Ctx* c, const SweepArgs& a, cudaStream_t st) {
     if (c->n == 0) return cudaSuccess;
     CellTabs T{c->sorted_key, c->perm, c->cell_start, c->cell_end, c->hglob, c->cell_hmin, c->is_level ? 1 : 0, c->cell_hmax};
-    const int64_t want = (c->n + 127) / 128;
+    const int64_t want = (c->n + REF_THREADS - 1) / REF_THREADS;
     const int blocks = (int)(want < 148 * 64 ? want : 148 * 64);
-    if (c->kernel == SPRAY_KERNEL_WENDLAND_C2) k_ref_sweep<SWEEP, 1><<<blocks, 128, 0, st>>>(c->dg, c->n, T, a);
-    else k_ref_sweep<SWEEP, 0><<<blocks, 128, 0, st>>>(c->dg, c->n, T, a);
+    if (c->kernel == SPRAY_KERNEL_WENDLAND_C2) k_ref_sweep<SWEEP, 1><<<blocks, REF_THREADS, 0, st>>>(c->dg, c->n, T, a);
+    else k_ref_sweep<SWEEP, 0><<<blocks, REF_THREADS, 0, st>>>(c->dg, c->n, T, a);
     c->launches += 1;
     return cudaGetLastError();
 }
