@@ -58,7 +58,7 @@ struct Tiled {
 // outside the tile's fp32 range)
 // CTR_NALL: n (level contexts: the per-call prologues compare it with n and skip the structure-of-arrays copies)
 // CTR_NFAST_ALL: particles served by the tiled kernels of the context or of one of its levels
-enum { CTR_NFAST = 1, CTR_NTILES = 2, CTR_NNONUNI = 3, CTR_POOL = 4, CTR_NALL = 5, CTR_NFAST_ALL = 6, CTR_NLEFT = 7, CTR_DECL = 8, CTR_COUNT = 12 };
+enum { CTR_NFAST = 1, CTR_NTILES = 2, CTR_NNONUNI = 3, CTR_POOL = 4, CTR_NALL = 5, CTR_NFAST_ALL = 6, CTR_NLEFT = 7, CTR_DECL = 8, CTR_NMULTI = 12, CTR_COUNT = 16 };   // CTR_NMULTI: tile groups of more than one part (tiles.cuh)
 
 struct Ctx {
     int device = 0;

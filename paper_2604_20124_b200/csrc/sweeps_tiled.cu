@@ -333,7 +333,10 @@ template <int SWEEP, int MODE> struct MinBlocks {
     static constexpr int v = (SWEEP == SW_DENSITY || SWEEP == SW_LIMITER || SWEEP == SW_GRADN || (SWEEP == SW_APPLY && MODE == 1)) ? 2 : 1;
 };
 
-template <int SWEEP, int KERNEL, int MODE>
+// PARTS = false: the tiles that are one entry (nearly all; every tile of a particle set with uniform h).  PARTS = true: the
+// groups of several parts (tiles.cuh), in a launch of their own that returns at once when the build cut none -- carrying a
+// target and its sums from part to part costs registers that the 64-register kernels do not have to spare.
+template <int SWEEP, int KERNEL, int MODE, bool PARTS>
 __global__ void __launch_bounds__(TILE_THREADS, MinBlocks<SWEEP, MODE>::v)
 k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
     constexpr int NV = NRecM<SWEEP, MODE>::v;
@@ -348,6 +351,7 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
     const int u = tid & 1, tgt = tid >> 1;
     const uint32_t ntiles = (uint32_t)A.ctr[CTR_NTILES];
     if (MODE == 2 && A.ctr[CTR_NNONUNI] == 0) return;          // no tile with variable h (the usual case): nothing for this launch
+    if (PARTS && A.ctr[CTR_NMULTI] == 0) return;               // no group of several parts (the usual case)
     constexpr bool HYD = SWEEP == SW_HYDRO || SWEEP == SW_HYDLIM;
     const bool sym = HYD || (SWEEP == SW_APPLY && A.fld_sym != 0);
     // dummy slots: far away, every weight zero, so that a padded list entry adds exactly nothing
@@ -376,22 +380,37 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
     };
     fetch_tables(blockIdx.x, 0);
     int buf = 1;
-    for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    // A tile entry is part 0 of nparts (tiles.cuh): the CTA that meets part 0 runs all the parts one after the other -- same
+    // targets, another set of candidate rows and lists each -- and keeps its sums; a CTA whose stride lands on a later part passes.
+    for (uint32_t tile0 = blockIdx.x; tile0 < ntiles; tile0 += gridDim.x) {
+      uint32_t np = 1;
+      bool pass_group = false, active = false, grp_ok = true, uni = true;
+      uint32_t i = 0, ia = 0, ngat = 0;
+      Tgt T{};
+      Acc acc{};
+      for (uint32_t part = 0; part < (PARTS ? np : 1u); ++part) {
+        const uint32_t tile = tile0 + part;
         buf ^= 1;
         asm volatile("cp.async.wait_group 0;" ::: "memory");
         __syncthreads();                                         // tables in place; previous tile done with the staged records
-        fetch_tables(tile + gridDim.x, buf ^ 1);
         const TileS& S = Sb[buf];
         const uint32_t flags = Hb[buf].flags;
-        if (!(flags & TILE_FLAG_OK)) continue;
-        const bool tile_uni = (flags & TILE_FLAG_NONUNI) == 0;
-        const bool uni = MODE == 1 ? true : (MODE == 2 ? false : tile_uni);
-        if (MODE != 0 && tile_uni != (MODE == 1)) continue;
-        const bool half_ok = ((flags >> (warp / (TILE_WARPS / 2))) & 1u) != 0;   // this warp's half of the tile has lists
         const TileDesc td = Hb[buf].td;
+        if (part == 0) {
+            const bool tile_uni = (flags & TILE_FLAG_NONUNI) == 0;   // (of a group: the builder ORs every part's bit into part 0)
+            uni = MODE == 1 ? true : (MODE == 2 ? false : tile_uni);
+            if (td.part != 0 || (td.nparts > 1) != PARTS || (MODE != 0 && tile_uni != (MODE == 1))) pass_group = true;   // not mine / not this launch's kind
+            else if (PARTS) np = min((uint32_t)td.nparts, ntiles - tile0);
+        }
+        fetch_tables(PARTS && part + 1 < np ? tile + 1 : tile0 + gridDim.x, buf ^ 1);     // (a group that is passed has np = 1)
+        if (pass_group) break;
+        const bool half_ok = ((flags >> (warp / (TILE_WARPS / 2))) & 1u) != 0;   // this warp's half of the tile has lists
+        if (part == 0) active = half_ok && tgt < (int)td.nt;
+        if (!half_ok) grp_ok = false;                            // (the builder marked these targets: the general kernels redo them)
+        if (!(flags & TILE_FLAG_OK)) continue;
         // first three list rows: in flight while the records are staged
         uint2 wi = Hb[buf].winfo[warp];
-        if (!half_ok) wi.y = 0u;
+        if (!half_ok || !active) wi.y = 0u;
         const uint2* lp = A.pool + (size_t)wi.x * 32 + lane;
         const uint2 l0 = wi.y ? __ldcs(lp) : make_uint2(0u, 0u);
         const uint2 l1 = wi.y > 4 ? __ldcs(lp + 32) : make_uint2(0u, 0u);
@@ -399,11 +418,8 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
         // ---- this thread's target.  Except in the hydro kernel (register pressure: measured slower) its loads go out before
         //      the staging traffic, so they are back when the pair loop starts.
         constexpr bool EARLY_TARGET = !HYD;
-        const bool active = half_ok && tgt < (int)td.nt;
-        uint32_t i = 0, ia = 0;
-        Tgt T{};
         auto load_target = [&]() {
-            if (!active) return;
+            if (!active || part != 0) return;
             i = tile_target(td, S, tgt);
             ia = A.perm[i];                                      // caller index of the target: needed only in the epilogue
             const double2 xy = A.rec[0][i], zh = A.p1[i], hv = A.hh[i];
@@ -460,9 +476,12 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
         if (!EARLY_TARGET) load_target();
         asm volatile("cp.async.wait_group 0;" ::: "memory");
         __syncthreads();
-        Acc acc{};
         if (uni) pair_loop<SWEEP, KERNEL, true>(F, Ee, lp, wi.y, l0, l1, l2, T, A.beta, sym, acc);
         else pair_loop<SWEEP, KERNEL, false>(F, Ee, lp, wi.y, l0, l1, l2, T, A.beta, sym, acc);
+        if (SWEEP == SW_DENSITY && A.ocount && active && u == 0) ngat += A.lcount[(size_t)tile * TILE_T + tgt] & 0xFFFFu;
+      }
+      if (pass_group) continue;
+      {
         // ---- add the two half-lists of the target
         acc.a0 += __shfl_xor_sync(0xFFFFFFFFu, acc.a0, 1);
         if (SWEEP != SW_DENSITY) acc.a1 += __shfl_xor_sync(0xFFFFFFFFu, acc.a1, 1);
@@ -480,13 +499,13 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
             for (int e = 0; e < 15; ++e) acc.k[e] += __shfl_xor_sync(0xFFFFFFFFu, acc.k[e], 1);
         }
 
-        if (active && u == 0) {
+        if (active && grp_ok && u == 0) {
             const double sc = uni ? T.fn : 1.0;                  // kFn / h_a^4 where it was hoisted out of the loop
             if (SWEEP == SW_DENSITY) {
                 // self term m_a W(0; h_a) (A11)
                 const double wn = wn_k<KERNEL>() * (T.hinv * T.hinv) * T.hinv;
                 A.o0[ia] = wn * fma(T.c0, w0_k<KERNEL>(), acc.a0);
-                if (A.ocount) A.ocount[ia] = A.lcount[(size_t)tile * TILE_T + tgt] & 0xFFFFu;
+                if (A.ocount) A.ocount[ia] = ngat;
             } else if (HYD) {
                 A.o0[ia] = -(sc * acc.a0); A.o1[ia] = -(sc * acc.a1); A.o2[ia] = -(sc * acc.a2);
                 const double D = sc * acc.a3;
@@ -551,6 +570,7 @@ k_tiled_sweep(DevGrid g, CellTable ct, SweepIn A) {
                 if (A.o2) A.o2[ia] = fma(-lam, T.c0, yv);        // Gamma = y - Lambda E_a  (eq. (52))
             }
         }
+      }
     }
 }
 
@@ -562,8 +582,10 @@ constexpr size_t sweep_smem() {
 // that is launched, on the current device (spray_create calls this after cudaSetDevice).
 template <int SWEEP, int MODE>
 static cudaError_t set_attr() {
-    cudaError_t e = cudaFuncSetAttribute(k_tiled_sweep<SWEEP, 0, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sweep_smem<SWEEP, MODE>());
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_tiled_sweep<SWEEP, 1, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sweep_smem<SWEEP, MODE>());
+    cudaError_t e = cudaFuncSetAttribute(k_tiled_sweep<SWEEP, 0, MODE, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sweep_smem<SWEEP, MODE>());
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_tiled_sweep<SWEEP, 1, MODE, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sweep_smem<SWEEP, MODE>());
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_tiled_sweep<SWEEP, 0, MODE, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sweep_smem<SWEEP, MODE>());
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_tiled_sweep<SWEEP, 1, MODE, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sweep_smem<SWEEP, MODE>());
     return e;
 }
 cudaError_t sweeps_set_attributes() {
@@ -585,9 +607,14 @@ static cudaError_t launch_m(Ctx* c, const SweepIn& a, cudaStream_t st) {
     constexpr size_t smem = sweep_smem<SWEEP, MODE>();
     CellTable ct{c->cell_start, c->cell_end, c->is_level ? c->cell_tend : c->cell_end};
     const int grid = c->tl.sms * MinBlocks<SWEEP, MODE>::v;
-    if (c->kernel == SPRAY_KERNEL_WENDLAND_C2) k_tiled_sweep<SWEEP, 1, MODE><<<grid, TILE_THREADS, smem, st>>>(c->dg, ct, a);
-    else k_tiled_sweep<SWEEP, 0, MODE><<<grid, TILE_THREADS, smem, st>>>(c->dg, ct, a);
-    c->launches += 1;
+    if (c->kernel == SPRAY_KERNEL_WENDLAND_C2) {
+        k_tiled_sweep<SWEEP, 1, MODE, false><<<grid, TILE_THREADS, smem, st>>>(c->dg, ct, a);
+        k_tiled_sweep<SWEEP, 1, MODE, true><<<grid, TILE_THREADS, smem, st>>>(c->dg, ct, a);
+    } else {
+        k_tiled_sweep<SWEEP, 0, MODE, false><<<grid, TILE_THREADS, smem, st>>>(c->dg, ct, a);
+        k_tiled_sweep<SWEEP, 0, MODE, true><<<grid, TILE_THREADS, smem, st>>>(c->dg, ct, a);
+    }
+    c->launches += 2;
     return cudaGetLastError();
 }
 template <int SWEEP>

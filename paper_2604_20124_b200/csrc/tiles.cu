@@ -56,7 +56,8 @@ __device__ __forceinline__ uint32_t warp_sum(uint32_t v) {
 template <bool EMIT>
 __global__ void __launch_bounds__(256)
 k_make_tiles(DevGrid g, CellTable ct, const double* __restrict__ hglob, uint32_t* __restrict__ bcount,
-             TileDesc* __restrict__ tiles, uint32_t cap, unsigned long long* __restrict__ ctr, int level, unsigned long long n_all, int brows) {
+             TileDesc* __restrict__ tiles, uint32_t cap, unsigned long long* __restrict__ ctr, int level, unsigned long long n_all, int brows,
+             int parts) {
     // a bundle is brows x brows cell rows: 2 x 2 on the caller's grid (cells of ~18 particles: 4 x 4 candidate rows), 1 x 1 on the
     // internal levels, whose cells hold up to ~60 particles (3 x 3 candidate rows fit the staging budget)
     const int nby = (g.nc[1] + brows - 1) / brows, nbz = (g.nc[2] + brows - 1) / brows;
@@ -91,7 +92,43 @@ k_make_tiles(DevGrid g, CellTable ct, const double* __restrict__ hglob, uint32_t
     int cxa = 0;
     uint32_t skip = 0;
     while (ok && cxa < nx) {
-        if (warp_sum(row_count(row, cxa - 1, cxa + 1, nx, per)) > (uint32_t)TILE_CMAX) { ++cxa; skip = 0; continue; }   // column not tileable
+        {
+            const uint32_t myc = row_count(row, cxa - 1, cxa + 1, nx, per);             // lane l < 16: candidates of row l; others 0
+            if (warp_sum(myc) > (uint32_t)TILE_CMAX) {
+                // The column's own candidates do not fit one tile (cells holding a few hundred particles: the levels' junction
+                // zones): its targets still get tiles -- one column, up to TILE_T targets -- in several PARTS, each with a
+                // subset of the candidate rows that fits (greedy in row order).  A single row over the budget is hopeless.
+                // (parts = 0: the caller's grid when internal levels are set -- a finer level serves such a column far cheaper)
+                if (!parts || !__all_sync(0xFFFFFFFFu, myc <= (uint32_t)TILE_CMAX)) { ++cxa; skip = 0; continue; }
+                uint32_t accr = 0, part = 0, mypart = 0xFFu;
+                for (int l = 0; l < 16; ++l) {
+                    const uint32_t cl = __shfl_sync(0xFFFFFFFFu, myc, l);
+                    if (cl == 0u) continue;
+                    if (accr + cl > (uint32_t)TILE_CMAX) { ++part; accr = 0; }
+                    accr += cl;
+                    if (lane == l) mypart = part;
+                }
+                const uint32_t nparts = part + 1u;
+                uint32_t c = warp_sum(row.target ? row.te[cxa] - row.cs[cxa] : 0u) - skip;
+                const uint32_t take = min(c, (uint32_t)TILE_T);
+                if (take > 0) {
+                    for (uint32_t p = 0; p < nparts; ++p) {
+                        const uint32_t mask = __ballot_sync(0xFFFFFFFFu, mypart == p) & 0xFFFFu;
+                        if (EMIT && lane == 0 && obase + ntl + p < cap) {
+                            TileDesc td;
+                            td.y0 = (int16_t)y0; td.z0 = (int16_t)z0; td.cxa = (int16_t)cxa; td.cxb = (int16_t)cxa;
+                            td.nyr = (uint8_t)nyr; td.nzr = (uint8_t)nzr; td.part = (uint8_t)p; td.nparts = (uint8_t)nparts;
+                            td.skip = skip; td.nt = take; td.rowmask = mask;
+                            tiles[obase + ntl + p] = td;
+                        }
+                    }
+                    ntl += nparts;
+                    if (EMIT && lane == 0) atomicAdd(&ctr[CTR_NMULTI], 1ull);
+                }
+                if (take < c) skip += take; else { ++cxa; skip = 0; }
+                continue;
+            }
+        }
         uint32_t nt = 0;
         int cxb = cxa, next_cxa = nx;
         uint32_t next_skip = 0;
@@ -115,7 +152,7 @@ k_make_tiles(DevGrid g, CellTable ct, const double* __restrict__ hglob, uint32_t
             if (EMIT && lane == 0 && obase + ntl < cap) {
                 TileDesc td;
                 td.y0 = (int16_t)y0; td.z0 = (int16_t)z0; td.cxa = (int16_t)cxa; td.cxb = (int16_t)cxb;
-                td.nyr = (uint8_t)nyr; td.nzr = (uint8_t)nzr; td.pad = 0; td.skip = skip; td.nt = nt; td.pad2 = 0;
+                td.nyr = (uint8_t)nyr; td.nzr = (uint8_t)nzr; td.part = 0; td.nparts = 1; td.skip = skip; td.nt = nt; td.rowmask = 0xFFFFu;
                 tiles[obase + ntl] = td;
             }
             ++ntl;
@@ -177,6 +214,7 @@ struct ListArgs {
     uint32_t* tflags;                  // [tile], zeroed before the launch; each half ORs its bits in
     const uint32_t* tiletab;           // [tile][TILES_WORDS]
     uint8_t* fast;                     // [n] sorted order: 1 = served by the tiled kernels
+    uint8_t* fail;                     // [n] sorted order, zeroed before the launch: a target of a multi-part tile that some part declined
     const double* hglob;
     uint32_t* status;
     float rmax;                        // > 0: largest support radius the unit can meet (level contexts); else 2 max h from hglob
@@ -345,7 +383,9 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
         // an inactive thread sits far away from everything: it never hits
         const float fax = active ? (float)(xa - ox) : -3.0e18f, fay = (float)(ya - oy), faz = (float)(za - oz);
         if (active && !(fabsf(fax) <= extc && fabsf(fay) <= extc && fabsf(faz) <= extc)) tbad = true;
-        if (active && s_self == 0xFFFFFFFFu) tbad = true;               // cannot happen: the target's cell is among the candidates
+        const bool multi = td.nparts > 1;                               // one of several entries that share these targets (tiles.cuh)
+        if (active && s_self == 0xFFFFFFFFu && !multi) tbad = true;     // cannot happen: the target's cell is among the candidates
+        if (multi && tile - td.part + td.nparts > (nunits >> 1)) tbad = true;   // a group cut off at the tile capacity: nobody is served
         const float Ra = 2.0f * (float)ha;
         const float Ta = Ra * Ra;
         const float Ta_hi = fmaf(Ta, 1.00001f, Am), Ta_lo = fmaf(Ta, 0.99999f, -Am);
@@ -489,7 +529,7 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
         // Certain scan: no tested candidate within the uncertainty band of the support boundary, i.e. every fp32 decision
         // holds for the exact predicate too.  |t| >= band  <=>  r2_fp32 outside [T_lo, T_hi + (T_hi - T_lo)).
         const bool certain = uni && tmin >= (Ta_hi - Ta_lo);
-        const bool sees_self = active && ((s_self >> 2) & 1u) == (uint32_t)u;
+        const bool sees_self = active && s_self != 0xFFFFFFFFu && ((s_self >> 2) & 1u) == (uint32_t)u;   // (a part may not hold the target's own row)
         const bool full_settle = __any_sync(0xFFFFFFFFu, !certain && !ovf);
         if (!full_settle) {
             // the target itself (r = 0) is met by the thread that owns its bank: take that one entry out of its bucket
@@ -677,12 +717,18 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
         }
         const int served = __syncthreads_count(active && u == 0 && !tdecl);
         const bool bad = s_bad != 0;
-        if (!bad && active && u == 0 && !tdecl) A.fast[i] = 1;
+        // served = every part served: part 0 sets the flag and counts, any part that declines marks the target, and the pass
+        // after this kernel (k_apply_fail) takes the marked ones back
+        if (active && u == 0) {
+            if (!bad && !tdecl) { if (td.part == 0) A.fast[i] = 1; }
+            else if (multi) A.fail[i] = 1;
+        }
         if (tid == 0) {
             const uint32_t bits = (bad ? 0u : (TILE_FLAG_OK0 << half)) | (s_nonuni ? TILE_FLAG_NONUNI : 0u);
             if (bits) atomicOr(&A.tflags[tile], bits);
+            if (s_nonuni && td.part) atomicOr(&A.tflags[tile - td.part], TILE_FLAG_NONUNI);   // the sweeps pick a group's pair bodies by its first entry
             if (s_nonuni) atomicAdd(&A.ctr[CTR_NNONUNI], 1ull);
-            if (!bad) atomicAdd(&A.ctr[CTR_NFAST], (unsigned long long)served);
+            if (!bad && td.part == 0) atomicAdd(&A.ctr[CTR_NFAST], (unsigned long long)served);
         }
         }
         // the next unit's table goes into the other buffer (read after the barrier at the top of the loop)
@@ -693,6 +739,15 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
             if (tid < 6) s_td[buf ^ 1][tid] = pfd;
         }
     }
+}
+
+// targets of multi-part tiles that one of the parts declined: not served after all
+__global__ void k_apply_fail(uint8_t* __restrict__ fast, const uint8_t* __restrict__ fail, int64_t n, unsigned long long* __restrict__ ctr) {
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    const bool back = i < n && fail[i] && fast[i];
+    if (back) fast[i] = 0;
+    const unsigned m = __ballot_sync(0xFFFFFFFFu, back);
+    if ((threadIdx.x & 31) == 0 && m) atomicAdd(&ctr[CTR_NFAST], (unsigned long long)(0ll - (long long)__popc(m)));
 }
 
 // ------------------------------------------------------------------------------------------- parity exports
@@ -723,59 +778,69 @@ k_tiled_export(DevGrid g, ExportArgs A) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int u = tid & 1, tgt = tid >> 1;
     const uint32_t ntiles = (uint32_t)A.ctr[CTR_NTILES];
-    for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-        const uint32_t flags = A.tflags[tile];
-        if (!(flags & TILE_FLAG_OK)) continue;
-        const bool half_ok = ((flags >> (warp / (TILE_WARPS / 2))) & 1u) != 0;
-        const TileDesc td = A.tiles[tile];
-        __syncthreads();
-        {
-            const uint32_t* src = A.tiletab + (size_t)tile * TILES_WORDS;
-            uint32_t* dst = reinterpret_cast<uint32_t*>(&S);
-            for (int w = tid; w < TILES_WORDS; w += TILE_THREADS) dst[w] = src[w];
-        }
-        __syncthreads();
-        const bool active = half_ok && tgt < (int)td.nt;
+    // (a tile entry is part 0 of nparts, tiles.cuh: the parts' lists of a target are one list)
+    for (uint32_t tile0 = blockIdx.x; tile0 < ntiles; tile0 += gridDim.x) {
+        const TileDesc td0 = A.tiles[tile0];
+        if (td0.part != 0) continue;
+        const uint32_t np = td0.nparts > 1 ? min((uint32_t)td0.nparts, ntiles - tile0) : 1u;
+        bool active = false, grp_ok = true;
         uint32_t i = 0;
         double xa = 0, ya = 0, za = 0, ha = 0;
-        if (active) {
-            i = tile_target(td, S, tgt);
-            const double2 xy = A.p0[i], zh = A.p1[i];
-            xa = xy.x; ya = xy.y; za = zh.x; ha = zh.y;
-        }
-        uint2 wi = A.winfo[(size_t)tile * TILE_WARPS + warp];
-        if (!half_ok) wi.y = 0u;
-        const uint2* lp = A.pool + (size_t)wi.x * 32 + lane;
         uint32_t cnt = 0;
         uint64_t dsum = 0, dxr = 0;
-        // mode 1 needs the first half's count before the second half writes: two passes (count, then write)
+        // mode 1 needs the first thread's count before the second thread writes: two passes (count, then write)
         for (int pass = 0; pass < (MODE == 1 ? 2 : 1); ++pass) {
             uint32_t wpos = 0;
             if (MODE == 1 && pass == 1) {
                 const uint32_t other = __shfl_xor_sync(0xFFFFFFFFu, cnt, 1);
                 wpos = u ? other : 0u;                     // thread 1 writes after thread 0's entries
             }
-            const uint64_t lbase = (MODE == 1 && active) ? A.offsets[A.perm[i]] : 0;
             uint32_t c2 = 0;
-            for (uint32_t r = 0; r < wi.y; ++r) {
-                const uint2 w4 = lp[(size_t)(r >> 2) * 32];
-                const uint32_t half = (r & 2u) ? w4.y : w4.x;
-                const uint32_t s = (r & 1u) ? (half >> 16) : (half & 0xFFFFu);
-                if (s >= (uint32_t)TILE_CMAX || !active) continue;             // dummy entry
-                int q = 0;
-                while (q + 1 < (int)S.nranges && S.r_base[q + 1] <= s) ++q;
-                const uint32_t gi = S.r_vstart[q] + (s - S.r_base[q]);
-                if (!A.symmetric) {
-                    const double2 xy = A.p0[gi], zh = A.p1[gi];
-                    const double ex = min_image(__dsub_rn(xa, xy.x), g.per[0], g.L[0], g.halfL[0]);
-                    const double ey = min_image(__dsub_rn(ya, xy.y), g.per[1], g.L[1], g.halfL[1]);
-                    const double ez = min_image(__dsub_rn(za, zh.x), g.per[2], g.L[2], g.halfL[2]);
-                    if (!(r2_exact(ex, ey, ez) < support2(ha))) continue;
+            for (uint32_t part = 0; part < np; ++part) {
+                const uint32_t tile = tile0 + part;
+                const uint32_t flags = A.tflags[tile];
+                const bool half_ok = ((flags >> (warp / (TILE_WARPS / 2))) & 1u) != 0;
+                const TileDesc td = A.tiles[tile];
+                __syncthreads();
+                {
+                    const uint32_t* src = A.tiletab + (size_t)tile * TILES_WORDS;
+                    uint32_t* dst = reinterpret_cast<uint32_t*>(&S);
+                    for (int w = tid; w < TILES_WORDS; w += TILE_THREADS) dst[w] = src[w];
                 }
-                const uint32_t id = A.perm[gi];
-                if (MODE == 1 && pass == 1) A.onbr[lbase + wpos + c2] = id;
-                if (MODE == 2) { const uint64_t hsh = mix64((uint64_t)id); dsum += hsh; dxr ^= hsh; }
-                ++c2;
+                __syncthreads();
+                if (part == 0 && pass == 0) {
+                    active = half_ok && tgt < (int)td.nt;
+                    if (active) {
+                        i = tile_target(td, S, tgt);
+                        const double2 xy = A.p0[i], zh = A.p1[i];
+                        xa = xy.x; ya = xy.y; za = zh.x; ha = zh.y;
+                    }
+                }
+                if (!half_ok) grp_ok = false;
+                uint2 wi = A.winfo[(size_t)tile * TILE_WARPS + warp];
+                if (!half_ok || !active) wi.y = 0u;
+                const uint2* lp = A.pool + (size_t)wi.x * 32 + lane;
+                const uint64_t lbase = (MODE == 1 && active) ? A.offsets[A.perm[i]] : 0;
+                for (uint32_t r = 0; r < wi.y; ++r) {
+                    const uint2 w4 = lp[(size_t)(r >> 2) * 32];
+                    const uint32_t half = (r & 2u) ? w4.y : w4.x;
+                    const uint32_t s = (r & 1u) ? (half >> 16) : (half & 0xFFFFu);
+                    if (s >= (uint32_t)TILE_CMAX) continue;                          // dummy entry
+                    int q = 0;
+                    while (q + 1 < (int)S.nranges && S.r_base[q + 1] <= s) ++q;
+                    const uint32_t gi = S.r_vstart[q] + (s - S.r_base[q]);
+                    if (!A.symmetric) {
+                        const double2 xy = A.p0[gi], zh = A.p1[gi];
+                        const double ex = min_image(__dsub_rn(xa, xy.x), g.per[0], g.L[0], g.halfL[0]);
+                        const double ey = min_image(__dsub_rn(ya, xy.y), g.per[1], g.L[1], g.halfL[1]);
+                        const double ez = min_image(__dsub_rn(za, zh.x), g.per[2], g.L[2], g.halfL[2]);
+                        if (!(r2_exact(ex, ey, ez) < support2(ha))) continue;
+                    }
+                    const uint32_t id = A.perm[gi];
+                    if (MODE == 1 && pass == 1) A.onbr[lbase + wpos + c2] = id;
+                    if (MODE == 2) { const uint64_t hsh = mix64((uint64_t)id); dsum += hsh; dxr ^= hsh; }
+                    ++c2;
+                }
             }
             cnt = c2;
         }
@@ -785,7 +850,7 @@ k_tiled_export(DevGrid g, ExportArgs A) {
             dxr ^= __shfl_xor_sync(0xFFFFFFFFu, dxr, 1);
         }
         if (MODE == 1) __syncwarp();
-        if (active && u == 0) {
+        if (active && grp_ok && u == 0) {
             const uint32_t ia = A.perm[i];
             if (MODE == 0) A.ocount[ia] = total;
             if (MODE == 2) { A.odsum[ia] = dsum; A.odxor[ia] = dxr; }
@@ -841,19 +906,23 @@ cudaError_t launch_build_tiles(Ctx* c, cudaStream_t st) {
     cudaError_t e;
     if ((e = cudaMemsetAsync(t.ctr, 0, sizeof(unsigned long long) * CTR_COUNT, st)) != cudaSuccess) return e;
     if ((e = cudaMemsetAsync(t.fast, 0, (size_t)c->n, st)) != cudaSuccess) return e;
+    uint8_t* fail = c->fast_c;                        // free at this point of every build (written later, by the levels' bookkeeping, on the parent only)
+    if ((e = cudaMemsetAsync(fail, 0, (size_t)c->n, st)) != cudaSuccess) return e;
     CellTable ct{c->cell_start, c->cell_end, c->is_level ? c->cell_tend : c->cell_end};
     const int blocks = (int)((nb * 32 + 255) / 256);
     const int lvl = c->is_level ? 1 : 0;
-    k_make_tiles<false><<<blocks, 256, 0, st>>>(c->dg, ct, c->hglob, t.bcount, t.tiles, (uint32_t)t.tile_cap, t.ctr, lvl, (unsigned long long)c->n, brows);
+    const int parts = (c->is_level || c->nlevels == 0) ? 1 : 0;
+    k_make_tiles<false><<<blocks, 256, 0, st>>>(c->dg, ct, c->hglob, t.bcount, t.tiles, (uint32_t)t.tile_cap, t.ctr, lvl, (unsigned long long)c->n, brows, parts);
     if ((e = launch_excl_scan_u32(c, t.bcount, nb, t.bcount + t.bundle_cap, st)) != cudaSuccess) return e;
-    k_make_tiles<true><<<blocks, 256, 0, st>>>(c->dg, ct, c->hglob, t.bcount, t.tiles, (uint32_t)t.tile_cap, t.ctr, lvl, (unsigned long long)c->n, brows);
+    k_make_tiles<true><<<blocks, 256, 0, st>>>(c->dg, ct, c->hglob, t.bcount, t.tiles, (uint32_t)t.tile_cap, t.ctr, lvl, (unsigned long long)c->n, brows, parts);
     k_tile_tables<<<t.sms * 8, 128, 0, st>>>(c->dg, ct, t.tiles, t.ctr, t.tiletab);
     if ((e = cudaMemsetAsync(t.tflags, 0, sizeof(uint32_t) * (size_t)t.tile_cap, st)) != cudaSuccess) return e;
     if (c->ev[2]) cudaEventRecord(c->ev[2], st);
-    ListArgs A{c->pk.p0, c->pk.p1, t.tiles, t.ctr, t.pool, (uint32_t)t.pool_rows, t.winfo, t.lcount, t.tflags, t.tiletab, t.fast,
+    ListArgs A{c->pk.p0, c->pk.p1, t.tiles, t.ctr, t.pool, (uint32_t)t.pool_rows, t.winfo, t.lcount, t.tflags, t.tiletab, t.fast, fail,
                c->hglob, c->dev_status, c->is_level ? c->level_rmax : 0.f};
     k_build_lists<<<t.sms * 2, BL_THREADS, BL_SMEM, st>>>(c->dg, ct, A);
-    c->launches += 4;
+    k_apply_fail<<<(int)((c->n + 255) / 256), 256, 0, st>>>(t.fast, fail, c->n, t.ctr);
+    c->launches += 5;
     t.enabled = true;
     return cudaGetLastError();
 }

@@ -40,10 +40,12 @@ struct TileDesc {                    // 24 bytes
     int16_t y0, z0;                  // first row of the bundle
     int16_t cxa, cxb;                // first / last column
     uint8_t nyr, nzr;                // rows of the bundle present (1 or 2 each)
-    uint16_t pad;
+    uint8_t part, nparts;            // a column whose candidates exceed TILE_CMAX is cut into nparts consecutive tile entries with the same
+                                     // targets and disjoint sets of candidate rows (rowmask): a sweep's CTA runs them one after the other
+                                     // and keeps its sums; each part has lists of its own.  Ordinary tiles: part 0 of 1, every row.
     uint32_t skip;                   // targets of column cxa (column-major order) that belong to earlier tiles
     uint32_t nt;                     // targets of this tile (<= TILE_T)
-    uint32_t pad2;
+    uint32_t rowmask;                // bit rz * 4 + ry: candidate row of this entry
 };
 
 // Tile flags.  The lists of a tile are built in two halves (targets [0, TILE_T/2) and [TILE_T/2, TILE_T), i.e. the
@@ -122,6 +124,7 @@ __device__ __forceinline__ bool tile_range(int y0, int z0, int nyr, int nzr, int
 }
 __device__ __forceinline__ bool tile_range(const TileDesc& td, const DevGrid& g, const CellTable& ct, int row, int piece,
                                            RangeGeo& R) {
+    if (!((td.rowmask >> row) & 1u)) return false;
     return tile_range(td.y0, td.z0, td.nyr, td.nzr, td.cxa, td.cxb, g, ct, row, piece, R);
 }
 
