@@ -55,8 +55,8 @@ void free_all(Ctx* c) {
 // Scratch of the tiled path (tiles, tile tables, neighbour-list pool), allocated once by spray_create from n_max and
 // ncell_max -- spray_build_cells never allocates, frees or synchronises.  Capacities: a bundle is a 2 x 2 block of cell
 // rows, so a grid has ceil(ny/2) ceil(nz/2) of them: room for 4 ncell_max^(2/3) (at least 4096), which covers every
-// grid whose x extent is not much shorter than the other two; tiles: n_max / TILE_T plus the partial tiles at bundle
-// ends and column cuts; list pool: 208 bytes per particle (two bytes per neighbour and list padding; ~100 neighbours).
+// grid whose x extent is not much shorter than the other two; tiles: twice n_max / TILE_T plus the partial tiles at bundle
+// ends and column cuts (a tile cut into parts takes an entry per part; groups beyond the capacity are not served); list pool: 208 bytes per particle (two bytes per neighbour and list padding; ~100 neighbours).
 // A build that needs more than this is served by the general kernels (whole grid or, for the pool, unit by unit).
 // Failure to allocate is not an error either: the general kernels then serve every particle.
 void alloc_tiled(Ctx* c) {
@@ -65,7 +65,7 @@ void alloc_tiled(Ctx* c) {
     int64_t nb = 4 * (int64_t)ceil(pow((double)c->ncell_max, 2.0 / 3.0));
     nb = nb < 4096 ? 4096 : nb;
     nb = nb > c->ncell_max ? c->ncell_max : nb;
-    const int64_t tiles = (5 * ((n + TILE_T - 1) / TILE_T)) / 4 + 2 * nb + c->ncell_max / 64 + 64;
+    const int64_t tiles = 2 * ((n + TILE_T - 1) / TILE_T) + 2 * nb + c->ncell_max / 64 + 256;   // (tiles in several parts take an entry per part)
     const int64_t rows = (n * 208) / 256 + 4096;
     bool ok = dmalloc(&t.tiles, tiles, c) && dmalloc(&t.bcount, nb + 4096 + 64, c) && dmalloc(&t.winfo, tiles * TILE_WARPS, c) &&
               dmalloc(&t.lcount, tiles * TILE_T, c) && dmalloc(&t.tflags, tiles, c) && dmalloc(&t.tiletab, tiles * TILES_WORDS, c) &&

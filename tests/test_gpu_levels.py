@@ -49,6 +49,42 @@ def test_levels_parity(name, kmode):
         assert st["n_fast"] >= 0.7 * w.n, st           # most of the set is on the tiled path now
 
 
+@pytest.mark.parametrize("mk", [lambda: W.config1(24), lambda: W.config3(20)])
+@pytest.mark.parametrize("periodic", [(1, 1, 1), (0, 1, 0)])
+def test_tiles_in_several_parts(mk, periodic):
+    """Cells that hold ~200 particles each: the candidates of any column of a 2 x 2 bundle (48 cells) are several times what
+    a tile stages, so EVERY tile is a group of parts (tiles.cuh) -- same targets, disjoint candidate rows, lists per part,
+    sums carried from part to part.  Before the parts existed none of these particles could be tiled (n_fast = 0)."""
+    import dataclasses
+    from workloads import Grid
+    w0 = mk()
+    ncell = (4, 4, 4)
+    w = dataclasses.replace(w0, grid=Grid(w0.grid.lo, w0.grid.hi, ncell, periodic, w0.grid.h_max))
+    assert 2.0 * w.grid.h_max <= (w.grid.hi[0] - w.grid.lo[0]) / ncell[0] and w.n / 64 > 100
+    d = upload(w)
+    sp = make_ctx(w)
+    sp.build_cells(w.grid, w.kernel, d["x"], d["y"], d["z"], d["h"])
+    st = sp.path_stats_full()
+    assert st["n_fast"] >= 0.99 * w.n and st["tiles"] >= 2 * (w.n // 256), st
+    for sym, mode in ((False, O.GATHER), (True, O.SYM)):
+        cnt, ds, dx = O.neighbor_digest(w.grid, w.x, w.y, w.z, w.h, mode)
+        assert np.array_equal(u32(sp.neighbor_counts(sym)), cnt), sym
+        gs, gx = sp.neighbor_digest(sym)
+        assert np.array_equal(u64(gs), ds) and np.array_equal(u64(gx), dx), sym
+        off, nbr = sp.neighbor_lists(sym)
+        ooff, onbr = O.neighbor_lists(w.grid, w.x, w.y, w.z, w.h, mode)
+        assert np.array_equal(off.cpu().numpy().astype(np.uint64), ooff) and np.array_equal(u32(nbr), onbr)
+    mu_full = O.limiter(w.grid, w.kernel, w.x, w.y, w.z, w.h, w.m, w.rho_nom, w.kappa, w.E, w.c_light)["mu"]
+    g = gpu_isolated(sp, d, w, mu_in=mu_full)
+    o = oracle_isolated(w, mu_full=mu_full)
+    errs = compare_isolated(g, o)
+    g2 = gpu_isolated(sp, d, w, mu_in=mu_full)          # bitwise the same from run to run
+    for k in g:
+        assert np.array_equal(g[k], g2[k]), k
+    assert sp.check() == 0
+    print(st, {k: f"{v:.1e}" for k, v in errs.items()})
+
+
 def test_levels_are_optional_and_removable():
     w = W.make("c4_tiny")
     d = upload(w)
