@@ -114,7 +114,7 @@ int spray_path_stats(spray_ctx* ctx, void* stream, int64_t* n_tiles, int64_t* n_
  * than a tile can stage for others -- the library sorts the particles a second, third, ... time on grids of its own over
  * the same box: level k has ncell_d = floor(L_d / edges[k]) cells and serves the particles a with 2 hs_a (hs = symmetric
  * search length: max of h_a and the h of every particle that sees a) above the cell edge of level k - 1 and not above that
- * of level k; what no level can take (2 hs above the last edge, a tile's candidates over the staging budget) stays with the
+ * of level k; what no level can take (2 hs above the last edge, more than 160 neighbours in one part of a tile) stays with the
  * general kernels, so results are complete and identical either way.  edges: host, [nlevels], ascending, > 0 (a good
  * choice: a geometric sequence of ratio ~1.5 from 2 min(h) to 2 max(h)); ncell_max: host, [nlevels], cell capacity of each
  * level (>= prod floor(L_d / edges[k])).  Allocates the levels' scratch (synchronises the device; call it once, before
