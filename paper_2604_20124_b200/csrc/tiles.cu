@@ -743,6 +743,7 @@ k_build_lists(DevGrid g, CellTable ct, ListArgs A) {
 
 // targets of multi-part tiles that one of the parts declined: not served after all
 __global__ void k_apply_fail(uint8_t* __restrict__ fast, const uint8_t* __restrict__ fail, int64_t n, unsigned long long* __restrict__ ctr) {
+    if (ctr[CTR_NMULTI] == 0) return;                 // no tile in several parts: nothing can be marked
     const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     const bool back = i < n && fail[i] && fast[i];
     if (back) fast[i] = 0;
