@@ -88,6 +88,33 @@ def test_tiles_in_several_parts(mk, periodic):
         assert np.array_equal(g[k], g2[k]), k
     assert sp.check() == 0
     print(st, {k: f"{v:.1e}" for k, v in errs.items()})
+    # the other calls that run on the same lists (rows N1-N4), against the general kernels of a second context
+    import torch
+    s0 = make_ctx(w, path=0)
+    s0.build_cells(w.grid, w.kernel, d["x"], d["y"], d["z"], d["h"])
+    tp = 2.0 * np.pi
+    kk, T = 1.0 + 0.5 * torch.sin(tp * d["x"]), 1.0 + 0.3 * torch.cos(tp * d["y"])      # smooth fields of order one
+    mu, En, one = 0.3 + 0.1 * torch.sin(tp * d["z"]), T ** 4, torch.ones_like(T)
+    ca, cb = sp.conduction(d["m"], d["rho_nom"], kk, T), s0.conduction(d["m"], d["rho_nom"], kk, T)
+    ka, kb = sp.kgc_continuity(d["m"], d["rho_nom"], d["vx"], d["vy"], d["vz"]), s0.kgc_continuity(d["m"], d["rho_nom"], d["vx"], d["vy"], d["vz"])
+    i = np.arange(8, dtype=np.int64)
+    rays = torch.from_numpy(np.vstack([0.9 - 0.05 * W.u01(5, i, 0), W.u01(5, i, 1), W.u01(5, i, 2), -np.ones(8), 0.1 * (W.u01(5, i, 3) - 0.5),
+                                       0.1 * (W.u01(5, i, 4) - 0.5), 1.0 + W.u01(5, i, 5)])).cuda()
+    fq = 0.8 * torch.exp(-2.0 * d["x"])
+    kib = 4.0 * (0.2 + fq * fq)
+    ra, rb = sp.ray_deposit(d["m"], d["rho_nom"], fq, kib, rays, 0.01, 30), s0.ray_deposit(d["m"], d["rho_nom"], fq, kib, rays, 0.01, 30)
+    ja = sp.rad_jacobi(d["m"], d["rho_nom"], mu, one, En, T.clone(), T, one, 1e-3, niter=3)
+    jb = s0.rad_jacobi(d["m"], d["rho_nom"], mu, one, En, T.clone(), T, one, 1e-3, niter=3)
+
+    def close(a, b, what):
+        sc = float(b.abs().max()) + 1e-300
+        assert float((a - b).abs().max()) <= 1e-10 * sc, (what, float((a - b).abs().max()), sc)
+    close(ca, cb, "conduction")
+    close(ka["drhodt"], kb["drhodt"], "kgc drhodt")
+    close(ka["L"], kb["L"], "kgc L")
+    close(ra["gradn"], rb["gradn"], "ray gradn")
+    close(ra["edep"], rb["edep"], "ray edep")
+    close(ja["E"], jb["E"], "rad E")
 
 
 def test_levels_are_optional_and_removable():
