@@ -453,6 +453,15 @@ int spray_build_cells(spray_ctx* ctx, const spray_grid_t* g, spray_kernel_t kern
     if (n > 0) CK(cudaMemcpyAsync(c->s.hs, c->s.h, sizeof(double) * (size_t)n, cudaMemcpyDeviceToDevice, st), "hs init");
     SweepArgs a = base_args(c);
     a.o0 = c->s.hs;
+    if (c->tl.pool && (int64_t)c->tl.pool_rows * 256 >= 16 * n) {
+        // fp32 copies for the pre-test, in the list pool (free until the lists of this build are written)
+        float4* f4 = reinterpret_cast<float4*>(c->tl.pool);
+        CK(launch_pack_f4(c, f4, st), "search lengths: fp32 positions");
+        a.f4 = f4;
+        double cm = 0.0;
+        for (int d = 0; d < 3; ++d) cm = fmax(cm, fmax(fabs(g->lo[d]), fabs(g->hi[d])));
+        a.f4_cmax = (float)cm;
+    }
     CK(launch_ref_sweep(c, SW_HSEARCH, a, st), "search-length sweep");
     if (c->ev[1]) cudaEventRecord(c->ev[1], st);
     if (c->path == 1) CK(launch_build_tiles(c, st), "tiles + neighbour lists");

@@ -516,6 +516,20 @@ cudaError_t launch_excl_scan_u32(Ctx* c, uint32_t* a, int64_t total, uint32_t* s
     return cudaGetLastError();
 }
 
+// fp32 copies of the sorted positions and smoothing lengths for the pre-test of the search-length pre-pass (sweeps_ref.cu)
+__global__ void k_pack_f4(const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z, const double* __restrict__ h,
+                          const double* __restrict__ hglob, int64_t n, float4* __restrict__ f4) {
+    if (!(hglob[0] < hglob[1])) return;               // uniform h: the pre-pass has nothing to do and reads nothing
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i < n) f4[i] = make_float4((float)x[i], (float)y[i], (float)z[i], (float)h[i]);
+}
+cudaError_t launch_pack_f4(Ctx* c, float4* f4, cudaStream_t st) {
+    if (c->n == 0) return cudaSuccess;
+    k_pack_f4<<<cdiv64(c->n, 256), 256, 0, st>>>(c->s.x, c->s.y, c->s.z, c->s.h, c->hglob, c->n, f4);
+    c->launches += 1;
+    return cudaGetLastError();
+}
+
 cudaError_t launch_cell_hmax(Ctx* c, cudaStream_t st) {
     k_init_hglob<<<1, 1, 0, st>>>(c->hglob);
     k_cell_hmax<<<cdiv64(c->ncell, 256), 256, 0, st>>>(c->cell_start, c->cell_end, c->s.h, (uint32_t)c->ncell, c->grid.h_max,

@@ -122,6 +122,7 @@ cudaError_t launch_radix_sort(Ctx* c, cudaStream_t st);      // sets c->sorted_k
 cudaError_t launch_cell_table(Ctx* c, cudaStream_t st);
 cudaError_t launch_reorder_build(Ctx* c, const double* x, const double* y, const double* z, const double* h, cudaStream_t st);
 cudaError_t launch_cell_hmax(Ctx* c, cudaStream_t st);
+cudaError_t launch_pack_f4(Ctx* c, float4* f4, cudaStream_t st);             // (x, y, z, h) sorted, fp32 (skipped on the device when h is uniform)
 cudaError_t launch_compact_left(Ctx* c, const uint8_t* fast, cudaStream_t st);   // c->left, ctr[CTR_NLEFT] from the served flags
 cudaError_t launch_excl_scan_u32(Ctx* c, uint32_t* a, int64_t total, uint32_t* scratch, cudaStream_t st);
 
@@ -145,6 +146,8 @@ struct SweepArgs {
     const uint8_t* skip;        // nullable: particles with skip[i] != 0 are served by the tiled kernels
     const uint32_t* left;       // nullable: the particles with skip[i] == 0, compacted (then the kernel runs over this list)
     const unsigned long long* nleft;
+    const float4* f4;           // SW_HSEARCH, nullable: (x, y, z, h) of the sorted particles in fp32, for the pre-test of the pre-pass
+    float f4_cmax;              // largest absolute coordinate of the box (bounds the fp32 rounding of a position)
     const unsigned long long* nfast;   // nullable: device count of such particles (== n: nothing to do)
 };
 cudaError_t launch_ref_sweep(Ctx* c, int sweep, const SweepArgs& a, cudaStream_t st);

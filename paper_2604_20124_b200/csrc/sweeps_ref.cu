@@ -240,6 +240,15 @@ __device__ __forceinline__ void ref_particle(const DevGrid& g, int64_t n, const 
         }
         return true;
     };
+    // SW_HSEARCH, fp32 pre-test: a position carries a rounding of at most cmax 2^-24, so a distance r ~ 2 h_a is off by less than
+    // 4 cmax 2^-24 and r^2 by the relative 4 cmax 2^-24 / h_a; four times that is allowed for (and the fp64 path is taken when
+    // even this is not small, i.e. h tiny against the box)
+    const float tolf = 16.0f * 5.97e-8f * A.f4_cmax / (float)ha;
+    const bool use_f4 = SWEEP == SW_HSEARCH && !WARP && A.f4 != nullptr && tolf < 0.25f &&
+                        fmax(fabs(xa), fmax(fabs(ya), fabs(za))) <= 2.0 * (double)A.f4_cmax;   // (a particle far outside an open box: fp64)
+    const float xaf = (float)xa, yaf = (float)ya, zaf = (float)za, haf = (float)ha;
+    const float supf = (float)sup_a * (1.0f + tolf) * 1.000001f;
+    const float Lf[3] = {(float)g.L[0], (float)g.L[1], (float)g.L[2]}, hLf[3] = {(float)g.halfL[0], (float)g.halfL[1], (float)g.halfL[2]};
     if (WARP) {
         // The lanes take one cell ROW (fixed y, z; the cells of a row are consecutive ranges of sorted slots) each and cull
         // its cells in parallel -- the per-cell loads of the culling are then 32 wide instead of one dependent chain per
@@ -343,7 +352,24 @@ __device__ __forceinline__ void ref_particle(const DevGrid& g, int64_t n, const 
                     const uint32_t c = (uint32_t)((czz * g.nc[1] + cyy) * g.nc[0] + cxx);
                     if (!cell_wanted(c, gap2)) continue;
                     const uint32_t jb = __ldg(T.cell_start + c), je = __ldg(T.cell_end + c);
-                    for (uint32_t j = jb; j < je; ++j) pair_term(j, geometry(j));
+                    if (SWEEP == SW_HSEARCH && use_f4) {
+                        // pre-test in fp32 (one 16-byte load per candidate instead of four 8-byte ones): only a candidate that
+                        // cannot be excluded -- h_b > h_a even after rounding, or farther than the support widened by the
+                        // rounding bound -- is looked at in fp64.  The widened test can only add to the particles raised: the
+                        // search length is an upper bound by nature (it bounds a search range and picks a level).
+                        for (uint32_t j = jb; j < je; ++j) {
+                            const float4 b = __ldg(A.f4 + j);
+                            if (b.w > haf) continue;
+                            float dx = xaf - b.x, dy = yaf - b.y, dz = zaf - b.z;
+                            if (g.per[0]) { if (dx > hLf[0]) dx -= Lf[0]; else if (dx < -hLf[0]) dx += Lf[0]; }
+                            if (g.per[1]) { if (dy > hLf[1]) dy -= Lf[1]; else if (dy < -hLf[1]) dy += Lf[1]; }
+                            if (g.per[2]) { if (dz > hLf[2]) dz -= Lf[2]; else if (dz < -hLf[2]) dz += Lf[2]; }
+                            if (fmaf(dz, dz, fmaf(dy, dy, dx * dx)) > supf) continue;
+                            if (__ldg(A.h + j) < ha) atomicMax((unsigned long long*)(A.o0 + j), (unsigned long long)__double_as_longlong(ha));
+                        }
+                    } else {
+                        for (uint32_t j = jb; j < je; ++j) pair_term(j, geometry(j));
+                    }
                 }
             }
         }
